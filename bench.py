@@ -1,0 +1,350 @@
+"""bench.py — frames/s and visible Gaussians/s of hyrf_render on one B200 (N>1: frame-parallel replicas).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+A step = one pass of the whole hot path (S1..S6) for one camera of the workload. Default workload: BASELINE.json
+config 3 (1M Gaussians in 64 clusters + far shell, fp16 grids/MLPs, 1280x720, 20 cameras on a circle) — the
+config the north_star target is stated on. Inputs are synthetic (paper_2509_17083_b200/synth.py).
+`value` is timed with CUDA events on the stream the kernels run on, scene resident in HBM, L2 flushed between
+steps; `e2e` goes through hyrf_render_host (camera from host memory, image copied back to pinned host memory).
+`--impl reference` times the CPU oracle (oracle/) on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "frames_per_s"
+UNIT = "frames/s"
+
+
+def _dist():
+    import torch.distributed as dist
+    return dist if (dist.is_available() and dist.is_initialized()) else None
+
+
+def max_over_ranks(x: float) -> float:
+    d = _dist()
+    if d is None:
+        return float(x)
+    import torch
+    dev = "cuda" if d.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([float(x)], dtype=torch.float64, device=dev)
+    d.all_reduce(t, op=d.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(x: float) -> float:
+    d = _dist()
+    if d is None:
+        return float(x)
+    import torch
+    dev = "cuda" if d.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([float(x)], dtype=torch.float64, device=dev)
+    d.all_reduce(t, op=d.ReduceOp.SUM)
+    return float(t.item())
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index: int = 0):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 8:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx = float(f[1])
+            except ValueError:
+                continue
+            for n, v in zip(names, f[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def workload(cfg: int, args):
+    from paper_2509_17083_b200 import synth
+    kw = {}
+    if args.n_gaussians:
+        kw["n_gaussians"] = args.n_gaussians
+    if args.width and args.height:
+        kw["width"], kw["height"] = args.width, args.height
+    scene = synth.make_scene(cfg, **kw)
+    cam = scene.cameras[0]
+    name = (f"BASELINE.json configs[{cfg - 1}]: {scene.n} Gaussians, {'fp16' if scene.fp16 else 'fp32'} grids/MLPs, "
+            f"{cam.W}x{cam.H}, {len(scene.cameras)} cameras")
+    return scene, name
+
+
+# Algorithmic work per unit.
+def stage_rooflines(scene, V, D, evaluated_pairs, n_bg, peaks):
+    esz = 2 if scene.fp16 else 4
+    gathers = (scene.geo_grid.levels + scene.app_grid.levels) * 8
+    hbm = peaks["hbm_gbs"]
+    field_bytes = V * (gathers * 2 * esz + 12 + 20 + 4 + 48 + 4 + 16 + 4)   # gathers + explicit in + idx + record/keys out
+    return {
+        "cull": {"bound": "hbm", "bytes": scene.n * 12 + V * 4, "peak": hbm},
+        "field": {"bound": "hbm", "bytes": field_bytes, "peak": hbm},
+        "bin": {"bound": "hbm", "bytes": V * (4 * 16 + 12) + D * (8 + 2 * 16 + 4), "peak": hbm},
+    }
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        d["source"] = "measured"
+        return d
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0,
+            "source": "fallback"}
+
+
+def oracle_frames(scene, cams, max_seconds: float, threads: int = 0):
+    """Time the CPU oracle as it stands on `cams` (stops after max_seconds). Returns (frames, seconds, V_total)."""
+    from oracle import hyrf_oracle as ho
+    ho.build()
+    if threads:
+        ho.set_num_threads(threads)
+    osc = ho.OracleScene(scene)
+    t0 = time.perf_counter()
+    frames, vtot = 0, 0
+    for cam in cams:
+        r = ho.render(osc, cam)
+        frames += 1
+        vtot += len(r["vis_idx"])
+        if time.perf_counter() - t0 > max_seconds:
+            break
+    return frames, time.perf_counter() - t0, vtot, ho.num_threads()
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores; each step is one frame (bounded sample)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    scene, name = workload(args.config, args)
+    cams = scene.cameras
+    steps, warm = args.steps, min(args.warmup, 1)
+    seq = [cams[i % len(cams)] for i in range(warm + steps)]
+    from oracle import hyrf_oracle as ho
+    ho.build()
+    osc = ho.OracleScene(scene)
+    for cam in seq[:warm]:
+        ho.render(osc, cam)
+    t0 = time.perf_counter()
+    done = 0
+    for cam in seq[warm:]:
+        ho.render(osc, cam)
+        done += 1
+        if time.perf_counter() - t0 > 150:
+            break
+    dt = time.perf_counter() - t0
+    v = done / dt
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": done,
+            "warmup": warm, "ms_per_step": 1e3 * dt / done, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": name, "note": "CPU oracle (oracle/hyrf_oracle.c) on host cores, one frame per step"},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": ho.num_threads(), "kind": "oracle",
+                             "sample": f"{done} whole frames of the workload"},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    from paper_2509_17083_b200 import binding as B
+    from paper_2509_17083_b200 import synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = local if world > 1 else 0
+    torch.cuda.set_device(dev)
+    peaks = load_peaks()
+
+    scene, name = workload(args.config, args)
+    cams_all = scene.cameras
+    mine = synth.shard_cameras(len(cams_all), rank, world) or [rank % len(cams_all)]
+    cams = [cams_all[i] for i in mine]                      # frame-parallel replicas: no data-path collective
+    path = {"auto": B.HYRF_MLP_AUTO, "fma": B.HYRF_MLP_FMA, "mma": B.HYRF_MLP_MMA}[args.mlp]
+    hs = B.HyrfScene(scene, device=dev, mlp_path=path)
+    W, H = cams[0].W, cams[0].H
+    out = torch.empty((H, W, 3), dtype=torch.float32, device=f"cuda:{dev}")
+    cstructs = [B.camera_struct(c) for c in cams]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{dev}")      # > 126 MB L2
+    stream = torch.cuda.current_stream(dev)
+    K, Wm = args.steps, max(args.warmup, 3)
+
+    def step(i):
+        hs.render_struct(cstructs[i % len(cstructs)], W, H, out.data_ptr())
+
+    for i in range(Wm):
+        step(i)
+    torch.cuda.synchronize()
+
+    # --- timed region: K steps, CUDA events on the launching stream, L2 flushed between steps -----------------
+    sampler = ClockSampler(dev)
+    sampler.start()
+    if world > 1:
+        torch.distributed.barrier()
+    torch.cuda.synchronize()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    launches = 0
+    for i in range(K):
+        flush.fill_(i & 0xFF)
+        evs[i][0].record(stream)
+        step(Wm + i)
+        evs[i][1].record(stream)
+        launches += hs.last_launch_count()
+    torch.cuda.synchronize()
+    if world > 1:
+        torch.distributed.barrier()
+    clocks = sampler.stop()
+    t_ms = sum(a.elapsed_time(b) for a, b in evs)
+    t_max = max_over_ranks(t_ms)
+    frames_total = sum_over_ranks(K)
+    value = frames_total / (t_max * 1e-3)
+
+    # --- per-stage times + counters (separate pass, same L2 protocol) ------------------------------------------
+    hs.set_timing(True)
+    stage = []
+    Vs, Ds = [], []
+    for i in range(min(K, 2 * len(cstructs))):
+        flush.fill_(i & 0xFF)
+        step(i)
+        torch.cuda.synchronize()
+        stage.append(hs.stage_times())
+        c = hs.debug_fetch(B.DBG_COUNTERS)
+        Vs.append(int(c[1]))
+        Ds.append(int(c[2]))
+    hs.set_timing(False)
+    import numpy as np
+    stage_ms = np.median(np.array(stage), axis=0)
+    Vm, Dm = float(np.mean(Vs)), float(np.mean(Ds))
+    vis_per_s = sum_over_ranks(Vm * K) / (t_max * 1e-3)
+
+    # --- warm-L2 figure (no flush), for context ---------------------------------------------------------------
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(K):
+        step(i)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    warm_ms = e0.elapsed_time(e1) / K
+
+    # --- end to end through the public host API: camera from host, image back to pinned host memory ------------
+    host_img = torch.empty((H, W, 3), dtype=torch.float32).pin_memory()
+    for i in range(2):
+        hs.render_host(cams[i % len(cams)], out=host_img)
+    if world > 1:
+        torch.distributed.barrier()
+    t0 = time.perf_counter()
+    for i in range(K):
+        hs.render_host(cams[i % len(cams)], out=host_img)
+    torch.cuda.synchronize()
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    e2e = frames_total / e2e_s
+
+    if rank != 0:
+        return
+    names = ["cull", "field", "bin", "raster", "background"]
+    dom = int(np.argmax(stage_ms[:5]))
+    rl = stage_rooflines(scene, Vm, Dm, None, None, peaks)
+    roof = {"stage": names[dom], "bound": None, "achieved": None, "peak": None, "unit": None, "frac": None, "traffic": None}
+    if names[dom] in rl:
+        r = rl[names[dom]]
+        ach = r["bytes"] / (stage_ms[dom] * 1e-3) / 1e9
+        roof.update(bound=r["bound"], achieved=ach, peak=r["peak"], unit="GB/s", frac=ach / r["peak"],
+                    peak_source=peaks["source"])
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f16" if scene.fp16 else "f32", "data": "synthetic",
+            "config": {"workload": name, "l2": "flushed between steps (256 MiB write)", "mlp_path": args.mlp,
+                       "parallelism": f"replicas x{world} (cameras round-robin)"},
+            "visible_gaussians_per_s": vis_per_s, "V_mean": Vm, "D_mean": Dm,
+            "stage_ms": {n: float(stage_ms[i]) for i, n in enumerate(names)} | {"frame": float(stage_ms[5])},
+            "warm_l2_ms_per_step": warm_ms,
+            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 64, "d2h_bytes_per_step": W * H * 12},
+            "gpu_launches": launches, "clocks": clocks, "roofline": roof}
+    if world == 1 and not args.no_cpu:
+        fr, sec, vtot, thr = oracle_frames(scene, cams_all, max_seconds=args.cpu_seconds)
+        line["cpu_baseline"] = {"value": fr / sec, "unit": UNIT, "cores": thr, "kind": "oracle",
+                                "sample": f"{fr} whole frame(s) of the workload ({vtot / fr:.0f} visible Gaussians each)"}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--mlp", default="auto", choices=["auto", "fma", "mma"])
+    ap.add_argument("--n-gaussians", type=int, default=0)
+    ap.add_argument("--width", type=int, default=0)
+    ap.add_argument("--height", type=int, default=0)
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+    d = _dist()
+    if d is not None:
+        d.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,167 @@
+/*
+ * hyrf.h — C-ABI of the B200-native HyRF hybrid forward render pass (arxiv 2509.17083, §3.2–3.3).
+ *
+ * One scene = explicit compact Gaussians + decoupled grid fields + tiny MLP decoders + background field
+ * (PAPER.md:61–63, :124–126); one camera = R, t and an image frame; result = pixel colours
+ * (PAPER.md:55 Eq. 1, :132 Eq. 11). Arithmetic of every stage: DESIGN.md §2.
+ *
+ * Conventions
+ *  - Every call returns a hyrf_status and never throws, aborts or prints. On error, outputs are untouched and
+ *    hyrf_last_error() describes the failure (thread-local string, never NULL).
+ *  - Pointers in hyrf_params are DEVICE pointers unless host_ptrs != 0. The library copies; the caller keeps
+ *    ownership of everything it passes in. hyrf_render's out_rgb is a DEVICE pointer; hyrf_render_host's is HOST.
+ *  - hyrf_render is asynchronous on the scene's stream except for one small device→host readback of the frame's
+ *    counters (visible count V, tile-entry count D) that sizes the binning launches; the caller synchronises
+ *    the stream before reading out_rgb. Steady-state renders allocate nothing unless D outgrows the scratch.
+ *  - One scene lives on one device. A scene is not thread-safe; the library is.
+ *  - There is no CPU fallback anywhere: without a CUDA device every compute call returns HYRF_ERR_CUDA.
+ */
+#ifndef HYRF_H
+#define HYRF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HYRF_MAX_LEVELS 16u
+#define HYRF_MAX_WIDTH 64u /* widest MLP layer (inputs, hidden units) the kernels are compiled for */
+
+typedef struct hyrf_scene hyrf_scene; /* opaque, library-owned */
+
+typedef enum {
+    HYRF_OK = 0,
+    HYRF_ERR_INVALID_ARG = 1, /* NULL pointer, W/H outside [1, max], n_gaussians == 0 ... */
+    HYRF_ERR_NOT_READY = 2,   /* render before upload_params */
+    HYRF_ERR_UNSUPPORTED = 3, /* feats != 2, table not a power of two, dims beyond HYRF_MAX_* */
+    HYRF_ERR_CAMERA = 4,      /* non-finite camera, or centre outside the background sphere */
+    HYRF_ERR_OOM = 5,         /* device allocation failed, or D >= 2^32 */
+    HYRF_ERR_CUDA = 6         /* any CUDA runtime failure, incl. no device */
+} hyrf_status;
+
+typedef enum { HYRF_F32 = 0, HYRF_F16 = 1 } hyrf_dtype; /* dtype of grid tables and MLP weights */
+
+/* How the MLP decoders are evaluated.
+ *  FMA: CUDA-core fp32 fma in the oracle's order — geometry decisions bit-reproducible (any param_dtype).
+ *  MMA: fp16 tensor cores with fp32 accumulation (param_dtype F16 only) — the fast path for configs 3–5.
+ *  AUTO: MMA when param_dtype is F16 and the layer shapes are supported, else FMA. */
+typedef enum { HYRF_MLP_AUTO = 0, HYRF_MLP_FMA = 1, HYRF_MLP_MMA = 2 } hyrf_mlp_path;
+
+/* Multi-resolution grid (layout DESIGN.md §2 D3). level_res is a HOST array. */
+typedef struct {
+    uint32_t levels;     /* 1..HYRF_MAX_LEVELS */
+    uint32_t feats;      /* must be 2 ("feature of size 2") */
+    uint32_t log2_table; /* hashed levels have 2^log2_table entries; <= 24 */
+    const uint32_t* level_res;
+} hyrf_grid_desc;
+
+/* Decoder MLP: in_dim → hidden × n_hidden (ReLU) → out_dim (linear), no biases. */
+typedef struct {
+    uint32_t in_dim, hidden, n_hidden, out_dim;
+} hyrf_mlp_desc;
+
+typedef struct {
+    uint32_t n_gaussians;
+    float aabb_min[3], aabb_max[3]; /* scene box B0 used by the contraction */
+    hyrf_grid_desc geo_grid, app_grid, bg_grid;
+    hyrf_mlp_desc geo_mlp; /* in = 2*geo levels,            out = 8 (alpha_n, s_n[3], r_n[4]) — Eq. 4 */
+    hyrf_mlp_desc app_mlp; /* in >= 2*app levels + 6*octaves, out = 3 (c_n)                     — Eq. 6 */
+    hyrf_mlp_desc bg_mlp;  /* in >= 2*bg levels  + 6*octaves, out = 3 (background colour)       — Eq. 10 */
+    uint32_t dir_pe_octaves; /* 4 */
+    hyrf_dtype param_dtype;
+    hyrf_mlp_path mlp_path;
+    float cull_tol;  /* Eq. 9 tolerance band, default 0.1 */
+    float z_near;    /* "too close to the image plane", default 0.2 */
+    float bg_radius; /* background sphere radius, default 100 */
+    float tau_T;     /* background composited where T > tau_T, default 0.2 */
+    uint32_t max_width, max_height;
+    int32_t device;
+    /* optional allocator (e.g. torch-backed); NULL → cudaMalloc / cudaFree */
+    void* (*alloc)(size_t bytes, void* user);
+    void (*release)(void* ptr, void* user);
+    void* user;
+} hyrf_scene_desc;
+
+typedef struct {
+    const float* pos;           /* [3][N] SoA: x[N], y[N], z[N] — p_e */
+    const float* rgb_logit;     /* [3][N] — c_e (pre-sigmoid) */
+    const float* scale_logit;   /* [N]    — s_e (pre-sigmoid, isotropic) */
+    const float* opacity_logit; /* [N]    — alpha_e (pre-sigmoid) */
+    const void *geo_table, *app_table, *bg_table; /* levels concatenated, [entry][2], param_dtype */
+    const void *geo_w, *app_w, *bg_w;             /* layers concatenated, each row-major [out][in] */
+    int32_t host_ptrs;                            /* 0: device pointers, else host pointers */
+} hyrf_params;
+
+/* Camera frame: +x right, +y down, +z forward; pixel (i, j) centre at integer coordinates. */
+typedef struct {
+    float R[9]; /* row-major world → camera */
+    float t[3];
+    float fx, fy, cx, cy;
+} hyrf_camera;
+
+/* Validates the descriptor, allocates every persistent device buffer (Gaussian SoA, tables, weights, per-frame
+ * scratch sized from n_gaussians and max_width × max_height). */
+hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene** out);
+
+/* Copies the parameters into library-owned buffers (H2D or D2D on the scene's stream) and re-lays the weights
+ * out for the kernels. May be called again to replace the parameters. */
+hyrf_status hyrf_upload_params(hyrf_scene* scene, const hyrf_params* params);
+
+/* Stream all later work of this scene is enqueued on (a cudaStream_t). Default: the legacy stream 0. */
+hyrf_status hyrf_set_stream(hyrf_scene* scene, void* cuda_stream);
+
+/* The hybrid forward render pass, §3.2–3.3 in the order of PAPER.md:27:
+ * (1) visibility pre-culling Eq. 8–9; (2) geometry + appearance field query Eq. 2–6; (3) aggregation Eq. 7;
+ * (4) EWA projection, tile binning, depth order; (5) alpha blending Eq. 1; (6) background Eq. 10–11, 15–18.
+ * out_rgb: DEVICE float [H][W][3]. */
+hyrf_status hyrf_render(hyrf_scene* scene, const hyrf_camera* camera, int32_t W, int32_t H, float* out_rgb);
+
+/* Same pass, HOST result: renders into a library-owned device image, copies it to out_rgb_host
+ * (float [H][W][3], ideally pinned) and synchronises the stream. The end-to-end call bench.py's "e2e" times. */
+hyrf_status hyrf_render_host(hyrf_scene* scene, const hyrf_camera* camera, int32_t W, int32_t H,
+                             float* out_rgb_host);
+
+hyrf_status hyrf_destroy_scene(hyrf_scene* scene);
+
+const char* hyrf_last_error(void);
+
+/* ---- parity / measurement exports (not on the hot path) ------------------------------------------------ */
+
+typedef enum {
+    HYRF_DBG_VIS_MASK = 0,    /* u8  [N] */
+    HYRF_DBG_VIS_IDX = 1,     /* u32 [V] ascending Gaussian ids */
+    HYRF_DBG_STAGE2_RAW = 2,  /* f32 [V][11] (alpha_n, s_n[3], r_n[4], c_n[3]) */
+    HYRF_DBG_STAGE3_ATTRS = 3,/* f32 [V][11] (s[3], r[4] wxyz, alpha, c[3]) */
+    HYRF_DBG_PROJ = 4,        /* f32 [V][10] (u, v, depth, A, B, C, opacity, r, g, b) */
+    HYRF_DBG_RECT = 5,        /* u32 [V][4] (x0, x1, y0, y1), all zero when dropped */
+    HYRF_DBG_TILE_RANGES = 6, /* u32 [tiles][2] [start, end) into the tile list */
+    HYRF_DBG_TILE_LIST = 7,   /* u32 [D] Gaussian ids ordered by (tile, depth bits, id) */
+    HYRF_DBG_FINAL_T = 8,     /* f32 [H][W] residual transmittance after stage 5 */
+    HYRF_DBG_BG_MASK = 9,     /* u8  [H][W] 1 where the background was composited */
+    HYRF_DBG_COUNTERS = 10,   /* u64 [4]: N, V, D, tiles */
+    HYRF_DBG_FG = 11          /* f32 [H][W][3] foreground colour C_fg before stage 6 */
+} hyrf_debug_kind;
+
+/* mask bit k enables retention of kind k for later fetches (STAGE2_RAW / STAGE3_ATTRS / VIS_MASK / BG_MASK / FG
+ * cost extra writes in the kernels; everything else is retained anyway). */
+hyrf_status hyrf_debug_enable(hyrf_scene* scene, uint32_t mask);
+
+/* Synchronises the stream and copies data of the LAST render to host_dst. *bytes receives the size needed; if it
+ * exceeds cap nothing is copied and HYRF_ERR_INVALID_ARG is returned (host_dst may be NULL to query the size). */
+hyrf_status hyrf_debug_fetch(hyrf_scene* scene, uint32_t kind, void* host_dst, size_t cap, size_t* bytes);
+
+/* CUDA-event times (ms) of the last render's stages 1..6 (S1 cull; S2+S3+S4a field query, aggregation and
+ * projection — one fused kernel; S4b–c binning and ordering; S5 rasterise; S6 background; [5] = whole frame).
+ * Timing is recorded only after hyrf_debug_enable or hyrf_set_timing(scene, 1). Synchronises the stream. */
+hyrf_status hyrf_set_timing(hyrf_scene* scene, int32_t enabled);
+hyrf_status hyrf_stage_times(hyrf_scene* scene, float ms[6]);
+
+/* Number of kernels the last render launched (for bench.py's gpu_launches). */
+hyrf_status hyrf_last_launch_count(hyrf_scene* scene, uint32_t* launches);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HYRF_H */

@@ -1,0 +1,285 @@
+"""Thin Python binding of the C-ABI in include/hyrf.h (same names, argument marshalling only).
+
+Every step of the render pass runs inside libhyrf.so's CUDA kernels. PyTorch is used for device memory (the
+parameter tensors, the output image) and streams (torch's current stream is handed to hyrf_set_stream). There is
+no fallback: if the library is missing or no CUDA device exists, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhyrf.so")
+
+HYRF_OK, HYRF_ERR_INVALID_ARG, HYRF_ERR_NOT_READY, HYRF_ERR_UNSUPPORTED, HYRF_ERR_CAMERA, HYRF_ERR_OOM, HYRF_ERR_CUDA = range(7)
+STATUS_NAMES = ["HYRF_OK", "HYRF_ERR_INVALID_ARG", "HYRF_ERR_NOT_READY", "HYRF_ERR_UNSUPPORTED", "HYRF_ERR_CAMERA",
+                "HYRF_ERR_OOM", "HYRF_ERR_CUDA"]
+HYRF_F32, HYRF_F16 = 0, 1
+HYRF_MLP_AUTO, HYRF_MLP_FMA, HYRF_MLP_MMA = 0, 1, 2
+(DBG_VIS_MASK, DBG_VIS_IDX, DBG_STAGE2_RAW, DBG_STAGE3_ATTRS, DBG_PROJ, DBG_RECT, DBG_TILE_RANGES, DBG_TILE_LIST,
+ DBG_FINAL_T, DBG_BG_MASK, DBG_COUNTERS, DBG_FG) = range(12)
+DBG_ALL = (1 << 12) - 1
+
+EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_render", "hyrf_render_host",
+           "hyrf_destroy_scene", "hyrf_last_error", "hyrf_debug_enable", "hyrf_debug_fetch", "hyrf_set_timing",
+           "hyrf_stage_times", "hyrf_last_launch_count"]
+
+
+class GridDesc(C.Structure):
+    _fields_ = [("levels", C.c_uint32), ("feats", C.c_uint32), ("log2_table", C.c_uint32),
+                ("level_res", C.POINTER(C.c_uint32))]
+
+
+class MlpDesc(C.Structure):
+    _fields_ = [("in_dim", C.c_uint32), ("hidden", C.c_uint32), ("n_hidden", C.c_uint32), ("out_dim", C.c_uint32)]
+
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+RELEASE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class SceneDesc(C.Structure):
+    _fields_ = [("n_gaussians", C.c_uint32), ("aabb_min", C.c_float * 3), ("aabb_max", C.c_float * 3),
+                ("geo_grid", GridDesc), ("app_grid", GridDesc), ("bg_grid", GridDesc),
+                ("geo_mlp", MlpDesc), ("app_mlp", MlpDesc), ("bg_mlp", MlpDesc),
+                ("dir_pe_octaves", C.c_uint32), ("param_dtype", C.c_int), ("mlp_path", C.c_int),
+                ("cull_tol", C.c_float), ("z_near", C.c_float), ("bg_radius", C.c_float), ("tau_T", C.c_float),
+                ("max_width", C.c_uint32), ("max_height", C.c_uint32), ("device", C.c_int32),
+                ("alloc", ALLOC_FN), ("release", RELEASE_FN), ("user", C.c_void_p)]
+
+
+class Params(C.Structure):
+    _fields_ = [("pos", C.c_void_p), ("rgb_logit", C.c_void_p), ("scale_logit", C.c_void_p),
+                ("opacity_logit", C.c_void_p), ("geo_table", C.c_void_p), ("app_table", C.c_void_p),
+                ("bg_table", C.c_void_p), ("geo_w", C.c_void_p), ("app_w", C.c_void_p), ("bg_w", C.c_void_p),
+                ("host_ptrs", C.c_int32)]
+
+
+class CameraC(C.Structure):
+    _fields_ = [("R", C.c_float * 9), ("t", C.c_float * 3), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float)]
+
+
+class HyrfError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{STATUS_NAMES[status] if 0 <= status < len(STATUS_NAMES) else status}: {msg}")
+        self.status = status
+
+
+_lib: Optional[C.CDLL] = None
+
+
+def load_library() -> C.CDLL:
+    """Load libhyrf.so (built by paper_2509_17083_b200.build). Raises if it is missing: there is no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(f"{LIB_PATH} not found: run `python -m paper_2509_17083_b200.build` "
+                                    "(the CUDA extension is the only implementation; there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp = C.c_void_p
+        L.hyrf_create_scene.argtypes = [C.POINTER(SceneDesc), C.POINTER(vp)]
+        L.hyrf_upload_params.argtypes = [vp, C.POINTER(Params)]
+        L.hyrf_set_stream.argtypes = [vp, vp]
+        L.hyrf_render.argtypes = [vp, C.POINTER(CameraC), C.c_int32, C.c_int32, vp]
+        L.hyrf_render_host.argtypes = [vp, C.POINTER(CameraC), C.c_int32, C.c_int32, vp]
+        L.hyrf_destroy_scene.argtypes = [vp]
+        L.hyrf_last_error.restype = C.c_char_p
+        L.hyrf_debug_enable.argtypes = [vp, C.c_uint32]
+        L.hyrf_debug_fetch.argtypes = [vp, C.c_uint32, vp, C.c_size_t, C.POINTER(C.c_size_t)]
+        L.hyrf_set_timing.argtypes = [vp, C.c_int32]
+        L.hyrf_stage_times.argtypes = [vp, C.POINTER(C.c_float)]
+        L.hyrf_last_launch_count.argtypes = [vp, C.POINTER(C.c_uint32)]
+        for name in EXPORTS:
+            if name != "hyrf_last_error":
+                getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def last_error() -> str:
+    return load_library().hyrf_last_error().decode(errors="replace")
+
+
+def _check(status: int) -> None:
+    if status != HYRF_OK:
+        raise HyrfError(status, last_error())
+
+
+def camera_struct(cam) -> CameraC:
+    c = CameraC()
+    R = np.asarray(cam.R, dtype=np.float32).reshape(9)
+    t = np.asarray(cam.t, dtype=np.float32).reshape(3)
+    for i in range(9):
+        c.R[i] = float(R[i])
+    for i in range(3):
+        c.t[i] = float(t[i])
+    c.fx, c.fy, c.cx, c.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
+    return c
+
+
+def _grid_desc(g, keep: list) -> GridDesc:
+    arr = (C.c_uint32 * len(g.level_res))(*[int(r) for r in g.level_res])
+    keep.append(arr)
+    return GridDesc(len(g.level_res), int(g.feats), int(g.log2_table), C.cast(arr, C.POINTER(C.c_uint32)))
+
+
+def make_desc(scene, max_width: int, max_height: int, device: int = 0, mlp_path: int = HYRF_MLP_AUTO,
+              keep: Optional[list] = None) -> SceneDesc:
+    """hyrf_scene_desc from an object with the attribute names of synth.Scene."""
+    keep = keep if keep is not None else []
+    d = SceneDesc()
+    d.n_gaussians = int(scene.n)
+    for i in range(3):
+        d.aabb_min[i] = float(scene.aabb_min[i])
+        d.aabb_max[i] = float(scene.aabb_max[i])
+    d.geo_grid, d.app_grid, d.bg_grid = (_grid_desc(scene.geo_grid, keep), _grid_desc(scene.app_grid, keep),
+                                         _grid_desc(scene.bg_grid, keep))
+    for name in ("geo_mlp", "app_mlp", "bg_mlp"):
+        m = getattr(scene, name)
+        setattr(d, name, MlpDesc(m.in_dim, m.hidden, m.n_hidden, m.out_dim))
+    d.dir_pe_octaves = int(scene.dir_pe_octaves)
+    d.param_dtype = HYRF_F16 if scene.fp16 else HYRF_F32
+    d.mlp_path = int(mlp_path)
+    d.cull_tol, d.z_near, d.bg_radius, d.tau_T = (float(scene.cull_tol), float(scene.z_near),
+                                                  float(scene.bg_radius), float(scene.tau_T))
+    d.max_width, d.max_height, d.device = int(max_width), int(max_height), int(device)
+    d.alloc = ALLOC_FN()
+    d.release = RELEASE_FN()
+    d.user = None
+    d._keep = keep
+    return d
+
+
+_DBG_DTYPE = {DBG_VIS_MASK: np.uint8, DBG_VIS_IDX: np.uint32, DBG_STAGE2_RAW: np.float32,
+              DBG_STAGE3_ATTRS: np.float32, DBG_PROJ: np.float32, DBG_RECT: np.uint32, DBG_TILE_RANGES: np.uint32,
+              DBG_TILE_LIST: np.uint32, DBG_FINAL_T: np.float32, DBG_BG_MASK: np.uint8, DBG_COUNTERS: np.uint64,
+              DBG_FG: np.float32}
+_DBG_COLS = {DBG_STAGE2_RAW: 11, DBG_STAGE3_ATTRS: 11, DBG_PROJ: 10, DBG_RECT: 4, DBG_TILE_RANGES: 2}
+
+
+class HyrfScene:
+    """hyrf_scene handle. `scene` has synth.Scene's attribute names; parameters are uploaded from torch CUDA
+    tensors (device pointers) unless `host_upload=True` (numpy host pointers)."""
+
+    def __init__(self, scene, max_width: Optional[int] = None, max_height: Optional[int] = None, device: int = 0,
+                 mlp_path: int = HYRF_MLP_AUTO, host_upload: bool = False):
+        import torch
+        self._torch = torch
+        self.lib = load_library()
+        self.device = device
+        cams = getattr(scene, "cameras", [])
+        mw = max_width or max([c.W for c in cams] + [16])
+        mh = max_height or max([c.H for c in cams] + [16])
+        self._keep: list = []
+        self.desc = make_desc(scene, mw, mh, device, mlp_path, self._keep)
+        self.handle = C.c_void_p()
+        _check(self.lib.hyrf_create_scene(C.byref(self.desc), C.byref(self.handle)))
+        self.fp16 = bool(scene.fp16)
+        self.n = int(scene.n)
+        self.upload(scene, host_upload)
+
+    # -- hyrf_upload_params -------------------------------------------------------------------------------
+    def upload(self, scene, host_upload: bool = False) -> None:
+        torch = self._torch
+        tdt = np.float16 if self.fp16 else np.float32
+        host = dict(pos=np.ascontiguousarray(scene.pos, np.float32), rgb_logit=np.ascontiguousarray(scene.rgb_logit, np.float32),
+                    scale_logit=np.ascontiguousarray(scene.scale_logit, np.float32),
+                    opacity_logit=np.ascontiguousarray(scene.opacity_logit, np.float32),
+                    geo_table=np.ascontiguousarray(scene.geo_table, tdt), app_table=np.ascontiguousarray(scene.app_table, tdt),
+                    bg_table=np.ascontiguousarray(scene.bg_table, tdt), geo_w=np.ascontiguousarray(scene.geo_w, tdt),
+                    app_w=np.ascontiguousarray(scene.app_w, tdt), bg_w=np.ascontiguousarray(scene.bg_w, tdt))
+        p = Params()
+        if host_upload:
+            for k, a in host.items():
+                setattr(p, k, a.ctypes.data)
+            p.host_ptrs = 1
+            hold = host
+        else:
+            dev = {k: torch.from_numpy(a).to(f"cuda:{self.device}") for k, a in host.items()}
+            torch.cuda.synchronize(self.device)
+            for k, tns in dev.items():
+                setattr(p, k, tns.data_ptr())
+            p.host_ptrs = 0
+            hold = dev
+        self.set_stream()
+        _check(self.lib.hyrf_upload_params(self.handle, C.byref(p)))
+        del hold
+
+    def set_stream(self, stream=None) -> None:
+        torch = self._torch
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        _check(self.lib.hyrf_set_stream(self.handle, C.c_void_p(st.cuda_stream)))
+
+    # -- hyrf_render / hyrf_render_host --------------------------------------------------------------------
+    def render(self, cam, W: Optional[int] = None, H: Optional[int] = None, out=None):
+        torch = self._torch
+        W = int(cam.W if W is None else W)
+        H = int(cam.H if H is None else H)
+        if out is None:
+            out = torch.empty((H, W, 3), dtype=torch.float32, device=f"cuda:{self.device}")
+        c = camera_struct(cam)
+        _check(self.lib.hyrf_render(self.handle, C.byref(c), W, H, C.c_void_p(out.data_ptr())))
+        return out
+
+    def render_struct(self, cam_struct: CameraC, W: int, H: int, out_ptr: int) -> None:
+        _check(self.lib.hyrf_render(self.handle, C.byref(cam_struct), W, H, C.c_void_p(out_ptr)))
+
+    def render_host(self, cam, W: Optional[int] = None, H: Optional[int] = None, out=None):
+        torch = self._torch
+        W = int(cam.W if W is None else W)
+        H = int(cam.H if H is None else H)
+        if out is None:
+            out = torch.empty((H, W, 3), dtype=torch.float32).pin_memory()
+        c = camera_struct(cam)
+        _check(self.lib.hyrf_render_host(self.handle, C.byref(c), W, H, C.c_void_p(out.data_ptr())))
+        return out
+
+    # -- debug / measurement --------------------------------------------------------------------------------
+    def debug_enable(self, mask: int = DBG_ALL) -> None:
+        _check(self.lib.hyrf_debug_enable(self.handle, C.c_uint32(mask)))
+
+    def debug_fetch(self, kind: int) -> np.ndarray:
+        need = C.c_size_t(0)
+        _check(self.lib.hyrf_debug_fetch(self.handle, kind, None, 0, C.byref(need)))
+        dt = np.dtype(_DBG_DTYPE[kind])
+        buf = np.zeros(max(need.value // dt.itemsize, 0), dtype=dt)
+        if need.value:
+            _check(self.lib.hyrf_debug_fetch(self.handle, kind, buf.ctypes.data, buf.nbytes, C.byref(need)))
+        cols = _DBG_COLS.get(kind)
+        return buf.reshape(-1, cols) if cols else buf
+
+    def debug_all(self, W: int, H: int) -> Dict[str, np.ndarray]:
+        f = self.debug_fetch
+        return dict(mask=f(DBG_VIS_MASK), vis_idx=f(DBG_VIS_IDX), raw=f(DBG_STAGE2_RAW), attrs=f(DBG_STAGE3_ATTRS),
+                    proj=f(DBG_PROJ), rect=f(DBG_RECT), ranges=f(DBG_TILE_RANGES), list_id=f(DBG_TILE_LIST),
+                    T=f(DBG_FINAL_T).reshape(H, W), bg_mask=f(DBG_BG_MASK).reshape(H, W), counters=f(DBG_COUNTERS),
+                    cfg=f(DBG_FG).reshape(H, W, 3))
+
+    def set_timing(self, on: bool = True) -> None:
+        _check(self.lib.hyrf_set_timing(self.handle, int(on)))
+
+    def stage_times(self) -> np.ndarray:
+        ms = (C.c_float * 6)()
+        _check(self.lib.hyrf_stage_times(self.handle, ms))
+        return np.array(list(ms), dtype=np.float64)
+
+    def last_launch_count(self) -> int:
+        n = C.c_uint32(0)
+        _check(self.lib.hyrf_last_launch_count(self.handle, C.byref(n)))
+        return int(n.value)
+
+    def close(self) -> None:
+        if self.handle:
+            self.lib.hyrf_destroy_scene(self.handle)
+            self.handle = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,514 @@
+// api.cu — the C-ABI of include/hyrf.h: scene creation, parameter upload, the render pass orchestration,
+// debug fetches. Host logic only; every step of the path runs in the kernels of the other .cu files.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "scene.h"
+
+static thread_local char g_err[512] = "";
+
+hyrf_status hy_fail(hyrf_status st, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+hyrf_status hy_cuda_fail(cudaError_t e, const char* what) {
+    snprintf(g_err, sizeof(g_err), "CUDA error %d (%s) at %s", (int)e, cudaGetErrorString(e), what);
+    cudaGetLastError();
+    return (e == cudaErrorMemoryAllocation) ? HYRF_ERR_OOM : HYRF_ERR_CUDA;
+}
+
+extern "C" const char* hyrf_last_error(void) { return g_err; }
+
+hyrf_status hy_launch_field_fma(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
+
+namespace {
+
+hyrf_status dev_alloc(hyrf_scene* s, void** p, size_t bytes) {
+    *p = nullptr;
+    if (bytes == 0) bytes = 16;
+    if (s->desc.alloc) {
+        *p = s->desc.alloc(bytes, s->desc.user);
+        if (!*p) return hy_fail(HYRF_ERR_OOM, "user allocator returned NULL for %zu bytes", bytes);
+        return HYRF_OK;
+    }
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) { *p = nullptr; return hy_cuda_fail(e, "cudaMalloc"); }
+    return HYRF_OK;
+}
+
+void dev_free(hyrf_scene* s, void* p) {
+    if (!p) return;
+    if (s->desc.release) s->desc.release(p, s->desc.user);
+    else if (!s->desc.alloc) cudaFree(p);
+}
+
+template <typename T>
+hyrf_status dev_alloc_t(hyrf_scene* s, T** p, size_t count) {
+    return dev_alloc(s, reinterpret_cast<void**>(p), count * sizeof(T));
+}
+
+hyrf_status check_grid(const hyrf_grid_desc& g, const char* name) {
+    if (g.levels == 0 || g.levels > HYRF_MAX_LEVELS)
+        return hy_fail(HYRF_ERR_UNSUPPORTED, "%s: levels %u outside [1, %u]", name, g.levels, HYRF_MAX_LEVELS);
+    if (g.feats != 2) return hy_fail(HYRF_ERR_UNSUPPORTED, "%s: feats must be 2 (got %u)", name, g.feats);
+    if (g.log2_table == 0 || g.log2_table > 24)
+        return hy_fail(HYRF_ERR_UNSUPPORTED, "%s: log2_table %u outside [1, 24]", name, g.log2_table);
+    if (!g.level_res) return hy_fail(HYRF_ERR_INVALID_ARG, "%s: level_res is NULL", name);
+    for (uint32_t l = 0; l < g.levels; ++l)
+        if (g.level_res[l] == 0 || g.level_res[l] > 65535u)
+            return hy_fail(HYRF_ERR_UNSUPPORTED, "%s: level_res[%u] = %u outside [1, 65535]", name, l, g.level_res[l]);
+    return HYRF_OK;
+}
+
+hyrf_status check_mlp(const hyrf_mlp_desc& m, uint32_t min_in, uint32_t out, const char* name) {
+    if (m.out_dim != out) return hy_fail(HYRF_ERR_UNSUPPORTED, "%s: out_dim must be %u (got %u)", name, out, m.out_dim);
+    if (m.n_hidden == 0 || m.n_hidden > 4) return hy_fail(HYRF_ERR_UNSUPPORTED, "%s: n_hidden %u outside [1, 4]", name, m.n_hidden);
+    if (m.hidden == 0 || m.hidden > HYRF_MAX_WIDTH) return hy_fail(HYRF_ERR_UNSUPPORTED, "%s: hidden %u outside [1, %u]", name, m.hidden, HYRF_MAX_WIDTH);
+    if (m.in_dim < min_in || m.in_dim > HYRF_MAX_WIDTH)
+        return hy_fail(HYRF_ERR_UNSUPPORTED, "%s: in_dim %u outside [%u, %u]", name, m.in_dim, min_in, HYRF_MAX_WIDTH);
+    return HYRF_OK;
+}
+
+size_t mlp_weights(const hyrf_mlp_desc& m) {
+    return (size_t)m.in_dim * m.hidden + (size_t)(m.n_hidden - 1) * m.hidden * m.hidden + (size_t)m.hidden * m.out_dim;
+}
+
+// DESIGN.md §2 D3 layout: dense iff (N+1)^3 <= T; dense size rounded up to a multiple of 8.
+size_t build_grid(const hyrf_grid_desc& d, GridDev* g) {
+    const uint64_t T = 1ull << d.log2_table;
+    g->levels = d.levels;
+    g->table_mask = (uint32_t)(T - 1);
+    g->dense_mask = 0;
+    uint64_t off = 0;
+    for (uint32_t l = 0; l < d.levels; ++l) {
+        const uint64_t n1 = (uint64_t)d.level_res[l] + 1;
+        const uint64_t dense = n1 * n1 * n1;
+        g->res[l] = d.level_res[l];
+        g->offset[l] = (uint32_t)off;
+        if (dense <= T) {
+            g->dense_mask |= 1u << l;
+            off += (dense + 7) / 8 * 8;
+        } else {
+            off += T;
+        }
+    }
+    return (size_t)off;
+}
+
+void free_entries(hyrf_scene* s) {
+    for (int i = 0; i < 2; ++i) {
+        dev_free(s, s->ent_key[i]); s->ent_key[i] = nullptr;
+        dev_free(s, s->ent_val[i]); s->ent_val[i] = nullptr;
+    }
+    dev_free(s, s->hist); s->hist = nullptr;
+    s->d_capacity = 0;
+}
+
+// Scratch that depends on the number of tile entries D (keys/values ping-pong + radix histograms).
+hyrf_status ensure_entries(hyrf_scene* s, size_t need) {
+    if (need <= s->d_capacity) return HYRF_OK;
+    if (need >= 0xFFFFFFFFull) return hy_fail(HYRF_ERR_OOM, "tile-entry count %zu does not fit 32-bit offsets", need);
+    cudaStreamSynchronize(s->stream);
+    free_entries(s);
+    size_t cap = need + need / 4 + 4096;
+    if (cap > 0xFFFFFFF0ull) cap = 0xFFFFFFF0ull;
+    hyrf_status st;
+    for (int i = 0; i < 2; ++i) {
+        if ((st = dev_alloc_t(s, &s->ent_key[i], cap)) != HYRF_OK) { free_entries(s); return st; }
+        if ((st = dev_alloc_t(s, &s->ent_val[i], cap)) != HYRF_OK) { free_entries(s); return st; }
+    }
+    const size_t cap_sort = cap > s->N ? cap : s->N;
+    s->hist_elems = hy_radix_hist_elems(cap_sort);
+    if ((st = dev_alloc_t(s, &s->hist, s->hist_elems)) != HYRF_OK) { free_entries(s); return st; }
+    const size_t need_scan = hy_scan_scratch_elems(s->hist_elems) + hy_scan_scratch_elems(s->N) + 64;
+    if (need_scan > s->scan_scratch_elems) {
+        dev_free(s, s->scan_scratch);
+        s->scan_scratch = nullptr;
+        s->scan_scratch_elems = 0;
+        if ((st = dev_alloc_t(s, &s->scan_scratch, need_scan)) != HYRF_OK) { free_entries(s); return st; }
+        s->scan_scratch_elems = need_scan;
+    }
+    s->d_capacity = cap;
+    return HYRF_OK;
+}
+
+void destroy(hyrf_scene* s) {
+    if (!s) return;
+    cudaStreamSynchronize(s->stream);
+    void* ptrs[] = {s->pos, s->rgb, s->scale, s->opac, (void*)s->geo_grid.table, (void*)s->app_grid.table,
+                    (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w,
+                    s->flag_words, s->block_counts, s->vis_idx, s->rec, s->depth_key, s->rect, s->tiles,
+                    s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->tt_sorted, s->offs,
+                    s->scan_scratch, s->counters, s->ranges, s->fg, s->finalT, s->image, s->bg_mask,
+                    s->dbg_vis_mask, s->dbg_raw, s->dbg_attrs};
+    for (void* p : ptrs) dev_free(s, p);
+    free_entries(s);
+    if (s->counters_host) cudaFreeHost(s->counters_host);
+    if (s->ev_valid)
+        for (auto& e : s->ev) cudaEventDestroy(e);
+    delete s;
+}
+
+}  // namespace
+
+extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene** out) {
+    if (!desc || !out) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_create_scene: NULL argument");
+    *out = nullptr;
+    if (desc->n_gaussians == 0) return hy_fail(HYRF_ERR_INVALID_ARG, "n_gaussians must be > 0");
+    if (desc->max_width == 0 || desc->max_height == 0 || desc->max_width > 16384 || desc->max_height > 16384)
+        return hy_fail(HYRF_ERR_INVALID_ARG, "max_width / max_height outside [1, 16384]");
+    for (int a = 0; a < 3; ++a)
+        if (!(desc->aabb_max[a] > desc->aabb_min[a]) || !isfinite(desc->aabb_min[a]) || !isfinite(desc->aabb_max[a]))
+            return hy_fail(HYRF_ERR_INVALID_ARG, "aabb axis %d is empty or non-finite", a);
+    if (desc->param_dtype != HYRF_F32 && desc->param_dtype != HYRF_F16)
+        return hy_fail(HYRF_ERR_INVALID_ARG, "unknown param_dtype %d", (int)desc->param_dtype);
+    if (!(desc->bg_radius > 0.0f) || !isfinite(desc->cull_tol) || desc->cull_tol < 0.0f || !isfinite(desc->z_near) ||
+        !isfinite(desc->tau_T))
+        return hy_fail(HYRF_ERR_INVALID_ARG, "bg_radius / cull_tol / z_near / tau_T out of range");
+    if ((desc->alloc == nullptr) != (desc->release == nullptr))
+        return hy_fail(HYRF_ERR_INVALID_ARG, "alloc and release must be given together");
+    if (desc->dir_pe_octaves == 0 || desc->dir_pe_octaves > 6)
+        return hy_fail(HYRF_ERR_UNSUPPORTED, "dir_pe_octaves %u outside [1, 6]", desc->dir_pe_octaves);
+    hyrf_status st;
+    if ((st = check_grid(desc->geo_grid, "geo_grid")) != HYRF_OK) return st;
+    if ((st = check_grid(desc->app_grid, "app_grid")) != HYRF_OK) return st;
+    if ((st = check_grid(desc->bg_grid, "bg_grid")) != HYRF_OK) return st;
+    const uint32_t pe = 6 * desc->dir_pe_octaves;
+    if ((st = check_mlp(desc->geo_mlp, 2 * desc->geo_grid.levels, 8, "geo_mlp")) != HYRF_OK) return st;
+    if ((st = check_mlp(desc->app_mlp, 2 * desc->app_grid.levels + pe, 3, "app_mlp")) != HYRF_OK) return st;
+    if ((st = check_mlp(desc->bg_mlp, 2 * desc->bg_grid.levels + pe, 3, "bg_mlp")) != HYRF_OK) return st;
+    if (desc->mlp_path == HYRF_MLP_MMA)
+        return hy_fail(HYRF_ERR_UNSUPPORTED, "mlp_path MMA is not available in this build for the given shapes");
+
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return hy_fail(HYRF_ERR_CUDA, "no CUDA device available (%s)", e == cudaSuccess ? "count 0" : cudaGetErrorString(e));
+    }
+    if (desc->device < 0 || desc->device >= ndev) return hy_fail(HYRF_ERR_INVALID_ARG, "device %d outside [0, %d)", desc->device, ndev);
+    if ((e = cudaSetDevice(desc->device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
+
+    hyrf_scene* s = new (std::nothrow) hyrf_scene();
+    if (!s) return hy_fail(HYRF_ERR_OOM, "host allocation failed");
+    s->desc = *desc;
+    s->res_geo.assign(desc->geo_grid.level_res, desc->geo_grid.level_res + desc->geo_grid.levels);
+    s->res_app.assign(desc->app_grid.level_res, desc->app_grid.level_res + desc->app_grid.levels);
+    s->res_bg.assign(desc->bg_grid.level_res, desc->bg_grid.level_res + desc->bg_grid.levels);
+    s->desc.geo_grid.level_res = s->res_geo.data();
+    s->desc.app_grid.level_res = s->res_app.data();
+    s->desc.bg_grid.level_res = s->res_bg.data();
+    s->N = desc->n_gaussians;
+    s->fp16 = desc->param_dtype == HYRF_F16;
+    s->use_mma = false;
+    s->geo_entries = build_grid(s->desc.geo_grid, &s->geo_grid);
+    s->app_entries = build_grid(s->desc.app_grid, &s->app_grid);
+    s->bg_entries = build_grid(s->desc.bg_grid, &s->bg_grid);
+    s->geo_mlp = MlpDev{nullptr, desc->geo_mlp.in_dim, desc->geo_mlp.hidden, desc->geo_mlp.n_hidden, 8};
+    s->app_mlp = MlpDev{nullptr, desc->app_mlp.in_dim, desc->app_mlp.hidden, desc->app_mlp.n_hidden, 3};
+    s->bg_mlp = MlpDev{nullptr, desc->bg_mlp.in_dim, desc->bg_mlp.hidden, desc->bg_mlp.n_hidden, 3};
+
+    const size_t N = s->N;
+    const size_t esz = s->fp16 ? 2 : 4;
+    const size_t P = (size_t)desc->max_width * desc->max_height;
+    const size_t tiles = (size_t)((desc->max_width + HY_TILE - 1) / HY_TILE) * ((desc->max_height + HY_TILE - 1) / HY_TILE);
+    const size_t cull_blocks = (N + 1023) / 1024;
+    void *tg = nullptr, *ta = nullptr, *tb = nullptr, *wg = nullptr, *wa = nullptr, *wb = nullptr;
+#define HY_TRY(x) if ((st = (x)) != HYRF_OK) { destroy(s); return st; }
+    HY_TRY(dev_alloc_t(s, &s->pos, 3 * N));
+    HY_TRY(dev_alloc_t(s, &s->rgb, 3 * N));
+    HY_TRY(dev_alloc_t(s, &s->scale, N));
+    HY_TRY(dev_alloc_t(s, &s->opac, N));
+    HY_TRY(dev_alloc(s, &tg, s->geo_entries * 2 * esz)); s->geo_grid.table = tg;
+    HY_TRY(dev_alloc(s, &ta, s->app_entries * 2 * esz)); s->app_grid.table = ta;
+    HY_TRY(dev_alloc(s, &tb, s->bg_entries * 2 * esz)); s->bg_grid.table = tb;
+    HY_TRY(dev_alloc(s, &wg, mlp_weights(s->desc.geo_mlp) * esz)); s->geo_mlp.w = wg;
+    HY_TRY(dev_alloc(s, &wa, mlp_weights(s->desc.app_mlp) * esz)); s->app_mlp.w = wa;
+    HY_TRY(dev_alloc(s, &wb, mlp_weights(s->desc.bg_mlp) * esz)); s->bg_mlp.w = wb;
+    HY_TRY(dev_alloc_t(s, &s->flag_words, (N + 31) / 32 + 32));
+    HY_TRY(dev_alloc_t(s, &s->block_counts, 2 * cull_blocks + 8));
+    HY_TRY(dev_alloc_t(s, &s->vis_idx, N));
+    HY_TRY(dev_alloc_t(s, &s->rec, 3 * N));
+    HY_TRY(dev_alloc_t(s, &s->depth_key, N));
+    HY_TRY(dev_alloc_t(s, &s->rect, N));
+    HY_TRY(dev_alloc_t(s, &s->tiles, N));
+    HY_TRY(dev_alloc_t(s, &s->sort_a_key, N));
+    HY_TRY(dev_alloc_t(s, &s->sort_a_val, N));
+    HY_TRY(dev_alloc_t(s, &s->sort_b_key, N));
+    HY_TRY(dev_alloc_t(s, &s->sort_b_val, N));
+    HY_TRY(dev_alloc_t(s, &s->tt_sorted, N));
+    HY_TRY(dev_alloc_t(s, &s->offs, N));
+    HY_TRY(dev_alloc_t(s, &s->counters, 1));
+    HY_TRY(dev_alloc_t(s, &s->ranges, tiles));
+    HY_TRY(dev_alloc_t(s, &s->finalT, P));
+    if ((e = cudaMallocHost(reinterpret_cast<void**>(&s->counters_host), sizeof(FrameCounters))) != cudaSuccess) {
+        destroy(s);
+        return hy_cuda_fail(e, "cudaMallocHost");
+    }
+    HY_TRY(ensure_entries(s, 8 * N + 65536));   // initial guess; grows on demand (hyrf_render)
+#undef HY_TRY
+    *out = s;
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_set_stream(hyrf_scene* s, void* cuda_stream) {
+    if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_stream: NULL scene");
+    cudaStreamSynchronize(s->stream);
+    s->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_upload_params(hyrf_scene* s, const hyrf_params* p) {
+    if (!s || !p) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_upload_params: NULL argument");
+    if (!p->pos || !p->rgb_logit || !p->scale_logit || !p->opacity_logit || !p->geo_table || !p->app_table ||
+        !p->bg_table || !p->geo_w || !p->app_w || !p->bg_w)
+        return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_upload_params: NULL parameter pointer");
+    cudaError_t e;
+    if ((e = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
+    const cudaMemcpyKind kind = p->host_ptrs ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    const size_t N = s->N, esz = s->fp16 ? 2 : 4;
+    struct { void* dst; const void* src; size_t bytes; } copies[] = {
+        {s->pos, p->pos, 3 * N * 4}, {s->rgb, p->rgb_logit, 3 * N * 4}, {s->scale, p->scale_logit, N * 4},
+        {s->opac, p->opacity_logit, N * 4},
+        {(void*)s->geo_grid.table, p->geo_table, s->geo_entries * 2 * esz},
+        {(void*)s->app_grid.table, p->app_table, s->app_entries * 2 * esz},
+        {(void*)s->bg_grid.table, p->bg_table, s->bg_entries * 2 * esz},
+        {(void*)s->geo_mlp.w, p->geo_w, mlp_weights(s->desc.geo_mlp) * esz},
+        {(void*)s->app_mlp.w, p->app_w, mlp_weights(s->desc.app_mlp) * esz},
+        {(void*)s->bg_mlp.w, p->bg_w, mlp_weights(s->desc.bg_mlp) * esz}};
+    for (auto& c : copies)
+        if ((e = cudaMemcpyAsync(c.dst, c.src, c.bytes, kind, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpyAsync(params)");
+    if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(upload)");
+    s->ready = true;
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_destroy_scene(hyrf_scene* s) {
+    if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_destroy_scene: NULL scene");
+    cudaSetDevice(s->desc.device);
+    destroy(s);
+    return HYRF_OK;
+}
+
+namespace {
+
+hyrf_status build_frame(const hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_t H, FrameDev* f) {
+    for (int k = 0; k < 9; ++k) if (!isfinite(cam->R[k])) return hy_fail(HYRF_ERR_CAMERA, "camera R is not finite");
+    for (int k = 0; k < 3; ++k) if (!isfinite(cam->t[k])) return hy_fail(HYRF_ERR_CAMERA, "camera t is not finite");
+    if (!isfinite(cam->fx) || !isfinite(cam->fy) || !(cam->fx > 0.0f) || !(cam->fy > 0.0f) || !isfinite(cam->cx) || !isfinite(cam->cy))
+        return hy_fail(HYRF_ERR_CAMERA, "camera intrinsics are not finite / positive");
+    memcpy(f->R, cam->R, sizeof(f->R));
+    memcpy(f->t, cam->t, sizeof(f->t));
+    f->fx = cam->fx; f->fy = cam->fy; f->cx = cam->cx; f->cy = cam->cy;
+    for (int k = 0; k < 3; ++k)   // DESIGN.md §2 "Camera": o = -R^T t
+        f->o[k] = -(fmaf(cam->R[6 + k], cam->t[2], fmaf(cam->R[3 + k], cam->t[1], cam->R[k] * cam->t[0])));
+    const double on = sqrt((double)f->o[0] * f->o[0] + (double)f->o[1] * f->o[1] + (double)f->o[2] * f->o[2]);
+    if (!(on < (double)s->desc.bg_radius))
+        return hy_fail(HYRF_ERR_CAMERA, "camera centre (|o| = %g) is not inside the background sphere (r = %g)", on, (double)s->desc.bg_radius);
+    f->limx = (1.0f + s->desc.cull_tol) * ((float)W / (2.0f * cam->fx));
+    f->limy = (1.0f + s->desc.cull_tol) * ((float)H / (2.0f * cam->fy));
+    f->z_near = s->desc.z_near; f->tau_T = s->desc.tau_T; f->bg_radius = s->desc.bg_radius;
+    for (int a = 0; a < 3; ++a) {
+        f->aabb_c[a] = 0.5f * (s->desc.aabb_min[a] + s->desc.aabb_max[a]);
+        f->aabb_h[a] = 0.5f * (s->desc.aabb_max[a] - s->desc.aabb_min[a]);
+    }
+    f->W = W; f->H = H;
+    f->gx = (W + HY_TILE - 1) / HY_TILE; f->gy = (H + HY_TILE - 1) / HY_TILE;
+    return HYRF_OK;
+}
+
+hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_t H, float* out_rgb) {
+    if (!s || !cam || !out_rgb) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_render: NULL argument");
+    if (!s->ready) return hy_fail(HYRF_ERR_NOT_READY, "hyrf_render before hyrf_upload_params");
+    if (W < 1 || H < 1 || (uint32_t)W > s->desc.max_width || (uint32_t)H > s->desc.max_height)
+        return hy_fail(HYRF_ERR_INVALID_ARG, "W x H = %d x %d outside [1, %u] x [1, %u]", W, H, s->desc.max_width, s->desc.max_height);
+    FrameDev f;
+    hyrf_status st = build_frame(s, cam, W, H, &f);
+    if (st != HYRF_OK) return st;
+    cudaError_t e;
+    if ((e = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
+    const bool timing = s->timing;
+    if (timing && !s->ev_valid) {
+        for (auto& ev : s->ev) if ((e = cudaEventCreate(&ev)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventCreate");
+        s->ev_valid = true;
+    }
+    uint32_t launches = 0;
+    s->lastW = W; s->lastH = H;
+    s->rendered = false;
+    if (timing) cudaEventRecord(s->ev[0], s->stream);
+
+    // S1: visibility pre-culling
+    hy_launch_cull(s, f, &launches);
+    if (timing) cudaEventRecord(s->ev[1], s->stream);
+
+    // S2 + S3 + S4a: field query, aggregation, projection
+    if ((st = hy_launch_field_fma(s, f, &launches)) != HYRF_OK) return st;
+    if (timing) cudaEventRecord(s->ev[2], s->stream);
+
+    // S4b-c: order the visible Gaussians by (depth bits, id), lay out the tile entries, order them by tile
+    hy_launch_depth_prepare(s, &launches);
+    uint32_t *order_key = nullptr, *order = nullptr;
+    hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, s->hist,
+                    s->scan_scratch, s->stream, &order_key, &order, &launches);
+    hy_launch_tiles_gather(s, order, &launches);
+    hy_launch_scan(s->tt_sorted, s->offs, s->N, s->scan_scratch, s->stream, &launches);
+    if ((e = cudaMemcpyAsync(s->counters_host, s->counters, sizeof(FrameCounters), cudaMemcpyDeviceToHost, s->stream)) != cudaSuccess)
+        return hy_cuda_fail(e, "cudaMemcpyAsync(counters)");
+    if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(counters)");
+    const uint32_t V = s->counters_host->V;
+    const uint64_t D = s->counters_host->D;
+    if (D >= 0xFFFFFFFFull) return hy_fail(HYRF_ERR_OOM, "tile-entry count %llu does not fit 32-bit offsets", (unsigned long long)D);
+    if ((st = ensure_entries(s, (size_t)D)) != HYRF_OK) return st;
+    hy_launch_emit(s, order, V, &launches);
+    const uint32_t n_tiles = (uint32_t)(f.gx * f.gy);
+    int tile_bits = 1;
+    while ((1u << tile_bits) < n_tiles) ++tile_bits;
+    uint32_t *sorted_key = nullptr, *sorted_val = nullptr;
+    hy_launch_radix(s->ent_key[0], s->ent_val[0], s->ent_key[1], s->ent_val[1], (size_t)D, nullptr, tile_bits, s->hist,
+                    s->scan_scratch, s->stream, &sorted_key, &sorted_val, &launches);
+    hy_launch_ranges(s, sorted_key, D, n_tiles, &launches);
+    s->list_final = sorted_val;
+    if (timing) cudaEventRecord(s->ev[3], s->stream);
+
+    // S5: alpha blending (Eq. 1)
+    hy_launch_raster(s, f, sorted_val, out_rgb, &launches);
+    if (timing) cudaEventRecord(s->ev[4], s->stream);
+
+    // S6: background (Eq. 10-11, A.2)
+    if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;
+    if (timing) cudaEventRecord(s->ev[5], s->stream);
+
+    if ((e = cudaGetLastError()) != cudaSuccess) return hy_cuda_fail(e, "kernel launch");
+    s->last_launches = launches;
+    s->lastV = V; s->lastD = D;
+    s->rendered = true;
+    return HYRF_OK;
+}
+
+}  // namespace
+
+extern "C" hyrf_status hyrf_render(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_t H, float* out_rgb) {
+    return render_impl(s, cam, W, H, out_rgb);
+}
+
+extern "C" hyrf_status hyrf_render_host(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_t H, float* out_host) {
+    if (!s || !out_host) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_render_host: NULL argument");
+    if (!s->image) {
+        hyrf_status st = dev_alloc_t(s, &s->image, (size_t)s->desc.max_width * s->desc.max_height * 3);
+        if (st != HYRF_OK) return st;
+    }
+    hyrf_status st = render_impl(s, cam, W, H, s->image);
+    if (st != HYRF_OK) return st;
+    cudaError_t e = cudaMemcpyAsync(out_host, s->image, (size_t)W * H * 3 * sizeof(float), cudaMemcpyDeviceToHost, s->stream);
+    if (e != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpyAsync(image)");
+    if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(image)");
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_set_timing(hyrf_scene* s, int32_t enabled) {
+    if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_timing: NULL scene");
+    s->timing = enabled != 0;
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_stage_times(hyrf_scene* s, float ms[6]) {
+    if (!s || !ms) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_stage_times: NULL argument");
+    if (!s->rendered || !s->timing || !s->ev_valid) return hy_fail(HYRF_ERR_NOT_READY, "no timed render yet");
+    cudaError_t e = cudaEventSynchronize(s->ev[5]);
+    if (e != cudaSuccess) return hy_cuda_fail(e, "cudaEventSynchronize");
+    for (int k = 0; k < 5; ++k)
+        if ((e = cudaEventElapsedTime(&ms[k], s->ev[k], s->ev[k + 1])) != cudaSuccess) return hy_cuda_fail(e, "cudaEventElapsedTime");
+    if ((e = cudaEventElapsedTime(&ms[5], s->ev[0], s->ev[5])) != cudaSuccess) return hy_cuda_fail(e, "cudaEventElapsedTime");
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_last_launch_count(hyrf_scene* s, uint32_t* launches) {
+    if (!s || !launches) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_last_launch_count: NULL argument");
+    *launches = s->last_launches;
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_debug_enable(hyrf_scene* s, uint32_t mask) {
+    if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_debug_enable: NULL scene");
+    cudaError_t e;
+    if ((e = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
+    cudaStreamSynchronize(s->stream);
+    const size_t N = s->N, P = (size_t)s->desc.max_width * s->desc.max_height;
+    hyrf_status st;
+    if (((mask >> HYRF_DBG_VIS_MASK) & 1u) && !s->dbg_vis_mask && (st = dev_alloc_t(s, &s->dbg_vis_mask, N)) != HYRF_OK) return st;
+    if (((mask >> HYRF_DBG_STAGE2_RAW) & 1u) && !s->dbg_raw && (st = dev_alloc_t(s, &s->dbg_raw, 11 * N)) != HYRF_OK) return st;
+    if (((mask >> HYRF_DBG_STAGE3_ATTRS) & 1u) && !s->dbg_attrs && (st = dev_alloc_t(s, &s->dbg_attrs, 11 * N)) != HYRF_OK) return st;
+    if (((mask >> HYRF_DBG_BG_MASK) & 1u) && !s->bg_mask && (st = dev_alloc_t(s, &s->bg_mask, P)) != HYRF_OK) return st;
+    if (((mask >> HYRF_DBG_FG) & 1u) && !s->fg && (st = dev_alloc_t(s, &s->fg, 3 * P)) != HYRF_OK) return st;
+    s->debug_mask = mask;
+    s->rendered = false;
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_debug_fetch(hyrf_scene* s, uint32_t kind, void* host_dst, size_t cap, size_t* bytes) {
+    if (!s || !bytes) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_debug_fetch: NULL argument");
+    if (!s->rendered) return hy_fail(HYRF_ERR_NOT_READY, "hyrf_debug_fetch: no completed render");
+    cudaError_t e;
+    if ((e = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
+    if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(debug)");
+    const size_t N = s->N, V = s->lastV, D = (size_t)s->lastD, P = (size_t)s->lastW * s->lastH;
+    const size_t n_tiles = (size_t)((s->lastW + HY_TILE - 1) / HY_TILE) * ((s->lastH + HY_TILE - 1) / HY_TILE);
+    const bool on = (kind < 32) && ((s->debug_mask >> kind) & 1u);
+    const void* src = nullptr;
+    size_t need = 0;
+    switch (kind) {
+        case HYRF_DBG_VIS_MASK: if (!on) goto off; src = s->dbg_vis_mask; need = N; break;
+        case HYRF_DBG_VIS_IDX: src = s->vis_idx; need = V * 4; break;
+        case HYRF_DBG_STAGE2_RAW: if (!on) goto off; src = s->dbg_raw; need = V * 44; break;
+        case HYRF_DBG_STAGE3_ATTRS: if (!on) goto off; src = s->dbg_attrs; need = V * 44; break;
+        case HYRF_DBG_PROJ: need = V * 40; break;
+        case HYRF_DBG_RECT: src = s->rect; need = V * 16; break;
+        case HYRF_DBG_TILE_RANGES: src = s->ranges; need = n_tiles * 8; break;
+        case HYRF_DBG_TILE_LIST: need = D * 4; break;
+        case HYRF_DBG_FINAL_T: src = s->finalT; need = P * 4; break;
+        case HYRF_DBG_BG_MASK: if (!on) goto off; src = s->bg_mask; need = P; break;
+        case HYRF_DBG_COUNTERS: need = 32; break;
+        case HYRF_DBG_FG: if (!on) goto off; src = s->fg; need = P * 12; break;
+        default: return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_debug_fetch: unknown kind %u", kind);
+    }
+    *bytes = need;
+    if (!host_dst) return HYRF_OK;
+    if (need > cap) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_debug_fetch: need %zu bytes, cap %zu", need, cap);
+    if (need == 0) return HYRF_OK;
+    if (kind == HYRF_DBG_COUNTERS) {
+        uint64_t c[4] = {N, V, D, n_tiles};
+        memcpy(host_dst, c, sizeof(c));
+        return HYRF_OK;
+    }
+    if (kind == HYRF_DBG_PROJ) {   // records -> (u, v, depth, A, B, C, opacity, r, g, b)
+        std::vector<float> rec(12 * V);
+        if ((e = cudaMemcpy(rec.data(), s->rec, rec.size() * 4, cudaMemcpyDeviceToHost)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpy(rec)");
+        float* o = static_cast<float*>(host_dst);
+        for (size_t j = 0; j < V; ++j) {
+            const float* r = &rec[12 * j];
+            float* d = o + 10 * j;
+            d[0] = r[0]; d[1] = r[1]; d[2] = r[9]; d[3] = r[2]; d[4] = r[3]; d[5] = r[4]; d[6] = r[5]; d[7] = r[6]; d[8] = r[7]; d[9] = r[8];
+        }
+        return HYRF_OK;
+    }
+    if (kind == HYRF_DBG_TILE_LIST) {   // visible ranks -> Gaussian ids
+        std::vector<uint32_t> idx(V);
+        if (V && (e = cudaMemcpy(idx.data(), s->vis_idx, V * 4, cudaMemcpyDeviceToHost)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpy(vis_idx)");
+        uint32_t* o = static_cast<uint32_t*>(host_dst);
+        if ((e = cudaMemcpy(o, s->list_final, D * 4, cudaMemcpyDeviceToHost)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpy(list)");
+        for (size_t q = 0; q < D; ++q) o[q] = o[q] < V ? idx[o[q]] : 0xFFFFFFFFu;
+        return HYRF_OK;
+    }
+    if ((e = cudaMemcpy(host_dst, src, need, cudaMemcpyDeviceToHost)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpy(debug)");
+    return HYRF_OK;
+off:
+    return hy_fail(HYRF_ERR_NOT_READY, "hyrf_debug_fetch: kind %u was not enabled with hyrf_debug_enable before the render", kind);
+}

