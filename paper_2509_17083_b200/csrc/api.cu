@@ -28,6 +28,10 @@ hyrf_status hy_cuda_fail(cudaError_t e, const char* what) {
 extern "C" const char* hyrf_last_error(void) { return g_err; }
 
 hyrf_status hy_launch_field_fma(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
+hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
+bool hy_field_mma_supported(const hyrf_scene_desc& d);
+hyrf_status hy_field_mma_prepare(hyrf_scene* s);
+size_t hy_field_mma_packed_bytes();
 
 namespace {
 
@@ -185,8 +189,10 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     if ((st = check_mlp(desc->geo_mlp, 2 * desc->geo_grid.levels, 8, "geo_mlp")) != HYRF_OK) return st;
     if ((st = check_mlp(desc->app_mlp, 2 * desc->app_grid.levels + pe, 3, "app_mlp")) != HYRF_OK) return st;
     if ((st = check_mlp(desc->bg_mlp, 2 * desc->bg_grid.levels + pe, 3, "bg_mlp")) != HYRF_OK) return st;
-    if (desc->mlp_path == HYRF_MLP_MMA)
-        return hy_fail(HYRF_ERR_UNSUPPORTED, "mlp_path MMA is not available in this build for the given shapes");
+    if (desc->mlp_path != HYRF_MLP_AUTO && desc->mlp_path != HYRF_MLP_FMA && desc->mlp_path != HYRF_MLP_MMA)
+        return hy_fail(HYRF_ERR_INVALID_ARG, "unknown mlp_path %d", (int)desc->mlp_path);
+    if (desc->mlp_path == HYRF_MLP_MMA && !hy_field_mma_supported(*desc))
+        return hy_fail(HYRF_ERR_UNSUPPORTED, "mlp_path MMA needs fp16 parameters, 16-level grids, 32->64->64->8 and 56->64->64->3 decoders");
 
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
@@ -208,7 +214,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     s->desc.bg_grid.level_res = s->res_bg.data();
     s->N = desc->n_gaussians;
     s->fp16 = desc->param_dtype == HYRF_F16;
-    s->use_mma = false;
+    s->use_mma = desc->mlp_path != HYRF_MLP_FMA && hy_field_mma_supported(*desc);
     s->geo_entries = build_grid(s->desc.geo_grid, &s->geo_grid);
     s->app_entries = build_grid(s->desc.app_grid, &s->app_grid);
     s->bg_entries = build_grid(s->desc.bg_grid, &s->bg_grid);
@@ -233,6 +239,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc(s, &wg, mlp_weights(s->desc.geo_mlp) * esz)); s->geo_mlp.w = wg;
     HY_TRY(dev_alloc(s, &wa, mlp_weights(s->desc.app_mlp) * esz)); s->app_mlp.w = wa;
     HY_TRY(dev_alloc(s, &wb, mlp_weights(s->desc.bg_mlp) * esz)); s->bg_mlp.w = wb;
+    if (s->use_mma) HY_TRY(dev_alloc(s, &s->mma_w, hy_field_mma_packed_bytes()));
     HY_TRY(dev_alloc_t(s, &s->flag_words, (N + 31) / 32 + 32));
     HY_TRY(dev_alloc_t(s, &s->block_counts, 2 * cull_blocks + 8));
     HY_TRY(dev_alloc_t(s, &s->vis_idx, N));
@@ -286,6 +293,10 @@ extern "C" hyrf_status hyrf_upload_params(hyrf_scene* s, const hyrf_params* p) {
         {(void*)s->bg_mlp.w, p->bg_w, mlp_weights(s->desc.bg_mlp) * esz}};
     for (auto& c : copies)
         if ((e = cudaMemcpyAsync(c.dst, c.src, c.bytes, kind, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpyAsync(params)");
+    if (s->use_mma) {
+        hyrf_status st = hy_field_mma_prepare(s);
+        if (st != HYRF_OK) return st;
+    }
     if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(upload)");
     s->ready = true;
     return HYRF_OK;
@@ -350,7 +361,7 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     if (timing) cudaEventRecord(s->ev[1], s->stream);
 
     // S2 + S3 + S4a: field query, aggregation, projection
-    if ((st = hy_launch_field_fma(s, f, &launches)) != HYRF_OK) return st;
+    if ((st = s->use_mma ? hy_launch_field_mma(s, f, &launches) : hy_launch_field_fma(s, f, &launches)) != HYRF_OK) return st;
     if (timing) cudaEventRecord(s->ev[2], s->stream);
 
     // S4b-c: order the visible Gaussians by (depth bits, id), lay out the tile entries, order them by tile

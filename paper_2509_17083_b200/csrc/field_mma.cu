@@ -1,0 +1,243 @@
+// field_mma.cu — S2 + S3 + S4a fused, tensor-core path for fp16 parameters (BASELINE configs 3–5):
+//   contraction (Eq. 2) -> grid encodes (Eq. 3) -> direction PE (Eq. 5) -> decoders (Eq. 4, 6, "fully-fused
+//   MLP, 2 hidden layers x 64") -> aggregation (Eq. 7) -> EWA projection.
+// B200 design: a CTA owns a tile of 128 visible Gaussians = the 128 TMEM lanes. 256 threads: warps 0–3 gather the
+// geometry field, warps 4–7 the appearance field + PE, one thread per Gaussian each. Features go registers -> TMEM
+// (tcgen05.st, fp16 pairs) as the A operand; the weights sit in shared memory as the B operand (K-major core
+// matrices); tcgen05.mma accumulates fp32 in TMEM; the epilogue (tcgen05.ld, ReLU, round to fp16, tcgen05.st)
+// feeds the next layer without touching shared or global memory. Only the 48-byte projected record leaves the SM.
+// The two decoders run as independent chains with their own mbarrier. Accumulation order inside an MMA is
+// unspecified, so this path is compared with the oracle by tolerance, not bit for bit.
+#include "field_common.cuh"
+#include "tcgen05.cuh"
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kTile = 128;
+constexpr int kTmemCols = 256;
+constexpr uint32_t kColDg = 0, kColDa = 64, kColAg = 128, kColAa = 160;
+// packed weight block (bytes): geo W1 [64 x 32], W2 [64 x 64], W3 [16 x 64]; app W1 [64 x 64], W2, W3
+constexpr uint32_t kOffG1 = 0, kOffG2 = 4096, kOffG3 = 12288, kOffA1 = 14336, kOffA2 = 22528, kOffA3 = 30720;
+constexpr uint32_t kPackedBytes = 32768;
+constexpr uint32_t kSmemBytes = 80 * 1024;   // > 227 KB / 3: at most two CTAs (2 x 256 TMEM columns) per SM
+
+// element (n, k) of an [N x Kp] K-major operand stored as 8x8 core matrices: half-index inside the operand
+__host__ __device__ inline uint32_t core_index(uint32_t n, uint32_t k, uint32_t Kp) {
+    return (n >> 3) * (Kp * 8) + (k >> 3) * 64 + (n & 7) * 8 + (k & 7);
+}
+
+// raw row-major [out][in] fp16 weights -> packed operand block
+__global__ void pack_weights_kernel(const __half* __restrict__ geo, const __half* __restrict__ app,
+                                    __half* __restrict__ packed) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= kPackedBytes / 2) return;
+    packed[i] = __float2half(0.0f);
+    struct Op { uint32_t off, N, Kp, n_real, k_real, src; bool app; };
+    const Op ops[6] = {{kOffG1, 64, 32, 64, 32, 0, false},        {kOffG2, 64, 64, 64, 64, 64 * 32, false},
+                       {kOffG3, 16, 64, 8, 64, 64 * 32 + 64 * 64, false}, {kOffA1, 64, 64, 64, 56, 0, true},
+                       {kOffA2, 64, 64, 64, 64, 64 * 56, true},   {kOffA3, 16, 64, 3, 64, 64 * 56 + 64 * 64, true}};
+    for (int o = 0; o < 6; ++o) {
+        const Op& op = ops[o];
+        const uint32_t lo = op.off / 2, hi = lo + op.N * op.Kp;
+        if (i < lo || i >= hi) continue;
+        const uint32_t r = i - lo;
+        const uint32_t grp = r / (op.Kp * 8), rem = r % (op.Kp * 8);
+        const uint32_t kc = rem / 64, n = grp * 8 + (rem % 64) / 8, k = kc * 8 + (rem % 8);
+        if (n < op.n_real && k < op.k_real) packed[i] = (op.app ? app : geo)[op.src + n * op.k_real + k];
+    }
+}
+
+__device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
+    __half2 h = __floats2half2_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&h);
+}
+
+// ReLU + round to fp16 of 32 fp32 accumulator columns -> 16 packed A columns
+__device__ __forceinline__ void relu_pack32(const uint32_t* d, uint32_t* a) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i)
+        a[i] = pack_h2(fmaxf(__uint_as_float(d[2 * i]), 0.0f), fmaxf(__uint_as_float(d[2 * i + 1]), 0.0f));
+}
+
+__global__ void __launch_bounds__(kThreads, 2)
+field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    __shared__ __align__(8) uint64_t mbar[2];
+    __shared__ uint32_t tmem_slot;
+    __shared__ float s_col[kTile][3];
+
+    const uint32_t warp = threadIdx.x >> 5;
+    const uint32_t chain = warp >> 2;                 // 0: geometry, 1: appearance
+    const uint32_t row = threadIdx.x & (kTile - 1);   // Gaussian within the tile == TMEM lane
+    for (uint32_t i = threadIdx.x; i < kPackedBytes / 16; i += kThreads)
+        reinterpret_cast<uint4*>(smem)[i] = __ldg(packed_w + i);
+    tc::fence_proxy_async_smem();
+    if (warp == 0) tc::tmem_alloc<kTmemCols>(&tmem_slot);
+    if (threadIdx.x == 32) {
+        tc::mbar_init(&mbar[0], 1);
+        tc::mbar_init(&mbar[1], 1);
+        tc::fence_mbar_init();
+    }
+    tc::fence_before_sync();
+    __syncthreads();
+    tc::fence_after_sync();
+    const uint32_t tmem = tmem_slot;
+    const uint32_t lane_base = ((warp & 3u) * 32u) << 16;
+    const uint32_t tD = tmem + (chain ? kColDa : kColDg);
+    const uint32_t tA = tmem + (chain ? kColAa : kColAg);
+    const uint32_t sb = tc::smem_u32(smem);
+    const uint32_t off1 = chain ? kOffA1 : kOffG1, off2 = chain ? kOffA2 : kOffG2, off3 = chain ? kOffA3 : kOffG3;
+    const uint32_t k1 = chain ? 64u : 32u;            // padded K of layer 1
+    constexpr uint32_t idesc64 = tc::idesc_f16_f32(128, 64), idesc16 = tc::idesc_f16_f32(128, 16);
+    uint64_t* bar = &mbar[chain];
+    uint32_t phase = 0;
+    const bool leader = row == 0;
+    const uint32_t V = A.counters->V;
+    const GridDev& grid = chain ? A.app : A.geo;
+
+    for (uint32_t tile = blockIdx.x; tile * kTile < V; tile += gridDim.x) {
+        const uint32_t j = tile * kTile + row;
+        const bool valid = j < V;
+        uint32_t gid = 0;
+        float px = 0.0f, py = 0.0f, pz = 0.0f;
+        uint32_t a[32];
+#pragma unroll
+        for (int i = 0; i < 32; ++i) a[i] = 0u;
+        if (valid) {
+            gid = A.vis_idx[j];
+            px = __ldg(A.pos + gid); py = __ldg(A.pos + A.N + gid); pz = __ldg(A.pos + 2ull * A.N + gid);
+            float x[3];
+            hy_contract(A.f, px, py, pz, x);
+#pragma unroll
+            for (int l = 0; l < 16; ++l) {
+                float f0, f1;
+                hy_grid_level<true>(grid, l, x, f0, f1);
+                a[l] = pack_h2(f0, f1);
+            }
+            if (chain) {
+                const float dx = __fsub_rn(px, A.f.o[0]), dy = __fsub_rn(py, A.f.o[1]), dz = __fsub_rn(pz, A.f.o[2]);
+                const float n = __fsqrt_rn(__fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx))));
+                const float d[3] = {__fdiv_rn(dx, n), __fdiv_rn(dy, n), __fdiv_rn(dz, n)};
+                float pe[24];
+                hy_dir_pe<false>(d, 4, pe);
+#pragma unroll
+                for (int i = 0; i < 12; ++i) a[16 + i] = pack_h2(pe[2 * i], pe[2 * i + 1]);
+            }
+        }
+        // ---- layer 1: A <- features, D = A W1^T ----
+        tc::st_x16(tA + lane_base, a);
+        if (chain) tc::st_x16(tA + lane_base + 16, a + 16);
+        tc::wait_st();
+        tc::fence_before_sync();
+        asm volatile("bar.sync %0, 128;" ::"r"(1 + chain) : "memory");
+        if (leader) {
+            tc::fence_after_sync();
+            for (uint32_t s = 0; s < k1 / 16; ++s)
+                tc::mma_f16_ts(tD, tA + s * 8, tc::smem_desc_kmajor_noswizzle(sb + off1 + s * 256, 128, k1 * 16), idesc64, s);
+            tc::commit(bar);
+        }
+        tc::mbar_wait(bar, phase); phase ^= 1;
+        tc::fence_after_sync();
+        // ---- layer 2: A <- relu(D) in fp16, D = A W2^T ----
+        {
+            uint32_t d[32];
+            tc::ld_x32(tD + lane_base, d); tc::wait_ld();
+            relu_pack32(d, a);
+            tc::ld_x32(tD + lane_base + 32, d); tc::wait_ld();
+            relu_pack32(d, a + 16);
+        }
+        tc::st_x16(tA + lane_base, a);
+        tc::st_x16(tA + lane_base + 16, a + 16);
+        tc::wait_st();
+        tc::fence_before_sync();
+        asm volatile("bar.sync %0, 128;" ::"r"(1 + chain) : "memory");
+        if (leader) {
+            tc::fence_after_sync();
+            for (uint32_t s = 0; s < 4; ++s)
+                tc::mma_f16_ts(tD, tA + s * 8, tc::smem_desc_kmajor_noswizzle(sb + off2 + s * 256, 128, 1024), idesc64, s);
+            tc::commit(bar);
+        }
+        tc::mbar_wait(bar, phase); phase ^= 1;
+        tc::fence_after_sync();
+        // ---- output layer: A <- relu(D) in fp16, D[:, 0:16] = A W3^T ----
+        {
+            uint32_t d[32];
+            tc::ld_x32(tD + lane_base, d); tc::wait_ld();
+            relu_pack32(d, a);
+            tc::ld_x32(tD + lane_base + 32, d); tc::wait_ld();
+            relu_pack32(d, a + 16);
+        }
+        tc::st_x16(tA + lane_base, a);
+        tc::st_x16(tA + lane_base + 16, a + 16);
+        tc::wait_st();
+        tc::fence_before_sync();
+        asm volatile("bar.sync %0, 128;" ::"r"(1 + chain) : "memory");
+        if (leader) {
+            tc::fence_after_sync();
+            for (uint32_t s = 0; s < 4; ++s)
+                tc::mma_f16_ts(tD, tA + s * 8, tc::smem_desc_kmajor_noswizzle(sb + off3 + s * 256, 128, 1024), idesc16, s);
+            tc::commit(bar);
+        }
+        tc::mbar_wait(bar, phase); phase ^= 1;
+        tc::fence_after_sync();
+        float raw[11];
+        if (chain) {
+            uint32_t o[4];
+            tc::ld_x4(tD + lane_base, o); tc::wait_ld();
+            s_col[row][0] = __uint_as_float(o[0]); s_col[row][1] = __uint_as_float(o[1]); s_col[row][2] = __uint_as_float(o[2]);
+        } else {
+            uint32_t o[8];
+            tc::ld_x8(tD + lane_base, o); tc::wait_ld();
+#pragma unroll
+            for (int i = 0; i < 8; ++i) raw[i] = __uint_as_float(o[i]);
+        }
+        tc::fence_before_sync();
+        __syncthreads();
+        if (!chain && valid) {
+            raw[8] = s_col[row][0]; raw[9] = s_col[row][1]; raw[10] = s_col[row][2];
+            aggregate_project(A, j, gid, px, py, pz, raw);
+        }
+        __syncthreads();
+        tc::fence_after_sync();
+    }
+    tc::fence_before_sync();
+    __syncthreads();
+    if (warp == 0) tc::tmem_dealloc<kTmemCols>(tmem);
+}
+
+}  // namespace
+
+bool hy_field_mma_supported(const hyrf_scene_desc& d) {
+    return d.param_dtype == HYRF_F16 && d.geo_grid.levels == 16 && d.app_grid.levels == 16 && d.dir_pe_octaves == 4 &&
+           d.geo_mlp.in_dim == 32 && d.geo_mlp.hidden == 64 && d.geo_mlp.n_hidden == 2 && d.app_mlp.in_dim == 56 &&
+           d.app_mlp.hidden == 64 && d.app_mlp.n_hidden == 2;
+}
+
+// re-lay the uploaded weights out as tcgen05 B operands (called from hyrf_upload_params)
+hyrf_status hy_field_mma_prepare(hyrf_scene* s) {
+    pack_weights_kernel<<<(kPackedBytes / 2 + 255) / 256, 256, 0, s->stream>>>(
+        reinterpret_cast<const __half*>(s->geo_mlp.w), reinterpret_cast<const __half*>(s->app_mlp.w),
+        reinterpret_cast<__half*>(s->mma_w));
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return hy_cuda_fail(e, "pack_weights_kernel");
+    return HYRF_OK;
+}
+
+size_t hy_field_mma_packed_bytes() { return kPackedBytes; }
+
+hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* launches) {
+    FieldArgs A;
+    hy_fill_field_args(s, f, &A);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(field_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+        if (e != cudaSuccess) return hy_cuda_fail(e, "cudaFuncSetAttribute(field_mma)");
+        attr_set = true;
+    }
+    const int need = (int)((s->N + kTile - 1) / kTile);
+    const int grid = need < 148 * 2 ? need : 148 * 2;
+    field_mma_kernel<<<grid, kThreads, kSmemBytes, s->stream>>>(A, reinterpret_cast<const uint4*>(s->mma_w));
+    ++*launches;
+    return HYRF_OK;
+}

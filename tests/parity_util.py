@@ -68,7 +68,7 @@ def compare_frame(orc, gpu, out_gpu, tau_T, fp16=False, exact_geometry=True, lab
     # image
     Tg, To = gpu["T"], orc["T"]
     ma, ms = orc["m_alpha"], orc["m_stop"]
-    scale = 1.0 if exact_geometry else 2e3       # attribute noise of the tensor path widens every margin
+    scale = 1.0 if exact_geometry else 50.0      # attribute noise of the tensor path (~1e-4) widens every margin
     frag_alpha = ma < 5e-8 * scale
     frag_stop = ms < 5e-5 * scale
     frag_tau = (np.abs(To - np.float32(tau_T)) < 1e-5 * scale) & (orc["n_blend"] > 0)   # T = 1 exactly when nothing blended

@@ -152,3 +152,38 @@ def test_render_is_deterministic_and_scratch_grows(B, synth):
     hs.render(s.cameras[0])
     assert int(hs.debug_fetch(B.DBG_COUNTERS)[2]) > 8 * s.n + 65536
     hs.close()
+
+
+def test_config3_scaled_fp16_tensor_core_path(B, ho, synth):
+    # the launch configuration bench.py times (AUTO -> tcgen05 decoders): mask bit-exact, raw logits within 2e-3,
+    # list symmetric difference reported and bounded, image within 1e-2 (SURVEY §8c H1 protocol)
+    s = synth.make_scene(3, n_gaussians=60_000, width=320, height=180, n_cameras=3)
+    st = _run(B, ho, s, mlp_path=B.HYRF_MLP_MMA, exact=False)
+    assert max(x["raw_geo_maxdiff"] for x in st) > 0.0          # really a different arithmetic path
+    print("tensor-core path stats:", st[0])
+
+
+def test_tensor_core_path_high_gain(B, ho, synth):
+    # large table entries: decoder outputs O(1), so operand layout / K-order mistakes cannot hide in the tolerance
+    s = synth.make_scene(3, n_gaussians=20_000, width=160, height=96, n_cameras=1, table_amp=1.0)
+    import torch
+    hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_MMA)
+    hs.debug_enable()
+    hs.render(s.cameras[0])
+    torch.cuda.synchronize()
+    raw = hs.debug_fetch(B.DBG_STAGE2_RAW)
+    idx = hs.debug_fetch(B.DBG_VIS_IDX)
+    osc = ho.OracleScene(s)
+    ref = ho.stage_query(osc, s.cameras[0], idx)
+    assert np.abs(ref).max() > 0.3
+    err = np.abs(raw - ref)
+    assert err.max() < 2e-2 and err.mean() < 1e-3, (err.max(), err.mean())
+    hs.close()
+
+
+def test_config3_full_one_camera_both_paths(B, ho, synth):
+    # BASELINE config 3 at full size (1M Gaussians, 1280x720), camera 0: exact path bit-exact lists, tensor path by
+    # tolerance; this is the workload and launch configuration bench.py times
+    s = synth.make_scene(3, n_cameras=1)
+    _run(B, ho, s, mlp_path=B.HYRF_MLP_FMA, exact=True)
+    _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False)
