@@ -156,6 +156,7 @@ void destroy(hyrf_scene* s) {
     for (void* p : ptrs) dev_free(s, p);
     free_entries(s);
     if (s->counters_host) cudaFreeHost(s->counters_host);
+    if (s->ev_counters) cudaEventDestroy(s->ev_counters);
     if (s->ev_valid)
         for (auto& e : s->ev) cudaEventDestroy(e);
     delete s;
@@ -259,6 +260,10 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     if ((e = cudaMallocHost(reinterpret_cast<void**>(&s->counters_host), sizeof(FrameCounters))) != cudaSuccess) {
         destroy(s);
         return hy_cuda_fail(e, "cudaMallocHost");
+    }
+    if ((e = cudaEventCreateWithFlags(&s->ev_counters, cudaEventDisableTiming)) != cudaSuccess) {
+        destroy(s);
+        return hy_cuda_fail(e, "cudaEventCreate");
     }
     HY_TRY(ensure_entries(s, 8 * N + 65536));   // initial guess; grows on demand (hyrf_render)
 #undef HY_TRY
@@ -364,20 +369,30 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     if ((st = s->use_mma ? hy_launch_field_mma(s, f, &launches) : hy_launch_field_fma(s, f, &launches)) != HYRF_OK) return st;
     if (timing) cudaEventRecord(s->ev[2], s->stream);
 
+    // counters (V, D) start their way to the host now; the depth ordering below does not need them, so the copy
+    // and the host's wake-up hide behind it
+    if ((e = cudaMemcpyAsync(s->counters_host, s->counters, sizeof(FrameCounters), cudaMemcpyDeviceToHost, s->stream)) != cudaSuccess)
+        return hy_cuda_fail(e, "cudaMemcpyAsync(counters)");
+    if ((e = cudaEventRecord(s->ev_counters, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(counters)");
+
     // S4b-c: order the visible Gaussians by (depth bits, id), lay out the tile entries, order them by tile
     hy_launch_depth_prepare(s, &launches);
     uint32_t *order_key = nullptr, *order = nullptr;
     hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, s->hist,
                     s->scan_scratch, s->stream, &order_key, &order, &launches);
-    hy_launch_tiles_gather(s, order, &launches);
-    hy_launch_scan(s->tt_sorted, s->offs, s->N, s->scan_scratch, s->stream, &launches);
-    if ((e = cudaMemcpyAsync(s->counters_host, s->counters, sizeof(FrameCounters), cudaMemcpyDeviceToHost, s->stream)) != cudaSuccess)
-        return hy_cuda_fail(e, "cudaMemcpyAsync(counters)");
-    if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(counters)");
+    if ((e = cudaEventSynchronize(s->ev_counters)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventSynchronize(counters)");
     const uint32_t V = s->counters_host->V;
     const uint64_t D = s->counters_host->D;
-    if (D >= 0xFFFFFFFFull) return hy_fail(HYRF_ERR_OOM, "tile-entry count %llu does not fit 32-bit offsets", (unsigned long long)D);
-    if ((st = ensure_entries(s, (size_t)D)) != HYRF_OK) return st;
+    if (D >= 0xFFFFFFFFull || D > hy_radix_max_items())
+        return hy_fail(HYRF_ERR_OOM, "tile-entry count %llu exceeds the supported maximum", (unsigned long long)D);
+    if (D > s->d_capacity) {
+        // growing frees the sort workspace the depth ordering is still using: wait for it first
+        if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(grow)");
+        // the depth order lives in the N-sized buffers, which are not reallocated
+        if ((st = ensure_entries(s, (size_t)D)) != HYRF_OK) return st;
+    }
+    hy_launch_tiles_gather(s, order, V, &launches);
+    hy_launch_scan(s->tt_sorted, s->offs, V, s->scan_scratch, s->stream, &launches);
     hy_launch_emit(s, order, V, &launches);
     const uint32_t n_tiles = (uint32_t)(f.gx * f.gy);
     int tile_bits = 1;

@@ -15,46 +15,48 @@ __global__ void depth_prepare_kernel(const uint32_t* __restrict__ depth_key, con
     val[j] = j;
 }
 
-// tt_sorted[k] = tiles touched by the k-th Gaussian in depth order (0 beyond V); counters->D += block sums.
+// tt_sorted[k] = tiles touched by the k-th Gaussian in depth order
 __global__ void __launch_bounds__(256)
-tiles_gather_kernel(const uint32_t* __restrict__ order, const uint32_t* __restrict__ tiles,
-                    FrameCounters* __restrict__ c, uint32_t* __restrict__ tt_sorted, uint32_t N) {
-    __shared__ unsigned long long wsum[8];
+tiles_gather_kernel(const uint32_t* __restrict__ order, const uint32_t* __restrict__ tiles, uint32_t V,
+                    uint32_t* __restrict__ tt_sorted) {
     const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
-    uint32_t t = 0;
-    if (k < N) {
-        if (k < c->V) t = tiles[order[k]];
-        tt_sorted[k] = t;
-    }
-    unsigned long long s = t;
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) s += __shfl_down_sync(0xffffffffu, s, d);
-    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = s;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        unsigned long long b = 0;
-        for (int w = 0; w < 8; ++w) b += wsum[w];
-        if (b) atomicAdd(&c->D, b);
-    }
+    if (k < V) tt_sorted[k] = tiles[order[k]];
 }
 
-// One warp per Gaussian (in depth order): lanes stride over the rectangle's tiles.
+// A warp takes 32 consecutive Gaussians of the depth order. Each lane writes the first entries of its own Gaussian
+// (neighbouring lanes own neighbouring output slots), then the warp sweeps the long rectangles together.
 __global__ void __launch_bounds__(256)
 emit_kernel(const uint32_t* __restrict__ order, const uint32_t* __restrict__ offs, const uint4* __restrict__ rect,
             const uint32_t* __restrict__ tiles, uint32_t V, uint32_t gx, uint32_t* __restrict__ ent_key,
             uint32_t* __restrict__ ent_val) {
-    const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (warp >= V) return;
-    const uint32_t g = order[warp];
-    const uint32_t nt = tiles[g];
-    if (nt == 0) return;
-    const uint4 rc = rect[g];
-    const uint32_t w = rc.y - rc.x;
-    const uint32_t base = offs[warp];
-    for (uint32_t i = lane; i < nt; i += 32) {
-        const uint32_t ty = rc.z + i / w, tx = rc.x + i % w;
-        ent_key[base + i] = ty * gx + tx;
+    constexpr uint32_t kOwn = 4;
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    uint32_t g = 0, nt = 0, base = 0;
+    uint4 rc = make_uint4(0, 1, 0, 0);
+    if (k < V) {
+        g = order[k];
+        nt = tiles[g];
+        rc = rect[g];
+        base = offs[k];
+    }
+    uint32_t w = rc.y - rc.x;
+    const uint32_t own = nt < kOwn ? nt : kOwn;
+    for (uint32_t i = 0; i < own; ++i) {
+        ent_key[base + i] = (rc.z + i / w) * gx + rc.x + i % w;
         ent_val[base + i] = g;
+    }
+    uint32_t big = __ballot_sync(0xffffffffu, nt > kOwn);
+    while (big) {
+        const int src = __ffs(big) - 1;
+        big &= big - 1;
+        const uint32_t g2 = __shfl_sync(0xffffffffu, g, src), nt2 = __shfl_sync(0xffffffffu, nt, src);
+        const uint32_t b2 = __shfl_sync(0xffffffffu, base, src);
+        const uint32_t x0 = __shfl_sync(0xffffffffu, rc.x, src), y0 = __shfl_sync(0xffffffffu, rc.z, src);
+        const uint32_t w2 = __shfl_sync(0xffffffffu, w, src);
+        for (uint32_t i = kOwn + lane; i < nt2; i += 32) {
+            ent_key[b2 + i] = (y0 + i / w2) * gx + x0 + i % w2;
+            ent_val[b2 + i] = g2;
+        }
     }
 }
 
@@ -74,16 +76,16 @@ void hy_launch_depth_prepare(hyrf_scene* s, uint32_t* launches) {
     ++*launches;
 }
 
-void hy_launch_tiles_gather(hyrf_scene* s, const uint32_t* order, uint32_t* launches) {
-    tiles_gather_kernel<<<(s->N + 255) / 256, 256, 0, s->stream>>>(order, s->tiles, s->counters, s->tt_sorted, s->N);
+void hy_launch_tiles_gather(hyrf_scene* s, const uint32_t* order, uint32_t V, uint32_t* launches) {
+    if (V == 0) return;
+    tiles_gather_kernel<<<(V + 255) / 256, 256, 0, s->stream>>>(order, s->tiles, V, s->tt_sorted);
     ++*launches;
 }
 
 void hy_launch_emit(hyrf_scene* s, const uint32_t* order, uint32_t V, uint32_t* launches) {
     if (V == 0) return;
     const uint32_t gx = (uint32_t)((s->lastW + HY_TILE - 1) / HY_TILE);
-    const uint64_t threads = (uint64_t)V * 32ull;
-    emit_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, s->stream>>>(order, s->offs, s->rect, s->tiles, V, gx,
+    emit_kernel<<<(V + 255) / 256, 256, 0, s->stream>>>(order, s->offs, s->rect, s->tiles, V, gx,
                                                                           s->ent_key[0], s->ent_val[0]);
     ++*launches;
 }

@@ -14,7 +14,7 @@ struct FieldArgs {
     uint32_t N;
     uint32_t pe_octaves;
     const uint32_t* vis_idx;
-    const FrameCounters* counters;
+    FrameCounters* counters;
     float4* rec;
     uint32_t* depth_key;
     uint4* rect;
@@ -114,6 +114,11 @@ static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, uin
             rc = make_uint4((uint32_t)fx0, (uint32_t)fx1, (uint32_t)fy0, (uint32_t)fy1);
             if (rc.y > rc.x && rc.w > rc.z) nt = (rc.y - rc.x) * (rc.w - rc.z);
         }
+    }
+    {   // D = sum of tiles touched: one atomic per warp
+        const unsigned am = __activemask();
+        const uint32_t wsum = __reduce_add_sync(am, nt);
+        if ((threadIdx.x & 31u) == (uint32_t)(__ffs(am) - 1) && wsum) atomicAdd(&A.counters->D, (unsigned long long)wsum);
     }
     A.rec[3ull * j + 0] = make_float4(u, v, cA, cB);
     A.rec[3ull * j + 1] = make_float4(cC, alpha, c0, c1);

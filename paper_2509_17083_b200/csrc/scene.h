@@ -82,6 +82,7 @@ struct hyrf_scene {
     float* dbg_attrs = nullptr;       // [N][11]
     bool timing = false;
     cudaEvent_t ev[7] = {};
+    cudaEvent_t ev_counters = nullptr;
     bool ev_valid = false;
     uint32_t last_launches = 0;
     uint32_t lastV = 0;
@@ -106,12 +107,13 @@ void hy_launch_scan(const uint32_t* in, uint32_t* out, size_t n, uint32_t* scrat
 // stable LSD radix sort of (key, val) pairs on bits [0, key_bits) (radix.cu). n_dev: device count (may be null ->
 // n_cap). Result ends in (*out_key, *out_val) which is either buffer pair.
 size_t hy_radix_hist_elems(size_t n_cap);
+size_t hy_radix_max_items();
 void hy_launch_radix(uint32_t* key_a, uint32_t* val_a, uint32_t* key_b, uint32_t* val_b, size_t n_cap,
                      const uint32_t* n_dev, int key_bits, uint32_t* hist, uint32_t* scan_scratch, cudaStream_t st,
                      uint32_t** out_key, uint32_t** out_val, uint32_t* launches);
 // S4b-c (bin.cu)
 void hy_launch_depth_prepare(hyrf_scene* s, uint32_t* launches);                       // (depth, rank) pairs
-void hy_launch_tiles_gather(hyrf_scene* s, const uint32_t* order, uint32_t* launches); // tt_sorted + D
+void hy_launch_tiles_gather(hyrf_scene* s, const uint32_t* order, uint32_t V, uint32_t* launches);
 void hy_launch_emit(hyrf_scene* s, const uint32_t* order, uint32_t V, uint32_t* launches);
 void hy_launch_ranges(hyrf_scene* s, const uint32_t* keys, uint64_t D, uint32_t n_tiles, uint32_t* launches);
 // S5 (raster.cu)
