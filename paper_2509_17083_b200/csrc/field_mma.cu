@@ -2,7 +2,10 @@
 //   contraction (Eq. 2) -> grid encodes (Eq. 3) -> direction PE (Eq. 5) -> decoders (Eq. 4, 6, "fully-fused
 //   MLP, 2 hidden layers x 64") -> aggregation (Eq. 7) -> EWA projection.
 // B200 design: a CTA owns a tile of 128 visible Gaussians = the 128 TMEM lanes. 256 threads: warps 0–3 gather the
-// geometry field, warps 4–7 the appearance field + PE, one thread per Gaussian each. Features go registers -> TMEM
+// geometry field, warps 4–7 the appearance field + PE. The gathers are bound by L1TEX wavefronts (one per distinct
+// 128-B line per instruction, profiles/r1a_README.md), so a warp takes 16 Gaussians at a time with TWO lanes per
+// Gaussian: lane l and lane l^16 fetch the x and x+1 corners, which share a line 31/32 of the time, in the same
+// instruction — 4 wavefronts per (Gaussian, level) instead of 8. Features go registers -> TMEM
 // (tcgen05.st, fp16 pairs) as the A operand; the weights sit in shared memory as the B operand (K-major core
 // matrices); tcgen05.mma accumulates fp32 in TMEM; the epilogue (tcgen05.ld, ReLU, round to fp16, tcgen05.st)
 // feeds the next layer without touching shared or global memory. Only the 48-byte projected record leaves the SM.
@@ -20,7 +23,7 @@ constexpr uint32_t kColDg = 0, kColDa = 64, kColAg = 128, kColAa = 160;
 // packed weight block (bytes): geo W1 [64 x 32], W2 [64 x 64], W3 [16 x 64]; app W1 [64 x 64], W2, W3
 constexpr uint32_t kOffG1 = 0, kOffG2 = 4096, kOffG3 = 12288, kOffA1 = 14336, kOffA2 = 22528, kOffA3 = 30720;
 constexpr uint32_t kPackedBytes = 32768;
-constexpr uint32_t kSmemBytes = 80 * 1024;   // > 227 KB / 3: at most two CTAs (2 x 256 TMEM columns) per SM
+constexpr uint32_t kSmemBytes = kPackedBytes;   // two CTAs (2 x 256 TMEM columns) per SM by registers; the rest of the 228 KB is L1
 
 // element (n, k) of an [N x Kp] K-major operand stored as 8x8 core matrices: half-index inside the operand
 __host__ __device__ inline uint32_t core_index(uint32_t n, uint32_t k, uint32_t Kp) {
@@ -51,6 +54,51 @@ __global__ void pack_weights_kernel(const __half* __restrict__ geo, const __half
 __device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
     __half2 h = __floats2half2_rn(lo, hi);
     return *reinterpret_cast<uint32_t*>(&h);
+}
+
+// D3 for one level with two lanes per Gaussian: this lane blends the four corners whose x bit is xb; the partner
+// lane (lane ^ 16) takes the other four; the sum of both (fp32) is rounded to a packed half2 feature pair.
+__device__ __forceinline__ uint32_t gather_level_pair(const GridDev& g, uint32_t l, const float x[3], uint32_t xb) {
+    const uint32_t N = g.res[l];
+    const float Nf = (float)N;
+    uint32_t ci[3];
+    float w[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const float u = __fmul_rn(x[a], Nf);
+        int i = (int)floorf(u);
+        i = min(i, (int)N - 1);
+        ci[a] = (uint32_t)i;
+        w[a] = __fsub_rn(u, (float)i);
+    }
+    const uint32_t vx = ci[0] + xb;
+    uint32_t idx[4];
+    if ((g.dense_mask >> l) & 1u) {
+        const uint32_t n1 = N + 1u;
+        const uint32_t b = vx + n1 * (ci[1] + n1 * ci[2]);
+        idx[0] = b; idx[1] = b + n1; idx[2] = b + n1 * n1; idx[3] = b + n1 * n1 + n1;
+    } else {
+        const uint32_t hy0 = ci[1] * 2654435761u, hy1 = hy0 + 2654435761u;
+        const uint32_t hz0 = ci[2] * 805459861u, hz1 = hz0 + 805459861u;
+        idx[0] = (vx ^ hy0 ^ hz0) & g.table_mask; idx[1] = (vx ^ hy1 ^ hz0) & g.table_mask;
+        idx[2] = (vx ^ hy0 ^ hz1) & g.table_mask; idx[3] = (vx ^ hy1 ^ hz1) & g.table_mask;
+    }
+    const __half2* tab = reinterpret_cast<const __half2*>(g.table) + g.offset[l];
+    float2 v[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v[k] = __half22float2(__ldg(tab + idx[k]));
+    const float ax = xb ? w[0] : __fsub_rn(1.0f, w[0]);
+    const float wy0 = __fsub_rn(1.0f, w[1]), wz0 = __fsub_rn(1.0f, w[2]);
+    float a0 = 0.0f, a1 = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float wt = __fmul_rn(__fmul_rn(ax, (k & 1) ? w[1] : wy0), (k & 2) ? w[2] : wz0);
+        a0 = __fmaf_rn(wt, v[k].x, a0);
+        a1 = __fmaf_rn(wt, v[k].y, a1);
+    }
+    a0 = __fadd_rn(a0, __shfl_xor_sync(0xffffffffu, a0, 16));
+    a1 = __fadd_rn(a1, __shfl_xor_sync(0xffffffffu, a1, 16));
+    return pack_h2(a0, a1);
 }
 
 // ReLU + round to fp16 of 32 fp32 accumulator columns -> 16 packed A columns
@@ -104,17 +152,30 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w) {
         uint32_t a[32];
 #pragma unroll
         for (int i = 0; i < 32; ++i) a[i] = 0u;
+        float x[3] = {0.5f, 0.5f, 0.5f};
         if (valid) {
             gid = A.vis_idx[j];
             px = __ldg(A.pos + gid); py = __ldg(A.pos + A.N + gid); pz = __ldg(A.pos + 2ull * A.N + gid);
-            float x[3];
             hy_contract(A.f, px, py, pz, x);
+        }
+        {   // two lanes per Gaussian: half h covers rows 16h..16h+15 of this warp; row r's own lane keeps the result
+            const uint32_t lane = threadIdx.x & 31u, xb = lane >> 4;
 #pragma unroll
-            for (int l = 0; l < 16; ++l) {
-                float f0, f1;
-                hy_grid_level<true>(grid, l, x, f0, f1);
-                a[l] = pack_h2(f0, f1);
+            for (uint32_t h = 0; h < 2; ++h) {
+                const int src = (int)((h << 4) | (lane & 15u));
+                float xs[3];
+                xs[0] = __shfl_sync(0xffffffffu, x[0], src);
+                xs[1] = __shfl_sync(0xffffffffu, x[1], src);
+                xs[2] = __shfl_sync(0xffffffffu, x[2], src);
+                const bool own = xb == h;
+#pragma unroll
+                for (int l = 0; l < 16; ++l) {
+                    const uint32_t p = gather_level_pair(grid, l, xs, xb);
+                    a[l] = own ? p : a[l];
+                }
             }
+        }
+        if (valid) {
             if (chain) {
                 const float dx = __fsub_rn(px, A.f.o[0]), dy = __fsub_rn(py, A.f.o[1]), dz = __fsub_rn(pz, A.f.o[2]);
                 const float n = __fsqrt_rn(__fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx))));
@@ -124,6 +185,10 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w) {
 #pragma unroll
                 for (int i = 0; i < 12; ++i) a[16 + i] = pack_h2(pe[2 * i], pe[2 * i + 1]);
             }
+        }
+        if (!valid) {
+#pragma unroll
+            for (int l = 0; l < 16; ++l) a[l] = 0u;
         }
         // ---- layer 1: A <- features, D = A W1^T ----
         tc::st_x16(tA + lane_base, a);
