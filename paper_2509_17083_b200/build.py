@@ -45,13 +45,28 @@ def build(force: bool = False, verbose: bool = False) -> str:
     bdir = os.path.join(HERE, "build")
     os.makedirs(bdir, exist_ok=True)
 
+    hdr = hashlib.sha1()
+    for f in sorted(os.listdir(CSRC)):
+        if not f.endswith(".cu"):
+            with open(os.path.join(CSRC, f), "rb") as fh:
+                hdr.update(f.encode() + b"\0" + fh.read())
+    with open(os.path.join(ROOT, "include", "hyrf.h"), "rb") as fh:
+        hdr.update(fh.read())
+    hdr.update(" ".join(FLAGS).encode())
+
     def compile_one(src: str) -> str:
         obj = os.path.join(bdir, os.path.basename(src)[:-3] + ".o")
+        with open(src, "rb") as fh:
+            key = hashlib.sha1(hdr.digest() + fh.read()).hexdigest()
+        if not force and os.path.exists(obj) and os.path.exists(obj + ".key") and open(obj + ".key").read() == key:
+            return obj                       # this translation unit and every header are unchanged
         r = subprocess.run([NVCC, *FLAGS, "-c", src, "-o", obj], capture_output=True, text=True)
         with open(obj + ".log", "w") as f:
             f.write(r.stdout + r.stderr)
         if r.returncode != 0:
             raise RuntimeError(f"nvcc failed for {src}:\n{r.stdout}\n{r.stderr}")
+        with open(obj + ".key", "w") as f:
+            f.write(key)
         if verbose:
             print(r.stderr)
         return obj

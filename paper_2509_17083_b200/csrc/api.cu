@@ -151,7 +151,7 @@ void destroy(hyrf_scene* s) {
                     (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w,
                     s->flag_words, s->block_counts, s->vis_idx, s->rec, s->depth_key, s->rect, s->tiles,
                     s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->tt_sorted, s->offs,
-                    s->scan_scratch, s->counters, s->ranges, s->fg, s->finalT, s->image, s->bg_mask,
+                    s->scan_scratch, s->bin_ws, s->counters, s->ranges, s->fg, s->finalT, s->image, s->bg_mask,
                     s->dbg_vis_mask, s->dbg_raw, s->dbg_attrs};
     for (void* p : ptrs) dev_free(s, p);
     free_entries(s);
@@ -257,6 +257,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc_t(s, &s->counters, 1));
     HY_TRY(dev_alloc_t(s, &s->ranges, tiles));
     HY_TRY(dev_alloc_t(s, &s->finalT, P));
+    if (hy_bin_ordered_ws_elems(s->N, (uint32_t)tiles)) HY_TRY(dev_alloc_t(s, &s->bin_ws, hy_bin_ordered_ws_elems(s->N, (uint32_t)tiles)));
     if ((e = cudaMallocHost(reinterpret_cast<void**>(&s->counters_host), sizeof(FrameCounters))) != cudaSuccess) {
         destroy(s);
         return hy_cuda_fail(e, "cudaMallocHost");
@@ -375,42 +376,64 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
         return hy_cuda_fail(e, "cudaMemcpyAsync(counters)");
     if ((e = cudaEventRecord(s->ev_counters, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(counters)");
 
-    // S4b-c: order the visible Gaussians by (depth bits, id), lay out the tile entries, order them by tile
+    // S4b-c: order the visible Gaussians by (depth bits, id), then build the per-tile lists in that order
     hy_launch_depth_prepare(s, &launches);
     uint32_t *order_key = nullptr, *order = nullptr;
     hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, s->hist,
                     s->scan_scratch, s->stream, &order_key, &order, &launches);
-    if ((e = cudaEventSynchronize(s->ev_counters)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventSynchronize(counters)");
-    const uint32_t V = s->counters_host->V;
-    const uint64_t D = s->counters_host->D;
-    if (D >= 0xFFFFFFFFull || D > hy_radix_max_items())
-        return hy_fail(HYRF_ERR_OOM, "tile-entry count %llu exceeds the supported maximum", (unsigned long long)D);
-    if (D > s->d_capacity) {
-        // growing frees the sort workspace the depth ordering is still using: wait for it first
-        if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(grow)");
-        // the depth order lives in the N-sized buffers, which are not reallocated
-        if ((st = ensure_entries(s, (size_t)D)) != HYRF_OK) return st;
-    }
-    hy_launch_tiles_gather(s, order, V, &launches);
-    hy_launch_scan(s->tt_sorted, s->offs, V, s->scan_scratch, s->stream, &launches);
-    hy_launch_emit(s, order, V, &launches);
     const uint32_t n_tiles = (uint32_t)(f.gx * f.gy);
-    int tile_bits = 1;
-    while ((1u << tile_bits) < n_tiles) ++tile_bits;
-    uint32_t *sorted_key = nullptr, *sorted_val = nullptr;
-    hy_launch_radix(s->ent_key[0], s->ent_val[0], s->ent_key[1], s->ent_val[1], (size_t)D, nullptr, tile_bits, s->hist,
-                    s->scan_scratch, s->stream, &sorted_key, &sorted_val, &launches);
-    hy_launch_ranges(s, sorted_key, D, n_tiles, &launches);
-    s->list_final = sorted_val;
-    if (timing) cudaEventRecord(s->ev[3], s->stream);
-
-    // S5: alpha blending (Eq. 1)
-    hy_launch_raster(s, f, sorted_val, out_rgb, &launches);
-    if (timing) cudaEventRecord(s->ev[4], s->stream);
-
-    // S6: background (Eq. 10-11, A.2)
-    if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;
-    if (timing) cudaEventRecord(s->ev[5], s->stream);
+    uint32_t V = 0;
+    uint64_t D = 0;
+    if (s->bin_ws && hy_bin_ordered_supported(s->N, n_tiles)) {
+        // ordered counting route: everything is sized on the device, so the whole frame is enqueued before the host
+        // looks at the counters; only a frame whose D outgrew the list buffer is re-binned after growing it
+        for (int attempt = 0;; ++attempt) {
+            if ((st = hy_launch_bin_ordered(s, order, n_tiles, (uint32_t)f.gx, &launches)) != HYRF_OK) return st;
+            s->list_final = s->ent_val[0];
+            if (timing) cudaEventRecord(s->ev[3], s->stream);
+            hy_launch_raster(s, f, s->list_final, out_rgb, &launches);      // S5 (Eq. 1)
+            if (timing) cudaEventRecord(s->ev[4], s->stream);
+            if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;   // S6 (Eq. 10-11, A.2)
+            if (timing) cudaEventRecord(s->ev[5], s->stream);
+            if (attempt == 0 && (e = cudaEventSynchronize(s->ev_counters)) != cudaSuccess)
+                return hy_cuda_fail(e, "cudaEventSynchronize(counters)");
+            V = s->counters_host->V;
+            D = s->counters_host->D;
+            if (D >= 0xFFFFFFFFull) return hy_fail(HYRF_ERR_OOM, "tile-entry count %llu does not fit 32-bit offsets", (unsigned long long)D);
+            if (D <= s->d_capacity) break;
+            if (attempt > 0) return hy_fail(HYRF_ERR_OOM, "tile-entry scratch still too small after growing");
+            if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(grow)");
+            if ((st = ensure_entries(s, (size_t)D)) != HYRF_OK) return st;
+        }
+    } else {
+        // radix route (very large tile grids): (tile, rank) pairs emitted in depth order, stable sort by tile id
+        if ((e = cudaEventSynchronize(s->ev_counters)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventSynchronize(counters)");
+        V = s->counters_host->V;
+        D = s->counters_host->D;
+        if (D >= 0xFFFFFFFFull || D > hy_radix_max_items())
+            return hy_fail(HYRF_ERR_OOM, "tile-entry count %llu exceeds the supported maximum", (unsigned long long)D);
+        if (D > s->d_capacity) {
+            // growing frees the sort workspace the depth ordering is still using: wait for it first
+            if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(grow)");
+            // the depth order lives in the N-sized buffers, which are not reallocated
+            if ((st = ensure_entries(s, (size_t)D)) != HYRF_OK) return st;
+        }
+        hy_launch_tiles_gather(s, order, V, &launches);
+        hy_launch_scan(s->tt_sorted, s->offs, V, s->scan_scratch, s->stream, &launches);
+        hy_launch_emit(s, order, V, &launches);
+        int tile_bits = 1;
+        while ((1u << tile_bits) < n_tiles) ++tile_bits;
+        uint32_t *sorted_key = nullptr, *sorted_val = nullptr;
+        hy_launch_radix(s->ent_key[0], s->ent_val[0], s->ent_key[1], s->ent_val[1], (size_t)D, nullptr, tile_bits, s->hist,
+                        s->scan_scratch, s->stream, &sorted_key, &sorted_val, &launches);
+        hy_launch_ranges(s, sorted_key, D, n_tiles, &launches);
+        s->list_final = sorted_val;
+        if (timing) cudaEventRecord(s->ev[3], s->stream);
+        hy_launch_raster(s, f, sorted_val, out_rgb, &launches);             // S5 (Eq. 1)
+        if (timing) cudaEventRecord(s->ev[4], s->stream);
+        if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;       // S6 (Eq. 10-11, A.2)
+        if (timing) cudaEventRecord(s->ev[5], s->stream);
+    }
 
     if ((e = cudaGetLastError()) != cudaSuccess) return hy_cuda_fail(e, "kernel launch");
     s->last_launches = launches;

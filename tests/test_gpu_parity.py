@@ -106,6 +106,14 @@ def test_edge_cases(B, ho, synth):
         _run(B, ho, s, cams=s.cameras[:1])
 
 
+def test_large_tile_grid_takes_radix_route(B, ho, synth):
+    # 104 x 100 = 10,400 tiles > the ordered-counting limit: binning falls back to (tile, rank) pairs + radix sort
+    s = synth.tiny_scene(n=400, W=1664, H=1600, scale_mean=-3.0)
+    s.tau_T = 1.0                                                  # no background pixels: keeps the oracle quick
+    st = _run(B, ho, s, cams=s.cameras[:1])
+    assert st[0]["D"] > st[0]["V"]
+
+
 def test_status_codes_on_device(B, synth):
     import ctypes as C
     import torch
