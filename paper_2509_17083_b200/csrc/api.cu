@@ -151,7 +151,7 @@ void destroy(hyrf_scene* s) {
                     (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w,
                     s->flag_words, s->block_counts, s->vis_idx, s->rec, s->depth_key, s->rect, s->tiles,
                     s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->tt_sorted, s->offs,
-                    s->scan_scratch, s->bin_ws, s->counters, s->ranges, s->fg, s->finalT, s->image, s->bg_mask,
+                    s->scan_scratch, s->bin_ws, s->counters, s->ranges, s->fg, s->finalT, s->image, s->bg_mask, s->bg_list,
                     s->dbg_vis_mask, s->dbg_raw, s->dbg_attrs};
     for (void* p : ptrs) dev_free(s, p);
     free_entries(s);
@@ -257,6 +257,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc_t(s, &s->counters, 1));
     HY_TRY(dev_alloc_t(s, &s->ranges, tiles));
     HY_TRY(dev_alloc_t(s, &s->finalT, P));
+    HY_TRY(dev_alloc_t(s, &s->bg_list, P));
     if (hy_bin_ordered_ws_elems(s->N, (uint32_t)tiles)) HY_TRY(dev_alloc_t(s, &s->bin_ws, hy_bin_ordered_ws_elems(s->N, (uint32_t)tiles)));
     if ((e = cudaMallocHost(reinterpret_cast<void**>(&s->counters_host), sizeof(FrameCounters))) != cudaSuccess) {
         destroy(s);
@@ -388,6 +389,8 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
         // ordered counting route: everything is sized on the device, so the whole frame is enqueued before the host
         // looks at the counters; only a frame whose D outgrew the list buffer is re-binned after growing it
         for (int attempt = 0;; ++attempt) {
+            if (attempt > 0 && (e = cudaMemsetAsync(&s->counters->n_bg, 0, sizeof(uint32_t), s->stream)) != cudaSuccess)
+                return hy_cuda_fail(e, "cudaMemsetAsync(n_bg)");   // the first attempt's rasterizer already filled it
             if ((st = hy_launch_bin_ordered(s, order, n_tiles, (uint32_t)f.gx, &launches)) != HYRF_OK) return st;
             s->list_final = s->ent_val[0];
             if (timing) cudaEventRecord(s->ev[3], s->stream);

@@ -16,7 +16,8 @@ struct BgArgs {
     uint32_t pe_octaves;
     const float* finalT;
     float* out_rgb;
-    uint8_t* bg_mask;
+    const uint32_t* bg_list;          // pixels with T > tau_T, compacted by the rasterizer
+    const FrameCounters* counters;
 };
 
 template <int CL, int CHID, int CNH, bool FP16>
@@ -35,13 +36,11 @@ background_kernel(const BgArgs A) {
     }
     __syncthreads();
     const FrameDev& f = A.f;
-    const int P = f.W * f.H;
     constexpr int MAXD = CL > 0 ? (2 * CL + 24 > CHID ? 2 * CL + 24 : CHID) : HYRF_MAX_WIDTH;
-    for (int p = blockIdx.x * kBgThreads + threadIdx.x; p < P; p += gridDim.x * kBgThreads) {
+    const uint32_t n_bg = A.counters->n_bg;
+    for (uint32_t q = blockIdx.x * kBgThreads + threadIdx.x; q < n_bg; q += gridDim.x * kBgThreads) {
+        const int p = (int)A.bg_list[q];
         const float T = A.finalT[p];
-        const bool on = T > f.tau_T;
-        if (A.bg_mask) A.bg_mask[p] = on ? 1 : 0;
-        if (!on) continue;
         const int pi = p % f.W, pj = p / f.W;
         const float dcx = __fdiv_rn(__fsub_rn((float)pi, f.cx), f.fx), dcy = __fdiv_rn(__fsub_rn((float)pj, f.cy), f.fy);
         float dw[3], d[3], ps[3];
@@ -97,7 +96,7 @@ hyrf_status hy_launch_background(hyrf_scene* s, const FrameDev& f, float* out_rg
     A.grid = s->bg_grid; A.mlp = s->bg_mlp; A.f = f;
     A.pe_octaves = s->desc.dir_pe_octaves;
     A.finalT = s->finalT; A.out_rgb = out_rgb;
-    A.bg_mask = ((s->debug_mask >> HYRF_DBG_BG_MASK) & 1u) ? s->bg_mask : nullptr;
+    A.bg_list = s->bg_list; A.counters = s->counters;
     const hyrf_mlp_desc& m = s->desc.bg_mlp;
     const size_t smem = ((size_t)m.in_dim * m.hidden + (size_t)(m.n_hidden - 1) * m.hidden * m.hidden + (size_t)m.hidden * 3) * sizeof(float);
     const int P = f.W * f.H;

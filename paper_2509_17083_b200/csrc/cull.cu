@@ -78,6 +78,7 @@ cull_compact_kernel(const uint32_t* __restrict__ flag_words, const uint32_t* __r
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) {
         counters->V = boff + block_counts[blockIdx.x];
         counters->D = 0ull;
+        counters->n_bg = 0u;
     }
 }
 

@@ -11,7 +11,8 @@ constexpr int kBatch = HY_TILE * HY_TILE;
 
 __global__ void __launch_bounds__(kBatch)
 raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ list, const float4* __restrict__ rec,
-              int W, int H, int gx, float* __restrict__ out_rgb, float* __restrict__ finalT,
+              int W, int H, int gx, float tau_T, float* __restrict__ out_rgb, float* __restrict__ finalT,
+              uint32_t* __restrict__ bg_list, FrameCounters* __restrict__ counters, uint8_t* __restrict__ bg_mask,
               float* __restrict__ dbg_fg) {
     __shared__ float4 s_r0[kBatch];
     __shared__ float4 s_r1[kBatch];
@@ -61,6 +62,18 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
         finalT[o] = T;
         if (dbg_fg) { dbg_fg[3 * o] = C0; dbg_fg[3 * o + 1] = C1; dbg_fg[3 * o + 2] = C2; }
     }
+    // S6 work list: pixels with T > tau_T, appended with one atomic per warp. The order of the list is
+    // arbitrary; the background of a pixel does not depend on it.
+    const bool want_bg = inside && T > tau_T;
+    if (inside && bg_mask) bg_mask[(size_t)py * W + px] = want_bg ? 1 : 0;
+    const uint32_t bal = __ballot_sync(0xffffffffu, want_bg);
+    if (bal) {
+        const uint32_t lane = threadIdx.x & 31u;
+        uint32_t base = 0;
+        if (lane == 0) base = atomicAdd(&counters->n_bg, (uint32_t)__popc(bal));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (want_bg) bg_list[base + __popc(bal & ((1u << lane) - 1u))] = (uint32_t)(py * W + px);
+    }
 }
 
 }  // namespace
@@ -68,7 +81,9 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
 void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint32_t* list, float* out_rgb, uint32_t* launches) {
     dim3 grid((unsigned)f.gx, (unsigned)f.gy);
     const bool want_fg = (s->debug_mask >> HYRF_DBG_FG) & 1u;
-    raster_kernel<<<grid, kBatch, 0, s->stream>>>(s->ranges, list, s->rec, f.W, f.H, f.gx, out_rgb, s->finalT,
+    const bool want_mask = (s->debug_mask >> HYRF_DBG_BG_MASK) & 1u;
+    raster_kernel<<<grid, kBatch, 0, s->stream>>>(s->ranges, list, s->rec, f.W, f.H, f.gx, f.tau_T, out_rgb, s->finalT,
+                                                  s->bg_list, s->counters, want_mask ? s->bg_mask : nullptr,
                                                   want_fg ? s->fg : nullptr);
     ++*launches;
 }

@@ -19,7 +19,8 @@ struct FrameCounters {
     uint32_t V;           // visible Gaussians after S1
     uint32_t pad0;
     unsigned long long D; // tile entries (sum of tiles touched)
-    uint32_t pad[4];
+    uint32_t n_bg;        // pixels whose residual transmittance passes tau_T (S6 work list)
+    uint32_t pad[3];
 };
 
 struct hyrf_scene {
@@ -75,6 +76,7 @@ struct hyrf_scene {
     float* finalT = nullptr;  // [H][W]
     float* image = nullptr;   // [H][W][3] for hyrf_render_host
     uint8_t* bg_mask = nullptr;
+    uint32_t* bg_list = nullptr;  // [H*W] pixels S6 has to shade, appended by the rasterizer
 
     // debug / measurement
     uint32_t debug_mask = 0;
