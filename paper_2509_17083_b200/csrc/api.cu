@@ -113,6 +113,7 @@ void free_entries(hyrf_scene* s) {
         dev_free(s, s->ent_val[i]); s->ent_val[i] = nullptr;
     }
     dev_free(s, s->hist); s->hist = nullptr;
+    dev_free(s, s->bin_ws); s->bin_ws = nullptr;
     s->d_capacity = 0;
 }
 
@@ -132,6 +133,12 @@ hyrf_status ensure_entries(hyrf_scene* s, size_t need) {
     const size_t cap_sort = cap > s->N ? cap : s->N;
     s->hist_elems = hy_radix_hist_elems(cap_sort);
     if ((st = dev_alloc_t(s, &s->hist, s->hist_elems)) != HYRF_OK) { free_entries(s); return st; }
+    {   // ordered-binning workspace scales with the list capacity (bin_ordered.cu); look-back words start cleared
+        const size_t tiles_max = (size_t)((s->desc.max_width + HY_TILE - 1) / HY_TILE) * ((s->desc.max_height + HY_TILE - 1) / HY_TILE);
+        const size_t elems = hy_bin_ordered_ws_elems(s->N, cap, (uint32_t)tiles_max);
+        if ((st = dev_alloc_t(s, &s->bin_ws, elems)) != HYRF_OK) { free_entries(s); return st; }
+        if (cudaMemsetAsync(s->bin_ws, 0, elems * sizeof(uint32_t), s->stream) != cudaSuccess) { free_entries(s); return hy_cuda_fail(cudaGetLastError(), "cudaMemsetAsync(bin_ws)"); }
+    }
     const size_t need_scan = hy_scan_scratch_elems(s->hist_elems) + hy_scan_scratch_elems(s->N) + 64;
     if (need_scan > s->scan_scratch_elems) {
         dev_free(s, s->scan_scratch);
@@ -151,7 +158,7 @@ void destroy(hyrf_scene* s) {
                     (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w,
                     s->flag_words, s->block_counts, s->vis_idx, s->rec, s->depth_key, s->rect, s->tiles,
                     s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->tt_sorted, s->offs,
-                    s->scan_scratch, s->bin_ws, s->counters, s->ranges, s->fg, s->finalT, s->image, s->bg_mask, s->bg_list,
+                    s->scan_scratch, s->counters, s->ranges, s->fg, s->finalT, s->image, s->bg_mask, s->bg_list,
                     s->dbg_vis_mask, s->dbg_raw, s->dbg_attrs};
     for (void* p : ptrs) dev_free(s, p);
     free_entries(s);
@@ -258,7 +265,6 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc_t(s, &s->ranges, tiles));
     HY_TRY(dev_alloc_t(s, &s->finalT, P));
     HY_TRY(dev_alloc_t(s, &s->bg_list, P));
-    if (hy_bin_ordered_ws_elems(s->N, (uint32_t)tiles)) HY_TRY(dev_alloc_t(s, &s->bin_ws, hy_bin_ordered_ws_elems(s->N, (uint32_t)tiles)));
     if ((e = cudaMallocHost(reinterpret_cast<void**>(&s->counters_host), sizeof(FrameCounters))) != cudaSuccess) {
         destroy(s);
         return hy_cuda_fail(e, "cudaMallocHost");
@@ -389,10 +395,10 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
         // ordered counting route: everything is sized on the device, so the whole frame is enqueued before the host
         // looks at the counters; only a frame whose D outgrew the list buffer is re-binned after growing it
         for (int attempt = 0;; ++attempt) {
-            if (attempt > 0 && (e = cudaMemsetAsync(&s->counters->n_bg, 0, sizeof(uint32_t), s->stream)) != cudaSuccess)
-                return hy_cuda_fail(e, "cudaMemsetAsync(n_bg)");   // the first attempt's rasterizer already filled it
+            if (attempt > 0 && (e = cudaMemsetAsync(&s->counters->n_bg, 0, 3 * sizeof(uint32_t), s->stream)) != cudaSuccess)
+                return hy_cuda_fail(e, "cudaMemsetAsync(n_bg)");   // n_bg, bin_ticket, bin_done: the first attempt used them
             if ((st = hy_launch_bin_ordered(s, order, n_tiles, (uint32_t)f.gx, &launches)) != HYRF_OK) return st;
-            s->list_final = s->ent_val[0];
+            s->list_final = s->ent_val[1];
             if (timing) cudaEventRecord(s->ev[3], s->stream);
             hy_launch_raster(s, f, s->list_final, out_rgb, &launches);      // S5 (Eq. 1)
             if (timing) cudaEventRecord(s->ev[4], s->stream);

@@ -3,105 +3,209 @@
 // PAPER.md:47 ("ordered by depth"), :57 (the sorted set a pixel blends); order defined in DESIGN.md §2 D9.
 //
 // Input: the visible Gaussians already in (depth bits, id) order (radix.cu, V items). Output: list[D] of visible ranks
-// and ranges[tile] = [start, end). The depth order is cut into chunks of `chunk` consecutive Gaussians, one CTA each:
-//   bin_count_kernel : cnt[chunk][tile]  = entries chunk c sends to tile t            (shared-memory histogram)
-//   bin_prefix_kernel: cnt[chunk][tile] <- sum over earlier chunks; totals[tile]      (column prefix)
-//   bin_emit_kernel  : start[tile] = exclusive scan of totals; every entry goes to
-//                      start[t] + cnt[c][t] + (entries of earlier Gaussians of the chunk in tile t).
-// Inside a chunk, warp w owns chunk/8 consecutive Gaussians; it walks their tile rectangles flattened 32 entries
-// at a time, in order, so "earlier" is: earlier warps (per-warp counts, prefixed) + earlier iterations (running
-// per-warp counter) + lower lanes of this iteration (match.any on the tile id). No atomics decide an output slot,
-// so the lists are deterministic and bit-equal to the oracle's. Traffic: 3 reads of the 16-B rectangle per visible
-// Gaussian + 4 B written per entry + the count matrix (rows x tiles x 4 B, L2-resident) three times, against
-// 8 B written + 2 x 16 B sorted + 8 B histogram + 4 B range scan per entry on the radix route (bin.cu).
+// and ranges[tile] = [start, end).
+//   bin_offsets_kernel: offs[k] = tile entries of the Gaussians before k in depth order (single-pass scan, look-back)
+//   bin_pairs_kernel  : the (tile, rank) pairs of every Gaussian, written at offs[k] — i.e. in depth order
+//   The pair sequence 0..D-1 is cut into chunks of Ec pairs, one CTA each (near Gaussians cover hundreds of tiles and
+//   far ones a few, so cutting by pairs — not by Gaussians — is what balances the CTAs):
+//   bin_count_kernel  : cnt[chunk][tile]  = pairs of chunk c in tile t                 (shared-memory histogram)
+//   bin_prefix_kernel : cnt[chunk][tile] <- sum over earlier chunks; totals[tile]      (column prefix)
+//   bin_scatter_kernel: start[tile] = exclusive scan of totals; a pair goes to
+//                       start[t] + cnt[c][t] + (earlier pairs of the chunk in tile t).
+// This is one stable counting-sort pass over all tile ids at once (up to 10240 bins) where the radix route needs
+// ceil(log2(tiles) / 8) passes. Inside a chunk warp w owns Ec/8 consecutive pairs and takes them 32 at a time, in
+// order, so "earlier" is: earlier warps (per-warp counts, prefixed) + earlier iterations (running per-warp counter) +
+// lower lanes of this iteration (match.any on the tile id). No atomic decides an output slot, so the lists are
+// deterministic and bit-equal to the oracle's.
 #include "scene.h"
 
 namespace {
 
 constexpr int kBinThreads = 256;
 constexpr int kBinWarps = kBinThreads / 32;
-constexpr uint32_t kMaxTiles = 10240;   // 20 B of shared memory per tile in bin_emit_kernel
-constexpr uint32_t kMaxRows = 1024;
+constexpr uint32_t kMaxTiles = 10240;     // 20 B of shared memory per tile in bin_emit_kernel
+constexpr uint32_t kMinChunk = 16384;     // entries per CTA
+constexpr uint32_t kMaxChunk = 61440;     // per-chunk per-tile counts are kept in 16 bits
+constexpr int kOffItems = 2048;           // Gaussians per CTA of the offsets scan
 
 struct BinArgs {
     const uint32_t* order;   // [V] visible rank of the k-th Gaussian in depth order
     const uint4* rect;       // [V] (x0, x1, y0, y1) by visible rank
     const uint32_t* tiles;   // [V] tiles touched by visible rank
-    const FrameCounters* counters;
-    uint32_t chunk;          // Gaussians per CTA (multiple of 256)
+    FrameCounters* counters;
+    uint32_t* offs;          // [V] exclusive prefix of tiles touched, in depth order
+    unsigned long long* scan_state;   // look-back words of bin_offsets_kernel, tagged with the frame number
+    uint32_t frame;
+    uint32_t Ec;             // entries per CTA (multiple of 8)
+    uint32_t rows_cap;       // rows of M
     uint32_t T, gx;
-    uint32_t* M;             // [rows][T]
+    uint32_t* M;             // [rows_cap][T]
     uint32_t* totals;        // [T]
+    uint32_t* starts;        // [T] exclusive scan of totals
     uint2* ranges;           // [T]
+    uint32_t* pair_tile;     // [cap] tile id of every pair, depth order
+    uint32_t* pair_rank;     // [cap] visible rank of every pair
     uint32_t* list;          // [cap]
     uint32_t cap;
 };
 
-// Warp-collective: visits the tile entries of Gaussians k0..k1-1 of the depth order, 32 entries per call of f,
-// ordered by (k, tile index inside the rectangle: y outer, x inner). f(tile, g, active).
-template <class F>
-__device__ __forceinline__ void walk_entries(const BinArgs& A, uint32_t k0, uint32_t k1, F&& f) {
-    const uint32_t lane = threadIdx.x & 31u;
-    for (uint32_t kb = k0; kb < k1; kb += 32) {
-        const uint32_t k = kb + lane;
-        uint32_t g = 0, nt = 0, x0 = 0, y0 = 0, w = 1;
-        if (k < k1) {
-            g = __ldg(A.order + k);
-            nt = __ldg(A.tiles + g);
-            if (nt) {
-                const uint4 rc = __ldg(A.rect + g);
-                x0 = rc.x; y0 = rc.z; w = rc.y - rc.x;
-            }
-        }
-        uint32_t incl = nt;
+__device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, uint32_t lane) {
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t u = __shfl_up_sync(0xffffffffu, incl, d);
-            if (lane >= (uint32_t)d) incl += u;
-        }
-        const uint32_t E = __shfl_sync(0xffffffffu, incl, 31);
-        const uint32_t excl = incl - nt;
-        for (uint32_t e0 = 0; e0 < E; e0 += 32) {
-            const uint32_t e = e0 + lane;
-            const bool act = e < E;
-            uint32_t q = 0;   // number of Gaussians of the batch whose entries all precede e
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t u = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane >= (uint32_t)d) v += u;
+    }
+    return v;
+}
+
+// ---- offs[k] = sum of tiles touched by the Gaussians before k (depth order): one pass, decoupled look-back ------
+// Look-back word: [63:34] frame number, [33:32] 1 = block aggregate / 2 = inclusive prefix, [31:0] value. Tagging with
+// the frame number means the words never have to be cleared between frames.
+__device__ __forceinline__ unsigned long long off_word(uint32_t frame, uint32_t kind, uint32_t v) {
+    return ((unsigned long long)frame << 34) | ((unsigned long long)kind << 32) | v;
+}
+
+__global__ void __launch_bounds__(kBinThreads)
+bin_offsets_kernel(const BinArgs A) {
+    __shared__ uint32_t s_tile, s_prefix;
+    __shared__ uint32_t s_warp[kBinWarps];
+    if (threadIdx.x == 0) s_tile = atomicAdd(&A.counters->bin_ticket, 1u);
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const uint32_t V = A.counters->V;
+    const uint32_t base = tile * kOffItems;
+    if (base >= V) return;   // tickets are handed out in order: every earlier tile exists and is running or done
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    constexpr int kPer = kOffItems / kBinThreads;   // 8 rounds; a warp owns 256 consecutive Gaussians
+    const uint32_t wbase = base + warp * (kPer * 32);
+    uint32_t v[kPer], ex[kPer];
+    uint32_t run = 0;
 #pragma unroll
-            for (int s = 16; s >= 1; s >>= 1) {
-                const uint32_t v = __shfl_sync(0xffffffffu, incl, (int)(q + s - 1));
-                if (v <= e) q += s;
+    for (int i = 0; i < kPer; ++i) {
+        const uint32_t k = wbase + i * 32 + lane;
+        v[i] = k < V ? __ldg(A.tiles + __ldg(A.order + k)) : 0u;
+    }
+#pragma unroll
+    for (int i = 0; i < kPer; ++i) {
+        const uint32_t incl = warp_incl_scan(v[i], lane);
+        ex[i] = run + incl - v[i];
+        run += __shfl_sync(0xffffffffu, incl, 31);
+    }
+    if (lane == 0) s_warp[warp] = run;
+    __syncthreads();
+    uint32_t woff = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < kBinWarps; ++w) {
+        if (w < (int)warp) woff += s_warp[w];
+        total += s_warp[w];
+    }
+    volatile unsigned long long* st = A.scan_state;
+    if (warp == 0) {
+        if (lane == 0) st[tile] = off_word(A.frame, tile == 0 ? 2u : 1u, total);
+        uint32_t prefix = 0;
+        if (tile > 0) {
+            int p = (int)tile - 1;
+            while (true) {
+                const int idx = p - (int)lane;
+                unsigned long long w = off_word(A.frame, 2u, 0u);   // before the first tile: inclusive 0
+                if (idx >= 0) {
+                    do { w = st[idx]; } while ((uint32_t)(w >> 34) != A.frame);
+                }
+                const uint32_t kind = (uint32_t)(w >> 32) & 3u, val = (uint32_t)w;
+                const uint32_t incl_mask = __ballot_sync(0xffffffffu, kind == 2u);
+                const uint32_t upto = incl_mask ? (uint32_t)__ffs(incl_mask) - 1u : 31u;
+                uint32_t part = lane <= upto ? val : 0u;
+#pragma unroll
+                for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(0xffffffffu, part, d);
+                prefix += part;
+                if (incl_mask) break;
+                p -= 32;
             }
-            q = q > 31u ? 31u : q;
-            const uint32_t i = e - __shfl_sync(0xffffffffu, excl, (int)q);
-            const uint32_t xq = __shfl_sync(0xffffffffu, x0, (int)q), yq = __shfl_sync(0xffffffffu, y0, (int)q);
-            const uint32_t wq = __shfl_sync(0xffffffffu, w, (int)q), gq = __shfl_sync(0xffffffffu, g, (int)q);
-            const uint32_t ii = act ? i : 0u;
-            const uint32_t row = (uint32_t)__fdividef((float)ii + 0.5f, (float)wq);   // exact: |error| << 0.5 / w
-            const uint32_t tile = (yq + row) * A.gx + xq + (ii - row * wq);
-            f(tile, gq, act);
+            if (lane == 0) st[tile] = off_word(A.frame, 2u, prefix + total);
+        }
+        if (lane == 0) s_prefix = prefix;
+    }
+    __syncthreads();
+    const uint32_t add = s_prefix + woff;
+#pragma unroll
+    for (int i = 0; i < kPer; ++i) {
+        const uint32_t k = wbase + i * 32 + lane;
+        if (k < V) A.offs[k] = add + ex[i];
+    }
+}
+
+
+// ---- (tile, rank) pairs in depth order ----------------------------------------------------------------------------
+// A warp takes 32 consecutive Gaussians of the depth order. Each lane writes the first pairs of its own Gaussian
+// (neighbouring lanes own neighbouring output slots), then the warp sweeps the long rectangles together.
+__global__ void __launch_bounds__(kBinThreads)
+bin_pairs_kernel(const BinArgs A) {
+    constexpr uint32_t kOwn = 4;
+    const uint32_t V = A.counters->V;
+    const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31u;
+    if (blockIdx.x * blockDim.x >= V) return;
+    uint32_t g = 0, nt = 0, base = 0;
+    uint4 rc = make_uint4(0, 1, 0, 0);
+    if (k < V) {
+        g = __ldg(A.order + k);
+        nt = __ldg(A.tiles + g);
+        rc = __ldg(A.rect + g);
+        base = A.offs[k];
+        if (nt == 0) rc = make_uint4(0, 1, 0, 0);
+    }
+    const uint32_t w = rc.y - rc.x;
+    const uint32_t own = nt < kOwn ? nt : kOwn;
+    for (uint32_t i = 0; i < own; ++i) {
+        const uint32_t row = i / w;
+        if (base + i < A.cap) {
+            A.pair_tile[base + i] = (rc.z + row) * A.gx + rc.x + (i - row * w);
+            A.pair_rank[base + i] = g;
+        }
+    }
+    uint32_t big = __ballot_sync(0xffffffffu, nt > kOwn);
+    while (big) {
+        const int src = __ffs(big) - 1;
+        big &= big - 1;
+        const uint32_t g2 = __shfl_sync(0xffffffffu, g, src), nt2 = __shfl_sync(0xffffffffu, nt, src);
+        const uint32_t b2 = __shfl_sync(0xffffffffu, base, src);
+        const uint32_t x0 = __shfl_sync(0xffffffffu, rc.x, src), y0 = __shfl_sync(0xffffffffu, rc.z, src);
+        const uint32_t w2 = __shfl_sync(0xffffffffu, w, src);
+        const float rw = 1.0f / (float)w2;
+        for (uint32_t i = kOwn + lane; i < nt2; i += 32) {
+            const uint32_t row = (uint32_t)(((float)i + 0.5f) * rw);   // exact: |error| << 0.5 / w
+            if (b2 + i < A.cap) {
+                A.pair_tile[b2 + i] = (y0 + row) * A.gx + x0 + (i - row * w2);
+                A.pair_rank[b2 + i] = g2;
+            }
         }
     }
 }
 
-__device__ __forceinline__ void chunk_bounds(const BinArgs& A, uint32_t& k0, uint32_t& k1, uint32_t& V) {
-    V = A.counters->V;
-    k0 = blockIdx.x * A.chunk;
-    k1 = k0 + A.chunk < V ? k0 + A.chunk : V;
+__device__ __forceinline__ uint32_t pair_count(const BinArgs& A) {
+    const unsigned long long D = A.counters->D;
+    return (uint32_t)(D < A.cap ? D : A.cap);
 }
 
 __global__ void __launch_bounds__(kBinThreads)
 bin_count_kernel(const BinArgs A) {
     extern __shared__ uint32_t s_cnt[];
-    uint32_t k0, k1, V;
-    chunk_bounds(A, k0, k1, V);
-    if (k0 >= V) return;
+    const uint32_t D = pair_count(A);
+    const uint32_t e0 = blockIdx.x * A.Ec;
+    if (e0 >= D) return;
+    const uint32_t e1 = e0 + A.Ec < D ? e0 + A.Ec : D;
     for (uint32_t t = threadIdx.x; t < A.T; t += kBinThreads) s_cnt[t] = 0;
     __syncthreads();
-    const uint32_t warp = threadIdx.x >> 5, seg = A.chunk / kBinWarps;
-    const uint32_t w0 = k0 + warp * seg, w1 = w0 + seg < k1 ? w0 + seg : k1;
-    if (w0 < k1)
-        walk_entries(A, w0, w1, [&](uint32_t tile, uint32_t, bool act) {
-            if (act) atomicAdd(&s_cnt[tile], 1u);
-        });
+    for (uint32_t eb = e0; eb < e1; eb += kBinThreads * 8) {
+        uint32_t tl[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const uint32_t e = eb + u * kBinThreads + threadIdx.x;
+            tl[u] = e < e1 ? __ldg(A.pair_tile + e) : 0xFFFFFFFFu;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            if (tl[u] != 0xFFFFFFFFu) atomicAdd(&s_cnt[tl[u]], 1u);
+    }
     __syncthreads();
     uint32_t* row = A.M + (size_t)blockIdx.x * A.T;
     for (uint32_t t = threadIdx.x; t < A.T; t += kBinThreads) row[t] = s_cnt[t];
@@ -111,12 +215,12 @@ bin_count_kernel(const BinArgs A) {
 __global__ void __launch_bounds__(1024)
 bin_prefix_kernel(const BinArgs A) {
     __shared__ uint32_t s_part[32][33];
-    const uint32_t V = A.counters->V;
-    const uint32_t rows = (V + A.chunk - 1) / A.chunk;
+    const uint32_t D = pair_count(A);
+    const uint32_t rows = (D + A.Ec - 1) / A.Ec;
     const uint32_t lane = threadIdx.x & 31u, grp = threadIdx.x >> 5;
     const uint32_t t = blockIdx.x * 32 + lane;
     const uint32_t per = (rows + 31) / 32;
-    const uint32_t r0 = grp * per, r1 = r0 + per < rows ? r0 + per : rows;
+    const uint32_t r0 = grp * per < rows ? grp * per : rows, r1 = r0 + per < rows ? r0 + per : rows;
     uint32_t sum = 0;
     if (t < A.T)
         for (uint32_t r = r0; r < r1; ++r) sum += A.M[(size_t)r * A.T + t];
@@ -138,50 +242,64 @@ bin_prefix_kernel(const BinArgs A) {
         }
         if (grp == 0) A.totals[t] = total;
     }
+    // the last CTA to finish turns totals[] into start[] (exclusive scan over the tiles) and writes ranges[]
+    __shared__ bool s_last;
+    __shared__ uint32_t s_wsum[32];
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(&A.counters->bin_done, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    const uint32_t per_t = (A.T + 1023u) / 1024u;
+    const uint32_t t0 = threadIdx.x * per_t < A.T ? threadIdx.x * per_t : A.T, t1 = t0 + per_t < A.T ? t0 + per_t : A.T;
+    uint32_t mine = 0;
+    for (uint32_t t2 = t0; t2 < t1; ++t2) mine += __ldcg(A.totals + t2);
+    const uint32_t incl = warp_incl_scan(mine, lane);
+    if (lane == 31) s_wsum[grp] = incl;
+    __syncthreads();
+    uint32_t start = incl - mine;
+    for (uint32_t w2 = 0; w2 < grp; ++w2) start += s_wsum[w2];
+    for (uint32_t t2 = t0; t2 < t1; ++t2) {
+        const uint32_t n = __ldcg(A.totals + t2);
+        A.ranges[t2] = n ? make_uint2(start, start + n) : make_uint2(0u, 0u);   // empty: [0, 0)
+        A.starts[t2] = start;
+        start += n;
+    }
 }
 
 __global__ void __launch_bounds__(kBinThreads)
-bin_emit_kernel(const BinArgs A) {
+bin_scatter_kernel(const BinArgs A) {
     extern __shared__ uint32_t s_mem[];
-    __shared__ uint32_t s_warp[kBinWarps];
     uint32_t* s_base = s_mem;                                               // [T] first slot of this chunk per tile
     unsigned short* s_wcnt = reinterpret_cast<unsigned short*>(s_mem + A.T); // [warps][Tp] per-warp counts -> running
     const uint32_t Tp = (A.T + 1u) & ~1u;
-    uint32_t k0, k1, V;
-    chunk_bounds(A, k0, k1, V);
-    if (k0 >= V && blockIdx.x != 0) return;   // CTA 0 always runs: it owns ranges[] (all empty when V = 0)
+    const uint32_t D = pair_count(A);
+    const uint32_t c0 = blockIdx.x * A.Ec;
+    if (c0 >= D) return;
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    // start[t] = exclusive scan of totals over the tiles (every CTA recomputes it: T <= 10240 values from L2)
-    const uint32_t per = (A.T + kBinThreads - 1) / kBinThreads;
-    const uint32_t t0 = threadIdx.x * per, t1 = t0 + per < A.T ? t0 + per : A.T;
-    uint32_t mine = 0;
-    for (uint32_t t = t0; t < t1; ++t) mine += A.totals[t];
-    uint32_t incl = mine;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t u = __shfl_up_sync(0xffffffffu, incl, d);
-        if (lane >= (uint32_t)d) incl += u;
-    }
-    if (lane == 31) s_warp[warp] = incl;
+    const uint32_t* row = A.M + (size_t)blockIdx.x * A.T;
+    for (uint32_t t = threadIdx.x; t < A.T; t += kBinThreads) s_base[t] = __ldg(A.starts + t) + __ldg(row + t);
     for (uint32_t i = threadIdx.x; i < kBinWarps * Tp / 2; i += kBinThreads) reinterpret_cast<uint32_t*>(s_wcnt)[i] = 0;
     __syncthreads();
-    uint32_t start = incl - mine;
-    for (uint32_t w2 = 0; w2 < warp; ++w2) start += s_warp[w2];
-    const uint32_t* row = A.M + (size_t)blockIdx.x * A.T;
-    for (uint32_t t = t0; t < t1; ++t) {
-        const uint32_t n = A.totals[t];
-        if (blockIdx.x == 0) A.ranges[t] = n ? make_uint2(start, start + n) : make_uint2(0u, 0u);   // empty: [0, 0)
-        s_base[t] = start + row[t];
-        start += n;
-    }
-    // per-warp counts
-    const uint32_t seg = A.chunk / kBinWarps;
-    const uint32_t w0 = k0 + warp * seg, w1 = w0 + seg < k1 ? w0 + seg : k1;
+    // warp w owns pairs [w0, w1) of the chunk
+    const uint32_t Ew = A.Ec / kBinWarps;
+    const uint32_t c1 = c0 + A.Ec < D ? c0 + A.Ec : D;
+    const uint32_t w0 = c0 + warp * Ew < c1 ? c0 + warp * Ew : c1, w1 = w0 + Ew < c1 ? w0 + Ew : c1;
+    // per-warp counts (two 16-bit counters per word; <= Ew <= 7680 pairs per warp: no carry)
     uint32_t* wc32 = reinterpret_cast<uint32_t*>(s_wcnt + (size_t)warp * Tp);
-    if (w0 < k1)
-        walk_entries(A, w0, w1, [&](uint32_t tile, uint32_t, bool act) {
-            if (act) atomicAdd(&wc32[tile >> 1], (tile & 1u) ? 0x10000u : 1u);   // seg <= 8191: no carry
-        });
+    constexpr int kU = 16;   // pairs per lane fetched together: the loads of 512 pairs are in flight at once
+    for (uint32_t eb = w0; eb < w1; eb += 32 * kU) {
+        uint32_t tl[kU];
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            const uint32_t e = eb + u * 32 + lane;
+            tl[u] = e < w1 ? __ldg(A.pair_tile + e) : 0xFFFFFFFFu;
+        }
+#pragma unroll
+        for (int u = 0; u < kU; ++u)
+            if (tl[u] != 0xFFFFFFFFu) atomicAdd(&wc32[tl[u] >> 1], (tl[u] & 1u) ? 0x10000u : 1u);
+    }
     __syncthreads();
     // per tile: counts -> exclusive prefix over the warps
     for (uint32_t t = threadIdx.x; t < A.T; t += kBinThreads) {
@@ -194,69 +312,87 @@ bin_emit_kernel(const BinArgs A) {
         }
     }
     __syncthreads();
-    // ordered emission
+    // ordered scatter, 32 pairs per step
     unsigned short* wc = s_wcnt + (size_t)warp * Tp;
-    if (w0 < k1)
-        walk_entries(A, w0, w1, [&](uint32_t tile, uint32_t g, bool act) {
+    for (uint32_t eb = w0; eb < w1; eb += 32 * kU) {
+        uint32_t tl[kU], gl[kU];
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            const uint32_t e = eb + u * 32 + lane;
+            const bool in = e < w1;
+            tl[u] = in ? __ldg(A.pair_tile + e) : 0xFFFFFFFFu;
+            gl[u] = in ? __ldg(A.pair_rank + e) : 0u;
+        }
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            if (eb + u * 32 >= w1) break;                    // warp-uniform
+            const uint32_t tile = tl[u];
+            const bool act = tile != 0xFFFFFFFFu;
             const uint32_t peers = __match_any_sync(0xffffffffu, act ? tile : (0x80000000u | lane));
             uint32_t c = 0;
             if (act) c = wc[tile];
             __syncwarp();
             if (act && lane == (uint32_t)(__ffs(peers) - 1)) wc[tile] = (unsigned short)(c + __popc(peers));
             __syncwarp();
-            if (act) {
-                const uint32_t slot = s_base[tile] + c + __popc(peers & ((1u << lane) - 1u));
-                if (slot < A.cap) A.list[slot] = g;
-            }
-        });
+            if (act) A.list[s_base[tile] + c + __popc(peers & ((1u << lane) - 1u))] = gl[u];   // slot < D <= cap
+        }
+    }
 }
 
-uint32_t chunk_for(uint32_t N) {
-    uint32_t c = (N + kMaxRows - 1) / kMaxRows;
-    c = (c + 255u) / 256u * 256u;
-    return c < 1024u ? 1024u : c;
+uint32_t chunk_entries(size_t cap) {
+    size_t c = (cap + 1023) / 1024;
+    c = (c + 2047) / 2048 * 2048;
+    if (c < kMinChunk) c = kMinChunk;
+    if (c > kMaxChunk) c = kMaxChunk;
+    return (uint32_t)c;
 }
 
 }  // namespace
 
-bool hy_bin_ordered_supported(uint32_t N, uint32_t n_tiles) {
-    return n_tiles <= kMaxTiles && chunk_for(N) / kBinWarps <= 8191u;
-}
+bool hy_bin_ordered_supported(uint32_t /*N*/, uint32_t n_tiles) { return n_tiles <= kMaxTiles; }
 
-// uint32 elements of workspace: count matrix + totals
-size_t hy_bin_ordered_ws_elems(uint32_t N, uint32_t max_tiles) {
-    if (!hy_bin_ordered_supported(N, 1)) return 0;
+// uint32 elements of workspace for a list capacity of `cap` entries: count matrix + totals + look-back words
+size_t hy_bin_ordered_ws_elems(uint32_t N, size_t cap, uint32_t max_tiles) {
     const uint32_t T = max_tiles < kMaxTiles ? max_tiles : kMaxTiles;
-    const size_t rows = (N + chunk_for(N) - 1) / chunk_for(N);
-    return rows * T + T + 64;
+    const size_t rows = (cap + chunk_entries(cap) - 1) / chunk_entries(cap) + 1;
+    return rows * T + 2 * T + 2 * ((size_t)N / kOffItems + 2) + 64;
 }
 
 hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t n_tiles, uint32_t gx,
                                   uint32_t* launches) {
     BinArgs A;
     A.order = order; A.rect = s->rect; A.tiles = s->tiles; A.counters = s->counters;
-    A.chunk = chunk_for(s->N);
+    A.offs = s->offs;
+    A.cap = (uint32_t)(s->d_capacity > 0xFFFFFFF0ull ? 0xFFFFFFF0ull : s->d_capacity);
+    A.Ec = chunk_entries(s->d_capacity);
+    A.rows_cap = (uint32_t)((s->d_capacity + A.Ec - 1) / A.Ec + 1);
     A.T = n_tiles; A.gx = gx;
-    const uint32_t rows = (s->N + A.chunk - 1) / A.chunk;
+    const uint32_t T_max = (uint32_t)(((s->desc.max_width + HY_TILE - 1) / HY_TILE) * ((s->desc.max_height + HY_TILE - 1) / HY_TILE));
+    const uint32_t T_ws = T_max < kMaxTiles ? T_max : kMaxTiles;
     A.M = s->bin_ws;
-    A.totals = s->bin_ws + (size_t)rows * n_tiles;
+    A.totals = s->bin_ws + (size_t)A.rows_cap * T_ws;
+    A.starts = A.totals + T_ws;
+    A.scan_state = reinterpret_cast<unsigned long long*>(s->bin_ws + (((size_t)A.rows_cap * T_ws + 2 * T_ws + 1) & ~(size_t)1));
+    A.frame = ++s->bin_frame & 0x3FFFFFFFu;
+    if (A.frame == 0) A.frame = ++s->bin_frame & 0x3FFFFFFFu;   // 0 is the tag of freshly cleared words
     A.ranges = s->ranges;
-    A.list = s->ent_val[0];
-    A.cap = (uint32_t)(s->d_capacity > 0xFFFFFFFFull ? 0xFFFFFFFFull : s->d_capacity);
+    A.pair_tile = s->ent_key[0];
+    A.pair_rank = s->ent_val[0];
+    A.list = s->ent_val[1];
     const size_t smem_count = (size_t)n_tiles * 4;
-    const size_t smem_emit = (size_t)n_tiles * 4 + (size_t)kBinWarps * ((n_tiles + 1u) & ~1u) * 2;
-    static size_t attr_count = 0, attr_emit = 0;
-    if (smem_count > attr_count) {
+    const size_t smem_scatter = (size_t)n_tiles * 4 + (size_t)kBinWarps * ((n_tiles + 1u) & ~1u) * 2;
+    static bool attr_set = false;
+    if (!attr_set) {
         HY_CUDA_OK(cudaFuncSetAttribute(bin_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxTiles * 4)));
-        attr_count = kMaxTiles * 4;
+        HY_CUDA_OK(cudaFuncSetAttribute(bin_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxTiles * 20)));
+        attr_set = true;
     }
-    if (smem_emit > attr_emit) {
-        HY_CUDA_OK(cudaFuncSetAttribute(bin_emit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxTiles * 20)));
-        attr_emit = kMaxTiles * 20;
-    }
-    bin_count_kernel<<<rows, kBinThreads, smem_count, s->stream>>>(A);
+    const uint32_t off_blocks = (s->N + kOffItems - 1) / kOffItems;
+    bin_offsets_kernel<<<off_blocks, kBinThreads, 0, s->stream>>>(A);
+    bin_pairs_kernel<<<(s->N + kBinThreads - 1) / kBinThreads, kBinThreads, 0, s->stream>>>(A);
+    bin_count_kernel<<<A.rows_cap, kBinThreads, smem_count, s->stream>>>(A);
     bin_prefix_kernel<<<(n_tiles + 31) / 32, 1024, 0, s->stream>>>(A);
-    bin_emit_kernel<<<rows, kBinThreads, smem_emit, s->stream>>>(A);
-    *launches += 3;
+    bin_scatter_kernel<<<A.rows_cap, kBinThreads, smem_scatter, s->stream>>>(A);
+    *launches += 5;
     return HYRF_OK;
 }

@@ -79,6 +79,8 @@ cull_compact_kernel(const uint32_t* __restrict__ flag_words, const uint32_t* __r
         counters->V = boff + block_counts[blockIdx.x];
         counters->D = 0ull;
         counters->n_bg = 0u;
+        counters->bin_ticket = 0u;
+        counters->bin_done = 0u;
     }
 }
 

@@ -20,7 +20,9 @@ struct FrameCounters {
     uint32_t pad0;
     unsigned long long D; // tile entries (sum of tiles touched)
     uint32_t n_bg;        // pixels whose residual transmittance passes tau_T (S6 work list)
-    uint32_t pad[3];
+    uint32_t bin_ticket;  // block tickets of bin_offsets_kernel
+    uint32_t bin_done;    // finished CTAs of bin_prefix_kernel
+    uint32_t pad[1];
 };
 
 struct hyrf_scene {
@@ -58,7 +60,8 @@ struct hyrf_scene {
     uint32_t* offs = nullptr;         // [N] exclusive scan of tt_sorted
     uint32_t* scan_scratch = nullptr; // pyramid for the device-wide scan
     size_t scan_scratch_elems = 0;
-    uint32_t* bin_ws = nullptr;       // ordered binning: count matrix [chunks][tiles] + totals (bin_ordered.cu)
+    uint32_t* bin_ws = nullptr;       // ordered binning: count matrix [chunks][tiles] + totals + look-back words
+    uint32_t bin_frame = 0;           // tag of the look-back words (bin_ordered.cu)
     uint32_t* hist = nullptr;         // [256][radix blocks] block histograms
     size_t hist_elems = 0;
     FrameCounters* counters = nullptr;       // device
@@ -121,7 +124,7 @@ void hy_launch_emit(hyrf_scene* s, const uint32_t* order, uint32_t V, uint32_t* 
 void hy_launch_ranges(hyrf_scene* s, const uint32_t* keys, uint64_t D, uint32_t n_tiles, uint32_t* launches);
 // S4b-c in one ordered counting pass (bin_ordered.cu), for frames of a bounded tile count; no host-side V or D
 bool hy_bin_ordered_supported(uint32_t N, uint32_t n_tiles);
-size_t hy_bin_ordered_ws_elems(uint32_t N, uint32_t max_tiles);
+size_t hy_bin_ordered_ws_elems(uint32_t N, size_t cap, uint32_t max_tiles);
 hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t n_tiles, uint32_t gx,
                                   uint32_t* launches);
 // S5 (raster.cu)
