@@ -1,58 +1,106 @@
 // raster.cu — S5: front-to-back alpha blending, Eq. 1, per 16x16 tile over its depth-ordered list.
 // Arithmetic DESIGN.md §2 D10 (constants of the 3DGS rasterizer the paper defers to).
 // One CTA per tile, one thread per pixel; list entries are staged through shared memory in batches of 256 so each
-// projected record is fetched once per tile; the CTA stops as soon as every pixel has terminated. Bound by plain
-// fp32 ALU issue + one MUFU.EX2 per pair — no tensor cores (nothing here is a dense contraction).
+// projected record is fetched once per tile, and entries that cannot reach alpha >= 1/255 anywhere in the tile are
+// dropped while staging (stable compaction, so the order is untouched). The per-pair body is branch-free
+// (profiles/r1a: divergent skip/stop branches cost 45 issue slots per pair against ~30 predicated); warps stop
+// when all of their pixels have terminated, the CTA when all warps have. Bound by plain fp32 ALU issue + one
+// MUFU.EX2 per pair — no tensor cores (nothing here is a dense contraction).
 #include "scene.h"
 
 namespace {
 
 constexpr int kBatch = HY_TILE * HY_TILE;
+constexpr int kWarps = kBatch / 32;
+
+// Can list entry (mean (u, v), conic (A, B, C), opacity o) reach alpha >= 1/255 at ANY pixel of the tile
+// [X0, X1] x [Y0, Y1]? The quadratic form q = A dx^2 + 2 B dx dy + C dy^2 is convex, so its minimum over the pixel box
+// is 0 when the mean lies inside, else it sits on a face whose plane separates the mean from the box: at most two
+// one-dimensional minimisations. alpha <= o exp(-q_min / 2) everywhere in the tile; entries below the threshold
+// (with a 1 % margin against rounding) would be skipped by every pixel, so dropping them changes no output bit.
+__device__ __forceinline__ bool entry_reaches_tile(float u, float v, float A, float B, float C, float o, float X0,
+                                                   float X1, float Y0, float Y1) {
+    const float ex = fminf(fmaxf(u, X0), X1) - u, ey = fminf(fmaxf(v, Y0), Y1) - v;
+    if (ex == 0.0f && ey == 0.0f) return true;
+    float qmin = 3.0e38f;
+    if (ex != 0.0f) {
+        const float dy = fminf(fmaxf(__fdividef(-B * ex, C), Y0 - v), Y1 - v);
+        qmin = A * ex * ex + 2.0f * B * ex * dy + C * dy * dy;
+    }
+    if (ey != 0.0f) {
+        const float dx = fminf(fmaxf(__fdividef(-B * ey, A), X0 - u), X1 - u);
+        qmin = fminf(qmin, A * dx * dx + 2.0f * B * dx * ey + C * ey * ey);
+    }
+    return !(o * __expf(-0.5f * qmin) < 0.99f / 255.0f);   // NaN keeps the entry
+}
 
 __global__ void __launch_bounds__(kBatch)
 raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ list, const float4* __restrict__ rec,
               int W, int H, int gx, float tau_T, float* __restrict__ out_rgb, float* __restrict__ finalT,
               uint32_t* __restrict__ bg_list, FrameCounters* __restrict__ counters, uint8_t* __restrict__ bg_mask,
               float* __restrict__ dbg_fg) {
-    __shared__ float4 s_r0[kBatch];
-    __shared__ float4 s_r1[kBatch];
+    __shared__ float4 s_r0[kBatch];   // (u, v, A, B)
+    __shared__ float4 s_r1[kBatch];   // (C, opacity, r, g)
     __shared__ float s_b[kBatch];
+    __shared__ uint32_t s_wcnt[kWarps];
     const int tile = blockIdx.y * gx + blockIdx.x;
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const int px = blockIdx.x * HY_TILE + (threadIdx.x & (HY_TILE - 1));
     const int py = blockIdx.y * HY_TILE + (threadIdx.x >> 4);
     const bool inside = px < W && py < H;
     const float fi = (float)px, fj = (float)py;
+    const float X0 = (float)(blockIdx.x * HY_TILE), Y0 = (float)(blockIdx.y * HY_TILE);
+    const float X1 = fminf(X0 + (float)(HY_TILE - 1), (float)(W - 1)), Y1 = fminf(Y0 + (float)(HY_TILE - 1), (float)(H - 1));
     const uint2 rg = ranges[tile];
     float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f;
     bool done = !inside;
     for (uint32_t b0 = rg.x; b0 < rg.y; b0 += kBatch) {
         if (__syncthreads_count(done) == kBatch) break;
+        // stage up to 256 entries, keeping (in order) only those that can reach this tile
         const uint32_t q = b0 + threadIdx.x;
+        bool keep = false;
+        float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
+        float r2 = 0.0f;
         if (q < rg.y) {
             const uint32_t g = list[q];
-            s_r0[threadIdx.x] = __ldg(rec + 3ull * g);
-            s_r1[threadIdx.x] = __ldg(rec + 3ull * g + 1);
-            s_b[threadIdx.x] = __ldg(reinterpret_cast<const float*>(rec + 3ull * g + 2));
+            r0 = __ldg(rec + 3ull * g);
+            r1 = __ldg(rec + 3ull * g + 1);
+            r2 = __ldg(reinterpret_cast<const float*>(rec + 3ull * g + 2));
+            keep = entry_reaches_tile(r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, X0, X1, Y0, Y1);
         }
+        const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+        if (lane == 0) s_wcnt[warp] = __popc(bal);
         __syncthreads();
-        const int cnt = min((int)kBatch, (int)(rg.y - b0));
-        if (!done) {
-            for (int k = 0; k < cnt; ++k) {
-                const float4 r0 = s_r0[k];
-                const float4 r1 = s_r1[k];
-                const float dx = __fsub_rn(r0.x, fi), dy = __fsub_rn(r0.y, fj);
-                const float power = __fmaf_rn(-0.5f, __fmaf_rn(__fmul_rn(r0.z, dx), dx, __fmul_rn(__fmul_rn(r1.x, dy), dy)),
-                                              -__fmul_rn(__fmul_rn(r0.w, dx), dy));
-                if (power > 0.0f) continue;
-                const float alpha = fminf(0.99f, __fmul_rn(r1.y, __expf(power)));
-                if (alpha < 1.0f / 255.0f) continue;
+        uint32_t pos = __popc(bal & ((1u << lane) - 1u)), cnt = 0;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) {
+            const uint32_t c = s_wcnt[w];
+            pos += (w < (int)warp) ? c : 0u;
+            cnt += c;
+        }
+        if (keep) { s_r0[pos] = r0; s_r1[pos] = r1; s_b[pos] = r2; }
+        __syncthreads();
+        // blend: branch-free per pair; a warp leaves the batch as soon as all of its pixels have terminated
+        for (uint32_t k0 = 0; k0 < cnt; k0 += 8) {
+            if (__all_sync(0xffffffffu, done)) break;
+            const uint32_t kend = k0 + 8 < cnt ? k0 + 8 : cnt;
+            for (uint32_t k = k0; k < kend; ++k) {
+                const float4 a0 = s_r0[k];
+                const float4 a1 = s_r1[k];
+                const float dx = __fsub_rn(a0.x, fi), dy = __fsub_rn(a0.y, fj);
+                const float power = __fmaf_rn(-0.5f, __fmaf_rn(__fmul_rn(a0.z, dx), dx, __fmul_rn(__fmul_rn(a1.x, dy), dy)),
+                                              -__fmul_rn(__fmul_rn(a0.w, dx), dy));
+                const float alpha = fminf(0.99f, __fmul_rn(a1.y, __expf(power)));
                 const float Tn = __fmul_rn(T, __fsub_rn(1.0f, alpha));
-                if (Tn < 1e-4f) { done = true; break; }
-                const float wgt = __fmul_rn(alpha, T);
-                C0 = __fmaf_rn(r1.z, wgt, C0);
-                C1 = __fmaf_rn(r1.w, wgt, C1);
+                const bool valid = !done && !(power > 0.0f) && !(alpha < 1.0f / 255.0f);
+                const bool stop = valid && (Tn < 1e-4f);
+                const bool blend = valid && !stop;
+                done = done || stop;
+                const float wgt = blend ? __fmul_rn(alpha, T) : 0.0f;
+                C0 = __fmaf_rn(a1.z, wgt, C0);
+                C1 = __fmaf_rn(a1.w, wgt, C1);
                 C2 = __fmaf_rn(s_b[k], wgt, C2);
-                T = Tn;
+                T = blend ? Tn : T;
             }
         }
     }
@@ -66,13 +114,12 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
     // arbitrary; the background of a pixel does not depend on it.
     const bool want_bg = inside && T > tau_T;
     if (inside && bg_mask) bg_mask[(size_t)py * W + px] = want_bg ? 1 : 0;
-    const uint32_t bal = __ballot_sync(0xffffffffu, want_bg);
-    if (bal) {
-        const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t bgb = __ballot_sync(0xffffffffu, want_bg);
+    if (bgb) {
         uint32_t base = 0;
-        if (lane == 0) base = atomicAdd(&counters->n_bg, (uint32_t)__popc(bal));
+        if (lane == 0) base = atomicAdd(&counters->n_bg, (uint32_t)__popc(bgb));
         base = __shfl_sync(0xffffffffu, base, 0);
-        if (want_bg) bg_list[base + __popc(bal & ((1u << lane) - 1u))] = (uint32_t)(py * W + px);
+        if (want_bg) bg_list[base + __popc(bgb & ((1u << lane) - 1u))] = (uint32_t)(py * W + px);
     }
 }
 
