@@ -156,10 +156,10 @@ void destroy(hyrf_scene* s) {
     cudaStreamSynchronize(s->stream);
     void* ptrs[] = {s->pos, s->rgb, s->scale, s->opac, (void*)s->geo_grid.table, (void*)s->app_grid.table,
                     (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w,
-                    s->flag_words, s->block_counts, s->vis_idx, s->rec, s->depth_key, s->rect, s->tiles,
+                    s->gm, s->gm_id, s->flag_words, s->id_words, s->word_rank, s->vis_by_id, s->vis_m, s->block_counts, s->vis_idx, s->rec, s->depth_key, s->rect, s->tiles,
                     s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->tt_sorted, s->offs,
                     s->scan_scratch, s->counters, s->ranges, s->fg, s->finalT, s->image, s->bg_mask, s->bg_list,
-                    s->dbg_vis_mask, s->dbg_raw, s->dbg_attrs};
+                    s->dbg_raw, s->dbg_attrs};
     for (void* p : ptrs) dev_free(s, p);
     free_entries(s);
     if (s->counters_host) cudaFreeHost(s->counters_host);
@@ -248,8 +248,14 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc(s, &wa, mlp_weights(s->desc.app_mlp) * esz)); s->app_mlp.w = wa;
     HY_TRY(dev_alloc(s, &wb, mlp_weights(s->desc.bg_mlp) * esz)); s->bg_mlp.w = wb;
     if (s->use_mma) HY_TRY(dev_alloc(s, &s->mma_w, hy_field_mma_packed_bytes()));
+    HY_TRY(dev_alloc_t(s, &s->gm, 2 * N));
+    HY_TRY(dev_alloc_t(s, &s->gm_id, N));
     HY_TRY(dev_alloc_t(s, &s->flag_words, (N + 31) / 32 + 32));
-    HY_TRY(dev_alloc_t(s, &s->block_counts, 2 * cull_blocks + 8));
+    HY_TRY(dev_alloc_t(s, &s->id_words, (N + 31) / 32 + 32));
+    HY_TRY(dev_alloc_t(s, &s->word_rank, (N + 31) / 32 + 32));
+    HY_TRY(dev_alloc_t(s, &s->vis_by_id, N));
+    HY_TRY(dev_alloc_t(s, &s->vis_m, N));
+    HY_TRY(dev_alloc_t(s, &s->block_counts, 4 * cull_blocks + 8));
     HY_TRY(dev_alloc_t(s, &s->vis_idx, N));
     HY_TRY(dev_alloc_t(s, &s->rec, 3 * N));
     HY_TRY(dev_alloc_t(s, &s->depth_key, N));
@@ -308,6 +314,10 @@ extern "C" hyrf_status hyrf_upload_params(hyrf_scene* s, const hyrf_params* p) {
         if ((e = cudaMemcpyAsync(c.dst, c.src, c.bytes, kind, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpyAsync(params)");
     if (s->use_mma) {
         hyrf_status st = hy_field_mma_prepare(s);
+        if (st != HYRF_OK) return st;
+    }
+    {
+        hyrf_status st = hy_prepare_morton(s);
         if (st != HYRF_OK) return st;
     }
     if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(upload)");
@@ -501,7 +511,6 @@ extern "C" hyrf_status hyrf_debug_enable(hyrf_scene* s, uint32_t mask) {
     cudaStreamSynchronize(s->stream);
     const size_t N = s->N, P = (size_t)s->desc.max_width * s->desc.max_height;
     hyrf_status st;
-    if (((mask >> HYRF_DBG_VIS_MASK) & 1u) && !s->dbg_vis_mask && (st = dev_alloc_t(s, &s->dbg_vis_mask, N)) != HYRF_OK) return st;
     if (((mask >> HYRF_DBG_STAGE2_RAW) & 1u) && !s->dbg_raw && (st = dev_alloc_t(s, &s->dbg_raw, 11 * N)) != HYRF_OK) return st;
     if (((mask >> HYRF_DBG_STAGE3_ATTRS) & 1u) && !s->dbg_attrs && (st = dev_alloc_t(s, &s->dbg_attrs, 11 * N)) != HYRF_OK) return st;
     if (((mask >> HYRF_DBG_BG_MASK) & 1u) && !s->bg_mask && (st = dev_alloc_t(s, &s->bg_mask, P)) != HYRF_OK) return st;
@@ -523,7 +532,7 @@ extern "C" hyrf_status hyrf_debug_fetch(hyrf_scene* s, uint32_t kind, void* host
     const void* src = nullptr;
     size_t need = 0;
     switch (kind) {
-        case HYRF_DBG_VIS_MASK: if (!on) goto off; src = s->dbg_vis_mask; need = N; break;
+        case HYRF_DBG_VIS_MASK: src = s->vis_by_id; need = N; break;
         case HYRF_DBG_VIS_IDX: src = s->vis_idx; need = V * 4; break;
         case HYRF_DBG_STAGE2_RAW: if (!on) goto off; src = s->dbg_raw; need = V * 44; break;
         case HYRF_DBG_STAGE3_ATTRS: if (!on) goto off; src = s->dbg_attrs; need = V * 44; break;

@@ -1,7 +1,13 @@
 // cull.cu — S1: visibility pre-culling against the camera frustum + order-preserving compaction.
 // PAPER.md:112–122 (Eq. 8–9): eliminate points that will not project into the image frame BEFORE the neural
-// fields are queried. Arithmetic: DESIGN.md §2 D1. HBM-bound streaming: 12 B read per stored Gaussian,
-// 4 B written per visible one; warp ballots give the stable (id-ordered) compaction the depth tie-break needs.
+// fields are queried. Arithmetic: DESIGN.md §2 D1.
+//
+// The Gaussians are kept twice in HBM: as uploaded (id order, the order every list and tie-break is defined in) and
+// as a 32-byte record in Morton order of the contracted position (built once at upload). The cull streams the
+// Morton copy, so the visible set comes out spatially coherent — neighbouring lanes of the field kernel then gather
+// from the same grid cells on the coarse and middle levels — while the visible RANK of a Gaussian (its slot in
+// every later array) is still its rank in id order: the per-id visibility bytes are compacted a second time in id
+// order, which yields vis_idx (ascending ids) and a rank lookup (word prefix + popcount) for the field kernel.
 #include "scene.h"
 
 namespace {
@@ -9,23 +15,63 @@ namespace {
 constexpr int kCullThreads = 256;
 constexpr int kCullItems = 1024;  // per block: 4 coalesced sweeps of 256
 
+// Morton code of the contracted position: 10 bits per axis
+__device__ __forceinline__ uint32_t spread10(uint32_t v) {
+    v &= 0x3FFu;
+    v = (v | (v << 16)) & 0x030000FFu;
+    v = (v | (v << 8)) & 0x0300F00Fu;
+    v = (v | (v << 4)) & 0x030C30C3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+
+__global__ void morton_code_kernel(const float* __restrict__ pos, uint32_t N, FrameDev f, uint32_t* __restrict__ code,
+                                   uint32_t* __restrict__ id) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    float x[3];
+    hy_contract(f, pos[i], pos[N + i], pos[2ull * N + i], x);
+    uint32_t q[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const float v = x[a] == x[a] ? x[a] : 0.0f;
+        q[a] = (uint32_t)fminf(v * 1024.0f, 1023.0f);
+    }
+    code[i] = spread10(q[0]) | (spread10(q[1]) << 1) | (spread10(q[2]) << 2);
+    id[i] = i;
+}
+
+// gm[m] = (pos.xyz, scale | opacity, rgb) of the m-th Gaussian in Morton order; gm_id[m] = its id
+__global__ void morton_gather_kernel(const uint32_t* __restrict__ order, const float* __restrict__ pos,
+                                     const float* __restrict__ rgb, const float* __restrict__ scale,
+                                     const float* __restrict__ opac, uint32_t N, float4* __restrict__ gm,
+                                     uint32_t* __restrict__ gm_id) {
+    const uint32_t m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= N) return;
+    const uint32_t i = order[m];
+    gm[2ull * m] = make_float4(pos[i], pos[N + i], pos[2ull * N + i], scale[i]);
+    gm[2ull * m + 1] = make_float4(opac[i], rgb[i], rgb[N + i], rgb[2ull * N + i]);
+    gm_id[m] = i;
+}
+
+// Morton order: test, visibility bits + block counts (Morton), visibility byte by id
 __global__ void __launch_bounds__(kCullThreads)
-cull_mark_kernel(const float* __restrict__ pos, uint32_t N, FrameDev f, uint32_t* __restrict__ flag_words,
-                 uint32_t* __restrict__ block_counts, uint8_t* __restrict__ dbg_mask) {
+cull_mark_kernel(const float4* __restrict__ gm, const uint32_t* __restrict__ gm_id, uint32_t N, FrameDev f,
+                 uint32_t* __restrict__ flag_words, uint32_t* __restrict__ block_counts, uint8_t* __restrict__ vis_by_id) {
     __shared__ uint32_t warp_cnt[kCullThreads / 32];
     const uint32_t base = blockIdx.x * kCullItems;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint32_t cnt = 0;
 #pragma unroll
     for (int k = 0; k < kCullItems / kCullThreads; ++k) {
-        const uint32_t i = base + k * kCullThreads + threadIdx.x;
+        const uint32_t m = base + k * kCullThreads + threadIdx.x;
         bool keep = false;
-        if (i < N) {
-            const float px = __ldg(pos + i), py = __ldg(pos + N + i), pz = __ldg(pos + 2ull * N + i);
+        if (m < N) {
+            const float4 p = __ldg(gm + 2ull * m);
             float X, Y, Z;
-            hy_to_camera(f, px, py, pz, X, Y, Z);
+            hy_to_camera(f, p.x, p.y, p.z, X, Y, Z);
             keep = (Z > f.z_near) && (fabsf(X) <= __fmul_rn(f.limx, Z)) && (fabsf(Y) <= __fmul_rn(f.limy, Z));
-            if (dbg_mask) dbg_mask[i] = keep ? 1 : 0;
+            vis_by_id[__ldg(gm_id + m)] = keep ? 1 : 0;
         }
         const uint32_t bal = __ballot_sync(0xffffffffu, keep);
         if (lane == 0) {
@@ -44,39 +90,80 @@ cull_mark_kernel(const float* __restrict__ pos, uint32_t N, FrameDev f, uint32_t
     }
 }
 
+// id order: visibility bytes -> bits + block counts
 __global__ void __launch_bounds__(kCullThreads)
-cull_compact_kernel(const uint32_t* __restrict__ flag_words, const uint32_t* __restrict__ block_offs,
-                    const uint32_t* __restrict__ block_counts, uint32_t N, uint32_t* __restrict__ vis_idx,
-                    FrameCounters* __restrict__ counters) {
-    __shared__ uint32_t word_prefix[kCullItems / 32];
+cull_idbits_kernel(const uint8_t* __restrict__ vis_by_id, uint32_t N, uint32_t* __restrict__ id_words,
+                   uint32_t* __restrict__ block_counts) {
+    __shared__ uint32_t warp_cnt[kCullThreads / 32];
     const uint32_t base = blockIdx.x * kCullItems;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t cnt = 0;
+#pragma unroll
+    for (int k = 0; k < kCullItems / kCullThreads; ++k) {
+        const uint32_t i = base + k * kCullThreads + threadIdx.x;
+        const bool keep = i < N && vis_by_id[i] != 0;
+        const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+        if (lane == 0) {
+            const uint32_t word = (base >> 5) + k * (kCullThreads / 32) + warp;
+            if (word * 32u < N) id_words[word] = bal;
+            cnt += __popc(bal);
+        }
+    }
+    if (lane == 0) warp_cnt[warp] = cnt;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t s = 0;
+#pragma unroll
+        for (int w = 0; w < kCullThreads / 32; ++w) s += warp_cnt[w];
+        block_counts[blockIdx.x] = s;
+    }
+}
+
+// Stable compaction of one bit array: out[rank] = index of the set bit; optionally word_rank[word] = rank of the
+// word's first bit (the lookup the field kernel turns an id into its visible rank with).
+__device__ __forceinline__ void compact_bits(const uint32_t* __restrict__ words, const uint32_t* __restrict__ block_offs,
+                                             uint32_t N, uint32_t* __restrict__ out, uint32_t* __restrict__ word_rank,
+                                             uint32_t* s_prefix /*[32]*/) {
+    const uint32_t base = blockIdx.x * kCullItems;
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t boff = block_offs[blockIdx.x];
     if (warp == 0) {  // 32 words per block: exclusive scan of their popcounts by one warp
         const uint32_t word = (base >> 5) + lane;
-        const uint32_t c = (word * 32u < N) ? __popc(flag_words[word]) : 0u;
+        const bool in = word * 32u < N;
+        const uint32_t c = in ? __popc(words[word]) : 0u;
         uint32_t incl = c;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
             uint32_t v = __shfl_up_sync(0xffffffffu, incl, d);
             if (lane >= (uint32_t)d) incl += v;
         }
-        word_prefix[lane] = incl - c;
+        s_prefix[lane] = incl - c;
+        if (word_rank && in) word_rank[word] = boff + incl - c;
     }
     __syncthreads();
-    const uint32_t boff = block_offs[blockIdx.x];
 #pragma unroll
     for (int k = 0; k < kCullItems / kCullThreads; ++k) {
         const uint32_t wl = k * (kCullThreads / 32) + warp;
         const uint32_t word = (base >> 5) + wl;
         if (word * 32u >= N) continue;
-        const uint32_t bits = flag_words[word];
-        if ((bits >> lane) & 1u) {
-            const uint32_t rank = boff + word_prefix[wl] + __popc(bits & ((1u << lane) - 1u));
-            vis_idx[rank] = base + k * kCullThreads + threadIdx.x;
-        }
+        const uint32_t bits = words[word];
+        if ((bits >> lane) & 1u)
+            out[boff + s_prefix[wl] + __popc(bits & ((1u << lane) - 1u))] = base + k * kCullThreads + threadIdx.x;
     }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(kCullThreads)
+cull_compact_kernel(const uint32_t* __restrict__ m_words, const uint32_t* __restrict__ m_offs,
+                    const uint32_t* __restrict__ m_counts, const uint32_t* __restrict__ id_words,
+                    const uint32_t* __restrict__ id_offs, uint32_t N, uint32_t* __restrict__ vis_m,
+                    uint32_t* __restrict__ vis_idx, uint32_t* __restrict__ word_rank,
+                    FrameCounters* __restrict__ counters) {
+    __shared__ uint32_t s_prefix[kCullItems / 32];
+    compact_bits(m_words, m_offs, N, vis_m, nullptr, s_prefix);
+    compact_bits(id_words, id_offs, N, vis_idx, word_rank, s_prefix);
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) {
-        counters->V = boff + block_counts[blockIdx.x];
+        counters->V = m_offs[blockIdx.x] + m_counts[blockIdx.x];
         counters->D = 0ull;
         counters->n_bg = 0u;
         counters->bin_ticket = 0u;
@@ -86,16 +173,37 @@ cull_compact_kernel(const uint32_t* __restrict__ flag_words, const uint32_t* __r
 
 }  // namespace
 
+// Built once per hyrf_upload_params: Morton order of the contracted positions + the 32-byte records in that order.
+hyrf_status hy_prepare_morton(hyrf_scene* s) {
+    FrameDev f{};
+    for (int a = 0; a < 3; ++a) {
+        f.aabb_c[a] = 0.5f * (s->desc.aabb_min[a] + s->desc.aabb_max[a]);
+        f.aabb_h[a] = 0.5f * (s->desc.aabb_max[a] - s->desc.aabb_min[a]);
+    }
+    const uint32_t N = s->N;
+    morton_code_kernel<<<(N + 255) / 256, 256, 0, s->stream>>>(s->pos, N, f, s->sort_a_key, s->sort_a_val);
+    uint32_t *key = nullptr, *order = nullptr, launches = 0;
+    hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, N, nullptr, 30, s->hist, s->scan_scratch,
+                    s->stream, &key, &order, &launches);
+    morton_gather_kernel<<<(N + 255) / 256, 256, 0, s->stream>>>(order, s->pos, s->rgb, s->scale, s->opac, N, s->gm,
+                                                                 s->gm_id);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return hy_cuda_fail(e, "hy_prepare_morton");
+    return HYRF_OK;
+}
+
 void hy_launch_cull(hyrf_scene* s, const FrameDev& f, uint32_t* launches) {
     const uint32_t nb = (s->N + kCullItems - 1) / kCullItems;
-    uint32_t* counts = s->block_counts;
-    uint32_t* offs = s->block_counts + nb;
-    const bool want_mask = (s->debug_mask >> HYRF_DBG_VIS_MASK) & 1u;
-    cull_mark_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->pos, s->N, f, s->flag_words, counts,
-                                                         want_mask ? s->dbg_vis_mask : nullptr);
-    ++*launches;
-    hy_launch_scan(counts, offs, nb, s->scan_scratch, s->stream, launches);
-    cull_compact_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->flag_words, offs, counts, s->N, s->vis_idx,
-                                                            s->counters);
+    uint32_t* m_counts = s->block_counts;
+    uint32_t* m_offs = s->block_counts + nb;
+    uint32_t* id_counts = s->block_counts + 2 * nb;
+    uint32_t* id_offs = s->block_counts + 3 * nb;
+    cull_mark_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->gm, s->gm_id, s->N, f, s->flag_words, m_counts, s->vis_by_id);
+    cull_idbits_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->vis_by_id, s->N, s->id_words, id_counts);
+    *launches += 2;
+    hy_launch_scan(m_counts, m_offs, nb, s->scan_scratch, s->stream, launches);
+    hy_launch_scan(id_counts, id_offs, nb, s->scan_scratch, s->stream, launches);
+    cull_compact_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->flag_words, m_offs, m_counts, s->id_words, id_offs, s->N,
+                                                            s->vis_m, s->vis_idx, s->word_rank, s->counters);
     ++*launches;
 }

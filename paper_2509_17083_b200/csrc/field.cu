@@ -41,9 +41,9 @@ field_fma_kernel(const FieldArgs A) {
     __syncthreads();
     const uint32_t V = A.counters->V;
     constexpr int MAXD = CL > 0 ? (2 * CL + 24 > CHID ? 2 * CL + 24 : CHID) : HYRF_MAX_WIDTH;
-    for (uint32_t j = blockIdx.x * kFieldThreads + threadIdx.x; j < V; j += gridDim.x * kFieldThreads) {
-        const uint32_t gid = A.vis_idx[j];
-        const float px = __ldg(A.pos + gid), py = __ldg(A.pos + A.N + gid), pz = __ldg(A.pos + 2ull * A.N + gid);
+    for (uint32_t wi = blockIdx.x * kFieldThreads + threadIdx.x; wi < V; wi += gridDim.x * kFieldThreads) {
+        const Explicit ex = fetch_visible(A, wi);
+        const float px = ex.px, py = ex.py, pz = ex.pz;
         float x[3];
         hy_contract(A.f, px, py, pz, x);
         float bufa[MAXD], bufb[MAXD], raw[11];
@@ -82,7 +82,7 @@ field_fma_kernel(const FieldArgs A) {
             for (int k = 2 * La + 6 * (int)A.pe_octaves; k < app_in; ++k) bufa[k] = 0.0f;
             mlp_eval<0, 0, 0, 3, FP16>(wa, app_in, hid_a, nh_a, bufa, bufb, raw + 8);
         }
-        aggregate_project(A, j, gid, px, py, pz, raw);
+        aggregate_project(A, ex, raw);
     }
 }
 
@@ -102,9 +102,9 @@ void hy_fill_field_args(hyrf_scene* s, const FrameDev& f, FieldArgs* out) {
     A.geo = s->geo_grid; A.app = s->app_grid;
     A.geo_mlp = s->geo_mlp; A.app_mlp = s->app_mlp;
     A.f = f;
-    A.pos = s->pos; A.rgb = s->rgb; A.scale = s->scale; A.opac = s->opac;
+    A.gm = s->gm; A.gm_id = s->gm_id; A.vis_m = s->vis_m; A.id_words = s->id_words; A.word_rank = s->word_rank;
     A.N = s->N; A.pe_octaves = s->desc.dir_pe_octaves;
-    A.vis_idx = s->vis_idx; A.counters = s->counters;
+    A.counters = s->counters;
     A.rec = s->rec; A.depth_key = s->depth_key; A.rect = s->rect; A.tiles = s->tiles;
     A.dbg_raw = ((s->debug_mask >> HYRF_DBG_STAGE2_RAW) & 1u) ? s->dbg_raw : nullptr;
     A.dbg_attrs = ((s->debug_mask >> HYRF_DBG_STAGE3_ATTRS) & 1u) ? s->dbg_attrs : nullptr;

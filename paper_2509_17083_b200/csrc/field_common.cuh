@@ -7,13 +7,13 @@ struct FieldArgs {
     GridDev geo, app;
     MlpDev geo_mlp, app_mlp;
     FrameDev f;
-    const float* pos;
-    const float* rgb;
-    const float* scale;
-    const float* opac;
+    const float4* gm;          // [N][2] Morton-ordered (pos.xyz, scale | opacity, rgb)
+    const uint32_t* gm_id;     // [N] id of the m-th Morton record
+    const uint32_t* vis_m;     // [V] Morton indices of the visible Gaussians, ascending
+    const uint32_t* id_words;  // visibility bits by id
+    const uint32_t* word_rank; // visible rank of the first bit of each id word
     uint32_t N;
     uint32_t pe_octaves;
-    const uint32_t* vis_idx;
     FrameCounters* counters;
     float4* rec;
     uint32_t* depth_key;
@@ -25,12 +25,28 @@ struct FieldArgs {
 
 void hy_fill_field_args(hyrf_scene* s, const FrameDev& f, FieldArgs* out);
 
+// One visible Gaussian of the work list: its explicit parameters (Morton record) and its visible rank j in id order,
+// the slot of every per-Gaussian output (j = rank of the first bit of its id word + set bits below it).
+struct Explicit { float px, py, pz, s_e, a_e, c_e0, c_e1, c_e2; uint32_t j; };
+
+static __device__ __forceinline__ Explicit fetch_visible(const FieldArgs& A, uint32_t work_index) {
+    const uint32_t m = __ldg(A.vis_m + work_index);
+    const float4 a = __ldg(A.gm + 2ull * m), b = __ldg(A.gm + 2ull * m + 1);
+    const uint32_t id = __ldg(A.gm_id + m);
+    Explicit e;
+    e.px = a.x; e.py = a.y; e.pz = a.z; e.s_e = a.w;
+    e.a_e = b.x; e.c_e0 = b.y; e.c_e1 = b.z; e.c_e2 = b.w;
+    e.j = __ldg(A.word_rank + (id >> 5)) + __popc(__ldg(A.id_words + (id >> 5)) & ((1u << (id & 31u)) - 1u));
+    return e;
+}
+
 // D7 + D8 for one Gaussian. raw = (alpha_n, s_n[3], r_n[4], c_n[3]).
-static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, uint32_t j, uint32_t gid, float px, float py,
-                                                  float pz, const float* raw) {
+static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, const Explicit& ex, const float* raw) {
     const FrameDev& f = A.f;
-    const float s_e = __ldg(A.scale + gid), a_e = __ldg(A.opac + gid);
-    const float c_e0 = __ldg(A.rgb + gid), c_e1 = __ldg(A.rgb + A.N + gid), c_e2 = __ldg(A.rgb + 2ull * A.N + gid);
+    const uint32_t j = ex.j;
+    const float px = ex.px, py = ex.py, pz = ex.pz;
+    const float s_e = ex.s_e, a_e = ex.a_e;
+    const float c_e0 = ex.c_e0, c_e1 = ex.c_e1, c_e2 = ex.c_e2;
     // Eq. 7
     const float s0 = hy_sigmoid(__fadd_rn(raw[1], s_e));
     const float s1 = hy_sigmoid(__fadd_rn(raw[2], s_e));

@@ -147,15 +147,15 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w) {
     for (uint32_t tile = blockIdx.x; tile * kTile < V; tile += gridDim.x) {
         const uint32_t j = tile * kTile + row;
         const bool valid = j < V;
-        uint32_t gid = 0;
+        Explicit ex{};
         float px = 0.0f, py = 0.0f, pz = 0.0f;
         uint32_t a[32];
 #pragma unroll
         for (int i = 0; i < 32; ++i) a[i] = 0u;
         float x[3] = {0.5f, 0.5f, 0.5f};
         if (valid) {
-            gid = A.vis_idx[j];
-            px = __ldg(A.pos + gid); py = __ldg(A.pos + A.N + gid); pz = __ldg(A.pos + 2ull * A.N + gid);
+            ex = fetch_visible(A, j);
+            px = ex.px; py = ex.py; pz = ex.pz;
             hy_contract(A.f, px, py, pz, x);
         }
         {   // two lanes per Gaussian: half h covers rows 16h..16h+15 of this warp; row r's own lane keeps the result
@@ -261,7 +261,7 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w) {
         __syncthreads();
         if (!chain && valid) {
             raw[8] = s_col[row][0]; raw[9] = s_col[row][1]; raw[10] = s_col[row][2];
-            aggregate_project(A, j, gid, px, py, pz, raw);
+            aggregate_project(A, ex, raw);
         }
         __syncthreads();
         tc::fence_after_sync();

@@ -43,9 +43,15 @@ struct hyrf_scene {
     size_t geo_entries = 0, app_entries = 0, bg_entries = 0;
     MlpDev geo_mlp{}, app_mlp{}, bg_mlp{};
     void* mma_w = nullptr;     // fp16 weights re-laid out for the tensor-core path (field_mma.cu)
+    float4* gm = nullptr;      // [N][2] Morton-ordered records (pos.xyz, scale | opacity, rgb), built at upload (cull.cu)
+    uint32_t* gm_id = nullptr; // [N] id of the m-th Gaussian in Morton order
 
     // per-frame scratch sized from N
-    uint32_t* flag_words = nullptr;   // [ceil(N/32)] visibility bits
+    uint32_t* flag_words = nullptr;   // [ceil(N/32)] visibility bits, Morton order
+    uint32_t* id_words = nullptr;     // [ceil(N/32)] visibility bits, id order
+    uint32_t* word_rank = nullptr;    // [ceil(N/32)] visible rank of the first bit of each id word
+    uint8_t* vis_by_id = nullptr;     // [N] visibility byte per id (also the VIS_MASK debug export)
+    uint32_t* vis_m = nullptr;        // [N] Morton indices of the visible Gaussians (the field kernels' work list)
     uint32_t* block_counts = nullptr; // cull block counts / scanned
     uint32_t* vis_idx = nullptr;      // [N]
     float4* rec = nullptr;            // [N][3] projected records
@@ -83,7 +89,6 @@ struct hyrf_scene {
 
     // debug / measurement
     uint32_t debug_mask = 0;
-    uint8_t* dbg_vis_mask = nullptr;  // [N]
     float* dbg_raw = nullptr;         // [N][11]
     float* dbg_attrs = nullptr;       // [N][11]
     bool timing = false;
@@ -102,7 +107,8 @@ hyrf_status hy_fail(hyrf_status st, const char* fmt, ...);
 hyrf_status hy_cuda_fail(cudaError_t e, const char* what);
 
 // ---- launchers (each returns the number of kernels it enqueued through *launches) -------------------------
-// S1 (cull.cu): visibility bits, stable compaction -> vis_idx, counters->V
+// S1 (cull.cu): visibility bits, stable compactions -> vis_m (Morton work list), vis_idx + rank lookup (id order)
+hyrf_status hy_prepare_morton(hyrf_scene* s);
 void hy_launch_cull(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
 // S2 + S3 + S4a (field.cu): per visible Gaussian query both fields, aggregate, project
 hyrf_status hy_launch_field(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
