@@ -156,7 +156,7 @@ void destroy(hyrf_scene* s) {
     cudaStreamSynchronize(s->stream);
     void* ptrs[] = {s->pos, s->rgb, s->scale, s->opac, (void*)s->geo_grid.table, (void*)s->app_grid.table,
                     (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w,
-                    s->gm, s->gm_id, s->flag_words, s->id_words, s->word_rank, s->vis_by_id, s->vis_m, s->block_counts, s->vis_idx, s->rec, s->depth_key, s->rect, s->tiles,
+                    s->gm, s->gm_id, s->flag_words, s->id_words, s->word_rank, s->vis_by_id, s->vis_m, s->block_counts, s->vis_idx, s->rec, s->rect, s->tiles,
                     s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->tt_sorted, s->offs,
                     s->scan_scratch, s->counters, s->ranges, s->fg, s->finalT, s->image, s->bg_mask, s->bg_list,
                     s->dbg_raw, s->dbg_attrs};
@@ -258,7 +258,6 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc_t(s, &s->block_counts, 4 * cull_blocks + 8));
     HY_TRY(dev_alloc_t(s, &s->vis_idx, N));
     HY_TRY(dev_alloc_t(s, &s->rec, 3 * N));
-    HY_TRY(dev_alloc_t(s, &s->depth_key, N));
     HY_TRY(dev_alloc_t(s, &s->rect, N));
     HY_TRY(dev_alloc_t(s, &s->tiles, N));
     HY_TRY(dev_alloc_t(s, &s->sort_a_key, N));
@@ -394,10 +393,9 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     if ((e = cudaEventRecord(s->ev_counters, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(counters)");
 
     // S4b-c: order the visible Gaussians by (depth bits, id), then build the per-tile lists in that order
-    hy_launch_depth_prepare(s, &launches);
     uint32_t *order_key = nullptr, *order = nullptr;
     hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, s->hist,
-                    s->scan_scratch, s->stream, &order_key, &order, &launches);
+                    s->scan_scratch, s->stream, &order_key, &order, &launches, /*iota_vals=*/true);
     const uint32_t n_tiles = (uint32_t)(f.gx * f.gy);
     uint32_t V = 0;
     uint64_t D = 0;

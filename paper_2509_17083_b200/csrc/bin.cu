@@ -1,19 +1,12 @@
 // bin.cu — S4b: tile binning. PAPER.md:47 ("ordered by depth ... projected onto 2D image planes"), :57 (the set of
 // sorted Gaussians projected onto the pixel); order defined in DESIGN.md §2 D9: (tile, depth bits, id) ascending.
-// Design: Gaussians are first ordered by (depth bits, id) — V items — and emit their tile entries in that order;
-// one stable sort of the D entries by tile id (only ceil(log2 tiles) key bits) then yields the final lists.
-// That moves 8 B per entry per pass over 2 passes instead of 12 B over 6 passes of a 64-bit (tile|depth) key.
+// Radix route, used only for tile grids beyond bin_ordered.cu's limit: Gaussians are first ordered by (depth bits, id)
+// — V items — and emit their tile entries in that order; one stable sort of the D entries by tile id (only
+// ceil(log2 tiles) key bits) then yields the final lists. That moves 8 B per entry per pass over 2 passes instead of
+// 12 B over 6 passes of a 64-bit (tile|depth) key.
 #include "scene.h"
 
 namespace {
-
-__global__ void depth_prepare_kernel(const uint32_t* __restrict__ depth_key, const FrameCounters* __restrict__ c,
-                                     uint32_t* __restrict__ key, uint32_t* __restrict__ val, uint32_t N) {
-    const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= N || j >= c->V) return;
-    key[j] = depth_key[j];
-    val[j] = j;
-}
 
 // tt_sorted[k] = tiles touched by the k-th Gaussian in depth order
 __global__ void __launch_bounds__(256)
@@ -69,12 +62,6 @@ __global__ void ranges_kernel(const uint32_t* __restrict__ keys, uint32_t D, uin
 }
 
 }  // namespace
-
-void hy_launch_depth_prepare(hyrf_scene* s, uint32_t* launches) {
-    depth_prepare_kernel<<<(s->N + 255) / 256, 256, 0, s->stream>>>(s->depth_key, s->counters, s->sort_a_key,
-                                                                    s->sort_a_val, s->N);
-    ++*launches;
-}
 
 void hy_launch_tiles_gather(hyrf_scene* s, const uint32_t* order, uint32_t V, uint32_t* launches) {
     if (V == 0) return;

@@ -139,7 +139,7 @@ static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, con
     A.rec[3ull * j + 0] = make_float4(u, v, cA, cB);
     A.rec[3ull * j + 1] = make_float4(cC, alpha, c0, c1);
     A.rec[3ull * j + 2] = make_float4(c2, Z, radius, __uint_as_float(nt));
-    A.depth_key[j] = __float_as_uint(Z);
+    A.depth_key[j] = __float_as_uint(Z);   // key of the depth sort (S4c); its value is the visible rank j itself
     A.rect[j] = rc;
     A.tiles[j] = nt;
 }

@@ -96,7 +96,7 @@ radix_onesweep_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __re
         const size_t i = wbase + (size_t)k * 32 + lane;
         const bool valid = i < n;
         key[k] = valid ? keys_in[i] : 0u;
-        val[k] = valid ? vals_in[i] : 0u;
+        val[k] = valid ? (vals_in ? vals_in[i] : (uint32_t)i) : 0u;   // no values yet: the value is the index
     }
 #pragma unroll
     for (int k = 0; k < kRadixPer; ++k) {
@@ -125,11 +125,23 @@ radix_onesweep_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __re
     const uint32_t dstart = block_scan256(total, s_warp);        // first slot of digit d inside this tile
     uint32_t prefix = 0;
     if (tile > 0) {
-        for (size_t p = tile; p-- > 0;) {
-            uint32_t v;
-            do { v = state[p * 256 + d]; } while ((v >> 30) == 0u);
-            prefix += v & kValMask;
-            if ((v >> 30) == 2u) break;
+        // look back 16 predecessors per round trip: the loads of a round are independent, so the latency of the
+        // walk is paid once per 16 tiles instead of once per tile
+        constexpr int kLook = 16;
+        long long p = (long long)tile - 1;
+        bool found = false;
+        while (!found) {
+            uint32_t v[kLook];
+#pragma unroll
+            for (int i = 0; i < kLook; ++i) v[i] = (p - i >= 0) ? state[(size_t)(p - i) * 256 + d] : (2u << 30);
+#pragma unroll
+            for (int i = 0; i < kLook; ++i) {
+                if (found) continue;
+                while ((v[i] >> 30) == 0u) v[i] = state[(size_t)(p - i) * 256 + d];
+                prefix += v[i] & kValMask;
+                found = (v[i] >> 30) == 2u;
+            }
+            p -= kLook;
         }
         state[(size_t)tile * 256 + d] = ((prefix + total) & kValMask) | kFlagIncl;
     }
@@ -175,7 +187,7 @@ size_t hy_radix_max_items() { return (size_t)kValMask; }
 
 void hy_launch_radix(uint32_t* key_a, uint32_t* val_a, uint32_t* key_b, uint32_t* val_b, size_t n_cap,
                      const uint32_t* n_dev, int key_bits, uint32_t* ws, uint32_t* /*scan_scratch*/, cudaStream_t st,
-                     uint32_t** out_key, uint32_t** out_val, uint32_t* launches) {
+                     uint32_t** out_key, uint32_t** out_val, uint32_t* launches, bool iota_vals) {
     uint32_t *ki = key_a, *vi = val_a, *ko = key_b, *vo = val_b;
     if (n_cap > 0 && key_bits > 0) {
         const size_t nb = (n_cap + kRadixItems - 1) / kRadixItems;
@@ -190,7 +202,7 @@ void hy_launch_radix(uint32_t* key_a, uint32_t* val_a, uint32_t* key_b, uint32_t
             const int bits = key_bits - 8 * p < 8 ? key_bits - 8 * p : 8;
             uint32_t* state = ws + kWsState + (slices > 1 ? (size_t)p * slice : 0);
             if (slices == 1) cudaMemsetAsync(state, 0, slice * sizeof(uint32_t), st);
-            radix_onesweep_kernel<<<(unsigned)nb, kRadixThreads, 0, st>>>(ki, vi, ko, vo, n_cap, n_dev, 8 * p,
+            radix_onesweep_kernel<<<(unsigned)nb, kRadixThreads, 0, st>>>(ki, (p == 0 && iota_vals) ? nullptr : vi, ko, vo, n_cap, n_dev, 8 * p,
                                                                          (1u << bits) - 1u, ws + kWsHist + p * 256,
                                                                          ws + kWsTicket + p, state);
             ++*launches;

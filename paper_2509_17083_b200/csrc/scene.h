@@ -55,10 +55,9 @@ struct hyrf_scene {
     uint32_t* block_counts = nullptr; // cull block counts / scanned
     uint32_t* vis_idx = nullptr;      // [N]
     float4* rec = nullptr;            // [N][3] projected records
-    uint32_t* depth_key = nullptr;    // [N] depth bits
     uint4* rect = nullptr;            // [N] (x0, x1, y0, y1)
     uint32_t* tiles = nullptr;        // [N] tiles touched
-    uint32_t* sort_a_key = nullptr;   // [N] ping-pong buffers of the depth sort
+    uint32_t* sort_a_key = nullptr;   // [N] ping-pong buffers of the depth sort; the field kernel writes (depth bits, rank) into a
     uint32_t* sort_a_val = nullptr;
     uint32_t* sort_b_key = nullptr;
     uint32_t* sort_b_val = nullptr;
@@ -117,14 +116,14 @@ size_t hy_scan_scratch_elems(size_t n);
 void hy_launch_scan(const uint32_t* in, uint32_t* out, size_t n, uint32_t* scratch, cudaStream_t st,
                     uint32_t* launches);
 // stable LSD radix sort of (key, val) pairs on bits [0, key_bits) (radix.cu). n_dev: device count (may be null ->
-// n_cap). Result ends in (*out_key, *out_val) which is either buffer pair.
+// n_cap). Result ends in (*out_key, *out_val) which is either buffer pair. iota_vals: val_a is not read, the value of
+// item i is i.
 size_t hy_radix_hist_elems(size_t n_cap);
 size_t hy_radix_max_items();
 void hy_launch_radix(uint32_t* key_a, uint32_t* val_a, uint32_t* key_b, uint32_t* val_b, size_t n_cap,
                      const uint32_t* n_dev, int key_bits, uint32_t* hist, uint32_t* scan_scratch, cudaStream_t st,
-                     uint32_t** out_key, uint32_t** out_val, uint32_t* launches);
+                     uint32_t** out_key, uint32_t** out_val, uint32_t* launches, bool iota_vals = false);
 // S4b-c (bin.cu)
-void hy_launch_depth_prepare(hyrf_scene* s, uint32_t* launches);                       // (depth, rank) pairs
 void hy_launch_tiles_gather(hyrf_scene* s, const uint32_t* order, uint32_t V, uint32_t* launches);
 void hy_launch_emit(hyrf_scene* s, const uint32_t* order, uint32_t V, uint32_t* launches);
 void hy_launch_ranges(hyrf_scene* s, const uint32_t* keys, uint64_t D, uint32_t n_tiles, uint32_t* launches);
