@@ -120,17 +120,48 @@ def workload(cfg: int, args):
     return scene, name
 
 
-# Algorithmic work per unit.
-def stage_rooflines(scene, V, D, evaluated_pairs, n_bg, peaks):
+# Algorithmic work per unit. Bytes are ALGORITHMIC: what the stage has to move if
+# every operand is read once and every result written once, not what the caches happened to move.
+def stage_rooflines(scene, V, D, n_bg, eval_pairs, peaks):
     esz = 2 if scene.fp16 else 4
     gathers = (scene.geo_grid.levels + scene.app_grid.levels) * 8
     hbm = peaks["hbm_gbs"]
-    field_bytes = V * (gathers * 2 * esz + 12 + 20 + 4 + 48 + 4 + 16 + 4)   # gathers + explicit in + idx + record/keys out
-    return {
-        "cull": {"bound": "hbm", "bytes": scene.n * 12 + V * 4, "peak": hbm},
-        "field": {"bound": "hbm", "bytes": field_bytes, "peak": hbm},
-        "bin": {"bound": "hbm", "bytes": V * (4 * 16 + 12) + D * (8 + 2 * 16 + 4), "peak": hbm},
+    # S2+S3+S4a: per visible Gaussian 256 gathers of one (2-feature) entry + 32 B explicit record + 4 B work index in;
+    # 48 B record + 4 B depth key + 16 B rectangle + 4 B tiles-touched out (1 KB + 32 B + 44-56 B)
+    field_bytes = V * (gathers * 2 * esz + 32 + 4 + 48 + 4 + 16 + 4)
+    # S1: 16 B of the Morton record + 4 B id read per stored Gaussian, 1 B visibility written; 4 B per visible x 2 lists
+    cull_bytes = scene.n * (16 + 4 + 1 + 1) + V * 8
+    # S4b-c: depth sort (4 passes x 16 B per visible) + 20 B read per visible for the pairs + 8 B per pair written,
+    # 4 + 8 B read by count / scatter, 4 B per list entry written
+    bin_bytes = V * (4 * 16 + 4 + 20) + D * (8 + 4 + 8 + 4)
+    out = {
+        "cull": {"bound": "hbm", "work": cull_bytes, "peak": hbm, "unit": "GB/s"},
+        "field": {"bound": "hbm", "work": field_bytes, "peak": hbm, "unit": "GB/s"},
+        "bin": {"bound": "hbm", "work": bin_bytes, "peak": hbm, "unit": "GB/s"},
     }
+    # S5: plain ALU issue. 20 issue slots per evaluated (pixel, Gaussian) pair (16 fp32 ops + ex2 + 3 predicates,
+    # SURVEY §8(d)); peak = 148 SMs x 4 schedulers x 32 lanes x SM clock
+    alu_peak = 148 * 4 * 32 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e9     # G lane-slots / s
+    if eval_pairs:
+        out["raster"] = {"bound": "alu", "work": eval_pairs * 20, "peak": alu_peak, "unit": "Gslot/s"}
+    if n_bg is not None:
+        bgl = scene.bg_grid.levels * 8
+        out["background"] = {"bound": "hbm", "work": n_bg * (bgl * 2 * esz + 4 + 4 + 12 + 12), "peak": hbm, "unit": "GB/s"}
+    return out
+
+
+def load_traffic(kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu --set full capture
+    of this workload (profiles/r1b_dram_traffic.csv); None if there is no capture."""
+    p = os.path.join(ROOT, "profiles", "r1b_dram_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    import csv
+    with open(p) as f:
+        for row in csv.DictReader(f):
+            if row["kernel"] == kernel:
+                return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
+    return None
 
 
 def load_peaks():
@@ -145,21 +176,23 @@ def load_peaks():
 
 
 def oracle_frames(scene, cams, max_seconds: float, threads: int = 0):
-    """Time the CPU oracle as it stands on `cams` (stops after max_seconds). Returns (frames, seconds, V_total)."""
+    """Time the CPU oracle as it stands on `cams` (stops after max_seconds). Returns (frames, seconds, V_total,
+    threads, evaluated (pixel, Gaussian) pairs as counted by the oracle)."""
     from oracle import hyrf_oracle as ho
     ho.build()
     if threads:
         ho.set_num_threads(threads)
     osc = ho.OracleScene(scene)
     t0 = time.perf_counter()
-    frames, vtot = 0, 0
+    frames, vtot, pairs = 0, 0, 0
     for cam in cams:
         r = ho.render(osc, cam)
         frames += 1
         vtot += len(r["vis_idx"])
+        pairs += int(r["n_eval"].sum()) if "n_eval" in r else 0
         if time.perf_counter() - t0 > max_seconds:
             break
-    return frames, time.perf_counter() - t0, vtot, ho.num_threads()
+    return frames, time.perf_counter() - t0, vtot, ho.num_threads(), pairs
 
 
 def run_reference(args):
@@ -232,45 +265,42 @@ def run_ours(args):
     torch.cuda.synchronize()
 
     # --- timed region: K steps, CUDA events on the launching stream, L2 flushed between steps -----------------
+    # Each step is bracketed by its own event pair (the flush sits outside the bracket); the library's per-stage
+    # events (cudaEventRecord on the same stream, between the kernels) are read after every step, so the kernel
+    # durations behind `roofline` come from this very region.
     sampler = ClockSampler(dev)
     sampler.start()
+    hs.set_timing(True)
     if world > 1:
         torch.distributed.barrier()
     torch.cuda.synchronize()
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
     launches = 0
+    stage, Vs, Ds = [], [], []
     for i in range(K):
         flush.fill_(i & 0xFF)
         evs[i][0].record(stream)
         step(Wm + i)
         evs[i][1].record(stream)
         launches += hs.last_launch_count()
+        stage.append(hs.stage_times())                 # synchronises the stream; outside the bracket
+        c = hs.debug_fetch(B.DBG_COUNTERS)
+        Vs.append(int(c[1]))
+        Ds.append(int(c[2]))
     torch.cuda.synchronize()
     if world > 1:
         torch.distributed.barrier()
     clocks = sampler.stop()
+    hs.set_timing(False)
     t_ms = sum(a.elapsed_time(b) for a, b in evs)
     t_max = max_over_ranks(t_ms)
     frames_total = sum_over_ranks(K)
     value = frames_total / (t_max * 1e-3)
-
-    # --- per-stage times + counters (separate pass, same L2 protocol) ------------------------------------------
-    hs.set_timing(True)
-    stage = []
-    Vs, Ds = [], []
-    for i in range(min(K, 2 * len(cstructs))):
-        flush.fill_(i & 0xFF)
-        step(i)
-        torch.cuda.synchronize()
-        stage.append(hs.stage_times())
-        c = hs.debug_fetch(B.DBG_COUNTERS)
-        Vs.append(int(c[1]))
-        Ds.append(int(c[2]))
-    hs.set_timing(False)
     import numpy as np
-    stage_ms = np.median(np.array(stage), axis=0)
+    stage_ms = np.mean(np.array(stage), axis=0)
     Vm, Dm = float(np.mean(Vs)), float(np.mean(Ds))
     vis_per_s = sum_over_ranks(Vm * K) / (t_max * 1e-3)
+    n_bg = float((hs.debug_fetch(B.DBG_FINAL_T) > scene.tau_T).sum())        # last frame's S6 work list length
 
     # --- warm-L2 figure (no flush), for context ---------------------------------------------------------------
     torch.cuda.synchronize()
@@ -298,14 +328,30 @@ def run_ours(args):
     if rank != 0:
         return
     names = ["cull", "field", "bin", "raster", "background"]
-    dom = int(np.argmax(stage_ms[:5]))
-    rl = stage_rooflines(scene, Vm, Dm, None, None, peaks)
-    roof = {"stage": names[dom], "bound": None, "achieved": None, "peak": None, "unit": None, "frac": None, "traffic": None}
-    if names[dom] in rl:
-        r = rl[names[dom]]
-        ach = r["bytes"] / (stage_ms[dom] * 1e-3) / 1e9
-        roof.update(bound=r["bound"], achieved=ach, peak=r["peak"], unit="GB/s", frac=ach / r["peak"],
-                    peak_source=peaks["source"])
+    kernels = {"field": "field_mma_kernel" if scene.fp16 and args.mlp != "fma" else "field_fma_kernel",
+               "raster": "raster_kernel"}
+    eval_pairs = None
+    cpu = None
+    if world == 1 and not args.no_cpu:
+        fr, sec, vtot, thr, pairs = oracle_frames(scene, [cams_all[i] for i in mine], max_seconds=args.cpu_seconds)
+        eval_pairs = pairs / fr
+        cpu = {"value": fr / sec, "unit": UNIT, "cores": thr, "kind": "oracle",
+               "sample": f"{fr} whole frame(s) of the workload ({vtot / fr:.0f} visible Gaussians each)"}
+    rl = stage_rooflines(scene, Vm, Dm, n_bg, eval_pairs, peaks)
+    per_stage = {}
+    for i, n in enumerate(names):
+        if n in rl:
+            r = rl[n]
+            ach = r["work"] / (stage_ms[i] * 1e-3) / 1e9
+            per_stage[n] = {"bound": r["bound"], "achieved": ach, "peak": r["peak"], "unit": r["unit"],
+                            "frac": ach / r["peak"], "ms": float(stage_ms[i])}
+    # the dominant KERNEL: S2+S3+S4a and S5 are one kernel each; S4b-c is nine short ones
+    dom = "field" if stage_ms[1] >= stage_ms[3] else "raster"
+    roof = {"kernel": kernels[dom], "stage": dom, "traffic": load_traffic(kernels[dom]) if args.config == 3 else None,
+            "peak_source": peaks["source"] + (" (burst HBM copy)" if per_stage.get(dom, {}).get("bound") == "hbm" else "")}
+    if dom in per_stage:
+        roof.update({k: per_stage[dom][k] for k in ("bound", "achieved", "peak", "unit", "frac")})
+        roof["launch_ms"] = per_stage[dom]["ms"]
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f16" if scene.fp16 else "f32", "data": "synthetic",
@@ -315,11 +361,9 @@ def run_ours(args):
             "stage_ms": {n: float(stage_ms[i]) for i, n in enumerate(names)} | {"frame": float(stage_ms[5])},
             "warm_l2_ms_per_step": warm_ms,
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 64, "d2h_bytes_per_step": W * H * 12},
-            "gpu_launches": launches, "clocks": clocks, "roofline": roof}
-    if world == 1 and not args.no_cpu:
-        fr, sec, vtot, thr = oracle_frames(scene, cams_all, max_seconds=args.cpu_seconds)
-        line["cpu_baseline"] = {"value": fr / sec, "unit": UNIT, "cores": thr, "kind": "oracle",
-                                "sample": f"{fr} whole frame(s) of the workload ({vtot / fr:.0f} visible Gaussians each)"}
+            "gpu_launches": launches, "clocks": clocks, "roofline": roof, "stage_rooflines": per_stage}
+    if cpu:
+        line["cpu_baseline"] = cpu
     print(json.dumps(line), flush=True)
 
 

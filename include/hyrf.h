@@ -10,9 +10,10 @@
  *    hyrf_last_error() describes the failure (thread-local string, never NULL).
  *  - Pointers in hyrf_params are DEVICE pointers unless host_ptrs != 0. The library copies; the caller keeps
  *    ownership of everything it passes in. hyrf_render's out_rgb is a DEVICE pointer; hyrf_render_host's is HOST.
- *  - hyrf_render is asynchronous on the scene's stream except for one small device→host readback of the frame's
- *    counters (visible count V, tile-entry count D) that sizes the binning launches; the caller synchronises
- *    the stream before reading out_rgb. Steady-state renders allocate nothing unless D outgrows the scratch.
+ *  - hyrf_render enqueues the whole frame on the scene's stream, then waits for one 32-byte device→host readback
+ *    of the frame's counters (visible count V, tile-entry count D; available once the field kernel has finished, while
+ *    binning and rasterisation are still running). If D outgrew the list scratch, the scratch is grown and the frame is
+ *    re-binned; otherwise nothing is allocated. The caller synchronises the stream before reading out_rgb.
  *  - One scene lives on one device. A scene is not thread-safe; the library is.
  *  - There is no CPU fallback anywhere: without a CUDA device every compute call returns HYRF_ERR_CUDA.
  */
