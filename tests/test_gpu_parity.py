@@ -195,3 +195,21 @@ def test_config3_full_one_camera_both_paths(B, ho, synth):
     s = synth.make_scene(3, n_cameras=1)
     _run(B, ho, s, mlp_path=B.HYRF_MLP_FMA, exact=True)
     _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False)
+
+
+def test_config4_full_one_camera_bench_path(B, ho, synth):
+    # BASELINE config 4 at full size (2M Gaussians, unbounded scene, 1245x825 with ragged tiles), camera 0, in the
+    # launch configuration bench.py --config 4 times (AUTO -> tensor-core decoders, ordered binning)
+    s = synth.make_scene(4, n_cameras=1)
+    st = _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False)
+    assert st[0]["V"] > 1_000_000
+
+
+def test_config5_points(B, ho, synth):
+    # BASELINE config 5: the 500k @ 256x256 point element by element on both paths, and the 500k @ 1920x1080 point
+    # (8160 tiles) on the exact path so that its lists are compared bit for bit
+    s = synth.make_scene(5, n_gaussians=500_000, width=256, height=256)
+    _run(B, ho, s, mlp_path=B.HYRF_MLP_FMA, exact=True)
+    _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False)
+    s = synth.make_scene(5, n_gaussians=500_000, width=1920, height=1080)
+    _run(B, ho, s, mlp_path=B.HYRF_MLP_FMA, exact=True)
