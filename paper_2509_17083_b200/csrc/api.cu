@@ -158,7 +158,7 @@ void destroy(hyrf_scene* s) {
                     (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w,
                     s->gm, s->gm_id, s->flag_words, s->id_words, s->word_rank, s->vis_by_id, s->vis_m, s->block_counts, s->vis_idx, s->rec, s->rect, s->tiles,
                     s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->tt_sorted, s->offs,
-                    s->scan_scratch, s->counters, s->ranges, s->fg, s->finalT, s->image, s->bg_mask, s->bg_list,
+                    s->scan_scratch, s->counters, s->ranges, s->tile_queue, s->fg, s->finalT, s->image, s->bg_mask, s->bg_list,
                     s->dbg_raw, s->dbg_attrs};
     for (void* p : ptrs) dev_free(s, p);
     free_entries(s);
@@ -268,6 +268,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc_t(s, &s->offs, N));
     HY_TRY(dev_alloc_t(s, &s->counters, 1));
     HY_TRY(dev_alloc_t(s, &s->ranges, tiles));
+    HY_TRY(dev_alloc_t(s, &s->tile_queue, tiles));
     HY_TRY(dev_alloc_t(s, &s->finalT, P));
     HY_TRY(dev_alloc_t(s, &s->bg_list, P));
     if ((e = cudaMallocHost(reinterpret_cast<void**>(&s->counters_host), sizeof(FrameCounters))) != cudaSuccess) {
@@ -408,7 +409,7 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
             if ((st = hy_launch_bin_ordered(s, order, n_tiles, (uint32_t)f.gx, &launches)) != HYRF_OK) return st;
             s->list_final = s->ent_val[1];
             if (timing) cudaEventRecord(s->ev[3], s->stream);
-            hy_launch_raster(s, f, s->list_final, out_rgb, &launches);      // S5 (Eq. 1)
+            hy_launch_raster(s, f, s->list_final, out_rgb, &launches, s->tile_queue);      // S5 (Eq. 1)
             if (timing) cudaEventRecord(s->ev[4], s->stream);
             if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;   // S6 (Eq. 10-11, A.2)
             if (timing) cudaEventRecord(s->ev[5], s->stream);
@@ -446,7 +447,7 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
         hy_launch_ranges(s, sorted_key, D, n_tiles, &launches);
         s->list_final = sorted_val;
         if (timing) cudaEventRecord(s->ev[3], s->stream);
-        hy_launch_raster(s, f, sorted_val, out_rgb, &launches);             // S5 (Eq. 1)
+        hy_launch_raster(s, f, sorted_val, out_rgb, &launches, nullptr);             // S5 (Eq. 1)
         if (timing) cudaEventRecord(s->ev[4], s->stream);
         if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;       // S6 (Eq. 10-11, A.2)
         if (timing) cudaEventRecord(s->ev[5], s->stream);

@@ -43,6 +43,7 @@ struct BinArgs {
     uint32_t* totals;        // [T]
     uint32_t* starts;        // [T] exclusive scan of totals
     uint2* ranges;           // [T]
+    uint32_t* tile_queue;    // [T] tile ids, longest list first (the rasterizer's launch order)
     uint32_t* pair_tile;     // [cap] tile id of every pair, depth order
     uint32_t* pair_rank;     // [cap] visible rank of every pair
     uint32_t* list;          // [cap]
@@ -276,8 +277,25 @@ bin_scatter_kernel(const BinArgs A) {
     const uint32_t Tp = (A.T + 1u) & ~1u;
     const uint32_t D = pair_count(A);
     const uint32_t c0 = blockIdx.x * A.Ec;
-    if (c0 >= D) return;
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    if (blockIdx.x == gridDim.x - 1) {
+        // one extra CTA orders the tiles for the rasterizer: 33 buckets by floor(log2(list length)), longest first;
+        // the order inside a bucket is arbitrary and only affects scheduling
+        __shared__ uint32_t s_bucket[33];
+        if (threadIdx.x < 33) s_bucket[threadIdx.x] = 0;
+        __syncthreads();
+        for (uint32_t t = threadIdx.x; t < A.T; t += kBinThreads) atomicAdd(&s_bucket[32 - __clz(__ldg(A.totals + t))], 1u);
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            uint32_t run = 0;
+            for (int b = 32; b >= 0; --b) { const uint32_t c = s_bucket[b]; s_bucket[b] = run; run += c; }
+        }
+        __syncthreads();
+        for (uint32_t t = threadIdx.x; t < A.T; t += kBinThreads)
+            A.tile_queue[atomicAdd(&s_bucket[32 - __clz(__ldg(A.totals + t))], 1u)] = t;
+        return;
+    }
+    if (c0 >= D) return;
     const uint32_t* row = A.M + (size_t)blockIdx.x * A.T;
     for (uint32_t t = threadIdx.x; t < A.T; t += kBinThreads) s_base[t] = __ldg(A.starts + t) + __ldg(row + t);
     for (uint32_t i = threadIdx.x; i < kBinWarps * Tp / 2; i += kBinThreads) reinterpret_cast<uint32_t*>(s_wcnt)[i] = 0;
@@ -376,6 +394,7 @@ hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t
     A.frame = ++s->bin_frame & 0x3FFFFFFFu;
     if (A.frame == 0) A.frame = ++s->bin_frame & 0x3FFFFFFFu;   // 0 is the tag of freshly cleared words
     A.ranges = s->ranges;
+    A.tile_queue = s->tile_queue;
     A.pair_tile = s->ent_key[0];
     A.pair_rank = s->ent_val[0];
     A.list = s->ent_val[1];
@@ -392,7 +411,7 @@ hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t
     bin_pairs_kernel<<<(s->N + kBinThreads - 1) / kBinThreads, kBinThreads, 0, s->stream>>>(A);
     bin_count_kernel<<<A.rows_cap, kBinThreads, smem_count, s->stream>>>(A);
     bin_prefix_kernel<<<(n_tiles + 31) / 32, 1024, 0, s->stream>>>(A);
-    bin_scatter_kernel<<<A.rows_cap, kBinThreads, smem_scatter, s->stream>>>(A);
+    bin_scatter_kernel<<<A.rows_cap + 1, kBinThreads, smem_scatter, s->stream>>>(A);   // + 1: the tile-queue CTA
     *launches += 5;
     return HYRF_OK;
 }

@@ -14,6 +14,10 @@
 #include "field_common.cuh"
 #include "tcgen05.cuh"
 
+#ifndef HY_FIELD_PAIR_LANES
+#define HY_FIELD_PAIR_LANES 0
+#endif
+
 namespace {
 
 constexpr int kThreads = 256;
@@ -158,6 +162,7 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w) {
             px = ex.px; py = ex.py; pz = ex.pz;
             hy_contract(A.f, px, py, pz, x);
         }
+#if HY_FIELD_PAIR_LANES
         {   // two lanes per Gaussian: half h covers rows 16h..16h+15 of this warp; row r's own lane keeps the result
             const uint32_t lane = threadIdx.x & 31u, xb = lane >> 4;
 #pragma unroll
@@ -175,6 +180,14 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w) {
                 }
             }
         }
+#else
+#pragma unroll
+        for (int l = 0; l < 16; ++l) {
+            float f0, f1;
+            hy_grid_level<true>(grid, l, x, f0, f1);
+            a[l] = pack_h2(f0, f1);
+        }
+#endif
         if (valid) {
             if (chain) {
                 const float dx = __fsub_rn(px, A.f.o[0]), dy = __fsub_rn(py, A.f.o[1]), dz = __fsub_rn(pz, A.f.o[2]);

