@@ -15,7 +15,7 @@
 #include "tcgen05.cuh"
 
 #ifndef HY_FIELD_PAIR_LANES
-#define HY_FIELD_PAIR_LANES 0
+#define HY_FIELD_PAIR_LANES 1
 #endif
 
 namespace {
