@@ -82,7 +82,7 @@ field_fma_kernel(const FieldArgs A) {
             for (int k = 2 * La + 6 * (int)A.pe_octaves; k < app_in; ++k) bufa[k] = 0.0f;
             mlp_eval<0, 0, 0, 3, FP16>(wa, app_in, hid_a, nh_a, bufa, bufb, raw + 8);
         }
-        aggregate_project(A, ex, raw);
+        aggregate_project<false>(A, ex, raw);
     }
 }
 

@@ -40,7 +40,15 @@ static __device__ __forceinline__ Explicit fetch_visible(const FieldArgs& A, uin
     return e;
 }
 
-// D7 + D8 for one Gaussian. raw = (alpha_n, s_n[3], r_n[4], c_n[3]).
+// sigmoid for the tensor-core path: MUFU exp2 + MUFU reciprocal (2-ulp class). That path is compared with the oracle
+// by tolerance and its decoder outputs already carry ~1e-4 of accumulation-order noise, so the soft
+// exponential and IEEE division of D6 — there for bit-reproducible geometry — buy nothing on it.
+static __device__ __forceinline__ float sigmoid_fast(float v) {
+    return __fdividef(1.0f, 1.0f + __expf(-v));
+}
+
+// D7 + D8 for one Gaussian. raw = (alpha_n, s_n[3], r_n[4], c_n[3]). FAST: tensor-core path arithmetic (see above).
+template <bool FAST>
 static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, const Explicit& ex, const float* raw) {
     const FrameDev& f = A.f;
     const uint32_t j = ex.j;
@@ -48,16 +56,26 @@ static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, con
     const float s_e = ex.s_e, a_e = ex.a_e;
     const float c_e0 = ex.c_e0, c_e1 = ex.c_e1, c_e2 = ex.c_e2;
     // Eq. 7
-    const float s0 = hy_sigmoid(__fadd_rn(raw[1], s_e));
-    const float s1 = hy_sigmoid(__fadd_rn(raw[2], s_e));
-    const float s2 = hy_sigmoid(__fadd_rn(raw[3], s_e));
-    const float m = __fsqrt_rn(__fmaf_rn(raw[7], raw[7], __fmaf_rn(raw[6], raw[6], __fmaf_rn(raw[5], raw[5], __fmul_rn(raw[4], raw[4])))));
-    const float den = fmaxf(m, 1e-12f);
-    const float w = __fdiv_rn(raw[4], den), x = __fdiv_rn(raw[5], den), y = __fdiv_rn(raw[6], den), z = __fdiv_rn(raw[7], den);
-    const float alpha = hy_sigmoid(__fadd_rn(raw[0], a_e));
-    const float c0 = hy_sigmoid(__fadd_rn(raw[8], c_e0));
-    const float c1 = hy_sigmoid(__fadd_rn(raw[9], c_e1));
-    const float c2 = hy_sigmoid(__fadd_rn(raw[10], c_e2));
+    float s0, s1, s2, w, x, y, z, alpha, c0, c1, c2;
+    if (FAST) {
+        s0 = sigmoid_fast(raw[1] + s_e); s1 = sigmoid_fast(raw[2] + s_e); s2 = sigmoid_fast(raw[3] + s_e);
+        const float m2 = raw[7] * raw[7] + raw[6] * raw[6] + raw[5] * raw[5] + raw[4] * raw[4];
+        const float inv = rsqrtf(fmaxf(m2, 1e-24f));
+        w = raw[4] * inv; x = raw[5] * inv; y = raw[6] * inv; z = raw[7] * inv;
+        alpha = sigmoid_fast(raw[0] + a_e);
+        c0 = sigmoid_fast(raw[8] + c_e0); c1 = sigmoid_fast(raw[9] + c_e1); c2 = sigmoid_fast(raw[10] + c_e2);
+    } else {
+        s0 = hy_sigmoid(__fadd_rn(raw[1], s_e));
+        s1 = hy_sigmoid(__fadd_rn(raw[2], s_e));
+        s2 = hy_sigmoid(__fadd_rn(raw[3], s_e));
+        const float m = __fsqrt_rn(__fmaf_rn(raw[7], raw[7], __fmaf_rn(raw[6], raw[6], __fmaf_rn(raw[5], raw[5], __fmul_rn(raw[4], raw[4])))));
+        const float den = fmaxf(m, 1e-12f);
+        w = __fdiv_rn(raw[4], den); x = __fdiv_rn(raw[5], den); y = __fdiv_rn(raw[6], den); z = __fdiv_rn(raw[7], den);
+        alpha = hy_sigmoid(__fadd_rn(raw[0], a_e));
+        c0 = hy_sigmoid(__fadd_rn(raw[8], c_e0));
+        c1 = hy_sigmoid(__fadd_rn(raw[9], c_e1));
+        c2 = hy_sigmoid(__fadd_rn(raw[10], c_e2));
+    }
     if (A.dbg_raw) {
         for (int k = 0; k < 11; ++k) A.dbg_raw[11ull * j + k] = raw[k];
     }

@@ -193,8 +193,21 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w) {
                 const float dx = __fsub_rn(px, A.f.o[0]), dy = __fsub_rn(py, A.f.o[1]), dz = __fsub_rn(pz, A.f.o[2]);
                 const float n = __fsqrt_rn(__fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx))));
                 const float d[3] = {__fdiv_rn(dx, n), __fdiv_rn(dy, n), __fdiv_rn(dz, n)};
+                // D4 by octave doubling: one sincospi per axis, then sin 2t = 2 sin t cos t, cos 2t = 1 - 2 sin^2 t.
+                // Three doublings amplify the 1-ulp start error to ~1e-6, far below the fp16 rounding that follows.
                 float pe[24];
-                hy_dir_pe<false>(d, 4, pe);
+#pragma unroll
+                for (int ax = 0; ax < 3; ++ax) {
+                    float sn, cs;
+                    sincospif(d[ax], &sn, &cs);
+                    pe[ax] = sn; pe[3 + ax] = cs;
+#pragma unroll
+                    for (int k = 1; k < 4; ++k) {
+                        const float s2 = 2.0f * sn * cs, c2 = 1.0f - 2.0f * sn * sn;
+                        sn = s2; cs = c2;
+                        pe[6 * k + ax] = sn; pe[6 * k + 3 + ax] = cs;
+                    }
+                }
 #pragma unroll
                 for (int i = 0; i < 12; ++i) a[16 + i] = pack_h2(pe[2 * i], pe[2 * i + 1]);
             }
@@ -274,7 +287,7 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w) {
         __syncthreads();
         if (!chain && valid) {
             raw[8] = s_col[row][0]; raw[9] = s_col[row][1]; raw[10] = s_col[row][2];
-            aggregate_project(A, ex, raw);
+            aggregate_project<true>(A, ex, raw);
         }
         __syncthreads();
         tc::fence_after_sync();
