@@ -250,6 +250,7 @@ def run_ours(args):
     cams = [cams_all[i] for i in mine]                      # frame-parallel replicas: no data-path collective
     path = {"auto": B.HYRF_MLP_AUTO, "fma": B.HYRF_MLP_FMA, "mma": B.HYRF_MLP_MMA}[args.mlp]
     hs = B.HyrfScene(scene, device=dev, mlp_path=path)
+    hs.set_ablation(args.ablation)
     W, H = cams[0].W, cams[0].H
     out = torch.empty((H, W, 3), dtype=torch.float32, device=f"cuda:{dev}")
     cstructs = [B.camera_struct(c) for c in cams]
@@ -332,7 +333,7 @@ def run_ours(args):
                "raster": "raster_kernel"}
     eval_pairs = None
     cpu = None
-    if world == 1 and not args.no_cpu:
+    if world == 1 and not args.no_cpu and args.ablation == 0:
         fr, sec, vtot, thr, pairs = oracle_frames(scene, [cams_all[i] for i in mine], max_seconds=args.cpu_seconds)
         eval_pairs = pairs / fr
         cpu = {"value": fr / sec, "unit": UNIT, "cores": thr, "kind": "oracle",
@@ -355,7 +356,7 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f16" if scene.fp16 else "f32", "data": "synthetic",
-            "config": {"workload": name, "l2": "flushed between steps (256 MiB write)", "mlp_path": args.mlp,
+            "config": {"workload": name, "l2": "flushed between steps (256 MiB write)", "mlp_path": args.mlp, "ablation": args.ablation,
                        "parallelism": f"replicas x{world} (cameras round-robin)"},
             "visible_gaussians_per_s": vis_per_s, "V_mean": Vm, "D_mean": Dm,
             "stage_ms": {n: float(stage_ms[i]) for i, n in enumerate(names)} | {"frame": float(stage_ms[5])},
@@ -378,6 +379,8 @@ def main():
     ap.add_argument("--n-gaussians", type=int, default=0)
     ap.add_argument("--width", type=int, default=0)
     ap.add_argument("--height", type=int, default=0)
+    ap.add_argument("--ablation", type=int, default=0,
+                    help="hyrf_ablation bits (PAPER.md Table 5): 1 no pre-culling, 2 no background, 4 no neural, 8 no explicit")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()

@@ -159,6 +159,19 @@ hyrf_status hyrf_debug_fetch(hyrf_scene* scene, uint32_t kind, void* host_dst, s
 hyrf_status hyrf_set_timing(hyrf_scene* scene, int32_t enabled);
 hyrf_status hyrf_stage_times(hyrf_scene* scene, float ms[6]);
 
+/* Ablation switches of the same pass (PAPER.md:214-223 Table 5, :233-237, :259-261). mask = OR of:
+ *  NO_CULL:     the fields are queried and aggregated for every stored Gaussian; those failing Eq. 9 are dropped at
+ *               projection instead (zero record, zero tiles), so the image is unchanged and only the cost moves
+ *               (the paper's "w/o pre-culling", 27 vs 106 FPS);
+ *  NO_BG:       no background compositing (out = C_fg);
+ *  NO_NEURAL:   decoder outputs taken as 0: explicit isotropic, diffuse Gaussians only (no field query at all);
+ *  NO_EXPLICIT: s_e = alpha_e = c_e = 0 in Eq. 7 (positions stay explicit).
+ * A single shared field needs no switch: upload the same table for geo and app. Default 0 = the full model. */
+typedef enum {
+    HYRF_ABL_NO_CULL = 1, HYRF_ABL_NO_BG = 2, HYRF_ABL_NO_NEURAL = 4, HYRF_ABL_NO_EXPLICIT = 8
+} hyrf_ablation;
+hyrf_status hyrf_set_ablation(hyrf_scene* scene, uint32_t mask);
+
 /* Number of kernels the last render launched (for bench.py's gpu_launches). */
 hyrf_status hyrf_last_launch_count(hyrf_scene* scene, uint32_t* launches);
 

@@ -389,22 +389,58 @@ def stage_background(osc: OracleScene, cam, W: int, H: int, cfg: np.ndarray, T: 
     return out, bg_mask
 
 
+# Ablation switches of the same pass (PAPER.md:214-223 Table 5, :233-237, :259-261).
+#  NO_CULL     "w/o pre-culling": the fields are queried and aggregated for EVERY stored Gaussian (the overhead the
+#              paper's 3.9x is about, :261); Gaussians that fail Eq. 9 are dropped at projection instead (their
+#              projected record, rectangle and tiles-touched are zero), so the image is the full model's.
+#  NO_BG       "w/o background": out = C_fg, nothing is composited.
+#  NO_NEURAL   "w/o neural": all decoder outputs are 0 -> isotropic, diffuse, identity-rotation Gaussians (:237, :259).
+#  NO_EXPLICIT "w/o explicit": s_e = alpha_e = c_e = 0 in Eq. 7 (the position stays explicit).
+# A single shared field (:233) needs no switch: pass the same table for geo and app.
+ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
+
+
+def _without_explicit(osc: OracleScene) -> OracleScene:
+    import copy
+    sc = copy.copy(osc.src)
+    sc.rgb_logit = np.zeros_like(_f32(osc.src.rgb_logit))
+    sc.scale_logit = np.zeros_like(_f32(osc.src.scale_logit))
+    sc.opacity_logit = np.zeros_like(_f32(osc.src.opacity_logit))
+    return OracleScene(sc)
+
+
 def render(osc: OracleScene, cam, W: Optional[int] = None, H: Optional[int] = None,
-           attrs_override: Optional[np.ndarray] = None) -> Dict[str, np.ndarray]:
+           attrs_override: Optional[np.ndarray] = None, ablation: int = 0) -> Dict[str, np.ndarray]:
     """The whole pass in the paper's order: cull -> query -> aggregate -> project/bin/sort ->
     rasterise -> background. Returns every intermediate. `attrs_override` replaces the stage-3 output (used by
-    the hand-off parity test of SURVEY §8c H1 to drive stages 4-6 from given attributes)."""
+    the hand-off parity test of SURVEY §8c H1 to drive stages 4-6 from given attributes). `ablation`: ABL_* bits."""
     W = int(cam.W if W is None else W)
     H = int(cam.H if H is None else H)
     mask, vis_idx = stage_cull(osc, cam, W, H)
-    raw = stage_query(osc, cam, vis_idx)
-    attrs = stage_aggregate(osc, vis_idx, raw)
+    in_frustum = None
+    if ablation & ABL_NO_CULL:
+        in_frustum = mask.astype(bool)
+        mask = np.ones(osc.n, np.uint8)
+        vis_idx = np.arange(osc.n, dtype=np.uint32)
+    raw = np.zeros((len(vis_idx), 11), np.float32) if ablation & ABL_NO_NEURAL else stage_query(osc, cam, vis_idx)
+    attrs = stage_aggregate(_without_explicit(osc) if ablation & ABL_NO_EXPLICIT else osc, vis_idx, raw)
     if attrs_override is not None:
         attrs = _f32(attrs_override, (len(vis_idx), 11))
     pr = stage_project(osc, cam, W, H, vis_idx, attrs)
+    if in_frustum is not None:
+        drop = ~in_frustum
+        pr["proj"][drop] = 0.0
+        pr["cov"][drop] = 0.0
+        pr["radius"][drop] = 0.0
+        pr["rect"][drop] = 0
+        pr["tiles"][drop] = 0
+        pr["D"] = int(pr["tiles"].astype(np.uint64).sum())
     bn = stage_bin(W, H, vis_idx, pr["proj"], pr["rect"], pr["tiles"])
     rs = stage_raster(W, H, pr["proj"], bn["list_rank"], bn["ranges"])
-    out, bg_mask = stage_background(osc, cam, W, H, rs["cfg"], rs["T"])
+    if ablation & ABL_NO_BG:
+        out, bg_mask = rs["cfg"].copy(), np.zeros((H, W), np.uint8)
+    else:
+        out, bg_mask = stage_background(osc, cam, W, H, rs["cfg"], rs["T"])
     res = dict(mask=mask, vis_idx=vis_idx, raw=raw, attrs=attrs, out=out, bg_mask=bg_mask, W=W, H=H)
     res.update(pr)
     res.update(bn)

@@ -26,7 +26,8 @@ DBG_ALL = (1 << 12) - 1
 
 EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_render", "hyrf_render_host",
            "hyrf_destroy_scene", "hyrf_last_error", "hyrf_debug_enable", "hyrf_debug_fetch", "hyrf_set_timing",
-           "hyrf_stage_times", "hyrf_last_launch_count"]
+           "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation"]
+ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
 
 
 class GridDesc(C.Structure):
@@ -94,6 +95,7 @@ def load_library() -> C.CDLL:
         L.hyrf_set_timing.argtypes = [vp, C.c_int32]
         L.hyrf_stage_times.argtypes = [vp, C.POINTER(C.c_float)]
         L.hyrf_last_launch_count.argtypes = [vp, C.POINTER(C.c_uint32)]
+        L.hyrf_set_ablation.argtypes = [vp, C.c_uint32]
         for name in EXPORTS:
             if name != "hyrf_last_error":
                 getattr(L, name).restype = C.c_int
@@ -259,6 +261,10 @@ class HyrfScene:
                     proj=f(DBG_PROJ), rect=f(DBG_RECT), ranges=f(DBG_TILE_RANGES), list_id=f(DBG_TILE_LIST),
                     T=f(DBG_FINAL_T).reshape(H, W), bg_mask=f(DBG_BG_MASK).reshape(H, W), counters=f(DBG_COUNTERS),
                     cfg=f(DBG_FG).reshape(H, W, 3))
+
+    def set_ablation(self, mask: int) -> None:
+        """Ablation switches of include/hyrf.h (Table 5): ABL_NO_CULL | ABL_NO_BG | ABL_NO_NEURAL | ABL_NO_EXPLICIT."""
+        _check(self.lib.hyrf_set_ablation(self.handle, int(mask)))
 
     def set_timing(self, on: bool = True) -> None:
         _check(self.lib.hyrf_set_timing(self.handle, int(on)))

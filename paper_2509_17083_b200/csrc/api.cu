@@ -354,6 +354,7 @@ hyrf_status build_frame(const hyrf_scene* s, const hyrf_camera* cam, int32_t W, 
         f->aabb_c[a] = 0.5f * (s->desc.aabb_min[a] + s->desc.aabb_max[a]);
         f->aabb_h[a] = 0.5f * (s->desc.aabb_max[a] - s->desc.aabb_min[a]);
     }
+    f->ablation = s->ablation;
     f->W = W; f->H = H;
     f->gx = (W + HY_TILE - 1) / HY_TILE; f->gy = (H + HY_TILE - 1) / HY_TILE;
     return HYRF_OK;
@@ -384,7 +385,9 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     if (timing) cudaEventRecord(s->ev[1], s->stream);
 
     // S2 + S3 + S4a: field query, aggregation, projection
-    if ((st = s->use_mma ? hy_launch_field_mma(s, f, &launches) : hy_launch_field_fma(s, f, &launches)) != HYRF_OK) return st;
+    // (explicit-only ablation: no field is queried, so the CUDA-core kernel's early-out path serves both dtypes)
+    const bool mma = s->use_mma && !(s->ablation & HYRF_ABL_NO_NEURAL);
+    if ((st = mma ? hy_launch_field_mma(s, f, &launches) : hy_launch_field_fma(s, f, &launches)) != HYRF_OK) return st;
     if (timing) cudaEventRecord(s->ev[2], s->stream);
 
     // counters (V, D) start their way to the host now; the depth ordering below does not need them, so the copy
@@ -494,6 +497,13 @@ extern "C" hyrf_status hyrf_stage_times(hyrf_scene* s, float ms[6]) {
     for (int k = 0; k < 5; ++k)
         if ((e = cudaEventElapsedTime(&ms[k], s->ev[k], s->ev[k + 1])) != cudaSuccess) return hy_cuda_fail(e, "cudaEventElapsedTime");
     if ((e = cudaEventElapsedTime(&ms[5], s->ev[0], s->ev[5])) != cudaSuccess) return hy_cuda_fail(e, "cudaEventElapsedTime");
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_set_ablation(hyrf_scene* s, uint32_t mask) {
+    if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_ablation: NULL scene");
+    if (mask & ~15u) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_ablation: unknown bits in mask %u", mask);
+    s->ablation = mask;
     return HYRF_OK;
 }
 

@@ -29,6 +29,7 @@ struct FrameDev {
     float z_near, tau_T, bg_radius;
     float aabb_c[3], aabb_h[3];
     int32_t W, H, gx, gy;
+    uint32_t ablation;  // hyrf_ablation bits (include/hyrf.h)
 };
 
 // D6 soft exponential: the one exp behind every sigmoid, so geometry decisions are bit-reproducible.

@@ -71,6 +71,7 @@ cull_mark_kernel(const float4* __restrict__ gm, const uint32_t* __restrict__ gm_
             float X, Y, Z;
             hy_to_camera(f, p.x, p.y, p.z, X, Y, Z);
             keep = (Z > f.z_near) && (fabsf(X) <= __fmul_rn(f.limx, Z)) && (fabsf(Y) <= __fmul_rn(f.limy, Z));
+            keep = keep || (f.ablation & HYRF_ABL_NO_CULL);   // "w/o pre-culling": everything goes to the fields
             vis_by_id[__ldg(gm_id + m)] = keep ? 1 : 0;
         }
         const uint32_t bal = __ballot_sync(0xffffffffu, keep);

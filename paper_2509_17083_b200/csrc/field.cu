@@ -47,6 +47,12 @@ field_fma_kernel(const FieldArgs A) {
         float x[3];
         hy_contract(A.f, px, py, pz, x);
         float bufa[MAXD], bufb[MAXD], raw[11];
+        if (A.f.ablation & HYRF_ABL_NO_NEURAL) {   // explicit-only ablation: the decoders contribute nothing
+#pragma unroll
+            for (int k = 0; k < 11; ++k) raw[k] = 0.0f;
+            aggregate_project<false>(A, ex, raw);
+            continue;
+        }
         // geometry field (Eq. 3, 4)
 #pragma unroll
         for (int l = 0; l < Lg; ++l) {

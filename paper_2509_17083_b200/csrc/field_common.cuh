@@ -36,6 +36,7 @@ static __device__ __forceinline__ Explicit fetch_visible(const FieldArgs& A, uin
     Explicit e;
     e.px = a.x; e.py = a.y; e.pz = a.z; e.s_e = a.w;
     e.a_e = b.x; e.c_e0 = b.y; e.c_e1 = b.z; e.c_e2 = b.w;
+    if (A.f.ablation & HYRF_ABL_NO_EXPLICIT) e.s_e = e.a_e = e.c_e0 = e.c_e1 = e.c_e2 = 0.0f;
     e.j = __ldg(A.word_rank + (id >> 5)) + __popc(__ldg(A.id_words + (id >> 5)) & ((1u << (id & 31u)) - 1u));
     return e;
 }
@@ -131,7 +132,10 @@ static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, con
     float cA = 0.0f, cB = 0.0f, cC = 0.0f, radius = 0.0f;
     uint4 rc = make_uint4(0, 0, 0, 0);
     uint32_t nt = 0;
-    if (det != 0.0f && isfinite(det)) {
+    // "w/o pre-culling" ablation: Eq. 9 is applied here instead of in S1 (D1's test on the same X, Y, Z)
+    const bool dropped = (f.ablation & HYRF_ABL_NO_CULL) &&
+                         !((Z > f.z_near) && (fabsf(X) <= __fmul_rn(f.limx, Z)) && (fabsf(Y) <= __fmul_rn(f.limy, Z)));
+    if (!dropped && det != 0.0f && isfinite(det)) {
         const float di = __fdiv_rn(1.0f, det);
         cA = __fmul_rn(c, di);
         cB = __fmul_rn(-b, di);
@@ -154,9 +158,14 @@ static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, con
         const uint32_t wsum = __reduce_add_sync(am, nt);
         if ((threadIdx.x & 31u) == (uint32_t)(__ffs(am) - 1) && wsum) atomicAdd(&A.counters->D, (unsigned long long)wsum);
     }
-    A.rec[3ull * j + 0] = make_float4(u, v, cA, cB);
-    A.rec[3ull * j + 1] = make_float4(cC, alpha, c0, c1);
-    A.rec[3ull * j + 2] = make_float4(c2, Z, radius, __uint_as_float(nt));
+    if (dropped) {
+        const float4 zero = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        A.rec[3ull * j + 0] = zero; A.rec[3ull * j + 1] = zero; A.rec[3ull * j + 2] = zero;
+    } else {
+        A.rec[3ull * j + 0] = make_float4(u, v, cA, cB);
+        A.rec[3ull * j + 1] = make_float4(cC, alpha, c0, c1);
+        A.rec[3ull * j + 2] = make_float4(c2, Z, radius, __uint_as_float(nt));
+    }
     A.depth_key[j] = __float_as_uint(Z);   // key of the depth sort (S4c); its value is the visible rank j itself
     A.rect[j] = rc;
     A.tiles[j] = nt;

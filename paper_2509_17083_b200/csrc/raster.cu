@@ -139,7 +139,8 @@ void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint32_t* list, fl
     const unsigned grid = (unsigned)(f.gx * f.gy);
     const bool want_fg = (s->debug_mask >> HYRF_DBG_FG) & 1u;
     const bool want_mask = (s->debug_mask >> HYRF_DBG_BG_MASK) & 1u;
-    raster_kernel<<<grid, kBatch, 0, s->stream>>>(s->ranges, list, s->rec, f.W, f.H, f.gx, f.tau_T, out_rgb, s->finalT,
+    const float tau = (f.ablation & HYRF_ABL_NO_BG) ? INFINITY : f.tau_T;   // no background: empty S6 list
+    raster_kernel<<<grid, kBatch, 0, s->stream>>>(s->ranges, list, s->rec, f.W, f.H, f.gx, tau, out_rgb, s->finalT,
                                                   s->bg_list, s->counters, want_mask ? s->bg_mask : nullptr,
                                                   want_fg ? s->fg : nullptr, tile_queue);
     ++*launches;

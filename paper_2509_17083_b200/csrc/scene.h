@@ -88,6 +88,7 @@ struct hyrf_scene {
     uint32_t* bg_list = nullptr;  // [H*W] pixels S6 has to shade, appended by the rasterizer
 
     // debug / measurement
+    uint32_t ablation = 0;            // hyrf_ablation bits
     uint32_t debug_mask = 0;
     float* dbg_raw = nullptr;         // [N][11]
     float* dbg_attrs = nullptr;       // [N][11]

@@ -18,10 +18,11 @@ def B():
     return binding
 
 
-def _run(B, ho, scene, cams=None, mlp_path=None, exact=True, label=""):
+def _run(B, ho, scene, cams=None, mlp_path=None, exact=True, label="", ablation=0):
     import torch
     mlp_path = B.HYRF_MLP_FMA if mlp_path is None else mlp_path
     hs = B.HyrfScene(scene, mlp_path=mlp_path)
+    hs.set_ablation(ablation)
     hs.debug_enable()
     osc = ho.OracleScene(scene)
     stats = []
@@ -29,7 +30,7 @@ def _run(B, ho, scene, cams=None, mlp_path=None, exact=True, label=""):
         out = hs.render(cam)
         torch.cuda.synchronize()
         gpu = hs.debug_all(cam.W, cam.H)
-        orc = ho.render(osc, cam)
+        orc = ho.render(osc, cam, ablation=ablation)
         stats.append(compare_frame(orc, gpu, out.cpu().numpy(), scene.tau_T, fp16=scene.fp16, exact_geometry=exact,
                                    label=f"{label or scene.name} cam{ci}"))
     hs.close()
@@ -213,3 +214,34 @@ def test_config5_points(B, ho, synth):
     _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False)
     s = synth.make_scene(5, n_gaussians=500_000, width=1920, height=1080)
     _run(B, ho, s, mlp_path=B.HYRF_MLP_FMA, exact=True)
+
+
+@pytest.mark.parametrize("abl", [1, 2, 4, 8, 1 | 2, 4 | 8, 15])
+def test_ablation_switches_exact_path(B, ho, synth, abl):
+    # PAPER.md Table 5 switches on the exact path: everything bit-exact against the oracle's
+    # same switch; config-3 recipe so that ~40 % of the Gaussians are outside the frustum (NO_CULL has work to do)
+    s = synth.make_scene(3, n_gaussians=30_000, width=208, height=120, n_cameras=2)
+    st = _run(B, ho, s, ablation=abl)
+    if abl & 1:
+        assert st[0]["V"] == s.n                      # every stored Gaussian was queried
+
+
+def test_ablation_switches_tensor_path(B, ho, synth):
+    s = synth.make_scene(3, n_gaussians=30_000, width=208, height=120, n_cameras=1)
+    for abl in (1, 8, 1 | 2 | 8, 4):
+        _run(B, ho, s, mlp_path=B.HYRF_MLP_MMA, exact=(abl & 4) != 0, ablation=abl)
+
+
+def test_no_cull_image_equals_full_model(B, synth):
+    # NO_CULL moves work, not pixels: same image bit for bit on the exact path
+    import torch
+    s = synth.make_scene(3, n_gaussians=30_000, width=208, height=120, n_cameras=1)
+    hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_FMA)
+    a = hs.render(s.cameras[0]).clone()
+    hs.set_ablation(B.ABL_NO_CULL)
+    b = hs.render(s.cameras[0]).clone()
+    torch.cuda.synchronize()
+    assert (a == b).all()
+    with pytest.raises(B.HyrfError):
+        hs.set_ablation(16)
+    hs.close()
