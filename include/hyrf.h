@@ -124,6 +124,14 @@ hyrf_status hyrf_render(hyrf_scene* scene, const hyrf_camera* camera, int32_t W,
 hyrf_status hyrf_render_host(hyrf_scene* scene, const hyrf_camera* camera, int32_t W, int32_t H,
                              float* out_rgb_host);
 
+/* Pipelined variant for a stream of frames: returns as soon as the frame is enqueued (and its counters are known);
+ * the device->host copy of the image runs on a second stream and overlaps the next hyrf_render_host_async. Two
+ * frames may be in flight, so the caller alternates between (at least) two host buffers and calls hyrf_host_sync
+ * before reading them. hyrf_host_sync waits for every render and copy enqueued so far. */
+hyrf_status hyrf_render_host_async(hyrf_scene* scene, const hyrf_camera* camera, int32_t W, int32_t H,
+                                   float* out_rgb_host);
+hyrf_status hyrf_host_sync(hyrf_scene* scene);
+
 hyrf_status hyrf_destroy_scene(hyrf_scene* scene);
 
 const char* hyrf_last_error(void);

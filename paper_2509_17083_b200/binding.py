@@ -26,7 +26,8 @@ DBG_ALL = (1 << 12) - 1
 
 EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_render", "hyrf_render_host",
            "hyrf_destroy_scene", "hyrf_last_error", "hyrf_debug_enable", "hyrf_debug_fetch", "hyrf_set_timing",
-           "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation"]
+           "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation", "hyrf_render_host_async",
+           "hyrf_host_sync"]
 ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
 
 
@@ -96,6 +97,8 @@ def load_library() -> C.CDLL:
         L.hyrf_stage_times.argtypes = [vp, C.POINTER(C.c_float)]
         L.hyrf_last_launch_count.argtypes = [vp, C.POINTER(C.c_uint32)]
         L.hyrf_set_ablation.argtypes = [vp, C.c_uint32]
+        L.hyrf_render_host_async.argtypes = [vp, C.POINTER(CameraC), C.c_int32, C.c_int32, vp]
+        L.hyrf_host_sync.argtypes = [vp]
         for name in EXPORTS:
             if name != "hyrf_last_error":
                 getattr(L, name).restype = C.c_int
@@ -240,6 +243,14 @@ class HyrfScene:
         c = camera_struct(cam)
         _check(self.lib.hyrf_render_host(self.handle, C.byref(c), W, H, C.c_void_p(out.data_ptr())))
         return out
+
+    def render_host_async(self, cam_struct: CameraC, W: int, H: int, out) -> None:
+        """Pipelined delivery (hyrf_render_host_async): `out` is a pinned host tensor; alternate between two of them
+        and call host_sync() before reading."""
+        _check(self.lib.hyrf_render_host_async(self.handle, C.byref(cam_struct), W, H, C.c_void_p(out.data_ptr())))
+
+    def host_sync(self) -> None:
+        _check(self.lib.hyrf_host_sync(self.handle))
 
     # -- debug / measurement --------------------------------------------------------------------------------
     def debug_enable(self, mask: int = DBG_ALL) -> None:

@@ -158,12 +158,17 @@ void destroy(hyrf_scene* s) {
                     (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w,
                     s->gm, s->gm_id, s->flag_words, s->id_words, s->word_rank, s->vis_by_id, s->vis_m, s->block_counts, s->vis_idx, s->rec, s->rect, s->tiles,
                     s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->tt_sorted, s->offs,
-                    s->scan_scratch, s->counters, s->ranges, s->tile_queue, s->fg, s->finalT, s->image, s->bg_mask, s->bg_list,
+                    s->scan_scratch, s->counters, s->ranges, s->tile_queue, s->fg, s->finalT, s->image, s->image2, s->bg_mask, s->bg_list,
                     s->dbg_raw, s->dbg_attrs};
     for (void* p : ptrs) dev_free(s, p);
     free_entries(s);
     if (s->counters_host) cudaFreeHost(s->counters_host);
     if (s->ev_counters) cudaEventDestroy(s->ev_counters);
+    if (s->copy_stream) {
+        cudaStreamSynchronize(s->copy_stream);
+        for (int k = 0; k < 2; ++k) { cudaEventDestroy(s->ev_rendered[k]); cudaEventDestroy(s->ev_copied[k]); }
+        cudaStreamDestroy(s->copy_stream);
+    }
     if (s->ev_valid)
         for (auto& e : s->ev) cudaEventDestroy(e);
     delete s;
@@ -480,6 +485,45 @@ extern "C" hyrf_status hyrf_render_host(hyrf_scene* s, const hyrf_camera* cam, i
     cudaError_t e = cudaMemcpyAsync(out_host, s->image, (size_t)W * H * 3 * sizeof(float), cudaMemcpyDeviceToHost, s->stream);
     if (e != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpyAsync(image)");
     if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(image)");
+    return HYRF_OK;
+}
+
+// Pipelined host delivery: frame k renders into one of two library-owned device images on the scene's stream; its
+// device->host copy runs on a second stream behind an event, so it overlaps the render of frame k+1.
+extern "C" hyrf_status hyrf_render_host_async(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_t H, float* out_host) {
+    if (!s || !out_host) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_render_host_async: NULL argument");
+    cudaError_t e;
+    if ((e = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
+    hyrf_status st;
+    if (!s->copy_stream) {
+        if ((e = cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamCreate(copy)");
+        for (int k = 0; k < 2; ++k) {
+            if ((e = cudaEventCreateWithFlags(&s->ev_rendered[k], cudaEventDisableTiming)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventCreate");
+            if ((e = cudaEventCreateWithFlags(&s->ev_copied[k], cudaEventDisableTiming)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventCreate");
+        }
+    }
+    const size_t P3 = (size_t)s->desc.max_width * s->desc.max_height * 3;
+    if (!s->image && (st = dev_alloc_t(s, &s->image, P3)) != HYRF_OK) return st;
+    if (!s->image2 && (st = dev_alloc_t(s, &s->image2, P3)) != HYRF_OK) return st;
+    const int slot = (s->host_slot ^= 1);
+    float* img = slot ? s->image2 : s->image;
+    // the copy that last read this image must have finished before it is rendered into again
+    if (s->slot_used[slot] && (e = cudaStreamWaitEvent(s->stream, s->ev_copied[slot], 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent");
+    if ((st = render_impl(s, cam, W, H, img)) != HYRF_OK) return st;
+    if ((e = cudaEventRecord(s->ev_rendered[slot], s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord");
+    if ((e = cudaStreamWaitEvent(s->copy_stream, s->ev_rendered[slot], 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent");
+    if ((e = cudaMemcpyAsync(out_host, img, (size_t)W * H * 3 * sizeof(float), cudaMemcpyDeviceToHost, s->copy_stream)) != cudaSuccess)
+        return hy_cuda_fail(e, "cudaMemcpyAsync(image)");
+    if ((e = cudaEventRecord(s->ev_copied[slot], s->copy_stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord");
+    s->slot_used[slot] = true;
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_host_sync(hyrf_scene* s) {
+    if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_host_sync: NULL scene");
+    cudaError_t e;
+    if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize");
+    if (s->copy_stream && (e = cudaStreamSynchronize(s->copy_stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(copy)");
     return HYRF_OK;
 }
 

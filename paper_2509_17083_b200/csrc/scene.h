@@ -84,6 +84,11 @@ struct hyrf_scene {
     float* fg = nullptr;      // [H][W][3] (debug only)
     float* finalT = nullptr;  // [H][W]
     float* image = nullptr;   // [H][W][3] for hyrf_render_host
+    float* image2 = nullptr;  // second image of hyrf_render_host_async's double buffer
+    cudaStream_t copy_stream = nullptr;       // device->host copies of hyrf_render_host_async
+    cudaEvent_t ev_rendered[2] = {}, ev_copied[2] = {};
+    bool slot_used[2] = {false, false};
+    int host_slot = 0;
     uint8_t* bg_mask = nullptr;
     uint32_t* bg_list = nullptr;  // [H*W] pixels S6 has to shade, appended by the rasterizer
 

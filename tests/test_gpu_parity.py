@@ -245,3 +245,27 @@ def test_no_cull_image_equals_full_model(B, synth):
     with pytest.raises(B.HyrfError):
         hs.set_ablation(16)
     hs.close()
+
+
+def test_pipelined_host_delivery_matches_synchronous(B, synth):
+    # hyrf_render_host_async: two frames in flight, copies on a second stream; every delivered image must be the
+    # image the synchronous call produces for the same camera
+    import torch
+    s = synth.make_scene(3, n_gaussians=40_000, width=320, height=180, n_cameras=5)
+    hs = B.HyrfScene(s)
+    ref = [hs.render_host(c).clone() for c in s.cameras]
+    bufs = [torch.empty((180, 320, 3), dtype=torch.float32).pin_memory() for _ in range(2)]
+    got = []
+    for i, c in enumerate(s.cameras):
+        if i >= 2:
+            hs.host_sync()                      # buffer i & 1 is about to be reused
+            got.append(bufs[i & 1].clone())
+        hs.render_host_async(B.camera_struct(c), 320, 180, bufs[i & 1])
+    hs.host_sync()
+    # frames 0..2 were cloned when their buffer came up for reuse; the last two are still in the buffers
+    got.append(bufs[1].clone() if len(s.cameras) % 2 == 0 else bufs[(len(s.cameras) - 2) & 1].clone())
+    got.append(bufs[(len(s.cameras) - 1) & 1].clone())
+    assert len(got) == len(ref)
+    for i, (a, b) in enumerate(zip(got, ref)):
+        assert (a == b).all(), f"frame {i} differs"
+    hs.close()
