@@ -23,7 +23,7 @@ struct BgArgs {
 template <int CL, int CHID, int CNH, bool FP16>
 __global__ void __launch_bounds__(kBgThreads)
 background_kernel(const BgArgs A) {
-    extern __shared__ float smem_w[];
+    extern __shared__ __align__(16) float smem_w[];
     const int L = CL > 0 ? CL : (int)A.grid.levels;
     const int in_dim = (int)A.mlp.in_dim, hid = (int)A.mlp.hidden, nh = (int)A.mlp.n_hidden;
     const int nw = in_dim * hid + (nh - 1) * hid * hid + hid * 3;

@@ -17,7 +17,7 @@ constexpr int kFieldThreads = 128;
 template <int CL, int CHID, int CNH, bool FP16>
 __global__ void __launch_bounds__(kFieldThreads)
 field_fma_kernel(const FieldArgs A) {
-    extern __shared__ float smem_w[];
+    extern __shared__ __align__(16) float smem_w[];
     const int Lg = CL > 0 ? CL : (int)A.geo.levels;
     const int La = CL > 0 ? CL : (int)A.app.levels;
     const int geo_in = (int)A.geo_mlp.in_dim, app_in = (int)A.app_mlp.in_dim;

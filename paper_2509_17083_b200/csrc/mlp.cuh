@@ -2,6 +2,29 @@
 #pragma once
 #include "common.cuh"
 
+// One neuron: acc = fma(w[k], h[k], acc), k ascending (D5's order). VEC: the row is 16-byte aligned and a multiple of
+// 4 long (compile-time shapes: rows of 32 / 40 / 56 / 64 floats in a 16-byte aligned block), so the weights come as
+// broadcast LDS.128 — a quarter of the shared-memory instructions of the scalar form, same arithmetic.
+template <bool VEC>
+__device__ __forceinline__ float mlp_dot(const float* __restrict__ w, const float* h, int n) {
+    float acc = 0.0f;
+    if (VEC) {
+        const float4* w4 = reinterpret_cast<const float4*>(w);
+#pragma unroll
+        for (int k = 0; k < n / 4; ++k) {
+            const float4 q = w4[k];
+            acc = __fmaf_rn(q.x, h[4 * k], acc);
+            acc = __fmaf_rn(q.y, h[4 * k + 1], acc);
+            acc = __fmaf_rn(q.z, h[4 * k + 2], acc);
+            acc = __fmaf_rn(q.w, h[4 * k + 3], acc);
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < n; ++k) acc = __fmaf_rn(w[k], h[k], acc);
+    }
+    return acc;
+}
+
 // One decoder: in[IN] -> hidden x NH (ReLU) -> out[OUT]. Weights in shared memory as fp32, row-major [out][in].
 // CIN/CHID/CNH > 0: compile-time shapes, fully unrolled, activations in registers. 0: run-time shapes.
 template <int CIN, int CHID, int CNH, int OUT, bool FP16>
@@ -16,23 +39,16 @@ __device__ __forceinline__ void mlp_eval(const float* __restrict__ w, int rin, i
 #pragma unroll
     for (int layer = 0; layer < NH; ++layer) {
 #pragma unroll
-        for (int j = 0; j < HID; ++j) {
-            float acc = 0.0f;
+        for (int j = 0; j < HID; ++j) dst[j] = fmaxf(mlp_dot<(CIN > 0 && CHID > 0)>(w + j * cur, src, cur), 0.0f);
+        if (FP16) {
 #pragma unroll
-            for (int k = 0; k < cur; ++k) acc = __fmaf_rn(w[j * cur + k], src[k], acc);
-            acc = fmaxf(acc, 0.0f);
-            dst[j] = FP16 ? hy_round_half(acc) : acc;
+            for (int j = 0; j < HID; ++j) dst[j] = hy_round_half(dst[j]);
         }
         w += HID * cur;
         cur = HID;
         float* t = src; src = dst; dst = t;
     }
 #pragma unroll
-    for (int j = 0; j < OUT; ++j) {
-        float acc = 0.0f;
-#pragma unroll
-        for (int k = 0; k < cur; ++k) acc = __fmaf_rn(w[j * cur + k], src[k], acc);
-        out[j] = acc;
-    }
+    for (int j = 0; j < OUT; ++j) out[j] = mlp_dot<(CIN > 0 && CHID > 0)>(w + j * cur, src, cur);
 }
 
