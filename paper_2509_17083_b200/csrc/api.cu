@@ -156,7 +156,7 @@ void destroy(hyrf_scene* s) {
     cudaStreamSynchronize(s->stream);
     void* ptrs[] = {s->pos, s->rgb, s->scale, s->opac, (void*)s->geo_grid.table, (void*)s->app_grid.table,
                     (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w,
-                    s->gm, s->gm_id, s->flag_words, s->id_words, s->word_rank, s->vis_by_id, s->vis_m, s->block_counts, s->vis_idx, s->rec, s->rect, s->tiles,
+                    s->gm, s->gm_id, s->flag_words, s->id_words, s->word_rank, s->vis_m, s->block_counts, s->vis_idx, s->rec, s->rect, s->tiles,
                     s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->tt_sorted, s->offs,
                     s->scan_scratch, s->counters, s->ranges, s->tile_queue, s->fg, s->finalT, s->image, s->image2, s->bg_mask, s->bg_list,
                     s->dbg_raw, s->dbg_attrs};
@@ -258,7 +258,6 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc_t(s, &s->flag_words, (N + 31) / 32 + 32));
     HY_TRY(dev_alloc_t(s, &s->id_words, (N + 31) / 32 + 32));
     HY_TRY(dev_alloc_t(s, &s->word_rank, (N + 31) / 32 + 32));
-    HY_TRY(dev_alloc_t(s, &s->vis_by_id, N));
     HY_TRY(dev_alloc_t(s, &s->vis_m, N));
     HY_TRY(dev_alloc_t(s, &s->block_counts, 4 * cull_blocks + 8));
     HY_TRY(dev_alloc_t(s, &s->vis_idx, N));
@@ -585,7 +584,7 @@ extern "C" hyrf_status hyrf_debug_fetch(hyrf_scene* s, uint32_t kind, void* host
     const void* src = nullptr;
     size_t need = 0;
     switch (kind) {
-        case HYRF_DBG_VIS_MASK: src = s->vis_by_id; need = N; break;
+        case HYRF_DBG_VIS_MASK: need = N; break;
         case HYRF_DBG_VIS_IDX: src = s->vis_idx; need = V * 4; break;
         case HYRF_DBG_STAGE2_RAW: if (!on) goto off; src = s->dbg_raw; need = V * 44; break;
         case HYRF_DBG_STAGE3_ATTRS: if (!on) goto off; src = s->dbg_attrs; need = V * 44; break;
@@ -606,6 +605,13 @@ extern "C" hyrf_status hyrf_debug_fetch(hyrf_scene* s, uint32_t kind, void* host
     if (kind == HYRF_DBG_COUNTERS) {
         uint64_t c[4] = {N, V, D, n_tiles};
         memcpy(host_dst, c, sizeof(c));
+        return HYRF_OK;
+    }
+    if (kind == HYRF_DBG_VIS_MASK) {   // visibility bits by id -> one byte per Gaussian
+        std::vector<uint32_t> words((N + 31) / 32);
+        if ((e = cudaMemcpy(words.data(), s->id_words, words.size() * 4, cudaMemcpyDeviceToHost)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpy(id_words)");
+        uint8_t* o = static_cast<uint8_t*>(host_dst);
+        for (size_t i = 0; i < N; ++i) o[i] = (words[i >> 5] >> (i & 31)) & 1u;
         return HYRF_OK;
     }
     if (kind == HYRF_DBG_PROJ) {   // records -> (u, v, depth, A, B, C, opacity, r, g, b)

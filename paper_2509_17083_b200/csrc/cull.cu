@@ -54,80 +54,78 @@ __global__ void morton_gather_kernel(const uint32_t* __restrict__ order, const f
     gm_id[m] = i;
 }
 
-// Morton order: test, visibility bits + block counts (Morton), visibility byte by id
-__global__ void __launch_bounds__(kCullThreads)
-cull_mark_kernel(const float4* __restrict__ gm, const uint32_t* __restrict__ gm_id, uint32_t N, FrameDev f,
-                 uint32_t* __restrict__ flag_words, uint32_t* __restrict__ block_counts, uint8_t* __restrict__ vis_by_id) {
-    __shared__ uint32_t warp_cnt[kCullThreads / 32];
-    const uint32_t base = blockIdx.x * kCullItems;
-    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t cnt = 0;
-#pragma unroll
-    for (int k = 0; k < kCullItems / kCullThreads; ++k) {
-        const uint32_t m = base + k * kCullThreads + threadIdx.x;
-        bool keep = false;
-        if (m < N) {
-            const float4 p = __ldg(gm + 2ull * m);
-            float X, Y, Z;
-            hy_to_camera(f, p.x, p.y, p.z, X, Y, Z);
-            keep = (Z > f.z_near) && (fabsf(X) <= __fmul_rn(f.limx, Z)) && (fabsf(Y) <= __fmul_rn(f.limy, Z));
-            keep = keep || (f.ablation & HYRF_ABL_NO_CULL);   // "w/o pre-culling": everything goes to the fields
-            vis_by_id[__ldg(gm_id + m)] = keep ? 1 : 0;
-        }
-        const uint32_t bal = __ballot_sync(0xffffffffu, keep);
-        if (lane == 0) {
-            const uint32_t word = (base >> 5) + k * (kCullThreads / 32) + warp;
-            if (word * 32u < N) flag_words[word] = bal;
-            cnt += __popc(bal);
-        }
-    }
-    if (lane == 0) warp_cnt[warp] = cnt;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        uint32_t s = 0;
-#pragma unroll
-        for (int w = 0; w < kCullThreads / 32; ++w) s += warp_cnt[w];
-        block_counts[blockIdx.x] = s;
-    }
+// One launch, two sweeps of the same Eq. 9 test (same function, same fp32 inputs, hence the same bits):
+// over the Morton records -> visibility bits + block counts in Morton order (the work list), and over the uploaded SoA
+// -> visibility bits + block counts in id order (ranks, vis_idx). Recomputing the test on the 12 MB SoA is cheaper
+// than scattering one byte per Gaussian from the Morton sweep into id order.
+__device__ __forceinline__ bool d1_keep(const FrameDev& f, float px, float py, float pz) {
+    float X, Y, Z;
+    hy_to_camera(f, px, py, pz, X, Y, Z);
+    const bool keep = (Z > f.z_near) && (fabsf(X) <= __fmul_rn(f.limx, Z)) && (fabsf(Y) <= __fmul_rn(f.limy, Z));
+    return keep || (f.ablation & HYRF_ABL_NO_CULL);   // "w/o pre-culling": everything goes to the fields
 }
 
-// id order: visibility bytes -> bits + block counts
 __global__ void __launch_bounds__(kCullThreads)
-cull_idbits_kernel(const uint8_t* __restrict__ vis_by_id, uint32_t N, uint32_t* __restrict__ id_words,
-                   uint32_t* __restrict__ block_counts) {
-    __shared__ uint32_t warp_cnt[kCullThreads / 32];
+cull_mark_kernel(const float4* __restrict__ gm, const float* __restrict__ pos, uint32_t N, FrameDev f,
+                 uint32_t* __restrict__ m_words, uint32_t* __restrict__ m_counts, uint32_t* __restrict__ id_words,
+                 uint32_t* __restrict__ id_counts) {
+    __shared__ uint32_t warp_cnt[2][kCullThreads / 32];
     const uint32_t base = blockIdx.x * kCullItems;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t cnt = 0;
+    uint32_t cnt_m = 0, cnt_i = 0;
 #pragma unroll
     for (int k = 0; k < kCullItems / kCullThreads; ++k) {
         const uint32_t i = base + k * kCullThreads + threadIdx.x;
-        const bool keep = i < N && vis_by_id[i] != 0;
-        const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+        bool keep_m = false, keep_i = false;
+        if (i < N) {
+            const float4 p = __ldg(gm + 2ull * i);
+            keep_m = d1_keep(f, p.x, p.y, p.z);
+            keep_i = d1_keep(f, __ldg(pos + i), __ldg(pos + N + i), __ldg(pos + 2ull * N + i));
+        }
+        const uint32_t bal_m = __ballot_sync(0xffffffffu, keep_m), bal_i = __ballot_sync(0xffffffffu, keep_i);
         if (lane == 0) {
             const uint32_t word = (base >> 5) + k * (kCullThreads / 32) + warp;
-            if (word * 32u < N) id_words[word] = bal;
-            cnt += __popc(bal);
+            if (word * 32u < N) { m_words[word] = bal_m; id_words[word] = bal_i; }
+            cnt_m += __popc(bal_m);
+            cnt_i += __popc(bal_i);
         }
     }
-    if (lane == 0) warp_cnt[warp] = cnt;
+    if (lane == 0) { warp_cnt[0][warp] = cnt_m; warp_cnt[1][warp] = cnt_i; }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        uint32_t s = 0;
+    if (threadIdx.x < 2) {
+        uint32_t sum = 0;
 #pragma unroll
-        for (int w = 0; w < kCullThreads / 32; ++w) s += warp_cnt[w];
-        block_counts[blockIdx.x] = s;
+        for (int w = 0; w < kCullThreads / 32; ++w) sum += warp_cnt[threadIdx.x][w];
+        (threadIdx.x ? id_counts : m_counts)[blockIdx.x] = sum;
     }
 }
 
 // Stable compaction of one bit array: out[rank] = index of the set bit; optionally word_rank[word] = rank of the
 // word's first bit (the lookup the field kernel turns an id into its visible rank with).
+// Sum of counts[0 .. blockIdx.x) by the whole block (when the host passed no scanned offsets): for the block counts
+// of a few million Gaussians this is a handful of loads per thread and saves the scan launches.
+__device__ __forceinline__ uint32_t block_offset(const uint32_t* __restrict__ counts, uint32_t* s_red /*[8]*/) {
+    uint32_t sum = 0;
+    for (uint32_t b = threadIdx.x; b < blockIdx.x; b += kCullThreads) sum += __ldg(counts + b);
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, d);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = sum;
+    __syncthreads();
+    uint32_t total = 0;
+#pragma unroll
+    for (int w = 0; w < kCullThreads / 32; ++w) total += s_red[w];
+    return total;
+}
+
 __device__ __forceinline__ void compact_bits(const uint32_t* __restrict__ words, const uint32_t* __restrict__ block_offs,
-                                             uint32_t N, uint32_t* __restrict__ out, uint32_t* __restrict__ word_rank,
-                                             uint32_t* s_prefix /*[32]*/) {
+                                             const uint32_t* __restrict__ block_counts, uint32_t N,
+                                             uint32_t* __restrict__ out, uint32_t* __restrict__ word_rank,
+                                             uint32_t* s_prefix /*[32]*/, uint32_t* s_red, uint32_t* boff_out) {
     const uint32_t base = blockIdx.x * kCullItems;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint32_t boff = block_offs[blockIdx.x];
+    const uint32_t boff = block_offs ? block_offs[blockIdx.x] : block_offset(block_counts, s_red);
+    *boff_out = boff;
     if (warp == 0) {  // 32 words per block: exclusive scan of their popcounts by one warp
         const uint32_t word = (base >> 5) + lane;
         const bool in = word * 32u < N;
@@ -157,14 +155,16 @@ __device__ __forceinline__ void compact_bits(const uint32_t* __restrict__ words,
 __global__ void __launch_bounds__(kCullThreads)
 cull_compact_kernel(const uint32_t* __restrict__ m_words, const uint32_t* __restrict__ m_offs,
                     const uint32_t* __restrict__ m_counts, const uint32_t* __restrict__ id_words,
-                    const uint32_t* __restrict__ id_offs, uint32_t N, uint32_t* __restrict__ vis_m,
-                    uint32_t* __restrict__ vis_idx, uint32_t* __restrict__ word_rank,
+                    const uint32_t* __restrict__ id_offs, const uint32_t* __restrict__ id_counts, uint32_t N,
+                    uint32_t* __restrict__ vis_m, uint32_t* __restrict__ vis_idx, uint32_t* __restrict__ word_rank,
                     FrameCounters* __restrict__ counters) {
     __shared__ uint32_t s_prefix[kCullItems / 32];
-    compact_bits(m_words, m_offs, N, vis_m, nullptr, s_prefix);
-    compact_bits(id_words, id_offs, N, vis_idx, word_rank, s_prefix);
+    __shared__ uint32_t s_red[kCullThreads / 32];
+    uint32_t boff_m, boff_i;
+    compact_bits(m_words, m_offs, m_counts, N, vis_m, nullptr, s_prefix, s_red, &boff_m);
+    compact_bits(id_words, id_offs, id_counts, N, vis_idx, word_rank, s_prefix, s_red, &boff_i);
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) {
-        counters->V = m_offs[blockIdx.x] + m_counts[blockIdx.x];
+        counters->V = boff_m + m_counts[blockIdx.x];
         counters->D = 0ull;
         counters->n_bg = 0u;
         counters->bin_ticket = 0u;
@@ -199,12 +199,16 @@ void hy_launch_cull(hyrf_scene* s, const FrameDev& f, uint32_t* launches) {
     uint32_t* m_offs = s->block_counts + nb;
     uint32_t* id_counts = s->block_counts + 2 * nb;
     uint32_t* id_offs = s->block_counts + 3 * nb;
-    cull_mark_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->gm, s->gm_id, s->N, f, s->flag_words, m_counts, s->vis_by_id);
-    cull_idbits_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->vis_by_id, s->N, s->id_words, id_counts);
-    *launches += 2;
-    hy_launch_scan(m_counts, m_offs, nb, s->scan_scratch, s->stream, launches);
-    hy_launch_scan(id_counts, id_offs, nb, s->scan_scratch, s->stream, launches);
-    cull_compact_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->flag_words, m_offs, m_counts, s->id_words, id_offs, s->N,
+    cull_mark_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->gm, s->pos, s->N, f, s->flag_words, m_counts, s->id_words,
+                                                         id_counts);
+    ++*launches;
+    const bool in_kernel = nb <= 8192;   // block offsets summed inside the compaction; beyond that, scan first
+    if (!in_kernel) {
+        hy_launch_scan(m_counts, m_offs, nb, s->scan_scratch, s->stream, launches);
+        hy_launch_scan(id_counts, id_offs, nb, s->scan_scratch, s->stream, launches);
+    }
+    cull_compact_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->flag_words, in_kernel ? nullptr : m_offs, m_counts,
+                                                            s->id_words, in_kernel ? nullptr : id_offs, id_counts, s->N,
                                                             s->vis_m, s->vis_idx, s->word_rank, s->counters);
     ++*launches;
 }

@@ -48,9 +48,8 @@ struct hyrf_scene {
 
     // per-frame scratch sized from N
     uint32_t* flag_words = nullptr;   // [ceil(N/32)] visibility bits, Morton order
-    uint32_t* id_words = nullptr;     // [ceil(N/32)] visibility bits, id order
+    uint32_t* id_words = nullptr;     // [ceil(N/32)] visibility bits, id order (also the VIS_MASK debug export)
     uint32_t* word_rank = nullptr;    // [ceil(N/32)] visible rank of the first bit of each id word
-    uint8_t* vis_by_id = nullptr;     // [N] visibility byte per id (also the VIS_MASK debug export)
     uint32_t* vis_m = nullptr;        // [N] Morton indices of the visible Gaussians (the field kernels' work list)
     uint32_t* block_counts = nullptr; // cull block counts / scanned
     uint32_t* vis_idx = nullptr;      // [N]
