@@ -152,8 +152,8 @@ def stage_rooflines(scene, V, D, n_bg, eval_pairs, peaks):
 
 def load_traffic(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu --set full capture
-    of this workload (profiles/r1b_dram_traffic.csv); None if there is no capture."""
-    p = os.path.join(ROOT, "profiles", "r1b_dram_traffic.csv")
+    of this workload (profiles/r1c_dram_traffic.csv); None if there is no capture."""
+    p = os.path.join(ROOT, "profiles", "r1c_dram_traffic.csv")
     if not os.path.exists(p):
         return None
     import csv
