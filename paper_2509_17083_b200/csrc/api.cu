@@ -155,7 +155,7 @@ void destroy(hyrf_scene* s) {
     if (!s) return;
     cudaStreamSynchronize(s->stream);
     void* ptrs[] = {s->pos, s->rgb, s->scale, s->opac, (void*)s->geo_grid.table, (void*)s->app_grid.table,
-                    (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w,
+                    (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w, s->both_table,
                     s->gm, s->gm_id, s->flag_words, s->id_words, s->word_rank, s->vis_m, s->block_counts, s->vis_idx, s->rec, s->rect, s->tiles,
                     s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->tt_sorted, s->offs,
                     s->scan_scratch, s->counters, s->ranges, s->tile_queue, s->fg, s->finalT, s->image, s->image2, s->bg_mask, s->bg_list,
@@ -253,6 +253,12 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc(s, &wa, mlp_weights(s->desc.app_mlp) * esz)); s->app_mlp.w = wa;
     HY_TRY(dev_alloc(s, &wb, mlp_weights(s->desc.bg_mlp) * esz)); s->bg_mlp.w = wb;
     if (s->use_mma) HY_TRY(dev_alloc(s, &s->mma_w, hy_field_mma_packed_bytes()));
+    {   // same grid geometry for both fields (every paper configuration): one interleaved table for the tensor path
+        const hyrf_grid_desc &g = s->desc.geo_grid, &a = s->desc.app_grid;
+        bool same = g.levels == a.levels && g.log2_table == a.log2_table;
+        for (uint32_t l = 0; same && l < g.levels; ++l) same = g.level_res[l] == a.level_res[l];
+        if (s->use_mma && same) HY_TRY(dev_alloc(s, &s->both_table, s->geo_entries * 8));
+    }
     HY_TRY(dev_alloc_t(s, &s->gm, 2 * N));
     HY_TRY(dev_alloc_t(s, &s->gm_id, N));
     HY_TRY(dev_alloc_t(s, &s->flag_words, (N + 31) / 32 + 32));

@@ -14,9 +14,6 @@
 #include "field_common.cuh"
 #include "tcgen05.cuh"
 
-#ifndef HY_FIELD_PAIR_LANES
-#define HY_FIELD_PAIR_LANES 1
-#endif
 
 namespace {
 
@@ -105,6 +102,66 @@ __device__ __forceinline__ uint32_t gather_level_pair(const GridDev& g, uint32_t
     return pack_h2(a0, a1);
 }
 
+// The same level for BOTH fields at once, when the two grids share their geometry (levels, resolutions, table size —
+// true of every paper configuration): the tables are interleaved at upload into one array of 8-byte entries
+// (geo f0, geo f1, app f0, app f1), so one index computation and one load serve both fields and the x / x+1
+// corners of both fields sit in one 16-byte span. Halves the sector look-ups and the index arithmetic.
+__device__ __forceinline__ void gather_level_pair2(const GridDev& g, const uint2* __restrict__ both, uint32_t l,
+                                                   const float x[3], uint32_t xb, uint32_t& geo, uint32_t& app) {
+    const uint32_t N = g.res[l];
+    const float Nf = (float)N;
+    uint32_t ci[3];
+    float w[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const float u = __fmul_rn(x[a], Nf);
+        int i = (int)floorf(u);
+        i = min(i, (int)N - 1);
+        ci[a] = (uint32_t)i;
+        w[a] = __fsub_rn(u, (float)i);
+    }
+    const uint32_t vx = ci[0] + xb;
+    uint32_t idx[4];
+    if ((g.dense_mask >> l) & 1u) {
+        const uint32_t n1 = N + 1u;
+        const uint32_t b = vx + n1 * (ci[1] + n1 * ci[2]);
+        idx[0] = b; idx[1] = b + n1; idx[2] = b + n1 * n1; idx[3] = b + n1 * n1 + n1;
+    } else {
+        const uint32_t hy0 = ci[1] * 2654435761u, hy1 = hy0 + 2654435761u;
+        const uint32_t hz0 = ci[2] * 805459861u, hz1 = hz0 + 805459861u;
+        idx[0] = (vx ^ hy0 ^ hz0) & g.table_mask; idx[1] = (vx ^ hy1 ^ hz0) & g.table_mask;
+        idx[2] = (vx ^ hy0 ^ hz1) & g.table_mask; idx[3] = (vx ^ hy1 ^ hz1) & g.table_mask;
+    }
+    const uint2* tab = both + g.offset[l];
+    uint2 v[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v[k] = __ldg(tab + idx[k]);
+    const float ax = xb ? w[0] : __fsub_rn(1.0f, w[0]);
+    const float wy0 = __fsub_rn(1.0f, w[1]), wz0 = __fsub_rn(1.0f, w[2]);
+    float g0 = 0.0f, g1 = 0.0f, a0 = 0.0f, a1 = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float wt = __fmul_rn(__fmul_rn(ax, (k & 1) ? w[1] : wy0), (k & 2) ? w[2] : wz0);
+        const float2 vg = __half22float2(*reinterpret_cast<const __half2*>(&v[k].x));
+        const float2 va = __half22float2(*reinterpret_cast<const __half2*>(&v[k].y));
+        g0 = __fmaf_rn(wt, vg.x, g0); g1 = __fmaf_rn(wt, vg.y, g1);
+        a0 = __fmaf_rn(wt, va.x, a0); a1 = __fmaf_rn(wt, va.y, a1);
+    }
+    g0 = __fadd_rn(g0, __shfl_xor_sync(0xffffffffu, g0, 16));
+    g1 = __fadd_rn(g1, __shfl_xor_sync(0xffffffffu, g1, 16));
+    a0 = __fadd_rn(a0, __shfl_xor_sync(0xffffffffu, a0, 16));
+    a1 = __fadd_rn(a1, __shfl_xor_sync(0xffffffffu, a1, 16));
+    geo = pack_h2(g0, g1);
+    app = pack_h2(a0, a1);
+}
+
+// geo / app tables [entry][2] half -> one table [entry][4] half
+__global__ void interleave_tables_kernel(const uint32_t* __restrict__ geo, const uint32_t* __restrict__ app, size_t n,
+                                         uint2* __restrict__ both) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) both[i] = make_uint2(geo[i], app[i]);
+}
+
 // ReLU + round to fp16 of 32 fp32 accumulator columns -> 16 packed A columns
 __device__ __forceinline__ void relu_pack32(const uint32_t* d, uint32_t* a) {
 #pragma unroll
@@ -113,11 +170,12 @@ __device__ __forceinline__ void relu_pack32(const uint32_t* d, uint32_t* a) {
 }
 
 __global__ void __launch_bounds__(kThreads, 2)
-field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w) {
+field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const uint2* __restrict__ both) {
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ __align__(8) uint64_t mbar[2];
     __shared__ uint32_t tmem_slot;
     __shared__ float s_col[kTile][3];
+    __shared__ uint32_t s_exch[2][4][16][16];   // [field sent][warp & 3][level][row & 15], interleaved-table path
 
     const uint32_t warp = threadIdx.x >> 5;
     const uint32_t chain = warp >> 2;                 // 0: geometry, 1: appearance
@@ -162,8 +220,30 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w) {
             px = ex.px; py = ex.py; pz = ex.pz;
             hy_contract(A.f, px, py, pz, x);
         }
-#if HY_FIELD_PAIR_LANES
-        {   // two lanes per Gaussian: half h covers rows 16h..16h+15 of this warp; row r's own lane keeps the result
+        if (both) {
+            // Interleaved tables: a warp gathers BOTH fields for 16 of its 32 rows (rows 16*chain .. 16*chain+15 of
+            // the quadrant it shares with warp ^ 4), two lanes per Gaussian. Each lane keeps the word of its own
+            // row and field; the words the partner warp needs go through shared memory.
+            const uint32_t lane = threadIdx.x & 31u, xb = lane >> 4;
+            const int src = (int)((chain << 4) | (lane & 15u));
+            float xs[3];
+            xs[0] = __shfl_sync(0xffffffffu, x[0], src);
+            xs[1] = __shfl_sync(0xffffffffu, x[1], src);
+            xs[2] = __shfl_sync(0xffffffffu, x[2], src);
+            const bool own = xb == chain;
+#pragma unroll
+            for (int l = 0; l < 16; ++l) {
+                uint32_t wg, wa;
+                gather_level_pair2(A.geo, both, l, xs, xb, wg, wa);
+                if (own) a[l] = chain ? wa : wg;
+                else s_exch[chain][warp & 3u][l][lane & 15u] = chain ? wg : wa;
+            }
+            __syncthreads();
+            if (!own) {
+#pragma unroll
+                for (int l = 0; l < 16; ++l) a[l] = s_exch[chain ^ 1u][warp & 3u][l][lane & 15u];
+            }
+        } else {   // separate tables: two lanes per Gaussian; half h covers rows 16h..16h+15 of this warp
             const uint32_t lane = threadIdx.x & 31u, xb = lane >> 4;
 #pragma unroll
             for (uint32_t h = 0; h < 2; ++h) {
@@ -180,14 +260,6 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w) {
                 }
             }
         }
-#else
-#pragma unroll
-        for (int l = 0; l < 16; ++l) {
-            float f0, f1;
-            hy_grid_level<true>(grid, l, x, f0, f1);
-            a[l] = pack_h2(f0, f1);
-        }
-#endif
         if (valid) {
             if (chain) {
                 const float dx = __fsub_rn(px, A.f.o[0]), dy = __fsub_rn(py, A.f.o[1]), dz = __fsub_rn(pz, A.f.o[2]);
@@ -310,6 +382,12 @@ hyrf_status hy_field_mma_prepare(hyrf_scene* s) {
     pack_weights_kernel<<<(kPackedBytes / 2 + 255) / 256, 256, 0, s->stream>>>(
         reinterpret_cast<const __half*>(s->geo_mlp.w), reinterpret_cast<const __half*>(s->app_mlp.w),
         reinterpret_cast<__half*>(s->mma_w));
+    if (s->both_table) {
+        const size_t n = s->geo_entries;
+        interleave_tables_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(
+            reinterpret_cast<const uint32_t*>(s->geo_grid.table), reinterpret_cast<const uint32_t*>(s->app_grid.table), n,
+            reinterpret_cast<uint2*>(s->both_table));
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return hy_cuda_fail(e, "pack_weights_kernel");
     return HYRF_OK;
@@ -328,7 +406,8 @@ hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* laun
     }
     const int need = (int)((s->N + kTile - 1) / kTile);
     const int grid = need < 148 * 2 ? need : 148 * 2;
-    field_mma_kernel<<<grid, kThreads, kSmemBytes, s->stream>>>(A, reinterpret_cast<const uint4*>(s->mma_w));
+    field_mma_kernel<<<grid, kThreads, kSmemBytes, s->stream>>>(A, reinterpret_cast<const uint4*>(s->mma_w),
+                                                               reinterpret_cast<const uint2*>(s->both_table));
     ++*launches;
     return HYRF_OK;
 }

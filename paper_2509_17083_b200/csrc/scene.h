@@ -43,6 +43,7 @@ struct hyrf_scene {
     size_t geo_entries = 0, app_entries = 0, bg_entries = 0;
     MlpDev geo_mlp{}, app_mlp{}, bg_mlp{};
     void* mma_w = nullptr;     // fp16 weights re-laid out for the tensor-core path (field_mma.cu)
+    void* both_table = nullptr;  // geo + app tables interleaved [entry][4] half, when the two grids share their geometry
     float4* gm = nullptr;      // [N][2] Morton-ordered records (pos.xyz, scale | opacity, rgb), built at upload (cull.cu)
     uint32_t* gm_id = nullptr; // [N] id of the m-th Gaussian in Morton order
 
