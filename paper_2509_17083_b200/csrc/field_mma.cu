@@ -369,6 +369,218 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const ui
     if (warp == 0) tc::tmem_dealloc<kTmemCols>(tmem);
 }
 
+
+// ---- software-pipelined variant for the interleaved tables ----------------------------------------------------------
+// Same decoders, same arithmetic. The difference is WHEN the gathers are issued: the grid look-ups of tile t+1 are
+// cut into three chunks that sit in the three windows where the warps of tile t would otherwise wait for their
+// tcgen05.mma to complete (commit -> mbarrier). The decoder chain of a tile is ~5 us of mostly latency; hidden this way
+// the kernel's time approaches that of the gathers alone.
+__global__ void __launch_bounds__(kThreads, 2)
+field_mma_pipe_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const uint2* __restrict__ both) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    __shared__ __align__(8) uint64_t mbar[2];
+    __shared__ uint32_t tmem_slot;
+    __shared__ float s_col[kTile][3];
+    __shared__ uint32_t s_exch[2][4][16][16];   // [field sent][warp & 3][level][row & 15]
+
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
+    const uint32_t chain = warp >> 2;                 // 0: geometry, 1: appearance
+    const uint32_t row = threadIdx.x & (kTile - 1);   // Gaussian within the tile == TMEM lane
+    for (uint32_t i = threadIdx.x; i < kPackedBytes / 16; i += kThreads)
+        reinterpret_cast<uint4*>(smem)[i] = __ldg(packed_w + i);
+    tc::fence_proxy_async_smem();
+    if (warp == 0) tc::tmem_alloc<kTmemCols>(&tmem_slot);
+    if (threadIdx.x == 32) {
+        tc::mbar_init(&mbar[0], 1);
+        tc::mbar_init(&mbar[1], 1);
+        tc::fence_mbar_init();
+    }
+    tc::fence_before_sync();
+    __syncthreads();
+    tc::fence_after_sync();
+    const uint32_t tmem = tmem_slot;
+    const uint32_t lane_base = ((warp & 3u) * 32u) << 16;
+    const uint32_t tD = tmem + (chain ? kColDa : kColDg);
+    const uint32_t tA = tmem + (chain ? kColAa : kColAg);
+    const uint32_t sb = tc::smem_u32(smem);
+    const uint32_t off1 = chain ? kOffA1 : kOffG1, off2 = chain ? kOffA2 : kOffG2, off3 = chain ? kOffA3 : kOffG3;
+    const uint32_t k1 = chain ? 64u : 32u;            // padded K of layer 1
+    constexpr uint32_t idesc64 = tc::idesc_f16_f32(128, 64), idesc16 = tc::idesc_f16_f32(128, 16);
+    uint64_t* bar = &mbar[chain];
+    uint32_t phase = 0;
+    const bool leader = row == 0;
+    const uint32_t V = A.counters->V;
+    // gather role of this lane: rows 16*chain .. 16*chain+15 of the quadrant, two lanes per Gaussian
+    const uint32_t xb = lane >> 4;
+    const bool own = xb == chain;
+    const int src = (int)((chain << 4) | (lane & 15u));
+    uint32_t(*exch_out)[16] = s_exch[chain][warp & 3u];
+    uint32_t(*exch_in)[16] = s_exch[chain ^ 1u][warp & 3u];
+
+    auto fetch = [&](uint32_t tile, Explicit& e, bool& v, float xs[3]) {
+        const uint32_t j = tile * kTile + row;
+        v = j < V;
+        float x[3] = {0.5f, 0.5f, 0.5f};
+        e = Explicit{};
+        if (v) {
+            e = fetch_visible(A, j);
+            hy_contract(A.f, e.px, e.py, e.pz, x);
+        }
+        xs[0] = __shfl_sync(0xffffffffu, x[0], src);
+        xs[1] = __shfl_sync(0xffffffffu, x[1], src);
+        xs[2] = __shfl_sync(0xffffffffu, x[2], src);
+    };
+#define HY_GATHER(L0, L1, XS, F)                                            \
+    _Pragma("unroll") for (int l = (L0); l < (L1); ++l) {                   \
+        uint32_t wg, wa;                                                    \
+        gather_level_pair2(A.geo, both, l, XS, xb, wg, wa);                 \
+        if (own) F[l] = chain ? wa : wg;                                    \
+        else exch_out[l][lane & 15u] = chain ? wg : wa;                     \
+    }
+    auto epilogue_to_A = [&]() {   // A <- relu(D) in fp16, 64 columns in two halves
+        uint32_t d[32], pk[16];
+        tc::ld_x32(tD + lane_base, d); tc::wait_ld();
+        relu_pack32(d, pk);
+        tc::st_x16(tA + lane_base, pk);
+        tc::ld_x32(tD + lane_base + 32, d); tc::wait_ld();
+        relu_pack32(d, pk);
+        tc::st_x16(tA + lane_base + 16, pk);
+        tc::wait_st();
+        tc::fence_before_sync();
+        asm volatile("bar.sync %0, 128;" ::"r"(1 + chain) : "memory");
+    };
+
+    uint32_t tile = blockIdx.x;
+    if (tile * kTile < V) {
+        Explicit ex;
+        bool valid;
+        float xs[3];
+        uint32_t f[16];
+        // prologue: the first tile's gathers are not hidden behind anything
+        fetch(tile, ex, valid, xs);
+        HY_GATHER(0, 16, xs, f)
+        __syncthreads();
+        if (!own) {
+#pragma unroll
+            for (int l = 0; l < 16; ++l) f[l] = exch_in[l][lane & 15u];
+        }
+        __syncthreads();
+        for (;;) {
+            const uint32_t next_tile = tile + gridDim.x;
+            const bool has_next = next_tile * kTile < V;
+            // ---- layer 1: A <- features (+ direction encoding), D = A W1^T ----
+            {
+                uint32_t a[16];
+#pragma unroll
+                for (int l = 0; l < 16; ++l) a[l] = valid ? f[l] : 0u;
+                tc::st_x16(tA + lane_base, a);
+                if (chain) {
+#pragma unroll
+                    for (int l = 0; l < 16; ++l) a[l] = 0u;
+                    if (valid) {
+                        const float dx = __fsub_rn(ex.px, A.f.o[0]), dy = __fsub_rn(ex.py, A.f.o[1]), dz = __fsub_rn(ex.pz, A.f.o[2]);
+                        const float n = __fsqrt_rn(__fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx))));
+                        const float d[3] = {__fdiv_rn(dx, n), __fdiv_rn(dy, n), __fdiv_rn(dz, n)};
+                        float pe[24];   // D4 by octave doubling (see field_mma_kernel)
+#pragma unroll
+                        for (int ax = 0; ax < 3; ++ax) {
+                            float sn, cs;
+                            sincospif(d[ax], &sn, &cs);
+                            pe[ax] = sn; pe[3 + ax] = cs;
+#pragma unroll
+                            for (int k = 1; k < 4; ++k) {
+                                const float s2 = 2.0f * sn * cs, c2 = 1.0f - 2.0f * sn * sn;
+                                sn = s2; cs = c2;
+                                pe[6 * k + ax] = sn; pe[6 * k + 3 + ax] = cs;
+                            }
+                        }
+#pragma unroll
+                        for (int i = 0; i < 12; ++i) a[i] = pack_h2(pe[2 * i], pe[2 * i + 1]);
+                    }
+                    tc::st_x16(tA + lane_base + 16, a);
+                }
+                tc::wait_st();
+                tc::fence_before_sync();
+                asm volatile("bar.sync %0, 128;" ::"r"(1 + chain) : "memory");
+            }
+            if (leader) {
+                tc::fence_after_sync();
+                for (uint32_t s = 0; s < k1 / 16; ++s)
+                    tc::mma_f16_ts(tD, tA + s * 8, tc::smem_desc_kmajor_noswizzle(sb + off1 + s * 256, 128, k1 * 16), idesc64, s);
+                tc::commit(bar);
+            }
+            // window 1: next tile's records, contraction, levels 0-5
+            Explicit exn{};
+            bool vn = false;
+            float xsn[3] = {0.5f, 0.5f, 0.5f};
+            uint32_t fn[16];
+#pragma unroll
+            for (int l = 0; l < 16; ++l) fn[l] = 0u;
+            if (has_next) {
+                fetch(next_tile, exn, vn, xsn);
+                HY_GATHER(0, 6, xsn, fn)
+            }
+            tc::mbar_wait(bar, phase); phase ^= 1;
+            tc::fence_after_sync();
+            // ---- layer 2 ----
+            epilogue_to_A();
+            if (leader) {
+                tc::fence_after_sync();
+                for (uint32_t s = 0; s < 4; ++s)
+                    tc::mma_f16_ts(tD, tA + s * 8, tc::smem_desc_kmajor_noswizzle(sb + off2 + s * 256, 128, 1024), idesc64, s);
+                tc::commit(bar);
+            }
+            if (has_next) { HY_GATHER(6, 11, xsn, fn) }   // window 2
+            tc::mbar_wait(bar, phase); phase ^= 1;
+            tc::fence_after_sync();
+            // ---- output layer ----
+            epilogue_to_A();
+            if (leader) {
+                tc::fence_after_sync();
+                for (uint32_t s = 0; s < 4; ++s)
+                    tc::mma_f16_ts(tD, tA + s * 8, tc::smem_desc_kmajor_noswizzle(sb + off3 + s * 256, 128, 1024), idesc16, s);
+                tc::commit(bar);
+            }
+            if (has_next) { HY_GATHER(11, 16, xsn, fn) }  // window 3
+            tc::mbar_wait(bar, phase); phase ^= 1;
+            tc::fence_after_sync();
+            float raw[11];
+            if (chain) {
+                uint32_t o[4];
+                tc::ld_x4(tD + lane_base, o); tc::wait_ld();
+                s_col[row][0] = __uint_as_float(o[0]); s_col[row][1] = __uint_as_float(o[1]); s_col[row][2] = __uint_as_float(o[2]);
+            } else {
+                uint32_t o[8];
+                tc::ld_x8(tD + lane_base, o); tc::wait_ld();
+#pragma unroll
+                for (int i = 0; i < 8; ++i) raw[i] = __uint_as_float(o[i]);
+            }
+            tc::fence_before_sync();
+            __syncthreads();
+            if (!chain && valid) {
+                raw[8] = s_col[row][0]; raw[9] = s_col[row][1]; raw[10] = s_col[row][2];
+                aggregate_project<true>(A, ex, raw);
+            }
+            if (has_next && !own) {
+#pragma unroll
+                for (int l = 0; l < 16; ++l) fn[l] = exch_in[l][lane & 15u];
+            }
+            __syncthreads();
+            tc::fence_after_sync();
+            if (!has_next) break;
+            tile = next_tile;
+            ex = exn;
+            valid = vn;
+#pragma unroll
+            for (int l = 0; l < 16; ++l) f[l] = fn[l];
+        }
+    }
+#undef HY_GATHER
+    tc::fence_before_sync();
+    __syncthreads();
+    if (warp == 0) tc::tmem_dealloc<kTmemCols>(tmem);
+}
+
 }  // namespace
 
 bool hy_field_mma_supported(const hyrf_scene_desc& d) {
@@ -402,12 +614,17 @@ hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* laun
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(field_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
         if (e != cudaSuccess) return hy_cuda_fail(e, "cudaFuncSetAttribute(field_mma)");
+        e = cudaFuncSetAttribute(field_mma_pipe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+        if (e != cudaSuccess) return hy_cuda_fail(e, "cudaFuncSetAttribute(field_mma_pipe)");
         attr_set = true;
     }
     const int need = (int)((s->N + kTile - 1) / kTile);
     const int grid = need < 148 * 2 ? need : 148 * 2;
-    field_mma_kernel<<<grid, kThreads, kSmemBytes, s->stream>>>(A, reinterpret_cast<const uint4*>(s->mma_w),
-                                                               reinterpret_cast<const uint2*>(s->both_table));
+    if (s->both_table)
+        field_mma_pipe_kernel<<<grid, kThreads, kSmemBytes, s->stream>>>(A, reinterpret_cast<const uint4*>(s->mma_w),
+                                                                        reinterpret_cast<const uint2*>(s->both_table));
+    else
+        field_mma_kernel<<<grid, kThreads, kSmemBytes, s->stream>>>(A, reinterpret_cast<const uint4*>(s->mma_w), nullptr);
     ++*launches;
     return HYRF_OK;
 }
