@@ -222,9 +222,17 @@ bin_prefix_kernel(const BinArgs A) {
     const uint32_t t = blockIdx.x * 32 + lane;
     const uint32_t per = (rows + 31) / 32;
     const uint32_t r0 = grp * per < rows ? grp * per : rows, r1 = r0 + per < rows ? r0 + per : rows;
+    // rows <= ~1024 -> at most 32 rows per group: kept in registers, all loads in flight at once
+    constexpr int kRows = 8;
     uint32_t sum = 0;
     if (t < A.T)
-        for (uint32_t r = r0; r < r1; ++r) sum += A.M[(size_t)r * A.T + t];
+        for (uint32_t rb = r0; rb < r1; rb += kRows) {
+            uint32_t v[kRows];
+#pragma unroll
+            for (int i = 0; i < kRows; ++i) v[i] = rb + i < r1 ? A.M[(size_t)(rb + i) * A.T + t] : 0u;
+#pragma unroll
+            for (int i = 0; i < kRows; ++i) sum += v[i];
+        }
     s_part[grp][lane] = sum;
     __syncthreads();
     uint32_t run = 0, total = 0;
@@ -235,11 +243,15 @@ bin_prefix_kernel(const BinArgs A) {
         total += v;
     }
     if (t < A.T) {
-        for (uint32_t r = r0; r < r1; ++r) {
-            uint32_t* p = A.M + (size_t)r * A.T + t;
-            const uint32_t v = *p;
-            *p = run;
-            run += v;
+        for (uint32_t rb = r0; rb < r1; rb += kRows) {
+            uint32_t v[kRows];
+#pragma unroll
+            for (int i = 0; i < kRows; ++i) v[i] = rb + i < r1 ? A.M[(size_t)(rb + i) * A.T + t] : 0u;
+#pragma unroll
+            for (int i = 0; i < kRows; ++i) {
+                if (rb + i < r1) A.M[(size_t)(rb + i) * A.T + t] = run;
+                run += v[i];
+            }
         }
         if (grp == 0) A.totals[t] = total;
     }
