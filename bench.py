@@ -114,8 +114,11 @@ def workload(cfg: int, args):
     if args.width and args.height:
         kw["width"], kw["height"] = args.width, args.height
     scene = synth.make_scene(cfg, **kw)
+    if args.quant8:
+        scene = synth.quantize8(scene)
     cam = scene.cameras[0]
-    name = (f"BASELINE.json configs[{cfg - 1}]: {scene.n} Gaussians, {'fp16' if scene.fp16 else 'fp32'} grids/MLPs, "
+    name = (f"BASELINE.json configs[{cfg - 1}]: {scene.n} Gaussians, "
+            f"{'8-bit tables + fp16 MLPs (compressed model)' if scene.quant8 else ('fp16' if scene.fp16 else 'fp32') + ' grids/MLPs'}, "
             f"{cam.W}x{cam.H}, {len(scene.cameras)} cameras")
     return scene, name
 
@@ -123,7 +126,7 @@ def workload(cfg: int, args):
 # Algorithmic work per unit. Bytes are ALGORITHMIC: what the stage has to move if
 # every operand is read once and every result written once, not what the caches happened to move.
 def stage_rooflines(scene, V, D, n_bg, eval_pairs, peaks):
-    esz = 2 if scene.fp16 else 4
+    esz = 1 if scene.quant8 else (2 if scene.fp16 else 4)
     gathers = (scene.geo_grid.levels + scene.app_grid.levels) * 8
     hbm = peaks["hbm_gbs"]
     # S2+S3+S4a: per visible Gaussian 256 gathers of one (2-feature) entry + 32 B explicit record + 4 B work index in;
@@ -393,6 +396,8 @@ def main():
     ap.add_argument("--height", type=int, default=0)
     ap.add_argument("--ablation", type=int, default=0,
                     help="hyrf_ablation bits (PAPER.md Table 5): 1 no pre-culling, 2 no background, 4 no neural, 8 no explicit")
+    ap.add_argument("--quant8", action="store_true",
+                    help="compressed model: 8-bit min-max tables decoded in the gather (PAPER.md:229)")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()

@@ -42,7 +42,10 @@ typedef enum {
     HYRF_ERR_CUDA = 6         /* any CUDA runtime failure, incl. no device */
 } hyrf_status;
 
-typedef enum { HYRF_F32 = 0, HYRF_F16 = 1 } hyrf_dtype; /* dtype of grid tables and MLP weights */
+/* dtype of grid tables and MLP weights. HYRF_U8 is the compressed model of PAPER.md:227-229 (3): tables are 8-bit
+ * min-max codes [entry][2] with value = fma(code, step, min) per level and feature (hyrf_params *_q), decoder
+ * weights are fp16 and the decoded feature is rounded to fp16 as with HYRF_F16 (DESIGN.md §2 D3'). */
+typedef enum { HYRF_F32 = 0, HYRF_F16 = 1, HYRF_U8 = 2 } hyrf_dtype;
 
 /* How the MLP decoders are evaluated.
  *  FMA: CUDA-core fp32 fma in the oracle's order — geometry decisions bit-reproducible (any param_dtype).
@@ -92,6 +95,7 @@ typedef struct {
     const float* opacity_logit; /* [N]    — alpha_e (pre-sigmoid) */
     const void *geo_table, *app_table, *bg_table; /* levels concatenated, [entry][2], param_dtype */
     const void *geo_w, *app_w, *bg_w;             /* layers concatenated, each row-major [out][in] */
+    const float *geo_q, *app_q, *bg_q;            /* HYRF_U8 only: [levels][2 features][2] = (min, step); else NULL */
     int32_t host_ptrs;                            /* 0: device pointers, else host pointers */
 } hyrf_params;
 

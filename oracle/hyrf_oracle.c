@@ -50,6 +50,10 @@ typedef struct {
     int32_t fp16;
     uint32_t pe_octaves;
     float cull_tol, z_near, bg_radius, tau_T;
+    /* compressed model (item 3): tables stored as 8-bit codes with per-level, per-feature
+     * (min, step); q[(level * feats + f) * 2 + {0, 1}]. table_u8 != 0 implies fp16 weights / activations. */
+    int32_t table_u8;
+    const float *geo_q, *app_q, *bg_q;
 } ho_scene;
 
 /* ------------------------------------------------------------------------------------------------ */
@@ -209,13 +213,21 @@ uint32_t ho_grid_index(const ho_grid *g, uint32_t level, uint32_t vx, uint32_t v
     return h & (uint32_t)(T - 1ull);
 }
 
-static inline float table_value(const void *table, int fp16, uint64_t entry, uint32_t f, uint32_t feats) {
-    if (fp16) return ho_half_to_float(((const uint16_t *)table)[entry * feats + f]);
+/* mode 0: fp32 entries; 1: fp16 entries (exact in fp32); 2: 8-bit min-max codes, value = fma(code, step, min)
+ * with the (min, step) of this level and feature (DESIGN.md §2 D3', "8-bit min-max quantization"). */
+static inline float table_value(const void *table, int mode, const float *q, uint32_t level, uint64_t entry, uint32_t f,
+                                uint32_t feats) {
+    if (mode == 2) {
+        const float *qp = q + ((size_t)level * feats + f) * 2;
+        return fmaf((float)((const uint8_t *)table)[entry * feats + f], qp[1], qp[0]);
+    }
+    if (mode == 1) return ho_half_to_float(((const uint16_t *)table)[entry * feats + f]);
     return ((const float *)table)[entry * feats + f];
 }
 
 /* D3 encode: PAPER.md:61, :74 Eq. 3, :152. x in [0,1]^3 -> feat[levels*feats], level-major. */
-void ho_grid_encode(const ho_grid *g, const void *table, int32_t fp16, const float x[3], float *feat) {
+void ho_grid_encode_q(const ho_grid *g, const void *table, int32_t mode, const float *q, const float x[3], float *feat) {
+    const int fp16 = mode != 0;   /* fp16 and 8-bit tables both feed fp16 decoders: the feature is rounded to fp16 */
     uint32_t offsets[HO_MAX_LEVELS];
     ho_grid_layout(g, NULL, offsets, NULL);
     for (uint32_t l = 0; l < g->levels; ++l) {
@@ -238,12 +250,16 @@ void ho_grid_encode(const ho_grid *g, const void *table, int32_t fp16, const flo
                 float az = bz ? w[2] : 1.0f - w[2];
                 float wt = (ax * ay) * az;
                 uint32_t e = ho_grid_index(g, l, ci[0] + bx, ci[1] + by, ci[2] + bz);
-                float val = table_value(table, fp16, (uint64_t)offsets[l] + e, f, g->feats);
+                float val = table_value(table, mode, q, l, (uint64_t)offsets[l] + e, f, g->feats);
                 acc = fmaf(wt, val, acc);
             }
             feat[l * g->feats + f] = fp16 ? round_h(acc) : acc;
         }
     }
+}
+
+void ho_grid_encode(const ho_grid *g, const void *table, int32_t fp16, const float x[3], float *feat) {
+    ho_grid_encode_q(g, table, fp16 ? 1 : 0, NULL, x, feat);
 }
 
 /* D4: unit view direction from camera centre o to p (Eq. 5). */
@@ -301,11 +317,11 @@ void ho_query_point(const ho_scene *s, const float p[3], const float o[3], float
     ho_contract(p, s->aabb_min, s->aabb_max, x);
     /* geometry field: Eq. 3, 4 */
     memset(in, 0, sizeof(in));
-    ho_grid_encode(&s->geo_grid, s->geo_table, s->fp16, x, in);
+    ho_grid_encode_q(&s->geo_grid, s->geo_table, s->table_u8 ? 2 : s->fp16, s->geo_q, x, in);
     ho_mlp_forward(&s->geo_mlp, s->geo_w, s->fp16, in, raw);
     /* appearance field: Eq. 3, 5, 6 */
     memset(in, 0, sizeof(in));
-    ho_grid_encode(&s->app_grid, s->app_table, s->fp16, x, in);
+    ho_grid_encode_q(&s->app_grid, s->app_table, s->table_u8 ? 2 : s->fp16, s->app_q, x, in);
     ho_view_dir(p, o, d);
     ho_dir_pe(d, s->pe_octaves, s->fp16, in + s->app_grid.levels * s->app_grid.feats);
     ho_mlp_forward(&s->app_mlp, s->app_w, s->fp16, in, raw + 8);
@@ -553,7 +569,7 @@ void ho_background_color(const ho_scene *s, const ho_camera *cam, float i, float
     ho_ray_sphere(cam, i, j, s->bg_radius, d, ps);
     ho_contract(ps, s->aabb_min, s->aabb_max, x);
     memset(in, 0, sizeof(in));
-    ho_grid_encode(&s->bg_grid, s->bg_table, s->fp16, x, in);
+    ho_grid_encode_q(&s->bg_grid, s->bg_table, s->table_u8 ? 2 : s->fp16, s->bg_q, x, in);
     ho_dir_pe(d, s->pe_octaves, s->fp16, in + s->bg_grid.levels * s->bg_grid.feats);
     ho_mlp_forward(&s->bg_mlp, s->bg_w, s->fp16, in, raw);
     for (int k = 0; k < 3; ++k) cs[k] = ho_sigmoid(raw[k]);

@@ -42,7 +42,8 @@ class HoScene(C.Structure):
                 ("geo_table", C.c_void_p), ("app_table", C.c_void_p), ("bg_table", C.c_void_p),
                 ("geo_w", C.c_void_p), ("app_w", C.c_void_p), ("bg_w", C.c_void_p),
                 ("fp16", C.c_int32), ("pe_octaves", C.c_uint32),
-                ("cull_tol", C.c_float), ("z_near", C.c_float), ("bg_radius", C.c_float), ("tau_T", C.c_float)]
+                ("cull_tol", C.c_float), ("z_near", C.c_float), ("bg_radius", C.c_float), ("tau_T", C.c_float),
+                ("table_u8", C.c_int32), ("geo_q", C.c_void_p), ("app_q", C.c_void_p), ("bg_q", C.c_void_p)]
 
 
 def _cpu_has_fma() -> bool:
@@ -146,12 +147,18 @@ class OracleScene:
     def __init__(self, scene):
         self.src = scene
         self.fp16 = bool(scene.fp16)
-        tdt = np.float16 if self.fp16 else np.float32
+        self.u8 = bool(getattr(scene, "quant8", False))    # 8-bit min-max tables; decoders stay fp16
+        if self.u8 and not self.fp16:
+            raise ValueError("8-bit tables go with fp16 decoder weights")
+        wdt = np.float16 if self.fp16 else np.float32
+        tdt = np.uint8 if self.u8 else wdt
         self._keep = dict(
             pos=_f32(scene.pos), rgb=_f32(scene.rgb_logit), sc=_f32(scene.scale_logit), op=_f32(scene.opacity_logit),
             gt=np.ascontiguousarray(scene.geo_table, dtype=tdt), at=np.ascontiguousarray(scene.app_table, dtype=tdt),
-            bt=np.ascontiguousarray(scene.bg_table, dtype=tdt), gw=np.ascontiguousarray(scene.geo_w, dtype=tdt),
-            aw=np.ascontiguousarray(scene.app_w, dtype=tdt), bw=np.ascontiguousarray(scene.bg_w, dtype=tdt))
+            bt=np.ascontiguousarray(scene.bg_table, dtype=tdt), gw=np.ascontiguousarray(scene.geo_w, dtype=wdt),
+            aw=np.ascontiguousarray(scene.app_w, dtype=wdt), bw=np.ascontiguousarray(scene.bg_w, dtype=wdt))
+        if self.u8:
+            self._keep.update(gq=_f32(scene.geo_q), aq=_f32(scene.app_q), bq=_f32(scene.bg_q))
         k = self._keep
         s = HoScene()
         s.n = int(scene.n)
@@ -169,6 +176,9 @@ class OracleScene:
         s.pe_octaves = int(scene.dir_pe_octaves)
         s.cull_tol, s.z_near, s.bg_radius, s.tau_T = (float(scene.cull_tol), float(scene.z_near),
                                                       float(scene.bg_radius), float(scene.tau_T))
+        s.table_u8 = int(self.u8)
+        if self.u8:
+            s.geo_q, s.app_q, s.bg_q = _p(k["gq"]), _p(k["aq"]), _p(k["bq"])
         self.c = s
         self.n = int(scene.n)
 
@@ -226,10 +236,15 @@ def grid_index(grid, level: int, vx: int, vy: int, vz: int) -> int:
     return int(lib().ho_grid_index(C.cast(C.byref(g), C.c_void_p), level, vx, vy, vz))
 
 
-def grid_encode(grid, table: np.ndarray, x, fp16: bool = False) -> np.ndarray:
+def grid_encode(grid, table: np.ndarray, x, fp16: bool = False, q: Optional[np.ndarray] = None) -> np.ndarray:
+    """q given: `table` holds 8-bit codes, q[level][feature] = (min, step)."""
     g = grid_struct(grid)
-    tab = np.ascontiguousarray(table, dtype=np.float16 if fp16 else np.float32)
     feat = np.zeros(g.levels * g.feats, np.float32)
+    if q is not None:
+        tab = np.ascontiguousarray(table, dtype=np.uint8)
+        lib().ho_grid_encode_q(C.byref(g), _p(tab), C.c_int32(2), _p(_f32(q)), _p(_f32(x)), _p(feat))
+        return feat
+    tab = np.ascontiguousarray(table, dtype=np.float16 if fp16 else np.float32)
     lib().ho_grid_encode(C.byref(g), _p(tab), C.c_int32(int(fp16)), _p(_f32(x)), _p(feat))
     return feat
 

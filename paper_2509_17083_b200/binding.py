@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libhyrf.so")
 HYRF_OK, HYRF_ERR_INVALID_ARG, HYRF_ERR_NOT_READY, HYRF_ERR_UNSUPPORTED, HYRF_ERR_CAMERA, HYRF_ERR_OOM, HYRF_ERR_CUDA = range(7)
 STATUS_NAMES = ["HYRF_OK", "HYRF_ERR_INVALID_ARG", "HYRF_ERR_NOT_READY", "HYRF_ERR_UNSUPPORTED", "HYRF_ERR_CAMERA",
                 "HYRF_ERR_OOM", "HYRF_ERR_CUDA"]
-HYRF_F32, HYRF_F16 = 0, 1
+HYRF_F32, HYRF_F16, HYRF_U8 = 0, 1, 2
 HYRF_MLP_AUTO, HYRF_MLP_FMA, HYRF_MLP_MMA = 0, 1, 2
 (DBG_VIS_MASK, DBG_VIS_IDX, DBG_STAGE2_RAW, DBG_STAGE3_ATTRS, DBG_PROJ, DBG_RECT, DBG_TILE_RANGES, DBG_TILE_LIST,
  DBG_FINAL_T, DBG_BG_MASK, DBG_COUNTERS, DBG_FG) = range(12)
@@ -58,6 +58,7 @@ class Params(C.Structure):
     _fields_ = [("pos", C.c_void_p), ("rgb_logit", C.c_void_p), ("scale_logit", C.c_void_p),
                 ("opacity_logit", C.c_void_p), ("geo_table", C.c_void_p), ("app_table", C.c_void_p),
                 ("bg_table", C.c_void_p), ("geo_w", C.c_void_p), ("app_w", C.c_void_p), ("bg_w", C.c_void_p),
+                ("geo_q", C.c_void_p), ("app_q", C.c_void_p), ("bg_q", C.c_void_p),
                 ("host_ptrs", C.c_int32)]
 
 
@@ -148,7 +149,7 @@ def make_desc(scene, max_width: int, max_height: int, device: int = 0, mlp_path:
         m = getattr(scene, name)
         setattr(d, name, MlpDesc(m.in_dim, m.hidden, m.n_hidden, m.out_dim))
     d.dir_pe_octaves = int(scene.dir_pe_octaves)
-    d.param_dtype = HYRF_F16 if scene.fp16 else HYRF_F32
+    d.param_dtype = HYRF_U8 if getattr(scene, "quant8", False) else (HYRF_F16 if scene.fp16 else HYRF_F32)
     d.mlp_path = int(mlp_path)
     d.cull_tol, d.z_near, d.bg_radius, d.tau_T = (float(scene.cull_tol), float(scene.z_near),
                                                   float(scene.bg_radius), float(scene.tau_T))
@@ -191,13 +192,18 @@ class HyrfScene:
     # -- hyrf_upload_params -------------------------------------------------------------------------------
     def upload(self, scene, host_upload: bool = False) -> None:
         torch = self._torch
-        tdt = np.float16 if self.fp16 else np.float32
+        wdt = np.float16 if self.fp16 else np.float32
+        u8 = bool(getattr(scene, "quant8", False))
+        tdt = np.uint8 if u8 else wdt                  # HYRF_U8: 8-bit codes + (min, step) per level and feature
         host = dict(pos=np.ascontiguousarray(scene.pos, np.float32), rgb_logit=np.ascontiguousarray(scene.rgb_logit, np.float32),
                     scale_logit=np.ascontiguousarray(scene.scale_logit, np.float32),
                     opacity_logit=np.ascontiguousarray(scene.opacity_logit, np.float32),
                     geo_table=np.ascontiguousarray(scene.geo_table, tdt), app_table=np.ascontiguousarray(scene.app_table, tdt),
-                    bg_table=np.ascontiguousarray(scene.bg_table, tdt), geo_w=np.ascontiguousarray(scene.geo_w, tdt),
-                    app_w=np.ascontiguousarray(scene.app_w, tdt), bg_w=np.ascontiguousarray(scene.bg_w, tdt))
+                    bg_table=np.ascontiguousarray(scene.bg_table, tdt), geo_w=np.ascontiguousarray(scene.geo_w, wdt),
+                    app_w=np.ascontiguousarray(scene.app_w, wdt), bg_w=np.ascontiguousarray(scene.bg_w, wdt))
+        if u8:
+            host.update(geo_q=np.ascontiguousarray(scene.geo_q, np.float32), app_q=np.ascontiguousarray(scene.app_q, np.float32),
+                        bg_q=np.ascontiguousarray(scene.bg_q, np.float32))
         p = Params()
         if host_upload:
             for k, a in host.items():

@@ -185,7 +185,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     for (int a = 0; a < 3; ++a)
         if (!(desc->aabb_max[a] > desc->aabb_min[a]) || !isfinite(desc->aabb_min[a]) || !isfinite(desc->aabb_max[a]))
             return hy_fail(HYRF_ERR_INVALID_ARG, "aabb axis %d is empty or non-finite", a);
-    if (desc->param_dtype != HYRF_F32 && desc->param_dtype != HYRF_F16)
+    if (desc->param_dtype != HYRF_F32 && desc->param_dtype != HYRF_F16 && desc->param_dtype != HYRF_U8)
         return hy_fail(HYRF_ERR_INVALID_ARG, "unknown param_dtype %d", (int)desc->param_dtype);
     if (!(desc->bg_radius > 0.0f) || !isfinite(desc->cull_tol) || desc->cull_tol < 0.0f || !isfinite(desc->z_near) ||
         !isfinite(desc->tau_T))
@@ -226,7 +226,8 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     s->desc.app_grid.level_res = s->res_app.data();
     s->desc.bg_grid.level_res = s->res_bg.data();
     s->N = desc->n_gaussians;
-    s->fp16 = desc->param_dtype == HYRF_F16;
+    s->fp16 = desc->param_dtype != HYRF_F32;
+    s->u8 = desc->param_dtype == HYRF_U8;
     s->use_mma = desc->mlp_path != HYRF_MLP_FMA && hy_field_mma_supported(*desc);
     s->geo_entries = build_grid(s->desc.geo_grid, &s->geo_grid);
     s->app_entries = build_grid(s->desc.app_grid, &s->app_grid);
@@ -236,7 +237,8 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     s->bg_mlp = MlpDev{nullptr, desc->bg_mlp.in_dim, desc->bg_mlp.hidden, desc->bg_mlp.n_hidden, 3};
 
     const size_t N = s->N;
-    const size_t esz = s->fp16 ? 2 : 4;
+    const size_t esz = s->fp16 ? 2 : 4;          // decoder weights
+    const size_t tsz = s->u8 ? 1 : esz;          // table features
     const size_t P = (size_t)desc->max_width * desc->max_height;
     const size_t tiles = (size_t)((desc->max_width + HY_TILE - 1) / HY_TILE) * ((desc->max_height + HY_TILE - 1) / HY_TILE);
     const size_t cull_blocks = (N + 1023) / 1024;
@@ -246,9 +248,9 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc_t(s, &s->rgb, 3 * N));
     HY_TRY(dev_alloc_t(s, &s->scale, N));
     HY_TRY(dev_alloc_t(s, &s->opac, N));
-    HY_TRY(dev_alloc(s, &tg, s->geo_entries * 2 * esz)); s->geo_grid.table = tg;
-    HY_TRY(dev_alloc(s, &ta, s->app_entries * 2 * esz)); s->app_grid.table = ta;
-    HY_TRY(dev_alloc(s, &tb, s->bg_entries * 2 * esz)); s->bg_grid.table = tb;
+    HY_TRY(dev_alloc(s, &tg, s->geo_entries * 2 * tsz)); s->geo_grid.table = tg;
+    HY_TRY(dev_alloc(s, &ta, s->app_entries * 2 * tsz)); s->app_grid.table = ta;
+    HY_TRY(dev_alloc(s, &tb, s->bg_entries * 2 * tsz)); s->bg_grid.table = tb;
     HY_TRY(dev_alloc(s, &wg, mlp_weights(s->desc.geo_mlp) * esz)); s->geo_mlp.w = wg;
     HY_TRY(dev_alloc(s, &wa, mlp_weights(s->desc.app_mlp) * esz)); s->app_mlp.w = wa;
     HY_TRY(dev_alloc(s, &wb, mlp_weights(s->desc.bg_mlp) * esz)); s->bg_mlp.w = wb;
@@ -257,7 +259,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
         const hyrf_grid_desc &g = s->desc.geo_grid, &a = s->desc.app_grid;
         bool same = g.levels == a.levels && g.log2_table == a.log2_table;
         for (uint32_t l = 0; same && l < g.levels; ++l) same = g.level_res[l] == a.level_res[l];
-        if (s->use_mma && same) HY_TRY(dev_alloc(s, &s->both_table, s->geo_entries * 8));
+        if (s->use_mma && same) HY_TRY(dev_alloc(s, &s->both_table, s->geo_entries * 4 * tsz));
     }
     HY_TRY(dev_alloc_t(s, &s->gm, 2 * N));
     HY_TRY(dev_alloc_t(s, &s->gm_id, N));
@@ -310,13 +312,28 @@ extern "C" hyrf_status hyrf_upload_params(hyrf_scene* s, const hyrf_params* p) {
     cudaError_t e;
     if ((e = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
     const cudaMemcpyKind kind = p->host_ptrs ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
-    const size_t N = s->N, esz = s->fp16 ? 2 : 4;
+    const size_t N = s->N, esz = s->fp16 ? 2 : 4, tsz = s->u8 ? 1 : esz;
+    if (s->u8) {   // (min, step) per level and feature travel with the kernel arguments
+        if (!p->geo_q || !p->app_q || !p->bg_q) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_upload_params: HYRF_U8 needs geo_q, app_q, bg_q");
+        struct { GridDev* g; const float* q; } qs[3] = {{&s->geo_grid, p->geo_q}, {&s->app_grid, p->app_q}, {&s->bg_grid, p->bg_q}};
+        for (auto& x : qs) {
+            float host[HY_MAX_LEVELS * 4];
+            const size_t bytes = (size_t)x.g->levels * 4 * sizeof(float);
+            if (p->host_ptrs) memcpy(host, x.q, bytes);
+            else if ((e = cudaMemcpy(host, x.q, bytes, cudaMemcpyDeviceToHost)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpy(q)");
+            for (uint32_t l = 0; l < x.g->levels; ++l)
+                for (int f = 0; f < 2; ++f) {
+                    if (!isfinite(host[(l * 2 + f) * 2]) || !isfinite(host[(l * 2 + f) * 2 + 1])) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_upload_params: non-finite quantisation parameter");
+                    x.g->q[l][f] = make_float2(host[(l * 2 + f) * 2], host[(l * 2 + f) * 2 + 1]);
+                }
+        }
+    }
     struct { void* dst; const void* src; size_t bytes; } copies[] = {
         {s->pos, p->pos, 3 * N * 4}, {s->rgb, p->rgb_logit, 3 * N * 4}, {s->scale, p->scale_logit, N * 4},
         {s->opac, p->opacity_logit, N * 4},
-        {(void*)s->geo_grid.table, p->geo_table, s->geo_entries * 2 * esz},
-        {(void*)s->app_grid.table, p->app_table, s->app_entries * 2 * esz},
-        {(void*)s->bg_grid.table, p->bg_table, s->bg_entries * 2 * esz},
+        {(void*)s->geo_grid.table, p->geo_table, s->geo_entries * 2 * tsz},
+        {(void*)s->app_grid.table, p->app_table, s->app_entries * 2 * tsz},
+        {(void*)s->bg_grid.table, p->bg_table, s->bg_entries * 2 * tsz},
         {(void*)s->geo_mlp.w, p->geo_w, mlp_weights(s->desc.geo_mlp) * esz},
         {(void*)s->app_mlp.w, p->app_w, mlp_weights(s->desc.app_mlp) * esz},
         {(void*)s->bg_mlp.w, p->bg_w, mlp_weights(s->desc.bg_mlp) * esz}};

@@ -20,10 +20,11 @@ struct BgArgs {
     const FrameCounters* counters;
 };
 
-template <int CL, int CHID, int CNH, bool FP16>
+template <int CL, int CHID, int CNH, int DT>   // DT: HY_DT_F32 / HY_DT_F16 / HY_DT_U8 (8-bit tables, fp16 decoders)
 __global__ void __launch_bounds__(kBgThreads)
 background_kernel(const BgArgs A) {
     extern __shared__ __align__(16) float smem_w[];
+    constexpr bool FP16 = DT != HY_DT_F32;
     const int L = CL > 0 ? CL : (int)A.grid.levels;
     const int in_dim = (int)A.mlp.in_dim, hid = (int)A.mlp.hidden, nh = (int)A.mlp.n_hidden;
     const int nw = in_dim * hid + (nh - 1) * hid * hid + hid * 3;
@@ -62,7 +63,7 @@ background_kernel(const BgArgs A) {
 #pragma unroll
         for (int l = 0; l < L; ++l) {
             float f0, f1;
-            hy_grid_level<FP16>(A.grid, l, x, f0, f1);
+            hy_grid_level<DT>(A.grid, l, x, f0, f1);
             bufa[2 * l] = FP16 ? hy_round_half(f0) : f0;
             bufa[2 * l + 1] = FP16 ? hy_round_half(f1) : f1;
         }
@@ -80,9 +81,9 @@ background_kernel(const BgArgs A) {
     }
 }
 
-template <int CL, int CHID, int CNH, bool FP16>
+template <int CL, int CHID, int CNH, int DT>
 hyrf_status launch_one(const BgArgs& A, size_t smem, int grid, cudaStream_t st) {
-    auto k = background_kernel<CL, CHID, CNH, FP16>;
+    auto k = background_kernel<CL, CHID, CNH, DT>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return hy_cuda_fail(e, "cudaFuncSetAttribute(background)");
     k<<<grid, kBgThreads, smem, st>>>(A);
@@ -105,12 +106,18 @@ hyrf_status hy_launch_background(hyrf_scene* s, const FrameDev& f, float* out_rg
     const uint32_t L = s->desc.bg_grid.levels;
     const bool std_in = m.in_dim == 2 * L + 24 && s->desc.dir_pe_octaves == 4 && m.n_hidden == 1;
     hyrf_status st;
+    const int dt = s->u8 ? HY_DT_U8 : (s->fp16 ? HY_DT_F16 : HY_DT_F32);
+#define HY_DISPATCH(CL, CH, CN)                                                                   \
+    (dt == HY_DT_U8 ? launch_one<CL, CH, CN, HY_DT_U8>(A, smem, grid, s->stream)                     \
+                    : dt == HY_DT_F16 ? launch_one<CL, CH, CN, HY_DT_F16>(A, smem, grid, s->stream)  \
+                                      : launch_one<CL, CH, CN, HY_DT_F32>(A, smem, grid, s->stream))
     if (std_in && L == 8 && m.hidden == 64)
-        st = s->fp16 ? launch_one<8, 64, 1, true>(A, smem, grid, s->stream) : launch_one<8, 64, 1, false>(A, smem, grid, s->stream);
-    else if (std_in && L == 4 && m.hidden == 32)
-        st = s->fp16 ? launch_one<4, 32, 1, true>(A, smem, grid, s->stream) : launch_one<4, 32, 1, false>(A, smem, grid, s->stream);
+        st = HY_DISPATCH(8, 64, 1);
+    else if (std_in && L == 4 && m.hidden == 32 && dt != HY_DT_U8)
+        st = s->fp16 ? launch_one<4, 32, 1, HY_DT_F16>(A, smem, grid, s->stream) : launch_one<4, 32, 1, HY_DT_F32>(A, smem, grid, s->stream);
     else
-        st = s->fp16 ? launch_one<0, 0, 0, true>(A, smem, grid, s->stream) : launch_one<0, 0, 0, false>(A, smem, grid, s->stream);
+        st = HY_DISPATCH(0, 0, 0);
+#undef HY_DISPATCH
     if (st == HYRF_OK) ++*launches;
     return st;
 }

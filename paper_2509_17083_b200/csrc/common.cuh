@@ -12,12 +12,13 @@
 
 // One multi-resolution grid as the kernels see it (DESIGN.md §2 D3).
 struct GridDev {
-    const void* table;               // [entries][2], float2 or __half2
+    const void* table;               // [entries][2], float2, __half2 or uchar2 (8-bit min-max codes)
     uint32_t levels;
     uint32_t table_mask;             // T - 1
     uint32_t dense_mask;             // bit l set: level l is dense
     uint32_t res[HY_MAX_LEVELS];     // N_l
     uint32_t offset[HY_MAX_LEVELS];  // first entry of level l
+    float2 q[HY_MAX_LEVELS][2];      // 8-bit tables only: (min, step) of level l, feature f (DESIGN.md §2 D3')
 };
 
 // Camera plus the per-frame constants derived from it on the host (DESIGN.md §2 "Camera", D1).
@@ -82,8 +83,13 @@ __device__ __forceinline__ void hy_contract(const FrameDev& f, float px, float p
     x[2] = fminf(fmaxf(__fmaf_rn(0.25f, q2, 0.5f), 0.0f), 1.0f);
 }
 
+// Table entry types: DT 0 = fp32, 1 = fp16, 2 = 8-bit min-max codes (decoders fp16).
+#define HY_DT_F32 0
+#define HY_DT_F16 1
+#define HY_DT_U8 2
+
 // D3: one level of one grid at contracted position x -> two features (fp32, not yet rounded to half).
-template <bool FP16>
+template <int DT>
 __device__ __forceinline__ void hy_grid_level(const GridDev& g, uint32_t l, const float x[3], float& f0, float& f1) {
     const uint32_t N = g.res[l];
     const float Nf = (float)N;
@@ -108,7 +114,16 @@ __device__ __forceinline__ void hy_grid_level(const GridDev& g, uint32_t l, cons
         idx[k] = g.offset[l] + e;
     }
     float v0[8], v1[8];
-    if (FP16) {
+    if (DT == HY_DT_U8) {   // D3': value = fma(code, step, min)
+        const uchar2* tab = reinterpret_cast<const uchar2*>(g.table);
+        const float2 q0 = g.q[l][0], q1 = g.q[l][1];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const uchar2 c = __ldg(tab + idx[k]);
+            v0[k] = __fmaf_rn((float)c.x, q0.y, q0.x);
+            v1[k] = __fmaf_rn((float)c.y, q1.y, q1.x);
+        }
+    } else if (DT == HY_DT_F16) {
         const __half2* tab = reinterpret_cast<const __half2*>(g.table);
 #pragma unroll
         for (int k = 0; k < 8; ++k) {

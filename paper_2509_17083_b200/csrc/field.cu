@@ -14,10 +14,11 @@ namespace {
 constexpr int kFieldThreads = 128;
 
 // CL: levels of both grids (0 = run-time), CHID / CNH: hidden width / count (0 = run-time).
-template <int CL, int CHID, int CNH, bool FP16>
+template <int CL, int CHID, int CNH, int DT>   // DT: HY_DT_F32 / HY_DT_F16 / HY_DT_U8 (8-bit tables, fp16 decoders)
 __global__ void __launch_bounds__(kFieldThreads)
 field_fma_kernel(const FieldArgs A) {
     extern __shared__ __align__(16) float smem_w[];
+    constexpr bool FP16 = DT != HY_DT_F32;
     const int Lg = CL > 0 ? CL : (int)A.geo.levels;
     const int La = CL > 0 ? CL : (int)A.app.levels;
     const int geo_in = (int)A.geo_mlp.in_dim, app_in = (int)A.app_mlp.in_dim;
@@ -57,7 +58,7 @@ field_fma_kernel(const FieldArgs A) {
 #pragma unroll
         for (int l = 0; l < Lg; ++l) {
             float f0, f1;
-            hy_grid_level<FP16>(A.geo, l, x, f0, f1);
+            hy_grid_level<DT>(A.geo, l, x, f0, f1);
             bufa[2 * l] = FP16 ? hy_round_half(f0) : f0;
             bufa[2 * l + 1] = FP16 ? hy_round_half(f1) : f1;
         }
@@ -71,7 +72,7 @@ field_fma_kernel(const FieldArgs A) {
 #pragma unroll
         for (int l = 0; l < La; ++l) {
             float f0, f1;
-            hy_grid_level<FP16>(A.app, l, x, f0, f1);
+            hy_grid_level<DT>(A.app, l, x, f0, f1);
             bufa[2 * l] = FP16 ? hy_round_half(f0) : f0;
             bufa[2 * l + 1] = FP16 ? hy_round_half(f1) : f1;
         }
@@ -92,9 +93,9 @@ field_fma_kernel(const FieldArgs A) {
     }
 }
 
-template <int CL, int CHID, int CNH, bool FP16>
+template <int CL, int CHID, int CNH, int DT>
 hyrf_status launch_one(const FieldArgs& A, size_t smem, int grid, cudaStream_t st) {
-    auto k = field_fma_kernel<CL, CHID, CNH, FP16>;
+    auto k = field_fma_kernel<CL, CHID, CNH, DT>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return hy_cuda_fail(e, "cudaFuncSetAttribute(field)");
     k<<<grid, kFieldThreads, smem, st>>>(A);
@@ -129,16 +130,20 @@ hyrf_status hy_launch_field_fma(hyrf_scene* s, const FrameDev& f, uint32_t* laun
     const bool same = s->desc.app_grid.levels == L && g.hidden == a.hidden && g.n_hidden == a.n_hidden &&
                       g.in_dim == 2 * L && a.in_dim == 2 * L + 24 && s->desc.dir_pe_octaves == 4;
     hyrf_status st;
+    const int dt = s->u8 ? HY_DT_U8 : (s->fp16 ? HY_DT_F16 : HY_DT_F32);
+#define HY_DISPATCH(CL, CH, CN)                                                                   \
+    (dt == HY_DT_U8 ? launch_one<CL, CH, CN, HY_DT_U8>(A, smem, grid, s->stream)                     \
+                    : dt == HY_DT_F16 ? launch_one<CL, CH, CN, HY_DT_F16>(A, smem, grid, s->stream)  \
+                                      : launch_one<CL, CH, CN, HY_DT_F32>(A, smem, grid, s->stream))
     if (same && L == 16 && g.hidden == 64 && g.n_hidden == 2) {
-        st = s->fp16 ? launch_one<16, 64, 2, true>(A, smem, grid, s->stream)
-                     : launch_one<16, 64, 2, false>(A, smem, grid, s->stream);
-    } else if (same && L == 8 && g.hidden == 32 && g.n_hidden == 1) {
-        st = s->fp16 ? launch_one<8, 32, 1, true>(A, smem, grid, s->stream)
-                     : launch_one<8, 32, 1, false>(A, smem, grid, s->stream);
+        st = HY_DISPATCH(16, 64, 2);
+    } else if (same && L == 8 && g.hidden == 32 && g.n_hidden == 1 && dt != HY_DT_U8) {
+        st = s->fp16 ? launch_one<8, 32, 1, HY_DT_F16>(A, smem, grid, s->stream)
+                     : launch_one<8, 32, 1, HY_DT_F32>(A, smem, grid, s->stream);
     } else {
-        st = s->fp16 ? launch_one<0, 0, 0, true>(A, smem, grid, s->stream)
-                     : launch_one<0, 0, 0, false>(A, smem, grid, s->stream);
+        st = HY_DISPATCH(0, 0, 0);
     }
+#undef HY_DISPATCH
     if (st == HYRF_OK) ++*launches;
     return st;
 }

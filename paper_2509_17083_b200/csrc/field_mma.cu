@@ -59,6 +59,7 @@ __device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
 
 // D3 for one level with two lanes per Gaussian: this lane blends the four corners whose x bit is xb; the partner
 // lane (lane ^ 16) takes the other four; the sum of both (fp32) is rounded to a packed half2 feature pair.
+template <bool U8>
 __device__ __forceinline__ uint32_t gather_level_pair(const GridDev& g, uint32_t l, const float x[3], uint32_t xb) {
     const uint32_t N = g.res[l];
     const float Nf = (float)N;
@@ -84,10 +85,20 @@ __device__ __forceinline__ uint32_t gather_level_pair(const GridDev& g, uint32_t
         idx[0] = (vx ^ hy0 ^ hz0) & g.table_mask; idx[1] = (vx ^ hy1 ^ hz0) & g.table_mask;
         idx[2] = (vx ^ hy0 ^ hz1) & g.table_mask; idx[3] = (vx ^ hy1 ^ hz1) & g.table_mask;
     }
-    const __half2* tab = reinterpret_cast<const __half2*>(g.table) + g.offset[l];
     float2 v[4];
+    if (U8) {   // D3': value = fma(code, step, min)
+        const uchar2* tab = reinterpret_cast<const uchar2*>(g.table) + g.offset[l];
+        const float2 q0 = g.q[l][0], q1 = g.q[l][1];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) v[k] = __half22float2(__ldg(tab + idx[k]));
+        for (int k = 0; k < 4; ++k) {
+            const uchar2 c = __ldg(tab + idx[k]);
+            v[k] = make_float2(__fmaf_rn((float)c.x, q0.y, q0.x), __fmaf_rn((float)c.y, q1.y, q1.x));
+        }
+    } else {
+        const __half2* tab = reinterpret_cast<const __half2*>(g.table) + g.offset[l];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) v[k] = __half22float2(__ldg(tab + idx[k]));
+    }
     const float ax = xb ? w[0] : __fsub_rn(1.0f, w[0]);
     const float wy0 = __fsub_rn(1.0f, w[1]), wz0 = __fsub_rn(1.0f, w[2]);
     float a0 = 0.0f, a1 = 0.0f;
@@ -106,8 +117,9 @@ __device__ __forceinline__ uint32_t gather_level_pair(const GridDev& g, uint32_t
 // true of every paper configuration): the tables are interleaved at upload into one array of 8-byte entries
 // (geo f0, geo f1, app f0, app f1), so one index computation and one load serve both fields and the x / x+1
 // corners of both fields sit in one 16-byte span. Halves the sector look-ups and the index arithmetic.
-__device__ __forceinline__ void gather_level_pair2(const GridDev& g, const uint2* __restrict__ both, uint32_t l,
-                                                   const float x[3], uint32_t xb, uint32_t& geo, uint32_t& app) {
+template <bool U8>
+__device__ __forceinline__ void gather_level_pair2(const GridDev& g, const GridDev& ga, const void* __restrict__ both,
+                                                   uint32_t l, const float x[3], uint32_t xb, uint32_t& geo, uint32_t& app) {
     const uint32_t N = g.res[l];
     const float Nf = (float)N;
     uint32_t ci[3];
@@ -132,18 +144,32 @@ __device__ __forceinline__ void gather_level_pair2(const GridDev& g, const uint2
         idx[0] = (vx ^ hy0 ^ hz0) & g.table_mask; idx[1] = (vx ^ hy1 ^ hz0) & g.table_mask;
         idx[2] = (vx ^ hy0 ^ hz1) & g.table_mask; idx[3] = (vx ^ hy1 ^ hz1) & g.table_mask;
     }
-    const uint2* tab = both + g.offset[l];
-    uint2 v[4];
+    float2 vgs[4], vas[4];
+    if (U8) {   // 4-byte entries (geo c0 c1 | app c0 c1), D3': value = fma(code, step, min)
+        const uchar4* tab = reinterpret_cast<const uchar4*>(both) + g.offset[l];
+        const float2 qg0 = g.q[l][0], qg1 = g.q[l][1], qa0 = ga.q[l][0], qa1 = ga.q[l][1];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) v[k] = __ldg(tab + idx[k]);
+        for (int k = 0; k < 4; ++k) {
+            const uchar4 c = __ldg(tab + idx[k]);
+            vgs[k] = make_float2(__fmaf_rn((float)c.x, qg0.y, qg0.x), __fmaf_rn((float)c.y, qg1.y, qg1.x));
+            vas[k] = make_float2(__fmaf_rn((float)c.z, qa0.y, qa0.x), __fmaf_rn((float)c.w, qa1.y, qa1.x));
+        }
+    } else {
+        const uint2* tab = reinterpret_cast<const uint2*>(both) + g.offset[l];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const uint2 v = __ldg(tab + idx[k]);
+            vgs[k] = __half22float2(*reinterpret_cast<const __half2*>(&v.x));
+            vas[k] = __half22float2(*reinterpret_cast<const __half2*>(&v.y));
+        }
+    }
     const float ax = xb ? w[0] : __fsub_rn(1.0f, w[0]);
     const float wy0 = __fsub_rn(1.0f, w[1]), wz0 = __fsub_rn(1.0f, w[2]);
     float g0 = 0.0f, g1 = 0.0f, a0 = 0.0f, a1 = 0.0f;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         const float wt = __fmul_rn(__fmul_rn(ax, (k & 1) ? w[1] : wy0), (k & 2) ? w[2] : wz0);
-        const float2 vg = __half22float2(*reinterpret_cast<const __half2*>(&v[k].x));
-        const float2 va = __half22float2(*reinterpret_cast<const __half2*>(&v[k].y));
+        const float2 vg = vgs[k], va = vas[k];
         g0 = __fmaf_rn(wt, vg.x, g0); g1 = __fmaf_rn(wt, vg.y, g1);
         a0 = __fmaf_rn(wt, va.x, a0); a1 = __fmaf_rn(wt, va.y, a1);
     }
@@ -162,6 +188,13 @@ __global__ void interleave_tables_kernel(const uint32_t* __restrict__ geo, const
     if (i < n) both[i] = make_uint2(geo[i], app[i]);
 }
 
+// 8-bit tables: [entry][2] codes x 2 -> [entry][4] codes
+__global__ void interleave_tables_u8_kernel(const uint16_t* __restrict__ geo, const uint16_t* __restrict__ app, size_t n,
+                                            uint32_t* __restrict__ both) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) both[i] = (uint32_t)geo[i] | ((uint32_t)app[i] << 16);
+}
+
 // ReLU + round to fp16 of 32 fp32 accumulator columns -> 16 packed A columns
 __device__ __forceinline__ void relu_pack32(const uint32_t* d, uint32_t* a) {
 #pragma unroll
@@ -169,8 +202,9 @@ __device__ __forceinline__ void relu_pack32(const uint32_t* d, uint32_t* a) {
         a[i] = pack_h2(fmaxf(__uint_as_float(d[2 * i]), 0.0f), fmaxf(__uint_as_float(d[2 * i + 1]), 0.0f));
 }
 
+template <bool U8>
 __global__ void __launch_bounds__(kThreads, 2)
-field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const uint2* __restrict__ both) {
+field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const void* __restrict__ both) {
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ __align__(8) uint64_t mbar[2];
     __shared__ uint32_t tmem_slot;
@@ -234,7 +268,7 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const ui
 #pragma unroll
             for (int l = 0; l < 16; ++l) {
                 uint32_t wg, wa;
-                gather_level_pair2(A.geo, both, l, xs, xb, wg, wa);
+                gather_level_pair2<U8>(A.geo, A.app, both, l, xs, xb, wg, wa);
                 if (own) a[l] = chain ? wa : wg;
                 else s_exch[chain][warp & 3u][l][lane & 15u] = chain ? wg : wa;
             }
@@ -255,7 +289,7 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const ui
                 const bool own = xb == h;
 #pragma unroll
                 for (int l = 0; l < 16; ++l) {
-                    const uint32_t p = gather_level_pair(grid, l, xs, xb);
+                    const uint32_t p = gather_level_pair<U8>(grid, l, xs, xb);
                     a[l] = own ? p : a[l];
                 }
             }
@@ -375,8 +409,9 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const ui
 // cut into three chunks that sit in the three windows where the warps of tile t would otherwise wait for their
 // tcgen05.mma to complete (commit -> mbarrier). The decoder chain of a tile is ~5 us of mostly latency; hidden this way
 // the kernel's time approaches that of the gathers alone.
+template <bool U8>
 __global__ void __launch_bounds__(kThreads, 2)
-field_mma_pipe_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const uint2* __restrict__ both) {
+field_mma_pipe_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const void* __restrict__ both) {
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ __align__(8) uint64_t mbar[2];
     __shared__ uint32_t tmem_slot;
@@ -433,7 +468,7 @@ field_mma_pipe_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, con
 #define HY_GATHER(L0, L1, XS, F)                                            \
     _Pragma("unroll") for (int l = (L0); l < (L1); ++l) {                   \
         uint32_t wg, wa;                                                    \
-        gather_level_pair2(A.geo, both, l, XS, xb, wg, wa);                 \
+        gather_level_pair2<U8>(A.geo, A.app, both, l, XS, xb, wg, wa);                \
         if (own) F[l] = chain ? wa : wg;                                    \
         else exch_out[l][lane & 15u] = chain ? wg : wa;                     \
     }
@@ -584,7 +619,7 @@ field_mma_pipe_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, con
 }  // namespace
 
 bool hy_field_mma_supported(const hyrf_scene_desc& d) {
-    return d.param_dtype == HYRF_F16 && d.geo_grid.levels == 16 && d.app_grid.levels == 16 && d.dir_pe_octaves == 4 &&
+    return (d.param_dtype == HYRF_F16 || d.param_dtype == HYRF_U8) && d.geo_grid.levels == 16 && d.app_grid.levels == 16 && d.dir_pe_octaves == 4 &&
            d.geo_mlp.in_dim == 32 && d.geo_mlp.hidden == 64 && d.geo_mlp.n_hidden == 2 && d.app_mlp.in_dim == 56 &&
            d.app_mlp.hidden == 64 && d.app_mlp.n_hidden == 2;
 }
@@ -596,9 +631,14 @@ hyrf_status hy_field_mma_prepare(hyrf_scene* s) {
         reinterpret_cast<__half*>(s->mma_w));
     if (s->both_table) {
         const size_t n = s->geo_entries;
-        interleave_tables_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(
-            reinterpret_cast<const uint32_t*>(s->geo_grid.table), reinterpret_cast<const uint32_t*>(s->app_grid.table), n,
-            reinterpret_cast<uint2*>(s->both_table));
+        if (s->u8)
+            interleave_tables_u8_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(
+                reinterpret_cast<const uint16_t*>(s->geo_grid.table), reinterpret_cast<const uint16_t*>(s->app_grid.table),
+                n, reinterpret_cast<uint32_t*>(s->both_table));
+        else
+            interleave_tables_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(
+                reinterpret_cast<const uint32_t*>(s->geo_grid.table), reinterpret_cast<const uint32_t*>(s->app_grid.table),
+                n, reinterpret_cast<uint2*>(s->both_table));
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return hy_cuda_fail(e, "pack_weights_kernel");
@@ -612,19 +652,24 @@ hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* laun
     hy_fill_field_args(s, f, &A);
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(field_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-        if (e != cudaSuccess) return hy_cuda_fail(e, "cudaFuncSetAttribute(field_mma)");
-        e = cudaFuncSetAttribute(field_mma_pipe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-        if (e != cudaSuccess) return hy_cuda_fail(e, "cudaFuncSetAttribute(field_mma_pipe)");
+        const void* ks[4] = {(const void*)field_mma_kernel<false>, (const void*)field_mma_kernel<true>,
+                             (const void*)field_mma_pipe_kernel<false>, (const void*)field_mma_pipe_kernel<true>};
+        for (const void* k : ks) {
+            cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+            if (e != cudaSuccess) return hy_cuda_fail(e, "cudaFuncSetAttribute(field_mma)");
+        }
         attr_set = true;
     }
     const int need = (int)((s->N + kTile - 1) / kTile);
     const int grid = need < 148 * 2 ? need : 148 * 2;
-    if (s->both_table)
-        field_mma_pipe_kernel<<<grid, kThreads, kSmemBytes, s->stream>>>(A, reinterpret_cast<const uint4*>(s->mma_w),
-                                                                        reinterpret_cast<const uint2*>(s->both_table));
-    else
-        field_mma_kernel<<<grid, kThreads, kSmemBytes, s->stream>>>(A, reinterpret_cast<const uint4*>(s->mma_w), nullptr);
+    const uint4* w = reinterpret_cast<const uint4*>(s->mma_w);
+    if (s->both_table) {
+        if (s->u8) field_mma_pipe_kernel<true><<<grid, kThreads, kSmemBytes, s->stream>>>(A, w, s->both_table);
+        else field_mma_pipe_kernel<false><<<grid, kThreads, kSmemBytes, s->stream>>>(A, w, s->both_table);
+    } else {
+        if (s->u8) field_mma_kernel<true><<<grid, kThreads, kSmemBytes, s->stream>>>(A, w, nullptr);
+        else field_mma_kernel<false><<<grid, kThreads, kSmemBytes, s->stream>>>(A, w, nullptr);
+    }
     ++*launches;
     return HYRF_OK;
 }

@@ -29,7 +29,8 @@ struct hyrf_scene {
     hyrf_scene_desc desc;
     std::vector<uint32_t> res_geo, res_app, res_bg;
     bool ready = false;
-    bool fp16 = false;
+    bool fp16 = false;         // decoder weights / activations in fp16 (param_dtype F16 or U8)
+    bool u8 = false;           // grid tables are 8-bit min-max codes (param_dtype U8)
     bool use_mma = false;
     cudaStream_t stream = 0;
     uint32_t N = 0;

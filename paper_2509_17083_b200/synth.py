@@ -102,6 +102,12 @@ class Scene:
     tau_T: float = 0.2
     dir_pe_octaves: int = 4
     cameras: List[Camera] = dataclasses.field(default_factory=list)
+    # compressed model: tables as 8-bit min-max codes, (entries, 2) uint8, with
+    # q[level][feature] = (min, step); decoder weights stay fp16
+    quant8: bool = False
+    geo_q: Optional[np.ndarray] = None
+    app_q: Optional[np.ndarray] = None
+    bg_q: Optional[np.ndarray] = None
 
 
 def look_at(eye, W: int, H: int, fov_x_deg: float = 60.0) -> Camera:
@@ -245,6 +251,34 @@ def make_scene(cfg: int, n_gaussians: Optional[int] = None, *, width: Optional[i
         eyes = eyes[:n_cameras]
     scene.cameras = [look_at(e, W, H) for e in eyes]
     return scene
+
+
+def quantize8(scene: Scene) -> Scene:
+    """The post-processing step of PAPER.md:229 (3) applied to a generated scene: every level of every table becomes
+    8-bit min-max codes, code = rint((v - min) / step), step = (max - min) / 255, per level and feature. This is the
+    ENCODER (input preparation); the decode the renderer performs is defined in DESIGN.md §2 D3'. Weights become fp16."""
+    import copy
+    s = copy.copy(scene)
+    for name, grid in (("geo", scene.geo_grid), ("app", scene.app_grid), ("bg", scene.bg_grid)):
+        tab = np.asarray(getattr(scene, name + "_table"), dtype=np.float32)
+        codes = np.zeros(tab.shape, np.uint8)
+        q = np.zeros((grid.levels, 2, 2), np.float32)
+        off = 0
+        for l, sz in enumerate(grid.level_sizes()):
+            seg = tab[off:off + sz]
+            for f in range(2):
+                mn, mx = np.float32(seg[:, f].min()), np.float32(seg[:, f].max())
+                step = np.float32((mx - mn) / np.float32(255.0)) if mx > mn else np.float32(1.0)
+                codes[off:off + sz, f] = np.clip(np.rint((seg[:, f] - mn) / step), 0, 255).astype(np.uint8)
+                q[l, f] = (mn, step)
+            off += sz
+        setattr(s, name + "_table", codes)
+        setattr(s, name + "_q", q)
+        setattr(s, name + "_w", np.asarray(getattr(scene, name + "_w")).astype(np.float16))
+    s.quant8 = True
+    s.fp16 = True
+    s.name = scene.name + "_q8"
+    return s
 
 
 def tiny_scene(n: int = 48, W: int = 32, H: int = 32, seed: int = 7, fp16: bool = False, levels: int = 4,

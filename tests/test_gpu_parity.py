@@ -269,3 +269,32 @@ def test_pipelined_host_delivery_matches_synchronous(B, synth):
     for i, (a, b) in enumerate(zip(got, ref)):
         assert (a == b).all(), f"frame {i} differs"
     hs.close()
+
+
+def test_quantised_tables_exact_path(B, ho, synth):
+    # compressed model (PAPER.md:227-229 (3)): 8-bit min-max tables decoded inside the gather.
+    # CUDA-core decoders: everything bit-exact against the oracle's same decode
+    s = synth.quantize8(synth.make_scene(3, n_gaussians=40_000, width=320, height=180, n_cameras=2, table_amp=0.5))
+    st = _run(B, ho, s)
+    assert st[0]["D"] > 0
+    t = synth.quantize8(synth.tiny_scene(n=64, W=48, H=40, seed=3))        # run-time-shaped kernels
+    _run(B, ho, t)
+
+
+def test_quantised_tables_tensor_path(B, ho, synth):
+    # interleaved 4-byte entries (geo c0 c1 | app c0 c1) on the tcgen05 path; high-gain tables so that a wrong
+    # (min, step) or a swapped field cannot hide in the tolerance
+    import torch
+    s = synth.quantize8(synth.make_scene(3, n_gaussians=40_000, width=320, height=180, n_cameras=2))
+    _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False)
+    s = synth.quantize8(synth.make_scene(3, n_gaussians=20_000, width=160, height=96, n_cameras=1, table_amp=1.0))
+    hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_MMA)
+    hs.debug_enable()
+    hs.render(s.cameras[0])
+    torch.cuda.synchronize()
+    raw = hs.debug_fetch(B.DBG_STAGE2_RAW)
+    ref = ho.stage_query(ho.OracleScene(s), s.cameras[0], hs.debug_fetch(B.DBG_VIS_IDX))
+    assert np.abs(ref).max() > 0.3
+    err = np.abs(raw - ref)
+    assert err.max() < 2e-2 and err.mean() < 1e-3, (err.max(), err.mean())
+    hs.close()
