@@ -46,9 +46,9 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
               int W, int H, int gx, float tau_T, float* __restrict__ out_rgb, float* __restrict__ finalT,
               uint32_t* __restrict__ bg_list, FrameCounters* __restrict__ counters, uint8_t* __restrict__ bg_mask,
               float* __restrict__ dbg_fg, const uint32_t* __restrict__ tile_queue) {
-    __shared__ float4 s_r0[kBatch];   // (u, v, A, B)
-    __shared__ float4 s_r1[kBatch];   // (C, opacity, r, g)
-    __shared__ float s_b[kBatch];
+    __shared__ float4 s_r0[kBatch + 8];   // (u, v, A, B)   (+ 8: padding to a multiple of 8)
+    __shared__ float4 s_r1[kBatch + 8];   // (C, opacity, r, g)
+    __shared__ float s_b[kBatch + 8];
     __shared__ uint32_t s_wcnt[kWarps];
     // tiles are taken longest list first (queue built by bin_ordered.cu), so the heavy tiles do not form the tail
     const int tile = tile_queue ? (int)tile_queue[blockIdx.x] : (int)blockIdx.x;
@@ -88,12 +88,19 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
             cnt += c;
         }
         if (keep) { s_r0[pos] = r0; s_r1[pos] = r1; s_b[pos] = r2; }
+        // pad the staged list to a multiple of 8 with null entries (opacity 0 -> alpha 0 -> skipped), so the blend loop
+        // runs in fixed groups of 8 with immediate shared-memory offsets
+        if (threadIdx.x < 8 && cnt + threadIdx.x < ((cnt + 7u) & ~7u)) {
+            s_r0[cnt + threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
+            s_r1[cnt + threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
+            s_b[cnt + threadIdx.x] = 0.0f;
+        }
         __syncthreads();
         // blend: branch-free per pair; a warp leaves the batch as soon as all of its pixels have terminated
         for (uint32_t k0 = 0; k0 < cnt; k0 += 8) {
             if (__all_sync(0xffffffffu, done)) break;
-            const uint32_t kend = k0 + 8 < cnt ? k0 + 8 : cnt;
-            for (uint32_t k = k0; k < kend; ++k) {
+#pragma unroll
+            for (uint32_t k = k0; k < k0 + 8; ++k) {
                 const float4 a0 = s_r0[k];
                 const float4 a1 = s_r1[k];
                 const float dx = __fsub_rn(a0.x, fi), dy = __fsub_rn(a0.y, fj);
