@@ -157,8 +157,10 @@ typedef enum {
     HYRF_DBG_FG = 11          /* f32 [H][W][3] foreground colour C_fg before stage 6 */
 } hyrf_debug_kind;
 
-/* mask bit k enables retention of kind k for later fetches (STAGE2_RAW / STAGE3_ATTRS / VIS_MASK / BG_MASK / FG
- * cost extra writes in the kernels; everything else is retained anyway). */
+/* mask bit k enables retention of kind k for later fetches (STAGE2_RAW / STAGE3_ATTRS / BG_MASK / FG cost extra writes
+ * in the kernels; TILE_RANGES / TILE_LIST make the pass materialise the per-tile lists, which it otherwise keeps per
+ * 4 x 4-tile macro tile: the ranges come from a tile-level run of the binning, the lists are written by the
+ * rasterizer as it consumes them; everything else is retained anyway). */
 hyrf_status hyrf_debug_enable(hyrf_scene* scene, uint32_t mask);
 
 /* Synchronises the stream and copies data of the LAST render to host_dst. *bytes receives the size needed; if it

@@ -156,7 +156,7 @@ void destroy(hyrf_scene* s) {
     cudaStreamSynchronize(s->stream);
     void* ptrs[] = {s->pos, s->rgb, s->scale, s->opac, (void*)s->geo_grid.table, (void*)s->app_grid.table,
                     (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w, s->both_table,
-                    s->gm, s->gm_id, s->flag_words, s->id_words, s->word_rank, s->vis_m, s->block_counts, s->vis_idx, s->rec, s->rect, s->tiles,
+                    s->gm, s->gm_id, s->flag_words, s->id_words, s->word_rank, s->vis_m, s->block_counts, s->vis_idx, s->rec, s->rect, s->tiles, s->mtiles, s->mranges,
                     s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->tt_sorted, s->offs,
                     s->scan_scratch, s->counters, s->ranges, s->tile_queue, s->fg, s->finalT, s->image, s->image2, s->bg_mask, s->bg_list,
                     s->dbg_raw, s->dbg_attrs};
@@ -272,6 +272,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc_t(s, &s->rec, 3 * N));
     HY_TRY(dev_alloc_t(s, &s->rect, N));
     HY_TRY(dev_alloc_t(s, &s->tiles, N));
+    HY_TRY(dev_alloc_t(s, &s->mtiles, N));
     HY_TRY(dev_alloc_t(s, &s->sort_a_key, N));
     HY_TRY(dev_alloc_t(s, &s->sort_a_val, N));
     HY_TRY(dev_alloc_t(s, &s->sort_b_key, N));
@@ -280,6 +281,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc_t(s, &s->offs, N));
     HY_TRY(dev_alloc_t(s, &s->counters, 1));
     HY_TRY(dev_alloc_t(s, &s->ranges, tiles));
+    HY_TRY(dev_alloc_t(s, &s->mranges, tiles));
     HY_TRY(dev_alloc_t(s, &s->tile_queue, tiles));
     HY_TRY(dev_alloc_t(s, &s->finalT, P));
     HY_TRY(dev_alloc_t(s, &s->bg_list, P));
@@ -291,7 +293,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
         destroy(s);
         return hy_cuda_fail(e, "cudaEventCreate");
     }
-    HY_TRY(ensure_entries(s, 8 * N + 65536));   // initial guess; grows on demand (hyrf_render)
+    HY_TRY(ensure_entries(s, 4 * N + 65536));   // initial guess (macro-tile entries); grows on demand (hyrf_render)
 #undef HY_TRY
     *out = s;
     return HYRF_OK;
@@ -384,6 +386,7 @@ hyrf_status build_frame(const hyrf_scene* s, const hyrf_camera* cam, int32_t W, 
     f->ablation = s->ablation;
     f->W = W; f->H = H;
     f->gx = (W + HY_TILE - 1) / HY_TILE; f->gy = (H + HY_TILE - 1) / HY_TILE;
+    f->mgx = (f->gx + HY_MACRO - 1) / HY_MACRO; f->mgy = (f->gy + HY_MACRO - 1) / HY_MACRO;
     return HYRF_OK;
 }
 
@@ -430,16 +433,29 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     const uint32_t n_tiles = (uint32_t)(f.gx * f.gy);
     uint32_t V = 0;
     uint64_t D = 0;
-    if (s->bin_ws && hy_bin_ordered_supported(s->N, n_tiles)) {
-        // ordered counting route: everything is sized on the device, so the whole frame is enqueued before the host
-        // looks at the counters; only a frame whose D outgrew the list buffer is re-binned after growing it
+    // The binning works on MACRO tiles (4 x 4 tiles): ~3 list entries per Gaussian instead of ~10, and the rasterizer
+    // picks each tile's subsequence out of its macro tile's depth-ordered list while staging. Per-TILE ranges and lists
+    // are only materialised when the debug export asks for them: the ranges by a second, tile-level run of the same
+    // binning, the lists by the rasterizer itself (what it consumed, in the order it consumed it).
+    const uint32_t n_macro = (uint32_t)(f.mgx * f.mgy);
+    const bool want_lists = ((s->debug_mask >> HYRF_DBG_TILE_LIST) | (s->debug_mask >> HYRF_DBG_TILE_RANGES)) & 1u;
+    if (s->bin_ws && hy_bin_ordered_supported(s->N, n_macro) && (!want_lists || hy_bin_ordered_supported(s->N, n_tiles))) {
+        // everything is sized on the device, so the whole frame is enqueued before the host looks at the counters;
+        // only a frame whose entry count outgrew the list buffer is re-binned after growing it
         for (int attempt = 0;; ++attempt) {
             if (attempt > 0 && (e = cudaMemsetAsync(&s->counters->n_bg, 0, 3 * sizeof(uint32_t), s->stream)) != cudaSuccess)
                 return hy_cuda_fail(e, "cudaMemsetAsync(n_bg)");   // n_bg, bin_ticket, bin_done: the first attempt used them
-            if ((st = hy_launch_bin_ordered(s, order, n_tiles, (uint32_t)f.gx, &launches)) != HYRF_OK) return st;
-            s->list_final = s->ent_val[1];
+            if (want_lists) {
+                if ((st = hy_launch_bin_ordered(s, order, n_tiles, (uint32_t)f.gx, &launches, /*macro=*/false)) != HYRF_OK) return st;
+                if ((e = cudaMemsetAsync(&s->counters->bin_ticket, 0, 2 * sizeof(uint32_t), s->stream)) != cudaSuccess)
+                    return hy_cuda_fail(e, "cudaMemsetAsync(bin_ticket)");
+            }
+            if ((st = hy_launch_bin_ordered(s, order, n_tiles, (uint32_t)f.gx, &launches, /*macro=*/true)) != HYRF_OK) return st;
+            // the per-tile lists are written by the rasterizer into the (by then dead) pair array of the macro run
+            s->list_final = want_lists ? s->ent_val[0] : nullptr;
             if (timing) cudaEventRecord(s->ev[3], s->stream);
-            hy_launch_raster(s, f, s->list_final, out_rgb, &launches, s->tile_queue);      // S5 (Eq. 1)
+            hy_launch_raster(s, f, s->mranges, s->ent_key[1], /*macro=*/true, out_rgb, &launches, s->tile_queue,
+                             want_lists ? s->ent_val[0] : nullptr);                            // S5 (Eq. 1)
             if (timing) cudaEventRecord(s->ev[4], s->stream);
             if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;   // S6 (Eq. 10-11, A.2)
             if (timing) cudaEventRecord(s->ev[5], s->stream);
@@ -447,11 +463,12 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
                 return hy_cuda_fail(e, "cudaEventSynchronize(counters)");
             V = s->counters_host->V;
             D = s->counters_host->D;
-            if (D >= 0xFFFFFFFFull) return hy_fail(HYRF_ERR_OOM, "tile-entry count %llu does not fit 32-bit offsets", (unsigned long long)D);
-            if (D <= s->d_capacity) break;
+            const uint64_t need = want_lists && D > s->counters_host->Dm ? D : s->counters_host->Dm;
+            if (need >= 0xFFFFFFFFull) return hy_fail(HYRF_ERR_OOM, "tile-entry count %llu does not fit 32-bit offsets", (unsigned long long)need);
+            if (need <= s->d_capacity) break;
             if (attempt > 0) return hy_fail(HYRF_ERR_OOM, "tile-entry scratch still too small after growing");
             if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(grow)");
-            if ((st = ensure_entries(s, (size_t)D)) != HYRF_OK) return st;
+            if ((st = ensure_entries(s, (size_t)need)) != HYRF_OK) return st;
         }
     } else {
         // radix route (very large tile grids): (tile, rank) pairs emitted in depth order, stable sort by tile id
@@ -477,7 +494,7 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
         hy_launch_ranges(s, sorted_key, D, n_tiles, &launches);
         s->list_final = sorted_val;
         if (timing) cudaEventRecord(s->ev[3], s->stream);
-        hy_launch_raster(s, f, sorted_val, out_rgb, &launches, nullptr);             // S5 (Eq. 1)
+        hy_launch_raster(s, f, s->ranges, sorted_val, /*macro=*/false, out_rgb, &launches, nullptr, nullptr);   // S5
         if (timing) cudaEventRecord(s->ev[4], s->stream);
         if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;       // S6 (Eq. 10-11, A.2)
         if (timing) cudaEventRecord(s->ev[5], s->stream);
@@ -613,8 +630,8 @@ extern "C" hyrf_status hyrf_debug_fetch(hyrf_scene* s, uint32_t kind, void* host
         case HYRF_DBG_STAGE3_ATTRS: if (!on) goto off; src = s->dbg_attrs; need = V * 44; break;
         case HYRF_DBG_PROJ: need = V * 40; break;
         case HYRF_DBG_RECT: src = s->rect; need = V * 16; break;
-        case HYRF_DBG_TILE_RANGES: src = s->ranges; need = n_tiles * 8; break;
-        case HYRF_DBG_TILE_LIST: need = D * 4; break;
+        case HYRF_DBG_TILE_RANGES: if (!on) goto off; src = s->ranges; need = n_tiles * 8; break;
+        case HYRF_DBG_TILE_LIST: if (!on || !s->list_final) goto off; need = D * 4; break;
         case HYRF_DBG_FINAL_T: src = s->finalT; need = P * 4; break;
         case HYRF_DBG_BG_MASK: if (!on) goto off; src = s->bg_mask; need = P; break;
         case HYRF_DBG_COUNTERS: need = 32; break;

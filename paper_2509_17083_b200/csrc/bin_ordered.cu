@@ -48,6 +48,8 @@ struct BinArgs {
     uint32_t* pair_rank;     // [cap] visible rank of every pair
     uint32_t* list;          // [cap]
     uint32_t cap;
+    uint32_t shift;          // 0: bins are tiles; HY_MACRO_SHIFT: bins are macro tiles (rectangles are coarsened)
+    uint32_t fine_T, fine_gx; // the tile grid (for the rasterizer's tile queue) when the bins are macro tiles
 };
 
 __device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, uint32_t lane) {
@@ -152,6 +154,10 @@ bin_pairs_kernel(const BinArgs A) {
         nt = __ldg(A.tiles + g);
         rc = __ldg(A.rect + g);
         base = A.offs[k];
+        if (A.shift) {   // tile rectangle -> macro-tile rectangle
+            const uint32_t r = (1u << A.shift) - 1u;
+            rc = make_uint4(rc.x >> A.shift, (rc.y + r) >> A.shift, rc.z >> A.shift, (rc.w + r) >> A.shift);
+        }
         if (nt == 0) rc = make_uint4(0, 1, 0, 0);
     }
     const uint32_t w = rc.y - rc.x;
@@ -183,7 +189,7 @@ bin_pairs_kernel(const BinArgs A) {
 }
 
 __device__ __forceinline__ uint32_t pair_count(const BinArgs& A) {
-    const unsigned long long D = A.counters->D;
+    const unsigned long long D = A.shift ? A.counters->Dm : A.counters->D;
     return (uint32_t)(D < A.cap ? D : A.cap);
 }
 
@@ -296,15 +302,21 @@ bin_scatter_kernel(const BinArgs A) {
         __shared__ uint32_t s_bucket[33];
         if (threadIdx.x < 33) s_bucket[threadIdx.x] = 0;
         __syncthreads();
-        for (uint32_t t = threadIdx.x; t < A.T; t += kBinThreads) atomicAdd(&s_bucket[32 - __clz(__ldg(A.totals + t))], 1u);
+        const uint32_t nq = A.shift ? A.fine_T : A.T;          // the queue holds TILES; their length is their bin's
+        auto len_of = [&](uint32_t t) {
+            if (!A.shift) return __ldg(A.totals + t);
+            const uint32_t tx = t % A.fine_gx, ty = t / A.fine_gx;
+            return __ldg(A.totals + (ty >> A.shift) * A.gx + (tx >> A.shift));
+        };
+        for (uint32_t t = threadIdx.x; t < nq; t += kBinThreads) atomicAdd(&s_bucket[32 - __clz(len_of(t))], 1u);
         __syncthreads();
         if (threadIdx.x == 0) {
             uint32_t run = 0;
             for (int b = 32; b >= 0; --b) { const uint32_t c = s_bucket[b]; s_bucket[b] = run; run += c; }
         }
         __syncthreads();
-        for (uint32_t t = threadIdx.x; t < A.T; t += kBinThreads)
-            A.tile_queue[atomicAdd(&s_bucket[32 - __clz(__ldg(A.totals + t))], 1u)] = t;
+        for (uint32_t t = threadIdx.x; t < nq; t += kBinThreads)
+            A.tile_queue[atomicAdd(&s_bucket[32 - __clz(len_of(t))], 1u)] = t;
         return;
     }
     if (c0 >= D) return;
@@ -388,10 +400,21 @@ size_t hy_bin_ordered_ws_elems(uint32_t N, size_t cap, uint32_t max_tiles) {
     return rows * T + 2 * T + 2 * ((size_t)N / kOffItems + 2) + 64;
 }
 
+// macro = false: bins are tiles -> s->ranges, list in ent_val[1] (the debug export of the per-tile lists).
+// macro = true : bins are macro tiles (HY_MACRO x HY_MACRO tiles) -> s->mranges, list in ent_key[1], s->tile_queue:
+//                what the rasterizer walks; n_tiles / gx are still those of the TILE grid.
 hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t n_tiles, uint32_t gx,
-                                  uint32_t* launches) {
+                                  uint32_t* launches, bool macro) {
     BinArgs A;
-    A.order = order; A.rect = s->rect; A.tiles = s->tiles; A.counters = s->counters;
+    A.shift = macro ? HY_MACRO_SHIFT : 0;
+    A.fine_T = n_tiles; A.fine_gx = gx;
+    if (macro) {
+        const uint32_t gy = n_tiles / gx;
+        const uint32_t mgx = (gx + HY_MACRO - 1) / HY_MACRO, mgy = (gy + HY_MACRO - 1) / HY_MACRO;
+        gx = mgx;
+        n_tiles = mgx * mgy;
+    }
+    A.order = order; A.rect = s->rect; A.tiles = macro ? s->mtiles : s->tiles; A.counters = s->counters;
     A.offs = s->offs;
     A.cap = (uint32_t)(s->d_capacity > 0xFFFFFFF0ull ? 0xFFFFFFF0ull : s->d_capacity);
     A.Ec = chunk_entries(s->d_capacity);
@@ -405,11 +428,11 @@ hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t
     A.scan_state = reinterpret_cast<unsigned long long*>(s->bin_ws + (((size_t)A.rows_cap * T_ws + 2 * T_ws + 1) & ~(size_t)1));
     A.frame = ++s->bin_frame & 0x3FFFFFFFu;
     if (A.frame == 0) A.frame = ++s->bin_frame & 0x3FFFFFFFu;   // 0 is the tag of freshly cleared words
-    A.ranges = s->ranges;
+    A.ranges = macro ? s->mranges : s->ranges;
     A.tile_queue = s->tile_queue;
     A.pair_tile = s->ent_key[0];
     A.pair_rank = s->ent_val[0];
-    A.list = s->ent_val[1];
+    A.list = macro ? s->ent_key[1] : s->ent_val[1];
     const size_t smem_count = (size_t)n_tiles * 4;
     const size_t smem_scatter = (size_t)n_tiles * 4 + (size_t)kBinWarps * ((n_tiles + 1u) & ~1u) * 2;
     static bool attr_set = false;

@@ -8,6 +8,8 @@
 
 #define HY_MAX_LEVELS 16
 #define HY_TILE 16
+#define HY_MACRO_SHIFT 2                  // binning granularity: 4 x 4 tiles (64 x 64 pixels) per macro tile
+#define HY_MACRO (1 << HY_MACRO_SHIFT)
 #define HY_REC_F4 3  // projected record = 3 x float4: (u, v, A, B) (C, opacity, r, g) (b, depth, radius, tiles)
 
 // One multi-resolution grid as the kernels see it (DESIGN.md §2 D3).
@@ -30,6 +32,7 @@ struct FrameDev {
     float z_near, tau_T, bg_radius;
     float aabb_c[3], aabb_h[3];
     int32_t W, H, gx, gy;
+    int32_t mgx, mgy;   // macro-tile grid: HY_MACRO x HY_MACRO tiles per macro tile
     uint32_t ablation;  // hyrf_ablation bits (include/hyrf.h)
 };
 

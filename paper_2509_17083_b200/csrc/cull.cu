@@ -166,6 +166,7 @@ cull_compact_kernel(const uint32_t* __restrict__ m_words, const uint32_t* __rest
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) {
         counters->V = boff_m + m_counts[blockIdx.x];
         counters->D = 0ull;
+        counters->Dm = 0ull;
         counters->n_bg = 0u;
         counters->bin_ticket = 0u;
         counters->bin_done = 0u;

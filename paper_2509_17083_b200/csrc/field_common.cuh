@@ -19,6 +19,7 @@ struct FieldArgs {
     uint32_t* depth_key;
     uint4* rect;
     uint32_t* tiles;
+    uint32_t* mtiles;
     float* dbg_raw;
     float* dbg_attrs;
 };
@@ -153,10 +154,17 @@ static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, con
             if (rc.y > rc.x && rc.w > rc.z) nt = (rc.y - rc.x) * (rc.w - rc.z);
         }
     }
-    {   // D = sum of tiles touched: one atomic per warp
+    // macro tiles (4 x 4 tile blocks) the rectangle touches: the unit the binning works in
+    uint32_t mt = 0;
+    if (nt) mt = (((rc.y + HY_MACRO - 1) >> HY_MACRO_SHIFT) - (rc.x >> HY_MACRO_SHIFT)) *
+                 (((rc.w + HY_MACRO - 1) >> HY_MACRO_SHIFT) - (rc.z >> HY_MACRO_SHIFT));
+    {   // D = sum of tiles touched, Dm = sum of macro tiles touched: one atomic each per warp
         const unsigned am = __activemask();
-        const uint32_t wsum = __reduce_add_sync(am, nt);
-        if ((threadIdx.x & 31u) == (uint32_t)(__ffs(am) - 1) && wsum) atomicAdd(&A.counters->D, (unsigned long long)wsum);
+        const uint32_t wsum = __reduce_add_sync(am, nt), msum = __reduce_add_sync(am, mt);
+        if ((threadIdx.x & 31u) == (uint32_t)(__ffs(am) - 1) && wsum) {
+            atomicAdd(&A.counters->D, (unsigned long long)wsum);
+            atomicAdd(&A.counters->Dm, (unsigned long long)msum);
+        }
     }
     if (dropped) {
         const float4 zero = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
@@ -169,5 +177,6 @@ static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, con
     A.depth_key[j] = __float_as_uint(Z);   // key of the depth sort (S4c); its value is the visible rank j itself
     A.rect[j] = rc;
     A.tiles[j] = nt;
+    A.mtiles[j] = mt;
 }
 

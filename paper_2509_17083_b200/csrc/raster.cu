@@ -45,11 +45,13 @@ __global__ void __launch_bounds__(kBatch)
 raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ list, const float4* __restrict__ rec,
               int W, int H, int gx, float tau_T, float* __restrict__ out_rgb, float* __restrict__ finalT,
               uint32_t* __restrict__ bg_list, FrameCounters* __restrict__ counters, uint8_t* __restrict__ bg_mask,
-              float* __restrict__ dbg_fg, const uint32_t* __restrict__ tile_queue) {
+              float* __restrict__ dbg_fg, const uint32_t* __restrict__ tile_queue, const uint4* __restrict__ rect,
+              int mshift, int mgx, uint32_t* __restrict__ dbg_list, const uint2* __restrict__ dbg_ranges) {
     __shared__ float4 s_r0[kBatch + 8];   // (u, v, A, B)   (+ 8: padding to a multiple of 8)
     __shared__ float4 s_r1[kBatch + 8];   // (C, opacity, r, g)
     __shared__ float s_b[kBatch + 8];
     __shared__ uint32_t s_wcnt[kWarps];
+    __shared__ uint32_t s_hcnt[kWarps];
     // tiles are taken longest list first (queue built by bin_ordered.cu), so the heavy tiles do not form the tail
     const int tile = tile_queue ? (int)tile_queue[blockIdx.x] : (int)blockIdx.x;
     const int tx = tile % gx, ty = tile / gx;
@@ -60,26 +62,51 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
     const float fi = (float)px, fj = (float)py;
     const float X0 = (float)(tx * HY_TILE), Y0 = (float)(ty * HY_TILE);
     const float X1 = fminf(X0 + (float)(HY_TILE - 1), (float)(W - 1)), Y1 = fminf(Y0 + (float)(HY_TILE - 1), (float)(H - 1));
-    const uint2 rg = ranges[tile];
+    // mshift > 0: the lists are per MACRO tile (HY_MACRO x HY_MACRO tiles, depth-ordered); this tile's list is the
+    // subsequence whose tile rectangle contains it, picked out while staging. mshift = 0: per-tile lists.
+    const uint2 rg = ranges[mshift ? (ty >> mshift) * mgx + (tx >> mshift) : tile];
+    uint32_t dbg_pos = dbg_list ? dbg_ranges[tile].x : 0u;   // debug export of the per-tile list this CTA consumed
     float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f;
     bool done = !inside;
     for (uint32_t b0 = rg.x; b0 < rg.y; b0 += kBatch) {
-        if (__syncthreads_count(done) == kBatch) break;
+        // every pixel terminated: stop — unless the per-tile list is being exported, which needs the whole list walked
+        const bool all_done = __syncthreads_count(done) == kBatch;
+        if (all_done && !dbg_list) break;
         // stage up to 256 entries, keeping (in order) only those that can reach this tile
         const uint32_t q = b0 + threadIdx.x;
-        bool keep = false;
+        bool keep = false, hit = false;
+        uint32_t g = 0;
         float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
         float r2 = 0.0f;
         if (q < rg.y) {
-            const uint32_t g = list[q];
-            r0 = __ldg(rec + 3ull * g);
-            r1 = __ldg(rec + 3ull * g + 1);
-            r2 = __ldg(reinterpret_cast<const float*>(rec + 3ull * g + 2));
-            keep = entry_reaches_tile(r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, X0, X1, Y0, Y1);
+            g = list[q];
+            hit = true;
+            if (mshift) {
+                const uint4 rc = __ldg(rect + g);
+                hit = (uint32_t)tx >= rc.x && (uint32_t)tx < rc.y && (uint32_t)ty >= rc.z && (uint32_t)ty < rc.w;
+            }
+            if (hit) {
+                r0 = __ldg(rec + 3ull * g);
+                r1 = __ldg(rec + 3ull * g + 1);
+                r2 = __ldg(reinterpret_cast<const float*>(rec + 3ull * g + 2));
+                keep = entry_reaches_tile(r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, X0, X1, Y0, Y1);
+            }
         }
         const uint32_t bal = __ballot_sync(0xffffffffu, keep);
-        if (lane == 0) s_wcnt[warp] = __popc(bal);
+        const uint32_t balh = __ballot_sync(0xffffffffu, hit);
+        if (lane == 0) { s_wcnt[warp] = __popc(bal); s_hcnt[warp] = __popc(balh); }
         __syncthreads();
+        if (dbg_list) {   // the entries of THIS tile, in list order (stable), whether or not they can reach alpha >= 1/255
+            uint32_t ph = __popc(balh & ((1u << lane) - 1u)), nh = 0;
+#pragma unroll
+            for (int w = 0; w < kWarps; ++w) {
+                const uint32_t c = s_hcnt[w];
+                ph += (w < (int)warp) ? c : 0u;
+                nh += c;
+            }
+            if (hit) dbg_list[dbg_pos + ph] = g;
+            dbg_pos += nh;
+        }
         uint32_t pos = __popc(bal & ((1u << lane) - 1u)), cnt = 0;
 #pragma unroll
         for (int w = 0; w < kWarps; ++w) {
@@ -97,7 +124,7 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
         }
         __syncthreads();
         // blend: branch-free per pair; a warp leaves the batch as soon as all of its pixels have terminated
-        for (uint32_t k0 = 0; k0 < cnt; k0 += 8) {
+        for (uint32_t k0 = 0; k0 < cnt && !all_done; k0 += 8) {
             if (__all_sync(0xffffffffu, done)) break;
 #pragma unroll
             for (uint32_t k = k0; k < k0 + 8; ++k) {
@@ -141,14 +168,15 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
 
 }  // namespace
 
-void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint32_t* list, float* out_rgb, uint32_t* launches,
-                      const uint32_t* tile_queue) {
+void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
+                      float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list) {
     const unsigned grid = (unsigned)(f.gx * f.gy);
     const bool want_fg = (s->debug_mask >> HYRF_DBG_FG) & 1u;
     const bool want_mask = (s->debug_mask >> HYRF_DBG_BG_MASK) & 1u;
     const float tau = (f.ablation & HYRF_ABL_NO_BG) ? INFINITY : f.tau_T;   // no background: empty S6 list
-    raster_kernel<<<grid, kBatch, 0, s->stream>>>(s->ranges, list, s->rec, f.W, f.H, f.gx, tau, out_rgb, s->finalT,
+    raster_kernel<<<grid, kBatch, 0, s->stream>>>(ranges, list, s->rec, f.W, f.H, f.gx, tau, out_rgb, s->finalT,
                                                   s->bg_list, s->counters, want_mask ? s->bg_mask : nullptr,
-                                                  want_fg ? s->fg : nullptr, tile_queue);
+                                                  want_fg ? s->fg : nullptr, tile_queue, s->rect,
+                                                  macro ? HY_MACRO_SHIFT : 0, f.mgx, dbg_list, s->ranges);
     ++*launches;
 }

@@ -23,6 +23,8 @@ struct FrameCounters {
     uint32_t bin_ticket;  // block tickets of bin_offsets_kernel
     uint32_t bin_done;    // finished CTAs of bin_prefix_kernel
     uint32_t pad[1];
+    unsigned long long Dm; // macro-tile entries (sum of 4x4-tile blocks touched): what the binning actually moves
+    uint32_t pad2[6];
 };
 
 struct hyrf_scene {
@@ -58,6 +60,7 @@ struct hyrf_scene {
     float4* rec = nullptr;            // [N][3] projected records
     uint4* rect = nullptr;            // [N] (x0, x1, y0, y1)
     uint32_t* tiles = nullptr;        // [N] tiles touched
+    uint32_t* mtiles = nullptr;       // [N] macro tiles (4x4-tile blocks) touched
     uint32_t* sort_a_key = nullptr;   // [N] ping-pong buffers of the depth sort; the field kernel writes (depth bits, rank) into a
     uint32_t* sort_a_val = nullptr;
     uint32_t* sort_b_key = nullptr;
@@ -80,7 +83,8 @@ struct hyrf_scene {
     uint32_t* list_final = nullptr;             // points at the sorted ent_val of the last frame
 
     // per-frame scratch sized from max W x H
-    uint2* ranges = nullptr;  // [tiles]
+    uint2* ranges = nullptr;  // [tiles] per-tile ranges (debug export; produced by the tile-level binning)
+    uint2* mranges = nullptr; // [macro tiles] ranges into the macro-tile lists the rasterizer walks
     uint32_t* tile_queue = nullptr;  // [tiles] tile ids, longest list first (bin_ordered.cu -> raster.cu)
     float* fg = nullptr;      // [H][W][3] (debug only)
     float* finalT = nullptr;  // [H][W]
@@ -139,9 +143,9 @@ void hy_launch_ranges(hyrf_scene* s, const uint32_t* keys, uint64_t D, uint32_t 
 bool hy_bin_ordered_supported(uint32_t N, uint32_t n_tiles);
 size_t hy_bin_ordered_ws_elems(uint32_t N, size_t cap, uint32_t max_tiles);
 hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t n_tiles, uint32_t gx,
-                                  uint32_t* launches);
+                                  uint32_t* launches, bool macro);
 // S5 (raster.cu)
-void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint32_t* list, float* out_rgb, uint32_t* launches,
-                      const uint32_t* tile_queue);
+void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
+                      float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list);
 // S6 (background.cu)
 hyrf_status hy_launch_background(hyrf_scene* s, const FrameDev& f, float* out_rgb, uint32_t* launches);

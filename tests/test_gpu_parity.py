@@ -150,8 +150,8 @@ def test_status_codes_on_device(B, synth):
 
 def test_render_is_deterministic_and_scratch_grows(B, synth):
     import torch
-    s = synth.make_scene(2, n_gaussians=5_000, width=256, height=256, n_cameras=1)
-    s.scale_logit[:] = 0.5                                        # big splats: D far above the initial 8N guess
+    s = synth.make_scene(2, n_gaussians=5_000, width=512, height=512, n_cameras=1)
+    s.scale_logit[:] = 0.5                                        # big splats: entry count far above the initial guess
     hs = B.HyrfScene(s)
     a = hs.render(s.cameras[0]).clone()
     b = hs.render(s.cameras[0]).clone()
