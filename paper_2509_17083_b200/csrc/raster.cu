@@ -47,9 +47,10 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
               uint32_t* __restrict__ bg_list, FrameCounters* __restrict__ counters, uint8_t* __restrict__ bg_mask,
               float* __restrict__ dbg_fg, const uint32_t* __restrict__ tile_queue, const uint4* __restrict__ rect,
               int mshift, int mgx, uint32_t* __restrict__ dbg_list, const uint2* __restrict__ dbg_ranges) {
-    __shared__ float4 s_r0[kBatch + 8];   // (u, v, A, B)   (+ 8: padding to a multiple of 8)
-    __shared__ float4 s_r1[kBatch + 8];   // (C, opacity, r, g)
-    __shared__ float s_b[kBatch + 8];
+    __shared__ float4 s_r0[2 * kBatch + 8];   // (u, v, A, B)   (+ 8: padding to a multiple of 8)
+    __shared__ float4 s_r1[2 * kBatch + 8];   // (C, opacity, r, g)
+    __shared__ float s_b[2 * kBatch + 8];
+    __shared__ uint32_t s_ids[2 * kBatch];    // ids waiting for stage B
     __shared__ uint32_t s_wcnt[kWarps];
     __shared__ uint32_t s_hcnt[kWarps];
     // tiles are taken longest list first (queue built by bin_ordered.cu), so the heavy tiles do not form the tail
@@ -68,53 +69,80 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
     uint32_t dbg_pos = dbg_list ? dbg_ranges[tile].x : 0u;   // debug export of the per-tile list this CTA consumed
     float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f;
     bool done = !inside;
-    for (uint32_t b0 = rg.x; b0 < rg.y; b0 += kBatch) {
+    uint32_t b0 = rg.x;
+    uint32_t g_next = 0;
+    uint4 rc_next = make_uint4(0, 0, 0, 0);
+    if (b0 + threadIdx.x < rg.y) {
+        g_next = list[b0 + threadIdx.x];
+        if (mshift) rc_next = __ldg(rect + g_next);
+    }
+    while (b0 < rg.y) {
         // every pixel terminated: stop — unless the per-tile list is being exported, which needs the whole list walked
         const bool all_done = __syncthreads_count(done) == kBatch;
         if (all_done && !dbg_list) break;
-        // stage up to 256 entries, keeping (in order) only those that can reach this tile
-        const uint32_t q = b0 + threadIdx.x;
-        bool keep = false, hit = false;
-        uint32_t g = 0;
-        float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
-        float r2 = 0.0f;
-        if (q < rg.y) {
-            g = list[q];
-            hit = true;
-            if (mshift) {
-                const uint4 rc = __ldg(rect + g);
-                hit = (uint32_t)tx >= rc.x && (uint32_t)tx < rc.y && (uint32_t)ty >= rc.z && (uint32_t)ty < rc.w;
+        // stage A: walk the list in chunks of 256 entries and collect, in order, the ids that belong to THIS tile (all of
+        // them when the lists are per tile; about one in five when they are per macro tile) until 256 are waiting
+        uint32_t nh = 0;
+        while (b0 < rg.y && nh < (uint32_t)kBatch) {
+            const uint32_t q = b0 + threadIdx.x;
+            bool hit = false;
+            const uint32_t g = g_next;
+            const uint4 rc = rc_next;
+            {   // the id and rectangle of the NEXT chunk's entry travel while this chunk is handled
+                const uint32_t qn = q + kBatch;
+                if (qn < rg.y) {
+                    g_next = list[qn];
+                    if (mshift) rc_next = __ldg(rect + g_next);
+                }
+            }
+            if (q < rg.y)
+                hit = !mshift || ((uint32_t)tx >= rc.x && (uint32_t)tx < rc.y && (uint32_t)ty >= rc.z && (uint32_t)ty < rc.w);
+            const uint32_t balh = __ballot_sync(0xffffffffu, hit);
+            if (lane == 0) s_hcnt[warp] = __popc(balh);
+            __syncthreads();
+            uint32_t ph = __popc(balh & ((1u << lane) - 1u)), tot = 0;
+#pragma unroll
+            for (int w = 0; w < kWarps; ++w) {
+                const uint32_t c = s_hcnt[w];
+                ph += (w < (int)warp) ? c : 0u;
+                tot += c;
             }
             if (hit) {
+                s_ids[nh + ph] = g;
+                if (dbg_list) dbg_list[dbg_pos + ph] = g;   // debug export: the per-tile list exactly as consumed
+            }
+            nh += tot;
+            dbg_pos += tot;
+            b0 += kBatch;
+            __syncthreads();
+        }
+        // stage B: the records of those ids; the ones that cannot reach alpha >= 1/255 anywhere in the tile are dropped
+        uint32_t cnt = 0;
+        for (uint32_t i0 = 0; i0 < nh; i0 += kBatch) {
+            const uint32_t i = i0 + threadIdx.x;
+            bool keep = false;
+            float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
+            float r2 = 0.0f;
+            if (i < nh) {
+                const uint32_t g = s_ids[i];
                 r0 = __ldg(rec + 3ull * g);
                 r1 = __ldg(rec + 3ull * g + 1);
                 r2 = __ldg(reinterpret_cast<const float*>(rec + 3ull * g + 2));
                 keep = entry_reaches_tile(r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, X0, X1, Y0, Y1);
             }
-        }
-        const uint32_t bal = __ballot_sync(0xffffffffu, keep);
-        const uint32_t balh = __ballot_sync(0xffffffffu, hit);
-        if (lane == 0) { s_wcnt[warp] = __popc(bal); s_hcnt[warp] = __popc(balh); }
-        __syncthreads();
-        if (dbg_list) {   // the entries of THIS tile, in list order (stable), whether or not they can reach alpha >= 1/255
-            uint32_t ph = __popc(balh & ((1u << lane) - 1u)), nh = 0;
+            const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+            if (lane == 0) s_wcnt[warp] = __popc(bal);
+            __syncthreads();
+            uint32_t pos = cnt + __popc(bal & ((1u << lane) - 1u));
 #pragma unroll
             for (int w = 0; w < kWarps; ++w) {
-                const uint32_t c = s_hcnt[w];
-                ph += (w < (int)warp) ? c : 0u;
-                nh += c;
+                const uint32_t c = s_wcnt[w];
+                pos += (w < (int)warp) ? c : 0u;
+                cnt += c;
             }
-            if (hit) dbg_list[dbg_pos + ph] = g;
-            dbg_pos += nh;
+            if (keep) { s_r0[pos] = r0; s_r1[pos] = r1; s_b[pos] = r2; }
+            __syncthreads();
         }
-        uint32_t pos = __popc(bal & ((1u << lane) - 1u)), cnt = 0;
-#pragma unroll
-        for (int w = 0; w < kWarps; ++w) {
-            const uint32_t c = s_wcnt[w];
-            pos += (w < (int)warp) ? c : 0u;
-            cnt += c;
-        }
-        if (keep) { s_r0[pos] = r0; s_r1[pos] = r1; s_b[pos] = r2; }
         // pad the staged list to a multiple of 8 with null entries (opacity 0 -> alpha 0 -> skipped), so the blend loop
         // runs in fixed groups of 8 with immediate shared-memory offsets
         if (threadIdx.x < 8 && cnt + threadIdx.x < ((cnt + 7u) & ~7u)) {
