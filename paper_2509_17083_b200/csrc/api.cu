@@ -386,7 +386,9 @@ hyrf_status build_frame(const hyrf_scene* s, const hyrf_camera* cam, int32_t W, 
     f->ablation = s->ablation;
     f->W = W; f->H = H;
     f->gx = (W + HY_TILE - 1) / HY_TILE; f->gy = (H + HY_TILE - 1) / HY_TILE;
-    f->mgx = (f->gx + HY_MACRO - 1) / HY_MACRO; f->mgy = (f->gy + HY_MACRO - 1) / HY_MACRO;
+    // small tile grids (<= 512 x 512 pixels) keep per-tile lists: with few tiles a macro tile's list is most of the scene
+    f->mshift = (f->gx * f->gy <= 1024) ? 0 : HY_MACRO_SHIFT;
+    f->mgx = (f->gx + (1 << f->mshift) - 1) >> f->mshift; f->mgy = (f->gy + (1 << f->mshift) - 1) >> f->mshift;
     return HYRF_OK;
 }
 
@@ -446,11 +448,11 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
             if (attempt > 0 && (e = cudaMemsetAsync(&s->counters->n_bg, 0, 3 * sizeof(uint32_t), s->stream)) != cudaSuccess)
                 return hy_cuda_fail(e, "cudaMemsetAsync(n_bg)");   // n_bg, bin_ticket, bin_done: the first attempt used them
             if (want_lists) {
-                if ((st = hy_launch_bin_ordered(s, order, n_tiles, (uint32_t)f.gx, &launches, /*macro=*/false)) != HYRF_OK) return st;
+                if ((st = hy_launch_bin_ordered(s, order, n_tiles, (uint32_t)f.gx, &launches, /*macro=*/false, 0)) != HYRF_OK) return st;
                 if ((e = cudaMemsetAsync(&s->counters->bin_ticket, 0, 2 * sizeof(uint32_t), s->stream)) != cudaSuccess)
                     return hy_cuda_fail(e, "cudaMemsetAsync(bin_ticket)");
             }
-            if ((st = hy_launch_bin_ordered(s, order, n_tiles, (uint32_t)f.gx, &launches, /*macro=*/true)) != HYRF_OK) return st;
+            if ((st = hy_launch_bin_ordered(s, order, n_tiles, (uint32_t)f.gx, &launches, /*macro=*/true, (uint32_t)f.mshift)) != HYRF_OK) return st;
             // the per-tile lists are written by the rasterizer into the (by then dead) pair array of the macro run
             s->list_final = want_lists ? s->ent_val[0] : nullptr;
             if (timing) cudaEventRecord(s->ev[3], s->stream);

@@ -49,6 +49,7 @@ struct BinArgs {
     uint32_t* list;          // [cap]
     uint32_t cap;
     uint32_t shift;          // 0: bins are tiles; HY_MACRO_SHIFT: bins are macro tiles (rectangles are coarsened)
+    uint32_t use_dm;         // pair count comes from counters->Dm (the run the rasterizer consumes) or ->D
     uint32_t fine_T, fine_gx; // the tile grid (for the rasterizer's tile queue) when the bins are macro tiles
 };
 
@@ -189,7 +190,7 @@ bin_pairs_kernel(const BinArgs A) {
 }
 
 __device__ __forceinline__ uint32_t pair_count(const BinArgs& A) {
-    const unsigned long long D = A.shift ? A.counters->Dm : A.counters->D;
+    const unsigned long long D = A.use_dm ? A.counters->Dm : A.counters->D;
     return (uint32_t)(D < A.cap ? D : A.cap);
 }
 
@@ -404,13 +405,14 @@ size_t hy_bin_ordered_ws_elems(uint32_t N, size_t cap, uint32_t max_tiles) {
 // macro = true : bins are macro tiles (HY_MACRO x HY_MACRO tiles) -> s->mranges, list in ent_key[1], s->tile_queue:
 //                what the rasterizer walks; n_tiles / gx are still those of the TILE grid.
 hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t n_tiles, uint32_t gx,
-                                  uint32_t* launches, bool macro) {
+                                  uint32_t* launches, bool macro, uint32_t shift) {
     BinArgs A;
-    A.shift = macro ? HY_MACRO_SHIFT : 0;
+    A.shift = macro ? shift : 0;
+    A.use_dm = macro;
     A.fine_T = n_tiles; A.fine_gx = gx;
     if (macro) {
         const uint32_t gy = n_tiles / gx;
-        const uint32_t mgx = (gx + HY_MACRO - 1) / HY_MACRO, mgy = (gy + HY_MACRO - 1) / HY_MACRO;
+        const uint32_t mgx = (gx + (1u << shift) - 1) >> shift, mgy = (gy + (1u << shift) - 1) >> shift;
         gx = mgx;
         n_tiles = mgx * mgy;
     }

@@ -32,7 +32,8 @@ struct FrameDev {
     float z_near, tau_T, bg_radius;
     float aabb_c[3], aabb_h[3];
     int32_t W, H, gx, gy;
-    int32_t mgx, mgy;   // macro-tile grid: HY_MACRO x HY_MACRO tiles per macro tile
+    int32_t mshift;     // binning granularity of this frame: macro tile = 2^mshift x 2^mshift tiles (0 on small grids)
+    int32_t mgx, mgy;   // macro-tile grid
     uint32_t ablation;  // hyrf_ablation bits (include/hyrf.h)
 };
 

@@ -156,8 +156,10 @@ static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, con
     }
     // macro tiles (4 x 4 tile blocks) the rectangle touches: the unit the binning works in
     uint32_t mt = 0;
-    if (nt) mt = (((rc.y + HY_MACRO - 1) >> HY_MACRO_SHIFT) - (rc.x >> HY_MACRO_SHIFT)) *
-                 (((rc.w + HY_MACRO - 1) >> HY_MACRO_SHIFT) - (rc.z >> HY_MACRO_SHIFT));
+    if (nt) {
+        const uint32_t sh = (uint32_t)f.mshift, r = (1u << sh) - 1u;
+        mt = (((rc.y + r) >> sh) - (rc.x >> sh)) * (((rc.w + r) >> sh) - (rc.z >> sh));
+    }
     {   // D = sum of tiles touched, Dm = sum of macro tiles touched: one atomic each per warp
         const unsigned am = __activemask();
         const uint32_t wsum = __reduce_add_sync(am, nt), msum = __reduce_add_sync(am, mt);

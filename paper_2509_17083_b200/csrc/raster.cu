@@ -205,6 +205,6 @@ void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, con
     raster_kernel<<<grid, kBatch, 0, s->stream>>>(ranges, list, s->rec, f.W, f.H, f.gx, tau, out_rgb, s->finalT,
                                                   s->bg_list, s->counters, want_mask ? s->bg_mask : nullptr,
                                                   want_fg ? s->fg : nullptr, tile_queue, s->rect,
-                                                  macro ? HY_MACRO_SHIFT : 0, f.mgx, dbg_list, s->ranges);
+                                                  macro ? f.mshift : 0, f.mgx, dbg_list, s->ranges);
     ++*launches;
 }

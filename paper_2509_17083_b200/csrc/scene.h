@@ -143,7 +143,7 @@ void hy_launch_ranges(hyrf_scene* s, const uint32_t* keys, uint64_t D, uint32_t 
 bool hy_bin_ordered_supported(uint32_t N, uint32_t n_tiles);
 size_t hy_bin_ordered_ws_elems(uint32_t N, size_t cap, uint32_t max_tiles);
 hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t n_tiles, uint32_t gx,
-                                  uint32_t* launches, bool macro);
+                                  uint32_t* launches, bool macro, uint32_t shift);
 // S5 (raster.cu)
 void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
                       float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list);
