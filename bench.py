@@ -125,7 +125,7 @@ def workload(cfg: int, args):
 
 # Algorithmic work per unit. Bytes are ALGORITHMIC: what the stage has to move if
 # every operand is read once and every result written once, not what the caches happened to move.
-def stage_rooflines(scene, V, D, n_bg, eval_pairs, peaks):
+def stage_rooflines(scene, V, D, Dm, n_bg, eval_pairs, peaks):
     esz = 1 if scene.quant8 else (2 if scene.fp16 else 4)
     gathers = (scene.geo_grid.levels + scene.app_grid.levels) * 8
     hbm = peaks["hbm_gbs"]
@@ -134,9 +134,9 @@ def stage_rooflines(scene, V, D, n_bg, eval_pairs, peaks):
     field_bytes = V * (gathers * 2 * esz + 32 + 4 + 48 + 4 + 16 + 4)
     # S1: 16 B of the Morton record + 4 B id read per stored Gaussian, 1 B visibility written; 4 B per visible x 2 lists
     cull_bytes = scene.n * (16 + 4 + 1 + 1) + V * 8
-    # S4b-c: depth sort (4 passes x 16 B per visible) + 20 B read per visible for the pairs + 8 B per pair written,
-    # 4 + 8 B read by count / scatter, 4 B per list entry written
-    bin_bytes = V * (4 * 16 + 4 + 20) + D * (8 + 4 + 8 + 4)
+    # S4b-c: depth sort (4 passes x 16 B per visible) + 20 B read per visible for the pairs + 8 B per binned pair
+    # written, 4 + 8 B read by count / scatter, 4 B per list entry written. The binned pairs are MACRO-tile entries (Dm).
+    bin_bytes = V * (4 * 16 + 4 + 20) + Dm * (8 + 4 + 8 + 4)
     out = {
         "cull": {"bound": "hbm", "work": cull_bytes, "peak": hbm, "unit": "GB/s"},
         "field": {"bound": "hbm", "work": field_bytes, "peak": hbm, "unit": "GB/s"},
@@ -280,7 +280,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
     launches = 0
-    stage, Vs, Ds = [], [], []
+    stage, Vs, Ds, Dms = [], [], [], []
     for i in range(K):
         flush.fill_(i & 0xFF)
         evs[i][0].record(stream)
@@ -291,6 +291,7 @@ def run_ours(args):
         c = hs.debug_fetch(B.DBG_COUNTERS)
         Vs.append(int(c[1]))
         Ds.append(int(c[2]))
+        Dms.append(int(c[4]))
     torch.cuda.synchronize()
     if world > 1:
         torch.distributed.barrier()
@@ -302,7 +303,7 @@ def run_ours(args):
     value = frames_total / (t_max * 1e-3)
     import numpy as np
     stage_ms = np.mean(np.array(stage), axis=0)
-    Vm, Dm = float(np.mean(Vs)), float(np.mean(Ds))
+    Vm, Dm, Dmm = float(np.mean(Vs)), float(np.mean(Ds)), float(np.mean(Dms))
     vis_per_s = sum_over_ranks(Vm * K) / (t_max * 1e-3)
     n_bg = float((hs.debug_fetch(B.DBG_FINAL_T) > scene.tau_T).sum())        # last frame's S6 work list length
 
@@ -352,7 +353,7 @@ def run_ours(args):
         eval_pairs = pairs / fr
         cpu = {"value": fr / sec, "unit": UNIT, "cores": thr, "kind": "oracle",
                "sample": f"{fr} whole frame(s) of the workload ({vtot / fr:.0f} visible Gaussians each)"}
-    rl = stage_rooflines(scene, Vm, Dm, n_bg, eval_pairs, peaks)
+    rl = stage_rooflines(scene, Vm, Dm, Dmm, n_bg, eval_pairs, peaks)
     per_stage = {}
     for i, n in enumerate(names):
         if n in rl:
@@ -372,7 +373,7 @@ def run_ours(args):
             "dtype": "f16" if scene.fp16 else "f32", "data": "synthetic",
             "config": {"workload": name, "l2": "flushed between steps (256 MiB write)", "mlp_path": args.mlp, "ablation": args.ablation,
                        "parallelism": f"replicas x{world} (cameras round-robin)"},
-            "visible_gaussians_per_s": vis_per_s, "V_mean": Vm, "D_mean": Dm,
+            "visible_gaussians_per_s": vis_per_s, "V_mean": Vm, "D_mean": Dm, "Dm_mean": Dmm,
             "stage_ms": {n: float(stage_ms[i]) for i, n in enumerate(names)} | {"frame": float(stage_ms[5])},
             "warm_l2_ms_per_step": warm_ms,
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 64, "d2h_bytes_per_step": W * H * 12,

@@ -153,7 +153,7 @@ typedef enum {
     HYRF_DBG_TILE_LIST = 7,   /* u32 [D] Gaussian ids ordered by (tile, depth bits, id) */
     HYRF_DBG_FINAL_T = 8,     /* f32 [H][W] residual transmittance after stage 5 */
     HYRF_DBG_BG_MASK = 9,     /* u8  [H][W] 1 where the background was composited */
-    HYRF_DBG_COUNTERS = 10,   /* u64 [4]: N, V, D, tiles */
+    HYRF_DBG_COUNTERS = 10,   /* u64 [5]: N, V, D (sum of tiles touched), tiles, Dm (macro-tile entries binned) */
     HYRF_DBG_FG = 11          /* f32 [H][W][3] foreground colour C_fg before stage 6 */
 } hyrf_debug_kind;
 

@@ -504,7 +504,7 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
 
     if ((e = cudaGetLastError()) != cudaSuccess) return hy_cuda_fail(e, "kernel launch");
     s->last_launches = launches;
-    s->lastV = V; s->lastD = D;
+    s->lastV = V; s->lastD = D; s->lastDm = s->counters_host->Dm;
     s->rendered = true;
     return HYRF_OK;
 }
@@ -636,7 +636,7 @@ extern "C" hyrf_status hyrf_debug_fetch(hyrf_scene* s, uint32_t kind, void* host
         case HYRF_DBG_TILE_LIST: if (!on || !s->list_final) goto off; need = D * 4; break;
         case HYRF_DBG_FINAL_T: src = s->finalT; need = P * 4; break;
         case HYRF_DBG_BG_MASK: if (!on) goto off; src = s->bg_mask; need = P; break;
-        case HYRF_DBG_COUNTERS: need = 32; break;
+        case HYRF_DBG_COUNTERS: need = 40; break;
         case HYRF_DBG_FG: if (!on) goto off; src = s->fg; need = P * 12; break;
         default: return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_debug_fetch: unknown kind %u", kind);
     }
@@ -645,7 +645,7 @@ extern "C" hyrf_status hyrf_debug_fetch(hyrf_scene* s, uint32_t kind, void* host
     if (need > cap) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_debug_fetch: need %zu bytes, cap %zu", need, cap);
     if (need == 0) return HYRF_OK;
     if (kind == HYRF_DBG_COUNTERS) {
-        uint64_t c[4] = {N, V, D, n_tiles};
+        uint64_t c[5] = {N, V, D, n_tiles, s->lastDm};
         memcpy(host_dst, c, sizeof(c));
         return HYRF_OK;
     }

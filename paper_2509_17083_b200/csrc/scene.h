@@ -108,7 +108,7 @@ struct hyrf_scene {
     bool ev_valid = false;
     uint32_t last_launches = 0;
     uint32_t lastV = 0;
-    uint64_t lastD = 0;
+    uint64_t lastD = 0, lastDm = 0;
     int32_t lastW = 0, lastH = 0;
     bool rendered = false;
 };
