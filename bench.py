@@ -155,8 +155,8 @@ def stage_rooflines(scene, V, D, Dm, n_bg, eval_pairs, peaks):
 
 def load_traffic(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu --set full capture
-    of this workload (profiles/r1c_dram_traffic.csv); None if there is no capture."""
-    p = os.path.join(ROOT, "profiles", "r1c_dram_traffic.csv")
+    of this workload (profiles/r1d_dram_traffic.csv); None if there is no capture."""
+    p = os.path.join(ROOT, "profiles", "r1d_dram_traffic.csv")
     if not os.path.exists(p):
         return None
     import csv
@@ -344,7 +344,7 @@ def run_ours(args):
     if rank != 0:
         return
     names = ["cull", "field", "bin", "raster", "background"]
-    kernels = {"field": "field_mma_kernel" if scene.fp16 and args.mlp != "fma" else "field_fma_kernel",
+    kernels = {"field": "field_mma_pipe_kernel" if scene.fp16 and args.mlp != "fma" else "field_fma_kernel",
                "raster": "raster_kernel"}
     eval_pairs = None
     cpu = None
