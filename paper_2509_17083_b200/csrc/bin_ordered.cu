@@ -382,10 +382,13 @@ bin_scatter_kernel(const BinArgs A) {
     }
 }
 
-uint32_t chunk_entries(size_t cap) {
+// pairs per CTA: at most ~1024 chunks; with few bins (macro tiles) the per-CTA set-up is cheap and small chunks give
+// the scatter more CTAs to fill the machine with, with thousands of bins it must be amortised over more pairs
+uint32_t chunk_entries(size_t cap, uint32_t T) {
     size_t c = (cap + 1023) / 1024;
     c = (c + 2047) / 2048 * 2048;
-    if (c < kMinChunk) c = kMinChunk;
+    const size_t lo = T <= 1024 ? 2048 : kMinChunk;
+    if (c < lo) c = lo;
     if (c > kMaxChunk) c = kMaxChunk;
     return (uint32_t)c;
 }
@@ -397,8 +400,11 @@ bool hy_bin_ordered_supported(uint32_t /*N*/, uint32_t n_tiles) { return n_tiles
 // uint32 elements of workspace for a list capacity of `cap` entries: count matrix + totals + look-back words
 size_t hy_bin_ordered_ws_elems(uint32_t N, size_t cap, uint32_t max_tiles) {
     const uint32_t T = max_tiles < kMaxTiles ? max_tiles : kMaxTiles;
-    const size_t rows = (cap + chunk_entries(cap) - 1) / chunk_entries(cap) + 1;
-    return rows * T + 2 * T + 2 * ((size_t)N / kOffItems + 2) + 64;
+    // the count matrix of the largest run: rows x bins grows with the bin count inside each chunk-size regime, so the
+    // two candidates are the most bins of the small-chunk regime and the most bins overall
+    auto cells = [&](uint32_t t) { return ((cap + chunk_entries(cap, t) - 1) / chunk_entries(cap, t) + 1) * (size_t)t; };
+    const size_t small = cells(T < 1024 ? T : 1024), m = cells(T) > small ? cells(T) : small;
+    return 2 * ((size_t)N / kOffItems + 2) + m + 2 * T + 64;
 }
 
 // macro = false: bins are tiles -> s->ranges, list in ent_val[1] (the debug export of the per-tile lists).
@@ -419,15 +425,18 @@ hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t
     A.order = order; A.rect = s->rect; A.tiles = macro ? s->mtiles : s->tiles; A.counters = s->counters;
     A.offs = s->offs;
     A.cap = (uint32_t)(s->d_capacity > 0xFFFFFFF0ull ? 0xFFFFFFF0ull : s->d_capacity);
-    A.Ec = chunk_entries(s->d_capacity);
+    A.Ec = chunk_entries(s->d_capacity, n_tiles);
     A.rows_cap = (uint32_t)((s->d_capacity + A.Ec - 1) / A.Ec + 1);
     A.T = n_tiles; A.gx = gx;
     const uint32_t T_max = (uint32_t)(((s->desc.max_width + HY_TILE - 1) / HY_TILE) * ((s->desc.max_height + HY_TILE - 1) / HY_TILE));
     const uint32_t T_ws = T_max < kMaxTiles ? T_max : kMaxTiles;
-    A.M = s->bin_ws;
-    A.totals = s->bin_ws + (size_t)A.rows_cap * T_ws;
-    A.starts = A.totals + T_ws;
-    A.scan_state = reinterpret_cast<unsigned long long*>(s->bin_ws + (((size_t)A.rows_cap * T_ws + 2 * T_ws + 1) & ~(size_t)1));
+    // workspace: look-back words first (their place must not depend on the run: they are only valid by frame tag),
+    // then the count matrix of this run, its totals and starts
+    A.scan_state = reinterpret_cast<unsigned long long*>(s->bin_ws);
+    A.M = s->bin_ws + 2 * ((size_t)s->N / kOffItems + 2);
+    A.totals = A.M + (size_t)A.rows_cap * n_tiles;
+    A.starts = A.totals + n_tiles;
+    (void)T_ws;
     A.frame = ++s->bin_frame & 0x3FFFFFFFu;
     if (A.frame == 0) A.frame = ++s->bin_frame & 0x3FFFFFFFu;   // 0 is the tag of freshly cleared words
     A.ranges = macro ? s->mranges : s->ranges;
