@@ -30,6 +30,25 @@ __device__ __forceinline__ float mlp_dot(const float* __restrict__ w, const floa
 template <int CIN, int CHID, int CNH, int OUT, bool FP16>
 __device__ __forceinline__ void mlp_eval(const float* __restrict__ w, int rin, int rhid, int rnh, float* a,
                                          float* b, float* out) {
+    if (CIN > 0 && CHID > 0 && CNH == 1) {
+        // one hidden layer, compile-time shapes: each hidden activation is consumed by the output neurons as soon as
+        // it exists, so the hidden vector never occupies registers. Every output still accumulates its inputs in
+        // ascending order, one fma at a time: same bits as the layer-by-layer form below.
+        const float* w2 = w + CHID * CIN;
+        float acc[OUT];
+#pragma unroll
+        for (int c = 0; c < OUT; ++c) acc[c] = 0.0f;
+#pragma unroll
+        for (int j = 0; j < CHID; ++j) {
+            float h = fmaxf(mlp_dot<true>(w + j * CIN, a, CIN), 0.0f);
+            if (FP16) h = hy_round_half(h);
+#pragma unroll
+            for (int c = 0; c < OUT; ++c) acc[c] = __fmaf_rn(w2[c * CHID + j], h, acc[c]);
+        }
+#pragma unroll
+        for (int c = 0; c < OUT; ++c) out[c] = acc[c];
+        return;
+    }
     const int IN = CIN > 0 ? CIN : rin;
     const int HID = CHID > 0 ? CHID : rhid;
     const int NH = CNH > 0 ? CNH : rnh;
