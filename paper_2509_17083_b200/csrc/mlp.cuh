@@ -38,12 +38,32 @@ __device__ __forceinline__ void mlp_eval(const float* __restrict__ w, int rin, i
         float acc[OUT];
 #pragma unroll
         for (int c = 0; c < OUT; ++c) acc[c] = 0.0f;
+        static_assert(CHID % 4 == 0 && CIN % 4 == 0, "compile-time decoder shapes are multiples of 4");
 #pragma unroll
-        for (int j = 0; j < CHID; ++j) {
-            float h = fmaxf(mlp_dot<true>(w + j * CIN, a, CIN), 0.0f);
-            if (FP16) h = hy_round_half(h);
+        for (int j = 0; j < CHID; j += 4) {
+            // four hidden neurons at a time: four independent fma chains over the same activations hide the fma and
+            // shared-memory latencies at the few warps per SM this kernel has; each chain is still k ascending
+            const float4* r0 = reinterpret_cast<const float4*>(w + (j + 0) * CIN);
+            const float4* r1 = reinterpret_cast<const float4*>(w + (j + 1) * CIN);
+            const float4* r2 = reinterpret_cast<const float4*>(w + (j + 2) * CIN);
+            const float4* r3 = reinterpret_cast<const float4*>(w + (j + 3) * CIN);
+            float h[4] = {0.0f, 0.0f, 0.0f, 0.0f};
 #pragma unroll
-            for (int c = 0; c < OUT; ++c) acc[c] = __fmaf_rn(w2[c * CHID + j], h, acc[c]);
+            for (int k = 0; k < CIN / 4; ++k) {
+                const float4 q0 = r0[k], q1 = r1[k], q2 = r2[k], q3 = r3[k];
+                const float x0 = a[4 * k], x1 = a[4 * k + 1], x2 = a[4 * k + 2], x3 = a[4 * k + 3];
+                h[0] = __fmaf_rn(q0.x, x0, h[0]); h[1] = __fmaf_rn(q1.x, x0, h[1]); h[2] = __fmaf_rn(q2.x, x0, h[2]); h[3] = __fmaf_rn(q3.x, x0, h[3]);
+                h[0] = __fmaf_rn(q0.y, x1, h[0]); h[1] = __fmaf_rn(q1.y, x1, h[1]); h[2] = __fmaf_rn(q2.y, x1, h[2]); h[3] = __fmaf_rn(q3.y, x1, h[3]);
+                h[0] = __fmaf_rn(q0.z, x2, h[0]); h[1] = __fmaf_rn(q1.z, x2, h[1]); h[2] = __fmaf_rn(q2.z, x2, h[2]); h[3] = __fmaf_rn(q3.z, x2, h[3]);
+                h[0] = __fmaf_rn(q0.w, x3, h[0]); h[1] = __fmaf_rn(q1.w, x3, h[1]); h[2] = __fmaf_rn(q2.w, x3, h[2]); h[3] = __fmaf_rn(q3.w, x3, h[3]);
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                float v = fmaxf(h[i], 0.0f);
+                if (FP16) v = hy_round_half(v);
+#pragma unroll
+                for (int c = 0; c < OUT; ++c) acc[c] = __fmaf_rn(w2[c * CHID + j + i], v, acc[c]);
+            }
         }
 #pragma unroll
         for (int c = 0; c < OUT; ++c) out[c] = acc[c];
