@@ -446,7 +446,8 @@ hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t
     A.list = macro ? s->ent_key[1] : s->ent_val[1];
     const size_t smem_count = (size_t)n_tiles * 4;
     const size_t smem_scatter = (size_t)n_tiles * 4 + (size_t)kBinWarps * ((n_tiles + 1u) & ~1u) * 2;
-    static bool attr_set = false;
+    static bool attr_done[64] = {};   // per device: function attributes belong to the device's context
+    bool& attr_set = attr_done[s->desc.device & 63];
     if (!attr_set) {
         HY_CUDA_OK(cudaFuncSetAttribute(bin_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxTiles * 4)));
         HY_CUDA_OK(cudaFuncSetAttribute(bin_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxTiles * 20)));

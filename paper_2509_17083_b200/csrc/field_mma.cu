@@ -650,7 +650,8 @@ size_t hy_field_mma_packed_bytes() { return kPackedBytes; }
 hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* launches) {
     FieldArgs A;
     hy_fill_field_args(s, f, &A);
-    static bool attr_set = false;
+    static bool attr_done[64] = {};   // per device: function attributes belong to the device's context
+    bool& attr_set = attr_done[s->desc.device & 63];
     if (!attr_set) {
         const void* ks[4] = {(const void*)field_mma_kernel<false>, (const void*)field_mma_kernel<true>,
                              (const void*)field_mma_pipe_kernel<false>, (const void*)field_mma_pipe_kernel<true>};
