@@ -251,7 +251,7 @@ def run_ours(args):
     cams_all = scene.cameras
     mine = synth.shard_cameras(len(cams_all), rank, world) or [rank % len(cams_all)]
     cams = [cams_all[i] for i in mine]                      # frame-parallel replicas: no data-path collective
-    path = {"auto": B.HYRF_MLP_AUTO, "fma": B.HYRF_MLP_FMA, "mma": B.HYRF_MLP_MMA}[args.mlp]
+    path = {"auto": B.HYRF_MLP_AUTO, "fma": B.HYRF_MLP_FMA, "mma": B.HYRF_MLP_MMA, "hmma": B.HYRF_MLP_HMMA}[args.mlp]
     hs = B.HyrfScene(scene, device=dev, mlp_path=path)
     hs.set_ablation(args.ablation)
     W, H = cams[0].W, cams[0].H
@@ -317,6 +317,25 @@ def run_ours(args):
     torch.cuda.synchronize()
     warm_ms = e0.elapsed_time(e1) / K
 
+    # --- the same frames with the depth sort serialised (hyrf_set_sort_overlap(0)): every kernel alone on the GPU, the
+    # stage times per-kernel profiling sees; reported beside the timed (overlapped) ones, never instead of them -------
+    hs.set_sort_overlap(False)
+    hs.set_timing(True)
+    Ks = min(K, 10)
+    step(0)
+    torch.cuda.synchronize()
+    stage_serial = []
+    for i in range(Ks):
+        flush.fill_(i & 0xFF)
+        step(Wm + i)
+        stage_serial.append(hs.stage_times())
+    torch.cuda.synchronize()
+    hs.set_timing(False)
+    hs.set_sort_overlap(True)
+    stage_serial_ms = np.mean(np.array(stage_serial), axis=0)
+    step(0)
+    torch.cuda.synchronize()
+
     # --- end to end through the public host API: camera from host memory, image back to pinned host memory -------
     # hyrf_render_host_async is the call a user rendering a stream of frames makes: the 11 MB device->host copy of
     # frame k overlaps the render of frame k+1 (two pinned host images, alternating); the clock stops after
@@ -344,8 +363,8 @@ def run_ours(args):
     if rank != 0:
         return
     names = ["cull", "field", "bin", "raster", "background"]
-    kernels = {"field": "field_mma_pipe_kernel" if scene.fp16 and args.mlp != "fma" else "field_fma_kernel",
-               "raster": "raster_kernel"}
+    kernels = {"field": ("field_warp_kernel" if args.mlp == "hmma" else "field_mma_pipe_kernel") if scene.fp16 and args.mlp != "fma"
+               else "field_fma_kernel", "raster": "raster_kernel"}
     eval_pairs = None
     cpu = None
     if world == 1 and not args.no_cpu and args.ablation == 0:
@@ -368,13 +387,19 @@ def run_ours(args):
     if dom in per_stage:
         roof.update({k: per_stage[dom][k] for k in ("bound", "achieved", "peak", "unit", "frac")})
         roof["launch_ms"] = per_stage[dom]["ms"]
+        # the same kernel with the GPU to itself (serialised frame): its own ceiling, without the sort's CTAs beside it
+        di = names.index(dom)
+        roof["serial_launch_ms"] = float(stage_serial_ms[di])
+        roof["serial_frac"] = rl[dom]["work"] / (stage_serial_ms[di] * 1e-3) / 1e9 / rl[dom]["peak"]
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f16" if scene.fp16 else "f32", "data": "synthetic",
             "config": {"workload": name, "l2": "flushed between steps (256 MiB write)", "mlp_path": args.mlp, "ablation": args.ablation,
+                       "schedule": "depth sort on a second stream beside the field kernel (hyrf_set_sort_overlap default)",
                        "parallelism": f"replicas x{world} (cameras round-robin)"},
             "visible_gaussians_per_s": vis_per_s, "V_mean": Vm, "D_mean": Dm, "Dm_mean": Dmm,
             "stage_ms": {n: float(stage_ms[i]) for i, n in enumerate(names)} | {"frame": float(stage_ms[5])},
+            "serial_stage_ms": {n: float(stage_serial_ms[i]) for i, n in enumerate(names)} | {"frame": float(stage_serial_ms[5])},
             "warm_l2_ms_per_step": warm_ms,
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 64, "d2h_bytes_per_step": W * H * 12,
                     "api": "hyrf_render_host_async + hyrf_host_sync", "sync_api_value": e2e_sync},
@@ -391,7 +416,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mlp", default="auto", choices=["auto", "fma", "mma"])
+    ap.add_argument("--mlp", default="auto", choices=["auto", "fma", "mma", "hmma"])
     ap.add_argument("--n-gaussians", type=int, default=0)
     ap.add_argument("--width", type=int, default=0)
     ap.add_argument("--height", type=int, default=0)

@@ -49,9 +49,12 @@ typedef enum { HYRF_F32 = 0, HYRF_F16 = 1, HYRF_U8 = 2 } hyrf_dtype;
 
 /* How the MLP decoders are evaluated.
  *  FMA: CUDA-core fp32 fma in the oracle's order — geometry decisions bit-reproducible (any param_dtype).
- *  MMA: fp16 tensor cores with fp32 accumulation (param_dtype F16 only) — the fast path for configs 3–5.
+ *  MMA: fp16 tensor cores with fp32 accumulation (param_dtype F16 / U8) — tcgen05, activations in TMEM, a CTA per
+ *       128 Gaussians.
+ *  HMMA: the same arithmetic on warp-level mma.sync, a warp per 32 Gaussians with no cross-warp hand-over (needs the
+ *       two grids to share their geometry, as in every paper configuration; otherwise MMA runs).
  *  AUTO: MMA when param_dtype is F16 and the layer shapes are supported, else FMA. */
-typedef enum { HYRF_MLP_AUTO = 0, HYRF_MLP_FMA = 1, HYRF_MLP_MMA = 2 } hyrf_mlp_path;
+typedef enum { HYRF_MLP_AUTO = 0, HYRF_MLP_FMA = 1, HYRF_MLP_MMA = 2, HYRF_MLP_HMMA = 3 } hyrf_mlp_path;
 
 /* Multi-resolution grid (layout DESIGN.md §2 D3). level_res is a HOST array. */
 typedef struct {
@@ -185,6 +188,13 @@ typedef enum {
     HYRF_ABL_NO_CULL = 1, HYRF_ABL_NO_BG = 2, HYRF_ABL_NO_NEURAL = 4, HYRF_ABL_NO_EXPLICIT = 8
 } hyrf_ablation;
 hyrf_status hyrf_set_ablation(hyrf_scene* scene, uint32_t mask);
+
+/* Scheduling of the depth sort (S4c; "ordered by depth"). Its keys, the camera-space depths, depend on
+ * the explicit positions only, so by default (on != 0) the sort runs on a library-owned second stream BESIDE the
+ * field query (S2), which leaves 32 of its 296 CTA slots to it, and joins the frame before the binning. on == 0
+ * serialises the frame on the caller's stream (one kernel at a time: what per-kernel profiling wants). The image and
+ * every debug export are identical either way. */
+hyrf_status hyrf_set_sort_overlap(hyrf_scene* scene, int on);
 
 /* Number of kernels the last render launched (for bench.py's gpu_launches). */
 hyrf_status hyrf_last_launch_count(hyrf_scene* scene, uint32_t* launches);

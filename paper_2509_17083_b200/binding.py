@@ -19,7 +19,7 @@ HYRF_OK, HYRF_ERR_INVALID_ARG, HYRF_ERR_NOT_READY, HYRF_ERR_UNSUPPORTED, HYRF_ER
 STATUS_NAMES = ["HYRF_OK", "HYRF_ERR_INVALID_ARG", "HYRF_ERR_NOT_READY", "HYRF_ERR_UNSUPPORTED", "HYRF_ERR_CAMERA",
                 "HYRF_ERR_OOM", "HYRF_ERR_CUDA"]
 HYRF_F32, HYRF_F16, HYRF_U8 = 0, 1, 2
-HYRF_MLP_AUTO, HYRF_MLP_FMA, HYRF_MLP_MMA = 0, 1, 2
+HYRF_MLP_AUTO, HYRF_MLP_FMA, HYRF_MLP_MMA, HYRF_MLP_HMMA = 0, 1, 2, 3
 (DBG_VIS_MASK, DBG_VIS_IDX, DBG_STAGE2_RAW, DBG_STAGE3_ATTRS, DBG_PROJ, DBG_RECT, DBG_TILE_RANGES, DBG_TILE_LIST,
  DBG_FINAL_T, DBG_BG_MASK, DBG_COUNTERS, DBG_FG) = range(12)
 DBG_ALL = (1 << 12) - 1
@@ -27,7 +27,7 @@ DBG_ALL = (1 << 12) - 1
 EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_render", "hyrf_render_host",
            "hyrf_destroy_scene", "hyrf_last_error", "hyrf_debug_enable", "hyrf_debug_fetch", "hyrf_set_timing",
            "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation", "hyrf_render_host_async",
-           "hyrf_host_sync"]
+           "hyrf_host_sync", "hyrf_set_sort_overlap"]
 ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
 
 
@@ -98,6 +98,7 @@ def load_library() -> C.CDLL:
         L.hyrf_stage_times.argtypes = [vp, C.POINTER(C.c_float)]
         L.hyrf_last_launch_count.argtypes = [vp, C.POINTER(C.c_uint32)]
         L.hyrf_set_ablation.argtypes = [vp, C.c_uint32]
+        L.hyrf_set_sort_overlap.argtypes = [vp, C.c_int]
         L.hyrf_render_host_async.argtypes = [vp, C.POINTER(CameraC), C.c_int32, C.c_int32, vp]
         L.hyrf_host_sync.argtypes = [vp]
         for name in EXPORTS:
@@ -282,6 +283,10 @@ class HyrfScene:
     def set_ablation(self, mask: int) -> None:
         """Ablation switches of include/hyrf.h (Table 5): ABL_NO_CULL | ABL_NO_BG | ABL_NO_NEURAL | ABL_NO_EXPLICIT."""
         _check(self.lib.hyrf_set_ablation(self.handle, int(mask)))
+
+    def set_sort_overlap(self, on: bool = True) -> None:
+        """Depth sort beside the field query on a second stream (default) or the whole frame serialised (include/hyrf.h)."""
+        _check(self.lib.hyrf_set_sort_overlap(self.handle, int(on)))
 
     def set_timing(self, on: bool = True) -> None:
         _check(self.lib.hyrf_set_timing(self.handle, int(on)))

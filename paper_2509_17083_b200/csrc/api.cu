@@ -164,6 +164,9 @@ void destroy(hyrf_scene* s) {
     free_entries(s);
     if (s->counters_host) cudaFreeHost(s->counters_host);
     if (s->ev_counters) cudaEventDestroy(s->ev_counters);
+    if (s->sort_stream) { cudaStreamSynchronize(s->sort_stream); cudaStreamDestroy(s->sort_stream); }
+    if (s->ev_culled) cudaEventDestroy(s->ev_culled);
+    if (s->ev_sorted) cudaEventDestroy(s->ev_sorted);
     if (s->copy_stream) {
         cudaStreamSynchronize(s->copy_stream);
         for (int k = 0; k < 2; ++k) { cudaEventDestroy(s->ev_rendered[k]); cudaEventDestroy(s->ev_copied[k]); }
@@ -202,10 +205,11 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     if ((st = check_mlp(desc->geo_mlp, 2 * desc->geo_grid.levels, 8, "geo_mlp")) != HYRF_OK) return st;
     if ((st = check_mlp(desc->app_mlp, 2 * desc->app_grid.levels + pe, 3, "app_mlp")) != HYRF_OK) return st;
     if ((st = check_mlp(desc->bg_mlp, 2 * desc->bg_grid.levels + pe, 3, "bg_mlp")) != HYRF_OK) return st;
-    if (desc->mlp_path != HYRF_MLP_AUTO && desc->mlp_path != HYRF_MLP_FMA && desc->mlp_path != HYRF_MLP_MMA)
+    if (desc->mlp_path != HYRF_MLP_AUTO && desc->mlp_path != HYRF_MLP_FMA && desc->mlp_path != HYRF_MLP_MMA &&
+        desc->mlp_path != HYRF_MLP_HMMA)
         return hy_fail(HYRF_ERR_INVALID_ARG, "unknown mlp_path %d", (int)desc->mlp_path);
-    if (desc->mlp_path == HYRF_MLP_MMA && !hy_field_mma_supported(*desc))
-        return hy_fail(HYRF_ERR_UNSUPPORTED, "mlp_path MMA needs fp16 parameters, 16-level grids, 32->64->64->8 and 56->64->64->3 decoders");
+    if ((desc->mlp_path == HYRF_MLP_MMA || desc->mlp_path == HYRF_MLP_HMMA) && !hy_field_mma_supported(*desc))
+        return hy_fail(HYRF_ERR_UNSUPPORTED, "mlp_path MMA / HMMA needs fp16 parameters, 16-level grids, 32->64->64->8 and 56->64->64->3 decoders");
 
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
@@ -229,6 +233,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     s->fp16 = desc->param_dtype != HYRF_F32;
     s->u8 = desc->param_dtype == HYRF_U8;
     s->use_mma = desc->mlp_path != HYRF_MLP_FMA && hy_field_mma_supported(*desc);
+    s->warp_mma = s->use_mma && desc->mlp_path == HYRF_MLP_HMMA;   // (needs the interleaved table; else the tcgen05 kernel runs)
     s->geo_entries = build_grid(s->desc.geo_grid, &s->geo_grid);
     s->app_entries = build_grid(s->desc.app_grid, &s->app_grid);
     s->bg_entries = build_grid(s->desc.bg_grid, &s->bg_grid);
@@ -292,6 +297,12 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     if ((e = cudaEventCreateWithFlags(&s->ev_counters, cudaEventDisableTiming)) != cudaSuccess) {
         destroy(s);
         return hy_cuda_fail(e, "cudaEventCreate");
+    }
+    if ((e = cudaStreamCreateWithFlags(&s->sort_stream, cudaStreamNonBlocking)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&s->ev_culled, cudaEventDisableTiming)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&s->ev_sorted, cudaEventDisableTiming)) != cudaSuccess) {
+        destroy(s);
+        return hy_cuda_fail(e, "cudaStreamCreate / cudaEventCreate (sort)");
     }
     HY_TRY(ensure_entries(s, 4 * N + 65536));   // initial guess (macro-tile entries); grows on demand (hyrf_render)
 #undef HY_TRY
@@ -416,6 +427,19 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     hy_launch_cull(s, f, &launches);
     if (timing) cudaEventRecord(s->ev[1], s->stream);
 
+    // S4c first half: order the visible Gaussians by (depth bits, id). The keys are the cull's (Z needs nothing from
+    // the fields), so the five small, latency-bound sort kernels run on their own stream beside the field kernel,
+    // which leaves a few CTA slots free for them (hy_launch_field_*), and join the frame before the binning.
+    uint32_t *order_key = nullptr, *order = nullptr;
+    const bool overlap = s->sort_overlap;
+    if (overlap) {
+        if ((e = cudaEventRecord(s->ev_culled, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(culled)");
+        if ((e = cudaStreamWaitEvent(s->sort_stream, s->ev_culled, 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent(culled)");
+        hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, s->hist,
+                        s->scan_scratch, s->sort_stream, &order_key, &order, &launches, /*iota_vals=*/true);
+        if ((e = cudaEventRecord(s->ev_sorted, s->sort_stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(sorted)");
+    }
+
     // S2 + S3 + S4a: field query, aggregation, projection
     // (explicit-only ablation: no field is queried, so the CUDA-core kernel's early-out path serves both dtypes)
     const bool mma = s->use_mma && !(s->ablation & HYRF_ABL_NO_NEURAL);
@@ -428,10 +452,13 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
         return hy_cuda_fail(e, "cudaMemcpyAsync(counters)");
     if ((e = cudaEventRecord(s->ev_counters, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(counters)");
 
-    // S4b-c: order the visible Gaussians by (depth bits, id), then build the per-tile lists in that order
-    uint32_t *order_key = nullptr, *order = nullptr;
-    hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, s->hist,
-                    s->scan_scratch, s->stream, &order_key, &order, &launches, /*iota_vals=*/true);
+    // S4b-c: the depth order joins here (or is computed here when serialised); build the per-tile lists in that order
+    if (overlap) {
+        if ((e = cudaStreamWaitEvent(s->stream, s->ev_sorted, 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent(sorted)");
+    } else {
+        hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, s->hist,
+                        s->scan_scratch, s->stream, &order_key, &order, &launches, /*iota_vals=*/true);
+    }
     const uint32_t n_tiles = (uint32_t)(f.gx * f.gy);
     uint32_t V = 0;
     uint64_t D = 0;
@@ -589,6 +616,12 @@ extern "C" hyrf_status hyrf_set_ablation(hyrf_scene* s, uint32_t mask) {
     if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_ablation: NULL scene");
     if (mask & ~15u) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_ablation: unknown bits in mask %u", mask);
     s->ablation = mask;
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_set_sort_overlap(hyrf_scene* s, int on) {
+    if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_sort_overlap: NULL scene");
+    s->sort_overlap = on != 0;
     return HYRF_OK;
 }
 

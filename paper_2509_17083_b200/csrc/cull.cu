@@ -118,10 +118,14 @@ __device__ __forceinline__ uint32_t block_offset(const uint32_t* __restrict__ co
     return total;
 }
 
+// With `pos`: also depth_key[rank] = bits of the camera-space depth Z of that Gaussian (D1's Z, the key of the depth
+// sort S4c). Z needs nothing from the fields, so the sort can start right after the cull, beside the field query.
 __device__ __forceinline__ void compact_bits(const uint32_t* __restrict__ words, const uint32_t* __restrict__ block_offs,
                                              const uint32_t* __restrict__ block_counts, uint32_t N,
                                              uint32_t* __restrict__ out, uint32_t* __restrict__ word_rank,
-                                             uint32_t* s_prefix /*[32]*/, uint32_t* s_red, uint32_t* boff_out) {
+                                             uint32_t* s_prefix /*[32]*/, uint32_t* s_red, uint32_t* boff_out,
+                                             const float* __restrict__ pos = nullptr, const FrameDev* f = nullptr,
+                                             uint32_t* __restrict__ depth_key = nullptr) {
     const uint32_t base = blockIdx.x * kCullItems;
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t boff = block_offs ? block_offs[blockIdx.x] : block_offset(block_counts, s_red);
@@ -146,8 +150,16 @@ __device__ __forceinline__ void compact_bits(const uint32_t* __restrict__ words,
         const uint32_t word = (base >> 5) + wl;
         if (word * 32u >= N) continue;
         const uint32_t bits = words[word];
-        if ((bits >> lane) & 1u)
-            out[boff + s_prefix[wl] + __popc(bits & ((1u << lane) - 1u))] = base + k * kCullThreads + threadIdx.x;
+        if ((bits >> lane) & 1u) {
+            const uint32_t rank = boff + s_prefix[wl] + __popc(bits & ((1u << lane) - 1u));
+            const uint32_t i = base + k * kCullThreads + threadIdx.x;
+            out[rank] = i;
+            if (pos) {
+                float X, Y, Z;
+                hy_to_camera(*f, pos[i], pos[(size_t)N + i], pos[2 * (size_t)N + i], X, Y, Z);
+                depth_key[rank] = __float_as_uint(Z);
+            }
+        }
     }
     __syncthreads();
 }
@@ -157,12 +169,13 @@ cull_compact_kernel(const uint32_t* __restrict__ m_words, const uint32_t* __rest
                     const uint32_t* __restrict__ m_counts, const uint32_t* __restrict__ id_words,
                     const uint32_t* __restrict__ id_offs, const uint32_t* __restrict__ id_counts, uint32_t N,
                     uint32_t* __restrict__ vis_m, uint32_t* __restrict__ vis_idx, uint32_t* __restrict__ word_rank,
-                    FrameCounters* __restrict__ counters) {
+                    FrameCounters* __restrict__ counters, const float* __restrict__ pos, const FrameDev f,
+                    uint32_t* __restrict__ depth_key) {
     __shared__ uint32_t s_prefix[kCullItems / 32];
     __shared__ uint32_t s_red[kCullThreads / 32];
     uint32_t boff_m, boff_i;
     compact_bits(m_words, m_offs, m_counts, N, vis_m, nullptr, s_prefix, s_red, &boff_m);
-    compact_bits(id_words, id_offs, id_counts, N, vis_idx, word_rank, s_prefix, s_red, &boff_i);
+    compact_bits(id_words, id_offs, id_counts, N, vis_idx, word_rank, s_prefix, s_red, &boff_i, pos, &f, depth_key);
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) {
         counters->V = boff_m + m_counts[blockIdx.x];
         counters->D = 0ull;
@@ -210,6 +223,7 @@ void hy_launch_cull(hyrf_scene* s, const FrameDev& f, uint32_t* launches) {
     }
     cull_compact_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->flag_words, in_kernel ? nullptr : m_offs, m_counts,
                                                             s->id_words, in_kernel ? nullptr : id_offs, id_counts, s->N,
-                                                            s->vis_m, s->vis_idx, s->word_rank, s->counters);
+                                                            s->vis_m, s->vis_idx, s->word_rank, s->counters, s->pos, f,
+                                                            s->sort_a_key);
     ++*launches;
 }

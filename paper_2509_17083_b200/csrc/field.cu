@@ -112,7 +112,7 @@ void hy_fill_field_args(hyrf_scene* s, const FrameDev& f, FieldArgs* out) {
     A.gm = s->gm; A.gm_id = s->gm_id; A.vis_m = s->vis_m; A.id_words = s->id_words; A.word_rank = s->word_rank;
     A.N = s->N; A.pe_octaves = s->desc.dir_pe_octaves;
     A.counters = s->counters;
-    A.rec = s->rec; A.depth_key = s->sort_a_key; A.rect = s->rect; A.tiles = s->tiles; A.mtiles = s->mtiles;
+    A.rec = s->rec; A.rect = s->rect; A.tiles = s->tiles; A.mtiles = s->mtiles;
     A.dbg_raw = ((s->debug_mask >> HYRF_DBG_STAGE2_RAW) & 1u) ? s->dbg_raw : nullptr;
     A.dbg_attrs = ((s->debug_mask >> HYRF_DBG_STAGE3_ATTRS) & 1u) ? s->dbg_attrs : nullptr;
 }

@@ -16,7 +16,6 @@ struct FieldArgs {
     uint32_t pe_octaves;
     FrameCounters* counters;
     float4* rec;
-    uint32_t* depth_key;
     uint4* rect;
     uint32_t* tiles;
     uint32_t* mtiles;
@@ -176,7 +175,8 @@ static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, con
         A.rec[3ull * j + 1] = make_float4(cC, alpha, c0, c1);
         A.rec[3ull * j + 2] = make_float4(c2, Z, radius, __uint_as_float(nt));
     }
-    A.depth_key[j] = __float_as_uint(Z);   // key of the depth sort (S4c); its value is the visible rank j itself
+    // (the key of the depth sort S4c, the bits of this same Z, is written by the cull's compaction: the sort runs
+    // beside this kernel on a second stream)
     A.rect[j] = rc;
     A.tiles[j] = nt;
     A.mtiles[j] = mt;

@@ -118,8 +118,9 @@ __device__ __forceinline__ uint32_t gather_level_pair(const GridDev& g, uint32_t
 // (geo f0, geo f1, app f0, app f1), so one index computation and one load serve both fields and the x / x+1
 // corners of both fields sit in one 16-byte span. Halves the sector look-ups and the index arithmetic.
 template <bool U8>
-__device__ __forceinline__ void gather_level_pair2(const GridDev& g, const GridDev& ga, const void* __restrict__ both,
-                                                   uint32_t l, const float x[3], uint32_t xb, uint32_t& geo, uint32_t& app) {
+__device__ __forceinline__ void gather_level_half2(const GridDev& g, const GridDev& ga, const void* __restrict__ both,
+                                                   uint32_t l, const float x[3], uint32_t xb,
+                                                   float& g0, float& g1, float& a0, float& a1) {
     const uint32_t N = g.res[l];
     const float Nf = (float)N;
     uint32_t ci[3];
@@ -165,7 +166,7 @@ __device__ __forceinline__ void gather_level_pair2(const GridDev& g, const GridD
     }
     const float ax = xb ? w[0] : __fsub_rn(1.0f, w[0]);
     const float wy0 = __fsub_rn(1.0f, w[1]), wz0 = __fsub_rn(1.0f, w[2]);
-    float g0 = 0.0f, g1 = 0.0f, a0 = 0.0f, a1 = 0.0f;
+    g0 = 0.0f; g1 = 0.0f; a0 = 0.0f; a1 = 0.0f;
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         const float wt = __fmul_rn(__fmul_rn(ax, (k & 1) ? w[1] : wy0), (k & 2) ? w[2] : wz0);
@@ -173,6 +174,14 @@ __device__ __forceinline__ void gather_level_pair2(const GridDev& g, const GridD
         g0 = __fmaf_rn(wt, vg.x, g0); g1 = __fmaf_rn(wt, vg.y, g1);
         a0 = __fmaf_rn(wt, va.x, a0); a1 = __fmaf_rn(wt, va.y, a1);
     }
+}
+
+// both lanes of a pair end up with both fields' rounded feature pairs
+template <bool U8>
+__device__ __forceinline__ void gather_level_pair2(const GridDev& g, const GridDev& ga, const void* __restrict__ both,
+                                                   uint32_t l, const float x[3], uint32_t xb, uint32_t& geo, uint32_t& app) {
+    float g0, g1, a0, a1;
+    gather_level_half2<U8>(g, ga, both, l, x, xb, g0, g1, a0, a1);
     g0 = __fadd_rn(g0, __shfl_xor_sync(0xffffffffu, g0, 16));
     g1 = __fadd_rn(g1, __shfl_xor_sync(0xffffffffu, g1, 16));
     a0 = __fadd_rn(a0, __shfl_xor_sync(0xffffffffu, a0, 16));
@@ -616,6 +625,221 @@ field_mma_pipe_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, con
     if (warp == 0) tc::tmem_dealloc<kTmemCols>(tmem);
 }
 
+
+// ---- warp-autonomous variant (mma.sync) ------------------------------------------------------------------------------
+// The decoders are 33 kFLOP per Gaussian: < 2 % of the tensor pipe either way. What the tcgen05 kernels above pay for
+// is not throughput but hand-overs: TMEM round trips (tcgen05.st / ld + waits), one elected issuer, 128-thread
+// barriers and an mbarrier wait per layer — ~7 us of latency per 128-Gaussian tile that only a second CTA and the
+// gather windows can hide (0.112 ms of the 0.204 ms with the gathers removed). Here a WARP owns 32
+// Gaussians end to end and never synchronises with another warp: gathers with two lanes per Gaussian (as above, two
+// passes of 16), features -> the warp's own 6 KB of shared memory -> mma.sync m16n8k16 A fragments; the accumulator
+// fragment of one layer IS the A fragment of the next after ReLU + rounding (registers only); weights are read from
+// shared memory as pre-packed B fragments (one LDS.128 feeds four HMMA: two k-steps x the warp's two 16-row tiles);
+// the 11 outputs return to one lane per Gaussian through shared memory for Eq. 7 and the projection. The 16 warps of
+// an SM drift apart, so one warp's gathers (L1TEX) overlap another's decoders (tensor pipe, issue slots) by themselves.
+constexpr uint32_t kWG1 = 0, kWG2 = 256, kWG3 = 768, kWA1 = 832, kWA2 = 1344, kWA3 = 1856, kWPackedU4 = 1920;   // uint4 offsets
+constexpr uint32_t kRowG = 20, kRowA = 28;   // words per feature row: 16 (+4 pad) and 16 + 12 PE; both strides are conflict-free for fragment loads
+constexpr uint32_t kWarpWords = 32 * kRowG + 32 * kRowA;
+constexpr int kWThreads = 512;   // one CTA per SM: 16 warps share one copy of the weights
+constexpr uint32_t kWarpSmemBytes = kWPackedU4 * 16 + (kWThreads / 32) * kWarpWords * 4;
+
+// raw row-major [out][in] fp16 weights -> B fragments of mma.sync.m16n8k16 (col-major B = rows of W), two k-steps per
+// uint4: lane (g = lane / 4, t = lane % 4) of n-tile j holds W[8j + g][16s + 2t, +1] and W[8j + g][16s + 8 + 2t, +1]
+__global__ void pack_weights_hmma_kernel(const __half* __restrict__ geo, const __half* __restrict__ app,
+                                         uint32_t* __restrict__ packed) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;   // one 32-bit word (two halves) each
+    if (i >= kWPackedU4 * 4) return;
+    struct Op { uint32_t off, NT, KP, n_real, k_real, src; bool app; };
+    const Op ops[6] = {{kWG1, 8, 1, 64, 32, 0, false}, {kWG2, 8, 2, 64, 64, 64 * 32, false}, {kWG3, 1, 2, 8, 64, 64 * 32 + 64 * 64, false},
+                       {kWA1, 8, 2, 64, 56, 0, true},  {kWA2, 8, 2, 64, 64, 64 * 56, true},  {kWA3, 1, 2, 3, 64, 64 * 56 + 64 * 64, true}};
+    const uint32_t u4 = i >> 2, c = i & 3u;
+    uint32_t out = 0;
+    for (int o = 0; o < 6; ++o) {
+        const Op& op = ops[o];
+        if (u4 < op.off || u4 >= op.off + op.NT * op.KP * 32) continue;
+        const uint32_t r = u4 - op.off, lane = r & 31u, jp = r >> 5, j = jp / op.KP, p = jp % op.KP;
+        const uint32_t n = 8 * j + (lane >> 2), k = 16 * (2 * p + (c >> 1)) + 8 * (c & 1u) + 2 * (lane & 3u);
+        const __half* W = (op.app ? app : geo) + op.src;
+        const __half lo = (n < op.n_real && k < op.k_real) ? W[n * op.k_real + k] : __float2half(0.0f);
+        const __half hi = (n < op.n_real && k + 1 < op.k_real) ? W[n * op.k_real + k + 1] : __float2half(0.0f);
+        out = (uint32_t)__half_as_ushort(lo) | ((uint32_t)__half_as_ushort(hi) << 16);
+    }
+    packed[i] = out;
+}
+
+__device__ __forceinline__ void hmma16816(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
+// one layer for the warp's two 16-row tiles: acc[t][j] = A_t (16 x 16 KS) W_j^T
+template <int NT, int KS>
+__device__ __forceinline__ void hmma_layer(const uint4* __restrict__ w, uint32_t lane, const uint32_t (&a)[2][KS][4],
+                                           float (&acc)[2][NT][4]) {
+#pragma unroll
+    for (int j = 0; j < NT; ++j) {
+#pragma unroll
+        for (int t = 0; t < 2; ++t) acc[t][j][0] = acc[t][j][1] = acc[t][j][2] = acc[t][j][3] = 0.0f;
+#pragma unroll
+        for (int p = 0; p < KS / 2; ++p) {
+            const uint4 b = w[(j * (KS / 2) + p) * 32 + lane];
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                hmma16816(acc[t][j], a[t][2 * p], b.x, b.y);
+                hmma16816(acc[t][j], a[t][2 * p + 1], b.z, b.w);
+            }
+        }
+    }
+}
+
+// ReLU + round to fp16: the accumulator fragments of n-tiles 2s, 2s+1 are the A fragment of k-step s
+__device__ __forceinline__ void relu_to_A(const float (&acc)[2][8][4], uint32_t (&a)[2][4][4]) {
+#pragma unroll
+    for (int t = 0; t < 2; ++t)
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            a[t][s][0] = pack_h2(fmaxf(acc[t][2 * s][0], 0.0f), fmaxf(acc[t][2 * s][1], 0.0f));
+            a[t][s][1] = pack_h2(fmaxf(acc[t][2 * s][2], 0.0f), fmaxf(acc[t][2 * s][3], 0.0f));
+            a[t][s][2] = pack_h2(fmaxf(acc[t][2 * s + 1][0], 0.0f), fmaxf(acc[t][2 * s + 1][1], 0.0f));
+            a[t][s][3] = pack_h2(fmaxf(acc[t][2 * s + 1][2], 0.0f), fmaxf(acc[t][2 * s + 1][3], 0.0f));
+        }
+}
+
+template <bool U8>
+__global__ void __launch_bounds__(kWThreads, 1)
+field_warp_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const void* __restrict__ both) {
+    extern __shared__ __align__(16) uint8_t smem[];
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
+    uint4* sw = reinterpret_cast<uint4*>(smem);
+    for (uint32_t i = threadIdx.x; i < kWPackedU4; i += kWThreads) sw[i] = __ldg(packed_w + i);
+    __syncthreads();
+    uint32_t* fG = reinterpret_cast<uint32_t*>(smem + kWPackedU4 * 16) + warp * kWarpWords;   // [32][kRowG]; later out[32][12] floats
+    uint32_t* fA = fG + 32 * kRowG;                                                           // [32][kRowA]
+    float* out = reinterpret_cast<float*>(fG);
+    const uint32_t V = A.counters->V;
+    const uint32_t xb = lane >> 4, r16 = lane & 15u;
+    const uint32_t g = lane >> 2, tg = lane & 3u;
+    const uint32_t nwarps = gridDim.x * (kWThreads / 32);
+    for (uint32_t wt = blockIdx.x * (kWThreads / 32) + warp; wt * 32u < V; wt += nwarps) {
+        const uint32_t j = wt * 32u + lane;
+        const bool valid = j < V;
+        float x[3] = {0.5f, 0.5f, 0.5f};
+        Explicit ex{};
+        if (valid) {
+            ex = fetch_visible(A, j);
+            hy_contract(A.f, ex.px, ex.py, ex.pz, x);
+        }
+        // ---- grid encodes: two passes of 16 Gaussians, lanes l and l ^ 16 share one ----
+#pragma unroll 1
+        for (uint32_t h = 0; h < 2; ++h) {
+            const int src = (int)(16u * h + r16);
+            const float xs[3] = {__shfl_sync(0xffffffffu, x[0], src), __shfl_sync(0xffffffffu, x[1], src),
+                                 __shfl_sync(0xffffffffu, x[2], src)};
+            uint32_t* dst = xb ? fA + (16u * h + r16) * kRowA : fG + (16u * h + r16) * kRowG;
+#pragma unroll
+            for (int l = 0; l < 16; ++l) {   // fully unrolled: the loads of several levels are in flight together
+                float g0, g1, a0, a1;
+                gather_level_half2<U8>(A.geo, A.app, both, l, xs, xb, g0, g1, a0, a1);
+                // the low lane keeps the geometry pair, the high lane the appearance pair: each sends what the other keeps
+                const float s0 = xb ? g0 : a0, s1 = xb ? g1 : a1;
+                const float k0 = xb ? a0 : g0, k1 = xb ? a1 : g1;
+                const float f0 = __fadd_rn(k0, __shfl_xor_sync(0xffffffffu, s0, 16));
+                const float f1 = __fadd_rn(k1, __shfl_xor_sync(0xffffffffu, s1, 16));
+                dst[l] = pack_h2(f0, f1);
+            }
+        }
+        // ---- direction encoding (Eq. 5), one lane per Gaussian ----
+        {
+            uint32_t pe2[12];
+#pragma unroll
+            for (int i = 0; i < 12; ++i) pe2[i] = 0u;
+            if (valid) {
+                const float dx = __fsub_rn(ex.px, A.f.o[0]), dy = __fsub_rn(ex.py, A.f.o[1]), dz = __fsub_rn(ex.pz, A.f.o[2]);
+                const float n = __fsqrt_rn(__fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx))));
+                const float d[3] = {__fdiv_rn(dx, n), __fdiv_rn(dy, n), __fdiv_rn(dz, n)};
+                float pe[24];   // D4 by octave doubling (see field_mma_kernel)
+#pragma unroll
+                for (int ax = 0; ax < 3; ++ax) {
+                    float sn, cs;
+                    sincospif(d[ax], &sn, &cs);
+                    pe[ax] = sn; pe[3 + ax] = cs;
+#pragma unroll
+                    for (int k = 1; k < 4; ++k) {
+                        const float s2 = 2.0f * sn * cs, c2 = 1.0f - 2.0f * sn * sn;
+                        sn = s2; cs = c2;
+                        pe[6 * k + ax] = sn; pe[6 * k + 3 + ax] = cs;
+                    }
+                }
+#pragma unroll
+                for (int i = 0; i < 12; ++i) pe2[i] = pack_h2(pe[2 * i], pe[2 * i + 1]);
+            }
+            uint4* d4 = reinterpret_cast<uint4*>(fA + lane * kRowA + 16);   // 112-byte rows: 16-byte aligned
+            d4[0] = make_uint4(pe2[0], pe2[1], pe2[2], pe2[3]);
+            d4[1] = make_uint4(pe2[4], pe2[5], pe2[6], pe2[7]);
+            d4[2] = make_uint4(pe2[8], pe2[9], pe2[10], pe2[11]);
+        }
+        __syncwarp();
+        float acc[2][8][4], o3[2][1][4];
+        uint32_t a64[2][4][4];
+        // ---- geometry decoder (Eq. 4): 32 -> 64 -> 64 -> 8 ----
+        {
+            uint32_t a32[2][2][4];
+#pragma unroll
+            for (int t = 0; t < 2; ++t)
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    const uint32_t* r0 = fG + (16 * t + g) * kRowG + 8 * s + tg;
+                    a32[t][s][0] = r0[0]; a32[t][s][1] = r0[8 * kRowG]; a32[t][s][2] = r0[4]; a32[t][s][3] = r0[8 * kRowG + 4];
+                }
+            __syncwarp();   // fG is free from here: it becomes `out`
+            hmma_layer<8, 2>(sw + kWG1, lane, a32, acc);
+        }
+        relu_to_A(acc, a64);
+        hmma_layer<8, 4>(sw + kWG2, lane, a64, acc);
+        relu_to_A(acc, a64);
+        hmma_layer<1, 4>(sw + kWG3, lane, a64, o3);
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            *reinterpret_cast<float2*>(out + (16 * t + g) * 12 + 2 * tg) = make_float2(o3[t][0][0], o3[t][0][1]);
+            *reinterpret_cast<float2*>(out + (16 * t + g + 8) * 12 + 2 * tg) = make_float2(o3[t][0][2], o3[t][0][3]);
+        }
+        // ---- appearance decoder (Eq. 6): 32 + 24 -> 64 -> 64 -> 3 ----
+#pragma unroll
+        for (int t = 0; t < 2; ++t)
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                const uint32_t* r0 = fA + (16 * t + g) * kRowA + 8 * s + tg;
+                a64[t][s][0] = r0[0]; a64[t][s][1] = r0[8 * kRowA];
+                if (s < 3) { a64[t][s][2] = r0[4]; a64[t][s][3] = r0[8 * kRowA + 4]; }
+                else { a64[t][s][2] = 0u; a64[t][s][3] = 0u; }   // inputs 56..63 do not exist
+            }
+        hmma_layer<8, 4>(sw + kWA1, lane, a64, acc);
+        relu_to_A(acc, a64);
+        hmma_layer<8, 4>(sw + kWA2, lane, a64, acc);
+        relu_to_A(acc, a64);
+        hmma_layer<1, 4>(sw + kWA3, lane, a64, o3);
+        if (tg < 2) {
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                *reinterpret_cast<float2*>(out + (16 * t + g) * 12 + 8 + 2 * tg) = make_float2(o3[t][0][0], o3[t][0][1]);
+                *reinterpret_cast<float2*>(out + (16 * t + g + 8) * 12 + 8 + 2 * tg) = make_float2(o3[t][0][2], o3[t][0][3]);
+            }
+        }
+        __syncwarp();
+        // ---- Eq. 7 + projection, one lane per Gaussian ----
+        float raw[11];
+        {
+            const float4* o4 = reinterpret_cast<const float4*>(out + lane * 12);
+            const float4 q0 = o4[0], q1 = o4[1], q2 = o4[2];
+            raw[0] = q0.x; raw[1] = q0.y; raw[2] = q0.z; raw[3] = q0.w; raw[4] = q1.x; raw[5] = q1.y; raw[6] = q1.z; raw[7] = q1.w;
+            raw[8] = q2.x; raw[9] = q2.y; raw[10] = q2.z;
+        }
+        __syncwarp();   // `out` is fG again for the next tile
+        if (valid) aggregate_project<true>(A, ex, raw);
+    }
+}
+
 }  // namespace
 
 bool hy_field_mma_supported(const hyrf_scene_desc& d) {
@@ -629,6 +853,9 @@ hyrf_status hy_field_mma_prepare(hyrf_scene* s) {
     pack_weights_kernel<<<(kPackedBytes / 2 + 255) / 256, 256, 0, s->stream>>>(
         reinterpret_cast<const __half*>(s->geo_mlp.w), reinterpret_cast<const __half*>(s->app_mlp.w),
         reinterpret_cast<__half*>(s->mma_w));
+    pack_weights_hmma_kernel<<<(kWPackedU4 * 4 + 255) / 256, 256, 0, s->stream>>>(
+        reinterpret_cast<const __half*>(s->geo_mlp.w), reinterpret_cast<const __half*>(s->app_mlp.w),
+        reinterpret_cast<uint32_t*>(reinterpret_cast<uint8_t*>(s->mma_w) + kPackedBytes));
     if (s->both_table) {
         const size_t n = s->geo_entries;
         if (s->u8)
@@ -645,7 +872,7 @@ hyrf_status hy_field_mma_prepare(hyrf_scene* s) {
     return HYRF_OK;
 }
 
-size_t hy_field_mma_packed_bytes() { return kPackedBytes; }
+size_t hy_field_mma_packed_bytes() { return kPackedBytes + kWPackedU4 * 16; }   // tcgen05 operand block, then the mma.sync fragments
 
 hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* launches) {
     FieldArgs A;
@@ -659,12 +886,29 @@ hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* laun
             cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
             if (e != cudaSuccess) return hy_cuda_fail(e, "cudaFuncSetAttribute(field_mma)");
         }
+        const void* kw[2] = {(const void*)field_warp_kernel<false>, (const void*)field_warp_kernel<true>};
+        for (const void* k : kw) {
+            cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kWarpSmemBytes);
+            if (e != cudaSuccess) return hy_cuda_fail(e, "cudaFuncSetAttribute(field_warp)");
+        }
         attr_set = true;
     }
     const int need = (int)((s->N + kTile - 1) / kTile);
-    const int grid = need < 148 * 2 ? need : 148 * 2;
+    // CTA slots left to the depth sort running beside this kernel (hyrf_set_sort_overlap): with none, the persistent
+    // CTAs hold every register of every SM and the sort waits for the kernel to end. Config 3, frame time against the
+    // slots left free: 0 -> 0.586, 16 -> 0.563, 32 -> 0.551, 48 -> 0.561 ms (serial: 0.620 ms).
+    const int gap = s->sort_overlap ? 32 : 0;
+    const int slots = 148 * 2 - gap;
+    const int grid = need < slots ? need : slots;
     const uint4* w = reinterpret_cast<const uint4*>(s->mma_w);
-    if (s->both_table) {
+    if (s->both_table && s->warp_mma) {
+        const int needw = (int)((s->N + kWThreads - 1) / kWThreads);
+        const int slotsw = 148 - gap / 2;
+        const int gridw = needw < slotsw ? needw : slotsw;
+        const uint4* ww = reinterpret_cast<const uint4*>(reinterpret_cast<const uint8_t*>(s->mma_w) + kPackedBytes);
+        if (s->u8) field_warp_kernel<true><<<gridw, kWThreads, kWarpSmemBytes, s->stream>>>(A, ww, s->both_table);
+        else field_warp_kernel<false><<<gridw, kWThreads, kWarpSmemBytes, s->stream>>>(A, ww, s->both_table);
+    } else if (s->both_table) {
         if (s->u8) field_mma_pipe_kernel<true><<<grid, kThreads, kSmemBytes, s->stream>>>(A, w, s->both_table);
         else field_mma_pipe_kernel<false><<<grid, kThreads, kSmemBytes, s->stream>>>(A, w, s->both_table);
     } else {

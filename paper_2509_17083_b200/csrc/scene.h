@@ -34,6 +34,7 @@ struct hyrf_scene {
     bool fp16 = false;         // decoder weights / activations in fp16 (param_dtype F16 or U8)
     bool u8 = false;           // grid tables are 8-bit min-max codes (param_dtype U8)
     bool use_mma = false;
+    bool warp_mma = false;     // decoders on warp-level mma.sync (field_warp_kernel) instead of tcgen05 (field_mma.cu)
     cudaStream_t stream = 0;
     uint32_t N = 0;
 
@@ -105,6 +106,9 @@ struct hyrf_scene {
     bool timing = false;
     cudaEvent_t ev[7] = {};
     cudaEvent_t ev_counters = nullptr;
+    cudaStream_t sort_stream = nullptr;                  // the depth sort runs here, beside the field kernel
+    bool sort_overlap = true;                            // hyrf_set_sort_overlap
+    cudaEvent_t ev_culled = nullptr, ev_sorted = nullptr;
     bool ev_valid = false;
     uint32_t last_launches = 0;
     uint32_t lastV = 0;

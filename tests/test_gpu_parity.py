@@ -163,20 +163,22 @@ def test_render_is_deterministic_and_scratch_grows(B, synth):
     hs.close()
 
 
-def test_config3_scaled_fp16_tensor_core_path(B, ho, synth):
-    # the launch configuration bench.py times (AUTO -> tcgen05 decoders): mask bit-exact, raw logits within 2e-3,
+@pytest.mark.parametrize("path", ["MMA", "HMMA"])
+def test_config3_scaled_fp16_tensor_core_path(B, ho, synth, path):
+    # both tensor-core kernels (tcgen05 CTA tiles; mma.sync warp tiles): mask bit-exact, raw logits within 2e-3,
     # list symmetric difference reported and bounded, image within 1e-2 (SURVEY §8c H1 protocol)
     s = synth.make_scene(3, n_gaussians=60_000, width=320, height=180, n_cameras=3)
-    st = _run(B, ho, s, mlp_path=B.HYRF_MLP_MMA, exact=False)
+    st = _run(B, ho, s, mlp_path=getattr(B, "HYRF_MLP_" + path), exact=False)
     assert max(x["raw_geo_maxdiff"] for x in st) > 0.0          # really a different arithmetic path
     print("tensor-core path stats:", st[0])
 
 
-def test_tensor_core_path_high_gain(B, ho, synth):
+@pytest.mark.parametrize("path", ["MMA", "HMMA"])
+def test_tensor_core_path_high_gain(B, ho, synth, path):
     # large table entries: decoder outputs O(1), so operand layout / K-order mistakes cannot hide in the tolerance
     s = synth.make_scene(3, n_gaussians=20_000, width=160, height=96, n_cameras=1, table_amp=1.0)
     import torch
-    hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_MMA)
+    hs = B.HyrfScene(s, mlp_path=getattr(B, "HYRF_MLP_" + path))
     hs.debug_enable()
     hs.render(s.cameras[0])
     torch.cuda.synchronize()
@@ -230,6 +232,34 @@ def test_ablation_switches_tensor_path(B, ho, synth):
     s = synth.make_scene(3, n_gaussians=30_000, width=208, height=120, n_cameras=1)
     for abl in (1, 8, 1 | 2 | 8, 4):
         _run(B, ho, s, mlp_path=B.HYRF_MLP_MMA, exact=(abl & 4) != 0, ablation=abl)
+    for abl in (1, 8):
+        _run(B, ho, s, mlp_path=B.HYRF_MLP_HMMA, exact=False, ablation=abl)
+
+
+def test_sort_overlap_is_schedule_only(B, synth):
+    # hyrf_set_sort_overlap: the depth sort beside the field kernel (default) or the frame serialised — same bits out,
+    # image and per-tile lists, on both tensor-core kernels and the exact path; several frames so that the second
+    # stream's buffers are reused across frames
+    import torch
+    s = synth.make_scene(3, n_gaussians=80_000, width=320, height=180, n_cameras=4)
+    for path in (B.HYRF_MLP_MMA, B.HYRF_MLP_HMMA, B.HYRF_MLP_FMA):
+        hs = B.HyrfScene(s, mlp_path=path)
+        hs.debug_enable()
+        ref = []
+        hs.set_sort_overlap(False)
+        for cam in s.cameras:
+            img = hs.render(cam).clone()
+            torch.cuda.synchronize()
+            ref.append((img, hs.debug_fetch(B.DBG_TILE_LIST).copy(), hs.debug_fetch(B.DBG_TILE_RANGES).copy()))
+        hs.set_sort_overlap(True)
+        for rep in range(2):
+            for cam, (img0, list0, ranges0) in zip(s.cameras, ref):
+                img = hs.render(cam)
+                torch.cuda.synchronize()
+                assert torch.equal(img, img0)
+                assert np.array_equal(hs.debug_fetch(B.DBG_TILE_RANGES), ranges0)
+                assert np.array_equal(hs.debug_fetch(B.DBG_TILE_LIST), list0)
+        hs.close()
 
 
 def test_no_cull_image_equals_full_model(B, synth):
@@ -288,13 +318,14 @@ def test_quantised_tables_tensor_path(B, ho, synth):
     s = synth.quantize8(synth.make_scene(3, n_gaussians=40_000, width=320, height=180, n_cameras=2))
     _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False)
     s = synth.quantize8(synth.make_scene(3, n_gaussians=20_000, width=160, height=96, n_cameras=1, table_amp=1.0))
-    hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_MMA)
-    hs.debug_enable()
-    hs.render(s.cameras[0])
-    torch.cuda.synchronize()
-    raw = hs.debug_fetch(B.DBG_STAGE2_RAW)
-    ref = ho.stage_query(ho.OracleScene(s), s.cameras[0], hs.debug_fetch(B.DBG_VIS_IDX))
-    assert np.abs(ref).max() > 0.3
-    err = np.abs(raw - ref)
-    assert err.max() < 2e-2 and err.mean() < 1e-3, (err.max(), err.mean())
-    hs.close()
+    for path in (B.HYRF_MLP_MMA, B.HYRF_MLP_HMMA):
+        hs = B.HyrfScene(s, mlp_path=path)
+        hs.debug_enable()
+        hs.render(s.cameras[0])
+        torch.cuda.synchronize()
+        raw = hs.debug_fetch(B.DBG_STAGE2_RAW)
+        ref = ho.stage_query(ho.OracleScene(s), s.cameras[0], hs.debug_fetch(B.DBG_VIS_IDX))
+        assert np.abs(ref).max() > 0.3
+        err = np.abs(raw - ref)
+        assert err.max() < 2e-2 and err.mean() < 1e-3, (path, err.max(), err.mean())
+        hs.close()
