@@ -155,8 +155,8 @@ def stage_rooflines(scene, V, D, Dm, n_bg, eval_pairs, peaks):
 
 def load_traffic(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu --set full capture
-    of this workload (profiles/r1e_dram_traffic.csv); None if there is no capture."""
-    p = os.path.join(ROOT, "profiles", "r1e_dram_traffic.csv")
+    of this workload (profiles/r1f_dram_traffic.csv); None if there is no capture."""
+    p = os.path.join(ROOT, "profiles", "r1f_dram_traffic.csv")
     if not os.path.exists(p):
         return None
     import csv
