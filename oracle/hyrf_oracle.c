@@ -596,6 +596,36 @@ void ho_stage_background(const ho_scene *s, const ho_camera *cam, int32_t W, int
     }
 }
 
+/* ------------------------------------------------------------------------------------------------ */
+/* Compressed explicit Gaussians (PAPER.md:227-229 items 1-2; DESIGN.md §2 D1'): positions stored as IEEE binary16,
+ * the five explicit properties (s_e, alpha_e, c_e[0..2]) as residual vector quantisation codes. The paper names
+ * R-VQ and gives no formula; this is the textbook decode: the reconstruction is the sum over stages of one
+ * codebook row per stage, x = C_0[k_0] + C_1[k_1] + ... + C_{S-1}[k_{S-1}], added in binary32 in stage order
+ * (left to right, starting from the stage-0 row itself).
+ *   pos_h      [3][n] binary16 bit patterns (SoA like the fp32 positions)
+ *   codes      [S][n] uint16, codes[s][i] < K
+ *   codebooks  [S][K][5] binary32, columns (s_e, alpha_e, c_e[0], c_e[1], c_e[2])
+ * outputs in the layout of ho_scene: pos [3][n], scale_logit [n], opacity_logit [n], rgb_logit [3][n].
+ * Returns 0, or 1 + the index of the first Gaussian with a code >= K (nothing is written for it). */
+uint32_t ho_decode_explicit(uint32_t n, const uint16_t *pos_h, uint32_t S, uint32_t K, const uint16_t *codes,
+                            const float *codebooks, float *pos, float *scale_logit, float *opacity_logit,
+                            float *rgb_logit) {
+    for (uint32_t i = 0; i < n; ++i) {
+        float x[5];
+        for (uint32_t s = 0; s < S; ++s) {
+            const uint32_t k = codes[(size_t)s * n + i];
+            if (k >= K) return 1u + i;
+            const float *row = codebooks + ((size_t)s * K + k) * 5;
+            for (int d = 0; d < 5; ++d) x[d] = (s == 0) ? row[d] : x[d] + row[d];
+        }
+        for (int a = 0; a < 3; ++a) pos[(size_t)a * n + i] = ho_half_to_float(pos_h[(size_t)a * n + i]);
+        scale_logit[i] = x[0];
+        opacity_logit[i] = x[1];
+        for (int c = 0; c < 3; ++c) rgb_logit[(size_t)c * n + i] = x[2 + c];
+    }
+    return 0;
+}
+
 int32_t ho_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -104,6 +104,7 @@ def lib() -> C.CDLL:
         L.ho_stage_bin.restype = C.c_int32
         L.ho_pair_alpha.restype = C.c_float
         L.ho_num_threads.restype = C.c_int32
+        L.ho_decode_explicit.restype = C.c_uint32
         _lib = L
     return _lib
 
@@ -145,6 +146,8 @@ class OracleScene:
     """Holds the numpy arrays alive and the C struct that points at them."""
 
     def __init__(self, scene):
+        if getattr(scene, "explicit_rvq", None) is not None:   # compressed explicit part: decode it first (D1')
+            scene = with_decoded_explicit(scene)
         self.src = scene
         self.fp16 = bool(scene.fp16)
         self.u8 = bool(getattr(scene, "quant8", False))    # 8-bit min-max tables (PAPER.md:229); decoders stay fp16
@@ -200,6 +203,38 @@ def half_to_float(h: int) -> float:
 
 def float_to_half(f: float) -> int:
     return int(lib().ho_float_to_half(C.c_float(f)))
+
+
+
+def decode_explicit(rvq) -> Dict[str, np.ndarray]:
+    """Compressed explicit Gaussians -> the fp32 SoA arrays of a scene (PAPER.md:227-229 items 1-2; DESIGN.md §2 D1').
+    `rvq` has the attribute names of synth.ExplicitRVQ: pos_h (3, N) uint16 binary16 bits, codes (S, N) uint16,
+    codebooks (S, K, 5) float32 with columns (s_e, alpha_e, c_e[3])."""
+    pos_h = np.ascontiguousarray(rvq.pos_h, np.uint16)
+    codes = np.ascontiguousarray(rvq.codes, np.uint16)
+    books = np.ascontiguousarray(rvq.codebooks, np.float32)
+    S, n = codes.shape
+    K = books.shape[1]
+    assert pos_h.shape == (3, n) and books.shape == (S, K, 5) and S >= 1
+    pos = np.zeros((3, n), np.float32)
+    sc = np.zeros(n, np.float32)
+    op = np.zeros(n, np.float32)
+    rgb = np.zeros((3, n), np.float32)
+    bad = lib().ho_decode_explicit(C.c_uint32(n), _p(pos_h), C.c_uint32(S), C.c_uint32(K), _p(codes), _p(books),
+                                   _p(pos), _p(sc), _p(op), _p(rgb))
+    if bad:
+        raise ValueError(f"R-VQ code of Gaussian {bad - 1} is outside the codebook (K = {K})")
+    return dict(pos=pos, scale_logit=sc, opacity_logit=op, rgb_logit=rgb)
+
+
+def with_decoded_explicit(scene):
+    """A shallow copy of `scene` whose explicit arrays are the decode of scene.explicit_rvq."""
+    import copy
+    s = copy.copy(scene)
+    for k, v in decode_explicit(scene.explicit_rvq).items():
+        setattr(s, k, v)
+    s.explicit_rvq = None
+    return s
 
 
 def camera_center(cam) -> np.ndarray:

@@ -74,6 +74,26 @@ class Camera:
 
 
 @dataclasses.dataclass
+class ExplicitRVQ:
+    """Compressed explicit Gaussians (PAPER.md:227-229 items 1-2): half-precision positions and residual-VQ codes of
+    the five explicit properties. Layout = include/hyrf.h hyrf_explicit_rvq."""
+    pos_h: np.ndarray      # (3, N) uint16: IEEE binary16 bit patterns of p_e, SoA
+    codes: np.ndarray      # (S, N) uint16: codebook row per stage
+    codebooks: np.ndarray  # (S, K, 5) float32: columns (s_e, alpha_e, c_e[0], c_e[1], c_e[2])
+
+    @property
+    def stages(self) -> int:
+        return int(self.codes.shape[0])
+
+    @property
+    def codebook_size(self) -> int:
+        return int(self.codebooks.shape[1])
+
+    def nbytes(self) -> int:
+        return int(self.pos_h.nbytes + self.codes.nbytes + self.codebooks.nbytes)
+
+
+@dataclasses.dataclass
 class Scene:
     name: str
     n: int
@@ -108,6 +128,9 @@ class Scene:
     geo_q: Optional[np.ndarray] = None
     app_q: Optional[np.ndarray] = None
     bg_q: Optional[np.ndarray] = None
+    # compressed explicit part (PAPER.md:227-229 items 1-2); when set, pos / *_logit above are NOT what is rendered:
+    # both sides decode explicit_rvq (the library in hyrf_upload_explicit_rvq, the oracle in decode_explicit)
+    explicit_rvq: Optional[ExplicitRVQ] = None
 
 
 def look_at(eye, W: int, H: int, fov_x_deg: float = 60.0) -> Camera:
@@ -278,6 +301,49 @@ def quantize8(scene: Scene) -> Scene:
     s.quant8 = True
     s.fp16 = True
     s.name = scene.name + "_q8"
+    return s
+
+
+def compress_explicit(scene: Scene, stages: int = 6, codebook_size: int = 64, seed: int = 0,
+                      lloyd_iters: int = 2) -> Scene:
+    """The post-processing steps of PAPER.md:229 (1)-(2) applied to a generated scene: positions rounded to binary16,
+    the rows (s_e, alpha_e, c_e) residual-vector-quantised: stage s clusters what stages 0..s-1 left over (codebook
+    seeded from random rows, a few Lloyd iterations) and stores the nearest row's index. This is the ENCODER (input
+    preparation, as quantize8 is); the decode the renderer performs is defined in DESIGN.md §2 D1'."""
+    import copy
+    rng = np.random.default_rng(np.random.PCG64(90_000 + seed))
+    n = scene.n
+    rows = np.concatenate([np.asarray(scene.scale_logit, np.float32)[:, None],
+                           np.asarray(scene.opacity_logit, np.float32)[:, None],
+                           np.asarray(scene.rgb_logit, np.float32).T], axis=1)          # (N, 5)
+    K = int(codebook_size)
+    books = np.zeros((stages, K, 5), np.float32)
+    codes = np.zeros((stages, n), np.uint16)
+    resid = rows.copy()
+
+    def nearest(x: np.ndarray, book: np.ndarray) -> np.ndarray:
+        out = np.zeros(len(x), np.int64)
+        b2 = (book.astype(np.float64) ** 2).sum(1)
+        for a in range(0, len(x), 65536):
+            blk = x[a:a + 65536].astype(np.float64)
+            out[a:a + 65536] = np.argmin(b2[None, :] - 2.0 * blk @ book.astype(np.float64).T, axis=1)
+        return out
+
+    for st in range(stages):
+        book = resid[rng.integers(0, n, size=K)].copy()
+        for _ in range(lloyd_iters):
+            k = nearest(resid, book)
+            cnt = np.bincount(k, minlength=K)
+            for d in range(5):
+                sums = np.bincount(k, weights=resid[:, d].astype(np.float64), minlength=K)
+                book[:, d] = np.where(cnt > 0, sums / np.maximum(cnt, 1), book[:, d]).astype(np.float32)
+        k = nearest(resid, book)
+        books[st], codes[st] = book, k.astype(np.uint16)
+        resid = (resid - book[k]).astype(np.float32)
+    s = copy.copy(scene)
+    s.explicit_rvq = ExplicitRVQ(pos_h=np.ascontiguousarray(np.asarray(scene.pos, np.float32).astype(np.float16).view(np.uint16)),
+                                 codes=codes, codebooks=books)
+    s.name = scene.name + f"_rvq{stages}x{K}"
     return s
 
 
