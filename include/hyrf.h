@@ -114,8 +114,39 @@ typedef struct {
 hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene** out);
 
 /* Copies the parameters into library-owned buffers (H2D or D2D on the scene's stream) and re-lays the weights
- * out for the kernels. May be called again to replace the parameters. */
+ * out for the kernels. May be called again to replace the parameters. pos, rgb_logit, scale_logit and
+ * opacity_logit may ALL be NULL when the explicit part arrives compressed through hyrf_upload_explicit_rvq; the
+ * scene can be rendered once both the fields and the explicit part have been uploaded. */
 hyrf_status hyrf_upload_params(hyrf_scene* scene, const hyrf_params* params);
+
+/* Compressed explicit Gaussians (post-processing items (1) "point positions as half-precision
+ * tensors" and (2) "residual vector quantization (R-VQ) ... [of the] explicit Gaussian properties"; arithmetic:
+ * DESIGN.md §2 D1'). The Huffman layer of item (2) is an entropy code of these same integers and is undone by the
+ * loader on the CPU before this call. All pointers are DEVICE pointers unless host_ptrs != 0; the caller keeps them.
+ *   pos_h     [3][N] IEEE binary16 bit patterns of p_e, SoA like hyrf_params.pos          p_e = float(pos_h), exact
+ *   codes     [stages][N] uint16, codes[s][i] < codebook_size
+ *   codebooks [stages][codebook_size][5] float, columns (s_e, alpha_e, c_e[0], c_e[1], c_e[2])
+ *   property row of Gaussian i = codebooks[0][codes[0][i]] + codebooks[1][codes[1][i]] + ... in binary32, added in
+ *   stage order (left to right). */
+typedef struct {
+    const uint16_t* pos_h;
+    uint32_t stages;        /* 1..16 */
+    uint32_t codebook_size; /* 1..65536 */
+    const uint16_t* codes;
+    const float* codebooks;
+    int32_t host_ptrs;
+} hyrf_explicit_rvq;
+
+/* Decodes the compressed explicit part on the GPU (one kernel over N, csrc/decode.cu) into the scene's own fp32
+ * arrays, replacing whatever explicit parameters the scene held, and rebuilds the Morton-ordered records from them;
+ * hyrf_render then runs exactly as after hyrf_upload_params. Synchronises the scene's stream. Errors:
+ * HYRF_ERR_INVALID_ARG for NULL pointers, stages / codebook_size out of range, or a code >= codebook_size (the
+ * message names the first such Gaussian; the explicit part is then undefined and the scene is not renderable until
+ * a successful upload of it). */
+hyrf_status hyrf_upload_explicit_rvq(hyrf_scene* scene, const hyrf_explicit_rvq* rvq);
+
+/* Duration (ms, CUDA events on the scene's stream) of the decode kernel of the last hyrf_upload_explicit_rvq. */
+hyrf_status hyrf_last_decode_time(hyrf_scene* scene, float* ms);
 
 /* Stream all later work of this scene is enqueued on (a cudaStream_t). Default: the legacy stream 0. */
 hyrf_status hyrf_set_stream(hyrf_scene* scene, void* cuda_stream);
@@ -157,7 +188,9 @@ typedef enum {
     HYRF_DBG_FINAL_T = 8,     /* f32 [H][W] residual transmittance after stage 5 */
     HYRF_DBG_BG_MASK = 9,     /* u8  [H][W] 1 where the background was composited */
     HYRF_DBG_COUNTERS = 10,   /* u64 [5]: N, V, D (sum of tiles touched), tiles, Dm (macro-tile entries binned) */
-    HYRF_DBG_FG = 11          /* f32 [H][W][3] foreground colour C_fg before stage 6 */
+    HYRF_DBG_FG = 11,         /* f32 [H][W][3] foreground colour C_fg before stage 6 */
+    HYRF_DBG_EXPLICIT = 12    /* f32 [8][N]: rows p_e.x, p_e.y, p_e.z, s_e, alpha_e, c_e[0..2] as the scene holds them
+                                 (needs no render and no hyrf_debug_enable: what the uploads left in the scene) */
 } hyrf_debug_kind;
 
 /* mask bit k enables retention of kind k for later fetches (STAGE2_RAW / STAGE3_ATTRS / BG_MASK / FG cost extra writes

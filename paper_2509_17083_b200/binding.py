@@ -22,12 +22,13 @@ HYRF_F32, HYRF_F16, HYRF_U8 = 0, 1, 2
 HYRF_MLP_AUTO, HYRF_MLP_FMA, HYRF_MLP_MMA, HYRF_MLP_HMMA = 0, 1, 2, 3
 (DBG_VIS_MASK, DBG_VIS_IDX, DBG_STAGE2_RAW, DBG_STAGE3_ATTRS, DBG_PROJ, DBG_RECT, DBG_TILE_RANGES, DBG_TILE_LIST,
  DBG_FINAL_T, DBG_BG_MASK, DBG_COUNTERS, DBG_FG) = range(12)
+DBG_EXPLICIT = 12   # f32 [8][N]: the explicit parameters as the scene holds them (needs no render, no debug_enable)
 DBG_ALL = (1 << 12) - 1
 
 EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_render", "hyrf_render_host",
            "hyrf_destroy_scene", "hyrf_last_error", "hyrf_debug_enable", "hyrf_debug_fetch", "hyrf_set_timing",
            "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation", "hyrf_render_host_async",
-           "hyrf_host_sync", "hyrf_set_sort_overlap"]
+           "hyrf_host_sync", "hyrf_set_sort_overlap", "hyrf_upload_explicit_rvq", "hyrf_last_decode_time"]
 ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
 
 
@@ -60,6 +61,11 @@ class Params(C.Structure):
                 ("bg_table", C.c_void_p), ("geo_w", C.c_void_p), ("app_w", C.c_void_p), ("bg_w", C.c_void_p),
                 ("geo_q", C.c_void_p), ("app_q", C.c_void_p), ("bg_q", C.c_void_p),
                 ("host_ptrs", C.c_int32)]
+
+
+class ExplicitRvqC(C.Structure):
+    _fields_ = [("pos_h", C.c_void_p), ("stages", C.c_uint32), ("codebook_size", C.c_uint32), ("codes", C.c_void_p),
+                ("codebooks", C.c_void_p), ("host_ptrs", C.c_int32)]
 
 
 class CameraC(C.Structure):
@@ -101,6 +107,8 @@ def load_library() -> C.CDLL:
         L.hyrf_set_sort_overlap.argtypes = [vp, C.c_int]
         L.hyrf_render_host_async.argtypes = [vp, C.POINTER(CameraC), C.c_int32, C.c_int32, vp]
         L.hyrf_host_sync.argtypes = [vp]
+        L.hyrf_upload_explicit_rvq.argtypes = [vp, C.POINTER(ExplicitRvqC)]
+        L.hyrf_last_decode_time.argtypes = [vp, C.POINTER(C.c_float)]
         for name in EXPORTS:
             if name != "hyrf_last_error":
                 getattr(L, name).restype = C.c_int
@@ -165,7 +173,7 @@ def make_desc(scene, max_width: int, max_height: int, device: int = 0, mlp_path:
 _DBG_DTYPE = {DBG_VIS_MASK: np.uint8, DBG_VIS_IDX: np.uint32, DBG_STAGE2_RAW: np.float32,
               DBG_STAGE3_ATTRS: np.float32, DBG_PROJ: np.float32, DBG_RECT: np.uint32, DBG_TILE_RANGES: np.uint32,
               DBG_TILE_LIST: np.uint32, DBG_FINAL_T: np.float32, DBG_BG_MASK: np.uint8, DBG_COUNTERS: np.uint64,
-              DBG_FG: np.float32}
+              DBG_FG: np.float32, DBG_EXPLICIT: np.float32}
 _DBG_COLS = {DBG_STAGE2_RAW: 11, DBG_STAGE3_ATTRS: 11, DBG_PROJ: 10, DBG_RECT: 4, DBG_TILE_RANGES: 2}
 
 
@@ -196,10 +204,12 @@ class HyrfScene:
         wdt = np.float16 if self.fp16 else np.float32
         u8 = bool(getattr(scene, "quant8", False))
         tdt = np.uint8 if u8 else wdt                  # HYRF_U8: 8-bit codes + (min, step) per level and feature
-        host = dict(pos=np.ascontiguousarray(scene.pos, np.float32), rgb_logit=np.ascontiguousarray(scene.rgb_logit, np.float32),
+        rvq = getattr(scene, "explicit_rvq", None)     # compressed explicit part: goes through hyrf_upload_explicit_rvq
+        host = {} if rvq is not None else dict(
+                    pos=np.ascontiguousarray(scene.pos, np.float32), rgb_logit=np.ascontiguousarray(scene.rgb_logit, np.float32),
                     scale_logit=np.ascontiguousarray(scene.scale_logit, np.float32),
-                    opacity_logit=np.ascontiguousarray(scene.opacity_logit, np.float32),
-                    geo_table=np.ascontiguousarray(scene.geo_table, tdt), app_table=np.ascontiguousarray(scene.app_table, tdt),
+                    opacity_logit=np.ascontiguousarray(scene.opacity_logit, np.float32))
+        host.update(geo_table=np.ascontiguousarray(scene.geo_table, tdt), app_table=np.ascontiguousarray(scene.app_table, tdt),
                     bg_table=np.ascontiguousarray(scene.bg_table, tdt), geo_w=np.ascontiguousarray(scene.geo_w, wdt),
                     app_w=np.ascontiguousarray(scene.app_w, wdt), bg_w=np.ascontiguousarray(scene.bg_w, wdt))
         if u8:
@@ -221,6 +231,41 @@ class HyrfScene:
         self.set_stream()
         _check(self.lib.hyrf_upload_params(self.handle, C.byref(p)))
         del hold
+        if rvq is not None:
+            self.upload_explicit_rvq(rvq, host_upload)
+
+    # -- hyrf_upload_explicit_rvq ---------------------------------------------------------------------------
+    def upload_explicit_rvq(self, rvq, host_upload: bool = False) -> None:
+        """rvq has synth.ExplicitRVQ's attribute names: pos_h (3, N) uint16, codes (S, N) uint16, codebooks (S, K, 5)."""
+        torch = self._torch
+        codes = np.ascontiguousarray(rvq.codes, np.uint16)
+        books = np.ascontiguousarray(rvq.codebooks, np.float32)
+        pos_h = np.ascontiguousarray(rvq.pos_h, np.uint16)
+        if pos_h.shape != (3, self.n) or codes.ndim != 2 or codes.shape[1] != self.n or books.shape != (codes.shape[0], books.shape[1], 5):
+            raise ValueError("explicit_rvq arrays do not have the shapes (3, N), (S, N), (S, K, 5)")
+        q = ExplicitRvqC()
+        q.stages, q.codebook_size = int(codes.shape[0]), int(books.shape[1])
+        if host_upload:
+            hold = (pos_h, codes, books)
+            q.pos_h, q.codes, q.codebooks, q.host_ptrs = pos_h.ctypes.data, codes.ctypes.data, books.ctypes.data, 1
+        else:
+            # torch has no uint16 arithmetic but carries the bytes: view as int16
+            hold = tuple(torch.from_numpy(a.view(np.int16) if a.dtype == np.uint16 else a).to(f"cuda:{self.device}")
+                         for a in (pos_h, codes, books))
+            torch.cuda.synchronize(self.device)
+            q.pos_h, q.codes, q.codebooks, q.host_ptrs = hold[0].data_ptr(), hold[1].data_ptr(), hold[2].data_ptr(), 0
+        self.set_stream()
+        _check(self.lib.hyrf_upload_explicit_rvq(self.handle, C.byref(q)))
+        del hold
+
+    def last_decode_time(self) -> float:
+        ms = C.c_float(0)
+        _check(self.lib.hyrf_last_decode_time(self.handle, C.byref(ms)))
+        return float(ms.value)
+
+    def explicit_params(self) -> np.ndarray:
+        """(8, N) float32: p_e[3], s_e, alpha_e, c_e[3] as the scene holds them (HYRF_DBG_EXPLICIT)."""
+        return self.debug_fetch(DBG_EXPLICIT).reshape(8, self.n)
 
     def set_stream(self, stream=None) -> None:
         torch = self._torch

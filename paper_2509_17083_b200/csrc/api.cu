@@ -319,9 +319,12 @@ extern "C" hyrf_status hyrf_set_stream(hyrf_scene* s, void* cuda_stream) {
 
 extern "C" hyrf_status hyrf_upload_params(hyrf_scene* s, const hyrf_params* p) {
     if (!s || !p) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_upload_params: NULL argument");
-    if (!p->pos || !p->rgb_logit || !p->scale_logit || !p->opacity_logit || !p->geo_table || !p->app_table ||
-        !p->bg_table || !p->geo_w || !p->app_w || !p->bg_w)
+    if (!p->geo_table || !p->app_table || !p->bg_table || !p->geo_w || !p->app_w || !p->bg_w)
         return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_upload_params: NULL parameter pointer");
+    // the explicit part may be left out as a whole (it then comes through hyrf_upload_explicit_rvq), not in part
+    const bool no_explicit = !p->pos && !p->rgb_logit && !p->scale_logit && !p->opacity_logit;
+    if (!no_explicit && (!p->pos || !p->rgb_logit || !p->scale_logit || !p->opacity_logit))
+        return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_upload_params: explicit parameters must be all given or all NULL");
     cudaError_t e;
     if ((e = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
     const cudaMemcpyKind kind = p->host_ptrs ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
@@ -351,17 +354,85 @@ extern "C" hyrf_status hyrf_upload_params(hyrf_scene* s, const hyrf_params* p) {
         {(void*)s->app_mlp.w, p->app_w, mlp_weights(s->desc.app_mlp) * esz},
         {(void*)s->bg_mlp.w, p->bg_w, mlp_weights(s->desc.bg_mlp) * esz}};
     for (auto& c : copies)
-        if ((e = cudaMemcpyAsync(c.dst, c.src, c.bytes, kind, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpyAsync(params)");
+        if (c.src && (e = cudaMemcpyAsync(c.dst, c.src, c.bytes, kind, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpyAsync(params)");
     if (s->use_mma) {
         hyrf_status st = hy_field_mma_prepare(s);
         if (st != HYRF_OK) return st;
     }
-    {
+    if (!no_explicit) {
         hyrf_status st = hy_prepare_morton(s);
         if (st != HYRF_OK) return st;
     }
     if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(upload)");
-    s->ready = true;
+    s->fields_ready = true;
+    if (!no_explicit) s->explicit_ready = true;
+    s->ready = s->fields_ready && s->explicit_ready;
+    return HYRF_OK;
+}
+
+// PAPER.md:227-229 (1)-(2): binary16 positions + R-VQ codes -> the scene's fp32 explicit arrays (decode.cu)
+extern "C" hyrf_status hyrf_upload_explicit_rvq(hyrf_scene* s, const hyrf_explicit_rvq* q) {
+    if (!s || !q) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_upload_explicit_rvq: NULL argument");
+    if (!q->pos_h || !q->codes || !q->codebooks) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_upload_explicit_rvq: NULL pointer");
+    if (q->stages < 1 || q->stages > 16) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_upload_explicit_rvq: stages %u outside [1, 16]", q->stages);
+    if (q->codebook_size < 1 || q->codebook_size > 65536)
+        return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_upload_explicit_rvq: codebook_size %u outside [1, 65536]", q->codebook_size);
+    cudaError_t e;
+    if ((e = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
+    const size_t N = s->N, S = q->stages, K = q->codebook_size;
+    const size_t pos_b = 3 * N * sizeof(uint16_t), code_b = S * N * sizeof(uint16_t), book_b = S * K * 5 * sizeof(float);
+    // staging: [first_bad | pad to 256][pos_h][codes][codebooks] (host sources), each part 256-byte aligned
+    auto up = [](size_t b) { return (b + 255) & ~(size_t)255; };
+    const size_t stage_bytes = 256 + (q->host_ptrs ? up(pos_b) + up(code_b) + up(book_b) : 0);
+    uint8_t* stage = nullptr;
+    hyrf_status st = dev_alloc_t(s, &stage, stage_bytes);
+    if (st != HYRF_OK) return st;
+    uint32_t* first_bad = reinterpret_cast<uint32_t*>(stage);
+    const uint16_t *pos_h = q->pos_h, *codes = q->codes;
+    const float* books = q->codebooks;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    uint32_t bad = 0xFFFFFFFFu;
+    auto done = [&](hyrf_status r) {
+        if (ev0) cudaEventDestroy(ev0);
+        if (ev1) cudaEventDestroy(ev1);
+        dev_free(s, stage);
+        return r;
+    };
+    s->explicit_ready = false;
+    s->ready = false;
+    if ((e = cudaMemsetAsync(first_bad, 0xFF, sizeof(uint32_t), s->stream)) != cudaSuccess) return done(hy_cuda_fail(e, "cudaMemsetAsync(first_bad)"));
+    if (q->host_ptrs) {
+        uint8_t* d_pos = stage + 256;
+        uint8_t* d_codes = d_pos + up(pos_b);
+        uint8_t* d_books = d_codes + up(code_b);
+        if ((e = cudaMemcpyAsync(d_pos, q->pos_h, pos_b, cudaMemcpyHostToDevice, s->stream)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(d_codes, q->codes, code_b, cudaMemcpyHostToDevice, s->stream)) != cudaSuccess ||
+            (e = cudaMemcpyAsync(d_books, q->codebooks, book_b, cudaMemcpyHostToDevice, s->stream)) != cudaSuccess)
+            return done(hy_cuda_fail(e, "cudaMemcpyAsync(rvq)"));
+        pos_h = reinterpret_cast<const uint16_t*>(d_pos);
+        codes = reinterpret_cast<const uint16_t*>(d_codes);
+        books = reinterpret_cast<const float*>(d_books);
+    }
+    if ((e = cudaEventCreate(&ev0)) != cudaSuccess || (e = cudaEventCreate(&ev1)) != cudaSuccess) return done(hy_cuda_fail(e, "cudaEventCreate"));
+    cudaEventRecord(ev0, s->stream);
+    if ((st = hy_launch_explicit_decode(s, pos_h, codes, books, (uint32_t)S, (uint32_t)K, first_bad)) != HYRF_OK) return done(st);
+    cudaEventRecord(ev1, s->stream);
+    if ((e = cudaMemcpyAsync(&bad, first_bad, sizeof(bad), cudaMemcpyDeviceToHost, s->stream)) != cudaSuccess) return done(hy_cuda_fail(e, "cudaMemcpyAsync(first_bad)"));
+    if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return done(hy_cuda_fail(e, "cudaStreamSynchronize(decode)"));
+    if (bad != 0xFFFFFFFFu)
+        return done(hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_upload_explicit_rvq: a code of Gaussian %u is >= codebook_size %u", bad, (uint32_t)K));
+    cudaEventElapsedTime(&s->decode_ms, ev0, ev1);
+    if ((st = hy_prepare_morton(s)) != HYRF_OK) return done(st);
+    if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return done(hy_cuda_fail(e, "cudaStreamSynchronize(upload)"));
+    s->explicit_ready = true;
+    s->ready = s->fields_ready && s->explicit_ready;
+    return done(HYRF_OK);
+}
+
+extern "C" hyrf_status hyrf_last_decode_time(hyrf_scene* s, float* ms) {
+    if (!s || !ms) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_last_decode_time: NULL argument");
+    if (s->decode_ms < 0.0f) return hy_fail(HYRF_ERR_NOT_READY, "hyrf_last_decode_time: no hyrf_upload_explicit_rvq yet");
+    *ms = s->decode_ms;
     return HYRF_OK;
 }
 
@@ -405,7 +476,7 @@ hyrf_status build_frame(const hyrf_scene* s, const hyrf_camera* cam, int32_t W, 
 
 hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_t H, float* out_rgb) {
     if (!s || !cam || !out_rgb) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_render: NULL argument");
-    if (!s->ready) return hy_fail(HYRF_ERR_NOT_READY, "hyrf_render before hyrf_upload_params");
+    if (!s->ready) return hy_fail(HYRF_ERR_NOT_READY, "hyrf_render before the fields (hyrf_upload_params) and the explicit Gaussians (hyrf_upload_params or hyrf_upload_explicit_rvq) were uploaded");
     if (W < 1 || H < 1 || (uint32_t)W > s->desc.max_width || (uint32_t)H > s->desc.max_height)
         return hy_fail(HYRF_ERR_INVALID_ARG, "W x H = %d x %d outside [1, %u] x [1, %u]", W, H, s->desc.max_width, s->desc.max_height);
     FrameDev f;
@@ -649,6 +720,23 @@ extern "C" hyrf_status hyrf_debug_enable(hyrf_scene* s, uint32_t mask) {
 
 extern "C" hyrf_status hyrf_debug_fetch(hyrf_scene* s, uint32_t kind, void* host_dst, size_t cap, size_t* bytes) {
     if (!s || !bytes) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_debug_fetch: NULL argument");
+    if (kind == HYRF_DBG_EXPLICIT) {   // what the uploads left in the scene: p_e[3], s_e, alpha_e, c_e[3], one row each
+        if (!s->explicit_ready) return hy_fail(HYRF_ERR_NOT_READY, "hyrf_debug_fetch: no explicit parameters uploaded");
+        const size_t row = (size_t)s->N * sizeof(float);
+        *bytes = 8 * row;
+        if (!host_dst) return HYRF_OK;
+        if (8 * row > cap) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_debug_fetch: need %zu bytes, cap %zu", 8 * row, cap);
+        cudaError_t ce;
+        if ((ce = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(ce, "cudaSetDevice");
+        if ((ce = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(ce, "cudaStreamSynchronize(debug)");
+        uint8_t* o = static_cast<uint8_t*>(host_dst);
+        if ((ce = cudaMemcpy(o, s->pos, 3 * row, cudaMemcpyDeviceToHost)) != cudaSuccess ||
+            (ce = cudaMemcpy(o + 3 * row, s->scale, row, cudaMemcpyDeviceToHost)) != cudaSuccess ||
+            (ce = cudaMemcpy(o + 4 * row, s->opac, row, cudaMemcpyDeviceToHost)) != cudaSuccess ||
+            (ce = cudaMemcpy(o + 5 * row, s->rgb, 3 * row, cudaMemcpyDeviceToHost)) != cudaSuccess)
+            return hy_cuda_fail(ce, "cudaMemcpy(explicit)");
+        return HYRF_OK;
+    }
     if (!s->rendered) return hy_fail(HYRF_ERR_NOT_READY, "hyrf_debug_fetch: no completed render");
     cudaError_t e;
     if ((e = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");

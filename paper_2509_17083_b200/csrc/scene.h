@@ -30,7 +30,10 @@ struct FrameCounters {
 struct hyrf_scene {
     hyrf_scene_desc desc;
     std::vector<uint32_t> res_geo, res_app, res_bg;
-    bool ready = false;
+    bool ready = false;          // fields_ready && explicit_ready
+    bool fields_ready = false;   // tables and decoder weights uploaded (hyrf_upload_params)
+    bool explicit_ready = false; // explicit Gaussians uploaded (hyrf_upload_params or hyrf_upload_explicit_rvq)
+    float decode_ms = -1.0f;     // decode kernel of the last hyrf_upload_explicit_rvq
     bool fp16 = false;         // decoder weights / activations in fp16 (param_dtype F16 or U8)
     bool u8 = false;           // grid tables are 8-bit min-max codes (param_dtype U8)
     bool use_mma = false;
@@ -122,6 +125,9 @@ hyrf_status hy_fail(hyrf_status st, const char* fmt, ...);
 hyrf_status hy_cuda_fail(cudaError_t e, const char* what);
 
 // ---- launchers (each returns the number of kernels it enqueued through *launches) -------------------------
+// decode of the compressed explicit Gaussians at upload (decode.cu); *first_bad must hold 0xFFFFFFFF
+hyrf_status hy_launch_explicit_decode(hyrf_scene* s, const uint16_t* pos_h, const uint16_t* codes,
+                                      const float* codebooks, uint32_t S, uint32_t K, uint32_t* first_bad);
 // S1 (cull.cu): visibility bits, stable compactions -> vis_m (Morton work list), vis_idx + rank lookup (id order)
 hyrf_status hy_prepare_morton(hyrf_scene* s);
 void hy_launch_cull(hyrf_scene* s, const FrameDev& f, uint32_t* launches);

@@ -324,9 +324,10 @@ def compress_explicit(scene: Scene, stages: int = 6, codebook_size: int = 64, se
     def nearest(x: np.ndarray, book: np.ndarray) -> np.ndarray:
         out = np.zeros(len(x), np.int64)
         b2 = (book.astype(np.float64) ** 2).sum(1)
-        for a in range(0, len(x), 65536):
-            blk = x[a:a + 65536].astype(np.float64)
-            out[a:a + 65536] = np.argmin(b2[None, :] - 2.0 * blk @ book.astype(np.float64).T, axis=1)
+        step = max(1, (1 << 22) // len(book))
+        for a in range(0, len(x), step):
+            blk = x[a:a + step].astype(np.float64)
+            out[a:a + step] = np.argmin(b2[None, :] - 2.0 * blk @ book.astype(np.float64).T, axis=1)
         return out
 
     for st in range(stages):

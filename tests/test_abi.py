@@ -30,15 +30,15 @@ def test_every_declared_symbol_is_exported(lib):
 def test_struct_layouts_match_header_sizes():
     # sizes computed by the C compiler from the header itself
     from paper_2509_17083_b200 import binding
-    src = ('#include "hyrf.h"\n#include <stdio.h>\nint main(){printf("%zu %zu %zu %zu %zu\\n", '
+    src = ('#include "hyrf.h"\n#include <stdio.h>\nint main(){printf("%zu %zu %zu %zu %zu %zu\\n", '
            'sizeof(hyrf_scene_desc), sizeof(hyrf_params), sizeof(hyrf_camera), sizeof(hyrf_grid_desc), '
-           'sizeof(hyrf_mlp_desc));return 0;}')
+           'sizeof(hyrf_mlp_desc), sizeof(hyrf_explicit_rvq));return 0;}')
     exe = "/tmp/hyrf_sizes"
     subprocess.run(["gcc", "-x", "c", "-I", os.path.join(ROOT, "include"), "-o", exe, "-"], input=src.encode(),
                    check=True)
     sizes = [int(x) for x in subprocess.run([exe], capture_output=True, check=True).stdout.split()]
     assert sizes == [C.sizeof(binding.SceneDesc), C.sizeof(binding.Params), C.sizeof(binding.CameraC),
-                     C.sizeof(binding.GridDesc), C.sizeof(binding.MlpDesc)]
+                     C.sizeof(binding.GridDesc), C.sizeof(binding.MlpDesc), C.sizeof(binding.ExplicitRvqC)]
 
 
 def test_argument_validation_without_device(lib, synth):
@@ -107,3 +107,12 @@ def test_camera_sharding_world2_gloo(tmp_path):
                         "--master-addr", "127.0.0.1", "--master-port", "29513", str(script)],
                        capture_output=True, text=True, env=env, timeout=300)
     assert r.returncode == 0, r.stdout + r.stderr
+
+
+def test_explicit_rvq_argument_validation_without_device(lib):
+    from paper_2509_17083_b200 import binding as B
+    q = B.ExplicitRvqC()
+    assert lib.hyrf_upload_explicit_rvq(None, C.byref(q)) == B.HYRF_ERR_INVALID_ARG
+    assert lib.hyrf_upload_explicit_rvq(None, None) == B.HYRF_ERR_INVALID_ARG
+    ms = C.c_float(0)
+    assert lib.hyrf_last_decode_time(None, C.byref(ms)) == B.HYRF_ERR_INVALID_ARG

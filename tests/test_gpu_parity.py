@@ -329,3 +329,85 @@ def test_quantised_tables_tensor_path(B, ho, synth):
         err = np.abs(raw - ref)
         assert err.max() < 2e-2 and err.mean() < 1e-3, (path, err.max(), err.mean())
         hs.close()
+
+
+def _decoded_rows(ho, rvq):
+    d = ho.decode_explicit(rvq)
+    return np.concatenate([d["pos"], d["scale_logit"][None], d["opacity_logit"][None], d["rgb_logit"]])
+
+
+@pytest.mark.parametrize("n,stages,K,host", [(4096, 6, 64, False), (4099, 3, 17, True), (1, 1, 1, True),
+                                             (50_000, 2, 4096, False), (30_001, 16, 5, False)])
+def test_explicit_rvq_decode_bit_exact(B, ho, synth, n, stages, K, host):
+    # compressed explicit Gaussians (PAPER.md:227-229 (1)-(2)): the decode kernel against the
+    # oracle's decode, bit for bit: vectorised (n % 4 == 0) and scalar (ragged n) variants, codebooks in shared memory
+    # and beyond 48 KB (2 x 4096 x 20 B), host and device sources, the 16-stage maximum, a single Gaussian
+    s = synth.compress_explicit(synth.make_scene(1, n_gaussians=n, n_cameras=1), stages=stages, codebook_size=K, seed=n)
+    if stages == 16:                                   # make the order of the additions matter in every row
+        s.explicit_rvq.codebooks[0] += np.float32(1e6)
+        s.explicit_rvq.codebooks[1] -= np.float32(1e6)
+    hs = B.HyrfScene(s, host_upload=host)
+    got = hs.explicit_params()
+    want = _decoded_rows(ho, s.explicit_rvq)
+    assert (got.view(np.uint32) == want.view(np.uint32)).all()
+    assert hs.last_decode_time() > 0.0
+    hs.close()
+
+
+def test_explicit_rvq_every_half_pattern_and_rejection(B, ho, synth):
+    import copy
+    base = synth.make_scene(1, n_gaussians=63488, n_cameras=1)           # 63488 = number of finite binary16 patterns
+    s = synth.compress_explicit(base, stages=2, codebook_size=8)
+    bits = np.arange(65536, dtype=np.uint16)
+    bits = bits[(bits & 0x7C00) != 0x7C00]
+    s.explicit_rvq.pos_h = np.stack([bits, bits[::-1], np.roll(bits, 7)])
+    hs = B.HyrfScene(s)
+    got = hs.explicit_params()
+    assert (got.view(np.uint32) == _decoded_rows(ho, s.explicit_rvq).view(np.uint32)).all()
+    # a code outside the codebook is refused, names its Gaussian, and leaves the scene not renderable
+    bad = copy.copy(s.explicit_rvq)
+    bad.codes = s.explicit_rvq.codes.copy()
+    bad.codes[1, 12345] = 8
+    bad.codes[0, 40000] = 9
+    with pytest.raises(B.HyrfError) as e:
+        hs.upload_explicit_rvq(bad)
+    assert e.value.status == B.HYRF_ERR_INVALID_ARG and "12345" in str(e.value)
+    with pytest.raises(B.HyrfError) as e:
+        hs.render(base.cameras[0])
+    assert e.value.status == B.HYRF_ERR_NOT_READY
+    hs.upload_explicit_rvq(s.explicit_rvq)                                # and recovers with a valid upload
+    assert (hs.explicit_params().view(np.uint32) == got.view(np.uint32)).all()
+    hs.close()
+
+
+def test_compressed_model_render_exact_path(B, ho, synth):
+    # the whole compressed model of PAPER.md:227-229: binary16 positions + R-VQ properties + 8-bit tables, rendered
+    # through the exact decoders: every stage bit-exact against the oracle rendering the same compressed scene
+    s = synth.make_scene(3, n_gaussians=40_000, width=320, height=180, n_cameras=2, table_amp=0.5)
+    st = _run(B, ho, synth.compress_explicit(synth.quantize8(s)))
+    assert st[0]["D"] > 0
+    _run(B, ho, synth.compress_explicit(synth.tiny_scene(n=61, W=48, H=40, seed=5), stages=4, codebook_size=16))
+    _run(B, ho, synth.compress_explicit(synth.make_scene(2, n_gaussians=20_000, width=200, height=136, n_cameras=2)))
+
+
+def test_compressed_model_render_tensor_path(B, ho, synth):
+    s = synth.compress_explicit(synth.quantize8(synth.make_scene(3, n_gaussians=40_000, width=320, height=180, n_cameras=2)))
+    _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False)
+
+
+def test_fields_then_explicit_upload_order(B, ho, synth):
+    # plain explicit arrays first, then replaced by the compressed ones: the render follows the last upload
+    import torch
+    plain = synth.tiny_scene(n=64, W=32, H=32)
+    comp = synth.compress_explicit(plain, stages=2, codebook_size=4)
+    hs = B.HyrfScene(plain)
+    a = hs.render(plain.cameras[0]).cpu().numpy()
+    hs.upload_explicit_rvq(comp.explicit_rvq)
+    b = hs.render(plain.cameras[0]).cpu().numpy()
+    torch.cuda.synchronize()
+    assert not (a == b).all()
+    want = ho.render(ho.OracleScene(comp), comp.cameras[0])["out"]
+    assert np.abs(b - want).mean() <= 1e-4 and (np.abs(b - want) <= 2e-3).mean() > 0.99
+    hs.upload(plain)                                                       # and back
+    assert (hs.render(plain.cameras[0]).cpu().numpy() == a).all()
+    hs.close()
