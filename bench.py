@@ -116,10 +116,15 @@ def workload(cfg: int, args):
     scene = synth.make_scene(cfg, **kw)
     if args.quant8:
         scene = synth.quantize8(scene)
+    if args.rvq:
+        scene = synth.compress_explicit(scene, lloyd_iters=1)
     cam = scene.cameras[0]
     name = (f"BASELINE.json configs[{cfg - 1}]: {scene.n} Gaussians, "
             f"{'8-bit tables + fp16 MLPs (compressed model)' if scene.quant8 else ('fp16' if scene.fp16 else 'fp32') + ' grids/MLPs'}, "
             f"{cam.W}x{cam.H}, {len(scene.cameras)} cameras")
+    if scene.explicit_rvq is not None:
+        q = scene.explicit_rvq
+        name += f"; explicit part compressed (binary16 positions, R-VQ {q.stages} x {q.codebook_size}), decoded at upload"
     return scene, name
 
 
@@ -209,6 +214,8 @@ def run_reference(args):
     seq = [cams[i % len(cams)] for i in range(warm + steps)]
     from oracle import hyrf_oracle as ho
     ho.build()
+    if args.cpu_threads:
+        ho.set_num_threads(args.cpu_threads)     # 1 = the single-thread baseline of SURVEY §8(d); 0 = every host core
     osc = ho.OracleScene(scene)
     for cam in seq[:warm]:
         ho.render(osc, cam)
@@ -232,6 +239,7 @@ def run_reference(args):
 
 
 def run_ours(args):
+    import numpy as np
     import torch
     from paper_2509_17083_b200 import binding as B
     from paper_2509_17083_b200 import synth
@@ -254,6 +262,24 @@ def run_ours(args):
     path = {"auto": B.HYRF_MLP_AUTO, "fma": B.HYRF_MLP_FMA, "mma": B.HYRF_MLP_MMA, "hmma": B.HYRF_MLP_HMMA}[args.mlp]
     hs = B.HyrfScene(scene, device=dev, mlp_path=path)
     hs.set_ablation(args.ablation)
+    upload = None
+    if scene.explicit_rvq is not None:
+        # the decode is an upload-time kernel (csrc/decode.cu), not part of a frame: timed on its own, device sources,
+        # L2 flushed before each repetition; algorithmic bytes per Gaussian = 6 (binary16 position) + 2 S (codes) + 32 out
+        q = scene.explicit_rvq
+        flush0 = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{dev}")
+        ts = []
+        for _ in range(7):
+            flush0.fill_(1)
+            hs.upload_explicit_rvq(q)
+            ts.append(hs.last_decode_time())
+        del flush0
+        ms = float(np.median(ts[2:]))
+        work = scene.n * (6 + 2 * q.stages + 32)
+        plain = scene.n * 32
+        upload = {"kernel": "explicit_decode_kernel", "decode_ms": ms, "bound": "hbm", "achieved": work / (ms * 1e-3) / 1e9,
+                  "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": work / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                  "explicit_bytes_compressed": q.nbytes(), "explicit_bytes_fp32": plain}
     W, H = cams[0].W, cams[0].H
     out = torch.empty((H, W, 3), dtype=torch.float32, device=f"cuda:{dev}")
     cstructs = [B.camera_struct(c) for c in cams]
@@ -406,6 +432,8 @@ def run_ours(args):
             "gpu_launches": launches, "clocks": clocks, "roofline": roof, "stage_rooflines": per_stage}
     if cpu:
         line["cpu_baseline"] = cpu
+    if upload:
+        line["upload_decode"] = upload
     print(json.dumps(line), flush=True)
 
 
@@ -424,8 +452,12 @@ def main():
                     help="hyrf_ablation bits (PAPER.md Table 5): 1 no pre-culling, 2 no background, 4 no neural, 8 no explicit")
     ap.add_argument("--quant8", action="store_true",
                     help="compressed model: 8-bit min-max tables decoded in the gather (PAPER.md:229)")
+    ap.add_argument("--rvq", action="store_true",
+                    help="compressed explicit Gaussians: binary16 positions + R-VQ codes decoded at upload (PAPER.md:229 (1)-(2))")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--cpu-threads", type=int, default=0,
+                    help="--impl reference: OpenMP threads of the oracle (0 = all host cores, 1 = single-thread baseline)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

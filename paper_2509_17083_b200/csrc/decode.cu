@@ -95,7 +95,7 @@ explicit_decode_kernel(const uint16_t* __restrict__ pos_h, const uint16_t* __res
 }  // namespace
 
 // Enqueues the decode on the scene's stream. first_bad (device u32) must hold 0xFFFFFFFF; afterwards it holds the
-// smallest Gaussian index with a code >= K, if any. sm_count sizes the grid (a multiple of the SM count).
+// smallest Gaussian index with a code >= K, if any. Grid: the SM count x the resident CTAs per SM.
 hyrf_status hy_launch_explicit_decode(hyrf_scene* s, const uint16_t* pos_h, const uint16_t* codes,
                                       const float* codebooks, uint32_t S, uint32_t K, uint32_t* first_bad) {
     const uint32_t n = s->N;
@@ -108,7 +108,10 @@ hyrf_status hy_launch_explicit_decode(hyrf_scene* s, const uint16_t* pos_h, cons
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const uint32_t groups = vec4 ? n / 4 : n;
     const uint32_t want = (groups + kDecodeThreads - 1) / kDecodeThreads;
-    const uint32_t cap = (uint32_t)sms * 8u;   // 8 resident CTAs of 256 threads per SM: one wave, grid-stride beyond
+    int per_sm = 1;   // one wave of resident CTAs, grid-stride beyond
+    if (vec4) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, explicit_decode_kernel<4>, kDecodeThreads, smem);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, explicit_decode_kernel<1>, kDecodeThreads, smem);
+    const uint32_t cap = (uint32_t)sms * (uint32_t)(per_sm > 0 ? per_sm : 1);
     const uint32_t grid = want < cap ? (want ? want : 1u) : cap;
     if (vec4)
         explicit_decode_kernel<4><<<grid, kDecodeThreads, smem, s->stream>>>(pos_h, codes, codebooks, n, S, K, in_smem,

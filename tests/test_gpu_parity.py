@@ -411,3 +411,84 @@ def test_fields_then_explicit_upload_order(B, ho, synth):
     hs.upload(plain)                                                       # and back
     assert (hs.render(plain.cameras[0]).cpu().numpy() == a).all()
     hs.close()
+
+
+def test_config5_largest_point_sampled(B, ho, synth):
+    # BASELINE config 5's largest point (4M Gaussians at 3840x2160, D ~ 4e8 tile entries) in the launch configuration
+    # bench.py --config 5 times (AUTO decoders, macro-tile binning, per-tile lists NOT materialised). The oracle cannot
+    # bin 4e8 entries in seconds, so: cull element by element; stages 2-4a on 4096 sampled Gaussians; stages 4b-5 on
+    # 24 sampled tiles whose depth-ordered lists are rebuilt one by one from the exported records (hand-off)
+    # and rasterised by the oracle; stage 6 on the whole image from the exported (C_fg, T); properties everywhere.
+    import torch
+    s = synth.make_scene(5, n_gaussians=4_000_000, width=3840, height=2160)
+    cam = s.cameras[0]
+    W, H = cam.W, cam.H
+    hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_AUTO)
+    hs.debug_enable(B.DBG_ALL & ~((1 << B.DBG_TILE_LIST) | (1 << B.DBG_TILE_RANGES)))
+    out = hs.render(cam)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    osc = ho.OracleScene(s)
+    mask, vis = ho.stage_cull(osc, cam, W, H)
+    assert (hs.debug_fetch(B.DBG_VIS_MASK) == mask).all()
+    assert (hs.debug_fetch(B.DBG_VIS_IDX) == vis).all()
+    V = len(vis)
+    assert V > 3_000_000
+    proj, rect = hs.debug_fetch(B.DBG_PROJ), hs.debug_fetch(B.DBG_RECT)
+    cnt = hs.debug_fetch(B.DBG_COUNTERS)
+    r64 = rect.astype(np.int64)
+    tiles = np.where((r64[:, 1] > r64[:, 0]) & (r64[:, 3] > r64[:, 2]), (r64[:, 1] - r64[:, 0]) * (r64[:, 3] - r64[:, 2]), 0)
+    assert int(cnt[1]) == V and int(cnt[2]) == int(tiles.sum())
+    # stages 2-4a on a sample
+    rng = np.random.default_rng(5)
+    pick = np.sort(rng.choice(V, 4096, replace=False))
+    raw_o = ho.stage_query(osc, cam, vis[pick])
+    at_o = ho.stage_aggregate(osc, vis[pick], raw_o)
+    pr_o = ho.stage_project(osc, cam, W, H, vis[pick], at_o)
+    assert np.abs(hs.debug_fetch(B.DBG_STAGE2_RAW)[pick] - raw_o).max() <= 2e-3
+    assert np.abs(hs.debug_fetch(B.DBG_STAGE3_ATTRS)[pick] - at_o).max() <= 2e-3
+    live = pr_o["tiles"] > 0
+    assert (proj[pick][live][:, :3].view(np.uint32) == pr_o["proj"][live][:, :3].view(np.uint32)).all()   # u, v, depth: no field input
+    assert np.allclose(proj[pick][live][:, 3:], pr_o["proj"][live][:, 3:], rtol=5e-3, atol=2e-3)
+    assert (rect[pick] == pr_o["rect"]).mean() > 0.995           # a rectangle edge can move by one tile under 1e-4 noise
+    # stages 4b-5 on sampled tiles (hand-off from the exported records)
+    gx, gy = (W + 15) // 16, (H + 15) // 16
+    depth_bits = np.ascontiguousarray(proj[:, 2]).view(np.uint32)
+    ranges = np.zeros((gx * gy, 2), np.uint32)
+    lists, pos, sampled = [], 0, []
+    cx, cy = gx // 2, gy // 2
+    cand = [(cx, cy), (cx - 7, cy + 3), (0, 0), (gx - 1, gy - 1), (gx - 1, 0)] + \
+           [(int(rng.integers(gx // 4, 3 * gx // 4)), int(rng.integers(gy // 4, 3 * gy // 4))) for _ in range(19)]
+    for tx, ty in cand:
+        t = ty * gx + tx
+        if t in sampled:
+            continue
+        mem = np.nonzero((tiles > 0) & (rect[:, 0] <= tx) & (tx < rect[:, 1]) & (rect[:, 2] <= ty) & (ty < rect[:, 3]))[0]
+        mem = mem[np.argsort(depth_bits[mem], kind="stable")]        # ranks ascend with ids: ties fall to the id
+        ranges[t] = (pos, pos + len(mem))
+        lists.append(mem.astype(np.uint32))
+        pos += len(mem)
+        sampled.append(t)
+    assert pos > 10_000
+    rs = ho.stage_raster(W, H, proj, np.concatenate(lists), ranges)
+    fg, T = hs.debug_fetch(B.DBG_FG).reshape(H, W, 3), hs.debug_fetch(B.DBG_FINAL_T).reshape(H, W)
+    assert np.isfinite(out).all() and (T >= 0).all() and (T <= 1).all()
+    n_px = n_fragile = 0
+    for t in sampled:
+        ty, tx = divmod(t, gx)
+        sl = (slice(ty * 16, min(ty * 16 + 16, H)), slice(tx * 16, min(tx * 16 + 16, W)))
+        fragile = (rs["m_alpha"][sl] < 5e-8) | (rs["m_stop"][sl] < 5e-5)
+        d = np.abs(fg[sl] - rs["cfg"][sl]).max(axis=-1)
+        dT = np.abs(T[sl] - rs["T"][sl])
+        assert d[~fragile].max(initial=0.0) <= 2e-3 and dT[~fragile].max(initial=0.0) <= 2e-3, (tx, ty, d.max(), dT.max())
+        assert d.max() <= 2e-3 + 1.0 / 255.0 + 1e-2
+        n_px += fragile.size
+        n_fragile += int(fragile.sum())
+    assert n_fragile < 0.01 * n_px
+    # stage 6 on the whole image, from the exported foreground and transmittance
+    want, bgm = ho.stage_background(osc, cam, W, H, fg, T)
+    near_tau = np.abs(T - np.float32(s.tau_T)) < 1e-5
+    assert (hs.debug_fetch(B.DBG_BG_MASK).reshape(H, W).astype(bool)[~near_tau] == bgm.astype(bool)[~near_tau]).all()
+    assert np.abs(out - want)[~near_tau].max() <= 1e-2
+    assert np.abs(out - want)[~near_tau].mean() <= 1e-4
+    hs.close()
