@@ -262,6 +262,7 @@ def run_ours(args):
     path = {"auto": B.HYRF_MLP_AUTO, "fma": B.HYRF_MLP_FMA, "mma": B.HYRF_MLP_MMA, "hmma": B.HYRF_MLP_HMMA}[args.mlp]
     hs = B.HyrfScene(scene, device=dev, mlp_path=path)
     hs.set_ablation(args.ablation)
+    hs.set_raster_mode({"auto": 0, "tile": 1, "warp": 2}[args.raster])
     upload = None
     if scene.explicit_rvq is not None:
         # the decode is an upload-time kernel (csrc/decode.cu), not part of a frame: timed on its own, device sources,
@@ -390,7 +391,7 @@ def run_ours(args):
         return
     names = ["cull", "field", "bin", "raster", "background"]
     kernels = {"field": ("field_warp_kernel" if args.mlp == "hmma" else "field_mma_pipe_kernel") if scene.fp16 and args.mlp != "fma"
-               else "field_fma_kernel", "raster": "raster_kernel"}
+               else "field_fma_kernel", "raster": "raster_warp_kernel" if hs.last_raster_mode() == 2 else "raster_kernel"}
     eval_pairs = None
     cpu = None
     if world == 1 and not args.no_cpu and args.ablation == 0:
@@ -420,7 +421,7 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f16" if scene.fp16 else "f32", "data": "synthetic",
-            "config": {"workload": name, "l2": "flushed between steps (256 MiB write)", "mlp_path": args.mlp, "ablation": args.ablation,
+            "config": {"workload": name, "l2": "flushed between steps (256 MiB write)", "mlp_path": args.mlp, "ablation": args.ablation, "raster": args.raster,
                        "schedule": "depth sort on a second stream beside the field kernel (hyrf_set_sort_overlap default)",
                        "parallelism": f"replicas x{world} (cameras round-robin)"},
             "visible_gaussians_per_s": vis_per_s, "V_mean": Vm, "D_mean": Dm, "Dm_mean": Dmm,
@@ -452,6 +453,8 @@ def main():
                     help="hyrf_ablation bits (PAPER.md Table 5): 1 no pre-culling, 2 no background, 4 no neural, 8 no explicit")
     ap.add_argument("--quant8", action="store_true",
                     help="compressed model: 8-bit min-max tables decoded in the gather (PAPER.md:229)")
+    ap.add_argument("--raster", default="auto", choices=["auto", "tile", "warp"],
+                    help="hyrf_set_raster_mode: per-frame choice (default), tile-level lists only, per-warp lists")
     ap.add_argument("--rvq", action="store_true",
                     help="compressed explicit Gaussians: binary16 positions + R-VQ codes decoded at upload (PAPER.md:229 (1)-(2))")
     ap.add_argument("--no-cpu", action="store_true")

@@ -229,6 +229,15 @@ hyrf_status hyrf_set_ablation(hyrf_scene* scene, uint32_t mask);
  * every debug export are identical either way. */
 hyrf_status hyrf_set_sort_overlap(hyrf_scene* scene, int on);
 
+/* Rasterizer variant (S5; Eq. 1). Both variants stage a tile's depth-ordered list once per tile and
+ * produce the same bits; they differ in cost. mode 1: every warp of the tile blends every staged entry. mode 2: a warp
+ * owns an 8 x 4 pixel block and blends only the entries that can reach alpha >= 1/255 somewhere in its block (per-warp
+ * lists built while staging) — faster when splats cover few tiles. mode 0 (default): chosen per frame from the tiles
+ * touched per visible Gaussian of the previous frame. HYRF_ERR_INVALID_ARG for any other mode. */
+hyrf_status hyrf_set_raster_mode(hyrf_scene* scene, int mode);
+/* The variant (1 or 2) the last render used. */
+hyrf_status hyrf_last_raster_mode(hyrf_scene* scene, int* mode);
+
 /* Number of kernels the last render launched (for bench.py's gpu_launches). */
 hyrf_status hyrf_last_launch_count(hyrf_scene* scene, uint32_t* launches);
 

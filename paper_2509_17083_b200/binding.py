@@ -28,7 +28,8 @@ DBG_ALL = (1 << 12) - 1
 EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_render", "hyrf_render_host",
            "hyrf_destroy_scene", "hyrf_last_error", "hyrf_debug_enable", "hyrf_debug_fetch", "hyrf_set_timing",
            "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation", "hyrf_render_host_async",
-           "hyrf_host_sync", "hyrf_set_sort_overlap", "hyrf_upload_explicit_rvq", "hyrf_last_decode_time"]
+           "hyrf_host_sync", "hyrf_set_sort_overlap", "hyrf_upload_explicit_rvq", "hyrf_last_decode_time", "hyrf_set_raster_mode",
+           "hyrf_last_raster_mode"]
 ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
 
 
@@ -109,6 +110,8 @@ def load_library() -> C.CDLL:
         L.hyrf_host_sync.argtypes = [vp]
         L.hyrf_upload_explicit_rvq.argtypes = [vp, C.POINTER(ExplicitRvqC)]
         L.hyrf_last_decode_time.argtypes = [vp, C.POINTER(C.c_float)]
+        L.hyrf_set_raster_mode.argtypes = [vp, C.c_int]
+        L.hyrf_last_raster_mode.argtypes = [vp, C.POINTER(C.c_int)]
         for name in EXPORTS:
             if name != "hyrf_last_error":
                 getattr(L, name).restype = C.c_int
@@ -332,6 +335,15 @@ class HyrfScene:
     def set_sort_overlap(self, on: bool = True) -> None:
         """Depth sort beside the field query on a second stream (default) or the whole frame serialised (include/hyrf.h)."""
         _check(self.lib.hyrf_set_sort_overlap(self.handle, int(on)))
+
+    def set_raster_mode(self, mode: int = 0) -> None:
+        """0 auto, 1 tile-level lists only, 2 per-warp lists (include/hyrf.h hyrf_set_raster_mode); same bits, different cost."""
+        _check(self.lib.hyrf_set_raster_mode(self.handle, int(mode)))
+
+    def last_raster_mode(self) -> int:
+        m = C.c_int(0)
+        _check(self.lib.hyrf_last_raster_mode(self.handle, C.byref(m)))
+        return int(m.value)
 
     def set_timing(self, on: bool = True) -> None:
         _check(self.lib.hyrf_set_timing(self.handle, int(on)))

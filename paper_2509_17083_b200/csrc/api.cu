@@ -429,6 +429,20 @@ extern "C" hyrf_status hyrf_upload_explicit_rvq(hyrf_scene* s, const hyrf_explic
     return done(HYRF_OK);
 }
 
+extern "C" hyrf_status hyrf_set_raster_mode(hyrf_scene* s, int mode) {
+    if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_raster_mode: NULL scene");
+    if (mode < 0 || mode > 2) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_raster_mode: mode %d outside [0, 2]", mode);
+    s->raster_mode = mode;
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_last_raster_mode(hyrf_scene* s, int* mode) {
+    if (!s || !mode) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_last_raster_mode: NULL argument");
+    if (!s->rendered) return hy_fail(HYRF_ERR_NOT_READY, "hyrf_last_raster_mode: no completed render");
+    *mode = s->last_raster_mode;
+    return HYRF_OK;
+}
+
 extern "C" hyrf_status hyrf_last_decode_time(hyrf_scene* s, float* ms) {
     if (!s || !ms) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_last_decode_time: NULL argument");
     if (s->decode_ms < 0.0f) return hy_fail(HYRF_ERR_NOT_READY, "hyrf_last_decode_time: no hyrf_upload_explicit_rvq yet");

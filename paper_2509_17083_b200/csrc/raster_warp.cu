@@ -1,11 +1,11 @@
-// raster.cu — S5: front-to-back alpha blending, Eq. 1, per 16x16 tile over its depth-ordered list.
-// Arithmetic DESIGN.md §2 D10 (constants of the 3DGS rasterizer the paper defers to).
-// One CTA per tile, one thread per pixel; list entries are staged through shared memory in batches of 256 so each
-// projected record is fetched once per tile, and entries that cannot reach alpha >= 1/255 anywhere in the tile are
-// dropped while staging (stable compaction, so the order is untouched). The per-pair body is branch-free
-// (profiles/r1a: divergent skip/stop branches cost 45 issue slots per pair against ~30 predicated); warps stop
-// when all of their pixels have terminated, the CTA when all warps have. Bound by plain fp32 ALU issue + one
-// MUFU.EX2 per pair — no tensor cores (nothing here is a dense contraction).
+// raster_warp.cu — S5, per-warp-list variant of the rasterizer in raster.cu (same arithmetic, DESIGN.md §2 D10; same
+// staging of a tile's depth-ordered list). Here a warp owns an 8 x 4 pixel block of the 16 x 16 tile and blends only the
+// staged entries that can reach alpha >= 1/255 somewhere in ITS block: while staging, every entry gets an 8-bit mask
+// (one convex minimisation of the conic's quadratic form per block, as for the tile), and each warp compacts the
+// byte offsets of its entries into its own list. About a third of the (warp, entry) combinations of a tile never get
+// there when splats cover ~10 tiles (config 3); with large splats nearly every block is reached and raster.cu's kernel
+// (no indirection, no masks) is faster — hy_launch_raster picks per frame. Dropped combinations are exactly
+// those every pixel of the block would skip, so no output bit changes.
 #include "scene.h"
 
 namespace {
@@ -34,6 +34,28 @@ __device__ __forceinline__ bool entry_reaches_tile(float u, float v, float A, fl
     return !(o * __expf(-0.5f * qmin) < 0.99f / 255.0f);   // NaN keeps the entry
 }
 
+// The same test for a sub-rectangle of the tile, with the per-entry work hoisted: iA = 1 / A, iC = 1 / C,
+// qthr = 2 ln(o * 255 / 0.99) (alpha >= 0.99 / 255  <=>  q <= qthr). NaN keeps the entry.
+__device__ __forceinline__ bool entry_reaches_block(float u, float v, float A, float B, float C, float iA, float iC,
+                                                    float qthr, float X0, float X1, float Y0, float Y1) {
+    const float ex = fminf(fmaxf(u, X0), X1) - u, ey = fminf(fmaxf(v, Y0), Y1) - v;
+    if (ex == 0.0f && ey == 0.0f) return true;
+    float qmin = 3.0e38f;
+    if (ex != 0.0f) {
+        const float dy = fminf(fmaxf(-B * ex * iC, Y0 - v), Y1 - v);
+        qmin = A * ex * ex + 2.0f * B * ex * dy + C * dy * dy;
+    }
+    if (ey != 0.0f) {
+        const float dx = fminf(fmaxf(-B * ey * iA, X0 - u), X1 - u);
+        qmin = fminf(qmin, A * dx * dx + 2.0f * B * dx * ey + C * ey * ey);
+    }
+    return !(qmin > qthr);
+}
+
+constexpr int kBlockW = 8, kBlockH = 4;            // pixel block of one warp inside the 16 x 16 tile
+constexpr uint32_t kNullSlot = 2 * kBatch;         // staged slot holding a null record (opacity 0 -> alpha 0 -> skipped)
+constexpr uint32_t kRecBytes = 48;                 // staged record: (u, v, A, B), (C, opacity, r, g), (b, -, -, -)
+
 // exp2 on the MUFU, flushing subnormal results to 0 (they are far below the 1/255 skip threshold anyway)
 __device__ __forceinline__ float ex2_ftz(float x) {
     float y;
@@ -42,14 +64,14 @@ __device__ __forceinline__ float ex2_ftz(float x) {
 }
 
 __global__ void __launch_bounds__(kBatch)
-raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ list, const float4* __restrict__ rec,
+raster_warp_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ list, const float4* __restrict__ rec,
               int W, int H, int gx, float tau_T, float* __restrict__ out_rgb, float* __restrict__ finalT,
               uint32_t* __restrict__ bg_list, FrameCounters* __restrict__ counters, uint8_t* __restrict__ bg_mask,
               float* __restrict__ dbg_fg, const uint32_t* __restrict__ tile_queue, const uint4* __restrict__ rect,
               int mshift, int mgx, uint32_t* __restrict__ dbg_list, const uint2* __restrict__ dbg_ranges) {
-    __shared__ float4 s_r0[2 * kBatch + 8];   // (u, v, A, B)   (+ 8: padding to a multiple of 8)
-    __shared__ float4 s_r1[2 * kBatch + 8];   // (C, opacity, r, g)
-    __shared__ float s_b[2 * kBatch + 8];
+    __shared__ float4 s_rec[3 * (2 * kBatch + 1)];                      // staged records, 48 B each; slot kNullSlot is the null record
+    __shared__ __align__(16) uint16_t s_widx[kWarps][2 * kBatch + 8];   // per warp: byte offsets of the records it blends
+    __shared__ uint8_t s_mask[2 * kBatch];    // per staged record: bit w set when warp w's pixel block can reach it
     __shared__ uint32_t s_ids[2 * kBatch];    // ids waiting for stage B
     __shared__ uint32_t s_wcnt[kWarps];
     __shared__ uint32_t s_hcnt[kWarps];
@@ -57,8 +79,8 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
     const int tile = tile_queue ? (int)tile_queue[blockIdx.x] : (int)blockIdx.x;
     const int tx = tile % gx, ty = tile / gx;
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const int px = tx * HY_TILE + (threadIdx.x & (HY_TILE - 1));
-    const int py = ty * HY_TILE + (threadIdx.x >> 4);
+    const int px = tx * HY_TILE + (int)(warp & 1u) * kBlockW + (int)(lane & 7u);
+    const int py = ty * HY_TILE + (int)(warp >> 1) * kBlockH + (int)(lane >> 3);
     const bool inside = px < W && py < H;
     const float fi = (float)px, fj = (float)py;
     const float X0 = (float)(tx * HY_TILE), Y0 = (float)(ty * HY_TILE);
@@ -76,6 +98,7 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
         g_next = list[b0 + threadIdx.x];
         if (mshift) rc_next = __ldg(rect + g_next);
     }
+    if (threadIdx.x < 3) s_rec[3 * kNullSlot + threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
     while (b0 < rg.y) {
         // every pixel terminated: stop — unless the per-tile list is being exported, which needs the whole list walked
         const bool all_done = __syncthreads_count(done) == kBatch;
@@ -123,12 +146,26 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
             bool keep = false;
             float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
             float r2 = 0.0f;
+            uint32_t wmask = 0;
             if (i < nh) {
                 const uint32_t g = s_ids[i];
                 r0 = __ldg(rec + 3ull * g);
                 r1 = __ldg(rec + 3ull * g + 1);
                 r2 = __ldg(reinterpret_cast<const float*>(rec + 3ull * g + 2));
                 keep = entry_reaches_tile(r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, X0, X1, Y0, Y1);
+                if (keep) {   // which warps' 8 x 4 pixel blocks can it reach? (blocks outside the image: nobody blends there)
+                    const float iA = __fdividef(1.0f, r0.z), iC = __fdividef(1.0f, r1.x);
+                    const float qthr = 2.0f * __logf(r1.y * (255.0f / 0.99f));
+#pragma unroll
+                    for (int w = 0; w < kWarps; ++w) {
+                        const float bx0 = X0 + (float)((w & 1) * kBlockW), by0 = Y0 + (float)((w >> 1) * kBlockH);
+                        const float bx1 = fminf(bx0 + (float)(kBlockW - 1), (float)(W - 1));
+                        const float by1 = fminf(by0 + (float)(kBlockH - 1), (float)(H - 1));
+                        const bool in_img = bx0 <= (float)(W - 1) && by0 <= (float)(H - 1);
+                        if (in_img && entry_reaches_block(r0.x, r0.y, r0.z, r0.w, r1.x, iA, iC, qthr, bx0, bx1, by0, by1))
+                            wmask |= 1u << w;
+                    }
+                }
             }
             const uint32_t bal = __ballot_sync(0xffffffffu, keep);
             if (lane == 0) s_wcnt[warp] = __popc(bal);
@@ -140,24 +177,36 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
                 pos += (w < (int)warp) ? c : 0u;
                 cnt += c;
             }
-            if (keep) { s_r0[pos] = r0; s_r1[pos] = r1; s_b[pos] = r2; }
+            if (keep) {
+                s_rec[3 * pos] = r0; s_rec[3 * pos + 1] = r1; s_rec[3 * pos + 2] = make_float4(r2, 0.f, 0.f, 0.f);
+                s_mask[pos] = (uint8_t)wmask;
+            }
             __syncthreads();
         }
-        // pad the staged list to a multiple of 8 with null entries (opacity 0 -> alpha 0 -> skipped), so the blend loop
-        // runs in fixed groups of 8 with immediate shared-memory offsets
-        if (threadIdx.x < 8 && cnt + threadIdx.x < ((cnt + 7u) & ~7u)) {
-            s_r0[cnt + threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
-            s_r1[cnt + threadIdx.x] = make_float4(0.f, 0.f, 0.f, 0.f);
-            s_b[cnt + threadIdx.x] = 0.0f;
+        // this warp's list: byte offsets of the staged records its pixel block can reach, in order, padded to a multiple
+        // of 8 with the null record so that the blend loop runs in fixed groups of 8
+        uint32_t n_w = 0;
+        for (uint32_t i0 = 0; i0 < cnt; i0 += 32) {
+            const uint32_t i = i0 + lane;
+            const bool h = i < cnt && ((s_mask[i] >> warp) & 1u);
+            const uint32_t bal = __ballot_sync(0xffffffffu, h);
+            if (h) s_widx[warp][n_w + __popc(bal & ((1u << lane) - 1u))] = (uint16_t)(i * kRecBytes);
+            n_w += __popc(bal);
         }
-        __syncthreads();
+        if (lane < 8 && n_w + lane < ((n_w + 7u) & ~7u)) s_widx[warp][n_w + lane] = (uint16_t)(kNullSlot * kRecBytes);
+        __syncwarp();
         // blend: branch-free per pair; a warp leaves the batch as soon as all of its pixels have terminated
-        for (uint32_t k0 = 0; k0 < cnt && !all_done; k0 += 8) {
+        const char* recs = reinterpret_cast<const char*>(s_rec);
+        for (uint32_t k0 = 0; k0 < n_w && !all_done; k0 += 8) {
             if (__all_sync(0xffffffffu, done)) break;
+            const uint4 offs = *reinterpret_cast<const uint4*>(&s_widx[warp][k0]);
+            const uint32_t ow[4] = {offs.x, offs.y, offs.z, offs.w};
 #pragma unroll
-            for (uint32_t k = k0; k < k0 + 8; ++k) {
-                const float4 a0 = s_r0[k];
-                const float4 a1 = s_r1[k];
+            for (uint32_t k = 0; k < 8; ++k) {
+                const char* r = recs + ((k & 1u) ? (ow[k >> 1] >> 16) : (ow[k >> 1] & 0xFFFFu));
+                const float4 a0 = *reinterpret_cast<const float4*>(r);
+                const float4 a1 = *reinterpret_cast<const float4*>(r + 16);
+                const float a2 = *reinterpret_cast<const float*>(r + 32);
                 const float dx = __fsub_rn(a0.x, fi), dy = __fsub_rn(a0.y, fj);
                 const float power = __fmaf_rn(-0.5f, __fmaf_rn(__fmul_rn(a0.z, dx), dx, __fmul_rn(__fmul_rn(a1.x, dy), dy)),
                                               -__fmul_rn(__fmul_rn(a0.w, dx), dy));
@@ -170,7 +219,7 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
                 const float wgt = blend ? __fmul_rn(alpha, T) : 0.0f;
                 C0 = __fmaf_rn(a1.z, wgt, C0);
                 C1 = __fmaf_rn(a1.w, wgt, C1);
-                C2 = __fmaf_rn(s_b[k], wgt, C2);
+                C2 = __fmaf_rn(a2, wgt, C2);
                 T = blend ? Tn : T;
             }
         }
@@ -196,28 +245,15 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
 
 }  // namespace
 
-void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
-                      float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list) {
-    // Per-warp lists (raster_warp.cu) pay when a splat covers few tiles: small splats leave many 8 x 4 blocks of a tile
-    // untouched. With large splats nearly every block is reached and this file's kernel (no masks, no
-    // indirection) is faster. Both give the same bits, so the choice is a cost heuristic: tiles touched per visible
-    // Gaussian in the previous frame (config 3: 10, config 4: 20 -> per-warp lists; the 1080p and 4K points of config 5:
-    // 35 - 120 -> this kernel). hyrf_set_raster_mode overrides it.
-    constexpr uint64_t kWarpListMaxTilesPerSplat = 28;
-    bool warp_lists = s->raster_mode == 2;
-    if (s->raster_mode == 0) warp_lists = s->lastV == 0 || s->lastD <= kWarpListMaxTilesPerSplat * s->lastV;
-    s->last_raster_mode = warp_lists ? 2 : 1;
-    if (warp_lists) {
-        hy_launch_raster_warp(s, f, ranges, list, macro, out_rgb, launches, tile_queue, dbg_list);
-        return;
-    }
+void hy_launch_raster_warp(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
+                           float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list) {
     const unsigned grid = (unsigned)(f.gx * f.gy);
     const bool want_fg = (s->debug_mask >> HYRF_DBG_FG) & 1u;
     const bool want_mask = (s->debug_mask >> HYRF_DBG_BG_MASK) & 1u;
     const float tau = (f.ablation & HYRF_ABL_NO_BG) ? INFINITY : f.tau_T;   // no background: empty S6 list
-    raster_kernel<<<grid, kBatch, 0, s->stream>>>(ranges, list, s->rec, f.W, f.H, f.gx, tau, out_rgb, s->finalT,
-                                                  s->bg_list, s->counters, want_mask ? s->bg_mask : nullptr,
-                                                  want_fg ? s->fg : nullptr, tile_queue, s->rect,
-                                                  macro ? f.mshift : 0, f.mgx, dbg_list, s->ranges);
+    raster_warp_kernel<<<grid, kBatch, 0, s->stream>>>(ranges, list, s->rec, f.W, f.H, f.gx, tau, out_rgb, s->finalT,
+                                                       s->bg_list, s->counters, want_mask ? s->bg_mask : nullptr,
+                                                       want_fg ? s->fg : nullptr, tile_queue, s->rect,
+                                                       macro ? f.mshift : 0, f.mgx, dbg_list, s->ranges);
     ++*launches;
 }

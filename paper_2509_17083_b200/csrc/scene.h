@@ -103,6 +103,8 @@ struct hyrf_scene {
 
     // debug / measurement
     uint32_t ablation = 0;            // hyrf_ablation bits
+    int raster_mode = 0;              // hyrf_set_raster_mode: 0 auto, 1 tile-level lists only, 2 per-warp lists
+    int last_raster_mode = 0;         // what the last hy_launch_raster picked
     uint32_t debug_mask = 0;
     float* dbg_raw = nullptr;         // [N][11]
     float* dbg_attrs = nullptr;       // [N][11]
@@ -157,5 +159,7 @@ hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t
 // S5 (raster.cu)
 void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
                       float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list);
+void hy_launch_raster_warp(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
+                           float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list);
 // S6 (background.cu)
 hyrf_status hy_launch_background(hyrf_scene* s, const FrameDev& f, float* out_rgb, uint32_t* launches);
