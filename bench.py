@@ -160,8 +160,9 @@ def stage_rooflines(scene, V, D, Dm, n_bg, eval_pairs, peaks):
 
 def load_traffic(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu --set full capture
-    of this workload (profiles/r1f_dram_traffic.csv); None if there is no capture."""
-    p = os.path.join(ROOT, "profiles", "r1f_dram_traffic.csv")
+    of this workload (profiles/r1h_dram_traffic.csv; raster_kernel, not launched in that run: r1f's); None if there is no
+    capture."""
+    p = os.path.join(ROOT, "profiles", "r1f_dram_traffic.csv" if kernel == "raster_kernel" else "r1h_dram_traffic.csv")
     if not os.path.exists(p):
         return None
     import csv
