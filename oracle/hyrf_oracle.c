@@ -546,6 +546,82 @@ void ho_stage_raster(int32_t W, int32_t H, const float *proj, const uint32_t *li
     }
 }
 
+/* ------------------------------------------------------------------------------------------------ */
+/* D12 backward of D10 (first piece; the training of PAPER.md:136-142 back-propagates through the
+ * 3DGS rasterizer the paper defers to, :108). The decisions of the forward pass are frozen: for every pixel, the
+ * set of blended pairs is the one D10 takes in binary32. On that set C_fg = sum_k c_k a_k T_k and
+ * T_final = prod_k (1 - a_k), with T_k = prod_{m<k} (1 - a_m), a_k = min(0.99, o_k exp(power_k)),
+ * power = -0.5 (A dx^2 + C dy^2) - B dx dy, dx = u - i, dy = v - j. Given g_cfg = dL/dC_fg and g_T = dL/dT_final:
+ *   dL/dc_k    += a_k T_k g_cfg
+ *   dL/da_k     = sum_c g_cfg_c (c_kc T_k - S_kc / (1 - a_k)) - g_T T_final / (1 - a_k),  S_k = sum_{m>k} c_m a_m T_m
+ *   a_k clamped at 0.99: nothing flows to o, power. Else dL/do += exp(power) dL/da, dL/dpower = a dL/da, and
+ *   dA += -0.5 dx^2 dP, dC += -0.5 dy^2 dP, dB += -dx dy dP, du += -(A dx + B dy) dP, dv += -(C dy + B dx) dP.
+ * The forward replay is D10's binary32; everything after it is binary64. grad: [V][9] = (u, v, A, B, C, o, r, g, b). */
+void ho_stage_raster_backward(int32_t W, int32_t H, uint32_t V, const float *proj, const uint32_t *list_rank,
+                              const uint32_t *ranges, const float *g_cfg, const float *g_T, double *grad) {
+    uint32_t gx = (uint32_t)((W + 15) / 16), gy = (uint32_t)((H + 15) / 16);
+    uint32_t maxlen = 1;
+    for (uint32_t t = 0; t < gx * gy; ++t)
+        if (ranges[2 * t + 1] - ranges[2 * t] > maxlen) maxlen = ranges[2 * t + 1] - ranges[2 * t];
+    memset(grad, 0, (size_t)V * 9 * sizeof(double));
+#pragma omp parallel
+    {
+        uint32_t *bq = (uint32_t *)malloc((size_t)maxlen * sizeof(uint32_t));
+        float *ba = (float *)malloc((size_t)maxlen * sizeof(float));
+        float *bT = (float *)malloc((size_t)maxlen * sizeof(float));
+        float *be = (float *)malloc((size_t)maxlen * sizeof(float));
+#pragma omp for schedule(dynamic, 4)
+        for (int32_t py = 0; py < H; ++py) {
+            for (int32_t px = 0; px < W; ++px) {
+                uint32_t tile = (uint32_t)(py / 16) * gx + (uint32_t)(px / 16);
+                uint32_t q0 = ranges[2 * tile], q1 = ranges[2 * tile + 1], nb = 0;
+                float T = 1.0f;
+                for (uint32_t q = q0; q < q1; ++q) {          /* D10, decisions in binary32 */
+                    const float *g = proj + 10ull * list_rank[q];
+                    float dx = g[0] - (float)px, dy = g[1] - (float)py;
+                    float power = fmaf(-0.5f, fmaf(g[3] * dx, dx, (g[5] * dy) * dy), -((g[4] * dx) * dy));
+                    if (power > 0.0f) continue;
+                    float e = ho_softexp(power);
+                    float alpha = fminf(0.99f, g[6] * e);
+                    if (alpha < 1.0f / 255.0f) continue;
+                    float Tn = T * (1.0f - alpha);
+                    if (Tn < 1e-4f) break;
+                    bq[nb] = q; ba[nb] = alpha; bT[nb] = T; be[nb] = (g[6] * e > 0.99f) ? -1.0f : e;
+                    ++nb;
+                    T = Tn;
+                }
+                uint64_t o = (uint64_t)py * (uint64_t)W + (uint64_t)px;
+                const double gc[3] = {g_cfg[3 * o], g_cfg[3 * o + 1], g_cfg[3 * o + 2]};
+                const double gT = g_T[o], Tfin = T;
+                double S[3] = {0.0, 0.0, 0.0};
+                for (uint32_t n = nb; n-- > 0;) {
+                    uint32_t r = list_rank[bq[n]];
+                    const float *g = proj + 10ull * r;
+                    double a = ba[n], Tk = bT[n], w = a * Tk, da = 0.0;
+                    double *G = grad + 9ull * r;
+                    for (int c = 0; c < 3; ++c) {
+                        da += gc[c] * ((double)g[7 + c] * Tk - S[c] / (1.0 - a));
+#pragma omp atomic
+                        G[6 + c] += w * gc[c];
+                    }
+                    da -= gT * Tfin / (1.0 - a);
+                    for (int c = 0; c < 3; ++c) S[c] += (double)g[7 + c] * w;
+                    if (be[n] < 0.0f) continue;               /* clamped at 0.99 */
+                    double dx = (double)g[0] - (double)px, dy = (double)g[1] - (double)py, dP = a * da;
+                    double A = g[3], B = g[4], C = g[5];
+                    double add[6] = {-(A * dx + B * dy) * dP, -(C * dy + B * dx) * dP, -0.5 * dx * dx * dP,
+                                     -dx * dy * dP, -0.5 * dy * dy * dP, (double)be[n] * da};
+                    for (int k = 0; k < 6; ++k) {
+#pragma omp atomic
+                        G[k] += add[k];
+                    }
+                }
+            }
+        }
+        free(bq); free(ba); free(bT); free(be);
+    }
+}
+
 /* D11: ray direction of pixel (i, j) and its hit point on the background sphere. */
 void ho_ray_sphere(const ho_camera *cam, float i, float j, float radius, float d[3], float ps[3]) {
     const float *R = cam->R;

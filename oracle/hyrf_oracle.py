@@ -430,6 +430,19 @@ def stage_raster(W: int, H: int, proj: np.ndarray, list_rank: np.ndarray, ranges
     return dict(cfg=cfg, T=T, wsum=wsum, m_alpha=m_alpha, m_stop=m_stop, n_eval=n_eval, n_blend=n_blend)
 
 
+def stage_raster_backward(W: int, H: int, proj: np.ndarray, list_rank: np.ndarray, ranges: np.ndarray,
+                          g_cfg: np.ndarray, g_T: np.ndarray) -> np.ndarray:
+    """D12: gradients of L w.r.t. the projected records (u, v, A, B, C, o, r, g, b), [V][9] float64, given
+    g_cfg = dL/dC_fg [H][W][3] and g_T = dL/dT_final [H][W], with D10's decisions frozen."""
+    V = len(proj)
+    grad = np.zeros((V, 9), np.float64)
+    lib().ho_stage_raster_backward(C.c_int32(W), C.c_int32(H), C.c_uint32(V), _p(_f32(proj)),
+                                   _p(np.ascontiguousarray(list_rank, dtype=np.uint32)),
+                                   _p(np.ascontiguousarray(ranges, dtype=np.uint32)), _p(_f32(g_cfg, (H, W, 3))),
+                                   _p(_f32(g_T, (H, W))), _p(grad))
+    return grad
+
+
 def stage_background(osc: OracleScene, cam, W: int, H: int, cfg: np.ndarray, T: np.ndarray):
     c = camera_struct(cam)
     out = np.zeros((H, W, 3), np.float32)
