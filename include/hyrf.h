@@ -238,6 +238,17 @@ hyrf_status hyrf_set_raster_mode(hyrf_scene* scene, int mode);
 /* The variant (1 or 2) the last render used. */
 hyrf_status hyrf_last_raster_mode(hyrf_scene* scene, int* mode);
 
+/* Backward of stage 5 for the LAST rendered frame (first piece of the training pass of PAPER.md:136-142, which
+ * back-propagates through the rasterizer the paper defers to, :108; arithmetic DESIGN.md §2 D12). With the frame's
+ * blending decisions frozen, C_fg and the final transmittance T of every pixel are differentiable in the projected
+ * records. g_cfg: DEVICE float [H][W][3] = dL/dC_fg; g_T: DEVICE float [H][W] = dL/dT (how a loss on the composited
+ * image reaches the foreground: out = C_fg + T c_s). grad: DEVICE float [V][9], row = visible rank (HYRF_DBG_VIS_IDX
+ * order), columns dL/d(u, v, A, B, C, opacity, r, g, b); overwritten. Enqueued on the scene's stream; the caller
+ * synchronises. The frame must have been rendered with HYRF_DBG_TILE_LIST | HYRF_DBG_TILE_RANGES enabled (the
+ * per-tile lists are then retained), else HYRF_ERR_NOT_READY. Sums use fp32 atomics: the result is reproducible to
+ * rounding, not bit for bit. */
+hyrf_status hyrf_raster_backward(hyrf_scene* scene, const float* g_cfg, const float* g_T, float* grad);
+
 /* Number of kernels the last render launched (for bench.py's gpu_launches). */
 hyrf_status hyrf_last_launch_count(hyrf_scene* scene, uint32_t* launches);
 

@@ -29,7 +29,7 @@ EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_r
            "hyrf_destroy_scene", "hyrf_last_error", "hyrf_debug_enable", "hyrf_debug_fetch", "hyrf_set_timing",
            "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation", "hyrf_render_host_async",
            "hyrf_host_sync", "hyrf_set_sort_overlap", "hyrf_upload_explicit_rvq", "hyrf_last_decode_time", "hyrf_set_raster_mode",
-           "hyrf_last_raster_mode"]
+           "hyrf_last_raster_mode", "hyrf_raster_backward"]
 ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
 
 
@@ -112,6 +112,7 @@ def load_library() -> C.CDLL:
         L.hyrf_last_decode_time.argtypes = [vp, C.POINTER(C.c_float)]
         L.hyrf_set_raster_mode.argtypes = [vp, C.c_int]
         L.hyrf_last_raster_mode.argtypes = [vp, C.POINTER(C.c_int)]
+        L.hyrf_raster_backward.argtypes = [vp, vp, vp, vp]
         for name in EXPORTS:
             if name != "hyrf_last_error":
                 getattr(L, name).restype = C.c_int
@@ -339,6 +340,15 @@ class HyrfScene:
     def set_raster_mode(self, mode: int = 0) -> None:
         """0 auto, 1 tile-level lists only, 2 per-warp lists (include/hyrf.h hyrf_set_raster_mode); same bits, different cost."""
         _check(self.lib.hyrf_set_raster_mode(self.handle, int(mode)))
+
+    def raster_backward(self, g_cfg, g_T, n_visible: int):
+        """hyrf_raster_backward: g_cfg (H, W, 3) and g_T (H, W) float32 CUDA tensors -> (V, 9) float32 CUDA tensor."""
+        torch = self._torch
+        grad = torch.empty((int(n_visible), 9), dtype=torch.float32, device=f"cuda:{self.device}")
+        g_cfg, g_T = g_cfg.contiguous(), g_T.contiguous()
+        _check(self.lib.hyrf_raster_backward(self.handle, C.c_void_p(g_cfg.data_ptr()), C.c_void_p(g_T.data_ptr()),
+                                             C.c_void_p(grad.data_ptr())))
+        return grad
 
     def last_raster_mode(self) -> int:
         m = C.c_int(0)

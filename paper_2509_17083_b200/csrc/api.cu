@@ -436,6 +436,17 @@ extern "C" hyrf_status hyrf_set_raster_mode(hyrf_scene* s, int mode) {
     return HYRF_OK;
 }
 
+extern "C" hyrf_status hyrf_raster_backward(hyrf_scene* s, const float* g_cfg, const float* g_T, float* grad) {
+    if (!s || !g_cfg || !g_T || !grad) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_raster_backward: NULL argument");
+    const uint32_t need = (1u << HYRF_DBG_TILE_LIST) | (1u << HYRF_DBG_TILE_RANGES);
+    if (!s->rendered || !s->list_final || (s->debug_mask & need) != need)
+        return hy_fail(HYRF_ERR_NOT_READY, "hyrf_raster_backward: the last frame was not rendered with HYRF_DBG_TILE_LIST | HYRF_DBG_TILE_RANGES enabled");
+    cudaError_t e;
+    if ((e = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
+    uint32_t launches = 0;
+    return hy_launch_raster_backward(s, g_cfg, g_T, grad, &launches);
+}
+
 extern "C" hyrf_status hyrf_last_raster_mode(hyrf_scene* s, int* mode) {
     if (!s || !mode) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_last_raster_mode: NULL argument");
     if (!s->rendered) return hy_fail(HYRF_ERR_NOT_READY, "hyrf_last_raster_mode: no completed render");

@@ -529,3 +529,59 @@ def test_rasterizer_choice_changes_no_bit(B, synth):
         hs.set_raster_mode(3)
     assert e.value.status == B.HYRF_ERR_INVALID_ARG
     hs.close()
+
+
+def _backward_case(B, ho, scene, cam, seed=0):
+    import torch
+    hs = B.HyrfScene(scene, mlp_path=B.HYRF_MLP_FMA)
+    hs.debug_enable()
+    hs.render(cam)
+    torch.cuda.synchronize()
+    orc = ho.render(ho.OracleScene(scene), cam)
+    W, H, V = cam.W, cam.H, len(orc["vis_idx"])
+    assert (hs.debug_fetch(B.DBG_TILE_LIST) == orc["list_id"]).all()      # same lists, same records: same frozen set
+    rng = np.random.default_rng(seed)
+    gc = rng.normal(0, 1, (H, W, 3)).astype(np.float32)
+    gt = rng.normal(0, 1, (H, W)).astype(np.float32)
+    got = hs.raster_backward(torch.from_numpy(gc).cuda(), torch.from_numpy(gt).cuda(), V)
+    torch.cuda.synchronize()
+    got = got.cpu().numpy().astype(np.float64)
+    want = ho.stage_raster_backward(W, H, orc["proj"], orc["list_rank"], orc["ranges"], gc, gt)
+    hs.close()
+    return got, want, orc
+
+
+@pytest.mark.parametrize("case", ["tiny", "tiny_big_splats", "config1", "config3_scaled"])
+def test_raster_backward_against_oracle(B, ho, synth, case):
+    # hyrf_raster_backward (DESIGN.md §2 D12, first piece) against the oracle's float64 backward
+    # on the same frozen decisions. fp32 sums in atomic order + T recovered by division: tolerance 2e-3 of each
+    # column's scale plus 2e-3 relative; a pair whose decision sits on the ex2.approx / exp difference may flip for a
+    # pixel or two, which stays inside that bound.
+    if case == "tiny":
+        s = synth.tiny_scene(n=48, W=32, H=32)
+    elif case == "tiny_big_splats":
+        s = synth.tiny_scene(n=64, W=45, H=37, seed=9, scale_mean=-1.0)      # ragged tiles, deep lists, clamped alphas
+    elif case == "config1":
+        s = synth.make_scene(1)
+    else:
+        s = synth.make_scene(3, n_gaussians=60_000, width=320, height=180, n_cameras=1)
+    got, want, orc = _backward_case(B, ho, s, s.cameras[0], seed=len(case))
+    assert np.isfinite(got).all()
+    scale = np.abs(want).max(axis=0)
+    assert (scale > 0).all()
+    err = np.abs(got - want)
+    assert (err <= 2e-3 * scale + 2e-3 * np.abs(want)).all(), (err.max(axis=0) / scale)
+    untouched = orc["tiles"] == 0
+    assert (got[untouched] == 0).all()                                       # a Gaussian in no list gets no gradient
+
+
+def test_raster_backward_needs_the_lists(B, synth):
+    import torch
+    s = synth.tiny_scene(n=16)
+    hs = B.HyrfScene(s)
+    hs.render(s.cameras[0])
+    z = torch.zeros(32, 32, 3, device="cuda")
+    with pytest.raises(B.HyrfError) as e:
+        hs.raster_backward(z, z[..., 0], 16)
+    assert e.value.status == B.HYRF_ERR_NOT_READY
+    hs.close()
