@@ -9,7 +9,7 @@
 // blended prefix and its final T. Phase 2 walks the list backwards in staged batches: alpha is recomputed, the
 // transmittance in front of a pair is recovered as T_k = T_{k+1} / (1 - alpha_k) (alpha <= 0.99 bounds the
 // amplification), the colour behind it is the running suffix sum. The nine per-pair contributions are reduced over
-// the warp with shuffles and added to the Gaussian's row with one atomic per value and warp. HBM traffic is small
+// the warp with 12 shuffles (halving exchange) and added to the Gaussian's row with one atomic per value and warp. HBM traffic is small
 // (records re-read per tile, as in the forward); the kernel is bound by ALU issue and shuffles.
 #include "scene.h"
 
@@ -119,10 +119,11 @@ raster_backward_kernel(const uint2* __restrict__ ranges, const uint32_t* __restr
 #pragma unroll
             for (int j = 0; j < 9; ++j) v[j] = 0.0f;
             if (mine) {
-                const float om = 1.0f - alpha;
-                const float Tk = T / om;          // transmittance in front of this pair
+                const float iom = __frcp_rn(1.0f - alpha);   // one reciprocal serves the four quotients (1 - alpha >= 0.01)
+                const float Tk = T * iom;                    // transmittance in front of this pair
                 const float w = alpha * Tk;
-                float da = gc0 * (a1.z * Tk - S0 / om) + gc1 * (a1.w * Tk - S1 / om) + gc2 * (cb * Tk - S2 / om) - gT * Tfin / om;
+                const float da = gc0 * (a1.z * Tk - S0 * iom) + gc1 * (a1.w * Tk - S1 * iom) + gc2 * (cb * Tk - S2 * iom) -
+                                 gT * Tfin * iom;
                 v[6] = w * gc0; v[7] = w * gc1; v[8] = w * gc2;
                 S0 = fmaf(a1.z, w, S0); S1 = fmaf(a1.w, w, S1); S2 = fmaf(cb, w, S2);
                 T = Tk;
@@ -136,17 +137,31 @@ raster_backward_kernel(const uint2* __restrict__ ranges, const uint32_t* __restr
                     v[5] = e * da;
                 }
             }
+            // nine sums over the warp in 12 shuffles instead of 45: at every step a lane keeps one half of its values and
+            // hands the other half to its partner (5 + 3 + 2 + 1 exchanges), then one plain step; the lane ends with value
+            // number idx (padding slots are zero and dropped)
+            const bool h16 = lane & 16u, h8 = lane & 8u, h4 = lane & 4u, h2 = lane & 2u;
+            float a[5], b[3], c[2], d;
 #pragma unroll
-            for (int j = 0; j < 9; ++j) {
-#pragma unroll
-                for (int sh = 16; sh > 0; sh >>= 1) v[j] += __shfl_xor_sync(0xffffffffu, v[j], sh);
+            for (int i = 0; i < 5; ++i) {
+                const float hi = i < 4 ? v[5 + i] : 0.0f;
+                a[i] = (h16 ? hi : v[i]) + __shfl_xor_sync(0xffffffffu, h16 ? v[i] : hi, 16);
             }
-            if (lane < 9) {
-                float mine_v = v[0];
 #pragma unroll
-                for (int j = 1; j < 9; ++j) mine_v = (lane == (uint32_t)j) ? v[j] : mine_v;
-                atomicAdd(grad + 9ull * s_id[k] + lane, mine_v);
+            for (int i = 0; i < 3; ++i) {
+                const float hi = i < 2 ? a[3 + i] : 0.0f;
+                b[i] = (h8 ? hi : a[i]) + __shfl_xor_sync(0xffffffffu, h8 ? a[i] : hi, 8);
             }
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const float hi = i < 1 ? b[2] : 0.0f;
+                c[i] = (h4 ? hi : b[i]) + __shfl_xor_sync(0xffffffffu, h4 ? b[i] : hi, 4);
+            }
+            d = (h2 ? c[1] : c[0]) + __shfl_xor_sync(0xffffffffu, h2 ? c[0] : c[1], 2);
+            d += __shfl_xor_sync(0xffffffffu, d, 1);
+            const uint32_t idx = (h16 ? 5u : 0u) + (h8 ? 3u : 0u) + (h4 ? 2u : 0u) + (h2 ? 1u : 0u);
+            const bool holds = !(lane & 1u) && !(h4 && h2) && !(h8 && h4) && idx < 9u;
+            if (holds) atomicAdd(grad + 9ull * s_id[k] + idx, d);
         }
     }
 }
