@@ -388,11 +388,35 @@ def run_ours(args):
     e2e_s = max_over_ranks(time.perf_counter() - t0)
     e2e = frames_total / e2e_s
 
+    raster_mode_used = hs.last_raster_mode()
+    backward = None
+    if args.backward and rank == 0:
+        # NEXT-3, first piece: hyrf_raster_backward for camera 0's frame (per-tile lists retained), outside the timed
+        # frames; CUDA events on the launching stream, L2 flushed before each repetition
+        hs.debug_enable((1 << B.DBG_TILE_LIST) | (1 << B.DBG_TILE_RANGES))
+        hs.render_struct(cstructs[0], W, H, out.data_ptr())
+        torch.cuda.synchronize(dev)
+        cnt = hs.debug_fetch(B.DBG_COUNTERS)
+        g_c = torch.randn((H, W, 3), dtype=torch.float32, device=f"cuda:{dev}")
+        g_t = torch.randn((H, W), dtype=torch.float32, device=f"cuda:{dev}")
+        ts = []
+        for _ in range(8):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            hs.raster_backward(g_c, g_t, int(cnt[1]))
+            e1.record(stream)
+            torch.cuda.synchronize(dev)
+            ts.append(e0.elapsed_time(e1))
+        backward = {"kernel": "raster_backward_kernel", "ms": float(np.median(ts[2:])), "V": int(cnt[1]), "D": int(cnt[2]),
+                    "note": "includes the memset of the [V][9] gradient rows"}
+        hs.debug_enable(0)
+
     if rank != 0:
         return
     names = ["cull", "field", "bin", "raster", "background"]
     kernels = {"field": ("field_warp_kernel" if args.mlp == "hmma" else "field_mma_pipe_kernel") if scene.fp16 and args.mlp != "fma"
-               else "field_fma_kernel", "raster": "raster_warp_kernel" if hs.last_raster_mode() == 2 else "raster_kernel"}
+               else "field_fma_kernel", "raster": "raster_warp_kernel" if raster_mode_used == 2 else "raster_kernel"}
     eval_pairs = None
     cpu = None
     if world == 1 and not args.no_cpu and args.ablation == 0:
@@ -436,6 +460,8 @@ def run_ours(args):
         line["cpu_baseline"] = cpu
     if upload:
         line["upload_decode"] = upload
+    if backward:
+        line["backward"] = backward
     print(json.dumps(line), flush=True)
 
 
@@ -456,6 +482,8 @@ def main():
                     help="compressed model: 8-bit min-max tables decoded in the gather (PAPER.md:229)")
     ap.add_argument("--raster", default="auto", choices=["auto", "tile", "warp"],
                     help="hyrf_set_raster_mode: per-frame choice (default), tile-level lists only, per-warp lists")
+    ap.add_argument("--backward", action="store_true",
+                    help="also time hyrf_raster_backward (backward of the alpha blend, NEXT-3 first piece) on camera 0's frame")
     ap.add_argument("--rvq", action="store_true",
                     help="compressed explicit Gaussians: binary16 positions + R-VQ codes decoded at upload (PAPER.md:229 (1)-(2))")
     ap.add_argument("--no-cpu", action="store_true")

@@ -47,8 +47,10 @@ raster_backward_kernel(const uint2* __restrict__ ranges, const uint32_t* __restr
     const int tile = (int)blockIdx.x;
     const int tx = tile % gx, ty = tile / gx;
     const uint32_t lane = threadIdx.x & 31u;
-    const int px = tx * HY_TILE + (int)(threadIdx.x & (HY_TILE - 1));
-    const int py = ty * HY_TILE + (int)(threadIdx.x >> 4);
+    // a warp owns an 8 x 4 pixel block (not 16 x 2 rows): more entries miss a whole block, and those cost it only the test
+    const uint32_t warp = threadIdx.x >> 5;
+    const int px = tx * HY_TILE + (int)(warp & 1u) * 8 + (int)(lane & 7u);
+    const int py = ty * HY_TILE + (int)(warp >> 1) * 4 + (int)(lane >> 3);
     const bool inside = px < W && py < H;
     const float fi = (float)px, fj = (float)py;
     const uint2 rg = ranges[tile];
