@@ -6,40 +6,13 @@
 // (profiles/r1a: divergent skip/stop branches cost 45 issue slots per pair against ~30 predicated); warps stop
 // when all of their pixels have terminated, the CTA when all warps have. Bound by plain fp32 ALU issue + one
 // MUFU.EX2 per pair — no tensor cores (nothing here is a dense contraction).
+#include "raster_common.cuh"
 #include "scene.h"
 
 namespace {
 
 constexpr int kBatch = HY_TILE * HY_TILE;
 constexpr int kWarps = kBatch / 32;
-
-// Can list entry (mean (u, v), conic (A, B, C), opacity o) reach alpha >= 1/255 at ANY pixel of the tile
-// [X0, X1] x [Y0, Y1]? The quadratic form q = A dx^2 + 2 B dx dy + C dy^2 is convex, so its minimum over the pixel box
-// is 0 when the mean lies inside, else it sits on a face whose plane separates the mean from the box: at most two
-// one-dimensional minimisations. alpha <= o exp(-q_min / 2) everywhere in the tile; entries below the threshold
-// (with a 1 % margin against rounding) would be skipped by every pixel, so dropping them changes no output bit.
-__device__ __forceinline__ bool entry_reaches_tile(float u, float v, float A, float B, float C, float o, float X0,
-                                                   float X1, float Y0, float Y1) {
-    const float ex = fminf(fmaxf(u, X0), X1) - u, ey = fminf(fmaxf(v, Y0), Y1) - v;
-    if (ex == 0.0f && ey == 0.0f) return true;
-    float qmin = 3.0e38f;
-    if (ex != 0.0f) {
-        const float dy = fminf(fmaxf(__fdividef(-B * ex, C), Y0 - v), Y1 - v);
-        qmin = A * ex * ex + 2.0f * B * ex * dy + C * dy * dy;
-    }
-    if (ey != 0.0f) {
-        const float dx = fminf(fmaxf(__fdividef(-B * ey, A), X0 - u), X1 - u);
-        qmin = fminf(qmin, A * dx * dx + 2.0f * B * dx * ey + C * ey * ey);
-    }
-    return !(o * __expf(-0.5f * qmin) < 0.99f / 255.0f);   // NaN keeps the entry
-}
-
-// exp2 on the MUFU, flushing subnormal results to 0 (they are far below the 1/255 skip threshold anyway)
-__device__ __forceinline__ float ex2_ftz(float x) {
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
 
 __global__ void __launch_bounds__(kBatch)
 raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ list, const float4* __restrict__ rec,

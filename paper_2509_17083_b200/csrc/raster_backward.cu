@@ -11,17 +11,12 @@
 // amplification), the colour behind it is the running suffix sum. The nine per-pair contributions are reduced over
 // the warp with 12 shuffles (halving exchange) and added to the Gaussian's row with one atomic per value and warp. HBM traffic is small
 // (records re-read per tile, as in the forward); the kernel is bound by ALU issue and shuffles.
+#include "raster_common.cuh"
 #include "scene.h"
 
 namespace {
 
 constexpr int kBatch = HY_TILE * HY_TILE;
-
-__device__ __forceinline__ float ex2_ftz(float x) {
-    float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
 
 // D10 for one pair: returns false when the pair is skipped; alpha and e = exp(power) otherwise (operations and order of
 // raster.cu's blend loop)
