@@ -551,7 +551,7 @@ def _backward_case(B, ho, scene, cam, seed=0):
     return got, want, orc
 
 
-@pytest.mark.parametrize("case", ["tiny", "tiny_big_splats", "config1", "config3_scaled"])
+@pytest.mark.parametrize("case", ["tiny", "tiny_big_splats", "config1", "config3_scaled", "config3_full"])
 def test_raster_backward_against_oracle(B, ho, synth, case):
     # hyrf_raster_backward (DESIGN.md §2 D12, first piece) against the oracle's float64 backward
     # on the same frozen decisions. fp32 sums in atomic order + T recovered by division: tolerance 2e-3 of each
@@ -563,8 +563,10 @@ def test_raster_backward_against_oracle(B, ho, synth, case):
         s = synth.tiny_scene(n=64, W=45, H=37, seed=9, scale_mean=-1.0)      # ragged tiles, deep lists, clamped alphas
     elif case == "config1":
         s = synth.make_scene(1)
-    else:
+    elif case == "config3_scaled":
         s = synth.make_scene(3, n_gaussians=60_000, width=320, height=180, n_cameras=1)
+    else:
+        s = synth.make_scene(3, n_cameras=1)          # BASELINE config 3 at full size: what bench.py --backward times
     got, want, orc = _backward_case(B, ho, s, s.cameras[0], seed=len(case))
     assert np.isfinite(got).all()
     scale = np.abs(want).max(axis=0)
