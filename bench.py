@@ -114,6 +114,8 @@ def workload(cfg: int, args):
     if args.width and args.height:
         kw["width"], kw["height"] = args.width, args.height
     scene = synth.make_scene(cfg, **kw)
+    if args.morton_input:
+        scene = synth.morton_sorted(scene)
     if args.quant8:
         scene = synth.quantize8(scene)
     if args.rvq:
@@ -122,6 +124,8 @@ def workload(cfg: int, args):
     name = (f"BASELINE.json configs[{cfg - 1}]: {scene.n} Gaussians, "
             f"{'8-bit tables + fp16 MLPs (compressed model)' if scene.quant8 else ('fp16' if scene.fp16 else 'fp32') + ' grids/MLPs'}, "
             f"{cam.W}x{cam.H}, {len(scene.cameras)} cameras")
+    if args.morton_input:
+        name += "; Gaussians stored in Morton order (secondary measurement)"
     if scene.explicit_rvq is not None:
         q = scene.explicit_rvq
         name += f"; explicit part compressed (binary16 positions, R-VQ {q.stages} x {q.codebook_size}), decoded at upload"
@@ -482,6 +486,8 @@ def main():
                     help="compressed model: 8-bit min-max tables decoded in the gather (PAPER.md:229)")
     ap.add_argument("--raster", default="auto", choices=["auto", "tile", "warp"],
                     help="hyrf_set_raster_mode: per-frame choice (default), tile-level lists only, per-warp lists")
+    ap.add_argument("--morton-input", action="store_true",
+                    help="store the Gaussians in Morton order of their positions (SURVEY 8(d): secondary, labelled measurement)")
     ap.add_argument("--backward", action="store_true",
                     help="also time hyrf_raster_backward (backward of the alpha blend, NEXT-3 first piece) on camera 0's frame")
     ap.add_argument("--rvq", action="store_true",

@@ -379,6 +379,33 @@ def tiny_scene(n: int = 48, W: int = 32, H: int = 32, seed: int = 7, fp16: bool 
     return s
 
 
+def morton_sorted(scene: Scene) -> Scene:
+    """The same scene with its Gaussians stored in Morton (Z-curve) order of their positions: SURVEY §8(d)'s secondary,
+    labelled measurement (a trained model's order is arbitrary, so the order as generated stays the primary one). A pure
+    permutation of the input arrays: 10 bits per axis over the bounding box of the positions."""
+    import copy
+    pos = np.asarray(scene.pos, np.float32)
+    lo, hi = pos.min(axis=1, keepdims=True), pos.max(axis=1, keepdims=True)
+    q = np.clip(((pos - lo) / np.maximum(hi - lo, 1e-30) * 1023.0).astype(np.uint64), 0, 1023)
+
+    def spread(v):
+        v = (v | (v << np.uint64(16))) & np.uint64(0x030000FF)
+        v = (v | (v << np.uint64(8))) & np.uint64(0x0300F00F)
+        v = (v | (v << np.uint64(4))) & np.uint64(0x030C30C3)
+        v = (v | (v << np.uint64(2))) & np.uint64(0x09249249)
+        return v
+
+    code = spread(q[0]) | (spread(q[1]) << np.uint64(1)) | (spread(q[2]) << np.uint64(2))
+    order = np.argsort(code, kind="stable")
+    s = copy.copy(scene)
+    s.pos = np.ascontiguousarray(pos[:, order])
+    s.rgb_logit = np.ascontiguousarray(np.asarray(scene.rgb_logit)[:, order])
+    s.scale_logit = np.ascontiguousarray(np.asarray(scene.scale_logit)[order])
+    s.opacity_logit = np.ascontiguousarray(np.asarray(scene.opacity_logit)[order])
+    s.name = scene.name + "_morton"
+    return s
+
+
 def shard_cameras(n_cameras: int, rank: int, world: int) -> List[int]:
     """Frame-parallel replicas: cameras dealt round-robin, no collective on the data path."""
     return list(range(rank, n_cameras, world))
