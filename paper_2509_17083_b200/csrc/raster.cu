@@ -174,9 +174,9 @@ void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, con
     // Per-warp lists (raster_warp.cu) pay when a splat covers few tiles: small splats leave many 8 x 4 blocks of a tile
     // untouched. With large splats nearly every block is reached and this file's kernel (no masks, no
     // indirection) is faster. Both give the same bits, so the choice is a cost heuristic: tiles touched per visible
-    // Gaussian in the previous frame (config 3: 10, config 4: 20 -> per-warp lists; the 1080p and 4K points of config 5:
-    // 35 - 120 -> this kernel). hyrf_set_raster_mode overrides it.
-    constexpr uint64_t kWarpListMaxTilesPerSplat = 28;
+    // Gaussian in the previous frame (config 3: 10, config 4: 15 -> per-warp lists; the 1080p and 4K points of config 5:
+    // 35 - 120 -> this kernel; config 3 rendered at 1080p, 19 tiles per Gaussian, is the tie). hyrf_set_raster_mode overrides it.
+    constexpr uint64_t kWarpListMaxTilesPerSplat = 19;   // measured crossover on config 3 at 900p / 1080p / 1260p
     bool warp_lists = s->raster_mode == 2;
     if (s->raster_mode == 0) warp_lists = s->lastV == 0 || s->lastD <= kWarpListMaxTilesPerSplat * s->lastV;
     s->last_raster_mode = warp_lists ? 2 : 1;
