@@ -35,7 +35,7 @@ typedef struct hyrf_scene hyrf_scene; /* opaque, library-owned */
 typedef enum {
     HYRF_OK = 0,
     HYRF_ERR_INVALID_ARG = 1, /* NULL pointer, W/H outside [1, max], n_gaussians == 0 ... */
-    HYRF_ERR_NOT_READY = 2,   /* render before upload_params */
+    HYRF_ERR_NOT_READY = 2,   /* render before the fields and the explicit Gaussians were uploaded; fetch / backward before a render */
     HYRF_ERR_UNSUPPORTED = 3, /* feats != 2, table not a power of two, dims beyond HYRF_MAX_* */
     HYRF_ERR_CAMERA = 4,      /* non-finite camera, or centre outside the background sphere */
     HYRF_ERR_OOM = 5,         /* device allocation failed, or D >= 2^32 */
@@ -92,7 +92,7 @@ typedef struct {
 } hyrf_scene_desc;
 
 typedef struct {
-    const float* pos;           /* [3][N] SoA: x[N], y[N], z[N] — p_e */
+    const float* pos;           /* [3][N] SoA: x[N], y[N], z[N] — p_e (these four: all given, or all NULL, see hyrf_upload_params) */
     const float* rgb_logit;     /* [3][N] — c_e (pre-sigmoid) */
     const float* scale_logit;   /* [N]    — s_e (pre-sigmoid, isotropic) */
     const float* opacity_logit; /* [N]    — alpha_e (pre-sigmoid) */
