@@ -24,9 +24,44 @@ __device__ __forceinline__ bool entry_reaches_tile(float u, float v, float A, fl
     return !(o * __expf(-0.5f * qmin) < 0.99f / 255.0f);   // NaN keeps the entry
 }
 
+// The same test for a sub-rectangle of the tile, with the per-entry work hoisted: iA = 1 / A, iC = 1 / C,
+// qthr = 2 ln(o * 255 / 0.99) (alpha >= 0.99 / 255  <=>  q <= qthr). NaN keeps the entry.
+__device__ __forceinline__ bool entry_reaches_block(float u, float v, float A, float B, float C, float iA, float iC,
+                                                    float qthr, float X0, float X1, float Y0, float Y1) {
+    const float ex = fminf(fmaxf(u, X0), X1) - u, ey = fminf(fmaxf(v, Y0), Y1) - v;
+    if (ex == 0.0f && ey == 0.0f) return true;
+    float qmin = 3.0e38f;
+    if (ex != 0.0f) {
+        const float dy = fminf(fmaxf(-B * ex * iC, Y0 - v), Y1 - v);
+        qmin = A * ex * ex + 2.0f * B * ex * dy + C * dy * dy;
+    }
+    if (ey != 0.0f) {
+        const float dx = fminf(fmaxf(-B * ey * iA, X0 - u), X1 - u);
+        qmin = fminf(qmin, A * dx * dx + 2.0f * B * dx * ey + C * ey * ey);
+    }
+    return !(qmin > qthr);
+}
+
 // exp2 on the MUFU, flushing subnormal results to 0 (they are far below the 1/255 skip threshold anyway)
 __device__ __forceinline__ float ex2_ftz(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
+}
+
+// Which of the eight 8 x 4 pixel blocks (block w: columns (w & 1) * 8 .., rows (w >> 1) * 4 ..) of the 16 x 16 tile at
+// (X0, Y0) can the entry reach with alpha >= 1/255? Blocks outside the W x H image are never set (nobody blends there).
+__device__ __forceinline__ uint32_t entry_block_mask(float u, float v, float A, float B, float C, float o, float X0,
+                                                     float Y0, int W, int H) {
+    const float iA = __fdividef(1.0f, A), iC = __fdividef(1.0f, C);
+    const float qthr = 2.0f * __logf(o * (255.0f / 0.99f));
+    uint32_t m = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+        const float bx0 = X0 + (float)((w & 1) * 8), by0 = Y0 + (float)((w >> 1) * 4);
+        const float bx1 = fminf(bx0 + 7.0f, (float)(W - 1)), by1 = fminf(by0 + 3.0f, (float)(H - 1));
+        const bool in_img = bx0 <= (float)(W - 1) && by0 <= (float)(H - 1);
+        if (in_img && entry_reaches_block(u, v, A, B, C, iA, iC, qthr, bx0, bx1, by0, by1)) m |= 1u << w;
+    }
+    return m;
 }

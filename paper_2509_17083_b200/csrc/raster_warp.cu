@@ -14,24 +14,6 @@ namespace {
 constexpr int kBatch = HY_TILE * HY_TILE;
 constexpr int kWarps = kBatch / 32;
 
-// The same test for a sub-rectangle of the tile, with the per-entry work hoisted: iA = 1 / A, iC = 1 / C,
-// qthr = 2 ln(o * 255 / 0.99) (alpha >= 0.99 / 255  <=>  q <= qthr). NaN keeps the entry.
-__device__ __forceinline__ bool entry_reaches_block(float u, float v, float A, float B, float C, float iA, float iC,
-                                                    float qthr, float X0, float X1, float Y0, float Y1) {
-    const float ex = fminf(fmaxf(u, X0), X1) - u, ey = fminf(fmaxf(v, Y0), Y1) - v;
-    if (ex == 0.0f && ey == 0.0f) return true;
-    float qmin = 3.0e38f;
-    if (ex != 0.0f) {
-        const float dy = fminf(fmaxf(-B * ex * iC, Y0 - v), Y1 - v);
-        qmin = A * ex * ex + 2.0f * B * ex * dy + C * dy * dy;
-    }
-    if (ey != 0.0f) {
-        const float dx = fminf(fmaxf(-B * ey * iA, X0 - u), X1 - u);
-        qmin = fminf(qmin, A * dx * dx + 2.0f * B * dx * ey + C * ey * ey);
-    }
-    return !(qmin > qthr);
-}
-
 constexpr int kBlockW = 8, kBlockH = 4;            // pixel block of one warp inside the 16 x 16 tile
 constexpr uint32_t kNullSlot = 2 * kBatch;         // staged slot holding a null record (opacity 0 -> alpha 0 -> skipped)
 constexpr uint32_t kRecBytes = 48;                 // staged record: (u, v, A, B), (C, opacity, r, g), (b, -, -, -)
@@ -126,19 +108,8 @@ raster_warp_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict_
                 r1 = __ldg(rec + 3ull * g + 1);
                 r2 = __ldg(reinterpret_cast<const float*>(rec + 3ull * g + 2));
                 keep = entry_reaches_tile(r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, X0, X1, Y0, Y1);
-                if (keep) {   // which warps' 8 x 4 pixel blocks can it reach? (blocks outside the image: nobody blends there)
-                    const float iA = __fdividef(1.0f, r0.z), iC = __fdividef(1.0f, r1.x);
-                    const float qthr = 2.0f * __logf(r1.y * (255.0f / 0.99f));
-#pragma unroll
-                    for (int w = 0; w < kWarps; ++w) {
-                        const float bx0 = X0 + (float)((w & 1) * kBlockW), by0 = Y0 + (float)((w >> 1) * kBlockH);
-                        const float bx1 = fminf(bx0 + (float)(kBlockW - 1), (float)(W - 1));
-                        const float by1 = fminf(by0 + (float)(kBlockH - 1), (float)(H - 1));
-                        const bool in_img = bx0 <= (float)(W - 1) && by0 <= (float)(H - 1);
-                        if (in_img && entry_reaches_block(r0.x, r0.y, r0.z, r0.w, r1.x, iA, iC, qthr, bx0, bx1, by0, by1))
-                            wmask |= 1u << w;
-                    }
-                }
+                // which warps' 8 x 4 pixel blocks can it reach?
+                if (keep) wmask = entry_block_mask(r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, X0, Y0, W, H);
             }
             const uint32_t bal = __ballot_sync(0xffffffffu, keep);
             if (lane == 0) s_wcnt[warp] = __popc(bal);
