@@ -243,6 +243,56 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_probe(args):
+    """--probe: the two microprobes of SURVEY.md §8(d) (csrc/probe.cu through hyrf_probe_gather / hyrf_probe_issue):
+    the scattered-sector look-up ceiling of an L2-resident table and the sustained issue rate of fp32 code. One JSON
+    line; the copy kept under profiles/ is what `roofline.l1tex_gather` and the raster `alu` peak refer to."""
+    import torch
+    from paper_2509_17083_b200 import binding as B
+    dev = 0
+    torch.cuda.set_device(dev)
+    props = torch.cuda.get_device_properties(dev)
+    sms = props.multi_processor_count
+    sampler = ClockSampler(dev)
+    sampler.start()
+    gather = []
+    for table_mb in (32, 64):
+        for eb in (4, 8):
+            for ctas in (1, 2, 4, 8):
+                lk, sec, ms = B.probe_gather(dev, table_mb << 20, eb, ctas, share=1, line=0, iters=128)
+                gather.append({"table_mb": table_mb, "entry_bytes": eb, "ctas_per_sm": ctas, "share": 1, "line": 0,
+                               "lookups_per_s": lk, "sectors_per_s": sec, "ms": ms})
+    for share, line in ((2, 0), (4, 0), (1, 1), (2, 1)):      # lanes sharing a sector / sectors sharing a line
+        for ctas in (2, 4):
+            lk, sec, ms = B.probe_gather(dev, 64 << 20, 8, ctas, share=share, line=line, iters=128)
+            gather.append({"table_mb": 64, "entry_bytes": 8, "ctas_per_sm": ctas, "share": share, "line": line,
+                           "lookups_per_s": lk, "sectors_per_s": sec, "ms": ms})
+    issue = []
+    for kind, name in ((0, "ffma"), (1, "ffma+alu"), (2, "blend mix (1 MUFU.EX2 per 26.75 instructions)")):
+        for ctas in (1, 2, 4, 8):
+            wi, ms = B.probe_issue(dev, kind, ctas, iters=8192)
+            issue.append({"kind": name, "ctas_per_sm": ctas, "warp_instr_per_s": wi, "lane_slots_per_s": 32.0 * wi, "ms": ms})
+    clocks = sampler.stop()
+    mhz = clocks.get("sm_mhz") or load_peaks().get("sm_max_mhz", 1965.0)
+    best_sec = max(g["sectors_per_s"] for g in gather if g["share"] == 1 and g["line"] == 0)
+    best_issue = {k: max(i["warp_instr_per_s"] for i in issue if i["kind"] == k) for k in {i["kind"] for i in issue}}
+    line = {"probe": "SURVEY.md 8(d) microprobes", "gpu": props.name, "sms": sms, "clocks": clocks,
+            "gather_sectors_per_s_best": best_sec, "gather_sectors_per_clk_per_sm": best_sec / (sms * mhz * 1e6),
+            "issue_warp_instr_per_s_best": best_issue,
+            "issue_per_clk_per_sm": {k: v / (sms * mhz * 1e6) for k, v in best_issue.items()},
+            "gather": gather, "issue": issue}
+    print(json.dumps(line), flush=True)
+
+
+def load_probes():
+    """profiles/r2_probes.json (written by `python bench.py --probe`), or None."""
+    p = os.path.join(ROOT, "profiles", "r2_probes.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        return json.load(f)
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -492,12 +542,16 @@ def main():
                     help="also time hyrf_raster_backward (backward of the alpha blend, NEXT-3 first piece) on camera 0's frame")
     ap.add_argument("--rvq", action="store_true",
                     help="compressed explicit Gaussians: binary16 positions + R-VQ codes decoded at upload (PAPER.md:229 (1)-(2))")
+    ap.add_argument("--probe", action="store_true",
+                    help="run the L2 gather and issue-rate microprobes of SURVEY 8(d) instead of the render benchmark")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--cpu-threads", type=int, default=0,
                     help="--impl reference: OpenMP threads of the oracle (0 = all host cores, 1 = single-thread baseline)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.probe:
+        run_probe(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -249,6 +249,24 @@ hyrf_status hyrf_last_raster_mode(hyrf_scene* scene, int* mode);
  * rounding, not bit for bit. */
 hyrf_status hyrf_raster_backward(hyrf_scene* scene, const float* g_cfg, const float* g_T, float* grad);
 
+/* ---- microprobes ("L2 gather throughput and sustained issue rate are not in MEASURED_PEAKS.json —
+ * measure them with two microprobes first and commit the numbers"). Not on the render path; no scene needed. ------- */
+
+/* Scattered look-ups of entry_bytes (4 or 8) from a table of table_bytes (power of two; 32-64 MB stays L2-resident)
+ * — the access pattern of the grid gathers of S2 (Eq. 3). ctas_per_sm x 256 threads per SM, 8 independent
+ * look-ups in flight per lane, iters x 8 look-ups per lane. share = 1 / 2 / 4 lanes read the same 32-byte sector
+ * (2 = the two-lane gather of the field kernel); line = 1 packs four sectors of one instruction into one 128-byte
+ * line. Outputs: lane look-ups per second, distinct sectors per second, best kernel time (ms, CUDA events). */
+hyrf_status hyrf_probe_gather(int32_t device, uint64_t table_bytes, uint32_t entry_bytes, uint32_t ctas_per_sm,
+                              uint32_t share, uint32_t line, uint32_t iters, double* lookups_per_s,
+                              double* sectors_per_s, float* ms);
+
+/* Sustained issue rate of dependent-free fp32 code: kind 0 FFMA only, 1 FFMA + integer ALU (two pipes), 2 the
+ * instruction mix of the alpha-blend loop of S5 (Eq. 1: fp32 ops + one MUFU.EX2 + compares / selects per
+ * pair). Output: warp instructions per second over the whole GPU (x 32 = lane slots per second). */
+hyrf_status hyrf_probe_issue(int32_t device, uint32_t kind, uint32_t ctas_per_sm, uint32_t iters,
+                             double* warp_instr_per_s, float* ms);
+
 /* Number of kernels the last render launched (for bench.py's gpu_launches). */
 hyrf_status hyrf_last_launch_count(hyrf_scene* scene, uint32_t* launches);
 

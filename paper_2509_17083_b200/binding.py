@@ -29,7 +29,7 @@ EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_r
            "hyrf_destroy_scene", "hyrf_last_error", "hyrf_debug_enable", "hyrf_debug_fetch", "hyrf_set_timing",
            "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation", "hyrf_render_host_async",
            "hyrf_host_sync", "hyrf_set_sort_overlap", "hyrf_upload_explicit_rvq", "hyrf_last_decode_time", "hyrf_set_raster_mode",
-           "hyrf_last_raster_mode", "hyrf_raster_backward"]
+           "hyrf_last_raster_mode", "hyrf_raster_backward", "hyrf_probe_gather", "hyrf_probe_issue"]
 ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
 
 
@@ -113,6 +113,10 @@ def load_library() -> C.CDLL:
         L.hyrf_set_raster_mode.argtypes = [vp, C.c_int]
         L.hyrf_last_raster_mode.argtypes = [vp, C.POINTER(C.c_int)]
         L.hyrf_raster_backward.argtypes = [vp, vp, vp, vp]
+        L.hyrf_probe_gather.argtypes = [C.c_int32, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32,
+                                        C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_float)]
+        L.hyrf_probe_issue.argtypes = [C.c_int32, C.c_uint32, C.c_uint32, C.c_uint32, C.POINTER(C.c_double),
+                                       C.POINTER(C.c_float)]
         for name in EXPORTS:
             if name != "hyrf_last_error":
                 getattr(L, name).restype = C.c_int
@@ -127,6 +131,22 @@ def last_error() -> str:
 def _check(status: int) -> None:
     if status != HYRF_OK:
         raise HyrfError(status, last_error())
+
+
+def probe_gather(device: int, table_bytes: int, entry_bytes: int, ctas_per_sm: int, share: int = 1, line: int = 0,
+                 iters: int = 256):
+    """hyrf_probe_gather (include/hyrf.h): (lane look-ups per second, distinct sectors per second, ms)."""
+    a, b, ms = C.c_double(0), C.c_double(0), C.c_float(0)
+    _check(load_library().hyrf_probe_gather(device, table_bytes, entry_bytes, ctas_per_sm, share, line, iters,
+                                            C.byref(a), C.byref(b), C.byref(ms)))
+    return float(a.value), float(b.value), float(ms.value)
+
+
+def probe_issue(device: int, kind: int, ctas_per_sm: int, iters: int = 4096):
+    """hyrf_probe_issue (include/hyrf.h): (warp instructions per second, ms)."""
+    a, ms = C.c_double(0), C.c_float(0)
+    _check(load_library().hyrf_probe_issue(device, kind, ctas_per_sm, iters, C.byref(a), C.byref(ms)))
+    return float(a.value), float(ms.value)
 
 
 def camera_struct(cam) -> CameraC:
@@ -148,8 +168,9 @@ def _grid_desc(g, keep: list) -> GridDesc:
 
 
 def make_desc(scene, max_width: int, max_height: int, device: int = 0, mlp_path: int = HYRF_MLP_AUTO,
-              keep: Optional[list] = None) -> SceneDesc:
-    """hyrf_scene_desc from an object with the attribute names of synth.Scene."""
+              keep: Optional[list] = None, allocator=None) -> SceneDesc:
+    """hyrf_scene_desc from an object with the attribute names of synth.Scene. `allocator`: optional object with
+    alloc(nbytes) -> device address (0 on failure) and release(address); it becomes hyrf_scene_desc.alloc / .release."""
     keep = keep if keep is not None else []
     d = SceneDesc()
     d.n_gaussians = int(scene.n)
@@ -167,8 +188,13 @@ def make_desc(scene, max_width: int, max_height: int, device: int = 0, mlp_path:
     d.cull_tol, d.z_near, d.bg_radius, d.tau_T = (float(scene.cull_tol), float(scene.z_near),
                                                   float(scene.bg_radius), float(scene.tau_T))
     d.max_width, d.max_height, d.device = int(max_width), int(max_height), int(device)
-    d.alloc = ALLOC_FN()
-    d.release = RELEASE_FN()
+    if allocator is None:
+        d.alloc = ALLOC_FN()
+        d.release = RELEASE_FN()
+    else:
+        d.alloc = ALLOC_FN(lambda nbytes, user: allocator.alloc(int(nbytes)) or None)
+        d.release = RELEASE_FN(lambda ptr, user: allocator.release(int(ptr or 0)))
+        keep.extend([d.alloc, d.release, allocator])
     d.user = None
     d._keep = keep
     return d
@@ -186,7 +212,7 @@ class HyrfScene:
     tensors (device pointers) unless `host_upload=True` (numpy host pointers)."""
 
     def __init__(self, scene, max_width: Optional[int] = None, max_height: Optional[int] = None, device: int = 0,
-                 mlp_path: int = HYRF_MLP_AUTO, host_upload: bool = False):
+                 mlp_path: int = HYRF_MLP_AUTO, host_upload: bool = False, allocator=None):
         import torch
         self._torch = torch
         self.lib = load_library()
@@ -195,7 +221,7 @@ class HyrfScene:
         mw = max_width or max([c.W for c in cams] + [16])
         mh = max_height or max([c.H for c in cams] + [16])
         self._keep: list = []
-        self.desc = make_desc(scene, mw, mh, device, mlp_path, self._keep)
+        self.desc = make_desc(scene, mw, mh, device, mlp_path, self._keep, allocator)
         self.handle = C.c_void_p()
         _check(self.lib.hyrf_create_scene(C.byref(self.desc), C.byref(self.handle)))
         self.fp16 = bool(scene.fp16)

@@ -190,9 +190,13 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
             return hy_fail(HYRF_ERR_INVALID_ARG, "aabb axis %d is empty or non-finite", a);
     if (desc->param_dtype != HYRF_F32 && desc->param_dtype != HYRF_F16 && desc->param_dtype != HYRF_U8)
         return hy_fail(HYRF_ERR_INVALID_ARG, "unknown param_dtype %d", (int)desc->param_dtype);
-    if (!(desc->bg_radius > 0.0f) || !isfinite(desc->cull_tol) || desc->cull_tol < 0.0f || !isfinite(desc->z_near) ||
-        !isfinite(desc->tau_T))
-        return hy_fail(HYRF_ERR_INVALID_ARG, "bg_radius / cull_tol / z_near / tau_T out of range");
+    // z_near > 0: the depth key is the bit pattern of Z and the projection divides by Z (DESIGN.md §2 D1, D8, D9);
+    // tau_T is a transmittance
+    if (!(desc->bg_radius > 0.0f) || !isfinite(desc->bg_radius) || !isfinite(desc->cull_tol) || desc->cull_tol < 0.0f ||
+        !isfinite(desc->z_near) || !(desc->z_near > 0.0f) || !(desc->tau_T >= 0.0f) || !(desc->tau_T <= 1.0f))
+        return hy_fail(HYRF_ERR_INVALID_ARG, "bg_radius (> 0) / cull_tol (>= 0) / z_near (> 0) / tau_T (in [0, 1]) out of range");
+    if ((size_t)desc->n_gaussians > hy_radix_max_items())
+        return hy_fail(HYRF_ERR_UNSUPPORTED, "n_gaussians %u exceeds the %zu items the depth sort supports", desc->n_gaussians, hy_radix_max_items());
     if ((desc->alloc == nullptr) != (desc->release == nullptr))
         return hy_fail(HYRF_ERR_INVALID_ARG, "alloc and release must be given together");
     if (desc->dir_pe_octaves == 0 || desc->dir_pe_octaves > 6)
@@ -219,10 +223,14 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     }
     if (desc->device < 0 || desc->device >= ndev) return hy_fail(HYRF_ERR_INVALID_ARG, "device %d outside [0, %d)", desc->device, ndev);
     if ((e = cudaSetDevice(desc->device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
+    int sm_count = 0;
+    if ((e = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, desc->device)) != cudaSuccess || sm_count < 1)
+        return hy_cuda_fail(e, "cudaDeviceGetAttribute(MultiProcessorCount)");
 
     hyrf_scene* s = new (std::nothrow) hyrf_scene();
     if (!s) return hy_fail(HYRF_ERR_OOM, "host allocation failed");
     s->desc = *desc;
+    s->sm_count = sm_count;   // persistent grids and the CTA slots left to the depth sort are sized from it
     s->res_geo.assign(desc->geo_grid.level_res, desc->geo_grid.level_res + desc->geo_grid.levels);
     s->res_app.assign(desc->app_grid.level_res, desc->app_grid.level_res + desc->app_grid.levels);
     s->res_bg.assign(desc->bg_grid.level_res, desc->bg_grid.level_res + desc->bg_grid.levels);
@@ -564,7 +572,21 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     // binning, the lists by the rasterizer itself (what it consumed, in the order it consumed it).
     const uint32_t n_macro = (uint32_t)(f.mgx * f.mgy);
     const bool want_lists = ((s->debug_mask >> HYRF_DBG_TILE_LIST) | (s->debug_mask >> HYRF_DBG_TILE_RANGES)) & 1u;
-    if (s->bin_ws && hy_bin_ordered_supported(s->N, n_macro) && (!want_lists || hy_bin_ordered_supported(s->N, n_tiles))) {
+    const bool ordered = s->bin_ws && hy_bin_ordered_supported(s->N, n_macro) && (!want_lists || hy_bin_ordered_supported(s->N, n_tiles));
+    if (ordered && want_lists) {
+        // The export makes the rasterizer write every tile's list (D entries) into the pair buffer, and nothing there
+        // checks a bound: learn D BEFORE anything is binned and grow first. (Without the export the frame is enqueued
+        // blind and only re-binned on overflow: the binning itself clamps to the capacity.) The stream has joined the
+        // depth sort by now, so synchronising it also covers the sort's use of the workspace that growing reallocates.
+        if ((e = cudaEventSynchronize(s->ev_counters)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventSynchronize(counters)");
+        const uint64_t need = s->counters_host->D > s->counters_host->Dm ? s->counters_host->D : s->counters_host->Dm;
+        if (need >= 0xFFFFFFFFull) return hy_fail(HYRF_ERR_OOM, "tile-entry count %llu does not fit 32-bit offsets", (unsigned long long)need);
+        if (need > s->d_capacity) {
+            if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(grow)");
+            if ((st = ensure_entries(s, (size_t)need)) != HYRF_OK) return st;
+        }
+    }
+    if (ordered) {
         // everything is sized on the device, so the whole frame is enqueued before the host looks at the counters;
         // only a frame whose entry count outgrew the list buffer is re-binned after growing it
         for (int attempt = 0;; ++attempt) {

@@ -102,7 +102,7 @@ hyrf_status hy_launch_background(hyrf_scene* s, const FrameDev& f, float* out_rg
     const size_t smem = ((size_t)m.in_dim * m.hidden + (size_t)(m.n_hidden - 1) * m.hidden * m.hidden + (size_t)m.hidden * 3) * sizeof(float);
     const int P = f.W * f.H;
     const int need = (P + kBgThreads - 1) / kBgThreads;
-    const int grid = need < 148 * 8 ? need : 148 * 8;
+    const int grid = need < s->sm_count * 8 ? need : s->sm_count * 8;
     const uint32_t L = s->desc.bg_grid.levels;
     const bool std_in = m.in_dim == 2 * L + 24 && s->desc.dir_pe_octaves == 4 && m.n_hidden == 1;
     hyrf_status st;

@@ -103,9 +103,7 @@ hyrf_status hy_launch_explicit_decode(hyrf_scene* s, const uint16_t* pos_h, cons
     const bool in_smem = book_bytes <= kBookSmemMax;
     const size_t smem = in_smem ? book_bytes : 0;
     const bool vec4 = (n % 4 == 0) && ((reinterpret_cast<uintptr_t>(pos_h) | reinterpret_cast<uintptr_t>(codes)) % 8 == 0);
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int sms = s->sm_count;
     const uint32_t groups = vec4 ? n / 4 : n;
     const uint32_t want = (groups + kDecodeThreads - 1) / kDecodeThreads;
     int per_sm = 1;   // one wave of resident CTAs, grid-stride beyond

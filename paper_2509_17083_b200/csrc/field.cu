@@ -125,7 +125,7 @@ hyrf_status hy_launch_field_fma(hyrf_scene* s, const FrameDev& f, uint32_t* laun
     const size_t nw_app = (size_t)a.in_dim * a.hidden + (size_t)(a.n_hidden - 1) * a.hidden * a.hidden + (size_t)a.hidden * 3;
     const size_t smem = (nw_geo + nw_app) * sizeof(float);
     const int need = (int)((s->N + kFieldThreads - 1) / kFieldThreads);
-    const int grid = need < 148 * 3 ? need : 148 * 3;
+    const int grid = need < s->sm_count * 3 ? need : s->sm_count * 3;
     const uint32_t L = s->desc.geo_grid.levels;
     const bool same = s->desc.app_grid.levels == L && g.hidden == a.hidden && g.n_hidden == a.n_hidden &&
                       g.in_dim == 2 * L && a.in_dim == 2 * L + 24 && s->desc.dir_pe_octaves == 4;

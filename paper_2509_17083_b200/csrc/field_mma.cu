@@ -877,8 +877,7 @@ size_t hy_field_mma_packed_bytes() { return kPackedBytes + kWPackedU4 * 16; }   
 hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* launches) {
     FieldArgs A;
     hy_fill_field_args(s, f, &A);
-    static bool attr_done[64] = {};   // per device: function attributes belong to the device's context
-    bool& attr_set = attr_done[s->desc.device & 63];
+    bool& attr_set = s->field_attr_set;   // per scene (one device each; a scene is used by one thread at a time)
     if (!attr_set) {
         const void* ks[4] = {(const void*)field_mma_kernel<false>, (const void*)field_mma_kernel<true>,
                              (const void*)field_mma_pipe_kernel<false>, (const void*)field_mma_pipe_kernel<true>};
@@ -897,13 +896,13 @@ hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* laun
     // CTA slots left to the depth sort running beside this kernel (hyrf_set_sort_overlap): with none, the persistent
     // CTAs hold every register of every SM and the sort waits for the kernel to end. Config 3, frame time against the
     // slots left free: 0 -> 0.586, 16 -> 0.563, 32 -> 0.551, 48 -> 0.561 ms (serial: 0.620 ms).
-    const int gap = s->sort_overlap ? 32 : 0;
-    const int slots = 148 * 2 - gap;
+    const int gap = s->sort_overlap ? (32 * s->sm_count) / 148 : 0;
+    const int slots = s->sm_count * 2 - gap;
     const int grid = need < slots ? need : slots;
     const uint4* w = reinterpret_cast<const uint4*>(s->mma_w);
     if (s->both_table && s->warp_mma) {
         const int needw = (int)((s->N + kWThreads - 1) / kWThreads);
-        const int slotsw = 148 - gap / 2;
+        const int slotsw = s->sm_count - gap / 2;
         const int gridw = needw < slotsw ? needw : slotsw;
         const uint4* ww = reinterpret_cast<const uint4*>(reinterpret_cast<const uint8_t*>(s->mma_w) + kPackedBytes);
         if (s->u8) field_warp_kernel<true><<<gridw, kWThreads, kWarpSmemBytes, s->stream>>>(A, ww, s->both_table);

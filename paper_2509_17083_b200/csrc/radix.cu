@@ -195,7 +195,9 @@ void hy_launch_radix(uint32_t* key_a, uint32_t* val_a, uint32_t* key_b, uint32_t
         const size_t slices = state_slices(nb + 1);
         const size_t slice = (nb + 1) * 256;
         cudaMemsetAsync(ws, 0, (kWsState + (slices > 1 ? (size_t)passes * slice : 0)) * sizeof(uint32_t), st);
-        const unsigned hgrid = (unsigned)(nb < 148 * 8 ? nb : 148 * 8);
+        int dev = 0, sms = 0;   // grid-stride histogram: one wave of resident CTAs
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) sms = 1;
+        const unsigned hgrid = (unsigned)(nb < (size_t)sms * 8 ? nb : (size_t)sms * 8);
         radix_global_hist_kernel<<<hgrid, kRadixThreads, 0, st>>>(ki, n_cap, n_dev, passes, key_bits, ws + kWsHist);
         ++*launches;
         for (int p = 0; p < passes; ++p) {

@@ -7,7 +7,17 @@
 // [X0, X1] x [Y0, Y1]? The quadratic form q = A dx^2 + 2 B dx dy + C dy^2 is convex, so its minimum over the pixel box
 // is 0 when the mean lies inside, else it sits on a face whose plane separates the mean from the box: at most two
 // one-dimensional minimisations. alpha <= o exp(-q_min / 2) everywhere in the tile; entries below the threshold
-// (with a 1 % margin against rounding) would be skipped by every pixel, so dropping them changes no output bit.
+// would be skipped by every pixel, so dropping them changes no output bit — PROVIDED the comparison allows for the
+// rounding of both sides: this q_min and every pixel's own `power` are binary32 sums of three terms that cancel on
+// long thin splats (near-degenerate conic: A ex^2 ~ 1e5-1e6 against q ~ 10), each off by a few ulp of its largest
+// term. hy_q_slack bounds the terms over the whole box (any pixel's |dx| <= max(|X0-u|, |X1-u|), same for dy) and
+// allows 16 ulp of that sum, on top of a fixed 1 % margin on alpha (0.02 in q) for the MUFU exp / log.
+__device__ __forceinline__ float hy_q_slack(float u, float v, float A, float B, float C, float X0, float X1, float Y0,
+                                            float Y1) {
+    const float mx = fmaxf(fabsf(X0 - u), fabsf(X1 - u)), my = fmaxf(fabsf(Y0 - v), fabsf(Y1 - v));
+    return 2.0e-6f * (A * mx * mx + 2.0f * fabsf(B) * mx * my + C * my * my);
+}
+
 __device__ __forceinline__ bool entry_reaches_tile(float u, float v, float A, float B, float C, float o, float X0,
                                                    float X1, float Y0, float Y1) {
     const float ex = fminf(fmaxf(u, X0), X1) - u, ey = fminf(fmaxf(v, Y0), Y1) - v;
@@ -21,11 +31,12 @@ __device__ __forceinline__ bool entry_reaches_tile(float u, float v, float A, fl
         const float dx = fminf(fmaxf(__fdividef(-B * ey, A), X0 - u), X1 - u);
         qmin = fminf(qmin, A * dx * dx + 2.0f * B * dx * ey + C * ey * ey);
     }
+    qmin -= hy_q_slack(u, v, A, B, C, X0, X1, Y0, Y1);
     return !(o * __expf(-0.5f * qmin) < 0.99f / 255.0f);   // NaN keeps the entry
 }
 
 // The same test for a sub-rectangle of the tile, with the per-entry work hoisted: iA = 1 / A, iC = 1 / C,
-// qthr = 2 ln(o * 255 / 0.99) (alpha >= 0.99 / 255  <=>  q <= qthr). NaN keeps the entry.
+// qthr = 2 ln(o * 255 / 0.99) + the tile's hy_q_slack (alpha >= 0.99 / 255  <=>  q <= 2 ln(o 255 / 0.99)). NaN keeps the entry.
 __device__ __forceinline__ bool entry_reaches_block(float u, float v, float A, float B, float C, float iA, float iC,
                                                     float qthr, float X0, float X1, float Y0, float Y1) {
     const float ex = fminf(fmaxf(u, X0), X1) - u, ey = fminf(fmaxf(v, Y0), Y1) - v;
@@ -54,7 +65,8 @@ __device__ __forceinline__ float ex2_ftz(float x) {
 __device__ __forceinline__ uint32_t entry_block_mask(float u, float v, float A, float B, float C, float o, float X0,
                                                      float Y0, int W, int H) {
     const float iA = __fdividef(1.0f, A), iC = __fdividef(1.0f, C);
-    const float qthr = 2.0f * __logf(o * (255.0f / 0.99f));
+    const float qthr = 2.0f * __logf(o * (255.0f / 0.99f)) +
+                       hy_q_slack(u, v, A, B, C, X0, fminf(X0 + 15.0f, (float)(W - 1)), Y0, fminf(Y0 + 15.0f, (float)(H - 1)));
     uint32_t m = 0;
 #pragma unroll
     for (int w = 0; w < 8; ++w) {

@@ -40,6 +40,8 @@ struct hyrf_scene {
     bool warp_mma = false;     // decoders on warp-level mma.sync (field_warp_kernel) instead of tcgen05 (field_mma.cu)
     cudaStream_t stream = 0;
     uint32_t N = 0;
+    int sm_count = 0;          // cudaDevAttrMultiProcessorCount of desc.device (148 on a full B200)
+    bool field_attr_set = false;   // cudaFuncSetAttribute of the tensor-core field kernels done for this scene's device
 
     // persistent parameters
     float* pos = nullptr;      // [3][N]

@@ -3,7 +3,7 @@ on the same seeded inputs. Marked gpu: they run on the B200 box."""
 import numpy as np
 import pytest
 
-from parity_util import compare_frame
+from parity_util import compare_frame, compare_handoff
 
 pytestmark = pytest.mark.gpu
 
@@ -32,8 +32,12 @@ def _run(B, ho, scene, cams=None, mlp_path=None, exact=True, label="", ablation=
         torch.cuda.synchronize()
         gpu = hs.debug_all(cam.W, cam.H)
         orc = ho.render(osc, cam, ablation=ablation)
-        stats.append(compare_frame(orc, gpu, out.cpu().numpy(), scene.tau_T, fp16=scene.fp16, exact_geometry=exact,
-                                   label=f"{label or scene.name} cam{ci}"))
+        lab = f"{label or scene.name} cam{ci} mlp{mlp_path} abl{ablation} r{raster_mode}"
+        if exact:
+            stats.append(compare_frame(orc, gpu, out.cpu().numpy(), scene.tau_T, fp16=scene.fp16, label=lab))
+        else:   # tensor-core decoders: stages 1-3 by tolerance, stages 4-6 by hand-off (bit-exact lists), SURVEY H1
+            stats.append(compare_handoff(ho, osc, cam, orc, gpu, out.cpu().numpy(), scene.tau_T, fp16=scene.fp16,
+                                         label=lab, ablation=ablation))
     hs.close()
     return stats
 
@@ -101,6 +105,11 @@ def test_edge_cases(B, ho, synth):
     s = synth.tiny_scene(n=40, W=64, H=48, scale_mean=1.5)
     st = _run(B, ho, s, cams=s.cameras[:1])
     assert st[0]["D"] >= 0.5 * st[0]["V"] * 12
+    # (e) fx != fy on a non-square image: limx / limy, the Jacobian and the ray directions each use their own focal length
+    s = synth.tiny_scene(n=200, W=80, H=48, seed=21)
+    for c in s.cameras:
+        c.fy = float(np.float32(2.0 * c.fx))
+    _run(B, ho, s)
     # (d) tau_T = 0 composites everywhere; tau_T = 1 nowhere
     for tau in (0.0, 1.0):
         s = synth.tiny_scene(n=48, W=32, H=32)
@@ -194,19 +203,24 @@ def test_tensor_core_path_high_gain(B, ho, synth, path):
 
 
 def test_config3_full_one_camera_both_paths(B, ho, synth):
-    # BASELINE config 3 at full size (1M Gaussians, 1280x720), camera 0: exact path bit-exact lists, tensor path by
-    # tolerance; this is the workload and launch configuration bench.py times
+    # BASELINE config 3 at full size (1M Gaussians, 1280x720), camera 0: exact path bit-exact lists; tensor paths by
+    # hand-off (lists bit-exact given the GPU's attributes); AUTO is the workload and launch configuration bench.py times
     s = synth.make_scene(3, n_cameras=1)
     _run(B, ho, s, mlp_path=B.HYRF_MLP_FMA, exact=True)
-    _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False)
+    st = _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False, label="config3_full_AUTO")
+    print("config 3 full, tcgen05 path:", {k: v for k, v in st[0].items() if not isinstance(v, list)})
+    _run(B, ho, s, mlp_path=B.HYRF_MLP_HMMA, exact=False, label="config3_full_HMMA")
 
 
-def test_config4_full_one_camera_bench_path(B, ho, synth):
-    # BASELINE config 4 at full size (2M Gaussians, unbounded scene, 1245x825 with ragged tiles), camera 0, in the
-    # launch configuration bench.py --config 4 times (AUTO -> tensor-core decoders, ordered binning)
+def test_config4_full_one_camera_both_paths(B, ho, synth):
+    # BASELINE config 4 at full size (2M Gaussians, unbounded scene, 1245x825 with ragged tiles), camera 0: the launch
+    # configuration bench.py --config 4 times (AUTO -> tensor-core decoders, ordered binning) by hand-off, and the exact
+    # path with every list compared bit for bit
     s = synth.make_scene(4, n_cameras=1)
-    st = _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False)
+    st = _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False, label="config4_full_AUTO")
     assert st[0]["V"] > 1_000_000
+    print("config 4 full, tcgen05 path:", {k: v for k, v in st[0].items() if not isinstance(v, list)})
+    _run(B, ho, s, mlp_path=B.HYRF_MLP_FMA, exact=True, label="config4_full_FMA")
 
 
 def test_config5_points(B, ho, synth):
@@ -217,6 +231,13 @@ def test_config5_points(B, ho, synth):
     _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False)
     s = synth.make_scene(5, n_gaussians=500_000, width=1920, height=1080)
     _run(B, ho, s, mlp_path=B.HYRF_MLP_FMA, exact=True)
+
+
+def test_config5_500k_at_4k_exact_lists(B, ho, synth):
+    # BASELINE config 5, 500k @ 3840x2160 (32,400 tiles, D ~ 57M entries): exact path, every per-tile list bit for bit
+    s = synth.make_scene(5, n_gaussians=500_000, width=3840, height=2160)
+    st = _run(B, ho, s, mlp_path=B.HYRF_MLP_FMA, exact=True, label="config5_500k_4K_FMA")
+    assert st[0]["D"] > 40_000_000
 
 
 @pytest.mark.parametrize("abl", [1, 2, 4, 8, 1 | 2, 4 | 8, 15])
@@ -414,16 +435,17 @@ def test_fields_then_explicit_upload_order(B, ho, synth):
     hs.close()
 
 
-def test_config5_largest_point_sampled(B, ho, synth):
+@pytest.mark.parametrize("n,W,H", [(4_000_000, 3840, 2160), (4_000_000, 1920, 1080), (4_000_000, 256, 256)])
+def test_config5_4m_points_sampled(B, ho, synth, n, W, H):
     # BASELINE config 5's largest point (4M Gaussians at 3840x2160, D ~ 4e8 tile entries) in the launch configuration
     # bench.py --config 5 times (AUTO decoders, macro-tile binning, per-tile lists NOT materialised). The oracle cannot
     # bin 4e8 entries in seconds, so: cull element by element; stages 2-4a on 4096 sampled Gaussians; stages 4b-5 on
     # 24 sampled tiles whose depth-ordered lists are rebuilt one by one from the exported records (hand-off)
     # and rasterised by the oracle; stage 6 on the whole image from the exported (C_fg, T); properties everywhere.
+    # (the 1080p and 256x256 points of the 4M row go through the same protocol)
     import torch
-    s = synth.make_scene(5, n_gaussians=4_000_000, width=3840, height=2160)
+    s = synth.make_scene(5, n_gaussians=n, width=W, height=H)
     cam = s.cameras[0]
-    W, H = cam.W, cam.H
     hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_AUTO)
     hs.debug_enable(B.DBG_ALL & ~((1 << B.DBG_TILE_LIST) | (1 << B.DBG_TILE_RANGES)))
     out = hs.render(cam)
@@ -458,8 +480,9 @@ def test_config5_largest_point_sampled(B, ho, synth):
     ranges = np.zeros((gx * gy, 2), np.uint32)
     lists, pos, sampled = [], 0, []
     cx, cy = gx // 2, gy // 2
-    cand = [(cx, cy), (cx - 7, cy + 3), (0, 0), (gx - 1, gy - 1), (gx - 1, 0)] + \
-           [(int(rng.integers(gx // 4, 3 * gx // 4)), int(rng.integers(gy // 4, 3 * gy // 4))) for _ in range(19)]
+    n_rand = 19 if W > 1000 else 3            # 256 x 256: every tile holds ~10^5 entries of the 4M scene
+    cand = [(cx, cy), (max(cx - 7, 0), min(cy + 3, gy - 1)), (0, 0), (gx - 1, gy - 1), (gx - 1, 0)] + \
+           [(int(rng.integers(gx // 4, 3 * gx // 4)), int(rng.integers(gy // 4, 3 * gy // 4))) for _ in range(n_rand)]
     for tx, ty in cand:
         t = ty * gx + tx
         if t in sampled:
@@ -587,3 +610,123 @@ def test_raster_backward_needs_the_lists(B, synth):
         hs.raster_backward(z, z[..., 0], 16)
     assert e.value.status == B.HYRF_ERR_NOT_READY
     hs.close()
+
+
+def _adversarial_scene(synth, n=600, W=1280, H=720, seed=31):
+    # Long thin splats for the reach tests of csrc/raster_common.cuh (VERDICT r1 finding 4): config-2 recipe with
+    # high-gain tables and the geometry decoder's output rows scaled so that s_n spreads over +-5 logits around
+    # s_e = 0: scales sigma(-5) .. sigma(5) = 0.0067 .. 0.993 world units -> anisotropy up to 150:1, splats hundreds of
+    # pixels long and a few pixels wide at random orientations (r_n is as random as s_n); opacity logits N(-2.5, 2.5)
+    # put many peak alphas near the 1/255 threshold. 3600 tiles -> macro-tile lists.
+    s = synth.make_scene(2, n_gaussians=n, width=W, height=H, n_cameras=1, table_amp=1.0, seed=seed)
+    rng = np.random.default_rng(seed)
+    s.scale_logit[:] = rng.normal(0.0, 0.5, n).astype(np.float32)
+    s.opacity_logit[:] = rng.normal(-2.5, 2.5, n).astype(np.float32)
+    w = s.geo_w.copy()
+    m = s.geo_mlp
+    off = m.in_dim * m.hidden + (m.n_hidden - 1) * m.hidden * m.hidden
+    out = w[off:].reshape(m.out_dim, m.hidden)
+    out[1:4] *= 40.0          # rows of s_n
+    out[4:8] *= 10.0          # rows of r_n
+    s.geo_w = w
+    s.cameras = [synth.look_at(np.array([0.3, 0.2, -3.0]), W, H)]
+    s.name = f"adversarial_n{n}_{W}x{H}"
+    return s
+
+
+def test_adversarial_long_thin_splats(B, ho, synth):
+    import torch
+    s = _adversarial_scene(synth)
+    osc = ho.OracleScene(s)
+    cam = s.cameras[0]
+    orc = ho.render(osc, cam)
+    # the scene really is adversarial: anisotropy >= 100:1 and splats >= 500 px long, peak alphas around the threshold
+    sc = orc["attrs"][:, :3]
+    assert (sc.max(axis=1) / sc.min(axis=1)).max() >= 100.0
+    assert orc["radius"].max() >= 250.0                       # 3 sigma on each side
+    live = orc["tiles"] > 0
+    assert (np.abs(orc["proj"][live][:, 6] - 1.0 / 255.0) < 2e-3).sum() >= 5
+    outs = {}
+    for mode in (1, 2):
+        st = _run(B, ho, s, raster_mode=mode, label=f"adversarial_mode{mode}")
+        assert st[0]["D"] > 50 * st[0]["V"]
+        hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_FMA)
+        hs.set_raster_mode(mode)
+        o = hs.render(cam)
+        torch.cuda.synchronize()
+        outs[mode] = (o.cpu().numpy().copy(), hs.debug_fetch(B.DBG_FINAL_T).copy())
+        hs.close()
+    assert (outs[1][0].view(np.uint32) == outs[2][0].view(np.uint32)).all()
+    assert (outs[1][1].view(np.uint32) == outs[2][1].view(np.uint32)).all()
+    # and at a ragged small resolution with per-tile lists (<= 1024 tiles)
+    s2 = _adversarial_scene(synth, n=200, W=333, H=250, seed=32)
+    for mode in (1, 2):
+        _run(B, ho, s2, raster_mode=mode, label=f"adversarial_small_mode{mode}")
+
+
+def test_single_shared_field(B, ho, synth):
+    # PAPER.md:233, Table 5 "w/o Decouple": one field for all properties. The pass has no switch for it: the SAME table
+    # is uploaded as the geometry and the appearance field (hyrf.h hyrf_set_ablation). Oracle vs GPU on every decoder
+    # path; high-gain entries so that reading the wrong half of an interleaved entry cannot hide.
+    s = synth.make_scene(3, n_gaussians=30_000, width=320, height=180, n_cameras=2, table_amp=1.0)
+    s.app_table = s.geo_table
+    _run(B, ho, s, mlp_path=B.HYRF_MLP_FMA, exact=True, label="shared_field_FMA")
+    for path in ("MMA", "HMMA"):
+        st = _run(B, ho, s, mlp_path=getattr(B, "HYRF_MLP_" + path), exact=False, label="shared_field_" + path)
+        assert st[0]["raw_geo_maxdiff"] > 0.0
+    t = synth.tiny_scene(n=64, W=48, H=40, seed=13)           # run-time-shaped kernels, fp32
+    t.app_table = t.geo_table
+    _run(B, ho, t, label="shared_field_tiny")
+
+
+class _GuardAllocator:
+    """hyrf_scene_desc.alloc backed by torch, with a canary-filled guard band on both sides of every allocation."""
+    GUARD = 1 << 16
+
+    def __init__(self, torch):
+        self.torch, self.live = torch, {}
+
+    def alloc(self, nbytes):
+        t = self.torch.full((nbytes + 2 * self.GUARD,), 0xA5, dtype=self.torch.uint8, device="cuda")
+        self.live[t.data_ptr() + self.GUARD] = (t, nbytes)
+        return t.data_ptr() + self.GUARD
+
+    def release(self, ptr):
+        self.check_one(ptr)
+        del self.live[ptr]
+
+    def check_one(self, ptr):
+        t, nbytes = self.live[ptr]
+        assert bool((t[:self.GUARD] == 0xA5).all()), "write below an allocation"
+        assert bool((t[self.GUARD + nbytes:] == 0xA5).all()), f"write beyond an allocation of {nbytes} bytes"
+
+    def check(self):
+        self.torch.cuda.synchronize()
+        for p in list(self.live):
+            self.check_one(p)
+
+
+def test_list_export_beyond_initial_capacity_stays_in_bounds(B, ho, synth):
+    # ADVICE r1 (high): with the per-tile lists exported and D above the scratch's first size, the rasterizer wrote the
+    # lists past the pair buffer before the host grew it. Every library allocation sits between canary bands here.
+    import torch
+    s = synth.make_scene(3, n_gaussians=20_000, width=640, height=360, n_cameras=1)     # 920 tiles -> per-tile lists
+    s.scale_logit[:] = -1.0                                     # big splats: D far above 4 N + 65536
+    for (W, H) in ((640, 360), (1280, 720)):                    # per-tile lists, then macro-tile lists (3600 tiles)
+        s.cameras = [synth.look_at(np.array([4.0, 0.0, 0.0]), W, H)]
+        ga = _GuardAllocator(torch)
+        hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_FMA, allocator=ga)
+        hs.debug_enable()
+        out = hs.render(s.cameras[0])
+        ga.check()
+        cnt = hs.debug_fetch(B.DBG_COUNTERS)
+        assert int(cnt[2]) > 4 * s.n + 65536 + (4 * s.n + 65536) // 4 + 4096      # above the first capacity
+        gpu = hs.debug_all(W, H)
+        orc = ho.render(ho.OracleScene(s), s.cameras[0])
+        compare_frame(orc, gpu, out.cpu().numpy(), s.tau_T, fp16=True, label=f"guarded_{W}x{H}")
+        hs.debug_enable(0)                                      # and the blind path: re-binned after growing
+        hs.render(s.cameras[0])
+        ga.check()
+        hs.close()
+        torch.cuda.synchronize()
+        assert not ga.live

@@ -88,6 +88,42 @@ def test_cull_hand_placed_points(ho, synth):
     assert idx.tolist() == [0, 1, 3, 4, 7, 9]
 
 
+def test_cull_non_square_image_and_anisotropic_focal(ho, synth):
+    # every other cull pin has W = H and fx = fy, so a W <-> H or fx <-> fy slip in limx / limy would pass.
+    # 160 x 96 image, fx = 50, fy = 100: W/(2 fx) = 1.6, H/(2 fy) = 0.48 (D1: limx = (1 + tol) W / (2 fx),
+    # limy = (1 + tol) H / (2 fy), fp32). z = 2 keeps lim * z exact, so "on the plane" is well defined.
+    cam = synth.Camera(R=np.eye(3, dtype=np.float32), t=np.zeros(3, np.float32), fx=50.0, fy=100.0, cx=79.5, cy=47.5,
+                       W=160, H=96)
+    one_tol = np.float32(1.0) + np.float32(0.1)
+    limx = one_tol * (np.float32(160.0) / (np.float32(2.0) * np.float32(50.0)))
+    limy = one_tol * (np.float32(96.0) / (np.float32(2.0) * np.float32(100.0)))
+    assert abs(float(limx) - 1.76) < 1e-6 and abs(float(limy) - 0.528) < 1e-6
+    up = lambda v: np.nextafter(np.float32(v), np.float32(1e9))
+    pts = [
+        (0, limy * 2, 2),            # exactly on the bottom plane: keep
+        (0, up(limy * 2), 2),        # one ulp below it: cull
+        (0, -limy * 2, 2),           # exactly on the top plane: keep
+        (0, -up(limy * 2), 2),       # one ulp above it: cull
+        (limx * 2, 0, 2),            # exactly on the right plane: keep
+        (up(limx * 2), 0, 2),        # one ulp outside: cull
+        (-limx * 2, 0, 2),           # exactly on the left plane: keep
+        (1.7 * 2, 0, 2),             # inside limx = 1.76; outside every swapped variant (H/(2fx): 1.056, W/(2fy): 0.88, H/(2fy): 0.528)
+        (0, 0.6 * 2, 2),             # outside limy = 0.528; inside every swapped variant (0.88, 1.056, 1.76)
+        (1.7 * 2, limy * 2, 2),      # corner of the band: keep
+    ]
+    s = _cull_scene(synth, pts)
+    mask, idx = ho.stage_cull(ho.OracleScene(s), cam, 160, 96)
+    assert mask.tolist() == [1, 0, 1, 0, 1, 0, 1, 1, 0, 1]
+    assert idx.tolist() == [0, 2, 4, 6, 7, 9]
+    # the same through a rotated camera (rows of R permuted: camera x = world y, camera y = world x), so that the
+    # limits are tied to the CAMERA axes, not to the world's
+    Rp = np.array([[0, 1, 0], [1, 0, 0], [0, 0, 1]], np.float32)
+    cam2 = synth.Camera(R=Rp, t=np.zeros(3, np.float32), fx=50.0, fy=100.0, cx=79.5, cy=47.5, W=160, H=96)
+    s2 = _cull_scene(synth, [(p[1], p[0], p[2]) for p in pts])
+    mask2, _ = ho.stage_cull(ho.OracleScene(s2), cam2, 160, 96)
+    assert mask2.tolist() == mask.tolist()
+
+
 def test_cull_infinite_tolerance_keeps_everything_in_front(ho, synth):
     s = synth.make_scene(1)
     s.cull_tol = 1e30
