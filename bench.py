@@ -314,7 +314,7 @@ def run_ours(args):
     cams_all = scene.cameras
     mine = synth.shard_cameras(len(cams_all), rank, world) or [rank % len(cams_all)]
     cams = [cams_all[i] for i in mine]                      # frame-parallel replicas: no data-path collective
-    path = {"auto": B.HYRF_MLP_AUTO, "fma": B.HYRF_MLP_FMA, "mma": B.HYRF_MLP_MMA, "hmma": B.HYRF_MLP_HMMA}[args.mlp]
+    path = {"auto": B.HYRF_MLP_AUTO, "fma": B.HYRF_MLP_FMA, "mma": B.HYRF_MLP_MMA, "hmma": B.HYRF_MLP_HMMA, "ws": B.HYRF_MLP_WS}[args.mlp]
     hs = B.HyrfScene(scene, device=dev, mlp_path=path)
     hs.set_ablation(args.ablation)
     hs.set_raster_mode({"auto": 0, "tile": 1, "warp": 2}[args.raster])
@@ -469,7 +469,7 @@ def run_ours(args):
     if rank != 0:
         return
     names = ["cull", "field", "bin", "raster", "background"]
-    kernels = {"field": ("field_warp_kernel" if args.mlp == "hmma" else "field_mma_pipe_kernel") if scene.fp16 and args.mlp != "fma"
+    kernels = {"field": ("field_warp_kernel" if args.mlp == "hmma" else ("field_ws_kernel" if args.mlp == "ws" else "field_mma_pipe_kernel")) if scene.fp16 and args.mlp != "fma"
                else "field_fma_kernel", "raster": "raster_warp_kernel" if raster_mode_used == 2 else "raster_kernel"}
     eval_pairs = None
     cpu = None
@@ -526,7 +526,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mlp", default="auto", choices=["auto", "fma", "mma", "hmma"])
+    ap.add_argument("--mlp", default="auto", choices=["auto", "fma", "mma", "hmma", "ws"])
     ap.add_argument("--n-gaussians", type=int, default=0)
     ap.add_argument("--width", type=int, default=0)
     ap.add_argument("--height", type=int, default=0)

@@ -53,8 +53,11 @@ typedef enum { HYRF_F32 = 0, HYRF_F16 = 1, HYRF_U8 = 2 } hyrf_dtype;
  *       128 Gaussians.
  *  HMMA: the same arithmetic on warp-level mma.sync, a warp per 32 Gaussians with no cross-warp hand-over (needs the
  *       two grids to share their geometry, as in every paper configuration; otherwise MMA runs).
+ *  WS:   the MMA arithmetic (tcgen05, fp32 accumulation) as a warp-specialised pipeline: gather warps write the
+ *        features into shared memory as tcgen05 A operands, decoder warpgroups consume them (needs the two grids to
+ *        share their geometry; otherwise MMA runs).
  *  AUTO: MMA when param_dtype is F16 and the layer shapes are supported, else FMA. */
-typedef enum { HYRF_MLP_AUTO = 0, HYRF_MLP_FMA = 1, HYRF_MLP_MMA = 2, HYRF_MLP_HMMA = 3 } hyrf_mlp_path;
+typedef enum { HYRF_MLP_AUTO = 0, HYRF_MLP_FMA = 1, HYRF_MLP_MMA = 2, HYRF_MLP_HMMA = 3, HYRF_MLP_WS = 4 } hyrf_mlp_path;
 
 /* Multi-resolution grid (layout DESIGN.md §2 D3). level_res is a HOST array. */
 typedef struct {

@@ -19,7 +19,7 @@ HYRF_OK, HYRF_ERR_INVALID_ARG, HYRF_ERR_NOT_READY, HYRF_ERR_UNSUPPORTED, HYRF_ER
 STATUS_NAMES = ["HYRF_OK", "HYRF_ERR_INVALID_ARG", "HYRF_ERR_NOT_READY", "HYRF_ERR_UNSUPPORTED", "HYRF_ERR_CAMERA",
                 "HYRF_ERR_OOM", "HYRF_ERR_CUDA"]
 HYRF_F32, HYRF_F16, HYRF_U8 = 0, 1, 2
-HYRF_MLP_AUTO, HYRF_MLP_FMA, HYRF_MLP_MMA, HYRF_MLP_HMMA = 0, 1, 2, 3
+HYRF_MLP_AUTO, HYRF_MLP_FMA, HYRF_MLP_MMA, HYRF_MLP_HMMA, HYRF_MLP_WS = 0, 1, 2, 3, 4
 (DBG_VIS_MASK, DBG_VIS_IDX, DBG_STAGE2_RAW, DBG_STAGE3_ATTRS, DBG_PROJ, DBG_RECT, DBG_TILE_RANGES, DBG_TILE_LIST,
  DBG_FINAL_T, DBG_BG_MASK, DBG_COUNTERS, DBG_FG) = range(12)
 DBG_EXPLICIT = 12   # f32 [8][N]: the explicit parameters as the scene holds them (needs no render, no debug_enable)

@@ -29,6 +29,7 @@ extern "C" const char* hyrf_last_error(void) { return g_err; }
 
 hyrf_status hy_launch_field_fma(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
 hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
+hyrf_status hy_launch_field_ws(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
 bool hy_field_mma_supported(const hyrf_scene_desc& d);
 hyrf_status hy_field_mma_prepare(hyrf_scene* s);
 size_t hy_field_mma_packed_bytes();
@@ -210,10 +211,10 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     if ((st = check_mlp(desc->app_mlp, 2 * desc->app_grid.levels + pe, 3, "app_mlp")) != HYRF_OK) return st;
     if ((st = check_mlp(desc->bg_mlp, 2 * desc->bg_grid.levels + pe, 3, "bg_mlp")) != HYRF_OK) return st;
     if (desc->mlp_path != HYRF_MLP_AUTO && desc->mlp_path != HYRF_MLP_FMA && desc->mlp_path != HYRF_MLP_MMA &&
-        desc->mlp_path != HYRF_MLP_HMMA)
+        desc->mlp_path != HYRF_MLP_HMMA && desc->mlp_path != HYRF_MLP_WS)
         return hy_fail(HYRF_ERR_INVALID_ARG, "unknown mlp_path %d", (int)desc->mlp_path);
-    if ((desc->mlp_path == HYRF_MLP_MMA || desc->mlp_path == HYRF_MLP_HMMA) && !hy_field_mma_supported(*desc))
-        return hy_fail(HYRF_ERR_UNSUPPORTED, "mlp_path MMA / HMMA needs fp16 parameters, 16-level grids, 32->64->64->8 and 56->64->64->3 decoders");
+    if ((desc->mlp_path == HYRF_MLP_MMA || desc->mlp_path == HYRF_MLP_HMMA || desc->mlp_path == HYRF_MLP_WS) && !hy_field_mma_supported(*desc))
+        return hy_fail(HYRF_ERR_UNSUPPORTED, "mlp_path MMA / HMMA / WS needs fp16 parameters, 16-level grids, 32->64->64->8 and 56->64->64->3 decoders");
 
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
@@ -273,6 +274,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
         bool same = g.levels == a.levels && g.log2_table == a.log2_table;
         for (uint32_t l = 0; same && l < g.levels; ++l) same = g.level_res[l] == a.level_res[l];
         if (s->use_mma && same) HY_TRY(dev_alloc(s, &s->both_table, s->geo_entries * 4 * tsz));
+        s->ws_mma = s->use_mma && same && desc->mlp_path == HYRF_MLP_WS;   // (needs the interleaved table)
     }
     HY_TRY(dev_alloc_t(s, &s->gm, 2 * N));
     HY_TRY(dev_alloc_t(s, &s->gm_id, N));
@@ -547,7 +549,8 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     // S2 + S3 + S4a: field query, aggregation, projection
     // (explicit-only ablation: no field is queried, so the CUDA-core kernel's early-out path serves both dtypes)
     const bool mma = s->use_mma && !(s->ablation & HYRF_ABL_NO_NEURAL);
-    if ((st = mma ? hy_launch_field_mma(s, f, &launches) : hy_launch_field_fma(s, f, &launches)) != HYRF_OK) return st;
+    if ((st = !mma ? hy_launch_field_fma(s, f, &launches)
+                   : (s->ws_mma ? hy_launch_field_ws(s, f, &launches) : hy_launch_field_mma(s, f, &launches))) != HYRF_OK) return st;
     if (timing) cudaEventRecord(s->ev[2], s->stream);
 
     // counters (V, D) start their way to the host now; the depth ordering below does not need them, so the copy

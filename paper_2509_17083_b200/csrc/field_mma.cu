@@ -12,6 +12,7 @@
 // The two decoders run as independent chains with their own mbarrier. Accumulation order inside an MMA is
 // unspecified, so this path is compared with the oracle by tolerance, not bit for bit.
 #include "field_common.cuh"
+#include "field_tc_common.cuh"
 #include "tcgen05.cuh"
 
 
@@ -21,16 +22,6 @@ constexpr int kThreads = 256;
 constexpr int kTile = 128;
 constexpr int kTmemCols = 256;
 constexpr uint32_t kColDg = 0, kColDa = 64, kColAg = 128, kColAa = 160;
-// packed weight block (bytes): geo W1 [64 x 32], W2 [64 x 64], W3 [16 x 64]; app W1 [64 x 64], W2, W3
-constexpr uint32_t kOffG1 = 0, kOffG2 = 4096, kOffG3 = 12288, kOffA1 = 14336, kOffA2 = 22528, kOffA3 = 30720;
-constexpr uint32_t kPackedBytes = 32768;
-constexpr uint32_t kSmemBytes = kPackedBytes;   // two CTAs (2 x 256 TMEM columns) per SM by registers; the rest of the 228 KB is L1
-
-// element (n, k) of an [N x Kp] K-major operand stored as 8x8 core matrices: half-index inside the operand
-__host__ __device__ inline uint32_t core_index(uint32_t n, uint32_t k, uint32_t Kp) {
-    return (n >> 3) * (Kp * 8) + (k >> 3) * 64 + (n & 7) * 8 + (k & 7);
-}
-
 // raw row-major [out][in] fp16 weights -> packed operand block
 __global__ void pack_weights_kernel(const __half* __restrict__ geo, const __half* __restrict__ app,
                                     __half* __restrict__ packed) {
@@ -50,11 +41,6 @@ __global__ void pack_weights_kernel(const __half* __restrict__ geo, const __half
         const uint32_t kc = rem / 64, n = grp * 8 + (rem % 64) / 8, k = kc * 8 + (rem % 8);
         if (n < op.n_real && k < op.k_real) packed[i] = (op.app ? app : geo)[op.src + n * op.k_real + k];
     }
-}
-
-__device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
-    __half2 h = __floats2half2_rn(lo, hi);
-    return *reinterpret_cast<uint32_t*>(&h);
 }
 
 // D3 for one level with two lanes per Gaussian: this lane blends the four corners whose x bit is xb; the partner
@@ -113,69 +99,6 @@ __device__ __forceinline__ uint32_t gather_level_pair(const GridDev& g, uint32_t
     return pack_h2(a0, a1);
 }
 
-// The same level for BOTH fields at once, when the two grids share their geometry (levels, resolutions, table size —
-// true of every paper configuration): the tables are interleaved at upload into one array of 8-byte entries
-// (geo f0, geo f1, app f0, app f1), so one index computation and one load serve both fields and the x / x+1
-// corners of both fields sit in one 16-byte span. Halves the sector look-ups and the index arithmetic.
-template <bool U8>
-__device__ __forceinline__ void gather_level_half2(const GridDev& g, const GridDev& ga, const void* __restrict__ both,
-                                                   uint32_t l, const float x[3], uint32_t xb,
-                                                   float& g0, float& g1, float& a0, float& a1) {
-    const uint32_t N = g.res[l];
-    const float Nf = (float)N;
-    uint32_t ci[3];
-    float w[3];
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        const float u = __fmul_rn(x[a], Nf);
-        int i = (int)floorf(u);
-        i = min(i, (int)N - 1);
-        ci[a] = (uint32_t)i;
-        w[a] = __fsub_rn(u, (float)i);
-    }
-    const uint32_t vx = ci[0] + xb;
-    uint32_t idx[4];
-    if ((g.dense_mask >> l) & 1u) {
-        const uint32_t n1 = N + 1u;
-        const uint32_t b = vx + n1 * (ci[1] + n1 * ci[2]);
-        idx[0] = b; idx[1] = b + n1; idx[2] = b + n1 * n1; idx[3] = b + n1 * n1 + n1;
-    } else {
-        const uint32_t hy0 = ci[1] * 2654435761u, hy1 = hy0 + 2654435761u;
-        const uint32_t hz0 = ci[2] * 805459861u, hz1 = hz0 + 805459861u;
-        idx[0] = (vx ^ hy0 ^ hz0) & g.table_mask; idx[1] = (vx ^ hy1 ^ hz0) & g.table_mask;
-        idx[2] = (vx ^ hy0 ^ hz1) & g.table_mask; idx[3] = (vx ^ hy1 ^ hz1) & g.table_mask;
-    }
-    float2 vgs[4], vas[4];
-    if (U8) {   // 4-byte entries (geo c0 c1 | app c0 c1), D3': value = fma(code, step, min)
-        const uchar4* tab = reinterpret_cast<const uchar4*>(both) + g.offset[l];
-        const float2 qg0 = g.q[l][0], qg1 = g.q[l][1], qa0 = ga.q[l][0], qa1 = ga.q[l][1];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const uchar4 c = __ldg(tab + idx[k]);
-            vgs[k] = make_float2(__fmaf_rn((float)c.x, qg0.y, qg0.x), __fmaf_rn((float)c.y, qg1.y, qg1.x));
-            vas[k] = make_float2(__fmaf_rn((float)c.z, qa0.y, qa0.x), __fmaf_rn((float)c.w, qa1.y, qa1.x));
-        }
-    } else {
-        const uint2* tab = reinterpret_cast<const uint2*>(both) + g.offset[l];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const uint2 v = __ldg(tab + idx[k]);
-            vgs[k] = __half22float2(*reinterpret_cast<const __half2*>(&v.x));
-            vas[k] = __half22float2(*reinterpret_cast<const __half2*>(&v.y));
-        }
-    }
-    const float ax = xb ? w[0] : __fsub_rn(1.0f, w[0]);
-    const float wy0 = __fsub_rn(1.0f, w[1]), wz0 = __fsub_rn(1.0f, w[2]);
-    g0 = 0.0f; g1 = 0.0f; a0 = 0.0f; a1 = 0.0f;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        const float wt = __fmul_rn(__fmul_rn(ax, (k & 1) ? w[1] : wy0), (k & 2) ? w[2] : wz0);
-        const float2 vg = vgs[k], va = vas[k];
-        g0 = __fmaf_rn(wt, vg.x, g0); g1 = __fmaf_rn(wt, vg.y, g1);
-        a0 = __fmaf_rn(wt, va.x, a0); a1 = __fmaf_rn(wt, va.y, a1);
-    }
-}
-
 // both lanes of a pair end up with both fields' rounded feature pairs
 template <bool U8>
 __device__ __forceinline__ void gather_level_pair2(const GridDev& g, const GridDev& ga, const void* __restrict__ both,
@@ -202,13 +125,6 @@ __global__ void interleave_tables_u8_kernel(const uint16_t* __restrict__ geo, co
                                             uint32_t* __restrict__ both) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) both[i] = (uint32_t)geo[i] | ((uint32_t)app[i] << 16);
-}
-
-// ReLU + round to fp16 of 32 fp32 accumulator columns -> 16 packed A columns
-__device__ __forceinline__ void relu_pack32(const uint32_t* d, uint32_t* a) {
-#pragma unroll
-    for (int i = 0; i < 16; ++i)
-        a[i] = pack_h2(fmaxf(__uint_as_float(d[2 * i]), 0.0f), fmaxf(__uint_as_float(d[2 * i + 1]), 0.0f));
 }
 
 template <bool U8>
@@ -305,26 +221,7 @@ field_mma_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const vo
         }
         if (valid) {
             if (chain) {
-                const float dx = __fsub_rn(px, A.f.o[0]), dy = __fsub_rn(py, A.f.o[1]), dz = __fsub_rn(pz, A.f.o[2]);
-                const float n = __fsqrt_rn(__fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx))));
-                const float d[3] = {__fdiv_rn(dx, n), __fdiv_rn(dy, n), __fdiv_rn(dz, n)};
-                // D4 by octave doubling: one sincospi per axis, then sin 2t = 2 sin t cos t, cos 2t = 1 - 2 sin^2 t.
-                // Three doublings amplify the 1-ulp start error to ~1e-6, far below the fp16 rounding that follows.
-                float pe[24];
-#pragma unroll
-                for (int ax = 0; ax < 3; ++ax) {
-                    float sn, cs;
-                    sincospif(d[ax], &sn, &cs);
-                    pe[ax] = sn; pe[3 + ax] = cs;
-#pragma unroll
-                    for (int k = 1; k < 4; ++k) {
-                        const float s2 = 2.0f * sn * cs, c2 = 1.0f - 2.0f * sn * sn;
-                        sn = s2; cs = c2;
-                        pe[6 * k + ax] = sn; pe[6 * k + 3 + ax] = cs;
-                    }
-                }
-#pragma unroll
-                for (int i = 0; i < 12; ++i) a[16 + i] = pack_h2(pe[2 * i], pe[2 * i + 1]);
+                dir_pe_packed(A.f, px, py, pz, a + 16);   // D4
             }
         }
         if (!valid) {
@@ -522,24 +419,7 @@ field_mma_pipe_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, con
 #pragma unroll
                     for (int l = 0; l < 16; ++l) a[l] = 0u;
                     if (valid) {
-                        const float dx = __fsub_rn(ex.px, A.f.o[0]), dy = __fsub_rn(ex.py, A.f.o[1]), dz = __fsub_rn(ex.pz, A.f.o[2]);
-                        const float n = __fsqrt_rn(__fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx))));
-                        const float d[3] = {__fdiv_rn(dx, n), __fdiv_rn(dy, n), __fdiv_rn(dz, n)};
-                        float pe[24];   // D4 by octave doubling (see field_mma_kernel)
-#pragma unroll
-                        for (int ax = 0; ax < 3; ++ax) {
-                            float sn, cs;
-                            sincospif(d[ax], &sn, &cs);
-                            pe[ax] = sn; pe[3 + ax] = cs;
-#pragma unroll
-                            for (int k = 1; k < 4; ++k) {
-                                const float s2 = 2.0f * sn * cs, c2 = 1.0f - 2.0f * sn * sn;
-                                sn = s2; cs = c2;
-                                pe[6 * k + ax] = sn; pe[6 * k + 3 + ax] = cs;
-                            }
-                        }
-#pragma unroll
-                        for (int i = 0; i < 12; ++i) a[i] = pack_h2(pe[2 * i], pe[2 * i + 1]);
+                        dir_pe_packed(A.f, ex.px, ex.py, ex.pz, a);   // D4
                     }
                     tc::st_x16(tA + lane_base + 16, a);
                 }
@@ -755,24 +635,7 @@ field_warp_kernel(const FieldArgs A, const uint4* __restrict__ packed_w, const v
 #pragma unroll
             for (int i = 0; i < 12; ++i) pe2[i] = 0u;
             if (valid) {
-                const float dx = __fsub_rn(ex.px, A.f.o[0]), dy = __fsub_rn(ex.py, A.f.o[1]), dz = __fsub_rn(ex.pz, A.f.o[2]);
-                const float n = __fsqrt_rn(__fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx))));
-                const float d[3] = {__fdiv_rn(dx, n), __fdiv_rn(dy, n), __fdiv_rn(dz, n)};
-                float pe[24];   // D4 by octave doubling (see field_mma_kernel)
-#pragma unroll
-                for (int ax = 0; ax < 3; ++ax) {
-                    float sn, cs;
-                    sincospif(d[ax], &sn, &cs);
-                    pe[ax] = sn; pe[3 + ax] = cs;
-#pragma unroll
-                    for (int k = 1; k < 4; ++k) {
-                        const float s2 = 2.0f * sn * cs, c2 = 1.0f - 2.0f * sn * sn;
-                        sn = s2; cs = c2;
-                        pe[6 * k + ax] = sn; pe[6 * k + 3 + ax] = cs;
-                    }
-                }
-#pragma unroll
-                for (int i = 0; i < 12; ++i) pe2[i] = pack_h2(pe[2 * i], pe[2 * i + 1]);
+                dir_pe_packed(A.f, ex.px, ex.py, ex.pz, pe2);   // D4
             }
             uint4* d4 = reinterpret_cast<uint4*>(fA + lane * kRowA + 16);   // 112-byte rows: 16-byte aligned
             d4[0] = make_uint4(pe2[0], pe2[1], pe2[2], pe2[3]);

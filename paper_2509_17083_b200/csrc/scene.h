@@ -42,6 +42,9 @@ struct hyrf_scene {
     uint32_t N = 0;
     int sm_count = 0;          // cudaDevAttrMultiProcessorCount of desc.device (148 on a full B200)
     bool field_attr_set = false;   // cudaFuncSetAttribute of the tensor-core field kernels done for this scene's device
+    bool field_ws_attr_set = false;
+    bool ws_mma = false;       // decoders on tcgen05 with warp-specialised gather / decoder roles (field_ws.cu)
+    int ws_sort_sms = 12;      // SMs the warp-specialised field kernel leaves to the depth sort running beside it
 
     // persistent parameters
     float* pos = nullptr;      // [3][N]

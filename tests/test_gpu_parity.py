@@ -173,7 +173,7 @@ def test_render_is_deterministic_and_scratch_grows(B, synth):
     hs.close()
 
 
-@pytest.mark.parametrize("path", ["MMA", "HMMA"])
+@pytest.mark.parametrize("path", ["MMA", "HMMA", "WS"])
 def test_config3_scaled_fp16_tensor_core_path(B, ho, synth, path):
     # both tensor-core kernels (tcgen05 CTA tiles; mma.sync warp tiles): mask bit-exact, raw logits within 2e-3,
     # list symmetric difference reported and bounded, image within 1e-2 (SURVEY §8c H1 protocol)
@@ -183,7 +183,7 @@ def test_config3_scaled_fp16_tensor_core_path(B, ho, synth, path):
     print("tensor-core path stats:", st[0])
 
 
-@pytest.mark.parametrize("path", ["MMA", "HMMA"])
+@pytest.mark.parametrize("path", ["MMA", "HMMA", "WS"])
 def test_tensor_core_path_high_gain(B, ho, synth, path):
     # large table entries: decoder outputs O(1), so operand layout / K-order mistakes cannot hide in the tolerance
     s = synth.make_scene(3, n_gaussians=20_000, width=160, height=96, n_cameras=1, table_amp=1.0)
@@ -210,6 +210,7 @@ def test_config3_full_one_camera_both_paths(B, ho, synth):
     st = _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False, label="config3_full_AUTO")
     print("config 3 full, tcgen05 path:", {k: v for k, v in st[0].items() if not isinstance(v, list)})
     _run(B, ho, s, mlp_path=B.HYRF_MLP_HMMA, exact=False, label="config3_full_HMMA")
+    _run(B, ho, s, mlp_path=B.HYRF_MLP_WS, exact=False, label="config3_full_WS")
 
 
 def test_config4_full_one_camera_both_paths(B, ho, synth):
@@ -256,6 +257,8 @@ def test_ablation_switches_tensor_path(B, ho, synth):
         _run(B, ho, s, mlp_path=B.HYRF_MLP_MMA, exact=(abl & 4) != 0, ablation=abl)
     for abl in (1, 8):
         _run(B, ho, s, mlp_path=B.HYRF_MLP_HMMA, exact=False, ablation=abl)
+    for abl in (1, 8, 1 | 2 | 8):
+        _run(B, ho, s, mlp_path=B.HYRF_MLP_WS, exact=False, ablation=abl)
 
 
 def test_sort_overlap_is_schedule_only(B, synth):
@@ -264,7 +267,7 @@ def test_sort_overlap_is_schedule_only(B, synth):
     # stream's buffers are reused across frames
     import torch
     s = synth.make_scene(3, n_gaussians=80_000, width=320, height=180, n_cameras=4)
-    for path in (B.HYRF_MLP_MMA, B.HYRF_MLP_HMMA, B.HYRF_MLP_FMA):
+    for path in (B.HYRF_MLP_MMA, B.HYRF_MLP_HMMA, B.HYRF_MLP_WS, B.HYRF_MLP_FMA):
         hs = B.HyrfScene(s, mlp_path=path)
         hs.debug_enable()
         ref = []
@@ -340,7 +343,7 @@ def test_quantised_tables_tensor_path(B, ho, synth):
     s = synth.quantize8(synth.make_scene(3, n_gaussians=40_000, width=320, height=180, n_cameras=2))
     _run(B, ho, s, mlp_path=B.HYRF_MLP_AUTO, exact=False)
     s = synth.quantize8(synth.make_scene(3, n_gaussians=20_000, width=160, height=96, n_cameras=1, table_amp=1.0))
-    for path in (B.HYRF_MLP_MMA, B.HYRF_MLP_HMMA):
+    for path in (B.HYRF_MLP_MMA, B.HYRF_MLP_HMMA, B.HYRF_MLP_WS):
         hs = B.HyrfScene(s, mlp_path=path)
         hs.debug_enable()
         hs.render(s.cameras[0])
@@ -671,7 +674,7 @@ def test_single_shared_field(B, ho, synth):
     s = synth.make_scene(3, n_gaussians=30_000, width=320, height=180, n_cameras=2, table_amp=1.0)
     s.app_table = s.geo_table
     _run(B, ho, s, mlp_path=B.HYRF_MLP_FMA, exact=True, label="shared_field_FMA")
-    for path in ("MMA", "HMMA"):
+    for path in ("MMA", "HMMA", "WS"):
         st = _run(B, ho, s, mlp_path=getattr(B, "HYRF_MLP_" + path), exact=False, label="shared_field_" + path)
         assert st[0]["raw_geo_maxdiff"] > 0.0
     t = synth.tiny_scene(n=64, W=48, H=40, seed=13)           # run-time-shaped kernels, fp32
