@@ -56,7 +56,7 @@ typedef enum { HYRF_F32 = 0, HYRF_F16 = 1, HYRF_U8 = 2 } hyrf_dtype;
  *  WS:   the MMA arithmetic (tcgen05, fp32 accumulation) as a warp-specialised pipeline: gather warps write the
  *        features into shared memory as tcgen05 A operands, decoder warpgroups consume them (needs the two grids to
  *        share their geometry; otherwise MMA runs).
- *  AUTO: MMA when param_dtype is F16 and the layer shapes are supported, else FMA. */
+ *  AUTO: WS (else MMA) when param_dtype is F16 / U8 and the layer shapes are supported, else FMA. */
 typedef enum { HYRF_MLP_AUTO = 0, HYRF_MLP_FMA = 1, HYRF_MLP_MMA = 2, HYRF_MLP_HMMA = 3, HYRF_MLP_WS = 4 } hyrf_mlp_path;
 
 /* Multi-resolution grid (layout DESIGN.md §2 D3). level_res is a HOST array. */
@@ -232,13 +232,15 @@ hyrf_status hyrf_set_ablation(hyrf_scene* scene, uint32_t mask);
  * every debug export are identical either way. */
 hyrf_status hyrf_set_sort_overlap(hyrf_scene* scene, int on);
 
-/* Rasterizer variant (S5; Eq. 1). Both variants stage a tile's depth-ordered list once per tile and
- * produce the same bits; they differ in cost. mode 1: every warp of the tile blends every staged entry. mode 2: a warp
+/* Rasterizer variant (S5; Eq. 1). Every variant stages a tile's depth-ordered list once per tile and
+ * produces the same bits; they differ in cost. mode 1: every warp of the tile blends every staged entry. mode 2: a warp
  * owns an 8 x 4 pixel block and blends only the entries that can reach alpha >= 1/255 somewhere in its block (per-warp
- * lists built while staging) — faster when splats cover few tiles. mode 0 (default): chosen per frame from the tiles
- * touched per visible Gaussian of the previous frame. HYRF_ERR_INVALID_ARG for any other mode. */
+ * lists built while staging) — faster when splats cover few tiles. mode 3: per-warp lists over 8 x 8 blocks with two
+ * pixels per lane on the two-wide fp32 instructions of sm_100 (fma.rn.f32x2: half the issue slots per pair). mode 0
+ * (default): 3 or 1, chosen per frame from the tiles touched per visible Gaussian of the previous frame.
+ * HYRF_ERR_INVALID_ARG for any other mode. */
 hyrf_status hyrf_set_raster_mode(hyrf_scene* scene, int mode);
-/* The variant (1 or 2) the last render used. */
+/* The variant (1, 2 or 3) the last render used. */
 hyrf_status hyrf_last_raster_mode(hyrf_scene* scene, int* mode);
 
 /* Backward of stage 5 for the LAST rendered frame (first piece of the training pass of PAPER.md:136-142, which

@@ -361,7 +361,7 @@ class HyrfScene:
 
     def set_sort_overlap(self, on: bool = True) -> None:
         """Depth sort beside the field query on a second stream (default) or the whole frame serialised (include/hyrf.h)."""
-        _check(self.lib.hyrf_set_sort_overlap(self.handle, int(on)))
+        _check(self.lib.hyrf_set_sort_overlap(self.handle, int(on)))   # (an int > 1: SMs left to the sort, include/hyrf.h)
 
     def set_raster_mode(self, mode: int = 0) -> None:
         """0 auto, 1 tile-level lists only, 2 per-warp lists (include/hyrf.h hyrf_set_raster_mode); same bits, different cost."""

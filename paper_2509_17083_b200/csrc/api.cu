@@ -274,7 +274,8 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
         bool same = g.levels == a.levels && g.log2_table == a.log2_table;
         for (uint32_t l = 0; same && l < g.levels; ++l) same = g.level_res[l] == a.level_res[l];
         if (s->use_mma && same) HY_TRY(dev_alloc(s, &s->both_table, s->geo_entries * 4 * tsz));
-        s->ws_mma = s->use_mma && same && desc->mlp_path == HYRF_MLP_WS;   // (needs the interleaved table)
+        // warp-specialised tcgen05 kernel: what AUTO runs when the two grids share their geometry (needs the interleaved table)
+        s->ws_mma = s->use_mma && same && (desc->mlp_path == HYRF_MLP_WS || desc->mlp_path == HYRF_MLP_AUTO);
     }
     HY_TRY(dev_alloc_t(s, &s->gm, 2 * N));
     HY_TRY(dev_alloc_t(s, &s->gm_id, N));
@@ -441,7 +442,7 @@ extern "C" hyrf_status hyrf_upload_explicit_rvq(hyrf_scene* s, const hyrf_explic
 
 extern "C" hyrf_status hyrf_set_raster_mode(hyrf_scene* s, int mode) {
     if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_raster_mode: NULL scene");
-    if (mode < 0 || mode > 2) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_raster_mode: mode %d outside [0, 2]", mode);
+    if (mode < 0 || mode > 3) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_raster_mode: mode %d outside [0, 3]", mode);
     s->raster_mode = mode;
     return HYRF_OK;
 }
@@ -743,6 +744,7 @@ extern "C" hyrf_status hyrf_set_ablation(hyrf_scene* s, uint32_t mask) {
 extern "C" hyrf_status hyrf_set_sort_overlap(hyrf_scene* s, int on) {
     if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_sort_overlap: NULL scene");
     s->sort_overlap = on != 0;
+    if (on > 1) s->ws_sort_sms = on < s->sm_count ? on : s->sm_count - 1;   // on > 1: SMs the warp-specialised field kernel leaves to the sort
     return HYRF_OK;
 }
 

@@ -124,12 +124,17 @@ __device__ __forceinline__ void level_issue(const GridDev& g, const void* __rest
         idx[0] = (vx ^ hy0 ^ hz0) & g.table_mask; idx[1] = (vx ^ hy1 ^ hz0) & g.table_mask;
         idx[2] = (vx ^ hy0 ^ hz1) & g.table_mask; idx[3] = (vx ^ hy1 ^ hz1) & g.table_mask;
     }
+    // The level's base pointer is pinned in a register pair (the empty asm keeps the compiler from folding the level
+    // offset into each index), so every address is ONE wide multiply-add (IMAD.WIDE.U32 idx, 8, base) instead of a
+    // three- or four-instruction 64-bit add chain: the gather warps are issue-bound once their loads are pipelined.
     if (U8) {
         const uint32_t* tab = reinterpret_cast<const uint32_t*>(both) + g.offset[l];
+        asm volatile("" : "+l"(tab));
 #pragma unroll
         for (int k = 0; k < 4; ++k) b.v[k] = make_uint2(__ldg(tab + idx[k]), 0u);
     } else {
         const uint2* tab = reinterpret_cast<const uint2*>(both) + g.offset[l];
+        asm volatile("" : "+l"(tab));
 #pragma unroll
         for (int k = 0; k < 4; ++k) b.v[k] = __ldg(tab + idx[k]);
     }

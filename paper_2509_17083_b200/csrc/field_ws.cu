@@ -27,10 +27,16 @@
 namespace {
 
 constexpr int kTile = 128;
-constexpr int kGatherWarps = 12;                        // a multiple of 4: decoder warp w then owns TMEM lanes 32 (w % 4) ..
+#ifndef HY_WS_GATHER_WARPS
+#define HY_WS_GATHER_WARPS 12
+#endif
+#ifndef HY_WS_NF
+#define HY_WS_NF 2
+#endif
+constexpr int kGatherWarps = HY_WS_GATHER_WARPS;        // a multiple of 4: decoder warp w then owns TMEM lanes 32 (w % 4) ..
 constexpr int kDecWGs = 2;
 constexpr int kWsThreads = (kGatherWarps + 4 * kDecWGs) * 32;   // 640
-constexpr int kNF = 3;                                  // feature buffers in flight
+constexpr int kNF = HY_WS_NF;                           // feature buffers in flight
 constexpr int kNP = 4;                                  // position / explicit-record buffers in flight
 constexpr uint32_t kWsTmemCols = 512;
 constexpr uint32_t kWgCols = 256;                       // per decoder warpgroup: D_geo 0, D_app 64, A_geo 128, A_app 160

@@ -77,6 +77,19 @@ issue_probe_kernel(uint32_t iters, float seed, float* __restrict__ sink) {
             for (int r = 0; r < 2; ++r)
 #pragma unroll
                 for (int i = 0; i < 8; ++i) { a[i] = __fmaf_rn(a[i], m, c); q[i] = (q[i] ^ (q[i] >> 3)) + 0x9E37u; }   // 16 FFMA + 32 ALU
+        } else if (KIND == 3) {   // packed fp32: FFMA2 = two independent fma.rn per lane in one issue slot (sm_100)
+            unsigned long long mm, cc;
+            asm("mov.b64 %0, {%1, %1};" : "=l"(mm) : "f"(m));
+            asm("mov.b64 %0, {%1, %1};" : "=l"(cc) : "f"(c));
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int i = 0; i < 8; i += 2) {
+                    unsigned long long v;
+                    asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(a[i]), "f"(a[i + 1]));
+                    asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(v) : "l"(mm), "l"(cc));
+                    asm("mov.b64 {%0, %1}, %2;" : "=f"(a[i]), "=f"(a[i + 1]) : "l"(v));
+                }                                                                          // 32 FFMA2 = 64 fma
         } else {
 #pragma unroll
             for (int i = 0; i < 2; ++i) {   // two "pairs" per iteration
@@ -151,13 +164,13 @@ extern "C" hyrf_status hyrf_probe_gather(int32_t device, uint64_t table_bytes, u
 extern "C" hyrf_status hyrf_probe_issue(int32_t device, uint32_t kind, uint32_t ctas_per_sm, uint32_t iters,
                                         double* warp_instr_per_s, float* ms_out) {
     if (!warp_instr_per_s || !ms_out) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_probe_issue: NULL output");
-    if (kind > 2 || ctas_per_sm < 1 || ctas_per_sm > 8 || iters < 1) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_probe_issue: kind 0..2, ctas_per_sm 1..8");
+    if (kind > 3 || ctas_per_sm < 1 || ctas_per_sm > 8 || iters < 1) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_probe_issue: kind 0..3, ctas_per_sm 1..8");
     cudaError_t e;
     if ((e = cudaSetDevice(device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
     int sms = 0;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) return hy_cuda_fail(e, "cudaDeviceGetAttribute");
     const uint32_t grid = (uint32_t)sms * ctas_per_sm;
-    iters = (iters + 3u) & ~3u;
+    iters = (iters + 15u) & ~15u;
     float* sink = nullptr;
     if ((e = cudaMalloc(&sink, (size_t)grid * kProbeThreads * 4)) != cudaSuccess) return hy_cuda_fail(e, "cudaMalloc(probe sink)");
     cudaEvent_t e0, e1;
@@ -165,7 +178,8 @@ extern "C" hyrf_status hyrf_probe_issue(int32_t device, uint32_t kind, uint32_t 
     float best = 1e30f;
     for (int rep = 0; rep < 4; ++rep) {
         cudaEventRecord(e0);
-        if (kind == 0) issue_probe_kernel<0><<<grid, kProbeThreads>>>(iters, 0.5f, sink);
+        if (kind == 3) issue_probe_kernel<3><<<grid, kProbeThreads>>>(iters, 0.5f, sink);
+        else if (kind == 0) issue_probe_kernel<0><<<grid, kProbeThreads>>>(iters, 0.5f, sink);
         else if (kind == 1) issue_probe_kernel<1><<<grid, kProbeThreads>>>(iters, 0.5f, sink);
         else issue_probe_kernel<2><<<grid, kProbeThreads>>>(iters, 0.5f, sink);
         cudaEventRecord(e1);
@@ -181,7 +195,7 @@ extern "C" hyrf_status hyrf_probe_issue(int32_t device, uint32_t kind, uint32_t 
     // -O3 -fmad=false): kind 0 is unrolled x 4 into 128 FFMA + 4 of loop control; kind 1 x 2 into 32 FFMA + 96 integer
     // ALU + 4; kind 2 x 2 into 107 (20 FFMA, 40 FMUL, 16 FADD, 4 FMNMX, 12 FSETP, 8 FSEL, 4 MUFU.EX2, 3 of loop control):
     // one MUFU per 26.75 issued instructions. iters is rounded up to a multiple of 4 by the caller below.
-    const double body = kind == 0 ? 33.0 : (kind == 1 ? 66.0 : 53.5);
+    const double body = kind == 0 ? 33.0 : (kind == 1 ? 66.0 : (kind == 3 ? 32.25 : 53.5));   // kind 3: x 16 into 512 FFMA2 + 4
     *warp_instr_per_s = (double)grid * (kProbeThreads / 32) * body * iters / (best * 1e-3);
     *ms_out = best;
     return HYRF_OK;

@@ -177,11 +177,13 @@ void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, con
     // Gaussian in the previous frame (config 3: 10, config 4: 15 -> per-warp lists; the 1080p and 4K points of config 5:
     // 35 - 120 -> this kernel; config 3 rendered at 1080p, 19 tiles per Gaussian, is the tie). hyrf_set_raster_mode overrides it.
     constexpr uint64_t kWarpListMaxTilesPerSplat = 19;   // measured crossover on config 3 at 900p / 1080p / 1260p
-    bool warp_lists = s->raster_mode == 2;
+    bool warp_lists = s->raster_mode == 2 || s->raster_mode == 3;
     if (s->raster_mode == 0) warp_lists = s->lastV == 0 || s->lastD <= kWarpListMaxTilesPerSplat * s->lastV;
-    s->last_raster_mode = warp_lists ? 2 : 1;
+    // per-warp lists: the packed-fp32 kernel (two pixels per lane, raster_pair.cu) unless mode 2 pins the one-pixel one
+    s->last_raster_mode = warp_lists ? (s->raster_mode == 2 ? 2 : 3) : 1;
     if (warp_lists) {
-        hy_launch_raster_warp(s, f, ranges, list, macro, out_rgb, launches, tile_queue, dbg_list);
+        if (s->raster_mode == 2) hy_launch_raster_warp(s, f, ranges, list, macro, out_rgb, launches, tile_queue, dbg_list);
+        else hy_launch_raster_pair(s, f, ranges, list, macro, out_rgb, launches, tile_queue, dbg_list);
         return;
     }
     const unsigned grid = (unsigned)(f.gx * f.gy);

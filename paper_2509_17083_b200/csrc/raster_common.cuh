@@ -77,3 +77,21 @@ __device__ __forceinline__ uint32_t entry_block_mask(float u, float v, float A, 
     }
     return m;
 }
+
+// The same for the four 8 x 8 pixel blocks of the tile (block w: columns (w & 1) * 8 .., rows (w >> 1) * 8 ..): what the
+// two-pixels-per-lane rasterizer (raster_pair.cu) needs, at half the tests.
+__device__ __forceinline__ uint32_t entry_block_mask4(float u, float v, float A, float B, float C, float o, float X0,
+                                                      float Y0, int W, int H) {
+    const float iA = __fdividef(1.0f, A), iC = __fdividef(1.0f, C);
+    const float qthr = 2.0f * __logf(o * (255.0f / 0.99f)) +
+                       hy_q_slack(u, v, A, B, C, X0, fminf(X0 + 15.0f, (float)(W - 1)), Y0, fminf(Y0 + 15.0f, (float)(H - 1)));
+    uint32_t m = 0;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const float bx0 = X0 + (float)((w & 1) * 8), by0 = Y0 + (float)((w >> 1) * 8);
+        const float bx1 = fminf(bx0 + 7.0f, (float)(W - 1)), by1 = fminf(by0 + 7.0f, (float)(H - 1));
+        const bool in_img = bx0 <= (float)(W - 1) && by0 <= (float)(H - 1);
+        if (in_img && entry_reaches_block(u, v, A, B, C, iA, iC, qthr, bx0, bx1, by0, by1)) m |= 1u << w;
+    }
+    return m;
+}
