@@ -398,6 +398,19 @@ def run_ours(args):
     e1.record(stream)
     torch.cuda.synchronize()
     warm_ms = e0.elapsed_time(e1) / K
+    # the same stream of frames pipelined (hyrf_set_pipelining: frame k+1's cull and depth sort beside frame k's
+    # rasterizer, field kernel on every SM); context for e2e, which adds the device->host copies
+    hs.set_pipelining(True)
+    for i in range(3):
+        step(i)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for i in range(K):
+        step(i)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    pipe_ms = e0.elapsed_time(e1) / K
+    hs.set_pipelining(False)
 
     # --- the same frames with the depth sort serialised (hyrf_set_sort_overlap(0)): every kernel alone on the GPU, the
     # stage times per-kernel profiling sees; reported beside the timed (overlapped) ones, never instead of them -------
@@ -441,6 +454,15 @@ def run_ours(args):
     hs.host_sync()
     e2e_s = max_over_ranks(time.perf_counter() - t0)
     e2e = frames_total / e2e_s
+    # what the copies alone cost on this box: the same K images device -> pinned host, nothing else
+    dimg = torch.empty((H, W, 3), dtype=torch.float32, device=f"cuda:{dev}")
+    host_imgs[0].copy_(dimg, non_blocking=True)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for i in range(K):
+        host_imgs[i & 1].copy_(dimg, non_blocking=True)
+    torch.cuda.synchronize()
+    d2h_gbs = K * W * H * 12 / (time.perf_counter() - t0) / 1e9
 
     raster_mode_used = hs.last_raster_mode()
     backward = None
@@ -506,9 +528,10 @@ def run_ours(args):
             "visible_gaussians_per_s": vis_per_s, "V_mean": Vm, "D_mean": Dm, "Dm_mean": Dmm,
             "stage_ms": {n: float(stage_ms[i]) for i, n in enumerate(names)} | {"frame": float(stage_ms[5])},
             "serial_stage_ms": {n: float(stage_serial_ms[i]) for i, n in enumerate(names)} | {"frame": float(stage_serial_ms[5])},
-            "warm_l2_ms_per_step": warm_ms,
+            "warm_l2_ms_per_step": warm_ms, "pipelined_warm_l2_ms_per_step": pipe_ms,
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 64, "d2h_bytes_per_step": W * H * 12,
-                    "api": "hyrf_render_host_async + hyrf_host_sync", "sync_api_value": e2e_sync},
+                    "api": "hyrf_render_host_async + hyrf_host_sync", "sync_api_value": e2e_sync,
+                    "d2h_copy_only_gbs": d2h_gbs, "d2h_copy_only_frames_per_s": d2h_gbs * 1e9 / (W * H * 12)},
             "gpu_launches": launches, "clocks": clocks, "roofline": roof, "stage_rooflines": per_stage}
     if cpu:
         line["cpu_baseline"] = cpu

@@ -211,6 +211,10 @@ hyrf_status hyrf_debug_fetch(hyrf_scene* scene, uint32_t kind, void* host_dst, s
  * Timing is recorded only after hyrf_debug_enable or hyrf_set_timing(scene, 1). Synchronises the stream. */
 hyrf_status hyrf_set_timing(hyrf_scene* scene, int32_t enabled);
 hyrf_status hyrf_stage_times(hyrf_scene* scene, float ms[6]);
+/* Time (ms) the caller's stream spent between the end of the previous timed frame's last kernel and the start of the
+ * last frame's first stage: what a stream of frames loses between frames (host enqueue latency, joins). Needs two
+ * consecutive timed renders, else HYRF_ERR_NOT_READY. */
+hyrf_status hyrf_frame_gap(hyrf_scene* scene, float* ms);
 
 /* Ablation switches of the same pass (PAPER.md:214-223 Table 5, :233-237, :259-261). mask = OR of:
  *  NO_CULL:     the fields are queried and aggregated for every stored Gaussian; those failing Eq. 9 are dropped at
@@ -231,6 +235,15 @@ hyrf_status hyrf_set_ablation(hyrf_scene* scene, uint32_t mask);
  * serialises the frame on the caller's stream (one kernel at a time: what per-kernel profiling wants). The image and
  * every debug export are identical either way. */
 hyrf_status hyrf_set_sort_overlap(hyrf_scene* scene, int on);
+
+/* Frame pipelining for a STREAM of hyrf_render calls (hyrf_render_host_async always works this way). S1 and the depth
+ * sort of a frame depend on the camera and the explicit positions only and write library-owned, double-buffered
+ * scratch, so with on != 0 they are enqueued on the library's own high-priority stream WITHOUT waiting for what the
+ * caller's stream still holds: frame k+1's cull and sort run beside frame k's rasterizer, and its field kernel then
+ * takes every SM. Everything that touches out_rgb stays on the caller's stream, in order; images are bit-identical.
+ * Default off: each hyrf_render starts behind all work enqueued before it (what a per-frame timing bracket on the
+ * caller's stream must see). Needs hyrf_set_sort_overlap on (the default). */
+hyrf_status hyrf_set_pipelining(hyrf_scene* scene, int on);
 
 /* Rasterizer variant (S5; Eq. 1). Every variant stages a tile's depth-ordered list once per tile and
  * produces the same bits; they differ in cost. mode 1: every warp of the tile blends every staged entry. mode 2: a warp

@@ -30,6 +30,7 @@ extern "C" const char* hyrf_last_error(void) { return g_err; }
 hyrf_status hy_launch_field_fma(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
 hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
 hyrf_status hy_launch_field_ws(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
+void hy_launch_counters_to_host(const FrameCounters* dev, FrameCounters* pinned_host, cudaStream_t st);
 bool hy_field_mma_supported(const hyrf_scene_desc& d);
 hyrf_status hy_field_mma_prepare(hyrf_scene* s);
 size_t hy_field_mma_packed_bytes();
@@ -152,18 +153,36 @@ hyrf_status ensure_entries(hyrf_scene* s, size_t need) {
     return HYRF_OK;
 }
 
+// the scene's S1 / depth-sort members become aliases of set k
+void hy_select_pre_set(hyrf_scene* s, int k) {
+    hyrf_scene::PreSet& P = s->pre[k];
+    s->pre_cur = k;
+    s->flag_words = P.flag_words; s->id_words = P.id_words; s->word_rank = P.word_rank; s->vis_m = P.vis_m;
+    s->block_counts = P.block_counts; s->vis_idx = P.vis_idx;
+    s->sort_a_key = P.sort_a_key; s->sort_a_val = P.sort_a_val; s->sort_b_key = P.sort_b_key; s->sort_b_val = P.sort_b_val;
+    s->counters = P.counters; s->counters_host = P.counters_host;
+}
+
 void destroy(hyrf_scene* s) {
     if (!s) return;
     cudaStreamSynchronize(s->stream);
     void* ptrs[] = {s->pos, s->rgb, s->scale, s->opac, (void*)s->geo_grid.table, (void*)s->app_grid.table,
                     (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w, s->both_table,
-                    s->gm, s->gm_id, s->flag_words, s->id_words, s->word_rank, s->vis_m, s->block_counts, s->vis_idx, s->rec, s->rect, s->tiles, s->mtiles, s->mranges,
-                    s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->tt_sorted, s->offs,
-                    s->scan_scratch, s->counters, s->ranges, s->tile_queue, s->fg, s->finalT, s->image, s->image2, s->bg_mask, s->bg_list,
+                    s->gm, s->gm_id, s->rec, s->rect, s->tiles, s->mtiles, s->mranges, s->tt_sorted, s->offs,
+                    s->scan_scratch, s->ranges, s->tile_queue, s->fg, s->finalT, s->image, s->image2, s->bg_mask, s->bg_list,
                     s->dbg_raw, s->dbg_attrs};
     for (void* p : ptrs) dev_free(s, p);
+    if (s->sort_stream) cudaStreamSynchronize(s->sort_stream);
+    for (auto& P : s->pre) {   // (the scene's members of the same names are aliases of one of the two sets)
+        void* pp[] = {P.flag_words, P.id_words, P.word_rank, P.vis_m, P.block_counts, P.vis_idx, P.sort_a_key, P.sort_a_val,
+                      P.sort_b_key, P.sort_b_val, P.hist, P.scan, P.counters};
+        for (void* p : pp) dev_free(s, p);
+        if (P.counters_host) cudaFreeHost(P.counters_host);
+        if (P.ev_free) cudaEventDestroy(P.ev_free);
+    }
     free_entries(s);
-    if (s->counters_host) cudaFreeHost(s->counters_host);
+    if (s->ev_start) cudaEventDestroy(s->ev_start);
+    if (s->ev_frame_done) cudaEventDestroy(s->ev_frame_done);
     if (s->ev_counters) cudaEventDestroy(s->ev_counters);
     if (s->sort_stream) { cudaStreamSynchronize(s->sort_stream); cudaStreamDestroy(s->sort_stream); }
     if (s->ev_culled) cudaEventDestroy(s->ev_culled);
@@ -279,37 +298,53 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     }
     HY_TRY(dev_alloc_t(s, &s->gm, 2 * N));
     HY_TRY(dev_alloc_t(s, &s->gm_id, N));
-    HY_TRY(dev_alloc_t(s, &s->flag_words, (N + 31) / 32 + 32));
-    HY_TRY(dev_alloc_t(s, &s->id_words, (N + 31) / 32 + 32));
-    HY_TRY(dev_alloc_t(s, &s->word_rank, (N + 31) / 32 + 32));
-    HY_TRY(dev_alloc_t(s, &s->vis_m, N));
-    HY_TRY(dev_alloc_t(s, &s->block_counts, 4 * cull_blocks + 8));
-    HY_TRY(dev_alloc_t(s, &s->vis_idx, N));
+    for (auto& P : s->pre) {
+        HY_TRY(dev_alloc_t(s, &P.flag_words, (N + 31) / 32 + 32));
+        HY_TRY(dev_alloc_t(s, &P.id_words, (N + 31) / 32 + 32));
+        HY_TRY(dev_alloc_t(s, &P.word_rank, (N + 31) / 32 + 32));
+        HY_TRY(dev_alloc_t(s, &P.vis_m, N));
+        HY_TRY(dev_alloc_t(s, &P.block_counts, 4 * cull_blocks + 8));
+        HY_TRY(dev_alloc_t(s, &P.vis_idx, N));
+        HY_TRY(dev_alloc_t(s, &P.sort_a_key, N));
+        HY_TRY(dev_alloc_t(s, &P.sort_a_val, N));
+        HY_TRY(dev_alloc_t(s, &P.sort_b_key, N));
+        HY_TRY(dev_alloc_t(s, &P.sort_b_val, N));
+        HY_TRY(dev_alloc_t(s, &P.hist, hy_radix_hist_elems(N)));
+        HY_TRY(dev_alloc_t(s, &P.scan, 2 * hy_scan_scratch_elems(N) + 64));
+        HY_TRY(dev_alloc_t(s, &P.counters, 1));
+        if ((e = cudaMallocHost(reinterpret_cast<void**>(&P.counters_host), sizeof(FrameCounters))) != cudaSuccess) {
+            destroy(s);
+            return hy_cuda_fail(e, "cudaMallocHost");
+        }
+        if ((e = cudaEventCreateWithFlags(&P.ev_free, cudaEventDisableTiming)) != cudaSuccess) {
+            destroy(s);
+            return hy_cuda_fail(e, "cudaEventCreate");
+        }
+    }
+    hy_select_pre_set(s, 0);
     HY_TRY(dev_alloc_t(s, &s->rec, 3 * N));
     HY_TRY(dev_alloc_t(s, &s->rect, N));
     HY_TRY(dev_alloc_t(s, &s->tiles, N));
     HY_TRY(dev_alloc_t(s, &s->mtiles, N));
-    HY_TRY(dev_alloc_t(s, &s->sort_a_key, N));
-    HY_TRY(dev_alloc_t(s, &s->sort_a_val, N));
-    HY_TRY(dev_alloc_t(s, &s->sort_b_key, N));
-    HY_TRY(dev_alloc_t(s, &s->sort_b_val, N));
     HY_TRY(dev_alloc_t(s, &s->tt_sorted, N));
     HY_TRY(dev_alloc_t(s, &s->offs, N));
-    HY_TRY(dev_alloc_t(s, &s->counters, 1));
     HY_TRY(dev_alloc_t(s, &s->ranges, tiles));
     HY_TRY(dev_alloc_t(s, &s->mranges, tiles));
     HY_TRY(dev_alloc_t(s, &s->tile_queue, tiles));
     HY_TRY(dev_alloc_t(s, &s->finalT, P));
     HY_TRY(dev_alloc_t(s, &s->bg_list, P));
-    if ((e = cudaMallocHost(reinterpret_cast<void**>(&s->counters_host), sizeof(FrameCounters))) != cudaSuccess) {
-        destroy(s);
-        return hy_cuda_fail(e, "cudaMallocHost");
-    }
-    if ((e = cudaEventCreateWithFlags(&s->ev_counters, cudaEventDisableTiming)) != cudaSuccess) {
+    if ((e = cudaEventCreateWithFlags(&s->ev_counters, cudaEventDisableTiming)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&s->ev_start, cudaEventDisableTiming)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&s->ev_frame_done, cudaEventDisableTiming)) != cudaSuccess) {
         destroy(s);
         return hy_cuda_fail(e, "cudaEventCreate");
     }
-    if ((e = cudaStreamCreateWithFlags(&s->sort_stream, cudaStreamNonBlocking)) != cudaSuccess ||
+    // S1 and the depth sort are short, latency-bound kernels that must slip in beside the field kernel (and, in a pipelined
+    // stream of frames, beside the previous frame's rasterizer): their stream gets the highest priority, so the block
+    // scheduler hands freed SM slots to their CTAs first
+    int prio_lo = 0, prio_hi = 0;
+    cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+    if ((e = cudaStreamCreateWithPriority(&s->sort_stream, cudaStreamNonBlocking, prio_hi)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&s->ev_culled, cudaEventDisableTiming)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&s->ev_sorted, cudaEventDisableTiming)) != cudaSuccess) {
         destroy(s);
@@ -528,24 +563,51 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     uint32_t launches = 0;
     s->lastW = W; s->lastH = H;
     s->rendered = false;
-    if (timing) cudaEventRecord(s->ev[0], s->stream);
+    // S1 and the depth sort write the OTHER set of their buffers than the previous frame (scene.h PreSet)
+    hy_select_pre_set(s, s->pre_cur ^ 1);
+    hyrf_scene::PreSet& P = s->pre[s->pre_cur];
+    const bool overlap = s->sort_overlap;
+    const bool pipeline = (s->pipeline || s->pipeline_all) && overlap;
+    cudaStream_t pst = overlap ? s->sort_stream : s->stream;   // where S1 and the depth sort run
+    if (timing) {
+        s->prev_timed = s->last_timed;
+        s->ev_end = s->ev_end == 5 ? 6 : 5;
+        cudaEventRecord(s->ev[0], s->stream);
+    }
+    s->last_timed = timing;
+    if (overlap) {
+        // the frame that last used this set (two frames ago) must have stopped reading it
+        if (P.in_use && (e = cudaStreamWaitEvent(pst, P.ev_free, 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent(set free)");
+        if (!pipeline) {
+            // one frame at a time (hyrf_render / hyrf_render_host): S1 starts behind everything already enqueued on the
+            // caller's stream. A pipelined stream of frames (hyrf_render_host_async) skips this: its cull and depth sort
+            // run beside the previous frame's rasterizer.
+            if ((e = cudaEventRecord(s->ev_start, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(start)");
+            if ((e = cudaStreamWaitEvent(pst, s->ev_start, 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent(start)");
+        }
+    }
 
     // S1: visibility pre-culling
-    hy_launch_cull(s, f, &launches);
+    hy_launch_cull(s, f, &launches, pst, P.scan);
+    if (overlap) {
+        if ((e = cudaEventRecord(s->ev_culled, pst)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(culled)");
+        if ((e = cudaStreamWaitEvent(s->stream, s->ev_culled, 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent(culled)");
+    }
     if (timing) cudaEventRecord(s->ev[1], s->stream);
 
     // S4c first half: order the visible Gaussians by (depth bits, id). The keys are the cull's (Z needs nothing from
     // the fields), so the five small, latency-bound sort kernels run on their own stream beside the field kernel,
-    // which leaves a few CTA slots free for them (hy_launch_field_*), and join the frame before the binning.
+    // which leaves a few SMs free for them (hy_launch_field_*), and join the frame before the binning.
     uint32_t *order_key = nullptr, *order = nullptr;
-    const bool overlap = s->sort_overlap;
     if (overlap) {
-        if ((e = cudaEventRecord(s->ev_culled, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(culled)");
-        if ((e = cudaStreamWaitEvent(s->sort_stream, s->ev_culled, 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent(culled)");
-        hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, s->hist,
-                        s->scan_scratch, s->sort_stream, &order_key, &order, &launches, /*iota_vals=*/true);
-        if ((e = cudaEventRecord(s->ev_sorted, s->sort_stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(sorted)");
+        hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, P.hist,
+                        P.scan, pst, &order_key, &order, &launches, /*iota_vals=*/true);
+        if ((e = cudaEventRecord(s->ev_sorted, pst)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(sorted)");
     }
+    // In a pipelined stream the sort has the previous frame's rasterizer to hide under, so the field kernel takes every
+    // SM; otherwise it leaves some to the sort running beside it.
+    s->field_full_grid = !overlap || (pipeline && s->frame_in_flight && cudaEventQuery(s->ev_frame_done) == cudaErrorNotReady);
+    cudaGetLastError();
 
     // S2 + S3 + S4a: field query, aggregation, projection
     // (explicit-only ablation: no field is queried, so the CUDA-core kernel's early-out path serves both dtypes)
@@ -556,16 +618,19 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
 
     // counters (V, D) start their way to the host now; the depth ordering below does not need them, so the copy
     // and the host's wake-up hide behind it
-    if ((e = cudaMemcpyAsync(s->counters_host, s->counters, sizeof(FrameCounters), cudaMemcpyDeviceToHost, s->stream)) != cudaSuccess)
-        return hy_cuda_fail(e, "cudaMemcpyAsync(counters)");
+    // (written by a one-warp kernel straight into the pinned host block, not by a memcpy: a device-to-host memcpy would
+    // queue on the copy engine behind the previous frame's 11 MB image copy of hyrf_render_host_async and hold this
+    // stream — and the host — back until that has finished)
+    hy_launch_counters_to_host(s->counters, s->counters_host, s->stream);
+    ++launches;
     if ((e = cudaEventRecord(s->ev_counters, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(counters)");
 
     // S4b-c: the depth order joins here (or is computed here when serialised); build the per-tile lists in that order
     if (overlap) {
         if ((e = cudaStreamWaitEvent(s->stream, s->ev_sorted, 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent(sorted)");
     } else {
-        hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, s->hist,
-                        s->scan_scratch, s->stream, &order_key, &order, &launches, /*iota_vals=*/true);
+        hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, P.hist,
+                        P.scan, s->stream, &order_key, &order, &launches, /*iota_vals=*/true);
     }
     const uint32_t n_tiles = (uint32_t)(f.gx * f.gy);
     uint32_t V = 0;
@@ -609,7 +674,7 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
                              want_lists ? s->ent_val[0] : nullptr);                            // S5 (Eq. 1)
             if (timing) cudaEventRecord(s->ev[4], s->stream);
             if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;   // S6 (Eq. 10-11, A.2)
-            if (timing) cudaEventRecord(s->ev[5], s->stream);
+            if (timing) cudaEventRecord(s->ev[s->ev_end], s->stream);
             if (attempt == 0 && (e = cudaEventSynchronize(s->ev_counters)) != cudaSuccess)
                 return hy_cuda_fail(e, "cudaEventSynchronize(counters)");
             V = s->counters_host->V;
@@ -648,10 +713,16 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
         hy_launch_raster(s, f, s->ranges, sorted_val, /*macro=*/false, out_rgb, &launches, nullptr, nullptr);   // S5
         if (timing) cudaEventRecord(s->ev[4], s->stream);
         if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;       // S6 (Eq. 10-11, A.2)
-        if (timing) cudaEventRecord(s->ev[5], s->stream);
+        if (timing) cudaEventRecord(s->ev[s->ev_end], s->stream);
     }
 
     if ((e = cudaGetLastError()) != cudaSuccess) return hy_cuda_fail(e, "kernel launch");
+    // from here on nothing of this frame reads the cull / sort set any more (the rasterizer and the background work from
+    // the records and lists): the frame after next may overwrite it
+    if ((e = cudaEventRecord(P.ev_free, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(set free)");
+    P.in_use = true;
+    if ((e = cudaEventRecord(s->ev_frame_done, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(frame done)");
+    s->frame_in_flight = true;
     s->last_launches = launches;
     s->lastV = V; s->lastD = D; s->lastDm = s->counters_host->Dm;
     s->rendered = true;
@@ -699,7 +770,10 @@ extern "C" hyrf_status hyrf_render_host_async(hyrf_scene* s, const hyrf_camera* 
     float* img = slot ? s->image2 : s->image;
     // the copy that last read this image must have finished before it is rendered into again
     if (s->slot_used[slot] && (e = cudaStreamWaitEvent(s->stream, s->ev_copied[slot], 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent");
-    if ((st = render_impl(s, cam, W, H, img)) != HYRF_OK) return st;
+    s->pipeline = true;   // a stream of frames: this one's cull and depth sort may run beside the previous one's rasterizer
+    st = render_impl(s, cam, W, H, img);
+    s->pipeline = false;
+    if (st != HYRF_OK) return st;
     if ((e = cudaEventRecord(s->ev_rendered[slot], s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord");
     if ((e = cudaStreamWaitEvent(s->copy_stream, s->ev_rendered[slot], 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent");
     if ((e = cudaMemcpyAsync(out_host, img, (size_t)W * H * 3 * sizeof(float), cudaMemcpyDeviceToHost, s->copy_stream)) != cudaSuccess)
@@ -726,11 +800,20 @@ extern "C" hyrf_status hyrf_set_timing(hyrf_scene* s, int32_t enabled) {
 extern "C" hyrf_status hyrf_stage_times(hyrf_scene* s, float ms[6]) {
     if (!s || !ms) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_stage_times: NULL argument");
     if (!s->rendered || !s->timing || !s->ev_valid) return hy_fail(HYRF_ERR_NOT_READY, "no timed render yet");
-    cudaError_t e = cudaEventSynchronize(s->ev[5]);
+    cudaError_t e = cudaEventSynchronize(s->ev[s->ev_end]);
     if (e != cudaSuccess) return hy_cuda_fail(e, "cudaEventSynchronize");
     for (int k = 0; k < 5; ++k)
-        if ((e = cudaEventElapsedTime(&ms[k], s->ev[k], s->ev[k + 1])) != cudaSuccess) return hy_cuda_fail(e, "cudaEventElapsedTime");
-    if ((e = cudaEventElapsedTime(&ms[5], s->ev[0], s->ev[5])) != cudaSuccess) return hy_cuda_fail(e, "cudaEventElapsedTime");
+        if ((e = cudaEventElapsedTime(&ms[k], s->ev[k], s->ev[k == 4 ? s->ev_end : k + 1])) != cudaSuccess) return hy_cuda_fail(e, "cudaEventElapsedTime");
+    if ((e = cudaEventElapsedTime(&ms[5], s->ev[0], s->ev[s->ev_end])) != cudaSuccess) return hy_cuda_fail(e, "cudaEventElapsedTime");
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_frame_gap(hyrf_scene* s, float* ms) {
+    if (!s || !ms) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_frame_gap: NULL argument");
+    if (!s->rendered || !s->timing || !s->ev_valid || !s->prev_timed) return hy_fail(HYRF_ERR_NOT_READY, "hyrf_frame_gap needs two consecutive timed renders");
+    cudaError_t e = cudaEventSynchronize(s->ev[s->ev_end]);
+    if (e != cudaSuccess) return hy_cuda_fail(e, "cudaEventSynchronize");
+    if ((e = cudaEventElapsedTime(ms, s->ev[s->ev_end == 5 ? 6 : 5], s->ev[0])) != cudaSuccess) return hy_cuda_fail(e, "cudaEventElapsedTime");
     return HYRF_OK;
 }
 
@@ -745,6 +828,12 @@ extern "C" hyrf_status hyrf_set_sort_overlap(hyrf_scene* s, int on) {
     if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_sort_overlap: NULL scene");
     s->sort_overlap = on != 0;
     if (on > 1) s->ws_sort_sms = on < s->sm_count ? on : s->sm_count - 1;   // on > 1: SMs the warp-specialised field kernel leaves to the sort
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_set_pipelining(hyrf_scene* s, int on) {
+    if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_pipelining: NULL scene");
+    s->pipeline_all = on != 0;
     return HYRF_OK;
 }
 

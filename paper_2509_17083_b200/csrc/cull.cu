@@ -207,21 +207,21 @@ hyrf_status hy_prepare_morton(hyrf_scene* s) {
     return HYRF_OK;
 }
 
-void hy_launch_cull(hyrf_scene* s, const FrameDev& f, uint32_t* launches) {
+void hy_launch_cull(hyrf_scene* s, const FrameDev& f, uint32_t* launches, cudaStream_t st, uint32_t* scan_scratch) {
     const uint32_t nb = (s->N + kCullItems - 1) / kCullItems;
     uint32_t* m_counts = s->block_counts;
     uint32_t* m_offs = s->block_counts + nb;
     uint32_t* id_counts = s->block_counts + 2 * nb;
     uint32_t* id_offs = s->block_counts + 3 * nb;
-    cull_mark_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->gm, s->pos, s->N, f, s->flag_words, m_counts, s->id_words,
+    cull_mark_kernel<<<nb, kCullThreads, 0, st>>>(s->gm, s->pos, s->N, f, s->flag_words, m_counts, s->id_words,
                                                          id_counts);
     ++*launches;
     const bool in_kernel = nb <= 8192;   // block offsets summed inside the compaction; beyond that, scan first
     if (!in_kernel) {
-        hy_launch_scan(m_counts, m_offs, nb, s->scan_scratch, s->stream, launches);
-        hy_launch_scan(id_counts, id_offs, nb, s->scan_scratch, s->stream, launches);
+        hy_launch_scan(m_counts, m_offs, nb, scan_scratch, st, launches);
+        hy_launch_scan(id_counts, id_offs, nb, scan_scratch, st, launches);
     }
-    cull_compact_kernel<<<nb, kCullThreads, 0, s->stream>>>(s->flag_words, in_kernel ? nullptr : m_offs, m_counts,
+    cull_compact_kernel<<<nb, kCullThreads, 0, st>>>(s->flag_words, in_kernel ? nullptr : m_offs, m_counts,
                                                             s->id_words, in_kernel ? nullptr : id_offs, id_counts, s->N,
                                                             s->vis_m, s->vis_idx, s->word_rank, s->counters, s->pos, f,
                                                             s->sort_a_key);

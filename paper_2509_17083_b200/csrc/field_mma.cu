@@ -759,7 +759,7 @@ hyrf_status hy_launch_field_mma(hyrf_scene* s, const FrameDev& f, uint32_t* laun
     // CTA slots left to the depth sort running beside this kernel (hyrf_set_sort_overlap): with none, the persistent
     // CTAs hold every register of every SM and the sort waits for the kernel to end. Config 3, frame time against the
     // slots left free: 0 -> 0.586, 16 -> 0.563, 32 -> 0.551, 48 -> 0.561 ms (serial: 0.620 ms).
-    const int gap = s->sort_overlap ? (32 * s->sm_count) / 148 : 0;
+    const int gap = s->field_full_grid ? 0 : (32 * s->sm_count) / 148;
     const int slots = s->sm_count * 2 - gap;
     const int grid = need < slots ? need : slots;
     const uint4* w = reinterpret_cast<const uint4*>(s->mma_w);

@@ -287,7 +287,7 @@ hyrf_status hy_launch_field_ws(hyrf_scene* s, const FrameDev& f, uint32_t* launc
     const int need = (int)((s->N + kTile - 1) / kTile);
     // One CTA per SM holds (nearly) every register of it: with the depth sort beside this kernel (hyrf_set_sort_overlap)
     // a few SMs are left to the sort's CTAs.
-    const int gap = s->sort_overlap ? s->ws_sort_sms : 0;
+    const int gap = s->field_full_grid ? 0 : s->ws_sort_sms;
     const int slots = s->sm_count - gap > 1 ? s->sm_count - gap : 1;
     const int grid = need < slots ? need : slots;
     const uint4* w = reinterpret_cast<const uint4*>(s->mma_w);

@@ -98,3 +98,16 @@ void hy_launch_scan(const uint32_t* in, uint32_t* out, size_t n, uint32_t* scrat
     scan_apply_kernel<<<(unsigned)nb, kScanThreads, 0, st>>>(in, out, n, partial_scanned);
     ++*launches;
 }
+
+// The frame's counters to the (pinned, device-visible) host block: 16 words by one warp (see api.cu render_impl).
+namespace {
+__global__ void counters_to_host_kernel(const uint32_t* __restrict__ dev, volatile uint32_t* __restrict__ host) {
+    if (threadIdx.x < sizeof(FrameCounters) / 4) host[threadIdx.x] = dev[threadIdx.x];
+    __threadfence_system();
+}
+}  // namespace
+
+void hy_launch_counters_to_host(const FrameCounters* dev, FrameCounters* pinned_host, cudaStream_t st) {
+    static_assert(sizeof(FrameCounters) % 4 == 0 && sizeof(FrameCounters) <= 128, "one warp copies the counters");
+    counters_to_host_kernel<<<1, 32, 0, st>>>(reinterpret_cast<const uint32_t*>(dev), reinterpret_cast<volatile uint32_t*>(pinned_host));
+}

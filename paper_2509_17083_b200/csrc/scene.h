@@ -59,6 +59,24 @@ struct hyrf_scene {
     float4* gm = nullptr;      // [N][2] Morton-ordered records (pos.xyz, scale | opacity, rgb), built at upload (cull.cu)
     uint32_t* gm_id = nullptr; // [N] id of the m-th Gaussian in Morton order
 
+    // What S1 and the depth sort write exists twice: a stream of frames (hyrf_render_host_async) runs frame k+1's cull and
+    // sort on `sort_stream` beside frame k's rasterizer. The members below with the same names alias the set of the frame
+    // being enqueued (and, afterwards, of the last frame: what the debug fetches read).
+    struct PreSet {
+        uint32_t *flag_words = nullptr, *id_words = nullptr, *word_rank = nullptr, *vis_m = nullptr, *block_counts = nullptr,
+                 *vis_idx = nullptr, *sort_a_key = nullptr, *sort_a_val = nullptr, *sort_b_key = nullptr, *sort_b_val = nullptr;
+        uint32_t *hist = nullptr, *scan = nullptr;        // radix / scan workspace of the depth sort and the cull's scans
+        FrameCounters *counters = nullptr, *counters_host = nullptr;
+        cudaEvent_t ev_free = nullptr;                    // main stream: the frame that used this set no longer reads it
+        bool in_use = false;
+    } pre[2];
+    int pre_cur = 0;
+    bool pipeline = false;            // the frame being enqueued belongs to a pipelined stream (no ordering behind the previous frame's tail)
+    bool pipeline_all = false;        // hyrf_set_pipelining: every hyrf_render is enqueued that way
+    bool frame_in_flight = false;     // a previous frame's end event has been recorded
+    bool field_full_grid = false;     // this frame's field kernel takes every SM (nothing runs beside it, or the sort hides elsewhere)
+    cudaEvent_t ev_start = nullptr, ev_frame_done = nullptr;
+
     // per-frame scratch sized from N
     uint32_t* flag_words = nullptr;   // [ceil(N/32)] visibility bits, Morton order
     uint32_t* id_words = nullptr;     // [ceil(N/32)] visibility bits, id order (also the VIS_MASK debug export)
@@ -114,7 +132,10 @@ struct hyrf_scene {
     float* dbg_raw = nullptr;         // [N][11]
     float* dbg_attrs = nullptr;       // [N][11]
     bool timing = false;
-    cudaEvent_t ev[7] = {};
+    cudaEvent_t ev[7] = {};           // [0..4] stage starts; [5], [6] frame ends, alternating by frame (ev_end)
+    int ev_end = 5;                   // which of ev[5] / ev[6] closes the last frame
+    bool last_timed = false;
+    bool prev_timed = false;          // the frame before the last one was timed too (hyrf_frame_gap)
     cudaEvent_t ev_counters = nullptr;
     cudaStream_t sort_stream = nullptr;                  // the depth sort runs here, beside the field kernel
     bool sort_overlap = true;                            // hyrf_set_sort_overlap
@@ -137,7 +158,7 @@ hyrf_status hy_launch_explicit_decode(hyrf_scene* s, const uint16_t* pos_h, cons
                                       const float* codebooks, uint32_t S, uint32_t K, uint32_t* first_bad);
 // S1 (cull.cu): visibility bits, stable compactions -> vis_m (Morton work list), vis_idx + rank lookup (id order)
 hyrf_status hy_prepare_morton(hyrf_scene* s);
-void hy_launch_cull(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
+void hy_launch_cull(hyrf_scene* s, const FrameDev& f, uint32_t* launches, cudaStream_t st, uint32_t* scan_scratch);
 // S2 + S3 + S4a (field.cu): per visible Gaussian query both fields, aggregate, project
 hyrf_status hy_launch_field(hyrf_scene* s, const FrameDev& f, uint32_t* launches);
 // device-wide exclusive scan of n u32 (scan.cu); scratch must hold hy_scan_scratch_elems(n)
