@@ -152,10 +152,18 @@ def stage_rooflines(scene, V, D, Dm, n_bg, eval_pairs, peaks):
         "bin": {"bound": "hbm", "work": bin_bytes, "peak": hbm, "unit": "GB/s"},
     }
     # S5: plain ALU issue. 20 issue slots per evaluated (pixel, Gaussian) pair (16 fp32 ops + ex2 + 3 predicates,
-    # SURVEY §8(d)); peak = 148 SMs x 4 schedulers x 32 lanes x SM clock
-    alu_peak = 148 * 4 * 32 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e9     # G lane-slots / s
+    # SURVEY §8(d)). Peak: the SUSTAINED issue rate measured by the blend-mix microprobe (profiles/r2_probes.json,
+    # `python bench.py --probe`), x 32 lanes; without it, the nominal SMs x 4 schedulers x 32 lanes x SM clock.
+    alu_nominal = peaks.get("sm_count", 148) * 4 * 32 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e9     # G lane-slots / s
+    probes = load_probes()
+    alu_peak, alu_src = alu_nominal, "nominal (SMs x 4 x 32 x clock)"
+    if probes:
+        mix = [v for k, v in probes["issue_warp_instr_per_s_best"].items() if k.startswith("blend mix")]
+        if mix:
+            alu_peak, alu_src = 32.0 * mix[0] / 1e9, "measured (blend-mix issue probe, profiles/r2_probes.json)"
     if eval_pairs:
-        out["raster"] = {"bound": "alu", "work": eval_pairs * 20, "peak": alu_peak, "unit": "Gslot/s"}
+        out["raster"] = {"bound": "alu", "work": eval_pairs * 20, "peak": alu_peak, "unit": "Gslot/s",
+                         "peak_source": alu_src, "nominal_peak": alu_nominal}
     if n_bg is not None:
         bgl = scene.bg_grid.levels * 8
         out["background"] = {"bound": "hbm", "work": n_bg * (bgl * 2 * esz + 4 + 4 + 12 + 12), "peak": hbm, "unit": "GB/s"}
@@ -163,18 +171,19 @@ def stage_rooflines(scene, V, D, Dm, n_bg, eval_pairs, peaks):
 
 
 def load_traffic(kernel: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu --set full capture
-    of this workload (profiles/r1h_dram_traffic.csv; raster_kernel, not launched in that run: r1f's); None if there is no
-    capture."""
-    p = os.path.join(ROOT, "profiles", "r1f_dram_traffic.csv" if kernel == "raster_kernel" else "r1h_dram_traffic.csv")
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` and, for the field kernel, its L1TEX global-load
+    sector look-ups per visible Gaussian, from the committed ncu --set full capture of this workload
+    (profiles/r2_dram_traffic.csv, made by the commands in profiles/r2_README.md). (None, None) without a capture."""
+    p = os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")
     if not os.path.exists(p):
-        return None
+        return None, None
     import csv
     with open(p) as f:
         for row in csv.DictReader(f):
             if row["kernel"] == kernel:
-                return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
-    return None
+                sec = row.get("l1tex_ld_sectors_per_visible") or ""
+                return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), (float(sec) if sec else None)
+    return None, None
 
 
 def load_peaks():
@@ -268,7 +277,8 @@ def run_probe(args):
             gather.append({"table_mb": 64, "entry_bytes": 8, "ctas_per_sm": ctas, "share": share, "line": line,
                            "lookups_per_s": lk, "sectors_per_s": sec, "ms": ms})
     issue = []
-    for kind, name in ((0, "ffma"), (1, "ffma+alu"), (2, "blend mix (1 MUFU.EX2 per 26.75 instructions)")):
+    for kind, name in ((0, "ffma"), (3, "ffma2 (fma.rn.f32x2: two fma per lane and issue slot)"), (1, "ffma+alu"),
+                       (2, "blend mix (1 MUFU.EX2 per 26.75 instructions)")):
         for ctas in (1, 2, 4, 8):
             wi, ms = B.probe_issue(dev, kind, ctas, iters=8192)
             issue.append({"kind": name, "ctas_per_sm": ctas, "warp_instr_per_s": wi, "lane_slots_per_s": 32.0 * wi, "ms": ms})
@@ -500,6 +510,8 @@ def run_ours(args):
         eval_pairs = pairs / fr
         cpu = {"value": fr / sec, "unit": UNIT, "cores": thr, "kind": "oracle",
                "sample": f"{fr} whole frame(s) of the workload ({vtot / fr:.0f} visible Gaussians each)"}
+    peaks["sm_count"] = torch.cuda.get_device_properties(dev).multi_processor_count
+    probes = load_probes()
     rl = stage_rooflines(scene, Vm, Dm, Dmm, n_bg, eval_pairs, peaks)
     per_stage = {}
     for i, n in enumerate(names):
@@ -508,10 +520,14 @@ def run_ours(args):
             ach = r["work"] / (stage_ms[i] * 1e-3) / 1e9
             per_stage[n] = {"bound": r["bound"], "achieved": ach, "peak": r["peak"], "unit": r["unit"],
                             "frac": ach / r["peak"], "ms": float(stage_ms[i])}
+            if "nominal_peak" in r:
+                per_stage[n].update({"peak_source": r["peak_source"], "frac_of_nominal": ach / r["nominal_peak"]})
     # the dominant KERNEL: S2+S3+S4a and S5 are one kernel each; S4b-c is nine short ones
     dom = "field" if stage_ms[1] >= stage_ms[3] else "raster"
-    roof = {"kernel": kernels[dom], "stage": dom, "traffic": load_traffic(kernels[dom]) if args.config == 3 else None,
-            "peak_source": peaks["source"] + (" (burst HBM copy)" if per_stage.get(dom, {}).get("bound") == "hbm" else "")}
+    traffic, sec_per_vis = load_traffic(kernels[dom]) if args.config == 3 else (None, None)
+    roof = {"kernel": kernels[dom], "stage": dom, "traffic": traffic,
+            "peak_source": per_stage.get(dom, {}).get("peak_source") or
+                           (peaks["source"] + (" (burst HBM copy)" if per_stage.get(dom, {}).get("bound") == "hbm" else ""))}
     if dom in per_stage:
         roof.update({k: per_stage[dom][k] for k in ("bound", "achieved", "peak", "unit", "frac")})
         roof["launch_ms"] = per_stage[dom]["ms"]
@@ -519,11 +535,23 @@ def run_ours(args):
         di = names.index(dom)
         roof["serial_launch_ms"] = float(stage_serial_ms[di])
         roof["serial_frac"] = rl[dom]["work"] / (stage_serial_ms[di] * 1e-3) / 1e9 / rl[dom]["peak"]
+    # What actually bounds the field kernel (its tables are L2-resident, DRAM moves a sixth of the algorithmic bytes): the
+    # rate at which an SM looks up scattered sectors. Achieved = the kernel's L1TEX global-load sector look-ups (ncu count
+    # per visible Gaussian of the committed capture x this run's V) / its launch time; peak = the gather microprobe.
+    _, field_sec = load_traffic(kernels["field"]) if args.config == 3 else (None, None)
+    if probes and field_sec:
+        ach = field_sec * Vm / (stage_ms[1] * 1e-3)
+        roof_l1 = {"bound": "l1tex_gather", "kernel": kernels["field"], "achieved": ach / 1e9, "peak": probes["gather_sectors_per_s_best"] / 1e9,
+                   "unit": "Gsector/s", "frac": ach / probes["gather_sectors_per_s_best"],
+                   "sectors_per_visible_gaussian": field_sec, "peak_source": "measured (gather microprobe, profiles/r2_probes.json)"}
+        if dom == "field":
+            roof["l1tex_gather"] = roof_l1
+        per_stage["field"]["l1tex_gather"] = roof_l1
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f16" if scene.fp16 else "f32", "data": "synthetic",
             "config": {"workload": name, "l2": "flushed between steps (256 MiB write)", "mlp_path": args.mlp, "ablation": args.ablation, "raster": args.raster,
-                       "schedule": "depth sort on a second stream beside the field kernel (hyrf_set_sort_overlap default)",
+                       "schedule": "one frame at a time; S1 + depth sort on the library's second stream, the sort beside the field kernel (hyrf_set_sort_overlap default); e2e: frames pipelined (hyrf_render_host_async)",
                        "parallelism": f"replicas x{world} (cameras round-robin)"},
             "visible_gaussians_per_s": vis_per_s, "V_mean": Vm, "D_mean": Dm, "Dm_mean": Dmm,
             "stage_ms": {n: float(stage_ms[i]) for i, n in enumerate(names)} | {"frame": float(stage_ms[5])},
