@@ -86,7 +86,9 @@ _lib: Optional[C.CDLL] = None
 def lib() -> C.CDLL:
     global _lib
     if _lib is None:
-        L = C.CDLL(build())
+        # HYRF_ORACLE_SO: a separately built oracle library (e.g. the -fsanitize=address,undefined build the
+        # sanitizer pass of profiles/r2_sanitizer.md runs the CPU tests against)
+        L = C.CDLL(os.environ.get("HYRF_ORACLE_SO") or build())
         L.ho_half_to_float.restype = C.c_float
         L.ho_half_to_float.argtypes = [C.c_uint16]
         L.ho_float_to_half.restype = C.c_uint16
