@@ -54,6 +54,32 @@ def sum_over_ranks(x: float) -> float:
     return float(t.item())
 
 
+def gather_strips(img, H: int, rank: int, world: int, align: int = 64):
+    """Screen-strip parallelism (hyrf_set_strip): `img` is a (rows >= H, W, 3) tensor whose rows
+    synth.strip_rows(H, rank, world) this rank has rendered; ONE all-gather of equal blocks of rows makes every row valid
+    on every rank. With NCCL the gather is in place (each rank's block already sits where it belongs in `img`, which
+    must then hold world x block rows); otherwise (gloo, CPU tests) through a staging copy. Returns img[:H]."""
+    import torch
+    d = _dist()
+    block = ((H + align - 1) // align + world - 1) // world * align
+    if d is None or world == 1:
+        return img[:H]
+    begin = min(rank * block, H)
+    if d.get_backend() == "nccl" and img.shape[0] >= world * block:
+        flat = img[:world * block]
+        d.all_gather_into_tensor(flat, flat[rank * block:(rank + 1) * block])
+        return img[:H]
+    send = torch.zeros((block,) + tuple(img.shape[1:]), dtype=img.dtype, device=img.device)
+    n = max(min(H, begin + block) - begin, 0)
+    if n:
+        send[:n] = img[begin:begin + n]
+    parts = [torch.empty_like(send) for _ in range(world)]
+    d.all_gather(parts, send)
+    full = torch.cat(parts, 0)
+    img[:H] = full[:H]
+    return img[:H]
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
 
@@ -322,7 +348,11 @@ def run_ours(args):
 
     scene, name = workload(args.config, args)
     cams_all = scene.cameras
-    mine = synth.shard_cameras(len(cams_all), rank, world) or [rank % len(cams_all)]
+    strips = args.parallel == "strips" and world > 1
+    if strips:
+        mine = list(range(len(cams_all)))                   # screen strips: every rank works on every frame
+    else:
+        mine = synth.shard_cameras(len(cams_all), rank, world) or [rank % len(cams_all)]
     cams = [cams_all[i] for i in mine]                      # frame-parallel replicas: no data-path collective
     path = {"auto": B.HYRF_MLP_AUTO, "fma": B.HYRF_MLP_FMA, "mma": B.HYRF_MLP_MMA, "hmma": B.HYRF_MLP_HMMA, "ws": B.HYRF_MLP_WS}[args.mlp]
     hs = B.HyrfScene(scene, device=dev, mlp_path=path)
@@ -348,6 +378,13 @@ def run_ours(args):
                   "explicit_bytes_compressed": q.nbytes(), "explicit_bytes_fp32": plain}
     W, H = cams[0].W, cams[0].H
     out = torch.empty((H, W, 3), dtype=torch.float32, device=f"cuda:{dev}")
+    if strips:
+        # S1-S4a replicated, S4b-S6 on this rank's strip of tile rows, then one all-gather of H/G x W x 3 floats; the
+        # image buffer holds G equal blocks of rows so that the gather is in place
+        y0, y1 = synth.strip_rows(H, rank, world)
+        block = ((H + 63) // 64 + world - 1) // world * 64
+        out = torch.empty((world * block, W, 3), dtype=torch.float32, device=f"cuda:{dev}")
+        hs.set_strip(y0, y1) if y1 > y0 else hs.set_strip(0, 16)     # (a rank beyond the image still joins the collective)
     cstructs = [B.camera_struct(c) for c in cams]
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{dev}")      # > 126 MB L2
     stream = torch.cuda.current_stream(dev)
@@ -355,6 +392,8 @@ def run_ours(args):
 
     def step(i):
         hs.render_struct(cstructs[i % len(cstructs)], W, H, out.data_ptr())
+        if strips:
+            gather_strips(out, H, rank, world)
 
     for i in range(Wm):
         step(i)
@@ -391,12 +430,12 @@ def run_ours(args):
     hs.set_timing(False)
     t_ms = sum(a.elapsed_time(b) for a, b in evs)
     t_max = max_over_ranks(t_ms)
-    frames_total = sum_over_ranks(K)
+    frames_total = float(K) if strips else sum_over_ranks(K)      # strips: the ranks share every frame (strong scaling)
     value = frames_total / (t_max * 1e-3)
     import numpy as np
     stage_ms = np.mean(np.array(stage), axis=0)
     Vm, Dm, Dmm = float(np.mean(Vs)), float(np.mean(Ds)), float(np.mean(Dms))
-    vis_per_s = sum_over_ranks(Vm * K) / (t_max * 1e-3)
+    vis_per_s = (Vm * K if strips else sum_over_ranks(Vm * K)) / (t_max * 1e-3)
     n_bg = float((hs.debug_fetch(B.DBG_FINAL_T) > scene.tau_T).sum())        # last frame's S6 work list length
 
     # --- warm-L2 figure (no flush), for context ---------------------------------------------------------------
@@ -446,24 +485,40 @@ def run_ours(args):
     # frame k overlaps the render of frame k+1 (two pinned host images, alternating); the clock stops after
     # hyrf_host_sync, when every image is in host memory. e2e_sync is the one-frame-at-a-time hyrf_render_host.
     host_imgs = [torch.empty((H, W, 3), dtype=torch.float32).pin_memory() for _ in range(2)]
-    for i in range(2):
-        hs.render_host(cams[i % len(cams)], out=host_imgs[0])
-    t0 = time.perf_counter()
-    for i in range(K):
-        hs.render_host(cams[i % len(cams)], out=host_imgs[0])
-    torch.cuda.synchronize()
-    e2e_sync = K / (time.perf_counter() - t0)
-    for i in range(2):
-        hs.render_host_async(cstructs[i % len(cstructs)], W, H, host_imgs[i & 1])
-    hs.host_sync()
-    if world > 1:
+    if strips:
+        # strips: a frame is complete after the all-gather; rank 0 then delivers it to pinned host memory
+        e2e_sync = None
+        for i in range(2):
+            step(i)
+        torch.cuda.synchronize()
         torch.distributed.barrier()
-    t0 = time.perf_counter()
-    for i in range(K):
-        hs.render_host_async(cstructs[i % len(cstructs)], W, H, host_imgs[i & 1])
-    hs.host_sync()
-    e2e_s = max_over_ranks(time.perf_counter() - t0)
-    e2e = frames_total / e2e_s
+        t0 = time.perf_counter()
+        for i in range(K):
+            step(i)
+            if rank == 0:
+                host_imgs[i & 1].copy_(out[:H], non_blocking=True)
+        torch.cuda.synchronize()
+        e2e_s = max_over_ranks(time.perf_counter() - t0)
+        e2e = frames_total / e2e_s
+    else:
+        for i in range(2):
+            hs.render_host(cams[i % len(cams)], out=host_imgs[0])
+        t0 = time.perf_counter()
+        for i in range(K):
+            hs.render_host(cams[i % len(cams)], out=host_imgs[0])
+        torch.cuda.synchronize()
+        e2e_sync = K / (time.perf_counter() - t0)
+        for i in range(2):
+            hs.render_host_async(cstructs[i % len(cstructs)], W, H, host_imgs[i & 1])
+        hs.host_sync()
+        if world > 1:
+            torch.distributed.barrier()
+        t0 = time.perf_counter()
+        for i in range(K):
+            hs.render_host_async(cstructs[i % len(cstructs)], W, H, host_imgs[i & 1])
+        hs.host_sync()
+        e2e_s = max_over_ranks(time.perf_counter() - t0)
+        e2e = frames_total / e2e_s
     # what the copies alone cost on this box: the same K images device -> pinned host, nothing else
     dimg = torch.empty((H, W, 3), dtype=torch.float32, device=f"cuda:{dev}")
     host_imgs[0].copy_(dimg, non_blocking=True)
@@ -548,17 +603,19 @@ def run_ours(args):
             roof["l1tex_gather"] = roof_l1
         per_stage["field"]["l1tex_gather"] = roof_l1
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
-            "ms_per_step": t_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": t_max / K, "higher_is_better": True, "scaling": "strong" if strips else "weak", "vs_baseline": None,
             "dtype": "f16" if scene.fp16 else "f32", "data": "synthetic",
             "config": {"workload": name, "l2": "flushed between steps (256 MiB write)", "mlp_path": args.mlp, "ablation": args.ablation, "raster": args.raster,
                        "schedule": "one frame at a time; S1 + depth sort on the library's second stream, the sort beside the field kernel (hyrf_set_sort_overlap default); e2e: frames pipelined (hyrf_render_host_async)",
-                       "parallelism": f"replicas x{world} (cameras round-robin)"},
+                       "parallelism": (f"screen strips x{world} (S1-S4a replicated, S4b-S6 per strip, one all-gather per frame)" if strips
+                                       else f"replicas x{world} (cameras round-robin)")},
             "visible_gaussians_per_s": vis_per_s, "V_mean": Vm, "D_mean": Dm, "Dm_mean": Dmm,
             "stage_ms": {n: float(stage_ms[i]) for i, n in enumerate(names)} | {"frame": float(stage_ms[5])},
             "serial_stage_ms": {n: float(stage_serial_ms[i]) for i, n in enumerate(names)} | {"frame": float(stage_serial_ms[5])},
             "warm_l2_ms_per_step": warm_ms, "pipelined_warm_l2_ms_per_step": pipe_ms,
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 64, "d2h_bytes_per_step": W * H * 12,
-                    "api": "hyrf_render_host_async + hyrf_host_sync", "sync_api_value": e2e_sync,
+                    "api": "hyrf_render (strip) + all-gather + copy to pinned host on rank 0" if strips else "hyrf_render_host_async + hyrf_host_sync",
+                    "sync_api_value": e2e_sync,
                     "d2h_copy_only_gbs": d2h_gbs, "d2h_copy_only_frames_per_s": d2h_gbs * 1e9 / (W * H * 12)},
             "gpu_launches": launches, "clocks": clocks, "roofline": roof, "stage_rooflines": per_stage}
     if cpu:
@@ -593,6 +650,9 @@ def main():
                     help="also time hyrf_raster_backward (backward of the alpha blend, NEXT-3 first piece) on camera 0's frame")
     ap.add_argument("--rvq", action="store_true",
                     help="compressed explicit Gaussians: binary16 positions + R-VQ codes decoded at upload (PAPER.md:229 (1)-(2))")
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "strips"],
+                    help="N > 1: frame-parallel replicas (default, no data-path collective) or screen strips with one "
+                         "all-gather per frame (SURVEY 8(e)(2); pays at the 4K / 4M points of config 5)")
     ap.add_argument("--probe", action="store_true",
                     help="run the L2 gather and issue-rate microprobes of SURVEY 8(d) instead of the render benchmark")
     ap.add_argument("--no-cpu", action="store_true")

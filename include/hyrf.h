@@ -236,6 +236,14 @@ hyrf_status hyrf_set_ablation(hyrf_scene* scene, uint32_t mask);
  * every debug export are identical either way. */
 hyrf_status hyrf_set_sort_overlap(hyrf_scene* scene, int on);
 
+/* Screen-strip parallelism over several devices: every device holds the whole scene and runs
+ * S1-S3 and the projection for the whole frame (a Gaussian's reach is known only after its fields have been queried),
+ * but bins, rasterises and composites only the pixel rows [row_begin, row_end) of out_rgb; the other rows of out_rgb are
+ * left untouched. row_begin must be a multiple of 16 (the tile size), row_end a multiple of 16 or >= H. The rows a
+ * device writes are bit-identical to the same rows of the whole-image render, so the strips of G devices, exchanged by
+ * ONE all-gather of H/G x W x 3 floats, are the single-device image. row_begin == row_end (default 0, 0): whole image. */
+hyrf_status hyrf_set_strip(hyrf_scene* scene, int32_t row_begin, int32_t row_end);
+
 /* Frame pipelining for a STREAM of hyrf_render calls (hyrf_render_host_async always works this way). S1 and the depth
  * sort of a frame depend on the camera and the explicit positions only and write library-owned, double-buffered
  * scratch, so with on != 0 they are enqueued on the library's own high-priority stream WITHOUT waiting for what the

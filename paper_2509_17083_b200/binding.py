@@ -29,7 +29,7 @@ EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_r
            "hyrf_destroy_scene", "hyrf_last_error", "hyrf_debug_enable", "hyrf_debug_fetch", "hyrf_set_timing",
            "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation", "hyrf_render_host_async",
            "hyrf_host_sync", "hyrf_set_sort_overlap", "hyrf_upload_explicit_rvq", "hyrf_last_decode_time", "hyrf_set_raster_mode",
-           "hyrf_last_raster_mode", "hyrf_raster_backward", "hyrf_probe_gather", "hyrf_probe_issue", "hyrf_set_pipelining", "hyrf_frame_gap"]
+           "hyrf_last_raster_mode", "hyrf_raster_backward", "hyrf_probe_gather", "hyrf_probe_issue", "hyrf_set_pipelining", "hyrf_frame_gap", "hyrf_set_strip"]
 ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
 
 
@@ -108,6 +108,7 @@ def load_library() -> C.CDLL:
         L.hyrf_set_sort_overlap.argtypes = [vp, C.c_int]
         L.hyrf_set_pipelining.argtypes = [vp, C.c_int]
         L.hyrf_frame_gap.argtypes = [vp, C.POINTER(C.c_float)]
+        L.hyrf_set_strip.argtypes = [vp, C.c_int32, C.c_int32]
         L.hyrf_render_host_async.argtypes = [vp, C.POINTER(CameraC), C.c_int32, C.c_int32, vp]
         L.hyrf_host_sync.argtypes = [vp]
         L.hyrf_upload_explicit_rvq.argtypes = [vp, C.POINTER(ExplicitRvqC)]
@@ -364,6 +365,10 @@ class HyrfScene:
     def set_sort_overlap(self, on: bool = True) -> None:
         """Depth sort beside the field query on a second stream (default) or the whole frame serialised (include/hyrf.h)."""
         _check(self.lib.hyrf_set_sort_overlap(self.handle, int(on)))   # (an int > 1: SMs left to the sort, include/hyrf.h)
+
+    def set_strip(self, row_begin: int = 0, row_end: int = 0) -> None:
+        """Screen strips over several devices (include/hyrf.h hyrf_set_strip); (0, 0) = the whole image."""
+        _check(self.lib.hyrf_set_strip(self.handle, int(row_begin), int(row_end)))
 
     def set_pipelining(self, on: bool = True) -> None:
         """A stream of hyrf_render calls: frame k+1's cull and depth sort beside frame k's rasterizer (include/hyrf.h)."""

@@ -542,6 +542,15 @@ hyrf_status build_frame(const hyrf_scene* s, const hyrf_camera* cam, int32_t W, 
     // small tile grids (<= 512 x 512 pixels) keep per-tile lists: with few tiles a macro tile's list is most of the scene
     f->mshift = (f->gx * f->gy <= 1024) ? 0 : HY_MACRO_SHIFT;
     f->mgx = (f->gx + (1 << f->mshift) - 1) >> f->mshift; f->mgy = (f->gy + (1 << f->mshift) - 1) >> f->mshift;
+    // screen strip (hyrf_set_strip): pixel rows [row0, row1) -> tile rows; the default is the whole image
+    f->ty0 = 0; f->ty1 = f->gy;
+    if (s->strip_row1 > s->strip_row0) {
+        if (s->strip_row0 % HY_TILE != 0 || (s->strip_row1 % HY_TILE != 0 && s->strip_row1 < H) || s->strip_row0 >= H)
+            return hy_fail(HYRF_ERR_INVALID_ARG, "strip rows [%d, %d) must start on a multiple of %d inside the image and end on one or at / beyond H = %d",
+                           s->strip_row0, s->strip_row1, HY_TILE, H);
+        f->ty0 = s->strip_row0 / HY_TILE;
+        f->ty1 = s->strip_row1 >= H ? f->gy : s->strip_row1 / HY_TILE;
+    }
     return HYRF_OK;
 }
 
@@ -828,6 +837,13 @@ extern "C" hyrf_status hyrf_set_sort_overlap(hyrf_scene* s, int on) {
     if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_sort_overlap: NULL scene");
     s->sort_overlap = on != 0;
     if (on > 1) s->ws_sort_sms = on < s->sm_count ? on : s->sm_count - 1;   // on > 1: SMs the warp-specialised field kernel leaves to the sort
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_set_strip(hyrf_scene* s, int32_t row_begin, int32_t row_end) {
+    if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_strip: NULL scene");
+    if (row_begin < 0 || row_end < row_begin) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_strip: rows [%d, %d)", row_begin, row_end);
+    s->strip_row0 = row_begin; s->strip_row1 = row_end;   // row_end == row_begin: the whole image again
     return HYRF_OK;
 }
 

@@ -35,6 +35,7 @@ struct FrameDev {
     int32_t mshift;     // binning granularity of this frame: macro tile = 2^mshift x 2^mshift tiles (0 on small grids)
     int32_t mgx, mgy;   // macro-tile grid
     uint32_t ablation;  // hyrf_ablation bits (include/hyrf.h)
+    int32_t ty0, ty1;   // tile rows [ty0, ty1) this device bins, rasterises and composites (hyrf_set_strip); 0, gy = the whole image
 };
 
 // D6 soft exponential: the one exp behind every sigmoid, so geometry decisions are bit-reproducible.

@@ -149,7 +149,9 @@ static __device__ __forceinline__ void aggregate_project(const FieldArgs& A, con
         const float fy0 = fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(v, radius), 0.0625f)), 0.0f), gy);
         const float fy1 = fminf(fmaxf(floorf(__fmul_rn(__fadd_rn(__fadd_rn(v, radius), 15.0f), 0.0625f)), 0.0f), gy);
         if (fx0 == fx0 && fx1 == fx1 && fy0 == fy0 && fy1 == fy1) {
-            rc = make_uint4((uint32_t)fx0, (uint32_t)fx1, (uint32_t)fy0, (uint32_t)fy1);
+            // (screen strips, hyrf_set_strip: only the tile rows of this device's strip are binned; a tile inside the strip
+            // sees exactly the rectangles it would see in the whole image)
+            rc = make_uint4((uint32_t)fx0, (uint32_t)fx1, max((uint32_t)fy0, (uint32_t)f.ty0), min((uint32_t)fy1, (uint32_t)f.ty1));
             if (rc.y > rc.x && rc.w > rc.z) nt = (rc.y - rc.x) * (rc.w - rc.z);
         }
     }

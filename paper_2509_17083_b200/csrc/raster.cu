@@ -19,7 +19,7 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
               int W, int H, int gx, float tau_T, float* __restrict__ out_rgb, float* __restrict__ finalT,
               uint32_t* __restrict__ bg_list, FrameCounters* __restrict__ counters, uint8_t* __restrict__ bg_mask,
               float* __restrict__ dbg_fg, const uint32_t* __restrict__ tile_queue, const uint4* __restrict__ rect,
-              int mshift, int mgx, uint32_t* __restrict__ dbg_list, const uint2* __restrict__ dbg_ranges) {
+              int mshift, int mgx, uint32_t* __restrict__ dbg_list, const uint2* __restrict__ dbg_ranges, int ty0, int ty1) {
     __shared__ float4 s_r0[2 * kBatch + 8];   // (u, v, A, B)   (+ 8: padding to a multiple of 8)
     __shared__ float4 s_r1[2 * kBatch + 8];   // (C, opacity, r, g)
     __shared__ float s_b[2 * kBatch + 8];
@@ -29,6 +29,7 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
     // tiles are taken longest list first (queue built by bin_ordered.cu), so the heavy tiles do not form the tail
     const int tile = tile_queue ? (int)tile_queue[blockIdx.x] : (int)blockIdx.x;
     const int tx = tile % gx, ty = tile / gx;
+    if (ty < ty0 || ty >= ty1) return;   // screen strips (hyrf_set_strip): another device's tile rows
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const int px = tx * HY_TILE + (threadIdx.x & (HY_TILE - 1));
     const int py = ty * HY_TILE + (threadIdx.x >> 4);
@@ -193,6 +194,6 @@ void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, con
     raster_kernel<<<grid, kBatch, 0, s->stream>>>(ranges, list, s->rec, f.W, f.H, f.gx, tau, out_rgb, s->finalT,
                                                   s->bg_list, s->counters, want_mask ? s->bg_mask : nullptr,
                                                   want_fg ? s->fg : nullptr, tile_queue, s->rect,
-                                                  macro ? f.mshift : 0, f.mgx, dbg_list, s->ranges);
+                                                  macro ? f.mshift : 0, f.mgx, dbg_list, s->ranges, f.ty0, f.ty1);
     ++*launches;
 }

@@ -39,7 +39,7 @@ raster_pair_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict_
                    int W, int H, int gx, float tau_T, float* __restrict__ out_rgb, float* __restrict__ finalT,
                    uint32_t* __restrict__ bg_list, FrameCounters* __restrict__ counters, uint8_t* __restrict__ bg_mask,
                    float* __restrict__ dbg_fg, const uint32_t* __restrict__ tile_queue, const uint4* __restrict__ rect,
-                   int mshift, int mgx, uint32_t* __restrict__ dbg_list, const uint2* __restrict__ dbg_ranges) {
+                   int mshift, int mgx, uint32_t* __restrict__ dbg_list, const uint2* __restrict__ dbg_ranges, int ty0, int ty1) {
     __shared__ __align__(16) uint8_t s_rec[(kStage + 1) * kRecBytes];
     __shared__ __align__(16) uint16_t s_widx[kWarps][kStage + 8];   // per warp: byte offsets of the records it blends
     __shared__ uint8_t s_mask[kStage];       // per staged record: bit w set when warp w's 8 x 8 block can reach it
@@ -47,6 +47,7 @@ raster_pair_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict_
     __shared__ uint32_t s_cnt[kWarps];
     const int tile = tile_queue ? (int)tile_queue[blockIdx.x] : (int)blockIdx.x;
     const int tx = tile % gx, ty = tile / gx;
+    if (ty < ty0 || ty >= ty1) return;   // screen strips (hyrf_set_strip): another device's tile rows
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const int px = tx * HY_TILE + (int)(warp & 1u) * 8 + (int)(lane & 7u);
     const int py0 = ty * HY_TILE + (int)(warp >> 1) * 8 + (int)(lane >> 3), py1 = py0 + 4;
@@ -231,6 +232,6 @@ void hy_launch_raster_pair(hyrf_scene* s, const FrameDev& f, const uint2* ranges
     raster_pair_kernel<<<grid, kThreads, 0, s->stream>>>(ranges, list, s->rec, f.W, f.H, f.gx, tau, out_rgb, s->finalT,
                                                          s->bg_list, s->counters, want_mask ? s->bg_mask : nullptr,
                                                          want_fg ? s->fg : nullptr, tile_queue, s->rect,
-                                                         macro ? f.mshift : 0, f.mgx, dbg_list, s->ranges);
+                                                         macro ? f.mshift : 0, f.mgx, dbg_list, s->ranges, f.ty0, f.ty1);
     ++*launches;
 }

@@ -124,6 +124,8 @@ struct hyrf_scene {
     uint8_t* bg_mask = nullptr;
     uint32_t* bg_list = nullptr;  // [H*W] pixels S6 has to shade, appended by the rasterizer
 
+    int32_t strip_row0 = 0, strip_row1 = 0;   // hyrf_set_strip: pixel rows this device renders (equal: the whole image)
+
     // debug / measurement
     uint32_t ablation = 0;            // hyrf_ablation bits
     int raster_mode = 0;              // hyrf_set_raster_mode: 0 auto, 1 tile-level lists only, 2 per-warp lists

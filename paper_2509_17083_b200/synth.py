@@ -409,3 +409,14 @@ def morton_sorted(scene: Scene) -> Scene:
 def shard_cameras(n_cameras: int, rank: int, world: int) -> List[int]:
     """Frame-parallel replicas: cameras dealt round-robin, no collective on the data path."""
     return list(range(rank, n_cameras, world))
+
+
+def strip_rows(H: int, rank: int, world: int, align: int = 64):
+    """Screen-strip parallelism: pixel rows [begin, end) of rank `rank` of `world`. Strips are equal
+    multiples of `align` rows (64 = one macro tile of 4 x 4 tiles, so that no macro-tile list is binned twice), the
+    last one takes what is left; a rank beyond the image gets an empty strip (begin == end == H)."""
+    units = (H + align - 1) // align
+    per = (units + world - 1) // world
+    begin = min(rank * per * align, H)
+    end = min((rank + 1) * per * align, H)
+    return begin, end

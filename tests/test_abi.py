@@ -109,6 +109,41 @@ def test_camera_sharding_world2_gloo(tmp_path):
     assert r.returncode == 0, r.stdout + r.stderr
 
 
+def test_screen_strips_world2_gloo(tmp_path):
+    """NEXT-4: screen strips. Each of 2 gloo ranks holds only ITS strip of rows of the oracle's image
+    (what hyrf_set_strip leaves in out_rgb on a device); after bench.gather_strips every rank must hold the whole image
+    bit for bit. Also the partition itself: strips tile the image, are multiples of 64 rows, the last takes the rest."""
+    script = tmp_path / "s.py"
+    script.write_text(
+        "import os, sys, numpy as np, torch, torch.distributed as dist\n"
+        f"sys.path.insert(0, {ROOT!r})\n"
+        "from paper_2509_17083_b200 import synth\n"
+        "from oracle import hyrf_oracle as ho\n"
+        "import bench\n"
+        "dist.init_process_group('gloo')\n"
+        "r, w = dist.get_rank(), dist.get_world_size()\n"
+        "for H in (720, 64, 100, 2160, 1):\n"
+        "    for world in (1, 2, 3, 8):\n"
+        "        rows = [synth.strip_rows(H, k, world) for k in range(world)]\n"
+        "        assert rows[0][0] == 0 and rows[-1][1] == H and all(a[1] == b[0] for a, b in zip(rows, rows[1:])), rows\n"
+        "        assert all(a % 64 == 0 for a, _ in rows if a < H)\n"
+        "s = synth.make_scene(3, n_gaussians=3000, width=96, height=200, n_cameras=1)\n"
+        "img = torch.from_numpy(ho.render(ho.OracleScene(s), s.cameras[0])['out'].copy())\n"
+        "H = img.shape[0]\n"
+        "y0, y1 = synth.strip_rows(H, r, w)\n"
+        "assert (y0, y1) == ((0, 128), (128, 200))[r]\n"
+        "mine = torch.full_like(img, float('nan'))\n"
+        "mine[y0:y1] = img[y0:y1]\n"
+        "got = bench.gather_strips(mine, H, r, w)\n"
+        "assert got.shape == img.shape and torch.equal(got.view(torch.int32), img.view(torch.int32))\n"
+        "dist.destroy_process_group()\n")
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29514")
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+                        "--master-addr", "127.0.0.1", "--master-port", "29514", str(script)],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stdout + r.stderr
+
+
 def test_explicit_rvq_argument_validation_without_device(lib):
     from paper_2509_17083_b200 import binding as B
     q = B.ExplicitRvqC()

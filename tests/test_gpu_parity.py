@@ -767,3 +767,40 @@ def test_list_export_beyond_initial_capacity_stays_in_bounds(B, ho, synth):
         hs.close()
         torch.cuda.synchronize()
         assert not ga.live
+
+
+def test_screen_strips_equal_the_whole_image(B, synth):
+    # a device bins, rasterises and composites only its strip of tile rows; the rows it writes
+    # must be the same bits as in the whole-image render, for macro-tile lists (1280x720, ragged last tile row at 720 =
+    # 45 tiles) and per-tile lists (<= 1024 tiles), on the exact and the tensor-core path, for 2, 3 and 5 strips (5 strips
+    # of 720 rows: the last rank's strip is empty); rows outside a strip stay untouched
+    import torch
+    for (n, W, H, path) in ((150_000, 1280, 720, B.HYRF_MLP_AUTO), (40_000, 400, 300, B.HYRF_MLP_FMA)):
+        s = synth.make_scene(3, n_gaussians=n, width=W, height=H, n_cameras=2)
+        hs = B.HyrfScene(s, mlp_path=path)
+        for cam in s.cameras:
+            full = hs.render(cam).clone()
+            torch.cuda.synchronize()
+            for world in (2, 3, 5):
+                got = torch.full((H, W, 3), -7.0, device="cuda")
+                covered = 0
+                for rank in range(world):
+                    y0, y1 = synth.strip_rows(H, rank, world)
+                    if y0 == y1:
+                        continue
+                    hs.set_strip(y0, y1)
+                    part = torch.full((H, W, 3), -7.0, device="cuda")
+                    hs.render(cam, out=part)
+                    torch.cuda.synchronize()
+                    assert (part[:y0] == -7.0).all() and (part[y1:] == -7.0).all()      # other devices' rows untouched
+                    got[y0:y1] = part[y0:y1]
+                    covered += y1 - y0
+                assert covered == H
+                assert torch.equal(got, full), f"strips of {world} differ from the whole image"
+            hs.set_strip(0, 0)
+            assert torch.equal(hs.render(cam), full)
+        with pytest.raises(B.HyrfError) as e:
+            hs.set_strip(8, 64)
+            hs.render(s.cameras[0])
+        assert e.value.status == B.HYRF_ERR_INVALID_ARG
+        hs.close()
