@@ -293,6 +293,33 @@ hyrf_status hyrf_probe_gather(int32_t device, uint64_t table_bytes, uint32_t ent
 hyrf_status hyrf_probe_issue(int32_t device, uint32_t kind, uint32_t ctas_per_sm, uint32_t iters,
                              double* warp_instr_per_s, float* ms);
 
+/* The whole backward pass for the LAST rendered frame (§3.4; arithmetic DESIGN.md §2 D13): given
+ * g_out = dL/d out_rgb (DEVICE float [H][W][3]), the gradients of L with respect to every parameter of the scene, with
+ * the forward's decisions frozen: S6 (background composite, Eq. 10-11) -> S5 (alpha blend, hyrf_raster_backward's
+ * kernel) -> S4a (EWA projection) -> S3 (Eq. 7) -> S2 (decoders Eq. 4, 6; direction encoding Eq. 5; grid encodes Eq. 3;
+ * contraction Eq. 2). Every pointer of hyrf_grads is a DEVICE float array shaped like the parameter it belongs to
+ * (tables and weights in fp32 whatever the scene's param_dtype; 8-bit tables: gradient with respect to the decoded
+ * values), or NULL when that gradient is not wanted. Gradients are ADDED to what the arrays hold (the caller zeroes
+ * them, or accumulates several cameras). Enqueued on the scene's stream; the caller synchronises. Like
+ * hyrf_raster_backward it needs the frame rendered with HYRF_DBG_TILE_LIST | HYRF_DBG_TILE_RANGES enabled, else
+ * HYRF_ERR_NOT_READY. Sums use fp32 atomics: reproducible to rounding, not bit for bit. */
+typedef struct {
+    float* pos;           /* [3][N] */
+    float* rgb_logit;     /* [3][N] */
+    float* scale_logit;   /* [N] */
+    float* opacity_logit; /* [N] */
+    float *geo_table, *app_table, *bg_table; /* [entries][2] */
+    float *geo_w, *app_w, *bg_w;             /* layers concatenated, row-major [out][in] */
+} hyrf_grads;
+hyrf_status hyrf_backward(hyrf_scene* scene, const float* g_out, const hyrf_grads* grads);
+
+/* The training loss of PAPER.md:138-140 Eq. 12 (reading A28): L = (1 - lambda) mean|image - target| +
+ * lambda (1 - SSIM(image, target)), SSIM with an 11 x 11 Gaussian window (sigma 1.5), zero padding, C1 = 0.01^2,
+ * C2 = 0.03^2. image, target: DEVICE float [H][W][3]; *loss_host receives L; g_image (DEVICE float [H][W][3], may be
+ * NULL) receives dL/d image — what hyrf_backward takes as g_out. Synchronises the scene's stream. */
+hyrf_status hyrf_loss_l1_ssim(hyrf_scene* scene, const float* image, const float* target, int32_t W, int32_t H,
+                              float lambda, double* loss_host, float* g_image);
+
 /* Number of kernels the last render launched (for bench.py's gpu_launches). */
 hyrf_status hyrf_last_launch_count(hyrf_scene* scene, uint32_t* launches);
 

@@ -83,15 +83,25 @@ def contract(p: torch.Tensor, amin, amax) -> torch.Tensor:
 
 
 # ---------------------------------------------------------------------------------------------- D3 grid encode
-def grid_encode(grid, table: torch.Tensor, x: torch.Tensor) -> torch.Tensor:
+def cells_fp32(grid, x32: np.ndarray):
+    """The cells the binary32 forward pass picks (D3: u = x N in binary32, i = min(floor(u), N - 1)), per level (V, 3)."""
+    out = []
+    for N in grid.level_res:
+        u = (x32.astype(np.float32) * np.float32(N)).astype(np.float32)
+        out.append(torch.from_numpy(np.minimum(np.floor(u), N - 1).astype(np.int64)))
+    return out
+
+
+def grid_encode(grid, table: torch.Tensor, x: torch.Tensor, cells=None) -> torch.Tensor:
     """x (V, 3) -> features (V, 2 L), level-major [l][f] (Eq. 3; layout and hash of DESIGN.md §2 D3). The cell
-    (integer part) is a frozen decision; the weights are differentiable in x, the values in the table."""
+    (integer part) is a frozen decision — `cells` (from cells_fp32) when given, else taken from x itself; the weights
+    are differentiable in x, the values in the table."""
     _, sizes, offs, dense = ho.grid_layout(grid)
     T = 1 << grid.log2_table
     feats = []
     for l, N in enumerate(grid.level_res):
         u = x * float(N)
-        i = torch.clamp(torch.floor(u.detach()), max=float(N - 1)).to(torch.int64)       # (V, 3)
+        i = cells[l] if cells is not None else torch.clamp(torch.floor(u.detach()), max=float(N - 1)).to(torch.int64)       # (V, 3)
         w = u - i.to(F64)
         acc = torch.zeros((x.shape[0], 2), dtype=F64)
         for k in range(8):
@@ -118,9 +128,28 @@ def dir_pe(d: torch.Tensor, octaves: int) -> torch.Tensor:
 
 
 # ---------------------------------------------------------------------------------------------- D5 MLP
-def mlp(spec, w: torch.Tensor, x: torch.Tensor) -> torch.Tensor:
+def relu_masks_fp32(spec, w32: np.ndarray, x32: np.ndarray, fp16: bool):
+    """Which hidden units the binary32 forward pass (hyrf_oracle.c ho_mlp_forward, D5's fma order) leaves on: one (V, hidden)
+    0 / 1 array per hidden layer. Hidden layer l is read out through a decoder truncated after it whose output layer
+    is the identity (fma with 1 and 0 is exact)."""
+    import types
+    V = x32.shape[0]
+    dims = [spec.in_dim] + [spec.hidden] * spec.n_hidden
+    masks, off = [], 0
+    eye = np.eye(spec.hidden, dtype=np.float32).ravel()
+    for l in range(spec.n_hidden):
+        off += dims[l + 1] * dims[l]
+        sub = types.SimpleNamespace(in_dim=spec.in_dim, hidden=spec.hidden, n_hidden=l + 1, out_dim=spec.hidden)
+        wl = np.concatenate([np.asarray(w32[:off], np.float32), eye])
+        h = np.stack([ho.mlp_forward(sub, wl, x32[v], fp16) for v in range(V)]) if V else np.zeros((0, spec.hidden), np.float32)
+        masks.append(torch.from_numpy((h > 0).astype(np.float64)))
+    return masks
+
+
+def mlp(spec, w: torch.Tensor, x: torch.Tensor, masks=None) -> torch.Tensor:
     """in -> hidden x n_hidden (ReLU) -> out (linear), no biases; weights flat, layers concatenated, row-major [out][in]
-    (Eq. 4, 6; reading A11). x is zero-padded to in_dim."""
+    (Eq. 4, 6; reading A11). x is zero-padded to in_dim. `masks` (from relu_masks_fp32): the ReLU decisions
+    of the binary32 forward pass, frozen; else the float64 values decide."""
     if x.shape[1] < spec.in_dim:
         x = torch.cat([x, torch.zeros((x.shape[0], spec.in_dim - x.shape[1]), dtype=F64)], dim=1)
     dims = [spec.in_dim] + [spec.hidden] * spec.n_hidden + [spec.out_dim]
@@ -132,7 +161,7 @@ def mlp(spec, w: torch.Tensor, x: torch.Tensor) -> torch.Tensor:
         off += o * i
         h = h @ W.T
         if li < len(dims) - 2:
-            h = torch.relu(h)
+            h = h * masks[li] if masks is not None else torch.relu(h)
     return h
 
 
@@ -179,8 +208,10 @@ def project(attrs: torch.Tensor, p: torch.Tensor, cam) -> torch.Tensor:
     return torch.stack([u, v, A, B, C, attrs[:, 7], attrs[:, 8], attrs[:, 9], attrs[:, 10]], -1)
 
 
-def fields_forward(P: Params, cam, vis_idx: np.ndarray, ablation: int = 0):
-    """Stages S2-S4a for the visible Gaussians in float64: returns (raw (V, 11), attrs (V, 11), rec (V, 9))."""
+def fields_forward(P: Params, cam, vis_idx: np.ndarray, ablation: int = 0, frozen: bool = False):
+    """Stages S2-S4a for the visible Gaussians in float64: returns (raw (V, 11), attrs (V, 11), rec (V, 9)). frozen: the
+    grid cells and ReLU masks are those of the binary32 forward pass (what the backward pass differentiates around);
+    otherwise the float64 values decide (the two differ for a Gaussian in a few thousand)."""
     sc = P.scene
     idx = torch.from_numpy(np.asarray(vis_idx, np.int64))
     p = P.pos[:, idx].T                                              # (V, 3)
@@ -188,13 +219,27 @@ def fields_forward(P: Params, cam, vis_idx: np.ndarray, ablation: int = 0):
     if ablation & ho.ABL_NO_NEURAL:
         raw = torch.zeros((len(idx), 11), dtype=F64)
     else:
-        f_geo = grid_encode(sc.geo_grid, P.geo_table, x)
-        f_app = grid_encode(sc.app_grid, P.app_table, x)
+        cg = ca = mg = ma = None
+        if frozen:
+            # the decisions of the binary32 forward pass: cells of every level, ReLU masks of both decoders
+            fp16 = bool(sc.fp16)
+            pos32 = np.asarray(sc.pos, np.float32)[:, np.asarray(vis_idx, np.int64)].T
+            x32 = np.stack([ho.contract(q, sc.aabb_min, sc.aabb_max) for q in pos32]) if len(pos32) else np.zeros((0, 3), np.float32)
+            cg, ca = cells_fp32(sc.geo_grid, x32), cells_fp32(sc.app_grid, x32)
+            o32 = ho.camera_center(cam)
+            fg = np.stack([ho.grid_encode(sc.geo_grid, sc.geo_table, q, fp16) for q in x32])
+            fa = np.stack([np.concatenate([ho.grid_encode(sc.app_grid, sc.app_table, q, fp16),
+                                           ho.dir_pe(ho.view_dir(pp, o32), sc.dir_pe_octaves, fp16)]) for q, pp in zip(x32, pos32)])
+            pad = lambda a, n: np.concatenate([a, np.zeros((a.shape[0], n - a.shape[1]), np.float32)], 1) if a.shape[1] < n else a
+            mg = relu_masks_fp32(sc.geo_mlp, np.asarray(sc.geo_w, np.float32), pad(fg, sc.geo_mlp.in_dim), fp16)
+            ma = relu_masks_fp32(sc.app_mlp, np.asarray(sc.app_w, np.float32), pad(fa, sc.app_mlp.in_dim), fp16)
+        f_geo = grid_encode(sc.geo_grid, P.geo_table, x, cg)
+        f_app = grid_encode(sc.app_grid, P.app_table, x, ca)
         o = _t(ho.camera_center(cam))
         delta = p - o
         d = delta / torch.sqrt((delta * delta).sum(-1, keepdim=True))
-        raw = torch.cat([mlp(sc.geo_mlp, P.geo_w, f_geo),
-                         mlp(sc.app_mlp, P.app_w, torch.cat([f_app, dir_pe(d, sc.dir_pe_octaves)], dim=1))], dim=1)
+        raw = torch.cat([mlp(sc.geo_mlp, P.geo_w, f_geo, mg),
+                         mlp(sc.app_mlp, P.app_w, torch.cat([f_app, dir_pe(d, sc.dir_pe_octaves)], dim=1), ma)], dim=1)
     if ablation & ho.ABL_NO_EXPLICIT:
         z = torch.zeros(len(idx), dtype=F64)
         attrs = aggregate(raw, z, z, torch.zeros((len(idx), 3), dtype=F64))
@@ -204,7 +249,7 @@ def fields_forward(P: Params, cam, vis_idx: np.ndarray, ablation: int = 0):
 
 
 # ---------------------------------------------------------------------------------------------- D11 background
-def background_colors(P: Params, cam, pix: np.ndarray) -> torch.Tensor:
+def background_colors(P: Params, cam, pix: np.ndarray, frozen: bool = False) -> torch.Tensor:
     """c_s (n, 3) for the pixels pix (n, 2) = (i, j) (PAPER.md:124-134 Eq. 10-11, :360-378 Eq. 15-18; D11)."""
     sc = P.scene
     R = _t(np.asarray(cam.R, np.float32).reshape(3, 3))
@@ -219,8 +264,19 @@ def background_colors(P: Params, cam, pix: np.ndarray) -> torch.Tensor:
     tt = 0.5 * (-Bq + torch.sqrt(Bq * Bq - 4.0 * Cq))
     ps = o + tt[:, None] * d
     x = contract(ps, sc.aabb_min, sc.aabb_max)
-    f = grid_encode(sc.bg_grid, P.bg_table, x)
-    return torch.sigmoid(mlp(sc.bg_mlp, P.bg_w, torch.cat([f, dir_pe(d, sc.dir_pe_octaves)], dim=1)))
+    cells = masks = None
+    if frozen and len(pix):
+        fp16 = bool(sc.fp16)
+        rays = [ho.ray_sphere(cam, float(i), float(j), float(sc.bg_radius)) for i, j in pix]
+        x32 = np.stack([ho.contract(ps32, sc.aabb_min, sc.aabb_max) for _, ps32 in rays])
+        cells = cells_fp32(sc.bg_grid, x32)
+        fin = np.stack([np.concatenate([ho.grid_encode(sc.bg_grid, sc.bg_table, q, fp16), ho.dir_pe(d32, sc.dir_pe_octaves, fp16)])
+                        for q, (d32, _) in zip(x32, rays)])
+        if fin.shape[1] < sc.bg_mlp.in_dim:
+            fin = np.concatenate([fin, np.zeros((fin.shape[0], sc.bg_mlp.in_dim - fin.shape[1]), np.float32)], 1)
+        masks = relu_masks_fp32(sc.bg_mlp, np.asarray(sc.bg_w, np.float32), fin, fp16)
+    f = grid_encode(sc.bg_grid, P.bg_table, x, cells)
+    return torch.sigmoid(mlp(sc.bg_mlp, P.bg_w, torch.cat([f, dir_pe(d, sc.dir_pe_octaves)], dim=1), masks))
 
 
 # ---------------------------------------------------------------------------------------------- Eq. 12 loss
@@ -277,7 +333,7 @@ def backward_from_image_grad(scene, cam, g_out: np.ndarray, ablation: int = 0, f
     scalar = torch.zeros((), dtype=F64)
     if mask.any():
         jj, ii = np.nonzero(mask)
-        cs = background_colors(P, cam, np.stack([ii, jj], -1).astype(np.float64))
+        cs = background_colors(P, cam, np.stack([ii, jj], -1).astype(np.float64), frozen=True)
         Tm = _t(fwd["T"][mask])
         g_sel = g_out_t[torch.from_numpy(jj), torch.from_numpy(ii)]
         g_T[mask] = (g_sel * cs.detach()).sum(-1).numpy()
@@ -288,7 +344,7 @@ def backward_from_image_grad(scene, cam, g_out: np.ndarray, ablation: int = 0, f
                                      np.asarray(g_out, np.float32).reshape(H, W, 3), g_T.astype(np.float32)) if V else np.zeros((0, 9))
     # ---- S4a .. S2
     if V:
-        _, _, rec = fields_forward(P, cam, fwd["vis_idx"], ablation)
+        _, _, rec = fields_forward(P, cam, fwd["vis_idx"], ablation, frozen=True)
         live = torch.from_numpy((fwd["tiles"] > 0).astype(np.float64))[:, None]      # dropped Gaussians are in no list
         scalar = scalar + (rec * _t(g_rec) * live).sum()
     grads = {k: np.zeros(tuple(v.shape)) for k, v in P.leaves().items()}

@@ -29,7 +29,7 @@ EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_r
            "hyrf_destroy_scene", "hyrf_last_error", "hyrf_debug_enable", "hyrf_debug_fetch", "hyrf_set_timing",
            "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation", "hyrf_render_host_async",
            "hyrf_host_sync", "hyrf_set_sort_overlap", "hyrf_upload_explicit_rvq", "hyrf_last_decode_time", "hyrf_set_raster_mode",
-           "hyrf_last_raster_mode", "hyrf_raster_backward", "hyrf_probe_gather", "hyrf_probe_issue", "hyrf_set_pipelining", "hyrf_frame_gap", "hyrf_set_strip"]
+           "hyrf_last_raster_mode", "hyrf_raster_backward", "hyrf_probe_gather", "hyrf_probe_issue", "hyrf_set_pipelining", "hyrf_frame_gap", "hyrf_set_strip", "hyrf_backward", "hyrf_loss_l1_ssim"]
 ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
 
 
@@ -67,6 +67,11 @@ class Params(C.Structure):
 class ExplicitRvqC(C.Structure):
     _fields_ = [("pos_h", C.c_void_p), ("stages", C.c_uint32), ("codebook_size", C.c_uint32), ("codes", C.c_void_p),
                 ("codebooks", C.c_void_p), ("host_ptrs", C.c_int32)]
+
+
+class GradsC(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("pos", "rgb_logit", "scale_logit", "opacity_logit", "geo_table", "app_table",
+                                          "bg_table", "geo_w", "app_w", "bg_w")]
 
 
 class CameraC(C.Structure):
@@ -109,6 +114,8 @@ def load_library() -> C.CDLL:
         L.hyrf_set_pipelining.argtypes = [vp, C.c_int]
         L.hyrf_frame_gap.argtypes = [vp, C.POINTER(C.c_float)]
         L.hyrf_set_strip.argtypes = [vp, C.c_int32, C.c_int32]
+        L.hyrf_backward.argtypes = [vp, vp, C.POINTER(GradsC)]
+        L.hyrf_loss_l1_ssim.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, C.c_float, C.POINTER(C.c_double), vp]
         L.hyrf_render_host_async.argtypes = [vp, C.POINTER(CameraC), C.c_int32, C.c_int32, vp]
         L.hyrf_host_sync.argtypes = [vp]
         L.hyrf_upload_explicit_rvq.argtypes = [vp, C.POINTER(ExplicitRvqC)]
@@ -229,6 +236,11 @@ class HyrfScene:
         _check(self.lib.hyrf_create_scene(C.byref(self.desc), C.byref(self.handle)))
         self.fp16 = bool(scene.fp16)
         self.n = int(scene.n)
+        n_w = lambda m: sum(o * i for o, i in m.layer_shapes())
+        self._scene_shapes = dict(pos=(3, self.n), rgb_logit=(3, self.n), scale_logit=(self.n,), opacity_logit=(self.n,),
+                                  geo_table=(scene.geo_grid.n_entries(), 2), app_table=(scene.app_grid.n_entries(), 2),
+                                  bg_table=(scene.bg_grid.n_entries(), 2), geo_w=(n_w(scene.geo_mlp),),
+                                  app_w=(n_w(scene.app_mlp),), bg_w=(n_w(scene.bg_mlp),))
         self.upload(scene, host_upload)
 
     # -- hyrf_upload_params -------------------------------------------------------------------------------
@@ -386,6 +398,33 @@ class HyrfScene:
         _check(self.lib.hyrf_raster_backward(self.handle, C.c_void_p(g_cfg.data_ptr()), C.c_void_p(g_T.data_ptr()),
                                              C.c_void_p(grad.data_ptr())))
         return grad
+
+    def backward(self, g_out, grads: Optional[Dict] = None, want=None) -> Dict:
+        """hyrf_backward: g_out (H, W, 3) float32 CUDA tensor = dL/d out of the last rendered frame -> dict of float32 CUDA
+        tensors shaped like the parameters (gradients are ADDED into `grads` when given, else into fresh zeros).
+        `want`: names to compute (default all)."""
+        torch = self._torch
+        sc = self._scene_shapes
+        names = list(sc) if want is None else list(want)
+        if grads is None:
+            grads = {k: torch.zeros(sc[k], dtype=torch.float32, device=f"cuda:{self.device}") for k in names}
+        g = GradsC()
+        for k in names:
+            setattr(g, k, grads[k].data_ptr())
+        g_out = g_out.contiguous()
+        _check(self.lib.hyrf_backward(self.handle, C.c_void_p(g_out.data_ptr()), C.byref(g)))
+        return grads
+
+    def loss_l1_ssim(self, image, target, lam: float = 0.2, want_grad: bool = True):
+        """hyrf_loss_l1_ssim (Eq. 12): (H, W, 3) float32 CUDA tensors -> (L, dL/d image or None)."""
+        torch = self._torch
+        image, target = image.contiguous(), target.contiguous()
+        H, W = int(image.shape[0]), int(image.shape[1])
+        g = torch.empty_like(image) if want_grad else None
+        loss = C.c_double(0)
+        _check(self.lib.hyrf_loss_l1_ssim(self.handle, C.c_void_p(image.data_ptr()), C.c_void_p(target.data_ptr()), W, H,
+                                          C.c_float(lam), C.byref(loss), C.c_void_p(g.data_ptr() if want_grad else None)))
+        return float(loss.value), g
 
     def last_raster_mode(self) -> int:
         m = C.c_int(0)

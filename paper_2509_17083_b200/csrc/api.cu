@@ -170,7 +170,7 @@ void destroy(hyrf_scene* s) {
                     (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w, s->both_table,
                     s->gm, s->gm_id, s->rec, s->rect, s->tiles, s->mtiles, s->mranges, s->tt_sorted, s->offs,
                     s->scan_scratch, s->ranges, s->tile_queue, s->fg, s->finalT, s->image, s->image2, s->bg_mask, s->bg_list,
-                    s->dbg_raw, s->dbg_attrs};
+                    s->dbg_raw, s->dbg_attrs, s->bwd_gT, s->bwd_grec, s->bwd_ssim};
     for (void* p : ptrs) dev_free(s, p);
     if (s->sort_stream) cudaStreamSynchronize(s->sort_stream);
     for (auto& P : s->pre) {   // (the scene's members of the same names are aliases of one of the two sets)
@@ -733,6 +733,7 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     if ((e = cudaEventRecord(s->ev_frame_done, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(frame done)");
     s->frame_in_flight = true;
     s->last_launches = launches;
+    s->last_frame = f;
     s->lastV = V; s->lastD = D; s->lastDm = s->counters_host->Dm;
     s->rendered = true;
     return HYRF_OK;

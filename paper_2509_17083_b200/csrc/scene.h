@@ -124,6 +124,11 @@ struct hyrf_scene {
     uint8_t* bg_mask = nullptr;
     uint32_t* bg_list = nullptr;  // [H*W] pixels S6 has to shade, appended by the rasterizer
 
+    FrameDev last_frame{};            // camera and frame constants of the last render (hyrf_backward)
+    float* bwd_gT = nullptr;          // backward scratch: dL/dT [H][W], dL/d(projected record) [V][9], SSIM maps
+    float* bwd_grec = nullptr;
+    float* bwd_ssim = nullptr;
+    uint32_t last_backward_launches = 0;
     int32_t strip_row0 = 0, strip_row1 = 0;   // hyrf_set_strip: pixel rows this device renders (equal: the whole image)
 
     // debug / measurement

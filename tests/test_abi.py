@@ -21,7 +21,7 @@ def lib():
 def test_every_declared_symbol_is_exported(lib):
     from paper_2509_17083_b200 import binding
     hdr = open(os.path.join(ROOT, "include", "hyrf.h")).read()
-    declared = set(re.findall(r"\b(hyrf_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(hyrf_[a-z0-9_]+)\s*\(", hdr))
     assert declared == set(binding.EXPORTS), declared ^ set(binding.EXPORTS)
     for name in declared:
         assert hasattr(lib, name), name
@@ -30,15 +30,16 @@ def test_every_declared_symbol_is_exported(lib):
 def test_struct_layouts_match_header_sizes():
     # sizes computed by the C compiler from the header itself
     from paper_2509_17083_b200 import binding
-    src = ('#include "hyrf.h"\n#include <stdio.h>\nint main(){printf("%zu %zu %zu %zu %zu %zu\\n", '
+    src = ('#include "hyrf.h"\n#include <stdio.h>\nint main(){printf("%zu %zu %zu %zu %zu %zu ", '
            'sizeof(hyrf_scene_desc), sizeof(hyrf_params), sizeof(hyrf_camera), sizeof(hyrf_grid_desc), '
-           'sizeof(hyrf_mlp_desc), sizeof(hyrf_explicit_rvq));return 0;}')
+           'sizeof(hyrf_mlp_desc), sizeof(hyrf_explicit_rvq));printf("%zu\\n", sizeof(hyrf_grads));return 0;}')
     exe = "/tmp/hyrf_sizes"
     subprocess.run(["gcc", "-x", "c", "-I", os.path.join(ROOT, "include"), "-o", exe, "-"], input=src.encode(),
                    check=True)
     sizes = [int(x) for x in subprocess.run([exe], capture_output=True, check=True).stdout.split()]
     assert sizes == [C.sizeof(binding.SceneDesc), C.sizeof(binding.Params), C.sizeof(binding.CameraC),
-                     C.sizeof(binding.GridDesc), C.sizeof(binding.MlpDesc), C.sizeof(binding.ExplicitRvqC)]
+                     C.sizeof(binding.GridDesc), C.sizeof(binding.MlpDesc), C.sizeof(binding.ExplicitRvqC),
+                     C.sizeof(binding.GradsC)]
 
 
 def test_argument_validation_without_device(lib, synth):

@@ -804,3 +804,57 @@ def test_screen_strips_equal_the_whole_image(B, synth):
             hs.render(s.cameras[0])
         assert e.value.status == B.HYRF_ERR_INVALID_ARG
         hs.close()
+
+
+def _grad_close(got, want, name, rel=2e-2, floor=2e-3):
+    # binary32 sums in atomic order against float64: every entry within `floor` of the array's largest magnitude plus
+    # `rel` of its own value
+    scale = np.abs(want).max()
+    err = np.abs(got - want)
+    assert np.isfinite(got).all(), name
+    assert (err <= floor * scale + rel * np.abs(want)).all(), (name, float(err.max()), float(scale))
+
+
+@pytest.mark.parametrize("case", ["tiny", "tiny_fp16", "cfg2_scaled", "cfg3_scaled"])
+def test_backward_against_oracle(B, ho, synth, case):
+    # hyrf_loss_l1_ssim + hyrf_backward (DESIGN.md §2 D13) against oracle/hyrf_oracle_backward.py:
+    # the loss value and dL/d image, then every parameter gradient of one camera's training step. Exact decoders, so the
+    # frozen decisions (lists, blended prefixes, background mask) coincide with the oracle's binary32 forward.
+    import torch
+    from oracle import hyrf_oracle_backward as hb
+    if case == "tiny":
+        s = synth.tiny_scene(n=48, W=32, H=32, table_amp=1.0)
+    elif case == "tiny_fp16":
+        s = synth.tiny_scene(n=64, W=45, H=37, seed=9, fp16=True, table_amp=1.0)
+    elif case == "cfg2_scaled":
+        s = synth.make_scene(2, n_gaussians=3000, width=96, height=80, n_cameras=1, table_amp=0.5)
+    else:
+        s = synth.make_scene(3, n_gaussians=20_000, width=160, height=96, n_cameras=1, table_amp=0.5)
+    cam = s.cameras[0]
+    rng = np.random.default_rng(len(case))
+    gt = rng.uniform(0, 1, (cam.H, cam.W, 3)).astype(np.float32)
+    hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_FMA)
+    hs.debug_enable()
+    out = hs.render(cam)
+    torch.cuda.synchronize()
+    fwd = ho.render(ho.OracleScene(s), cam)
+    assert (hs.debug_fetch(B.DBG_TILE_LIST) == fwd["list_id"]).all()
+    # loss (on the oracle's image, so that both sides differentiate at the same point)
+    img = torch.from_numpy(fwd["out"]).cuda()
+    L, g_img = hs.loss_l1_ssim(img, torch.from_numpy(gt).cuda(), 0.2)
+    L_o, g_o = hb.loss_and_grad(fwd["out"], gt, 0.2)
+    assert abs(L - L_o) <= 1e-5 * abs(L_o)
+    _grad_close(g_img.cpu().numpy().astype(np.float64), g_o, "dL/d image", rel=1e-3, floor=1e-4)
+    # the whole backward from the oracle's image gradient
+    want = hb.backward_from_image_grad(s, cam, g_o, fwd=fwd)
+    got = hs.backward(torch.from_numpy(g_o.astype(np.float32)).cuda())
+    torch.cuda.synchronize()
+    for k in ("opacity_logit", "rgb_logit", "scale_logit", "pos", "geo_w", "app_w", "bg_w", "geo_table", "app_table", "bg_table"):
+        # fp16 configs: the forward pass rounds features and hidden activations to binary16 (2^-11 relative each), which the
+        # float64 oracle treats as the identity: the floor widens from 2e-3 to 5e-3 of the array's largest magnitude
+        _grad_close(got[k].cpu().numpy().astype(np.float64), want[k], f"{case}: {k}", floor=5e-3 if s.fp16 else 2e-3)
+    # gradients accumulate (hyrf.h: ADDED to what the arrays hold)
+    again = hs.backward(torch.from_numpy(g_o.astype(np.float32)).cuda(), grads={k: v.clone() for k, v in got.items()})
+    torch.cuda.synchronize()
+    assert torch.allclose(again["opacity_logit"], 2 * got["opacity_logit"], rtol=1e-4, atol=1e-9)
+    hs.close()
