@@ -551,6 +551,24 @@ def run_ours(args):
             ts.append(e0.elapsed_time(e1))
         backward = {"kernel": "raster_backward_kernel", "ms": float(np.median(ts[2:])), "V": int(cnt[1]), "D": int(cnt[2]),
                     "note": "includes the memset of the [V][9] gradient rows"}
+        # the whole training step's backward: Eq. 12 loss + dL/d image, then hyrf_backward (S6 -> S5 ->
+        # S4a -> S3 -> S2 to every parameter); first version on CUDA cores
+        target = torch.rand((H, W, 3), dtype=torch.float32, device=f"cuda:{dev}")
+        grads = None
+        tl, tb = [], []
+        for _ in range(6):
+            flush.fill_(1)
+            e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            e0.record(stream)
+            loss, g_img = hs.loss_l1_ssim(out, target, 0.2)
+            e1.record(stream)
+            grads = hs.backward(g_img, grads)
+            e2.record(stream)
+            torch.cuda.synchronize(dev)
+            tl.append(e0.elapsed_time(e1)); tb.append(e1.elapsed_time(e2))
+        backward.update({"loss_l1_ssim_ms": float(np.median(tl[2:])), "whole_backward_ms": float(np.median(tb[2:])),
+                         "loss": loss, "whole_backward_note": "hyrf_backward: background, rasterizer, projection, Eq. 7, decoders, "
+                         "grid scatter-adds; gradients of all parameters accumulated over the repetitions"})
         hs.debug_enable(0)
 
     if rank != 0:

@@ -224,8 +224,10 @@ __device__ __forceinline__ void load_weights(float* dst, const void* src, int n)
 }
 
 // ---- S4a .. S2 ------------------------------------------------------------------------------------------------------
+constexpr int kFieldBwdThreads = 512;   // one CTA per SM (116 KB of weights + accumulators): 16 warps hide the local-memory and shared-memory latencies
+
 template <int DT>
-__global__ void __launch_bounds__(kBwdThreads)
+__global__ void __launch_bounds__(kFieldBwdThreads)
 field_backward_kernel(const BwdArgs B) {
     extern __shared__ __align__(16) float sm[];
     constexpr bool FP16 = DT != HY_DT_F32;
@@ -562,7 +564,7 @@ hyrf_status launch_backward(hyrf_scene* s, const BwdArgs& B, uint32_t* launches)
     }
     hyrf_status st = hy_launch_raster_backward(s, B.g_out, B.g_T, const_cast<float*>(B.g_rec), launches);
     if (st != HYRF_OK) return st;
-    field_backward_kernel<DT><<<s->sm_count, kBwdThreads, smem_f, s->stream>>>(B);
+    field_backward_kernel<DT><<<s->sm_count, kFieldBwdThreads, smem_f, s->stream>>>(B);
     ++*launches;
     if ((e = cudaGetLastError()) != cudaSuccess) return hy_cuda_fail(e, "backward kernels");
     return HYRF_OK;
