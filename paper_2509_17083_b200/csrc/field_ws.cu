@@ -8,17 +8,18 @@
 // gathering and decoding and carries both phases' state (128 registers, 16 warps per SM), so few loads are in
 // flight. Here the roles are separate warps:
 //   * 12 GATHER warps do nothing but table look-ups (two lanes per Gaussian, 16 Gaussians per instruction, the
-//     levels' index paths resolved at compile time). Their only state is the contracted position, so the compiler
-//     keeps many levels' loads in flight. Features are written straight into shared memory in the K-major
-//     core-matrix layout of a tcgen05 A operand (one 16-byte store per 4 levels).
+//     dense / hashed choice of a level a template constant where the scene allows). Their only state is the
+//     contracted position and a rolling window of 4 levels (16 loads per lane in flight: field_tc_common.cuh's
+//     level_issue / level_consume). Features are written straight into shared memory in the K-major core-matrix
+//     layout of a tcgen05 A operand (one 16-byte store per 4 levels).
 //   * 2 DECODER warpgroups (128 threads = the 128 TMEM lanes each) take turns on tiles of 128 Gaussians: fetch the
 //     explicit records and contract the positions two tiles ahead (the gather warps' input), then, when a tile's
 //     features are complete, issue layer 1 with BOTH operands from shared memory (tcgen05.mma SS form: no register or
 //     TMEM staging of the features), run the hidden layers with the activations in TMEM as in field_mma.cu, and
 //     finish with Eq. 7 and the projection. Geometry and appearance chains interleave, so one chain's epilogue
 //     covers the other's MMA latency.
-// Hand-overs are mbarriers: ready[4] (positions of a tile available), full[3] (a tile's features written;
-// 8 sixteen-row groups arrive), free[3] (the layer-1 MMAs that read a feature buffer have completed: tcgen05.commit),
+// Hand-overs are mbarriers: ready[kNP] (positions of a tile available), full[kNF] (a tile's features written;
+// 8 sixteen-row groups arrive), free[kNF] (the layer-1 MMAs that read a feature buffer have completed: tcgen05.commit),
 // and one mbarrier per chain and warpgroup for the MMA completions.
 #include "field_common.cuh"
 #include "field_tc_common.cuh"
