@@ -231,9 +231,9 @@ hyrf_status hyrf_set_ablation(hyrf_scene* scene, uint32_t mask);
 
 /* Scheduling of the depth sort (S4c; "ordered by depth"). Its keys, the camera-space depths, depend on
  * the explicit positions only, so by default (on != 0) the sort runs on a library-owned second stream BESIDE the
- * field query (S2), which leaves 32 of its 296 CTA slots to it, and joins the frame before the binning. on == 0
- * serialises the frame on the caller's stream (one kernel at a time: what per-kernel profiling wants). The image and
- * every debug export are identical either way. */
+ * field query (S2), which leaves a few SMs to it (24 by default; on > 1: that many), and joins the frame before the
+ * binning. on == 0 serialises the frame on the caller's stream (one kernel at a time: what per-kernel profiling
+ * wants). The image and every debug export are identical either way. */
 hyrf_status hyrf_set_sort_overlap(hyrf_scene* scene, int on);
 
 /* Screen-strip parallelism over several devices: every device holds the whole scene and runs

@@ -357,6 +357,7 @@ bin_scatter_kernel(const BinArgs A) {
     __syncthreads();
     // ordered scatter, 32 pairs per step
     unsigned short* wc = s_wcnt + (size_t)warp * Tp;
+    const uint32_t tbits = 32u - (uint32_t)__clz(A.T > 1u ? A.T - 1u : 1u);   // bits of the largest bin id
     for (uint32_t eb = w0; eb < w1; eb += 32 * kU) {
         uint32_t tl[kU], gl[kU];
 #pragma unroll
@@ -371,7 +372,14 @@ bin_scatter_kernel(const BinArgs A) {
             if (eb + u * 32 >= w1) break;                    // warp-uniform
             const uint32_t tile = tl[u];
             const bool act = tile != 0xFFFFFFFFu;
-            const uint32_t peers = __match_any_sync(0xffffffffu, act ? tile : (0x80000000u | lane));
+            // lanes with the same bin, one ballot per bit of the bin id (consecutive pairs mostly differ in their bin, the
+            // case in which match.any is slowest: radix.cu)
+            uint32_t peers = __ballot_sync(0xffffffffu, act);
+            for (uint32_t b = 0; b < tbits; ++b) {
+                const bool bit = (tile >> b) & 1u;
+                const uint32_t bal = __ballot_sync(0xffffffffu, bit);
+                peers &= bit ? bal : ~bal;
+            }
             uint32_t c = 0;
             if (act) c = wc[tile];
             __syncwarp();

@@ -44,7 +44,7 @@ struct hyrf_scene {
     bool field_attr_set = false;   // cudaFuncSetAttribute of the tensor-core field kernels done for this scene's device
     bool field_ws_attr_set = false;
     bool ws_mma = false;       // decoders on tcgen05 with warp-specialised gather / decoder roles (field_ws.cu)
-    int ws_sort_sms = 12;      // SMs the warp-specialised field kernel leaves to the depth sort running beside it
+    int ws_sort_sms = 24;      // SMs the warp-specialised field kernel leaves to the depth sort running beside it (swept 12..40 on configs 3, 4, 5: DESIGN.md section 11)
 
     // persistent parameters
     float* pos = nullptr;      // [3][N]
