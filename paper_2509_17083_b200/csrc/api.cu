@@ -554,6 +554,28 @@ hyrf_status build_frame(const hyrf_scene* s, const hyrf_camera* cam, int32_t W, 
     return HYRF_OK;
 }
 
+// hyrf_render_host_async leaves the device->host copy of the frame it has just enqueued PENDING; it is enqueued here,
+// from the next call (once that frame's kernels are enqueued and the host would only wait for its counters) or from
+// hyrf_host_sync. Two reasons. (1) The image travels in pieces of copy_chunk_bytes: while ONE 11 MB copy is in flight,
+// kernels launched beside it start late (measured on B200: the cull stage of the next frame 0.029 -> 0.089 ms, its
+// field kernel +0.016 ms; with 256 KB pieces the delay is gone). (2) 43 enqueues cost the host
+// ~0.1 ms: here that time is hidden in a wait instead of standing between two frames.
+hyrf_status hy_flush_pending_copy(hyrf_scene* s) {
+    hyrf_scene::PendingCopy& pc = s->pending_copy;
+    if (!pc.valid) return HYRF_OK;
+    pc.valid = false;
+    cudaError_t e;
+    if ((e = cudaStreamWaitEvent(s->copy_stream, s->ev_rendered[pc.slot], 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent");
+    const size_t chunk = s->copy_chunk_bytes ? s->copy_chunk_bytes : pc.bytes;
+    for (size_t o = 0; o < pc.bytes; o += chunk) {
+        const size_t nb = pc.bytes - o < chunk ? pc.bytes - o : chunk;
+        if ((e = cudaMemcpyAsync((char*)pc.dst + o, (const char*)pc.src + o, nb, cudaMemcpyDeviceToHost, s->copy_stream)) != cudaSuccess)
+            return hy_cuda_fail(e, "cudaMemcpyAsync(image)");
+    }
+    if ((e = cudaEventRecord(s->ev_copied[pc.slot], s->copy_stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord");
+    return HYRF_OK;
+}
+
 hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_t H, float* out_rgb) {
     if (!s || !cam || !out_rgb) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_render: NULL argument");
     if (!s->ready) return hy_fail(HYRF_ERR_NOT_READY, "hyrf_render before the fields (hyrf_upload_params) and the explicit Gaussians (hyrf_upload_params or hyrf_upload_explicit_rvq) were uploaded");
@@ -651,6 +673,7 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     const uint32_t n_macro = (uint32_t)(f.mgx * f.mgy);
     const bool want_lists = ((s->debug_mask >> HYRF_DBG_TILE_LIST) | (s->debug_mask >> HYRF_DBG_TILE_RANGES)) & 1u;
     const bool ordered = s->bin_ws && hy_bin_ordered_supported(s->N, n_macro) && (!want_lists || hy_bin_ordered_supported(s->N, n_tiles));
+    if ((!ordered || want_lists) && (st = hy_flush_pending_copy(s)) != HYRF_OK) return st;   // these routes wait for the counters first
     if (ordered && want_lists) {
         // The export makes the rasterizer write every tile's list (D entries) into the pair buffer, and nothing there
         // checks a bound: learn D BEFORE anything is binned and grow first. (Without the export the frame is enqueued
@@ -684,6 +707,7 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
             if (timing) cudaEventRecord(s->ev[4], s->stream);
             if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;   // S6 (Eq. 10-11, A.2)
             if (timing) cudaEventRecord(s->ev[s->ev_end], s->stream);
+            if (attempt == 0 && (st = hy_flush_pending_copy(s)) != HYRF_OK) return st;   // (the previous frame's image: see there)
             if (attempt == 0 && (e = cudaEventSynchronize(s->ev_counters)) != cudaSuccess)
                 return hy_cuda_fail(e, "cudaEventSynchronize(counters)");
             V = s->counters_host->V;
@@ -778,6 +802,8 @@ extern "C" hyrf_status hyrf_render_host_async(hyrf_scene* s, const hyrf_camera* 
     if (!s->image2 && (st = dev_alloc_t(s, &s->image2, P3)) != HYRF_OK) return st;
     const int slot = (s->host_slot ^= 1);
     float* img = slot ? s->image2 : s->image;
+    // (normally the pending copy is the OTHER image's and goes out during this call; after a failed call it may be this one's)
+    if (s->pending_copy.valid && s->pending_copy.slot == slot && (st = hy_flush_pending_copy(s)) != HYRF_OK) return st;
     // the copy that last read this image must have finished before it is rendered into again
     if (s->slot_used[slot] && (e = cudaStreamWaitEvent(s->stream, s->ev_copied[slot], 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent");
     s->pipeline = true;   // a stream of frames: this one's cull and depth sort may run beside the previous one's rasterizer
@@ -785,10 +811,7 @@ extern "C" hyrf_status hyrf_render_host_async(hyrf_scene* s, const hyrf_camera* 
     s->pipeline = false;
     if (st != HYRF_OK) return st;
     if ((e = cudaEventRecord(s->ev_rendered[slot], s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord");
-    if ((e = cudaStreamWaitEvent(s->copy_stream, s->ev_rendered[slot], 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent");
-    if ((e = cudaMemcpyAsync(out_host, img, (size_t)W * H * 3 * sizeof(float), cudaMemcpyDeviceToHost, s->copy_stream)) != cudaSuccess)
-        return hy_cuda_fail(e, "cudaMemcpyAsync(image)");
-    if ((e = cudaEventRecord(s->ev_copied[slot], s->copy_stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord");
+    s->pending_copy = {out_host, img, (size_t)W * H * 3 * sizeof(float), slot, true};   // enqueued by hy_flush_pending_copy
     s->slot_used[slot] = true;
     return HYRF_OK;
 }
@@ -796,6 +819,8 @@ extern "C" hyrf_status hyrf_render_host_async(hyrf_scene* s, const hyrf_camera* 
 extern "C" hyrf_status hyrf_host_sync(hyrf_scene* s) {
     if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_host_sync: NULL scene");
     cudaError_t e;
+    hyrf_status st = hy_flush_pending_copy(s);
+    if (st != HYRF_OK) return st;
     if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize");
     if (s->copy_stream && (e = cudaStreamSynchronize(s->copy_stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(copy)");
     return HYRF_OK;

@@ -72,6 +72,8 @@ struct hyrf_scene {
     } pre[2];
     int pre_cur = 0;
     bool pipeline = false;            // the frame being enqueued belongs to a pipelined stream (no ordering behind the previous frame's tail)
+    size_t copy_chunk_bytes = 256u << 10; // hyrf_render_host_async: the image goes to the host in pieces of this size (api.cu)
+    struct PendingCopy { float* dst; const float* src; size_t bytes; int slot; bool valid; } pending_copy = {nullptr, nullptr, 0, 0, false};
     bool pipeline_all = false;        // hyrf_set_pipelining: every hyrf_render is enqueued that way
     bool frame_in_flight = false;     // a previous frame's end event has been recorded
     bool field_full_grid = false;     // this frame's field kernel takes every SM (nothing runs beside it, or the sort hides elsewhere)
