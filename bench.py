@@ -534,7 +534,22 @@ def run_ours(args):
     if args.backward and rank == 0:
         # NEXT-3, first piece: hyrf_raster_backward for camera 0's frame (per-tile lists retained), outside the timed
         # frames; CUDA events on the launching stream, L2 flushed before each repetition
-        hs.debug_enable((1 << B.DBG_TILE_LIST) | (1 << B.DBG_TILE_RANGES))
+        # the forward pass in training mode (hyrf_set_retain_lists: per-tile ranges from a count-only tile-level binning,
+        # lists written by the rasterizer up to its early exit), timed like the inference frames beside it
+        def frame_ms(reps=8):
+            t = []
+            for i in range(reps):
+                flush.fill_(1)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                hs.render_struct(cstructs[i % len(cstructs)], W, H, out.data_ptr())
+                e1.record(stream)
+                torch.cuda.synchronize(dev)
+                t.append(e0.elapsed_time(e1))
+            return float(np.median(t[2:]))
+        fwd_plain = frame_ms()
+        hs.set_retain_lists(True)
+        fwd_retain = frame_ms()
         hs.render_struct(cstructs[0], W, H, out.data_ptr())
         torch.cuda.synchronize(dev)
         cnt = hs.debug_fetch(B.DBG_COUNTERS)
@@ -550,7 +565,8 @@ def run_ours(args):
             torch.cuda.synchronize(dev)
             ts.append(e0.elapsed_time(e1))
         backward = {"kernel": "raster_backward_kernel", "ms": float(np.median(ts[2:])), "V": int(cnt[1]), "D": int(cnt[2]),
-                    "note": "includes the memset of the [V][9] gradient rows"}
+                    "note": "includes the memset of the [V][9] gradient rows",
+                    "forward_ms": fwd_plain, "forward_retain_lists_ms": fwd_retain}
         # the whole training step's backward: Eq. 12 loss + dL/d image, then hyrf_backward (S6 -> S5 ->
         # S4a -> S3 -> S2 to every parameter); first version on CUDA cores
         target = torch.rand((H, W, 3), dtype=torch.float32, device=f"cuda:{dev}")
@@ -569,7 +585,7 @@ def run_ours(args):
         backward.update({"loss_l1_ssim_ms": float(np.median(tl[2:])), "whole_backward_ms": float(np.median(tb[2:])),
                          "loss": loss, "whole_backward_note": "hyrf_backward: background, rasterizer, projection, Eq. 7, decoders, "
                          "grid scatter-adds; gradients of all parameters accumulated over the repetitions"})
-        hs.debug_enable(0)
+        hs.set_retain_lists(False)
 
     if rank != 0:
         return

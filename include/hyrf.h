@@ -270,10 +270,19 @@ hyrf_status hyrf_last_raster_mode(hyrf_scene* scene, int* mode);
  * records. g_cfg: DEVICE float [H][W][3] = dL/dC_fg; g_T: DEVICE float [H][W] = dL/dT (how a loss on the composited
  * image reaches the foreground: out = C_fg + T c_s). grad: DEVICE float [V][9], row = visible rank (HYRF_DBG_VIS_IDX
  * order), columns dL/d(u, v, A, B, C, opacity, r, g, b); overwritten. Enqueued on the scene's stream; the caller
- * synchronises. The frame must have been rendered with HYRF_DBG_TILE_LIST | HYRF_DBG_TILE_RANGES enabled (the
- * per-tile lists are then retained), else HYRF_ERR_NOT_READY. Sums use fp32 atomics: the result is reproducible to
- * rounding, not bit for bit. */
-hyrf_status hyrf_raster_backward(hyrf_scene* scene, const float* g_cfg, const float* g_T, float* grad);
+ * synchronises. grad_rows: rows grad holds; fewer than the frame's V: HYRF_ERR_INVALID_ARG, nothing is written. The
+ * frame must have kept its per-tile lists (hyrf_set_retain_lists, or the debug export HYRF_DBG_TILE_LIST |
+ * HYRF_DBG_TILE_RANGES), else HYRF_ERR_NOT_READY. Sums use fp32 atomics: the result is reproducible to rounding, not
+ * bit for bit. */
+hyrf_status hyrf_raster_backward(hyrf_scene* scene, const float* g_cfg, const float* g_T, float* grad, uint64_t grad_rows);
+
+/* Training mode of the forward pass: with on != 0 every hyrf_render keeps what the backward entry points need — the
+ * per-tile ranges (one extra, count-only run of the binning at tile level) and each tile's list as the rasterizer
+ * consumed it, up to the entry at which all of the tile's pixels had terminated (the rasterizer keeps its early exit;
+ * nothing behind that entry was blended, so no gradient flows there). Separate from the debug export, which writes
+ * every list to its end, disables the early exit and is meant for parity tests. The image is bit-identical. Costs one
+ * host wait for the frame's counters before the binning (the list buffer is grown first if need be). Default off. */
+hyrf_status hyrf_set_retain_lists(hyrf_scene* scene, int on);
 
 /* ---- microprobes ("L2 gather throughput and sustained issue rate are not in MEASURED_PEAKS.json —
  * measure them with two microprobes first and commit the numbers"). Not on the render path; no scene needed. ------- */
@@ -301,7 +310,7 @@ hyrf_status hyrf_probe_issue(int32_t device, uint32_t kind, uint32_t ctas_per_sm
  * (tables and weights in fp32 whatever the scene's param_dtype; 8-bit tables: gradient with respect to the decoded
  * values), or NULL when that gradient is not wanted. Gradients are ADDED to what the arrays hold (the caller zeroes
  * them, or accumulates several cameras). Enqueued on the scene's stream; the caller synchronises. Like
- * hyrf_raster_backward it needs the frame rendered with HYRF_DBG_TILE_LIST | HYRF_DBG_TILE_RANGES enabled, else
+ * hyrf_raster_backward it needs a frame that kept its per-tile lists (hyrf_set_retain_lists or the debug export), else
  * HYRF_ERR_NOT_READY. Sums use fp32 atomics: reproducible to rounding, not bit for bit. */
 typedef struct {
     float* pos;           /* [3][N] */

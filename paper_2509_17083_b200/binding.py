@@ -29,7 +29,8 @@ EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_r
            "hyrf_destroy_scene", "hyrf_last_error", "hyrf_debug_enable", "hyrf_debug_fetch", "hyrf_set_timing",
            "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation", "hyrf_render_host_async",
            "hyrf_host_sync", "hyrf_set_sort_overlap", "hyrf_upload_explicit_rvq", "hyrf_last_decode_time", "hyrf_set_raster_mode",
-           "hyrf_last_raster_mode", "hyrf_raster_backward", "hyrf_probe_gather", "hyrf_probe_issue", "hyrf_set_pipelining", "hyrf_frame_gap", "hyrf_set_strip", "hyrf_backward", "hyrf_loss_l1_ssim"]
+           "hyrf_last_raster_mode", "hyrf_raster_backward", "hyrf_probe_gather", "hyrf_probe_issue", "hyrf_set_pipelining", "hyrf_frame_gap", "hyrf_set_strip", "hyrf_backward", "hyrf_loss_l1_ssim",
+           "hyrf_set_retain_lists"]
 ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
 
 
@@ -122,7 +123,8 @@ def load_library() -> C.CDLL:
         L.hyrf_last_decode_time.argtypes = [vp, C.POINTER(C.c_float)]
         L.hyrf_set_raster_mode.argtypes = [vp, C.c_int]
         L.hyrf_last_raster_mode.argtypes = [vp, C.POINTER(C.c_int)]
-        L.hyrf_raster_backward.argtypes = [vp, vp, vp, vp]
+        L.hyrf_raster_backward.argtypes = [vp, vp, vp, vp, C.c_uint64]
+        L.hyrf_set_retain_lists.argtypes = [vp, C.c_int]
         L.hyrf_probe_gather.argtypes = [C.c_int32, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32,
                                         C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_float)]
         L.hyrf_probe_issue.argtypes = [C.c_int32, C.c_uint32, C.c_uint32, C.c_uint32, C.POINTER(C.c_double),
@@ -325,10 +327,12 @@ class HyrfScene:
         if out is None:
             out = torch.empty((H, W, 3), dtype=torch.float32, device=f"cuda:{self.device}")
         c = camera_struct(cam)
+        self.set_stream()   # torch's current stream may have changed since the upload (`out` was allocated on it)
         _check(self.lib.hyrf_render(self.handle, C.byref(c), W, H, C.c_void_p(out.data_ptr())))
         return out
 
     def render_struct(self, cam_struct: CameraC, W: int, H: int, out_ptr: int) -> None:
+        """The bare call (what bench.py times): the scene keeps the stream of the last set_stream()."""
         _check(self.lib.hyrf_render(self.handle, C.byref(cam_struct), W, H, C.c_void_p(out_ptr)))
 
     def render_host(self, cam, W: Optional[int] = None, H: Optional[int] = None, out=None):
@@ -386,6 +390,10 @@ class HyrfScene:
         """A stream of hyrf_render calls: frame k+1's cull and depth sort beside frame k's rasterizer (include/hyrf.h)."""
         _check(self.lib.hyrf_set_pipelining(self.handle, int(on)))
 
+    def set_retain_lists(self, on: bool = True) -> None:
+        """Training mode: every render keeps the per-tile lists the backward entry points need (include/hyrf.h)."""
+        _check(self.lib.hyrf_set_retain_lists(self.handle, int(on)))
+
     def set_raster_mode(self, mode: int = 0) -> None:
         """0 auto, 1 tile-level lists only, 2 per-warp lists (include/hyrf.h hyrf_set_raster_mode); same bits, different cost."""
         _check(self.lib.hyrf_set_raster_mode(self.handle, int(mode)))
@@ -395,8 +403,9 @@ class HyrfScene:
         torch = self._torch
         grad = torch.empty((int(n_visible), 9), dtype=torch.float32, device=f"cuda:{self.device}")
         g_cfg, g_T = g_cfg.contiguous(), g_T.contiguous()
+        self.set_stream()
         _check(self.lib.hyrf_raster_backward(self.handle, C.c_void_p(g_cfg.data_ptr()), C.c_void_p(g_T.data_ptr()),
-                                             C.c_void_p(grad.data_ptr())))
+                                             C.c_void_p(grad.data_ptr()), C.c_uint64(grad.shape[0])))
         return grad
 
     def backward(self, g_out, grads: Optional[Dict] = None, want=None) -> Dict:
@@ -412,6 +421,7 @@ class HyrfScene:
         for k in names:
             setattr(g, k, grads[k].data_ptr())
         g_out = g_out.contiguous()
+        self.set_stream()
         _check(self.lib.hyrf_backward(self.handle, C.c_void_p(g_out.data_ptr()), C.byref(g)))
         return grads
 
@@ -422,6 +432,7 @@ class HyrfScene:
         H, W = int(image.shape[0]), int(image.shape[1])
         g = torch.empty_like(image) if want_grad else None
         loss = C.c_double(0)
+        self.set_stream()
         _check(self.lib.hyrf_loss_l1_ssim(self.handle, C.c_void_p(image.data_ptr()), C.c_void_p(target.data_ptr()), W, H,
                                           C.c_float(lam), C.byref(loss), C.c_void_p(g.data_ptr() if want_grad else None)))
         return float(loss.value), g

@@ -169,7 +169,7 @@ void destroy(hyrf_scene* s) {
     void* ptrs[] = {s->pos, s->rgb, s->scale, s->opac, (void*)s->geo_grid.table, (void*)s->app_grid.table,
                     (void*)s->bg_grid.table, (void*)s->geo_mlp.w, (void*)s->app_mlp.w, (void*)s->bg_mlp.w, s->mma_w, s->both_table,
                     s->gm, s->gm_id, s->rec, s->rect, s->tiles, s->mtiles, s->mranges, s->tt_sorted, s->offs,
-                    s->scan_scratch, s->ranges, s->tile_queue, s->fg, s->finalT, s->image, s->image2, s->bg_mask, s->bg_list,
+                    s->scan_scratch, s->ranges, s->list_len, s->tile_queue, s->fg, s->finalT, s->image, s->image2, s->bg_mask, s->bg_list,
                     s->dbg_raw, s->dbg_attrs, s->bwd_gT, s->bwd_grec, s->bwd_ssim};
     for (void* p : ptrs) dev_free(s, p);
     if (s->sort_stream) cudaStreamSynchronize(s->sort_stream);
@@ -330,6 +330,7 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
     HY_TRY(dev_alloc_t(s, &s->offs, N));
     HY_TRY(dev_alloc_t(s, &s->ranges, tiles));
     HY_TRY(dev_alloc_t(s, &s->mranges, tiles));
+    HY_TRY(dev_alloc_t(s, &s->list_len, tiles));
     HY_TRY(dev_alloc_t(s, &s->tile_queue, tiles));
     HY_TRY(dev_alloc_t(s, &s->finalT, P));
     HY_TRY(dev_alloc_t(s, &s->bg_list, P));
@@ -358,7 +359,8 @@ extern "C" hyrf_status hyrf_create_scene(const hyrf_scene_desc* desc, hyrf_scene
 
 extern "C" hyrf_status hyrf_set_stream(hyrf_scene* s, void* cuda_stream) {
     if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_stream: NULL scene");
-    cudaStreamSynchronize(s->stream);
+    if (s->stream == reinterpret_cast<cudaStream_t>(cuda_stream)) return HYRF_OK;   // (cheap to call before every frame)
+    cudaStreamSynchronize(s->stream);   // what is enqueued on the old stream reads and writes the scene's scratch
     s->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     return HYRF_OK;
 }
@@ -482,11 +484,12 @@ extern "C" hyrf_status hyrf_set_raster_mode(hyrf_scene* s, int mode) {
     return HYRF_OK;
 }
 
-extern "C" hyrf_status hyrf_raster_backward(hyrf_scene* s, const float* g_cfg, const float* g_T, float* grad) {
+extern "C" hyrf_status hyrf_raster_backward(hyrf_scene* s, const float* g_cfg, const float* g_T, float* grad, uint64_t grad_rows) {
     if (!s || !g_cfg || !g_T || !grad) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_raster_backward: NULL argument");
-    const uint32_t need = (1u << HYRF_DBG_TILE_LIST) | (1u << HYRF_DBG_TILE_RANGES);
-    if (!s->rendered || !s->list_final || (s->debug_mask & need) != need)
-        return hy_fail(HYRF_ERR_NOT_READY, "hyrf_raster_backward: the last frame was not rendered with HYRF_DBG_TILE_LIST | HYRF_DBG_TILE_RANGES enabled");
+    if (!s->rendered || !s->list_final)
+        return hy_fail(HYRF_ERR_NOT_READY, "hyrf_raster_backward: the last frame kept no per-tile lists (hyrf_set_retain_lists, or the debug export HYRF_DBG_TILE_LIST | HYRF_DBG_TILE_RANGES)");
+    if (grad_rows < s->lastV)
+        return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_raster_backward: grad holds %llu rows, the last frame has %u visible Gaussians", (unsigned long long)grad_rows, s->lastV);
     cudaError_t e;
     if ((e = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
     uint32_t launches = 0;
@@ -671,7 +674,11 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     // are only materialised when the debug export asks for them: the ranges by a second, tile-level run of the same
     // binning, the lists by the rasterizer itself (what it consumed, in the order it consumed it).
     const uint32_t n_macro = (uint32_t)(f.mgx * f.mgy);
-    const bool want_lists = ((s->debug_mask >> HYRF_DBG_TILE_LIST) | (s->debug_mask >> HYRF_DBG_TILE_RANGES)) & 1u;
+    const bool export_lists = ((s->debug_mask >> HYRF_DBG_TILE_LIST) | (s->debug_mask >> HYRF_DBG_TILE_RANGES)) & 1u;
+    // per-tile lists are kept for the backward pass (hyrf_set_retain_lists) or written out whole for the debug export;
+    // only the export needs every tile's list to its end, so a retained list stops where the tile's pixels all had
+    // terminated (list_len) and the rasterizer keeps its early exit
+    const bool want_lists = export_lists || s->retain_lists;
     const bool ordered = s->bin_ws && hy_bin_ordered_supported(s->N, n_macro) && (!want_lists || hy_bin_ordered_supported(s->N, n_tiles));
     if ((!ordered || want_lists) && (st = hy_flush_pending_copy(s)) != HYRF_OK) return st;   // these routes wait for the counters first
     if (ordered && want_lists) {
@@ -702,8 +709,11 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
             // the per-tile lists are written by the rasterizer into the (by then dead) pair array of the macro run
             s->list_final = want_lists ? s->ent_val[0] : nullptr;
             if (timing) cudaEventRecord(s->ev[3], s->stream);
+            s->list_partial = want_lists && !export_lists;
+            if (s->list_partial && (e = cudaMemsetAsync(s->list_len, 0, (size_t)n_tiles * sizeof(uint32_t), s->stream)) != cudaSuccess)
+                return hy_cuda_fail(e, "cudaMemsetAsync(list_len)");   // (tiles of another device's strip stay empty)
             hy_launch_raster(s, f, s->mranges, s->ent_key[1], /*macro=*/true, out_rgb, &launches, s->tile_queue,
-                             want_lists ? s->ent_val[0] : nullptr);                            // S5 (Eq. 1)
+                             want_lists ? s->ent_val[0] : nullptr, s->list_partial ? s->list_len : nullptr);                            // S5 (Eq. 1)
             if (timing) cudaEventRecord(s->ev[4], s->stream);
             if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;   // S6 (Eq. 10-11, A.2)
             if (timing) cudaEventRecord(s->ev[s->ev_end], s->stream);
@@ -743,7 +753,8 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
         hy_launch_ranges(s, sorted_key, D, n_tiles, &launches);
         s->list_final = sorted_val;
         if (timing) cudaEventRecord(s->ev[3], s->stream);
-        hy_launch_raster(s, f, s->ranges, sorted_val, /*macro=*/false, out_rgb, &launches, nullptr, nullptr);   // S5
+        s->list_partial = false;
+        hy_launch_raster(s, f, s->ranges, sorted_val, /*macro=*/false, out_rgb, &launches, nullptr, nullptr, nullptr);   // S5
         if (timing) cudaEventRecord(s->ev[4], s->stream);
         if ((st = hy_launch_background(s, f, out_rgb, &launches)) != HYRF_OK) return st;       // S6 (Eq. 10-11, A.2)
         if (timing) cudaEventRecord(s->ev[s->ev_end], s->stream);
@@ -863,6 +874,12 @@ extern "C" hyrf_status hyrf_set_sort_overlap(hyrf_scene* s, int on) {
     if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_sort_overlap: NULL scene");
     s->sort_overlap = on != 0;
     if (on > 1) s->ws_sort_sms = on < s->sm_count ? on : s->sm_count - 1;   // on > 1: SMs the warp-specialised field kernel leaves to the sort
+    return HYRF_OK;
+}
+
+extern "C" hyrf_status hyrf_set_retain_lists(hyrf_scene* s, int on) {
+    if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_retain_lists: NULL scene");
+    s->retain_lists = on != 0;
     return HYRF_OK;
 }
 

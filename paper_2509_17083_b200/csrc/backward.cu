@@ -574,9 +574,8 @@ hyrf_status launch_backward(hyrf_scene* s, const BwdArgs& B, uint32_t* launches)
 
 extern "C" hyrf_status hyrf_backward(hyrf_scene* s, const float* g_out, const hyrf_grads* grads) {
     if (!s || !g_out || !grads) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_backward: NULL argument");
-    const uint32_t need = (1u << HYRF_DBG_TILE_LIST) | (1u << HYRF_DBG_TILE_RANGES);
-    if (!s->rendered || !s->list_final || (s->debug_mask & need) != need)
-        return hy_fail(HYRF_ERR_NOT_READY, "hyrf_backward: the last frame was not rendered with HYRF_DBG_TILE_LIST | HYRF_DBG_TILE_RANGES enabled");
+    if (!s->rendered || !s->list_final)
+        return hy_fail(HYRF_ERR_NOT_READY, "hyrf_backward: the last frame kept no per-tile lists (hyrf_set_retain_lists, or the debug export HYRF_DBG_TILE_LIST | HYRF_DBG_TILE_RANGES)");
     cudaError_t e;
     if ((e = cudaSetDevice(s->desc.device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
     hyrf_status st;

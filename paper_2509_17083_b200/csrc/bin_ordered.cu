@@ -415,7 +415,8 @@ size_t hy_bin_ordered_ws_elems(uint32_t N, size_t cap, uint32_t max_tiles) {
     return 2 * ((size_t)N / kOffItems + 2) + m + 2 * T + 64;
 }
 
-// macro = false: bins are tiles -> s->ranges, list in ent_val[1] (the debug export of the per-tile lists).
+// macro = false: bins are tiles -> s->ranges only (the ranges of the per-tile lists the rasterizer writes for the debug
+//                export / the backward pass); no list is scattered.
 // macro = true : bins are macro tiles (HY_MACRO x HY_MACRO tiles) -> s->mranges, list in ent_key[1], s->tile_queue:
 //                what the rasterizer walks; n_tiles / gx are still those of the TILE grid.
 hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t n_tiles, uint32_t gx,
@@ -454,8 +455,7 @@ hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t
     A.list = macro ? s->ent_key[1] : s->ent_val[1];
     const size_t smem_count = (size_t)n_tiles * 4;
     const size_t smem_scatter = (size_t)n_tiles * 4 + (size_t)kBinWarps * ((n_tiles + 1u) & ~1u) * 2;
-    static bool attr_done[64] = {};   // per device: function attributes belong to the device's context
-    bool& attr_set = attr_done[s->desc.device & 63];
+    bool& attr_set = s->bin_attr_set;
     if (!attr_set) {
         HY_CUDA_OK(cudaFuncSetAttribute(bin_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxTiles * 4)));
         HY_CUDA_OK(cudaFuncSetAttribute(bin_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxTiles * 20)));
@@ -466,7 +466,9 @@ hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t
     bin_pairs_kernel<<<(s->N + kBinThreads - 1) / kBinThreads, kBinThreads, 0, s->stream>>>(A);
     bin_count_kernel<<<A.rows_cap, kBinThreads, smem_count, s->stream>>>(A);
     bin_prefix_kernel<<<(n_tiles + 31) / 32, 1024, 0, s->stream>>>(A);
-    bin_scatter_kernel<<<A.rows_cap + 1, kBinThreads, smem_scatter, s->stream>>>(A);   // + 1: the tile-queue CTA
-    *launches += 5;
+    // the tile-level run only supplies the per-tile ranges (the lists themselves are written by the rasterizer as it
+    // consumes them, api.cu): its scatter would produce a list nobody reads
+    if (macro) bin_scatter_kernel<<<A.rows_cap + 1, kBinThreads, smem_scatter, s->stream>>>(A);   // + 1: the tile-queue CTA
+    *launches += macro ? 5 : 4;
     return HYRF_OK;
 }

@@ -19,7 +19,8 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
               int W, int H, int gx, float tau_T, float* __restrict__ out_rgb, float* __restrict__ finalT,
               uint32_t* __restrict__ bg_list, FrameCounters* __restrict__ counters, uint8_t* __restrict__ bg_mask,
               float* __restrict__ dbg_fg, const uint32_t* __restrict__ tile_queue, const uint4* __restrict__ rect,
-              int mshift, int mgx, uint32_t* __restrict__ dbg_list, const uint2* __restrict__ dbg_ranges, int ty0, int ty1) {
+              int mshift, int mgx, uint32_t* __restrict__ dbg_list, const uint2* __restrict__ dbg_ranges, uint32_t* __restrict__ dbg_len,
+        int ty0, int ty1) {
     __shared__ float4 s_r0[2 * kBatch + 8];   // (u, v, A, B)   (+ 8: padding to a multiple of 8)
     __shared__ float4 s_r1[2 * kBatch + 8];   // (C, opacity, r, g)
     __shared__ float s_b[2 * kBatch + 8];
@@ -53,7 +54,7 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
     while (b0 < rg.y) {
         // every pixel terminated: stop — unless the per-tile list is being exported, which needs the whole list walked
         const bool all_done = __syncthreads_count(done) == kBatch;
-        if (all_done && !dbg_list) break;
+        if (all_done && (!dbg_list || dbg_len)) break;
         // stage A: walk the list in chunks of 256 entries and collect, in order, the ids that belong to THIS tile (all of
         // them when the lists are per tile; about one in five when they are per macro tile) until 256 are waiting
         uint32_t nh = 0;
@@ -149,6 +150,8 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
             }
         }
     }
+    // retained lists (hyrf_set_retain_lists): how much of this tile's list was written before every pixel had terminated
+    if (dbg_len && threadIdx.x == 0) dbg_len[tile] = dbg_pos - dbg_ranges[tile].x;
     if (inside) {
         const size_t o = (size_t)py * W + px;
         out_rgb[3 * o] = C0; out_rgb[3 * o + 1] = C1; out_rgb[3 * o + 2] = C2;
@@ -171,7 +174,7 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
 }  // namespace
 
 void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
-                      float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list) {
+                      float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list, uint32_t* dbg_len) {
     // Per-warp lists (raster_warp.cu) pay when a splat covers few tiles: small splats leave many 8 x 4 blocks of a tile
     // untouched. With large splats nearly every block is reached and this file's kernel (no masks, no
     // indirection) is faster. Both give the same bits, so the choice is a cost heuristic: tiles touched per visible
@@ -183,8 +186,8 @@ void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, con
     // per-warp lists: the packed-fp32 kernel (two pixels per lane, raster_pair.cu) unless mode 2 pins the one-pixel one
     s->last_raster_mode = warp_lists ? (s->raster_mode == 2 ? 2 : 3) : 1;
     if (warp_lists) {
-        if (s->raster_mode == 2) hy_launch_raster_warp(s, f, ranges, list, macro, out_rgb, launches, tile_queue, dbg_list);
-        else hy_launch_raster_pair(s, f, ranges, list, macro, out_rgb, launches, tile_queue, dbg_list);
+        if (s->raster_mode == 2) hy_launch_raster_warp(s, f, ranges, list, macro, out_rgb, launches, tile_queue, dbg_list, dbg_len);
+        else hy_launch_raster_pair(s, f, ranges, list, macro, out_rgb, launches, tile_queue, dbg_list, dbg_len);
         return;
     }
     const unsigned grid = (unsigned)(f.gx * f.gy);
@@ -194,6 +197,6 @@ void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, con
     raster_kernel<<<grid, kBatch, 0, s->stream>>>(ranges, list, s->rec, f.W, f.H, f.gx, tau, out_rgb, s->finalT,
                                                   s->bg_list, s->counters, want_mask ? s->bg_mask : nullptr,
                                                   want_fg ? s->fg : nullptr, tile_queue, s->rect,
-                                                  macro ? f.mshift : 0, f.mgx, dbg_list, s->ranges, f.ty0, f.ty1);
+                                                  macro ? f.mshift : 0, f.mgx, dbg_list, s->ranges, dbg_len, f.ty0, f.ty1);
     ++*launches;
 }

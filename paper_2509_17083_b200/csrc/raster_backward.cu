@@ -4,7 +4,7 @@
 // through the 3DGS rasterizer the paper defers to (:108); this is that step for the pass of raster.cu.
 //
 // One CTA per tile, one thread per pixel, over the tile's own depth-ordered list (the per-tile lists the forward
-// materialises when HYRF_DBG_TILE_LIST | HYRF_DBG_TILE_RANGES are enabled). Phase 1 replays D10 with the forward's
+// keeps under hyrf_set_retain_lists, or exports whole under HYRF_DBG_TILE_LIST | HYRF_DBG_TILE_RANGES). Phase 1 replays D10 with the forward's
 // exact binary32 operations (same ex2.approx, same order, hence the same decisions) to find, per pixel, the end of its
 // blended prefix and its final T. Phase 2 walks the list backwards in staged batches: alpha is recomputed, the
 // transmittance in front of a pair is recovered as T_k = T_{k+1} / (1 - alpha_k) (alpha <= 0.99 bounds the
@@ -32,7 +32,7 @@ __device__ __forceinline__ bool pair_alpha(const float4 a0, float C, float o, fl
 }
 
 __global__ void __launch_bounds__(kBatch)
-raster_backward_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ list,
+raster_backward_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ list_len, const uint32_t* __restrict__ list,
                        const float4* __restrict__ rec, int W, int H, int gx, const float* __restrict__ g_cfg,
                        const float* __restrict__ g_T, float* __restrict__ grad) {
     __shared__ float4 s_r0[kBatch];   // (u, v, A, B)
@@ -49,7 +49,8 @@ raster_backward_kernel(const uint2* __restrict__ ranges, const uint32_t* __restr
     const bool inside = px < W && py < H;
     const float fi = (float)px, fj = (float)py;
     const uint2 rg = ranges[tile];
-    const uint32_t len = rg.y - rg.x;
+    // retained lists end where the forward's tile stopped walking (every pixel terminated): nothing behind that point was blended
+    const uint32_t len = list_len ? min(rg.y - rg.x, list_len[tile]) : rg.y - rg.x;
 
     // phase 1: the forward's decisions -> n_mine = length of this pixel's blended prefix of the list, T = its final T
     float T = 1.0f;
@@ -172,7 +173,7 @@ hyrf_status hy_launch_raster_backward(hyrf_scene* s, const float* g_cfg, const f
     const int gx = (W + HY_TILE - 1) / HY_TILE, gy = (H + HY_TILE - 1) / HY_TILE;
     cudaError_t e = cudaMemsetAsync(grad, 0, (size_t)s->lastV * 9 * sizeof(float), s->stream);
     if (e != cudaSuccess) return hy_cuda_fail(e, "cudaMemsetAsync(grad)");
-    raster_backward_kernel<<<(unsigned)(gx * gy), kBatch, 0, s->stream>>>(s->ranges, s->list_final, s->rec, W, H, gx, g_cfg,
+    raster_backward_kernel<<<(unsigned)(gx * gy), kBatch, 0, s->stream>>>(s->ranges, s->list_partial ? s->list_len : nullptr, s->list_final, s->rec, W, H, gx, g_cfg,
                                                                           g_T, grad);
     if ((e = cudaGetLastError()) != cudaSuccess) return hy_cuda_fail(e, "raster_backward_kernel");
     ++*launches;

@@ -23,7 +23,8 @@ raster_warp_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict_
               int W, int H, int gx, float tau_T, float* __restrict__ out_rgb, float* __restrict__ finalT,
               uint32_t* __restrict__ bg_list, FrameCounters* __restrict__ counters, uint8_t* __restrict__ bg_mask,
               float* __restrict__ dbg_fg, const uint32_t* __restrict__ tile_queue, const uint4* __restrict__ rect,
-              int mshift, int mgx, uint32_t* __restrict__ dbg_list, const uint2* __restrict__ dbg_ranges, int ty0, int ty1) {
+              int mshift, int mgx, uint32_t* __restrict__ dbg_list, const uint2* __restrict__ dbg_ranges, uint32_t* __restrict__ dbg_len,
+        int ty0, int ty1) {
     __shared__ float4 s_rec[3 * (2 * kBatch + 1)];                      // staged records, 48 B each; slot kNullSlot is the null record
     __shared__ __align__(16) uint16_t s_widx[kWarps][2 * kBatch + 8];   // per warp: byte offsets of the records it blends
     __shared__ uint8_t s_mask[2 * kBatch];    // per staged record: bit w set when warp w's pixel block can reach it
@@ -58,7 +59,7 @@ raster_warp_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict_
     while (b0 < rg.y) {
         // every pixel terminated: stop — unless the per-tile list is being exported, which needs the whole list walked
         const bool all_done = __syncthreads_count(done) == kBatch;
-        if (all_done && !dbg_list) break;
+        if (all_done && (!dbg_list || dbg_len)) break;
         // stage A: walk the list in chunks of 256 entries and collect, in order, the ids that belong to THIS tile (all of
         // them when the lists are per tile; about one in five when they are per macro tile) until 256 are waiting
         uint32_t nh = 0;
@@ -169,6 +170,8 @@ raster_warp_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict_
             }
         }
     }
+    // retained lists (hyrf_set_retain_lists): how much of this tile's list was written before every pixel had terminated
+    if (dbg_len && threadIdx.x == 0) dbg_len[tile] = dbg_pos - dbg_ranges[tile].x;
     if (inside) {
         const size_t o = (size_t)py * W + px;
         out_rgb[3 * o] = C0; out_rgb[3 * o + 1] = C1; out_rgb[3 * o + 2] = C2;
@@ -191,7 +194,7 @@ raster_warp_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict_
 }  // namespace
 
 void hy_launch_raster_warp(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
-                           float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list) {
+                           float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list, uint32_t* dbg_len) {
     const unsigned grid = (unsigned)(f.gx * f.gy);
     const bool want_fg = (s->debug_mask >> HYRF_DBG_FG) & 1u;
     const bool want_mask = (s->debug_mask >> HYRF_DBG_BG_MASK) & 1u;
@@ -199,6 +202,6 @@ void hy_launch_raster_warp(hyrf_scene* s, const FrameDev& f, const uint2* ranges
     raster_warp_kernel<<<grid, kBatch, 0, s->stream>>>(ranges, list, s->rec, f.W, f.H, f.gx, tau, out_rgb, s->finalT,
                                                        s->bg_list, s->counters, want_mask ? s->bg_mask : nullptr,
                                                        want_fg ? s->fg : nullptr, tile_queue, s->rect,
-                                                       macro ? f.mshift : 0, f.mgx, dbg_list, s->ranges, f.ty0, f.ty1);
+                                                       macro ? f.mshift : 0, f.mgx, dbg_list, s->ranges, dbg_len, f.ty0, f.ty1);
     ++*launches;
 }

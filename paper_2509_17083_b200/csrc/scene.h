@@ -113,6 +113,10 @@ struct hyrf_scene {
 
     // per-frame scratch sized from max W x H
     uint2* ranges = nullptr;  // [tiles] per-tile ranges (debug export; produced by the tile-level binning)
+    uint32_t* list_len = nullptr; // [tiles] retained lists: entries of each tile's list the rasterizer wrote (list_partial)
+    bool bin_attr_set = false;    // bin_ordered.cu's function attributes set for this scene's device
+    bool retain_lists = false;    // hyrf_set_retain_lists
+    bool list_partial = false;    // the last frame's per-tile lists end at list_len (retained), not at their ranges (exported)
     uint2* mranges = nullptr; // [macro tiles] ranges into the macro-tile lists the rasterizer walks
     uint32_t* tile_queue = nullptr;  // [tiles] tile ids, longest list first (bin_ordered.cu -> raster.cu)
     float* fg = nullptr;      // [H][W][3] (debug only)
@@ -193,11 +197,11 @@ hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t
                                   uint32_t* launches, bool macro, uint32_t shift);
 // S5 (raster.cu)
 void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
-                      float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list);
+                      float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list, uint32_t* dbg_len);
 void hy_launch_raster_warp(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
-                           float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list);
+                           float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list, uint32_t* dbg_len);
 void hy_launch_raster_pair(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
-                           float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list);
+                           float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list, uint32_t* dbg_len);
 // backward of S5 for the last frame (raster_backward.cu); needs the per-tile lists (s->ranges, s->list_final)
 hyrf_status hy_launch_raster_backward(hyrf_scene* s, const float* g_cfg, const float* g_T, float* grad,
                                       uint32_t* launches);

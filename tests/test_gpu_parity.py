@@ -858,3 +858,46 @@ def test_backward_against_oracle(B, ho, synth, case):
     torch.cuda.synchronize()
     assert torch.allclose(again["opacity_logit"], 2 * got["opacity_logit"], rtol=1e-4, atol=1e-9)
     hs.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("raster_mode", [1, 2, 3])
+def test_retained_lists_give_the_export_paths_gradients(B, synth, raster_mode):
+    # hyrf_set_retain_lists: the training switch keeps per-tile lists only up to the entry at which a
+    # tile's pixels had all terminated and leaves the rasterizer its early exit. Image: bit-identical. Gradients: those
+    # of the debug-export path (whole lists, no early exit) up to the order of the fp32 atomics.
+    import torch
+    s = synth.make_scene(3, n_gaussians=20_000, width=160, height=96, n_cameras=1, table_amp=0.5)
+    s.opacity_logit[:] += 3.0   # opaque enough for tiles to terminate early: the retained lists are really shorter
+    cam = s.cameras[0]
+    g = torch.from_numpy(np.random.default_rng(3).normal(0, 1, (cam.H, cam.W, 3)).astype(np.float32)).cuda()
+    res = {}
+    for how in ("export", "retain"):
+        hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_FMA)
+        hs.set_raster_mode(raster_mode)
+        if how == "export":
+            hs.debug_enable((1 << B.DBG_TILE_LIST) | (1 << B.DBG_TILE_RANGES))
+        else:
+            hs.set_retain_lists(True)
+        img = hs.render(cam).clone()
+        grads = hs.backward(g)
+        torch.cuda.synchronize()
+        V = int(hs.debug_fetch(B.DBG_COUNTERS)[1])   # (N, V, D, tiles, Dm)
+        with pytest.raises(B.HyrfError) as e:   # a gradient buffer smaller than V is refused
+            B._check(hs.lib.hyrf_raster_backward(hs.handle, g.data_ptr(), g[..., 0].contiguous().data_ptr(),
+                                                 g.data_ptr(), max(V - 1, 0)))
+        assert e.value.status == B.HYRF_ERR_INVALID_ARG
+        res[how] = (img, {k: v.clone() for k, v in grads.items()})
+        hs.close()
+    assert torch.equal(res["export"][0], res["retain"][0])
+    for k, a in res["export"][1].items():
+        b = res["retain"][1][k]
+        scale = float(a.abs().max())
+        assert float((a - b).abs().max()) <= 1e-4 * scale + 1e-12, (k, float((a - b).abs().max()), scale)
+    # without either switch the backward is refused
+    hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_FMA)
+    hs.render(cam)
+    with pytest.raises(B.HyrfError) as e:
+        hs.backward(g)
+    assert e.value.status == B.HYRF_ERR_NOT_READY
+    hs.close()
