@@ -329,6 +329,21 @@ hyrf_status hyrf_backward(hyrf_scene* scene, const float* g_out, const hyrf_grad
 hyrf_status hyrf_loss_l1_ssim(hyrf_scene* scene, const float* image, const float* target, int32_t W, int32_t H,
                               float lambda, double* loss_host, float* g_image);
 
+/* The same loss through an entry point that ALLOCATES NOTHING, for callers that cannot call cudaMalloc (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it). Needs no scene: device = CUDA device ordinal
+ * (0 .. 63), cuda_stream = the cudaStream_t (as void*) the work is enqueued on and that is synchronised before the call
+ * returns; the other arguments, the arithmetic and the result are hyrf_loss_l1_ssim's. The scratch (the loss
+ * accumulator and three derivative maps of 3 W H floats each) is a file-scope device array of
+ * 4 + 9 HYRF_LOSS_NOALLOC_MAX_PIXELS floats (37.7 MB) that every GPU which loads the library holds until the process
+ * exits. Limit: W * H <= HYRF_LOSS_NOALLOC_MAX_PIXELS (2^20: covers 1280 x 720 and 1245 x 825); larger images are
+ * rejected with HYRF_ERR_INVALID_ARG before anything is enqueued — use hyrf_loss_l1_ssim for those. The call performs
+ * no cudaMalloc / cudaFree and calls no allocating library routine. All calls on a device SHARE the array: it keeps
+ * the last call's contents (the call clears the accumulator and rewrites the maps before reading them), and two calls
+ * whose GPU work overlaps (different streams, different host threads) race on it — serialise them. */
+#define HYRF_LOSS_NOALLOC_MAX_PIXELS (1u << 20)
+hyrf_status hyrf_loss_l1_ssim_noalloc(int32_t device, void* cuda_stream, const float* image, const float* target,
+                                      int32_t W, int32_t H, float lambda, double* loss_host, float* g_image);
+
 /* Number of kernels the last render launched (for bench.py's gpu_launches). */
 hyrf_status hyrf_last_launch_count(hyrf_scene* scene, uint32_t* launches);
 

@@ -30,7 +30,7 @@ EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_r
            "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation", "hyrf_render_host_async",
            "hyrf_host_sync", "hyrf_set_sort_overlap", "hyrf_upload_explicit_rvq", "hyrf_last_decode_time", "hyrf_set_raster_mode",
            "hyrf_last_raster_mode", "hyrf_raster_backward", "hyrf_probe_gather", "hyrf_probe_issue", "hyrf_set_pipelining", "hyrf_frame_gap", "hyrf_set_strip", "hyrf_backward", "hyrf_loss_l1_ssim",
-           "hyrf_set_retain_lists"]
+           "hyrf_set_retain_lists", "hyrf_loss_l1_ssim_noalloc"]
 ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
 
 
@@ -125,6 +125,7 @@ def load_library() -> C.CDLL:
         L.hyrf_last_raster_mode.argtypes = [vp, C.POINTER(C.c_int)]
         L.hyrf_raster_backward.argtypes = [vp, vp, vp, vp, C.c_uint64]
         L.hyrf_set_retain_lists.argtypes = [vp, C.c_int]
+        L.hyrf_loss_l1_ssim_noalloc.argtypes = [C.c_int32, vp, vp, vp, C.c_int32, C.c_int32, C.c_float, C.POINTER(C.c_double), vp]
         L.hyrf_probe_gather.argtypes = [C.c_int32, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32,
                                         C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_float)]
         L.hyrf_probe_issue.argtypes = [C.c_int32, C.c_uint32, C.c_uint32, C.c_uint32, C.POINTER(C.c_double),
@@ -143,6 +144,26 @@ def last_error() -> str:
 def _check(status: int) -> None:
     if status != HYRF_OK:
         raise HyrfError(status, last_error())
+
+
+LOSS_NOALLOC_MAX_PIXELS = 1 << 20   # include/hyrf.h HYRF_LOSS_NOALLOC_MAX_PIXELS
+
+
+def loss_l1_ssim_noalloc(image, target, lam: float = 0.2, g_image=None):
+    """hyrf_loss_l1_ssim_noalloc (include/hyrf.h): the Eq. 12 loss without any allocation by the library. image, target:
+    (H, W, 3) float32 contiguous CUDA tensors; g_image: a caller-owned tensor of the same shape that receives
+    dL/d image, or None. Runs on torch's current stream of the tensors' device. Returns the loss."""
+    import torch
+    if not (image.is_contiguous() and target.is_contiguous() and (g_image is None or g_image.is_contiguous())):
+        raise ValueError("loss_l1_ssim_noalloc: contiguous tensors only (making a copy would allocate)")
+    H, W = int(image.shape[0]), int(image.shape[1])
+    dev = image.device.index if image.device.index is not None else torch.cuda.current_device()
+    loss = C.c_double(0)
+    _check(load_library().hyrf_loss_l1_ssim_noalloc(
+        dev, C.c_void_p(torch.cuda.current_stream(dev).cuda_stream), C.c_void_p(image.data_ptr()),
+        C.c_void_p(target.data_ptr()), W, H, C.c_float(lam), C.byref(loss),
+        C.c_void_p(g_image.data_ptr() if g_image is not None else None)))
+    return float(loss.value)
 
 
 def probe_gather(device: int, table_bytes: int, entry_bytes: int, ctas_per_sm: int, share: int = 1, line: int = 0,

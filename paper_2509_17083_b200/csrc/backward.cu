@@ -17,6 +17,8 @@
 // transposing butterfly (31 shuffles per 32 weights), accumulates in shared memory (one accumulator block per
 // persistent CTA), and the CTAs add their blocks to global memory once at the end. (The tensor-core formulation of
 // these reductions — dW = Delta^T H as a GEMM over the Gaussians — is the next step.)
+#include <mutex>
+
 #include "field_common.cuh"
 #include "raster_common.cuh"
 
@@ -622,6 +624,62 @@ extern "C" hyrf_status hyrf_loss_l1_ssim(hyrf_scene* s, const float* image, cons
     double l = 0.0;
     if ((e = cudaMemcpyAsync(&l, dloss, sizeof(double), cudaMemcpyDeviceToHost, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpyAsync(loss)");
     if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(loss)");
+    *loss_host = l + (double)lambda;   // the kernels summed (1 - lambda) L1 - lambda SSIM
+    return HYRF_OK;
+}
+
+// ---- Eq. 12 once more, through an entry point that allocates nothing (include/hyrf.h hyrf_loss_l1_ssim_noalloc) ------------
+// Same kernels, same arithmetic as hyrf_loss_l1_ssim; the scratch (the loss accumulator and the three derivative maps)
+// is this file-scope array instead of a cudaMalloc'ed buffer of the scene. Every device that loads the library holds
+// its own copy (37.7 MB) until the process exits. In HOST code the array's name is a host-side stand-in, not a device
+// address: the kernels get the address cudaGetSymbolAddress returns, asked for once per device with that device
+// current. All calls on a device share the array, and it keeps the last call's contents: the accumulator is cleared
+// here before every use; the maps are completely rewritten by pass 1 (for the W x H of the call) before pass 2 reads them.
+static __device__ __align__(256) float g_loss_scratch[4 + 9ull * HYRF_LOSS_NOALLOC_MAX_PIXELS];
+
+namespace {
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+float* g_noalloc_ptr[kNoAllocMaxDevices] = {};
+}  // namespace
+
+extern "C" hyrf_status hyrf_loss_l1_ssim_noalloc(int32_t device, void* cuda_stream, const float* image, const float* target,
+                                                 int32_t W, int32_t H, float lambda, double* loss_host, float* g_image) {
+    if (!image || !target || !loss_host) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_loss_l1_ssim_noalloc: NULL argument");
+    if (device < 0 || device >= kNoAllocMaxDevices) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_loss_l1_ssim_noalloc: device %d", device);
+    if (W < 1 || H < 1 || !(lambda >= 0.0f) || !(lambda <= 1.0f))
+        return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_loss_l1_ssim_noalloc: W x H = %d x %d, lambda = %g", W, H, (double)lambda);
+    if ((uint64_t)W * (uint64_t)H > (uint64_t)HYRF_LOSS_NOALLOC_MAX_PIXELS)
+        return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_loss_l1_ssim_noalloc: %d x %d = %llu pixels exceed the built-in scratch of %u pixels "
+                       "(HYRF_LOSS_NOALLOC_MAX_PIXELS); use hyrf_loss_l1_ssim", W, H, (unsigned long long)W * (unsigned long long)H,
+                       (unsigned)HYRF_LOSS_NOALLOC_MAX_PIXELS);
+    cudaError_t e;
+    if ((e = cudaSetDevice(device)) != cudaSuccess) return hy_cuda_fail(e, "cudaSetDevice");
+    float* scratch = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_noalloc_mu);
+        if (!g_noalloc_ptr[device]) {
+            void* p = nullptr;
+            if ((e = cudaGetSymbolAddress(&p, g_loss_scratch)) != cudaSuccess) return hy_cuda_fail(e, "cudaGetSymbolAddress(g_loss_scratch)");
+            g_noalloc_ptr[device] = static_cast<float*>(p);
+        }
+        scratch = g_noalloc_ptr[device];
+    }
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    float win[11], sum = 0.0f;
+    for (int k = 0; k < 11; ++k) { win[k] = expf(-(float)((k - 5) * (k - 5)) / (2.0f * 1.5f * 1.5f)); sum += win[k]; }
+    for (int k = 0; k < 11; ++k) win[k] /= sum;
+    if ((e = cudaMemcpyToSymbolAsync(c_win, win, sizeof(win), 0, cudaMemcpyHostToDevice, st)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpyToSymbol");
+    double* dloss = reinterpret_cast<double*>(scratch);   // [0, 4): the loss accumulator; the three maps follow
+    float* maps = scratch + 4;
+    if ((e = cudaMemsetAsync(dloss, 0, sizeof(double), st)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemsetAsync(loss)");
+    const dim3 grid((W + 15) / 16, (H + 15) / 16, 3);
+    ssim_maps_kernel<<<grid, 256, 0, st>>>(image, target, W, H, lambda, maps, dloss);
+    if (g_image) ssim_grad_kernel<<<grid, 256, 0, st>>>(image, target, W, H, lambda, maps, g_image);
+    if ((e = cudaGetLastError()) != cudaSuccess) return hy_cuda_fail(e, "ssim kernels");
+    double l = 0.0;
+    if ((e = cudaMemcpyAsync(&l, dloss, sizeof(double), cudaMemcpyDeviceToHost, st)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpyAsync(loss)");
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(loss)");
     *loss_host = l + (double)lambda;   // the kernels summed (1 - lambda) L1 - lambda SSIM
     return HYRF_OK;
 }
