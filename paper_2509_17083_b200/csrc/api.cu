@@ -633,9 +633,27 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     // the fields), so the five small, latency-bound sort kernels run on their own stream beside the field kernel,
     // which leaves a few SMs free for them (hy_launch_field_*), and join the frame before the binning.
     uint32_t *order_key = nullptr, *order = nullptr;
+    // every visible Gaussian has Z > z_near > 0, so its key (the bits of Z) is above the bits of z_near: the sort works on
+    // the difference, which needs fewer digits (radix.cu). Without pre-culling (ablation) any Z can occur: plain keys.
+    uint32_t depth_key_sub = 0;
+    int depth_key_bits = 32;
+    if (!(f.ablation & HYRF_ABL_NO_CULL)) {
+        memcpy(&depth_key_sub, &f.z_near, sizeof(uint32_t));
+        // Z = r3 . p + t_z <= |r3| r_max + |t_z| (1 % and one float step above the three binary32 fmas that compute it):
+        // the keys to sort lie in (bits(z_near), bits(bound)], a range that normally fits 27 bits = three digits
+        const double r3 = sqrt((double)f.R[6] * f.R[6] + (double)f.R[7] * f.R[7] + (double)f.R[8] * f.R[8]);
+        const double zb = (r3 * s->r_max + fabs((double)f.t[2])) * 1.01;
+        if (zb < 1e37) {
+            const float zf = nextafterf((float)zb, INFINITY);
+            uint32_t top;
+            memcpy(&top, &zf, sizeof(uint32_t));
+            depth_key_bits = 1;
+            while (depth_key_bits < 32 && (top > depth_key_sub ? top - depth_key_sub : 0u) >> depth_key_bits) ++depth_key_bits;
+        }
+    }
     if (overlap) {
-        hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, P.hist,
-                        P.scan, pst, &order_key, &order, &launches, /*iota_vals=*/true);
+        hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, depth_key_bits, P.hist,
+                        P.scan, pst, &order_key, &order, &launches, /*iota_vals=*/true, depth_key_sub);
         if ((e = cudaEventRecord(s->ev_sorted, pst)) != cudaSuccess) return hy_cuda_fail(e, "cudaEventRecord(sorted)");
     }
     // In a pipelined stream the sort has the previous frame's rasterizer to hide under, so the field kernel takes every
@@ -663,8 +681,8 @@ hyrf_status render_impl(hyrf_scene* s, const hyrf_camera* cam, int32_t W, int32_
     if (overlap) {
         if ((e = cudaStreamWaitEvent(s->stream, s->ev_sorted, 0)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamWaitEvent(sorted)");
     } else {
-        hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, 32, P.hist,
-                        P.scan, s->stream, &order_key, &order, &launches, /*iota_vals=*/true);
+        hy_launch_radix(s->sort_a_key, s->sort_a_val, s->sort_b_key, s->sort_b_val, s->N, &s->counters->V, depth_key_bits, P.hist,
+                        P.scan, s->stream, &order_key, &order, &launches, /*iota_vals=*/true, depth_key_sub);
     }
     const uint32_t n_tiles = (uint32_t)(f.gx * f.gy);
     uint32_t V = 0;

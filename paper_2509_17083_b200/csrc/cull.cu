@@ -41,6 +41,20 @@ __global__ void morton_code_kernel(const float* __restrict__ pos, uint32_t N, Fr
     id[i] = i;
 }
 
+// max |p|^2 over the Gaussians, as the bits of a non-negative float (their integer order is the float order); NaN
+// positions never win a comparison (they are never visible either: Eq. 9 is false for them)
+__global__ void max_norm2_kernel(const float* __restrict__ pos, uint32_t N, uint32_t* __restrict__ out_bits) {
+    float m = 0.0f;
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+        const float x = pos[i], y = pos[N + i], z = pos[2ull * N + i];
+        const float d = x * x + y * y + z * z;
+        if (d > m) m = d;
+    }
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(out_bits, __float_as_uint(m));
+}
+
 // gm[m] = (pos.xyz, scale | opacity, rgb) of the m-th Gaussian in Morton order; gm_id[m] = its id
 __global__ void morton_gather_kernel(const uint32_t* __restrict__ order, const float* __restrict__ pos,
                                      const float* __restrict__ rgb, const float* __restrict__ scale,
@@ -204,6 +218,17 @@ hyrf_status hy_prepare_morton(hyrf_scene* s) {
                                                                  s->gm_id);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return hy_cuda_fail(e, "hy_prepare_morton");
+    // r_max = max |p|: every camera-space depth is then bounded on the host (|Z| <= |r3| r_max + |t_z|), which tells the
+    // depth sort of a frame how many key bits it has to look at (api.cu)
+    uint32_t bits = 0;
+    uint32_t* word = s->block_counts;   // (the cull's scratch: idle during an upload)
+    if ((e = cudaMemsetAsync(word, 0, sizeof(uint32_t), s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemsetAsync(r_max)");
+    max_norm2_kernel<<<s->sm_count * 4, 256, 0, s->stream>>>(s->pos, N, word);
+    if ((e = cudaMemcpyAsync(&bits, word, sizeof(uint32_t), cudaMemcpyDeviceToHost, s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemcpyAsync(r_max)");
+    if ((e = cudaStreamSynchronize(s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaStreamSynchronize(r_max)");
+    float n2;
+    memcpy(&n2, &bits, sizeof(float));
+    s->r_max = sqrt((double)n2) * (1.0 + 1e-6);
     return HYRF_OK;
 }
 

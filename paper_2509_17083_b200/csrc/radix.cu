@@ -1,4 +1,4 @@
-// radix.cu — stable LSD radix sort of (uint32 key, uint32 value) pairs, 8 bits per pass, only the key bits in use.
+// radix.cu — stable LSD radix sort of (uint32 key, uint32 value) pairs, 9 bits per pass, only the key bits in use.
 // S4c of the pass (PAPER.md:47 "ordered by depth", :57): the order (tile, depth bits, id) of DESIGN.md §2 D9 is
 // produced by two stable sorts — Gaussians by depth bits (ties keep id order because the compaction is stable),
 // then tile entries by tile id.
@@ -7,6 +7,15 @@
 // decoupled look-back over earlier tickets, re-orders the tile in shared memory and writes digit runs coalesced.
 // The digit histograms of all passes come from one upfront kernel. HBM traffic per pass = read 8 B + write 8 B per
 // pair, the minimum for an out-of-place pass.
+//
+// Two things keep the number of real passes at three for the depth sort of a frame, which runs beside the field
+// kernel on the few SMs that kernel leaves (every pass costs the frame SM-microseconds):
+//   * the digits are those of (key - key_sub) with key_sub <= every key (the depth sort passes the bits of z_near: the
+//     keys are the bits of depths Z > z_near, positive floats, whose order as integers is their order as floats);
+//     a depth range of 2^16 : 1 then fits 27 bits = three 9-bit digits whatever the absolute depths are;
+//   * a pass whose digit is the same for every key (seen in its histogram: one bin holds all n) permutes nothing; its
+//     blocks copy their tile and leave (no ranking, no look-back). Four passes are always launched for 32-bit keys,
+//     the fourth normally being such a copy.
 #include "scene.h"
 
 namespace {
@@ -16,16 +25,19 @@ constexpr int kRadixPer = 16;
 constexpr int kRadixItems = kRadixThreads * kRadixPer;  // 4096 pairs per block
 constexpr int kWarps = kRadixThreads / 32;
 constexpr int kWarpItems = kRadixItems / kWarps;        // 512 consecutive pairs per warp
-constexpr int kMaxPasses = 4;
+constexpr int kDigitBits = 9;
+constexpr int kBins = 1 << kDigitBits;                  // 512: thread t owns the adjacent bins 2t, 2t + 1
+constexpr int kMaxPasses = 4;                           // 36 bits >= 32
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kValMask = (1u << 30) - 1u;
 constexpr size_t kStateBudgetElems = (8u << 20) / 4;    // keep one state slice per pass while they fit in 8 MB
 
-// workspace (uint32 elements): [0, 1024) global digit histograms [pass][256]; [1024, 1028) tickets; [1040, ...) states
-constexpr size_t kWsHist = 0, kWsTicket = kMaxPasses * 256, kWsState = kWsTicket + 16;
+// workspace (uint32 elements): [0, 2048) global digit histograms [pass][512]; [2048, 2052) tickets; [2064, ...) states
+constexpr size_t kWsHist = 0, kWsTicket = kMaxPasses * kBins, kWsState = kWsTicket + 16;
 
-// exclusive scan of one value per thread over the 256 threads of the block
-__device__ __forceinline__ uint32_t block_scan256(uint32_t v, uint32_t* warp_sums /*[8]*/) {
+// exclusive scan over the 512 bins, two adjacent bins (v0, v1) per thread: returns the exclusive prefix of v0
+__device__ __forceinline__ uint32_t block_scan_pairs(uint32_t v0, uint32_t v1, uint32_t* warp_sums /*[8]*/) {
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t v = v0 + v1;
     uint32_t incl = v;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -43,120 +55,189 @@ __device__ __forceinline__ uint32_t block_scan256(uint32_t v, uint32_t* warp_sum
 
 // digit histograms of every pass in one read of the keys
 __global__ void __launch_bounds__(kRadixThreads)
-radix_global_hist_kernel(const uint32_t* __restrict__ keys, size_t n_cap, const uint32_t* __restrict__ n_dev,
-                         int passes, int key_bits, uint32_t* __restrict__ ghist) {
-    __shared__ uint32_t h[kMaxPasses][256];
-    const size_t n = n_dev ? (size_t)*n_dev : n_cap;
-    for (int p = 0; p < passes; ++p) h[p][threadIdx.x] = 0;
+radix_global_hist_kernel(const uint32_t* __restrict__ keys, uint32_t n_cap, const uint32_t* __restrict__ n_dev,
+                         int passes, uint32_t key_sub, uint32_t* __restrict__ ghist) {
+    __shared__ uint32_t h[kMaxPasses][kBins];
+    const uint32_t n = n_dev ? *n_dev : n_cap;
+    for (int i = threadIdx.x; i < passes * kBins; i += kRadixThreads) (&h[0][0])[i] = 0;
     __syncthreads();
-    for (size_t base = (size_t)blockIdx.x * kRadixItems; base < n; base += (size_t)gridDim.x * kRadixItems) {
+    const uint32_t lane = threadIdx.x & 31;
+    for (uint32_t base = blockIdx.x * kRadixItems; base < n; base += gridDim.x * kRadixItems) {
 #pragma unroll 4
         for (int k = 0; k < kRadixPer; ++k) {
-            const size_t i = base + (size_t)k * kRadixThreads + threadIdx.x;
-            if (i < n) {
-                const uint32_t key = keys[i];
-                for (int p = 0; p < passes; ++p) {
-                    const int bits = key_bits - 8 * p < 8 ? key_bits - 8 * p : 8;
-                    atomicAdd(&h[p][(key >> (8 * p)) & ((1u << bits) - 1u)], 1u);
+            const uint32_t i = base + k * kRadixThreads + threadIdx.x;
+            const bool in = i < n;
+            const uint32_t key = in ? keys[i] - key_sub : 0u;
+            for (int p = 0; p < passes; ++p) {
+                const uint32_t d = (key >> (kDigitBits * p)) & (kBins - 1);
+                // the high digits are often the same for a whole warp (depths share their exponent; the top digit is
+                // usually 0 for every key): one add for the warp instead of 32 serialised ones on the same address
+                bool uniform = false;
+                uint32_t bal = 0;
+                if (p >= 2) {   // (p is uniform; every lane takes part in the three warp operations)
+                    bal = __ballot_sync(0xffffffffu, in);
+                    const uint32_t d_first = __shfl_sync(0xffffffffu, d, __ffs(bal | 0x80000000u) - 1);
+                    uniform = __all_sync(0xffffffffu, !in || d == d_first);
+                }
+                if (uniform) {
+                    if (bal && lane == (uint32_t)(__ffs(bal) - 1)) atomicAdd(&h[p][d], (uint32_t)__popc(bal));
+                } else if (in) {
+                    atomicAdd(&h[p][d], 1u);
                 }
             }
         }
     }
     __syncthreads();
-    for (int p = 0; p < passes; ++p) {
-        const uint32_t c = h[p][threadIdx.x];
-        if (c) atomicAdd(&ghist[p * 256 + threadIdx.x], c);
+    for (int i = threadIdx.x; i < passes * kBins; i += kRadixThreads) {
+        const uint32_t c = (&h[0][0])[i];
+        if (c) atomicAdd(&ghist[i], c);
     }
 }
 
-__global__ void __launch_bounds__(kRadixThreads)
-radix_onesweep_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
-                      uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out, size_t n_cap,
-                      const uint32_t* __restrict__ n_dev, int shift, uint32_t mask, const uint32_t* __restrict__ ghist,
-                      uint32_t* __restrict__ ticket, volatile uint32_t* __restrict__ state) {
-    __shared__ uint32_t cnt[kWarps][256];
-    __shared__ uint32_t s_key[kRadixItems];
-    __shared__ uint32_t s_val[kRadixItems];
-    __shared__ uint32_t s_delta[256];
-    __shared__ uint32_t s_warp[kWarps];
-    __shared__ uint32_t s_tile;
-    const size_t n = n_dev ? (size_t)*n_dev : n_cap;
-    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
-    for (int d = threadIdx.x; d < kWarps * 256; d += kRadixThreads) (&cnt[0][0])[d] = 0;
-    __syncthreads();
-    const uint32_t tile = s_tile;
-    const size_t base = (size_t)tile * kRadixItems;
-    if (base >= n) return;   // tickets are handed out in order: every earlier tile exists and is running or done
-    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+__device__ __forceinline__ unsigned long long ld_state(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_state(unsigned long long* p, uint32_t a, uint32_t b) {
+    asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"((unsigned long long)a | ((unsigned long long)b << 32)) : "memory");
+}
 
-    uint32_t key[kRadixPer], val[kRadixPer], packed[kRadixPer];
-    const size_t wbase = base + (size_t)warp * kWarpItems;
+// ranks of the 16 rows of a warp's 512 keys within the warp, per digit (stable): packed[k] = digit << 16 | rank.
+// FULL: every key of the tile exists (no validity predicates in the ballots).
+template <bool FULL>
+__device__ __forceinline__ void rank_rows(const uint32_t (&key)[kRadixPer], uint32_t (&packed)[kRadixPer], uint32_t key_sub,
+                                          int shift, uint32_t wbase, uint32_t n, uint32_t lane, unsigned short* cw) {
+    const uint32_t below = (1u << lane) - 1u;
 #pragma unroll
     for (int k = 0; k < kRadixPer; ++k) {
-        const size_t i = wbase + (size_t)k * 32 + lane;
-        const bool valid = i < n;
-        key[k] = valid ? keys_in[i] : 0u;
-        val[k] = valid ? (vals_in ? vals_in[i] : (uint32_t)i) : 0u;   // no values yet: the value is the index
-    }
+        const bool valid = FULL || wbase + (uint32_t)k * 32u + lane < n;
+        const uint32_t d = ((key[k] - key_sub) >> shift) & (kBins - 1);
+        // lanes holding the same digit, from one ballot per digit bit: match.any costs several times that when most
+        // lanes of a warp hold distinct digits, which is the rule for the low bits of depth keys
+        uint32_t peers = FULL ? 0xffffffffu : __ballot_sync(0xffffffffu, valid);
 #pragma unroll
-    for (int k = 0; k < kRadixPer; ++k) {
-        const bool valid = wbase + (size_t)k * 32 + lane < n;
-        const uint32_t d = (key[k] >> shift) & mask;
-        // lanes holding the same digit, from one ballot per digit bit: 9 VOTE + 16 logic instructions. match.any costs
-        // several times that when most lanes of a warp hold distinct digits, which is the rule for the low bytes of
-        // depth keys; beside the field kernel, on the few SMs it leaves, a pass went from 101 to 74 us (config 3)
-        uint32_t peers = __ballot_sync(0xffffffffu, valid);
-#pragma unroll
-        for (int b = 0; b < 8; ++b) {
+        for (int b = 0; b < kDigitBits; ++b) {
             const bool bit = (d >> b) & 1u;
             const uint32_t bal = __ballot_sync(0xffffffffu, bit);
             peers &= bit ? bal : ~bal;
         }
         uint32_t c = 0;
-        if (valid) c = cnt[warp][d];
+        if (valid) c = cw[d];
         __syncwarp();
-        if (valid && lane == (uint32_t)(__ffs(peers) - 1)) cnt[warp][d] = c + __popc(peers);
+        if (valid && (peers & below) == 0u) cw[d] = (unsigned short)(c + __popc(peers));   // the lowest peer writes
         __syncwarp();
-        packed[k] = valid ? ((d << 16) | (c + __popc(peers & ((1u << lane) - 1u)))) : 0xffffffffu;
+        packed[k] = valid ? ((d << 16) | (c + __popc(peers & below))) : 0xffffffffu;
+    }
+}
+
+#ifndef HY_RADIX_MINB
+#define HY_RADIX_MINB 3
+#endif
+__global__ void __launch_bounds__(kRadixThreads, HY_RADIX_MINB)
+radix_onesweep_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
+                      uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out, uint32_t n_cap,
+                      const uint32_t* __restrict__ n_dev, int shift, uint32_t key_sub, const uint32_t* __restrict__ ghist,
+                      uint32_t* __restrict__ ticket, unsigned long long* __restrict__ state) {
+    __shared__ unsigned short cnt[kWarps][kBins];   // per warp and digit: count, then first slot in the re-ordered tile
+    __shared__ uint32_t s_key[kRadixItems];
+    __shared__ uint32_t s_val[kRadixItems];
+    __shared__ uint32_t s_delta[kBins];
+    __shared__ uint32_t s_warp[kWarps];
+    __shared__ uint32_t s_tile;
+    const uint32_t n = n_dev ? *n_dev : n_cap;
+    const uint32_t t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    const uint2 gh = *reinterpret_cast<const uint2*>(ghist + 2 * t);   // the whole array's counts of this thread's two digits
+    // one digit for every key: this pass permutes nothing. Copy the tile (tickets and look-back are not needed)
+    if (__syncthreads_or((gh.x == n) | (gh.y == n))) {
+        const uint32_t base = blockIdx.x * kRadixItems;
+#pragma unroll 4
+        for (int k = 0; k < kRadixPer; ++k) {
+            const uint32_t i = base + k * kRadixThreads + t;
+            if (i < n) {
+                keys_out[i] = keys_in[i];
+                vals_out[i] = vals_in ? vals_in[i] : i;
+            }
+        }
+        return;
+    }
+    if (t == 0) s_tile = atomicAdd(ticket, 1u);
+    for (int d = t; d < kWarps * kBins / 2; d += kRadixThreads) reinterpret_cast<uint32_t*>(&cnt[0][0])[d] = 0;
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const uint32_t base = tile * kRadixItems;
+    if (base >= n) return;   // tickets are handed out in order: every earlier tile exists and is running or done
+    const bool full = base + kRadixItems <= n;
+
+    uint32_t key[kRadixPer], val[kRadixPer], packed[kRadixPer];
+    const uint32_t wbase = base + warp * kWarpItems;
+    if (full) {
+#pragma unroll
+        for (int k = 0; k < kRadixPer; ++k) {
+            const uint32_t i = wbase + k * 32 + lane;
+            key[k] = keys_in[i];
+            val[k] = vals_in ? vals_in[i] : i;   // no values yet: the value is the index
+        }
+        rank_rows<true>(key, packed, key_sub, shift, wbase, n, lane, cnt[warp]);
+    } else {
+#pragma unroll
+        for (int k = 0; k < kRadixPer; ++k) {
+            const uint32_t i = wbase + k * 32 + lane;
+            const bool valid = i < n;
+            key[k] = valid ? keys_in[i] : 0u;
+            val[k] = valid ? (vals_in ? vals_in[i] : i) : 0u;
+        }
+        rank_rows<false>(key, packed, key_sub, shift, wbase, n, lane, cnt[warp]);
     }
     __syncthreads();
-    // thread d owns digit d: exclusive scan over the warps, block total, publish, look back
-    const uint32_t d = threadIdx.x;
-    uint32_t total = 0;
+    // thread t owns digits 2t, 2t + 1: exclusive scan over the warps, block totals, publish, look back
+    uint32_t total[2] = {0u, 0u};
 #pragma unroll
     for (int w = 0; w < kWarps; ++w) {
-        const uint32_t t = cnt[w][d];
-        cnt[w][d] = total;
-        total += t;
+        const uint32_t c2 = *reinterpret_cast<const uint32_t*>(&cnt[w][2 * t]);
+        *reinterpret_cast<uint32_t*>(&cnt[w][2 * t]) = total[0] | (total[1] << 16);
+        total[0] += c2 & 0xFFFFu;
+        total[1] += c2 >> 16;
     }
-    state[(size_t)tile * 256 + d] = total | (tile == 0 ? kFlagIncl : kFlagAgg);
-    const uint32_t gexcl = block_scan256(ghist[d], s_warp);      // first output slot of digit d over the whole array
-    const uint32_t dstart = block_scan256(total, s_warp);        // first slot of digit d inside this tile
-    uint32_t prefix = 0;
+    unsigned long long* const my_state = state + (size_t)tile * (kBins / 2) + t;
+    const uint32_t flag0 = tile == 0 ? kFlagIncl : kFlagAgg;
+    st_state(my_state, total[0] | flag0, total[1] | flag0);
+    const uint32_t gexcl = block_scan_pairs(gh.x, gh.y, s_warp);          // first output slot of digit 2t over the whole array
+    const uint32_t dstart = block_scan_pairs(total[0], total[1], s_warp); // first slot of digit 2t inside this tile
+    uint32_t prefix[2] = {0u, 0u};
     if (tile > 0) {
-        // look back 16 predecessors per round trip: the loads of a round are independent, so the latency of the
-        // walk is paid once per 16 tiles instead of once per tile
-        constexpr int kLook = 16;
-        long long p = (long long)tile - 1;
-        bool found = false;
-        while (!found) {
-            uint32_t v[kLook];
+        // look back 8 predecessors per round trip: the loads of a round are independent, so the latency of the walk is
+        // paid once per 8 tiles instead of once per tile
+        constexpr int kLook = 8;
+        int p = (int)tile - 1;
+        bool found0 = false, found1 = false;
+        while (!(found0 && found1)) {
+            unsigned long long v[kLook];
 #pragma unroll
-            for (int i = 0; i < kLook; ++i) v[i] = (p - i >= 0) ? state[(size_t)(p - i) * 256 + d] : (2u << 30);
+            for (int i = 0; i < kLook; ++i)
+                v[i] = (p - i >= 0) ? ld_state(state + (size_t)(p - i) * (kBins / 2) + t) : (((unsigned long long)kFlagIncl << 32) | kFlagIncl);
 #pragma unroll
             for (int i = 0; i < kLook; ++i) {
-                if (found) continue;
-                while ((v[i] >> 30) == 0u) v[i] = state[(size_t)(p - i) * 256 + d];
-                prefix += v[i] & kValMask;
-                found = (v[i] >> 30) == 2u;
+                if (found0 && found1) continue;
+                uint32_t a = (uint32_t)v[i], b = (uint32_t)(v[i] >> 32);
+                while ((!found0 && (a >> 30) == 0u) || (!found1 && (b >> 30) == 0u)) {
+                    const unsigned long long r = ld_state(state + (size_t)(p - i) * (kBins / 2) + t);
+                    a = (uint32_t)r; b = (uint32_t)(r >> 32);
+                }
+                if (!found0) { prefix[0] += a & kValMask; found0 = (a >> 30) == 2u; }
+                if (!found1) { prefix[1] += b & kValMask; found1 = (b >> 30) == 2u; }
             }
             p -= kLook;
         }
-        state[(size_t)tile * 256 + d] = ((prefix + total) & kValMask) | kFlagIncl;
+        st_state(my_state, ((prefix[0] + total[0]) & kValMask) | kFlagIncl, ((prefix[1] + total[1]) & kValMask) | kFlagIncl);
     }
-    s_delta[d] = gexcl + prefix - dstart;
+    s_delta[2 * t] = gexcl + prefix[0] - dstart;
+    s_delta[2 * t + 1] = gexcl + gh.x + prefix[1] - (dstart + total[0]);
+    {
+        const uint32_t add = dstart | ((dstart + total[0]) << 16);   // (no carry between the halves: slots < 4096)
 #pragma unroll
-    for (int w = 0; w < kWarps; ++w) cnt[w][d] += dstart;
+        for (int w = 0; w < kWarps; ++w) *reinterpret_cast<uint32_t*>(&cnt[w][2 * t]) += add;
+    }
     __syncthreads();
     // re-order the tile in shared memory, then write digit runs
 #pragma unroll
@@ -168,54 +249,54 @@ radix_onesweep_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __re
         }
     }
     __syncthreads();
-    const uint32_t count = (uint32_t)((n - base) < (size_t)kRadixItems ? (n - base) : (size_t)kRadixItems);
+    const uint32_t count = n - base < (uint32_t)kRadixItems ? n - base : (uint32_t)kRadixItems;
 #pragma unroll
     for (int k = 0; k < kRadixPer; ++k) {
-        const uint32_t i = k * kRadixThreads + threadIdx.x;
+        const uint32_t i = k * kRadixThreads + t;
         if (i < count) {
             const uint32_t kk = s_key[i];
-            const uint32_t pos = i + s_delta[(kk >> shift) & mask];
+            const uint32_t pos = i + s_delta[((kk - key_sub) >> shift) & (kBins - 1)];
             keys_out[pos] = kk;
             vals_out[pos] = s_val[i];
         }
     }
 }
 
-size_t state_slices(size_t nb) { return (nb * 256 * kMaxPasses <= kStateBudgetElems) ? kMaxPasses : 1; }
+size_t state_slices(size_t nb) { return (nb * kBins * kMaxPasses <= kStateBudgetElems) ? kMaxPasses : 1; }
 
 }  // namespace
 
 size_t hy_radix_hist_elems(size_t n_cap) {
     const size_t nb = (n_cap + kRadixItems - 1) / kRadixItems + 1;
-    const size_t one = nb * 256;
+    const size_t one = nb * kBins;
     return kWsState + (one > kStateBudgetElems ? one : kStateBudgetElems) + 64;
 }
 
 // Largest pair count one sort call supports (30-bit digit prefixes in the look-back words).
 size_t hy_radix_max_items() { return (size_t)kValMask; }
 
+// key_sub: a value no key is below; the digits are those of key - key_sub (see the head of this file). 0 = plain keys.
 void hy_launch_radix(uint32_t* key_a, uint32_t* val_a, uint32_t* key_b, uint32_t* val_b, size_t n_cap,
                      const uint32_t* n_dev, int key_bits, uint32_t* ws, uint32_t* /*scan_scratch*/, cudaStream_t st,
-                     uint32_t** out_key, uint32_t** out_val, uint32_t* launches, bool iota_vals) {
+                     uint32_t** out_key, uint32_t** out_val, uint32_t* launches, bool iota_vals, uint32_t key_sub) {
     uint32_t *ki = key_a, *vi = val_a, *ko = key_b, *vo = val_b;
     if (n_cap > 0 && key_bits > 0) {
         const size_t nb = (n_cap + kRadixItems - 1) / kRadixItems;
-        const int passes = (key_bits + 7) / 8;
+        const int passes = (key_bits + kDigitBits - 1) / kDigitBits;
         const size_t slices = state_slices(nb + 1);
-        const size_t slice = (nb + 1) * 256;
+        const size_t slice = (nb + 1) * kBins;
         cudaMemsetAsync(ws, 0, (kWsState + (slices > 1 ? (size_t)passes * slice : 0)) * sizeof(uint32_t), st);
         int dev = 0, sms = 0;   // grid-stride histogram: one wave of resident CTAs
         if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) sms = 1;
         const unsigned hgrid = (unsigned)(nb < (size_t)sms * 8 ? nb : (size_t)sms * 8);
-        radix_global_hist_kernel<<<hgrid, kRadixThreads, 0, st>>>(ki, n_cap, n_dev, passes, key_bits, ws + kWsHist);
+        radix_global_hist_kernel<<<hgrid, kRadixThreads, 0, st>>>(ki, (uint32_t)n_cap, n_dev, passes, key_sub, ws + kWsHist);
         ++*launches;
         for (int p = 0; p < passes; ++p) {
-            const int bits = key_bits - 8 * p < 8 ? key_bits - 8 * p : 8;
             uint32_t* state = ws + kWsState + (slices > 1 ? (size_t)p * slice : 0);
             if (slices == 1) cudaMemsetAsync(state, 0, slice * sizeof(uint32_t), st);
-            radix_onesweep_kernel<<<(unsigned)nb, kRadixThreads, 0, st>>>(ki, (p == 0 && iota_vals) ? nullptr : vi, ko, vo, n_cap, n_dev, 8 * p,
-                                                                         (1u << bits) - 1u, ws + kWsHist + p * 256,
-                                                                         ws + kWsTicket + p, state);
+            radix_onesweep_kernel<<<(unsigned)nb, kRadixThreads, 0, st>>>(ki, (p == 0 && iota_vals) ? nullptr : vi, ko, vo, (uint32_t)n_cap, n_dev,
+                                                                         kDigitBits * p, key_sub, ws + kWsHist + p * kBins,
+                                                                         ws + kWsTicket + p, reinterpret_cast<unsigned long long*>(state));
             ++*launches;
             uint32_t* t = ki; ki = ko; ko = t;
             t = vi; vi = vo; vo = t;

@@ -44,7 +44,8 @@ struct hyrf_scene {
     bool field_attr_set = false;   // cudaFuncSetAttribute of the tensor-core field kernels done for this scene's device
     bool field_ws_attr_set = false;
     bool ws_mma = false;       // decoders on tcgen05 with warp-specialised gather / decoder roles (field_ws.cu)
-    int ws_sort_sms = 24;      // SMs the warp-specialised field kernel leaves to the depth sort running beside it (swept 12..40 on configs 3, 4, 5: DESIGN.md section 11)
+    double r_max = INFINITY;   // max |position| over the Gaussians (hy_prepare_morton): bounds every camera-space depth
+    int ws_sort_sms = 16;      // SMs the warp-specialised field kernel leaves to the depth sort running beside it (swept 12..40 on configs 3, 4, 5: DESIGN.md section 11)
 
     // persistent parameters
     float* pos = nullptr;      // [3][N]
@@ -185,7 +186,8 @@ size_t hy_radix_hist_elems(size_t n_cap);
 size_t hy_radix_max_items();
 void hy_launch_radix(uint32_t* key_a, uint32_t* val_a, uint32_t* key_b, uint32_t* val_b, size_t n_cap,
                      const uint32_t* n_dev, int key_bits, uint32_t* hist, uint32_t* scan_scratch, cudaStream_t st,
-                     uint32_t** out_key, uint32_t** out_val, uint32_t* launches, bool iota_vals = false);
+                     uint32_t** out_key, uint32_t** out_val, uint32_t* launches, bool iota_vals = false,
+                     uint32_t key_sub = 0);
 // S4b-c (bin.cu)
 void hy_launch_tiles_gather(hyrf_scene* s, const uint32_t* order, uint32_t V, uint32_t* launches);
 void hy_launch_emit(hyrf_scene* s, const uint32_t* order, uint32_t V, uint32_t* launches);
