@@ -28,11 +28,14 @@ constexpr int kWarpItems = kRadixItems / kWarps;        // 512 consecutive pairs
 constexpr int kDigitBits = 9;
 constexpr int kBins = 1 << kDigitBits;                  // 512: thread t owns the adjacent bins 2t, 2t + 1
 constexpr int kMaxPasses = 4;                           // 36 bits >= 32
-constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kValMask = (1u << 30) - 1u;
-constexpr size_t kStateBudgetElems = (8u << 20) / 4;    // keep one state slice per pass while they fit in 8 MB
+constexpr uint32_t kValMask = (1u << 30) - 1u;            // largest pair count of one sort (32-bit indices with room to spare)
 
-// workspace (uint32 elements): [0, 2048) global digit histograms [pass][512]; [2048, 2052) tickets; [2064, ...) states
-constexpr size_t kWsHist = 0, kWsTicket = kMaxPasses * kBins, kWsState = kWsTicket + 16;
+// workspace (uint32 elements): [0, 2048) global digit histograms [pass][512]; [2048, 2052) tickets; then one status word
+// per tile and pass (these three are cleared per sort), the tiles' digit counts (two 16-bit counts per word) and their
+// inclusive prefixes (rows of 512 words) — both reused by every pass: a row is only read once its tile's status word
+// of the current pass says so
+constexpr size_t kWsHist = 0, kWsTicket = kMaxPasses * kBins, kWsFlags = kWsTicket + 16;
+size_t tiles_padded(size_t n_cap) { return ((n_cap + kRadixItems - 1) / kRadixItems + 1 + 31) / 32 * 32; }
 
 // exclusive scan over the 512 bins, two adjacent bins (v0, v1) per thread: returns the exclusive prefix of v0
 __device__ __forceinline__ uint32_t block_scan_pairs(uint32_t v0, uint32_t v1, uint32_t* warp_sums /*[8]*/) {
@@ -94,14 +97,12 @@ radix_global_hist_kernel(const uint32_t* __restrict__ keys, uint32_t n_cap, cons
     }
 }
 
-__device__ __forceinline__ unsigned long long ld_state(const unsigned long long* p) {
-    unsigned long long v;
-    asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+__device__ __forceinline__ uint32_t ld_flag(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void st_state(unsigned long long* p, uint32_t a, uint32_t b) {
-    asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"((unsigned long long)a | ((unsigned long long)b << 32)) : "memory");
-}
+__device__ __forceinline__ void st_flag(uint32_t* p, uint32_t v) { asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory"); }
 
 // ranks of the 16 rows of a warp's 512 keys within the warp, per digit (stable): packed[k] = digit << 16 | rank.
 // FULL: every key of the tile exists (no validity predicates in the ballots).
@@ -138,13 +139,13 @@ __global__ void __launch_bounds__(kRadixThreads, HY_RADIX_MINB)
 radix_onesweep_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
                       uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out, uint32_t n_cap,
                       const uint32_t* __restrict__ n_dev, int shift, uint32_t key_sub, const uint32_t* __restrict__ ghist,
-                      uint32_t* __restrict__ ticket, unsigned long long* __restrict__ state) {
+                      uint32_t* __restrict__ ticket, uint32_t* __restrict__ flags, uint32_t* __restrict__ agg, uint2* __restrict__ incl) {
     __shared__ unsigned short cnt[kWarps][kBins];   // per warp and digit: count, then first slot in the re-ordered tile
     __shared__ uint32_t s_key[kRadixItems];
     __shared__ uint32_t s_val[kRadixItems];
     __shared__ uint32_t s_delta[kBins];
     __shared__ uint32_t s_warp[kWarps];
-    __shared__ uint32_t s_tile;
+    __shared__ uint32_t s_tile, s_back;
     const uint32_t n = n_dev ? *n_dev : n_cap;
     const uint32_t t = threadIdx.x, lane = t & 31, warp = t >> 5;
     const uint2 gh = *reinterpret_cast<const uint2*>(ghist + 2 * t);   // the whole array's counts of this thread's two digits
@@ -199,37 +200,52 @@ radix_onesweep_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __re
         total[0] += c2 & 0xFFFFu;
         total[1] += c2 >> 16;
     }
-    unsigned long long* const my_state = state + (size_t)tile * (kBins / 2) + t;
-    const uint32_t flag0 = tile == 0 ? kFlagIncl : kFlagAgg;
-    st_state(my_state, total[0] | flag0, total[1] | flag0);
+    // Decoupled look-back with ONE status word per tile (0 nothing, 1 digit counts of the tile published, 2 inclusive
+    // prefixes published) and plain arrays of counts: a warp finds the nearest predecessor whose inclusive prefixes
+    // are out, then every thread adds that row and the count rows in between for its two digits. (Per-digit status
+    // words made every thread walk and test its own chain: a quarter of the kernel's instructions.)
+    agg[(size_t)tile * (kBins / 2) + t] = total[0] | (total[1] << 16);   // (counts of one tile: <= 4096)
+    if (tile == 0) incl[t] = make_uint2(total[0], total[1]);
+    __threadfence();
     const uint32_t gexcl = block_scan_pairs(gh.x, gh.y, s_warp);          // first output slot of digit 2t over the whole array
+    if (t == 0) st_flag(flags + tile, tile == 0 ? 2u : 1u);                // (after the barriers of the scan: every thread's rows are out)
     const uint32_t dstart = block_scan_pairs(total[0], total[1], s_warp); // first slot of digit 2t inside this tile
     uint32_t prefix[2] = {0u, 0u};
     if (tile > 0) {
-        // look back 8 predecessors per round trip: the loads of a round are independent, so the latency of the walk is
-        // paid once per 8 tiles instead of once per tile
-        constexpr int kLook = 8;
-        int p = (int)tile - 1;
-        bool found0 = false, found1 = false;
-        while (!(found0 && found1)) {
-            unsigned long long v[kLook];
-#pragma unroll
-            for (int i = 0; i < kLook; ++i)
-                v[i] = (p - i >= 0) ? ld_state(state + (size_t)(p - i) * (kBins / 2) + t) : (((unsigned long long)kFlagIncl << 32) | kFlagIncl);
-#pragma unroll
-            for (int i = 0; i < kLook; ++i) {
-                if (found0 && found1) continue;
-                uint32_t a = (uint32_t)v[i], b = (uint32_t)(v[i] >> 32);
-                while ((!found0 && (a >> 30) == 0u) || (!found1 && (b >> 30) == 0u)) {
-                    const unsigned long long r = ld_state(state + (size_t)(p - i) * (kBins / 2) + t);
-                    a = (uint32_t)r; b = (uint32_t)(r >> 32);
+        uint32_t top = tile - 1;   // the look-back window is tiles top, top - 1, ..., top - 31
+        for (;;) {
+            if (warp == 0) {
+                uint32_t back;
+                for (;;) {
+                    const uint32_t fl = lane <= top ? ld_flag(flags + (top - lane)) : 2u;
+                    const uint32_t two = __ballot_sync(0xffffffffu, fl == 2u), zero = __ballot_sync(0xffffffffu, fl == 0u);
+                    const uint32_t first2 = two ? (uint32_t)__ffs(two) - 1u : 32u;            // nearest tile with inclusive prefixes
+                    if ((zero & (first2 < 32u ? (1u << first2) - 1u : 0xffffffffu)) == 0u) { back = first2; break; }   // all in front of it counted
                 }
-                if (!found0) { prefix[0] += a & kValMask; found0 = (a >> 30) == 2u; }
-                if (!found1) { prefix[1] += b & kValMask; found1 = (b >> 30) == 2u; }
+                if (lane == 0) s_back = back;
             }
-            p -= kLook;
+            __syncthreads();
+            const uint32_t back = s_back;
+            __threadfence();
+            const uint32_t n_agg = back < 32u ? back : 32u;
+            for (uint32_t i = 0; i < n_agg; ++i) {
+                const uint32_t v = __ldcg(agg + (size_t)(top - i) * (kBins / 2) + t);
+                prefix[0] += v & 0xFFFFu; prefix[1] += v >> 16;
+            }
+            if (back < 32u) {
+                if (back <= top) {   // (beyond tile 0 the sentinel stands for an all-zero inclusive row)
+                    const uint2 v = __ldcg(incl + (size_t)(top - back) * (kBins / 2) + t);
+                    prefix[0] += v.x; prefix[1] += v.y;
+                }
+                break;
+            }
+            top -= 32u;   // 32 counted tiles and no inclusive one among them: go on further back (top >= 32 here)
+            __syncthreads();
         }
-        st_state(my_state, ((prefix[0] + total[0]) & kValMask) | kFlagIncl, ((prefix[1] + total[1]) & kValMask) | kFlagIncl);
+        incl[(size_t)tile * (kBins / 2) + t] = make_uint2(prefix[0] + total[0], prefix[1] + total[1]);
+        __threadfence();
+        __syncthreads();
+        if (t == 0) st_flag(flags + tile, 2u);
     }
     s_delta[2 * t] = gexcl + prefix[0] - dstart;
     s_delta[2 * t + 1] = gexcl + gh.x + prefix[1] - (dstart + total[0]);
@@ -262,17 +278,14 @@ radix_onesweep_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __re
     }
 }
 
-size_t state_slices(size_t nb) { return (nb * kBins * kMaxPasses <= kStateBudgetElems) ? kMaxPasses : 1; }
-
 }  // namespace
 
 size_t hy_radix_hist_elems(size_t n_cap) {
-    const size_t nb = (n_cap + kRadixItems - 1) / kRadixItems + 1;
-    const size_t one = nb * kBins;
-    return kWsState + (one > kStateBudgetElems ? one : kStateBudgetElems) + 64;
+    const size_t nbp = tiles_padded(n_cap);
+    return kWsFlags + kMaxPasses * nbp + nbp * (kBins / 2) + nbp * kBins + 64;
 }
 
-// Largest pair count one sort call supports (30-bit digit prefixes in the look-back words).
+// Largest pair count one sort call supports.
 size_t hy_radix_max_items() { return (size_t)kValMask; }
 
 // key_sub: a value no key is below; the digits are those of key - key_sub (see the head of this file). 0 = plain keys.
@@ -283,20 +296,19 @@ void hy_launch_radix(uint32_t* key_a, uint32_t* val_a, uint32_t* key_b, uint32_t
     if (n_cap > 0 && key_bits > 0) {
         const size_t nb = (n_cap + kRadixItems - 1) / kRadixItems;
         const int passes = (key_bits + kDigitBits - 1) / kDigitBits;
-        const size_t slices = state_slices(nb + 1);
-        const size_t slice = (nb + 1) * kBins;
-        cudaMemsetAsync(ws, 0, (kWsState + (slices > 1 ? (size_t)passes * slice : 0)) * sizeof(uint32_t), st);
+        const size_t nbp = tiles_padded(n_cap);
+        uint32_t* const agg = ws + kWsFlags + kMaxPasses * nbp;
+        uint2* const incl = reinterpret_cast<uint2*>(agg + nbp * (kBins / 2));
+        cudaMemsetAsync(ws, 0, (kWsFlags + (size_t)passes * nbp) * sizeof(uint32_t), st);
         int dev = 0, sms = 0;   // grid-stride histogram: one wave of resident CTAs
         if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) sms = 1;
         const unsigned hgrid = (unsigned)(nb < (size_t)sms * 8 ? nb : (size_t)sms * 8);
         radix_global_hist_kernel<<<hgrid, kRadixThreads, 0, st>>>(ki, (uint32_t)n_cap, n_dev, passes, key_sub, ws + kWsHist);
         ++*launches;
         for (int p = 0; p < passes; ++p) {
-            uint32_t* state = ws + kWsState + (slices > 1 ? (size_t)p * slice : 0);
-            if (slices == 1) cudaMemsetAsync(state, 0, slice * sizeof(uint32_t), st);
             radix_onesweep_kernel<<<(unsigned)nb, kRadixThreads, 0, st>>>(ki, (p == 0 && iota_vals) ? nullptr : vi, ko, vo, (uint32_t)n_cap, n_dev,
                                                                          kDigitBits * p, key_sub, ws + kWsHist + p * kBins,
-                                                                         ws + kWsTicket + p, reinterpret_cast<unsigned long long*>(state));
+                                                                         ws + kWsTicket + p, ws + kWsFlags + (size_t)p * nbp, agg, incl);
             ++*launches;
             uint32_t* t = ki; ki = ko; ko = t;
             t = vi; vi = vo; vo = t;
