@@ -199,8 +199,8 @@ def stage_rooflines(scene, V, D, Dm, n_bg, eval_pairs, peaks):
 def load_traffic(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` and, for the field kernel, its L1TEX global-load
     sector look-ups per visible Gaussian, from the committed ncu --set full capture of this workload
-    (profiles/r2_dram_traffic.csv, made by the commands in profiles/r2_README.md). (None, None) without a capture."""
-    p = os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")
+    (profiles/r2b_dram_traffic.csv, made by the commands in profiles/r2b_README.md). (None, None) without a capture."""
+    p = os.path.join(ROOT, "profiles", "r2b_dram_traffic.csv")
     if not os.path.exists(p):
         return None, None
     import csv
@@ -624,6 +624,10 @@ def run_ours(args):
         di = names.index(dom)
         roof["serial_launch_ms"] = float(stage_serial_ms[di])
         roof["serial_frac"] = rl[dom]["work"] / (stage_serial_ms[di] * 1e-3) / 1e9 / rl[dom]["peak"]
+    else:
+        # the rasterizer's work is counted in evaluated (pixel, Gaussian) pairs, which only the CPU oracle leg counts
+        roof.update({"bound": "alu", "achieved": None, "peak": None, "unit": "Gslot/s", "frac": None,
+                     "note": "the dominant kernel is the rasterizer; its pair count comes from the cpu_baseline leg (run without --no-cpu / --ablation)"})
     # What actually bounds the field kernel (its tables are L2-resident, DRAM moves a sixth of the algorithmic bytes): the
     # rate at which an SM looks up scattered sectors. Achieved = the kernel's L1TEX global-load sector look-ups (ncu count
     # per visible Gaussian of the committed capture x this run's V) / its launch time; peak = the gather microprobe.
