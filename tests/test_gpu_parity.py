@@ -901,3 +901,24 @@ def test_retained_lists_give_the_export_paths_gradients(B, synth, raster_mode):
         hs.backward(g)
     assert e.value.status == B.HYRF_ERR_NOT_READY
     hs.close()
+
+
+def test_depth_sort_over_a_wide_depth_range(B, ho, synth):
+    # csrc/radix.cu sorts the digits of key - bits(z_near) and the host bounds the key bits per frame from max |position|
+    # (api.cu): depths within 2^16 : 1 of z_near take three passes, wider ranges a fourth. Both cases, and a scene whose
+    # bound changes with a re-upload, against the oracle's per-tile lists bit for bit. The far Gaussians sit on the
+    # optical axis region so that they stay in the frustum; the low-pass of D8 keeps them at least a pixel wide.
+    rng = np.random.default_rng(5)
+    for far, label in ((40.0, "near_only"), (3.0e3, "three_passes"), (2.0e5, "four_passes")):
+        s = synth.make_scene(2, n_gaussians=6000, width=200, height=136, n_cameras=2, seed=77)
+        cam = s.cameras[0]
+        R = cam.R.astype(np.float64)
+        eye = -(R.T @ cam.t.astype(np.float64))
+        n_far = 400
+        z = np.exp(rng.uniform(np.log(5.0), np.log(far), n_far))
+        lateral = rng.uniform(-0.2, 0.2, (n_far, 2)) * z[:, None]          # well inside the 60 degree frustum
+        p = eye[None, :] + z[:, None] * R[2][None, :] + lateral[:, :1] * R[0][None, :] + lateral[:, 1:] * R[1][None, :]
+        s.pos[:, :n_far] = p.T.astype(np.float32)
+        s.opacity_logit[:n_far] = 2.0
+        st = _run(B, ho, s, exact=True, label=f"wide_depth_{label}")
+        assert st[0]["V"] >= n_far // 2
