@@ -585,6 +585,20 @@ def run_ours(args):
         backward.update({"loss_l1_ssim_ms": float(np.median(tl[2:])), "whole_backward_ms": float(np.median(tb[2:])),
                          "loss": loss, "whole_backward_note": "hyrf_backward: background, rasterizer, projection, Eq. 7, decoders, "
                          "grid scatter-adds; gradients of all parameters accumulated over the repetitions"})
+        # roofline of the whole backward: it is a CUDA-core pass, so the bound is fp32 issue. Useful
+        # work = the decoders' multiply-adds per visible Gaussian, three times over (activations recomputed, deltas
+        # propagated, weight gradients: one fma per weight each) + the same for the background pixels; peak = the FFMA
+        # rate of the issue microprobe (nominal 4 per clock and SM without it)
+        nw = lambda m: sum(o * i for o, i in m.layer_shapes())
+        fmas = 3.0 * (nw(scene.geo_mlp) + nw(scene.app_mlp)) * int(cnt[1]) + 3.0 * nw(scene.bg_mlp) * float(n_bg)
+        pr = load_probes()
+        ffma = pr["issue_warp_instr_per_s_best"].get("ffma") if pr else None
+        peak_fma = 32.0 * ffma if ffma else 32.0 * 4.0 * torch.cuda.get_device_properties(dev).multi_processor_count * peaks["sm_max_mhz"] * 1e6
+        ach = fmas / (backward["whole_backward_ms"] * 1e-3)
+        backward["roofline"] = {"bound": "alu", "achieved": ach / 1e12, "peak": peak_fma / 1e12, "unit": "Tfma/s", "frac": ach / peak_fma,
+                                "peak_source": "measured (FFMA issue probe, profiles/r2_probes.json)" if ffma else "nominal",
+                                "fma_per_visible_gaussian": 3.0 * (nw(scene.geo_mlp) + nw(scene.app_mlp)),
+                                "note": "first version on CUDA cores: a thread per Gaussian, ~15 issued instructions per useful fma"}
         hs.set_retain_lists(False)
 
     if rank != 0:

@@ -111,6 +111,97 @@ __device__ __forceinline__ void mlp_backward(const float* w, float* dW, int n_in
     for (int k = 0; k < n_in; ++k) g_in[k] = delta[k];
 }
 
+// ---- the same two routines for the paper's decoder shapes (NIN -> 64 -> 64 -> NOUT), sizes known at compile
+// time: inputs of a layer in registers, weight rows as 16-byte shared-memory loads, four neurons (forward) or one row of
+// 64 accumulators (backward) at a time. Every sum keeps the order of the run-time versions above (and of D5), so the
+// values are the same bits; the run-time versions cost ~4.5 issued instructions per multiply-add, these ~1.3.
+template <bool FP16, int NIN, bool RELU, int NJ>
+__device__ __forceinline__ void dense_ct(const float* __restrict__ w, const float* in, float* out) {
+    float x[NIN];
+#pragma unroll
+    for (int k = 0; k < NIN; ++k) x[k] = in[k];
+    static_assert(NIN % 4 == 0, "rows are read 16 bytes at a time");
+    constexpr int G = NJ % 4 == 0 ? 4 : 1;   // neurons per step
+#pragma unroll 1
+    for (int j = 0; j < NJ; j += G) {
+        float h[G];
+#pragma unroll
+        for (int u = 0; u < G; ++u) h[u] = 0.0f;
+#pragma unroll
+        for (int k = 0; k < NIN / 4; ++k) {
+#pragma unroll
+            for (int u = 0; u < G; ++u) {
+                const float4 q = reinterpret_cast<const float4*>(w + (j + u) * NIN)[k];
+                h[u] = fmaf(q.x, x[4 * k], h[u]);
+                h[u] = fmaf(q.y, x[4 * k + 1], h[u]);
+                h[u] = fmaf(q.z, x[4 * k + 2], h[u]);
+                h[u] = fmaf(q.w, x[4 * k + 3], h[u]);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < G; ++u) {
+            float v = h[u];
+            if (RELU) { v = fmaxf(v, 0.0f); if (FP16) v = hy_round_half(v); }
+            out[j + u] = v;
+        }
+    }
+}
+
+template <bool FP16, int NIN, int NOUT>
+__device__ __forceinline__ void mlp_forward_keep_ct(const float* w, float (*act)[kMaxW], float* out) {
+    dense_ct<FP16, NIN, true, 64>(w, act[0], act[1]);
+    dense_ct<FP16, 64, true, 64>(w + 64 * NIN, act[1], act[2]);
+    dense_ct<FP16, 64, false, NOUT>(w + 64 * NIN + 64 * 64, act[2], out);
+}
+
+// prev[k] = sum_j w[j][k] d[j] (j ascending for every k), k < NK
+template <int NK, int NJ>
+__device__ __forceinline__ void backprop_ct(const float* __restrict__ w, const float* d, float (&acc)[NK]) {
+#pragma unroll
+    for (int k = 0; k < NK; ++k) acc[k] = 0.0f;
+#pragma unroll 1
+    for (int j = 0; j < NJ; ++j) {
+        const float dj = d[j];
+        const float4* row = reinterpret_cast<const float4*>(w + j * NK);
+#pragma unroll
+        for (int k = 0; k < NK / 4; ++k) {
+            const float4 q = row[k];
+            acc[4 * k] = fmaf(q.x, dj, acc[4 * k]);
+            acc[4 * k + 1] = fmaf(q.y, dj, acc[4 * k + 1]);
+            acc[4 * k + 2] = fmaf(q.z, dj, acc[4 * k + 2]);
+            acc[4 * k + 3] = fmaf(q.w, dj, acc[4 * k + 3]);
+        }
+    }
+}
+
+template <int NIN, int NOUT>
+__device__ __forceinline__ void mlp_backward_ct(const float* w, float* dW, float (*act)[kMaxW], const float* g_out, float* g_in,
+                                                uint32_t lane) {
+    constexpr int o1 = 64 * NIN, o2 = o1 + 64 * 64;
+    float delta[kMaxW];
+    {
+        accumulate_dw(dW + o2, g_out, act[2], NOUT, 64, lane);
+        float acc[64];
+        backprop_ct<64, NOUT>(w + o2, g_out, acc);
+#pragma unroll
+        for (int k = 0; k < 64; ++k) delta[k] = act[2][k] > 0.0f ? acc[k] : 0.0f;      // ReLU mask of the forward pass
+    }
+    {
+        accumulate_dw(dW + o1, delta, act[1], 64, 64, lane);
+        float acc[64];
+        backprop_ct<64, 64>(w + o1, delta, acc);
+#pragma unroll
+        for (int k = 0; k < 64; ++k) delta[k] = act[1][k] > 0.0f ? acc[k] : 0.0f;
+    }
+    {
+        accumulate_dw(dW, delta, act[0], 64, NIN, lane);
+        float acc[NIN];
+        backprop_ct<NIN, 64>(w, delta, acc);
+#pragma unroll
+        for (int k = 0; k < NIN; ++k) g_in[k] = acc[k];
+    }
+}
+
 // One level of one grid, forward and backward in one corner loop: the feature gradient g (2 values) is scattered to the
 // eight entries (atomics on the fp32 gradient table, [entry][2]) and its derivative with respect to the contracted
 // position accumulated in gx. The cell is the forward's (frozen).
@@ -228,7 +319,8 @@ __device__ __forceinline__ void load_weights(float* dst, const void* src, int n)
 // ---- S4a .. S2 ------------------------------------------------------------------------------------------------------
 constexpr int kFieldBwdThreads = 512;   // one CTA per SM (116 KB of weights + accumulators): 16 warps hide the local-memory and shared-memory latencies
 
-template <int DT>
+// STD: the decoders have the paper's shapes (geometry 32 -> 64 -> 64 -> 8, appearance 56 -> 64 -> 64 -> 3)
+template <int DT, bool STD>
 __global__ void __launch_bounds__(kFieldBwdThreads)
 field_backward_kernel(const BwdArgs B) {
     extern __shared__ __align__(16) float sm[];
@@ -289,8 +381,8 @@ field_backward_kernel(const BwdArgs B) {
                 if (FP16) hy_dir_pe<true>(dvec, oct, pe); else hy_dir_pe<false>(dvec, oct, pe);
                 for (int k = 0; k < 6 * oct; ++k) act_a[0][2 * La + k] = pe[k];
             }
-            if (FP16) { mlp_forward_keep<true>(wg, gin, hg, nhg, 8, act_g, raw); mlp_forward_keep<true>(wa, ain, ha, nha, 3, act_a, raw + 8); }
-            else { mlp_forward_keep<false>(wg, gin, hg, nhg, 8, act_g, raw); mlp_forward_keep<false>(wa, ain, ha, nha, 3, act_a, raw + 8); }
+            if (STD) { mlp_forward_keep_ct<FP16, 32, 8>(wg, act_g, raw); mlp_forward_keep_ct<FP16, 56, 3>(wa, act_a, raw + 8); }
+            else { mlp_forward_keep<FP16>(wg, gin, hg, nhg, 8, act_g, raw); mlp_forward_keep<FP16>(wa, ain, ha, nha, 3, act_a, raw + 8); }
         }
         // Eq. 7
         const float s0 = hy_sigmoid(raw[1] + ex.s_e), s1 = hy_sigmoid(raw[2] + ex.s_e), s2 = hy_sigmoid(raw[3] + ex.s_e);
@@ -373,8 +465,13 @@ field_backward_kernel(const BwdArgs B) {
         // ---- decoders, encodings, contraction ----
         if (neural) {
             float g_in_g[kMaxW], g_in_a[kMaxW];
-            mlp_backward(wg, dwg, gin, hg, nhg, 8, act_g, g_raw, g_in_g, lane);
-            mlp_backward(wa, dwa, ain, ha, nha, 3, act_a, g_raw + 8, g_in_a, lane);
+            if (STD) {
+                mlp_backward_ct<32, 8>(wg, dwg, act_g, g_raw, g_in_g, lane);
+                mlp_backward_ct<56, 3>(wa, dwa, act_a, g_raw + 8, g_in_a, lane);
+            } else {
+                mlp_backward(wg, dwg, gin, hg, nhg, 8, act_g, g_raw, g_in_g, lane);
+                mlp_backward(wa, dwa, ain, ha, nha, 3, act_a, g_raw + 8, g_in_a, lane);
+            }
             if (live) {
                 float gx[3] = {0.0f, 0.0f, 0.0f};
                 for (int l = 0; l < Lg; ++l) grid_level_backward<DT>(A.geo, l, x, g_in_g[2 * l], g_in_g[2 * l + 1], B.g_geo_table, gx);
@@ -556,8 +653,11 @@ hyrf_status launch_backward(hyrf_scene* s, const BwdArgs& B, uint32_t* launches)
     const size_t smem_bg = 2 * nw(b) * sizeof(float), smem_f = 2 * (nw(g) + nw(a)) * sizeof(float);
     cudaError_t e;
     if ((e = cudaFuncSetAttribute(background_backward_kernel<DT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bg)) != cudaSuccess ||
-        (e = cudaFuncSetAttribute(field_backward_kernel<DT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_f)) != cudaSuccess)
+        (e = cudaFuncSetAttribute(field_backward_kernel<DT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_f)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(field_backward_kernel<DT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_f)) != cudaSuccess)
         return hy_cuda_fail(e, "cudaFuncSetAttribute(backward)");
+    const bool std_shapes = g.in_dim == 32 && g.hidden == 64 && g.n_hidden == 2 && g.out_dim == 8 &&
+                            a.in_dim == 56 && a.hidden == 64 && a.n_hidden == 2 && a.out_dim == 3;
     const int P = s->lastW * s->lastH;
     if ((e = cudaMemsetAsync(B.g_T, 0, (size_t)P * sizeof(float), s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemsetAsync(g_T)");
     if (!(s->last_frame.ablation & HYRF_ABL_NO_BG)) {
@@ -566,7 +666,8 @@ hyrf_status launch_backward(hyrf_scene* s, const BwdArgs& B, uint32_t* launches)
     }
     hyrf_status st = hy_launch_raster_backward(s, B.g_out, B.g_T, const_cast<float*>(B.g_rec), launches);
     if (st != HYRF_OK) return st;
-    field_backward_kernel<DT><<<s->sm_count, kFieldBwdThreads, smem_f, s->stream>>>(B);
+    if (std_shapes) field_backward_kernel<DT, true><<<s->sm_count, kFieldBwdThreads, smem_f, s->stream>>>(B);
+    else field_backward_kernel<DT, false><<<s->sm_count, kFieldBwdThreads, smem_f, s->stream>>>(B);
     ++*launches;
     if ((e = cudaGetLastError()) != cudaSuccess) return hy_cuda_fail(e, "backward kernels");
     return HYRF_OK;
