@@ -111,6 +111,83 @@ __device__ __forceinline__ void mlp_backward(const float* w, float* dW, int n_in
     for (int k = 0; k < n_in; ++k) g_in[k] = delta[k];
 }
 
+// dW[j][k] += sum over the warp's 32 Gaussians of delta[j] * h[k] on the tensor cores: D = Delta^T H as 16 x 8 tiles of
+// mma.m16n8k8 (tf32 x tf32 -> fp32), K = the 32 lanes in four steps. A lane holds ITS Gaussian's delta and h; the
+// fragments need other lanes' values (A: row j = 16 jt + lane / 4 (+ 8), column g = 8 ks + lane % 4 (+ 4); B: row g,
+// column k = 8 kt + lane / 4), so they are assembled with shuffles: for r = 0 .. 7 every lane offers element r of the
+// current row block and the lanes with lane / 4 == r keep what the owner of their column's Gaussian offered. ~1.3
+// shuffle + select pairs per weight instead of the butterfly's 6 instructions; the products are rounded to tf32
+// (10-bit mantissa, round to nearest: relative 2^-11 per factor, unbiased), the sums are fp32.
+__device__ __forceinline__ uint32_t to_tf32(float v) {
+    uint32_t r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(v));
+    return r;
+}
+
+template <int NOUT, int NIN>
+__device__ __forceinline__ void accumulate_dw_mma(float* dW, const float* delta, const float* h, uint32_t lane) {
+    static_assert(NIN % 8 == 0, "column tiles of 8");
+    constexpr int JT = (NOUT + 15) / 16, KT = NIN / 8;
+    constexpr bool HI = NOUT > 8;   // rows 8 .. 15 of a row block exist
+    const uint32_t gid = lane >> 2, tig = lane & 3u;
+#pragma unroll 1
+    for (int jt = 0; jt < JT; ++jt) {
+        // A fragments of this row block for the four k-steps
+        uint32_t a[4][4];
+        {
+            float lo[8], hi8[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                lo[r] = (jt * 16 + r < NOUT) ? delta[jt * 16 + r] : 0.0f;
+                hi8[r] = (HI && jt * 16 + 8 + r < NOUT) ? delta[jt * 16 + 8 + r] : 0.0f;
+            }
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks) {
+                float f0 = 0.0f, f1 = 0.0f, f2 = 0.0f, f3 = 0.0f;
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    const float u0 = __shfl_sync(0xffffffffu, lo[r], 8 * ks + tig), u2 = __shfl_sync(0xffffffffu, lo[r], 8 * ks + tig + 4);
+                    if (gid == (uint32_t)r) { f0 = u0; f2 = u2; }
+                    if (HI) {
+                        const float u1 = __shfl_sync(0xffffffffu, hi8[r], 8 * ks + tig), u3 = __shfl_sync(0xffffffffu, hi8[r], 8 * ks + tig + 4);
+                        if (gid == (uint32_t)r) { f1 = u1; f3 = u3; }
+                    }
+                }
+                a[ks][0] = to_tf32(f0); a[ks][1] = to_tf32(f1); a[ks][2] = to_tf32(f2); a[ks][3] = to_tf32(f3);
+            }
+        }
+#pragma unroll 1
+        for (int kt = 0; kt < KT; ++kt) {
+            float hv[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) hv[r] = h[kt * 8 + r];
+            float c0 = 0.0f, c1 = 0.0f, c2 = 0.0f, c3 = 0.0f;
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks) {
+                float g0 = 0.0f, g1 = 0.0f;
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    const float u0 = __shfl_sync(0xffffffffu, hv[r], 8 * ks + tig), u1 = __shfl_sync(0xffffffffu, hv[r], 8 * ks + tig + 4);
+                    if (gid == (uint32_t)r) { g0 = u0; g1 = u1; }
+                }
+                const uint32_t b0 = to_tf32(g0), b1 = to_tf32(g1);
+                asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
+                             : "+f"(c0), "+f"(c1), "+f"(c2), "+f"(c3)
+                             : "r"(a[ks][0]), "r"(a[ks][1]), "r"(a[ks][2]), "r"(a[ks][3]), "r"(b0), "r"(b1));
+            }
+            const int j0 = jt * 16 + (int)gid, k0 = kt * 8 + 2 * (int)tig;
+            if (j0 < NOUT) {
+                if (c0 != 0.0f) atomicAdd(&dW[j0 * NIN + k0], c0);
+                if (c1 != 0.0f) atomicAdd(&dW[j0 * NIN + k0 + 1], c1);
+            }
+            if (HI && j0 + 8 < NOUT) {
+                if (c2 != 0.0f) atomicAdd(&dW[(j0 + 8) * NIN + k0], c2);
+                if (c3 != 0.0f) atomicAdd(&dW[(j0 + 8) * NIN + k0 + 1], c3);
+            }
+        }
+    }
+}
+
 // ---- the same two routines for the paper's decoder shapes (NIN -> 64 -> 64 -> NOUT), sizes known at compile
 // time: inputs of a layer in registers, weight rows as 16-byte shared-memory loads, four neurons (forward) or one row of
 // 64 accumulators (backward) at a time. Every sum keeps the order of the run-time versions above (and of D5), so the
@@ -180,21 +257,21 @@ __device__ __forceinline__ void mlp_backward_ct(const float* w, float* dW, float
     constexpr int o1 = 64 * NIN, o2 = o1 + 64 * 64;
     float delta[kMaxW];
     {
-        accumulate_dw(dW + o2, g_out, act[2], NOUT, 64, lane);
+        accumulate_dw_mma<NOUT, 64>(dW + o2, g_out, act[2], lane);
         float acc[64];
         backprop_ct<64, NOUT>(w + o2, g_out, acc);
 #pragma unroll
         for (int k = 0; k < 64; ++k) delta[k] = act[2][k] > 0.0f ? acc[k] : 0.0f;      // ReLU mask of the forward pass
     }
     {
-        accumulate_dw(dW + o1, delta, act[1], 64, 64, lane);
+        accumulate_dw_mma<64, 64>(dW + o1, delta, act[1], lane);
         float acc[64];
         backprop_ct<64, 64>(w + o1, delta, acc);
 #pragma unroll
         for (int k = 0; k < 64; ++k) delta[k] = act[1][k] > 0.0f ? acc[k] : 0.0f;
     }
     {
-        accumulate_dw(dW, delta, act[0], 64, NIN, lane);
+        accumulate_dw_mma<64, NIN>(dW, delta, act[0], lane);
         float acc[NIN];
         backprop_ct<NIN, 64>(w, delta, acc);
 #pragma unroll
@@ -341,6 +418,7 @@ field_backward_kernel(const BwdArgs B) {
     const bool neural = !(f.ablation & HYRF_ABL_NO_NEURAL);
     const uint32_t per_pass = gridDim.x * blockDim.x;
     for (uint32_t base = blockIdx.x * blockDim.x; base < V; base += per_pass) {   // warps stay together: the reductions need every lane
+        if (STD) __syncthreads();
         const uint32_t wi = base + threadIdx.x;
         const bool have = wi < V;
         Explicit ex{};
@@ -357,7 +435,8 @@ field_backward_kernel(const BwdArgs B) {
         float x[3] = {0.5f, 0.5f, 0.5f};
         if (have) hy_contract(f, p[0], p[1], p[2], x);
         // ---- forward recompute (fp32, the exact path's arithmetic) ----
-        float act_g[5][kMaxW], act_a[5][kMaxW], raw[11];
+        constexpr int kRows = STD ? 3 : 5;   // input + hidden layers kept (the paper's decoders have two hidden layers)
+        float act_g[kRows][kMaxW], act_a[kRows][kMaxW], raw[11];
         float dvec[3] = {0.0f, 0.0f, 1.0f}, dn = 1.0f;
 #pragma unroll
         for (int k = 0; k < 11; ++k) raw[k] = 0.0f;
@@ -466,8 +545,13 @@ field_backward_kernel(const BwdArgs B) {
         if (neural) {
             float g_in_g[kMaxW], g_in_a[kMaxW];
             if (STD) {
+                // (the barriers keep the CTA's 16 warps in the same stretch of this long kernel: without them the warps
+                // spread over more code than the instruction cache holds and `no_instruction` is the first stall reason)
+                __syncthreads();
                 mlp_backward_ct<32, 8>(wg, dwg, act_g, g_raw, g_in_g, lane);
+                __syncthreads();
                 mlp_backward_ct<56, 3>(wa, dwa, act_a, g_raw + 8, g_in_a, lane);
+                __syncthreads();
             } else {
                 mlp_backward(wg, dwg, gin, hg, nhg, 8, act_g, g_raw, g_in_g, lane);
                 mlp_backward(wa, dwa, ain, ha, nha, 3, act_a, g_raw + 8, g_in_a, lane);
