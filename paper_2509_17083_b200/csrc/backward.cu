@@ -279,6 +279,34 @@ __device__ __forceinline__ void mlp_backward_ct(const float* w, float* dW, float
     }
 }
 
+// the background decoder's shape (NIN -> 64 -> 3, one hidden layer)
+template <bool FP16, int NIN>
+__device__ __forceinline__ void mlp_forward_keep_ct1(const float* w, float (*act)[kMaxW], float* out) {
+    dense_ct<FP16, NIN, true, 64>(w, act[0], act[1]);
+    dense_ct<FP16, 64, false, 3>(w + 64 * NIN, act[1], out);
+}
+
+template <int NIN>
+__device__ __forceinline__ void mlp_backward_ct1(const float* w, float* dW, float (*act)[kMaxW], const float* g_out, float* g_in,
+                                                 uint32_t lane) {
+    constexpr int o1 = 64 * NIN;
+    float delta[kMaxW];
+    {
+        accumulate_dw_mma<3, 64>(dW + o1, g_out, act[1], lane);
+        float acc[64];
+        backprop_ct<64, 3>(w + o1, g_out, acc);
+#pragma unroll
+        for (int k = 0; k < 64; ++k) delta[k] = act[1][k] > 0.0f ? acc[k] : 0.0f;      // ReLU mask of the forward pass
+    }
+    {
+        accumulate_dw_mma<64, NIN>(dW, delta, act[0], lane);
+        float acc[NIN];
+        backprop_ct<NIN, 64>(w, delta, acc);
+#pragma unroll
+        for (int k = 0; k < NIN; ++k) g_in[k] = acc[k];
+    }
+}
+
 // One level of one grid, forward and backward in one corner loop: the feature gradient g (2 values) is scattered to the
 // eight entries (atomics on the fp32 gradient table, [entry][2]) and its derivative with respect to the contracted
 // position accumulated in gx. The cell is the forward's (frozen).
@@ -580,7 +608,8 @@ field_backward_kernel(const BwdArgs B) {
 // out = C_fg + T c_s on the background pixels of the frame (the rasterizer's list): dL/dT = sum_c g_out c_s (the part of
 // dL/dT that comes through the composite; raster_backward adds nothing else to it), dL/dc_s = T g_out -> sigmoid ->
 // background decoder -> background table.
-template <int DT>
+// STD: the background decoder has the paper's shape (40 -> 64 -> 3)
+template <int DT, bool STD>
 __global__ void __launch_bounds__(kBwdThreads)
 background_backward_kernel(const BwdArgs B) {
     extern __shared__ __align__(16) float sm[];
@@ -626,7 +655,7 @@ background_backward_kernel(const BwdArgs B) {
             if (FP16) hy_dir_pe<true>(d, oct, pe); else hy_dir_pe<false>(d, oct, pe);
             for (int k = 0; k < 6 * oct; ++k) act[0][2 * L + k] = pe[k];
         }
-        if (FP16) mlp_forward_keep<true>(w, nin, hid, nh, 3, act, raw); else mlp_forward_keep<false>(w, nin, hid, nh, 3, act, raw);
+        if (STD) mlp_forward_keep_ct1<FP16, 40>(w, act, raw); else mlp_forward_keep<FP16>(w, nin, hid, nh, 3, act, raw);
         float g_raw[3] = {0.0f, 0.0f, 0.0f}, gT = 0.0f;
         if (have) {
             for (int c = 0; c < 3; ++c) {
@@ -637,7 +666,7 @@ background_backward_kernel(const BwdArgs B) {
             B.g_T[pix] = gT;
         }
         float g_in[kMaxW];
-        mlp_backward(w, dw, nin, hid, nh, 3, act, g_raw, g_in, lane);
+        if (STD) mlp_backward_ct1<40>(w, dw, act, g_raw, g_in, lane); else mlp_backward(w, dw, nin, hid, nh, 3, act, g_raw, g_in, lane);
         if (have && B.g_bg_table) {
             float gx[3] = {0.0f, 0.0f, 0.0f};
             for (int l = 0; l < L; ++l) grid_level_backward<DT>(B.bg_grid, l, x, g_in[2 * l], g_in[2 * l + 1], B.g_bg_table, gx);
@@ -736,7 +765,8 @@ hyrf_status launch_backward(hyrf_scene* s, const BwdArgs& B, uint32_t* launches)
     auto nw = [](const hyrf_mlp_desc& m) { return (size_t)m.in_dim * m.hidden + (size_t)(m.n_hidden - 1) * m.hidden * m.hidden + (size_t)m.hidden * m.out_dim; };
     const size_t smem_bg = 2 * nw(b) * sizeof(float), smem_f = 2 * (nw(g) + nw(a)) * sizeof(float);
     cudaError_t e;
-    if ((e = cudaFuncSetAttribute(background_backward_kernel<DT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bg)) != cudaSuccess ||
+    if ((e = cudaFuncSetAttribute(background_backward_kernel<DT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bg)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute(background_backward_kernel<DT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bg)) != cudaSuccess ||
         (e = cudaFuncSetAttribute(field_backward_kernel<DT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_f)) != cudaSuccess ||
         (e = cudaFuncSetAttribute(field_backward_kernel<DT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_f)) != cudaSuccess)
         return hy_cuda_fail(e, "cudaFuncSetAttribute(backward)");
@@ -745,7 +775,8 @@ hyrf_status launch_backward(hyrf_scene* s, const BwdArgs& B, uint32_t* launches)
     const int P = s->lastW * s->lastH;
     if ((e = cudaMemsetAsync(B.g_T, 0, (size_t)P * sizeof(float), s->stream)) != cudaSuccess) return hy_cuda_fail(e, "cudaMemsetAsync(g_T)");
     if (!(s->last_frame.ablation & HYRF_ABL_NO_BG)) {
-        background_backward_kernel<DT><<<s->sm_count * 4, kBwdThreads, smem_bg, s->stream>>>(B);
+        if (b.in_dim == 40 && b.hidden == 64 && b.n_hidden == 1 && b.out_dim == 3) background_backward_kernel<DT, true><<<s->sm_count * 4, kBwdThreads, smem_bg, s->stream>>>(B);
+        else background_backward_kernel<DT, false><<<s->sm_count * 4, kBwdThreads, smem_bg, s->stream>>>(B);
         ++*launches;
     }
     hyrf_status st = hy_launch_raster_backward(s, B.g_out, B.g_T, const_cast<float*>(B.g_rec), launches);
