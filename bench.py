@@ -568,7 +568,7 @@ def run_ours(args):
                     "note": "includes the memset of the [V][9] gradient rows",
                     "forward_ms": fwd_plain, "forward_retain_lists_ms": fwd_retain}
         # the whole training step's backward: Eq. 12 loss + dL/d image, then hyrf_backward (S6 -> S5 ->
-        # S4a -> S3 -> S2 to every parameter); first version on CUDA cores
+        # S4a -> S3 -> S2 to every parameter): a thread per Gaussian, weight gradients on the tensor cores
         target = torch.rand((H, W, 3), dtype=torch.float32, device=f"cuda:{dev}")
         grads = None
         tl, tb = [], []
@@ -598,7 +598,7 @@ def run_ours(args):
         backward["roofline"] = {"bound": "alu", "achieved": ach / 1e12, "peak": peak_fma / 1e12, "unit": "Tfma/s", "frac": ach / peak_fma,
                                 "peak_source": "measured (FFMA issue probe, profiles/r2_probes.json)" if ffma else "nominal",
                                 "fma_per_visible_gaussian": 3.0 * (nw(scene.geo_mlp) + nw(scene.app_mlp)),
-                                "note": "first version on CUDA cores: a thread per Gaussian, ~15 issued instructions per useful fma"}
+                                "note": "a thread per Gaussian on CUDA cores (recompute, delta propagation), weight gradients by tf32 mma.sync"}
         hs.set_retain_lists(False)
 
     if rank != 0:

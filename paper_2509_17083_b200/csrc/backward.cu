@@ -11,12 +11,13 @@
 //                                (atomics), decoder weights
 //   loss kernels                 Eq. 12: (1 - lambda) L1 + lambda (1 - SSIM), value and dL/d image
 //
-// First version, CUDA cores throughout: a thread owns one Gaussian (or background pixel), recomputes its forward
-// activations with the decoders' fp32 weights in shared memory, and back-propagates. Decoder weight gradients are
-// sums over ALL Gaussians of outer products delta x activation: a warp reduces 32 Gaussians' products with a
-// transposing butterfly (31 shuffles per 32 weights), accumulates in shared memory (one accumulator block per
-// persistent CTA), and the CTAs add their blocks to global memory once at the end. (The tensor-core formulation of
-// these reductions — dW = Delta^T H as a GEMM over the Gaussians — is the next step.)
+// A thread owns one Gaussian (or background pixel), recomputes its forward activations with the decoders' fp32 weights
+// in shared memory, and back-propagates on CUDA cores (for the paper's decoder shapes through routines with
+// compile-time sizes). Decoder weight gradients are sums over ALL Gaussians of outer products delta x activation:
+// per warp a 32-Gaussian slice of dW = Delta^T H on the tensor cores (mma.sync tf32, accumulate_dw_mma) — or, for
+// other decoder shapes, a transposing butterfly (accumulate_dw) — into one shared-memory accumulator block per
+// persistent CTA; the CTAs add their blocks to global memory once at the end. (Activations and deltas as tensor-core
+// tiles too, as in the forward kernel, is the next step: DESIGN.md §12.)
 #include <mutex>
 
 #include "field_common.cuh"
