@@ -21,6 +21,7 @@
 #include <mutex>
 
 #include "field_common.cuh"
+#include "mlp.cuh"
 #include "raster_common.cuh"
 
 namespace {
@@ -193,43 +194,11 @@ __device__ __forceinline__ void accumulate_dw_mma(float* dW, const float* delta,
 // time: inputs of a layer in registers, weight rows as 16-byte shared-memory loads, four neurons (forward) or one row of
 // 64 accumulators (backward) at a time. Every sum keeps the order of the run-time versions above (and of D5), so the
 // values are the same bits; the run-time versions cost ~4.5 issued instructions per multiply-add, these ~1.3.
-template <bool FP16, int NIN, bool RELU, int NJ>
-__device__ __forceinline__ void dense_ct(const float* __restrict__ w, const float* in, float* out) {
-    float x[NIN];
-#pragma unroll
-    for (int k = 0; k < NIN; ++k) x[k] = in[k];
-    static_assert(NIN % 4 == 0, "rows are read 16 bytes at a time");
-    constexpr int G = NJ % 4 == 0 ? 4 : 1;   // neurons per step
-#pragma unroll 1
-    for (int j = 0; j < NJ; j += G) {
-        float h[G];
-#pragma unroll
-        for (int u = 0; u < G; ++u) h[u] = 0.0f;
-#pragma unroll
-        for (int k = 0; k < NIN / 4; ++k) {
-#pragma unroll
-            for (int u = 0; u < G; ++u) {
-                const float4 q = reinterpret_cast<const float4*>(w + (j + u) * NIN)[k];
-                h[u] = fmaf(q.x, x[4 * k], h[u]);
-                h[u] = fmaf(q.y, x[4 * k + 1], h[u]);
-                h[u] = fmaf(q.z, x[4 * k + 2], h[u]);
-                h[u] = fmaf(q.w, x[4 * k + 3], h[u]);
-            }
-        }
-#pragma unroll
-        for (int u = 0; u < G; ++u) {
-            float v = h[u];
-            if (RELU) { v = fmaxf(v, 0.0f); if (FP16) v = hy_round_half(v); }
-            out[j + u] = v;
-        }
-    }
-}
-
 template <bool FP16, int NIN, int NOUT>
 __device__ __forceinline__ void mlp_forward_keep_ct(const float* w, float (*act)[kMaxW], float* out) {
-    dense_ct<FP16, NIN, true, 64>(w, act[0], act[1]);
-    dense_ct<FP16, 64, true, 64>(w + 64 * NIN, act[1], act[2]);
-    dense_ct<FP16, 64, false, NOUT>(w + 64 * NIN + 64 * 64, act[2], out);
+    mlp_dense_ct<FP16, NIN, true, 64>(w, act[0], act[1]);
+    mlp_dense_ct<FP16, 64, true, 64>(w + 64 * NIN, act[1], act[2]);
+    mlp_dense_ct<FP16, 64, false, NOUT>(w + 64 * NIN + 64 * 64, act[2], out);
 }
 
 // prev[k] = sum_j w[j][k] d[j] (j ascending for every k), k < NK
@@ -283,8 +252,8 @@ __device__ __forceinline__ void mlp_backward_ct(const float* w, float* dW, float
 // the background decoder's shape (NIN -> 64 -> 3, one hidden layer)
 template <bool FP16, int NIN>
 __device__ __forceinline__ void mlp_forward_keep_ct1(const float* w, float (*act)[kMaxW], float* out) {
-    dense_ct<FP16, NIN, true, 64>(w, act[0], act[1]);
-    dense_ct<FP16, 64, false, 3>(w + 64 * NIN, act[1], out);
+    mlp_dense_ct<FP16, NIN, true, 64>(w, act[0], act[1]);
+    mlp_dense_ct<FP16, 64, false, 3>(w + 64 * NIN, act[1], out);
 }
 
 template <int NIN>

@@ -62,7 +62,11 @@ field_fma_kernel(const FieldArgs A) {
             bufa[2 * l] = FP16 ? hy_round_half(f0) : f0;
             bufa[2 * l + 1] = FP16 ? hy_round_half(f1) : f1;
         }
-        if (CL > 0) {
+        if constexpr (CL > 0 && CNH == 2) {   // two hidden layers: layer by layer as loops (mlp.cuh mlp_dense_ct)
+            mlp_dense_ct<FP16, 2 * CL, true, CHID>(wg, bufa, bufb);
+            mlp_dense_ct<FP16, CHID, true, CHID>(wg + CHID * 2 * CL, bufb, bufa);
+            mlp_dense_ct<FP16, CHID, false, 8>(wg + CHID * 2 * CL + CHID * CHID, bufa, raw);
+        } else if (CL > 0) {
             mlp_eval<2 * CL, CHID, CNH, 8, FP16>(wg, 0, 0, 0, bufa, bufb, raw);
         } else {
             for (int k = 2 * Lg; k < geo_in; ++k) bufa[k] = 0.0f;
@@ -83,7 +87,11 @@ field_fma_kernel(const FieldArgs A) {
             if (CL > 0) hy_dir_pe<FP16>(d, 4, bufa + 2 * CL);
             else hy_dir_pe<FP16>(d, (int)A.pe_octaves, bufa + 2 * La);
         }
-        if (CL > 0) {
+        if constexpr (CL > 0 && CNH == 2) {
+            mlp_dense_ct<FP16, 2 * CL + 24, true, CHID>(wa, bufa, bufb);
+            mlp_dense_ct<FP16, CHID, true, CHID>(wa + CHID * (2 * CL + 24), bufb, bufa);
+            mlp_dense_ct<FP16, CHID, false, 3>(wa + CHID * (2 * CL + 24) + CHID * CHID, bufa, raw + 8);
+        } else if (CL > 0) {
             mlp_eval<2 * CL + 24, CHID, CNH, 3, FP16>(wa, 0, 0, 0, bufa, bufb, raw + 8);
         } else {
             for (int k = 2 * La + 6 * (int)A.pe_octaves; k < app_in; ++k) bufa[k] = 0.0f;

@@ -91,3 +91,43 @@ __device__ __forceinline__ void mlp_eval(const float* __restrict__ w, int rin, i
     for (int j = 0; j < OUT; ++j) out[j] = mlp_dot<(CIN > 0 && CHID > 0)>(w + j * cur, src, cur);
 }
 
+
+// One dense layer with compile-time sizes as a LOOP over groups of four neurons (not unrolled over the neurons): the
+// layer's inputs in registers, weight rows as 16-byte shared-memory loads, out[j] = act(sum_k w[j][k] in[k]) with k
+// ascending — D5's order, the bits of mlp_dot. `in` / `out` may be local arrays (indexed by the neuron at run time).
+// Unrolling a whole 64-wide decoder over its neurons (mlp_eval above with CNH = 2) makes ~20 k instructions of
+// straight-line code: longer than the instruction cache, and with a dozen warps per SM at different places in it the
+// kernel waits for instruction fetches (`no_instruction` 9.5 of 12 warps at config 2). This form is ~300 instructions
+// per layer.
+template <bool FP16, int NIN, bool RELU, int NJ>
+__device__ __forceinline__ void mlp_dense_ct(const float* __restrict__ w, const float* in, float* out) {
+    float x[NIN];
+#pragma unroll
+    for (int k = 0; k < NIN; ++k) x[k] = in[k];
+    static_assert(NIN % 4 == 0, "rows are read 16 bytes at a time");
+    constexpr int G = NJ % 4 == 0 ? 4 : 1;   // neurons per step
+#pragma unroll 1
+    for (int j = 0; j < NJ; j += G) {
+        float h[G];
+#pragma unroll
+        for (int u = 0; u < G; ++u) h[u] = 0.0f;
+#pragma unroll
+        for (int k = 0; k < NIN / 4; ++k) {
+#pragma unroll
+            for (int u = 0; u < G; ++u) {
+                const float4 q = reinterpret_cast<const float4*>(w + (j + u) * NIN)[k];
+                h[u] = fmaf(q.x, x[4 * k], h[u]);
+                h[u] = fmaf(q.y, x[4 * k + 1], h[u]);
+                h[u] = fmaf(q.z, x[4 * k + 2], h[u]);
+                h[u] = fmaf(q.w, x[4 * k + 3], h[u]);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < G; ++u) {
+            float v = h[u];
+            if (RELU) { v = fmaxf(v, 0.0f); if (FP16) v = hy_round_half(v); }
+            out[j + u] = v;
+        }
+    }
+}
+
