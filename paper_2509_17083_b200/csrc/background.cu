@@ -67,7 +67,13 @@ background_kernel(const BgArgs A) {
             bufa[2 * l] = FP16 ? hy_round_half(f0) : f0;
             bufa[2 * l + 1] = FP16 ? hy_round_half(f1) : f1;
         }
-        if (CL > 0) {
+        if constexpr (CL > 0 && CNH == 1) {
+            // layer by layer as loops over groups of four neurons: unrolled over its 64 neurons the decoder is ~4 500
+            // instructions, and 20 warps per SM at different places in them wait for instruction fetches (mlp.cuh)
+            hy_dir_pe<FP16>(d, 4, bufa + 2 * CL);
+            mlp_dense_ct<FP16, 2 * CL + 24, true, CHID>(smem_w, bufa, bufb);
+            mlp_dense_ct<FP16, CHID, false, 3>(smem_w + CHID * (2 * CL + 24), bufb, raw);
+        } else if constexpr (CL > 0) {
             hy_dir_pe<FP16>(d, 4, bufa + 2 * CL);
             mlp_eval<2 * CL + 24, CHID, CNH, 3, FP16>(smem_w, 0, 0, 0, bufa, bufb, raw);
         } else {
