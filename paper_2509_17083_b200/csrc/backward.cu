@@ -653,24 +653,58 @@ background_backward_kernel(const BwdArgs B) {
 // Pass 2: dL/da_p = (1 - lambda) sign(a_p - b_p) / n - (lambda / n) sum_q w(q - p) (D1_q + 2 a_p D2_q + b_p D3_q).
 __constant__ float c_win[11];
 
+// The 11 x 11 window is an outer product, so both passes run it as 11 + 11 taps: a tile's inputs (16 x 16 pixels + a
+// halo of 5, zeros outside the image) go to shared memory, the row pass leaves the horizontally filtered moments of
+// the tile's 26 rows there, the column pass finishes them per pixel. 5 x fewer multiply-adds than the direct window.
+constexpr int kSsimTile = 16, kSsimHalo = 5, kSsimIn = kSsimTile + 2 * kSsimHalo;   // 26
+
+// NM maps in: src(m, y, x) for the tile with halo -> s_h[m][26][16]: sum over di of win[di + 5] * src(m, y, x0 + col + di)
+template <int NM, typename F>
+__device__ __forceinline__ void ssim_row_pass(F src, float (*s_in)[kSsimIn][kSsimIn], float (*s_h)[kSsimIn][kSsimTile], int x0, int y0) {
+    for (int i = threadIdx.x; i < kSsimIn * kSsimIn; i += 256) {
+        const int r = i / kSsimIn, c = i - r * kSsimIn;
+        float v[NM];
+        src(y0 + r - kSsimHalo, x0 + c - kSsimHalo, v);
+#pragma unroll
+        for (int m = 0; m < NM; ++m) s_in[m][r][c] = v[m];
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < kSsimIn * kSsimTile; i += 256) {
+        const int r = i / kSsimTile, c = i - r * kSsimTile;
+#pragma unroll
+        for (int m = 0; m < NM; ++m) {
+            float acc = 0.0f;
+#pragma unroll
+            for (int d = 0; d < 11; ++d) acc += c_win[d] * s_in[m][r][c + d];
+            s_h[m][r][c] = acc;
+        }
+    }
+    __syncthreads();
+}
+
 __global__ void __launch_bounds__(256)
 ssim_maps_kernel(const float* __restrict__ a, const float* __restrict__ b, int W, int H, float lam, float* __restrict__ D,
                  double* __restrict__ loss) {
-    const int i = blockIdx.x * 16 + (threadIdx.x & 15), j = blockIdx.y * 16 + (threadIdx.x >> 4), c = blockIdx.z;
+    __shared__ float s_in[5][kSsimIn][kSsimIn];      // a, b, a a, b b, a b
+    __shared__ float s_h[5][kSsimIn][kSsimTile];
+    const int x0 = blockIdx.x * kSsimTile, y0 = blockIdx.y * kSsimTile, c = blockIdx.z;
+    const int ti = threadIdx.x & 15, tj = threadIdx.x >> 4, i = x0 + ti, j = y0 + tj;
+    ssim_row_pass<5>([&](int y, int x, float* v) {
+        float av = 0.0f, bv = 0.0f;
+        if (x >= 0 && x < W && y >= 0 && y < H) { av = a[3ull * ((size_t)y * W + x) + c]; bv = b[3ull * ((size_t)y * W + x) + c]; }
+        v[0] = av; v[1] = bv; v[2] = av * av; v[3] = bv * bv; v[4] = av * bv;
+    }, s_in, s_h, x0, y0);
     float l1 = 0.0f, ss = 0.0f;
     if (i < W && j < H) {
-        float ma = 0, mb = 0, saa = 0, sbb = 0, sab = 0;
-        for (int dj = -5; dj <= 5; ++dj) {
-            const int y = j + dj;
-            if (y < 0 || y >= H) continue;
-            for (int di = -5; di <= 5; ++di) {
-                const int x = i + di;
-                if (x < 0 || x >= W) continue;
-                const float wv = c_win[dj + 5] * c_win[di + 5];
-                const float av = a[3ull * ((size_t)y * W + x) + c], bv = b[3ull * ((size_t)y * W + x) + c];
-                ma += wv * av; mb += wv * bv; saa += wv * av * av; sbb += wv * bv * bv; sab += wv * av * bv;
-            }
+        float mo[5];
+#pragma unroll
+        for (int m = 0; m < 5; ++m) {
+            float acc = 0.0f;
+#pragma unroll
+            for (int d = 0; d < 11; ++d) acc += c_win[d] * s_h[m][tj + d][ti];
+            mo[m] = acc;
         }
+        const float ma = mo[0], mb = mo[1], saa = mo[2], sbb = mo[3], sab = mo[4];
         const float C1 = 1e-4f, C2 = 9e-4f;
         const float va = saa - ma * ma, vb = sbb - mb * mb, cab = sab - ma * mb;
         const float n1 = 2 * ma * mb + C1, n2 = 2 * cab + C2, d1 = ma * ma + mb * mb + C1, d2 = va + vb + C2;
@@ -683,7 +717,7 @@ ssim_maps_kernel(const float* __restrict__ a, const float* __restrict__ b, int W
         D[P3 + o] = dm_dd2;
         D[2 * P3 + o] = 2 * dm_dn2;
         ss = m;
-        l1 = fabsf(a[o] - b[o]);
+        l1 = fabsf(s_in[0][tj + kSsimHalo][ti + kSsimHalo] - s_in[1][tj + kSsimHalo][ti + kSsimHalo]);
     }
     const float n = 3.0f * W * H;
     float term = ((1.0f - lam) * l1 - lam * ss) / n;
@@ -694,24 +728,31 @@ ssim_maps_kernel(const float* __restrict__ a, const float* __restrict__ b, int W
 __global__ void __launch_bounds__(256)
 ssim_grad_kernel(const float* __restrict__ a, const float* __restrict__ b, int W, int H, float lam, const float* __restrict__ D,
                  float* __restrict__ g) {
-    const int i = blockIdx.x * 16 + (threadIdx.x & 15), j = blockIdx.y * 16 + (threadIdx.x >> 4), c = blockIdx.z;
-    if (i >= W || j >= H) return;
-    const size_t P3 = 3ull * W * H, o = 3ull * ((size_t)j * W + i) + c;
-    float s1 = 0, s2 = 0, s3 = 0;
-    for (int dj = -5; dj <= 5; ++dj) {
-        const int y = j + dj;
-        if (y < 0 || y >= H) continue;
-        for (int di = -5; di <= 5; ++di) {
-            const int x = i + di;
-            if (x < 0 || x >= W) continue;
-            const float wv = c_win[dj + 5] * c_win[di + 5];
+    __shared__ float s_in[3][kSsimIn][kSsimIn];      // D1, D2, D3
+    __shared__ float s_h[3][kSsimIn][kSsimTile];
+    const int x0 = blockIdx.x * kSsimTile, y0 = blockIdx.y * kSsimTile, c = blockIdx.z;
+    const int ti = threadIdx.x & 15, tj = threadIdx.x >> 4, i = x0 + ti, j = y0 + tj;
+    const size_t P3 = 3ull * W * H;
+    ssim_row_pass<3>([&](int y, int x, float* v) {
+        v[0] = v[1] = v[2] = 0.0f;
+        if (x >= 0 && x < W && y >= 0 && y < H) {
             const size_t q = 3ull * ((size_t)y * W + x) + c;
-            s1 += wv * D[q]; s2 += wv * D[P3 + q]; s3 += wv * D[2 * P3 + q];
+            v[0] = D[q]; v[1] = D[P3 + q]; v[2] = D[2 * P3 + q];
         }
+    }, s_in, s_h, x0, y0);
+    if (i >= W || j >= H) return;
+    float sacc[3];
+#pragma unroll
+    for (int m = 0; m < 3; ++m) {
+        float acc = 0.0f;
+#pragma unroll
+        for (int d = 0; d < 11; ++d) acc += c_win[d] * s_h[m][tj + d][ti];
+        sacc[m] = acc;
     }
+    const size_t o = 3ull * ((size_t)j * W + i) + c;
     const float n = 3.0f * W * H, av = a[o], bv = b[o];
     const float sgn = av > bv ? 1.0f : (av < bv ? -1.0f : 0.0f);
-    g[o] = ((1.0f - lam) * sgn - lam * (s1 + 2.0f * av * s2 + bv * s3)) / n;
+    g[o] = ((1.0f - lam) * sgn - lam * (sacc[0] + 2.0f * av * sacc[1] + bv * sacc[2])) / n;
 }
 
 }  // namespace
