@@ -288,12 +288,23 @@ bin_prefix_kernel(const BinArgs A) {
     }
 }
 
+// STAGED (long lists over few bins: the 4K frames of config 5, 43 M pairs over 2 040 macro tiles): the chunk's entries
+// are first put in bin order in shared memory and every bin's run is then written out as one piece. Written directly,
+// a bin's run of a chunk arrives as eight pieces of ~3 entries at eight different times, one from each warp; with
+// 740 resident CTAs x 2 040 bins x 8 warps there are far more partially written sectors than the L2 can hold, and
+// the scatter moved 1.04 GB to DRAM for a 173 MB list (and read 1.27 GB): 1.22 of the 3.7 ms of that frame.
+constexpr uint32_t kStagedMaxBins = 2560, kStagedChunk = 16384;
+constexpr size_t kStagedMinCap = 8u << 20;
+
+template <bool STAGED>
 __global__ void __launch_bounds__(kBinThreads)
 bin_scatter_kernel(const BinArgs A) {
     extern __shared__ uint32_t s_mem[];
     uint32_t* s_base = s_mem;                                               // [T] first slot of this chunk per tile
     unsigned short* s_wcnt = reinterpret_cast<unsigned short*>(s_mem + A.T); // [warps][Tp] per-warp counts -> running
     const uint32_t Tp = (A.T + 1u) & ~1u;
+    uint32_t* l_start = s_mem + A.T + kBinWarps * Tp / 2;                    // STAGED: [T + 1] first slot of a bin in s_list
+    uint32_t* s_list = l_start + A.T + 1;                                    // STAGED: [Ec] the chunk's entries in bin order
     const uint32_t D = pair_count(A);
     const uint32_t c0 = blockIdx.x * A.Ec;
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -353,8 +364,38 @@ bin_scatter_kernel(const BinArgs A) {
             s_wcnt[(size_t)w2 * Tp + t] = (unsigned short)run;
             run += c;
         }
+        if (STAGED) l_start[t] = run;   // the chunk's count of this bin, scanned below
     }
     __syncthreads();
+    if (STAGED) {
+        // exclusive scan of the bins' counts: a thread owns a contiguous stretch of bins
+        __shared__ uint32_t s_part[kBinThreads];
+        const uint32_t per = (A.T + kBinThreads - 1) / kBinThreads;
+        const uint32_t t0 = threadIdx.x * per, t1 = t0 + per < A.T ? t0 + per : A.T;
+        uint32_t sum = 0;
+        for (uint32_t t = t0; t < t1; ++t) sum += l_start[t];
+        s_part[threadIdx.x] = sum;
+        __syncthreads();
+        if (warp == 0) {   // 256 partial sums: 8 per lane
+            uint32_t v[kBinThreads / 32], tot = 0;
+#pragma unroll
+            for (int i = 0; i < kBinThreads / 32; ++i) { v[i] = s_part[lane * (kBinThreads / 32) + i]; tot += v[i]; }
+            uint32_t incl = tot;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= (uint32_t)d) incl += u;
+            }
+            uint32_t run = incl - tot;
+#pragma unroll
+            for (int i = 0; i < kBinThreads / 32; ++i) { s_part[lane * (kBinThreads / 32) + i] = run; run += v[i]; }
+        }
+        __syncthreads();
+        uint32_t run = s_part[threadIdx.x];
+        for (uint32_t t = t0; t < t1; ++t) { const uint32_t c = l_start[t]; l_start[t] = run; run += c; }
+        if (threadIdx.x == kBinThreads - 1) l_start[A.T] = c1 - c0;
+        __syncthreads();
+    }
     // ordered scatter, 32 pairs per step
     unsigned short* wc = s_wcnt + (size_t)warp * Tp;
     const uint32_t tbits = 32u - (uint32_t)__clz(A.T > 1u ? A.T - 1u : 1u);   // bits of the largest bin id
@@ -385,14 +426,31 @@ bin_scatter_kernel(const BinArgs A) {
             __syncwarp();
             if (act && lane == (uint32_t)(__ffs(peers) - 1)) wc[tile] = (unsigned short)(c + __popc(peers));
             __syncwarp();
-            if (act) A.list[s_base[tile] + c + __popc(peers & ((1u << lane) - 1u))] = gl[u];   // slot < D <= cap
+            if (act) {
+                const uint32_t k = c + __popc(peers & ((1u << lane) - 1u));   // place in the chunk's run of this bin
+                if (STAGED) s_list[l_start[tile] + k] = gl[u];
+                else A.list[s_base[tile] + k] = gl[u];   // slot < D <= cap
+            }
+        }
+    }
+    if (STAGED) {
+        // every bin's run of this chunk in one piece: a warp per bin, lanes along the run
+        __syncthreads();
+        for (uint32_t t = warp; t < A.T; t += kBinWarps) {
+            const uint32_t a = l_start[t], n = l_start[t + 1] - a, dst = s_base[t];
+            for (uint32_t k = lane; k < n; k += 32) A.list[dst + k] = s_list[a + k];
         }
     }
 }
 
 // pairs per CTA: at most ~1024 chunks; with few bins (macro tiles) the per-CTA set-up is cheap and small chunks give
 // the scatter more CTAs to fill the machine with, with thousands of bins it must be amortised over more pairs
+// (with a few hundred bins the pieces are long enough as they are, and the small chunks only add rows: config 4 and
+// 4M @ 1080p, 330 and 510 macro tiles, were 5 - 10 % slower staged)
+bool scatter_staged(size_t cap, uint32_t T) { return T > 1024 && T <= kStagedMaxBins && cap >= kStagedMinCap; }
+
 uint32_t chunk_entries(size_t cap, uint32_t T) {
+    if (scatter_staged(cap, T)) return kStagedChunk;   // the chunk is staged in shared memory (bin_scatter_kernel<true>)
     size_t c = (cap + 1023) / 1024;
     c = (c + 2047) / 2048 * 2048;
     const size_t lo = T <= 1024 ? 2048 : kMinChunk;
@@ -458,7 +516,8 @@ hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t
     bool& attr_set = s->bin_attr_set;
     if (!attr_set) {
         HY_CUDA_OK(cudaFuncSetAttribute(bin_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxTiles * 4)));
-        HY_CUDA_OK(cudaFuncSetAttribute(bin_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxTiles * 20)));
+        HY_CUDA_OK(cudaFuncSetAttribute(bin_scatter_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kMaxTiles * 20)));
+        HY_CUDA_OK(cudaFuncSetAttribute(bin_scatter_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kStagedMaxBins * 20 + 8 + kStagedChunk * 4)));
         attr_set = true;
     }
     const uint32_t off_blocks = (s->N + kOffItems - 1) / kOffItems;
@@ -468,7 +527,14 @@ hyrf_status hy_launch_bin_ordered(hyrf_scene* s, const uint32_t* order, uint32_t
     bin_prefix_kernel<<<(n_tiles + 31) / 32, 1024, 0, s->stream>>>(A);
     // the tile-level run only supplies the per-tile ranges (the lists themselves are written by the rasterizer as it
     // consumes them, api.cu): its scatter would produce a list nobody reads
-    if (macro) bin_scatter_kernel<<<A.rows_cap + 1, kBinThreads, smem_scatter, s->stream>>>(A);   // + 1: the tile-queue CTA
+    if (macro) {
+        if (scatter_staged(s->d_capacity, n_tiles)) {
+            const size_t smem_staged = smem_scatter + ((size_t)n_tiles + 1 + A.Ec) * 4;
+            bin_scatter_kernel<true><<<A.rows_cap + 1, kBinThreads, smem_staged, s->stream>>>(A);   // + 1: the tile-queue CTA
+        } else {
+            bin_scatter_kernel<false><<<A.rows_cap + 1, kBinThreads, smem_scatter, s->stream>>>(A);
+        }
+    }
     *launches += macro ? 5 : 4;
     return HYRF_OK;
 }
