@@ -357,7 +357,7 @@ def run_ours(args):
     path = {"auto": B.HYRF_MLP_AUTO, "fma": B.HYRF_MLP_FMA, "mma": B.HYRF_MLP_MMA, "hmma": B.HYRF_MLP_HMMA, "ws": B.HYRF_MLP_WS}[args.mlp]
     hs = B.HyrfScene(scene, device=dev, mlp_path=path)
     hs.set_ablation(args.ablation)
-    hs.set_raster_mode({"auto": 0, "tile": 1, "warp": 2, "pair": 3}[args.raster])
+    hs.set_raster_mode({"auto": 0, "tile": 1, "warp": 2, "pair": 3, "pairall": 4}[args.raster])
     upload = None
     if scene.explicit_rvq is not None:
         # the decode is an upload-time kernel (csrc/decode.cu), not part of a frame: timed on its own, device sources,
@@ -605,7 +605,7 @@ def run_ours(args):
         return
     names = ["cull", "field", "bin", "raster", "background"]
     kernels = {"field": {"hmma": "field_warp_kernel", "mma": "field_mma_pipe_kernel"}.get(args.mlp, "field_ws_kernel") if scene.fp16 and args.mlp != "fma"
-               else "field_fma_kernel", "raster": {2: "raster_warp_kernel", 3: "raster_pair_kernel"}.get(raster_mode_used, "raster_kernel")}
+               else "field_fma_kernel", "raster": {2: "raster_warp_kernel", 3: "raster_pair_kernel", 4: "raster_pair_kernel"}.get(raster_mode_used, "raster_kernel")}
     eval_pairs = None
     cpu = None
     if world == 1 and not args.no_cpu and args.ablation == 0:
@@ -694,7 +694,7 @@ def main():
                     help="hyrf_ablation bits (PAPER.md Table 5): 1 no pre-culling, 2 no background, 4 no neural, 8 no explicit")
     ap.add_argument("--quant8", action="store_true",
                     help="compressed model: 8-bit min-max tables decoded in the gather (PAPER.md:229)")
-    ap.add_argument("--raster", default="auto", choices=["auto", "tile", "warp", "pair"],
+    ap.add_argument("--raster", default="auto", choices=["auto", "tile", "warp", "pair", "pairall"],
                     help="hyrf_set_raster_mode: per-frame choice (default), tile-level lists only, per-warp lists")
     ap.add_argument("--morton-input", action="store_true",
                     help="store the Gaussians in Morton order of their positions (SURVEY 8(d): secondary, labelled measurement)")

@@ -254,14 +254,15 @@ hyrf_status hyrf_set_strip(hyrf_scene* scene, int32_t row_begin, int32_t row_end
 hyrf_status hyrf_set_pipelining(hyrf_scene* scene, int on);
 
 /* Rasterizer variant (S5; Eq. 1). Every variant stages a tile's depth-ordered list once per tile and
- * produces the same bits; they differ in cost. mode 1: every warp of the tile blends every staged entry. mode 2: a warp
- * owns an 8 x 4 pixel block and blends only the entries that can reach alpha >= 1/255 somewhere in its block (per-warp
- * lists built while staging) — faster when splats cover few tiles. mode 3: per-warp lists over 8 x 8 blocks with two
- * pixels per lane on the two-wide fp32 instructions of sm_100 (fma.rn.f32x2: half the issue slots per pair). mode 0
- * (default): 3 or 1, chosen per frame from the tiles touched per visible Gaussian of the previous frame.
- * HYRF_ERR_INVALID_ARG for any other mode. */
+ * produces the same bits; they differ in cost. mode 1: a pixel per thread, every warp of the tile blends every staged
+ * entry. mode 2: a warp owns an 8 x 4 pixel block and blends only the entries that can reach alpha >= 1/255 somewhere
+ * in its block (per-warp lists built while staging). mode 3: per-warp lists over 8 x 8 blocks with two pixels per lane
+ * on the two-wide fp32 instructions of sm_100 (fma.rn.f32x2: half the issue slots per pair) — fastest while splats
+ * cover few tiles. mode 4: the two-pixel loop of mode 3 over every staged entry, without masks and lists — fastest when
+ * a splat covers ~100 tiles (4K frames). mode 0 (default): 3 or 4, chosen per frame from the tiles touched per visible
+ * Gaussian of the previous frame. HYRF_ERR_INVALID_ARG for any other mode. */
 hyrf_status hyrf_set_raster_mode(hyrf_scene* scene, int mode);
-/* The variant (1, 2 or 3) the last render used. */
+/* The variant (1 .. 4) the last render used. */
 hyrf_status hyrf_last_raster_mode(hyrf_scene* scene, int* mode);
 
 /* Backward of stage 5 for the LAST rendered frame (first piece of the training pass of PAPER.md:136-142, which

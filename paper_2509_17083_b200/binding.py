@@ -416,7 +416,8 @@ class HyrfScene:
         _check(self.lib.hyrf_set_retain_lists(self.handle, int(on)))
 
     def set_raster_mode(self, mode: int = 0) -> None:
-        """0 auto, 1 tile-level lists only, 2 per-warp lists (include/hyrf.h hyrf_set_raster_mode); same bits, different cost."""
+        """0 auto, 1 a pixel per thread, 2 per-warp lists, 3 per-warp lists with two pixels per lane, 4 two pixels per lane over every
+        entry (include/hyrf.h hyrf_set_raster_mode); same bits, different cost."""
         _check(self.lib.hyrf_set_raster_mode(self.handle, int(mode)))
 
     def raster_backward(self, g_cfg, g_T, n_visible: int):

@@ -479,7 +479,7 @@ extern "C" hyrf_status hyrf_upload_explicit_rvq(hyrf_scene* s, const hyrf_explic
 
 extern "C" hyrf_status hyrf_set_raster_mode(hyrf_scene* s, int mode) {
     if (!s) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_raster_mode: NULL scene");
-    if (mode < 0 || mode > 3) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_raster_mode: mode %d outside [0, 3]", mode);
+    if (mode < 0 || mode > 4) return hy_fail(HYRF_ERR_INVALID_ARG, "hyrf_set_raster_mode: mode %d outside [0, 4]", mode);
     s->raster_mode = mode;
     return HYRF_OK;
 }

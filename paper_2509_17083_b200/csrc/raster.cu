@@ -175,19 +175,21 @@ raster_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ lis
 
 void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
                       float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list, uint32_t* dbg_len) {
-    // Per-warp lists (raster_warp.cu) pay when a splat covers few tiles: small splats leave many 8 x 4 blocks of a tile
-    // untouched. With large splats nearly every block is reached and this file's kernel (no masks, no
-    // indirection) is faster. Both give the same bits, so the choice is a cost heuristic: tiles touched per visible
-    // Gaussian in the previous frame (config 3: 10, config 4: 15 -> per-warp lists; the 1080p and 4K points of config 5:
-    // 35 - 120 -> this kernel; config 3 rendered at 1080p, 19 tiles per Gaussian, is the tie). hyrf_set_raster_mode overrides it.
-    constexpr uint64_t kWarpListMaxTilesPerSplat = 19;   // measured crossover on config 3 at 900p / 1080p / 1260p
-    bool warp_lists = s->raster_mode == 2 || s->raster_mode == 3;
-    if (s->raster_mode == 0) warp_lists = s->lastV == 0 || s->lastD <= kWarpListMaxTilesPerSplat * s->lastV;
-    // per-warp lists: the packed-fp32 kernel (two pixels per lane, raster_pair.cu) unless mode 2 pins the one-pixel one
-    s->last_raster_mode = warp_lists ? (s->raster_mode == 2 ? 2 : 3) : 1;
-    if (warp_lists) {
-        if (s->raster_mode == 2) hy_launch_raster_warp(s, f, ranges, list, macro, out_rgb, launches, tile_queue, dbg_list, dbg_len);
-        else hy_launch_raster_pair(s, f, ranges, list, macro, out_rgb, launches, tile_queue, dbg_list, dbg_len);
+    // Four kernels, the same bits (hyrf_set_raster_mode): 1 this file's (a pixel per thread, every warp blends every staged
+    // entry), 2 per-warp lists over 8 x 4 blocks (raster_warp.cu), 3 per-warp lists over 8 x 8 blocks with two pixels per
+    // lane on the two-wide fp32 instructions (raster_pair.cu), 4 the same two-pixel loop over every staged entry. Mode 0
+    // chooses between 3 and 4 from the tiles touched per visible Gaussian in the previous frame: per-warp lists pay as long
+    // as splats leave blocks of a tile untouched; when a splat covers ~100 tiles (the 4K points of config 5) nearly every
+    // block is reached and the masks and lists are pure cost. Measured raster stage, mode 3 / 4 / 1: config 3 (10 tiles per
+    // splat) 0.153 / 0.179 / 0.178 ms; 500k @ 1080p (35) 0.193 / 0.198 / 0.245; 4M @ 1080p (35) 0.229 / 0.236 / 0.281;
+    // 500k @ 4K (120) 0.657 / 0.632 / 0.840; 4M @ 4K (117) 0.728 / 0.704 / 0.925.
+    constexpr uint64_t kAllEntriesMinTilesPerSplat = 64;
+    int mode = s->raster_mode;
+    if (mode == 0) mode = (s->lastV != 0 && s->lastD > kAllEntriesMinTilesPerSplat * s->lastV) ? 4 : 3;
+    s->last_raster_mode = mode;
+    if (mode == 2) { hy_launch_raster_warp(s, f, ranges, list, macro, out_rgb, launches, tile_queue, dbg_list, dbg_len); return; }
+    if (mode == 3 || mode == 4) {
+        hy_launch_raster_pair(s, f, ranges, list, macro, out_rgb, launches, tile_queue, dbg_list, dbg_len, /*all=*/mode == 4);
         return;
     }
     const unsigned grid = (unsigned)(f.gx * f.gy);

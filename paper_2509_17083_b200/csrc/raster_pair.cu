@@ -34,6 +34,9 @@ __device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 d; asm("fma.rn.f32x2 %
 __device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 
+// ALL: every warp blends every staged record (no block masks, no per-warp lists): for splats that cover many tiles
+// nearly every 8 x 8 block is reached anyway (raster.cu's case), and what remains is this kernel's two-pixels-per-lane loop.
+template <bool ALL>
 __global__ void __launch_bounds__(kThreads)
 raster_pair_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict__ list, const float4* __restrict__ rec,
                    int W, int H, int gx, float tau_T, float* __restrict__ out_rgb, float* __restrict__ finalT,
@@ -123,7 +126,7 @@ raster_pair_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict_
                 r1 = __ldg(rec + 3ull * g + 1);
                 r2 = __ldg(reinterpret_cast<const float*>(rec + 3ull * g + 2));
                 keep = entry_reaches_tile(r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, X0, X1, Y0, Y1);
-                if (keep) wmask = entry_block_mask4(r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, X0, Y0, W, H);   // which warps' 8 x 8 blocks?
+                if (!ALL && keep) wmask = entry_block_mask4(r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, X0, Y0, W, H);   // which warps' 8 x 8 blocks?
             }
             const uint32_t bal = __ballot_sync(0xffffffffu, keep);
             if (lane == 0) s_cnt[warp] = __popc(bal);
@@ -142,30 +145,32 @@ raster_pair_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict_
                 o[2] = make_float4(r1.x, r1.x, r1.y, r1.y);
                 o[3] = make_float4(r1.z, r1.z, r1.w, r1.w);
                 *reinterpret_cast<float2*>(o + 4) = make_float2(r2, r2);
-                s_mask[pos] = (uint8_t)wmask;
+                if (!ALL) s_mask[pos] = (uint8_t)wmask;
             }
             __syncthreads();
         }
         // this warp's list: byte offsets of the staged records its 8 x 8 block can reach, in order, padded to a
         // multiple of 4 with the null record
-        uint32_t n_w = 0;
-        for (uint32_t i0 = 0; i0 < cnt; i0 += 32) {
+        uint32_t n_w = ALL ? cnt : 0u;
+        for (uint32_t i0 = 0; !ALL && i0 < cnt; i0 += 32) {
             const uint32_t i = i0 + lane;
             const bool h = i < cnt && ((s_mask[i] >> warp) & 1u);
             const uint32_t bal = __ballot_sync(0xffffffffu, h);
             if (h) s_widx[warp][n_w + __popc(bal & ((1u << lane) - 1u))] = (uint16_t)(i * kRecBytes);
             n_w += __popc(bal);
         }
-        if (lane < 4 && n_w + lane < ((n_w + 3u) & ~3u)) s_widx[warp][n_w + lane] = (uint16_t)(kNullSlot * kRecBytes);
+        if (!ALL && lane < 4 && n_w + lane < ((n_w + 3u) & ~3u)) s_widx[warp][n_w + lane] = (uint16_t)(kNullSlot * kRecBytes);
         __syncwarp();
         // blend: branch-free per entry, two pixels per lane; a warp leaves as soon as all of its 64 pixels have terminated
         for (uint32_t k0 = 0; k0 < n_w && !all_done; k0 += 4) {
             if (__all_sync(0xffffffffu, done0 && done1)) break;
-            const uint2 offs = *reinterpret_cast<const uint2*>(&s_widx[warp][k0]);
+            uint2 offs = make_uint2(0u, 0u);
+            if (!ALL) offs = *reinterpret_cast<const uint2*>(&s_widx[warp][k0]);
             const uint32_t ow[2] = {offs.x, offs.y};
 #pragma unroll
             for (uint32_t k = 0; k < 4; ++k) {
-                const uint8_t* r = s_rec + ((k & 1u) ? (ow[k >> 1] >> 16) : (ow[k >> 1] & 0xFFFFu));
+                const uint8_t* r = ALL ? s_rec + (k0 + k < cnt ? k0 + k : kNullSlot) * kRecBytes
+                                       : s_rec + ((k & 1u) ? (ow[k >> 1] >> 16) : (ow[k >> 1] & 0xFFFFu));
                 const ulonglong2 a0 = *reinterpret_cast<const ulonglong2*>(r);        // (u u) (v v)
                 const ulonglong2 a1 = *reinterpret_cast<const ulonglong2*>(r + 16);   // (A A) (-B -B)
                 const ulonglong2 a2 = *reinterpret_cast<const ulonglong2*>(r + 32);   // (C C) (o o)
@@ -227,12 +232,14 @@ raster_pair_kernel(const uint2* __restrict__ ranges, const uint32_t* __restrict_
 }  // namespace
 
 void hy_launch_raster_pair(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
-                           float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list, uint32_t* dbg_len) {
+                           float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list, uint32_t* dbg_len,
+                           bool all) {
     const unsigned grid = (unsigned)(f.gx * f.gy);
     const bool want_fg = (s->debug_mask >> HYRF_DBG_FG) & 1u;
     const bool want_mask = (s->debug_mask >> HYRF_DBG_BG_MASK) & 1u;
     const float tau = (f.ablation & HYRF_ABL_NO_BG) ? INFINITY : f.tau_T;   // no background: empty S6 list
-    raster_pair_kernel<<<grid, kThreads, 0, s->stream>>>(ranges, list, s->rec, f.W, f.H, f.gx, tau, out_rgb, s->finalT,
+    auto kern = all ? raster_pair_kernel<true> : raster_pair_kernel<false>;
+    kern<<<grid, kThreads, 0, s->stream>>>(ranges, list, s->rec, f.W, f.H, f.gx, tau, out_rgb, s->finalT,
                                                          s->bg_list, s->counters, want_mask ? s->bg_mask : nullptr,
                                                          want_fg ? s->fg : nullptr, tile_queue, s->rect,
                                                          macro ? f.mshift : 0, f.mgx, dbg_list, s->ranges, dbg_len, f.ty0, f.ty1);

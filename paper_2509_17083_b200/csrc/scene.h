@@ -203,7 +203,8 @@ void hy_launch_raster(hyrf_scene* s, const FrameDev& f, const uint2* ranges, con
 void hy_launch_raster_warp(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
                            float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list, uint32_t* dbg_len);
 void hy_launch_raster_pair(hyrf_scene* s, const FrameDev& f, const uint2* ranges, const uint32_t* list, bool macro,
-                           float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list, uint32_t* dbg_len);
+                           float* out_rgb, uint32_t* launches, const uint32_t* tile_queue, uint32_t* dbg_list, uint32_t* dbg_len,
+                           bool all = false);
 // backward of S5 for the last frame (raster_backward.cu); needs the per-tile lists (s->ranges, s->list_final)
 hyrf_status hy_launch_raster_backward(hyrf_scene* s, const float* g_cfg, const float* g_T, float* grad,
                                       uint32_t* launches);

@@ -553,7 +553,7 @@ def test_config5_4m_points_sampled(B, ho, synth, n, W, H):
     hs.close()
 
 
-@pytest.mark.parametrize("mode", [1, 2, 3])
+@pytest.mark.parametrize("mode", [1, 2, 3, 4])
 def test_both_rasterizers_against_the_oracle(B, ho, synth, mode):
     # hyrf_set_raster_mode: 1 = every warp blends every staged entry (raster.cu), 2 = per-warp lists over 8 x 4 pixel
     # blocks (raster_warp.cu). Each against the oracle on its own: small splats (config 3 recipe), large splats at a
@@ -570,7 +570,7 @@ def test_rasterizer_choice_changes_no_bit(B, synth):
     s = synth.make_scene(3, n_gaussians=200_000, width=640, height=360, n_cameras=2)
     hs = B.HyrfScene(s)
     outs = {}
-    for mode in (1, 2, 3, 0):
+    for mode in (1, 2, 3, 4, 0):
         hs.set_raster_mode(mode)
         frames = []
         for cam in s.cameras:
@@ -578,14 +578,15 @@ def test_rasterizer_choice_changes_no_bit(B, synth):
             torch.cuda.synchronize()
             frames.append((o.cpu().numpy().copy(), hs.debug_fetch(B.DBG_FINAL_T).copy()))
         outs[mode] = frames
-    for mode in (2, 3, 0):
+    for mode in (2, 3, 4, 0):
         for (a, ta), (b, tb) in zip(outs[1], outs[mode]):
             assert (a.view(np.uint32) == b.view(np.uint32)).all() and (ta.view(np.uint32) == tb.view(np.uint32)).all()
     hs.set_raster_mode(1); hs.render(s.cameras[0]); assert hs.last_raster_mode() == 1
     hs.set_raster_mode(2); hs.render(s.cameras[0]); assert hs.last_raster_mode() == 2
     hs.set_raster_mode(3); hs.render(s.cameras[0]); assert hs.last_raster_mode() == 3
+    hs.set_raster_mode(4); hs.render(s.cameras[0]); assert hs.last_raster_mode() == 4
     with pytest.raises(B.HyrfError) as e:
-        hs.set_raster_mode(4)
+        hs.set_raster_mode(5)
     assert e.value.status == B.HYRF_ERR_INVALID_ARG
     hs.close()
 
@@ -683,7 +684,7 @@ def test_adversarial_long_thin_splats(B, ho, synth):
     live = orc["tiles"] > 0
     assert (np.abs(orc["proj"][live][:, 6] - 1.0 / 255.0) < 2e-3).sum() >= 5
     outs = {}
-    for mode in (1, 2, 3):
+    for mode in (1, 2, 3, 4):
         st = _run(B, ho, s, raster_mode=mode, label=f"adversarial_mode{mode}")
         assert st[0]["D"] > 50 * st[0]["V"]
         hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_FMA)
@@ -692,12 +693,12 @@ def test_adversarial_long_thin_splats(B, ho, synth):
         torch.cuda.synchronize()
         outs[mode] = (o.cpu().numpy().copy(), hs.debug_fetch(B.DBG_FINAL_T).copy())
         hs.close()
-    for mode in (2, 3):
+    for mode in (2, 3, 4):
         assert (outs[1][0].view(np.uint32) == outs[mode][0].view(np.uint32)).all()
         assert (outs[1][1].view(np.uint32) == outs[mode][1].view(np.uint32)).all()
     # and at a ragged small resolution with per-tile lists (<= 1024 tiles)
     s2 = _adversarial_scene(synth, n=200, W=333, H=250, seed=32)
-    for mode in (1, 2, 3):
+    for mode in (1, 2, 3, 4):
         _run(B, ho, s2, raster_mode=mode, label=f"adversarial_small_mode{mode}")
 
 
@@ -861,7 +862,7 @@ def test_backward_against_oracle(B, ho, synth, case):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("raster_mode", [1, 2, 3])
+@pytest.mark.parametrize("raster_mode", [1, 2, 3, 4])
 def test_retained_lists_give_the_export_paths_gradients(B, synth, raster_mode):
     # hyrf_set_retain_lists: the training switch keeps per-tile lists only up to the entry at which a
     # tile's pixels had all terminated and leaves the rasterizer its early exit. Image: bit-identical. Gradients: those
