@@ -262,6 +262,13 @@ hyrf_status hyrf_set_pipelining(hyrf_scene* scene, int on);
  * a splat covers ~100 tiles (4K frames). mode 0 (default): 3 or 4, chosen per frame from the tiles touched per visible
  * Gaussian of the previous frame. HYRF_ERR_INVALID_ARG for any other mode. */
 hyrf_status hyrf_set_raster_mode(hyrf_scene* scene, int mode);
+/* Granularity of the binning (S4b): on tile grids of more than 1024 tiles the per-tile lists are not
+ * materialised; Gaussians are binned into MACRO tiles of 2^shift x 2^shift tiles and the rasterizer picks each tile's
+ * subsequence out of its macro tile's depth-ordered list. shift 0 (default): chosen per frame from the tiles touched per
+ * visible Gaussian of the previous frame (2, 3 or 4: the larger the splats, the coarser); 1 .. 4: fixed. The image and
+ * every debug export are identical for every value. HYRF_ERR_INVALID_ARG otherwise. */
+hyrf_status hyrf_set_bin_granularity(hyrf_scene* scene, int shift);
+
 /* The variant (1 .. 4) the last render used. */
 hyrf_status hyrf_last_raster_mode(hyrf_scene* scene, int* mode);
 

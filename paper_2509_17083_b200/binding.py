@@ -30,7 +30,7 @@ EXPORTS = ["hyrf_create_scene", "hyrf_upload_params", "hyrf_set_stream", "hyrf_r
            "hyrf_stage_times", "hyrf_last_launch_count", "hyrf_set_ablation", "hyrf_render_host_async",
            "hyrf_host_sync", "hyrf_set_sort_overlap", "hyrf_upload_explicit_rvq", "hyrf_last_decode_time", "hyrf_set_raster_mode",
            "hyrf_last_raster_mode", "hyrf_raster_backward", "hyrf_probe_gather", "hyrf_probe_issue", "hyrf_set_pipelining", "hyrf_frame_gap", "hyrf_set_strip", "hyrf_backward", "hyrf_loss_l1_ssim",
-           "hyrf_set_retain_lists", "hyrf_loss_l1_ssim_noalloc"]
+           "hyrf_set_retain_lists", "hyrf_loss_l1_ssim_noalloc", "hyrf_set_bin_granularity"]
 ABL_NO_CULL, ABL_NO_BG, ABL_NO_NEURAL, ABL_NO_EXPLICIT = 1, 2, 4, 8
 
 
@@ -125,6 +125,7 @@ def load_library() -> C.CDLL:
         L.hyrf_last_raster_mode.argtypes = [vp, C.POINTER(C.c_int)]
         L.hyrf_raster_backward.argtypes = [vp, vp, vp, vp, C.c_uint64]
         L.hyrf_set_retain_lists.argtypes = [vp, C.c_int]
+        L.hyrf_set_bin_granularity.argtypes = [vp, C.c_int]
         L.hyrf_loss_l1_ssim_noalloc.argtypes = [C.c_int32, vp, vp, vp, C.c_int32, C.c_int32, C.c_float, C.POINTER(C.c_double), vp]
         L.hyrf_probe_gather.argtypes = [C.c_int32, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32,
                                         C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_float)]
@@ -410,6 +411,10 @@ class HyrfScene:
     def set_pipelining(self, on: bool = True) -> None:
         """A stream of hyrf_render calls: frame k+1's cull and depth sort beside frame k's rasterizer (include/hyrf.h)."""
         _check(self.lib.hyrf_set_pipelining(self.handle, int(on)))
+
+    def set_bin_granularity(self, shift: int = 0) -> None:
+        """Macro tiles of 2^shift x 2^shift tiles for the binning (0: chosen per frame; include/hyrf.h); same bits, different cost."""
+        _check(self.lib.hyrf_set_bin_granularity(self.handle, int(shift)))
 
     def set_retain_lists(self, on: bool = True) -> None:
         """Training mode: every render keeps the per-tile lists the backward entry points need (include/hyrf.h)."""

@@ -8,7 +8,9 @@
 
 #define HY_MAX_LEVELS 16
 #define HY_TILE 16
+#ifndef HY_MACRO_SHIFT
 #define HY_MACRO_SHIFT 2                  // binning granularity: 4 x 4 tiles (64 x 64 pixels) per macro tile
+#endif
 #define HY_MACRO (1 << HY_MACRO_SHIFT)
 #define HY_REC_F4 3  // projected record = 3 x float4: (u, v, A, B) (C, opacity, r, g) (b, depth, radius, tiles)
 

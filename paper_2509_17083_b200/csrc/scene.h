@@ -140,6 +140,7 @@ struct hyrf_scene {
 
     // debug / measurement
     uint32_t ablation = 0;            // hyrf_ablation bits
+    int macro_shift = 0;              // hyrf_set_bin_granularity: 0 auto, else macro tiles of 2^shift x 2^shift tiles
     int raster_mode = 0;              // hyrf_set_raster_mode: 0 auto, 1 tile-level lists only, 2 per-warp lists
     int last_raster_mode = 0;         // what the last hy_launch_raster picked
     uint32_t debug_mask = 0;

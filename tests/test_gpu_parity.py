@@ -18,12 +18,13 @@ def B():
     return binding
 
 
-def _run(B, ho, scene, cams=None, mlp_path=None, exact=True, label="", ablation=0, raster_mode=0):
+def _run(B, ho, scene, cams=None, mlp_path=None, exact=True, label="", ablation=0, raster_mode=0, bin_shift=0):
     import torch
     mlp_path = B.HYRF_MLP_FMA if mlp_path is None else mlp_path
     hs = B.HyrfScene(scene, mlp_path=mlp_path)
     hs.set_ablation(ablation)
     hs.set_raster_mode(raster_mode)
+    hs.set_bin_granularity(bin_shift)
     hs.debug_enable()
     osc = ho.OracleScene(scene)
     stats = []
@@ -923,3 +924,31 @@ def test_depth_sort_over_a_wide_depth_range(B, ho, synth):
         s.opacity_logit[:n_far] = 2.0
         st = _run(B, ho, s, exact=True, label=f"wide_depth_{label}")
         assert st[0]["V"] >= n_far // 2
+
+
+def test_bin_granularity_changes_no_bit(B, ho, synth):
+    # hyrf_set_bin_granularity: macro tiles of 2 x 2 .. 16 x 16 tiles (and the per-frame choice) must give the image, the
+    # final transmittance and — through the debug export — every per-tile list of the 4 x 4 default, which the other tests
+    # compare with the oracle. Large splats over a 3 600-tile frame (the case the coarse settings are chosen for) and
+    # the config-3 recipe; then the same against the oracle directly with 8 x 8 macro tiles.
+    import torch
+    for s in (_adversarial_scene(synth, n=400, W=1280, H=720, seed=41),
+              synth.make_scene(3, n_gaussians=100_000, width=1280, height=720, n_cameras=1)):
+        cam = s.cameras[0]
+        outs = {}
+        for shift in (2, 1, 3, 4, 0):
+            hs = B.HyrfScene(s, mlp_path=B.HYRF_MLP_FMA)
+            hs.set_bin_granularity(shift)
+            hs.debug_enable((1 << B.DBG_TILE_LIST) | (1 << B.DBG_TILE_RANGES))
+            for _ in range(2):                       # (the per-frame choice looks at the previous frame)
+                o = hs.render(cam)
+            torch.cuda.synchronize()
+            outs[shift] = (o.cpu().numpy().copy(), hs.debug_fetch(B.DBG_FINAL_T).copy(),
+                           hs.debug_fetch(B.DBG_TILE_LIST).copy(), hs.debug_fetch(B.DBG_TILE_RANGES).copy())
+            hs.close()
+        for shift in (1, 3, 4, 0):
+            for a, b in zip(outs[2], outs[shift]):
+                assert a.shape == b.shape and (a.view(np.uint8) == b.view(np.uint8)).all(), shift
+        with pytest.raises(B.HyrfError):
+            hs = B.HyrfScene(s); hs.set_bin_granularity(5)
+    _run(B, ho, _adversarial_scene(synth, n=400, W=1280, H=720, seed=41), bin_shift=3, label="adversarial_bin8x8")
